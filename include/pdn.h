@@ -1,0 +1,143 @@
+/*
+ * pdn.h -- C ABI of the B200-native bump x load effective-resistance path.
+ *
+ * What the library computes: for a 3D-IC power delivery network modelled as a resistor network
+ * (d stacked 2D meshes joined by TSVs), the effective resistance
+ *
+ *      R_eff(b, l) = (e_b - e_l)^T G^+ (e_b - e_l)                  PAPER.md:40-43, Eq. (2)
+ *
+ * between bump b (a node of the top tier) and load l (a node of the bottom tier), for every
+ * requested pair, by the paper's divide-and-conquer method:
+ *   S1  each tier is reduced to its port nodes (TSV sites, bumps, loads) by batched
+ *       multi-right-hand-side solves on its 2D 5-point stencil (intra-die effective resistances,
+ *       the d x p x p, m x p, n x p arrays),
+ *   S2  the reusable coefficient matrix C = [K B; B^T 0] of Eq. (18) is assembled,
+ *   S3  decomposed ONCE and solved for the m + n right-hand sides b^1_i, b^d_j of
+ *       Eq. (21),
+ *   S4  R_eff(i, j) = -(x^1_i + x^d_j)^T (b^1_i + b^d_j), Eq. (22), for all pairs.
+ * pdn_create does S1-S3 (all the expensive work), pdn_reff does S4 and may be called repeatedly.
+ *
+ * Conventions.  0-based.  Tier 0 is the top tier (bumps; the paper's die_1), tier d-1 the bottom
+ * tier (loads; die_d).  Tier t is an n x n node mesh, node (y, x), local id y*n + x.  Interface i
+ * (0 <= i < d-1) joins tier i and tier i+1.  All floating point is IEEE FP64.  Every entry point
+ * is thread-compatible (one thread per context at a time), never throws, and returns a status
+ * (0 = PDN_OK).  There is NO CPU fallback: without a CUDA device every compute call fails with
+ * PDN_E_CUDA.
+ */
+#ifndef PDN_H_
+#define PDN_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pdn_ctx pdn_ctx; /* opaque; owned by the library; freed by pdn_destroy */
+
+/* status codes */
+enum {
+    PDN_OK = 0,
+    PDN_E_ARG = 1,          /* null pointer, negative size, d < 2, n < 2, site / interface out of range,
+                               r_ohm <= 0 or not finite, an interface without TSVs, a duplicate TSV site
+                               inside one interface, negative / non-finite conductance                    */
+    PDN_E_DISCONNECTED = 2, /* a tier is not one connected component (checked on the device)            */
+    PDN_E_NOCONV = 3,       /* a port solve did not reach rtol within max_iter iterations               */
+    PDN_E_CUDA = 4,         /* CUDA runtime error (pdn_last_error() has the string)                      */
+    PDN_E_NOMEM = 5,        /* device or host allocation failed                                          */
+    PDN_E_NUMERIC = 6       /* the port-level matrix K was not positive definite (should not happen for
+                               a connected network with r_ohm > 0)                                        */
+};
+
+/* flags for pdn_opts.flags */
+enum {
+    PDN_TIERS_ON_HOST = 1,  /* pdn_tier.gx / gy are HOST pointers (the library uploads them)            */
+    PDN_SKIP_CONNECTIVITY_CHECK = 2
+};
+
+/* One tier: an n x n mesh with per-edge conductances in siemens (0 = segment absent).
+ *   gx[y*n + x] joins (y,x)-(y,x+1); the last column (x = n-1) is ignored.
+ *   gy[y*n + x] joins (y,x)-(y+1,x); the last row    (y = n-1) is ignored.
+ * gx, gy are DEVICE pointers (HOST pointers if PDN_TIERS_ON_HOST), n*n doubles each, row-major.
+ * The library copies what it needs during pdn_create: the caller may free them afterwards. */
+typedef struct {
+    int32_t n;
+    const double *gx;
+    const double *gy;
+} pdn_tier;
+
+/* One TSV: joins node (y,x) of tier iface with node (y,x) of tier iface+1, resistance r_ohm
+ * (Table I: Rt_k^{i,i+1}).  HOST array. */
+typedef struct {
+    int32_t iface, y, x;
+    double r_ohm;
+} pdn_tsv;
+
+/* A bump (tier 0) or a load (tier d-1) node.  HOST arrays. */
+typedef struct {
+    int32_t y, x;
+} pdn_site;
+
+/* Options; pass NULL for the defaults.  Zero / negative fields mean "default". */
+typedef struct {
+    double rtol;        /* port solves stop at ||r||_2 <= rtol * ||b||_2          (default 1e-9)  */
+    int32_t max_iter;   /* iteration cap per port solve                           (default 200)   */
+    int32_t rhs_batch;  /* right-hand sides solved concurrently per tier          (default: auto) */
+    void *cuda_stream;  /* cudaStream_t to run on                                 (default: 0)    */
+    int32_t flags;      /* PDN_* flags                                                             */
+    int32_t nu;         /* Chebyshev smoothing steps per multigrid level and side (default 3)     */
+} pdn_opts;
+
+/* Counters and timings of the last pdn_create (device-event milliseconds). */
+typedef struct {
+    int32_t n_tiers, n_ports_total, n_levels, reserved;
+    int64_t kernel_launches;     /* kernels launched by pdn_create so far (+ pdn_reff calls)      */
+    int64_t stencil_launches;    /* of which S1 (stencil phase) kernels                            */
+    int32_t pcg_iters_max;       /* max PCG iterations over all port-solve batches                */
+    int32_t pcg_iters_sum;       /* sum over batches of the batch's iteration count               */
+    int64_t rhs_iterations;      /* sum over batches of (iterations x right-hand sides)           */
+    double worst_rel_residual;   /* max over all port solves of ||r|| / ||b|| at exit             */
+    double ms_upload, ms_stencil, ms_dense, ms_total;
+    double stencil_bytes;        /* algorithmic HBM bytes of the stencil phase (DESIGN.md model)  */
+} pdn_stats;
+
+/* S0-S3.  tiers: HOST array of n_tiers descriptors (all tiers must have the same n).  tsvs, bumps,
+ * loads: HOST arrays, copied.  On success *out owns all device memory it needs for pdn_reff.
+ * Work is ordered on opts->cuda_stream; the call returns after that work completed. */
+int pdn_create(pdn_ctx **out, int32_t n_tiers, const pdn_tier *tiers,
+               int32_t n_tsv, const pdn_tsv *tsvs,
+               int32_t n_bumps, const pdn_site *bumps,
+               int32_t n_loads, const pdn_site *loads,
+               const pdn_opts *opts);
+
+/* S4.  bump_idx / load_idx: DEVICE int32 arrays of length n_pairs indexing the create-time bump and
+ * load lists; both NULL => the full cross product, out[i*n_loads + j], and n_pairs must equal
+ * n_bumps*n_loads.  out: DEVICE fp64, caller-owned, n_pairs values; complete when the call returns.
+ * An index out of range yields NaN in that slot (no error). */
+int pdn_reff(pdn_ctx *ctx, int64_t n_pairs, const int32_t *bump_idx, const int32_t *load_idx, double *out);
+
+/* Same with HOST index arrays (or NULL, NULL) and a HOST output buffer (S4 + S5: PAPER.md:218,
+ * "transferred back to the CPU host"). */
+int pdn_reff_host(pdn_ctx *ctx, int64_t n_pairs, const int32_t *bump_idx, const int32_t *load_idx, double *out);
+
+/* NULL-safe; frees all device and host memory of ctx. */
+void pdn_destroy(pdn_ctx *ctx);
+
+/* Helpers. */
+const char *pdn_strerror(int status);
+const char *pdn_last_error(void);                       /* last CUDA error string of this thread  */
+int pdn_get_stats(const pdn_ctx *ctx, pdn_stats *out);
+
+/* Port matrix of one tier (the intra-die array of PAPER.md:218): q = pdn_port_count(ctx, tier);
+ * out (HOST, q*q doubles, row-major) receives Z_t = L_t^+ restricted to ports(t), where
+ * ports(t) = [lower ends of interface t-1] ++ [upper ends of interface t] ++ [bumps if t = 0]
+ * ++ [loads if t = d-1].  The intra-die effective resistance is R_jk = Z_jj + Z_kk - 2 Z_jk.
+ * Entries between two bump/load ports other than the diagonal are not computed (NaN): the method
+ * never needs them. */
+int32_t pdn_port_count(const pdn_ctx *ctx, int32_t tier);
+int pdn_get_port_matrix(const pdn_ctx *ctx, int32_t tier, double *out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PDN_H_ */
