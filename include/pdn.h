@@ -52,7 +52,21 @@ enum {
 /* flags for pdn_opts.flags */
 enum {
     PDN_TIERS_ON_HOST = 1,  /* pdn_tier.gx / gy are HOST pointers (the library uploads them)            */
-    PDN_SKIP_CONNECTIVITY_CHECK = 2
+    PDN_SKIP_CONNECTIVITY_CHECK = 2,
+    PDN_TIME_KERNELS = 4    /* bracket every kernel launch with CUDA events (per-class timers in pdn_stats) */
+};
+
+/* kernel classes of pdn_stats.class_* */
+enum {
+    PDN_KC_PQ = 0,     /* p = z + beta p ; q = L p ; p.q               (level 0)                   */
+    PDN_KC_DOWN0 = 1,  /* r -= alpha q ; pre-smooth ; residual ; restrict (level 0)                 */
+    PDN_KC_UP0 = 2,    /* prolong + correct ; post-smooth ; r.z          (level 0)                  */
+    PDN_KC_DOWNC = 3,  /* down stages of the coarse levels                                          */
+    PDN_KC_UPC = 4,    /* up stages of the coarse levels                                            */
+    PDN_KC_SMALL = 5,  /* scalars, port gather, right-hand-side setup, hierarchy setup              */
+    PDN_KC_DENSE = 6,  /* S2 + S3 port algebra                                                      */
+    PDN_KC_PAIR = 7,   /* S4 pair evaluation                                                        */
+    PDN_KC_COUNT = 8
 };
 
 /* One tier: an n x n mesh with per-edge conductances in siemens (0 = segment absent).
@@ -99,6 +113,9 @@ typedef struct {
     double worst_rel_residual;   /* max over all port solves of ||r|| / ||b|| at exit             */
     double ms_upload, ms_stencil, ms_dense, ms_total;
     double stencil_bytes;        /* algorithmic HBM bytes of the stencil phase (DESIGN.md model)  */
+    double class_ms[8];          /* device ms per kernel class (only with PDN_TIME_KERNELS)       */
+    double class_bytes[8];       /* algorithmic bytes moved per kernel class                      */
+    int64_t class_launches[8];   /* launches per kernel class                                     */
 } pdn_stats;
 
 /* S0-S3.  tiers: HOST array of n_tiers descriptors (all tiers must have the same n).  tsvs, bumps,

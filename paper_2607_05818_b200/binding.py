@@ -1,0 +1,206 @@
+"""ctypes binding of the C ABI in include/pdn.h -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind libpdn.so; this file only builds the C
+structs and passes pointers.  torch is used for device memory and streams, nothing else.  There is
+no fallback: if libpdn.so is missing or a call fails, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpdn.so")
+
+PDN_OK = 0
+PDN_TIERS_ON_HOST = 1
+PDN_SKIP_CONNECTIVITY_CHECK = 2
+PDN_TIME_KERNELS = 4
+KERNEL_CLASSES = ("pq", "down0", "up0", "down_coarse", "up_coarse", "small", "dense", "pair")
+
+
+class PdnTier(C.Structure):
+    _fields_ = [("n", C.c_int32), ("gx", C.c_void_p), ("gy", C.c_void_p)]
+
+
+class PdnTsv(C.Structure):
+    _fields_ = [("iface", C.c_int32), ("y", C.c_int32), ("x", C.c_int32), ("r_ohm", C.c_double)]
+
+
+class PdnSite(C.Structure):
+    _fields_ = [("y", C.c_int32), ("x", C.c_int32)]
+
+
+class PdnOpts(C.Structure):
+    _fields_ = [("rtol", C.c_double), ("max_iter", C.c_int32), ("rhs_batch", C.c_int32),
+                ("cuda_stream", C.c_void_p), ("flags", C.c_int32), ("nu", C.c_int32)]
+
+
+class PdnStats(C.Structure):
+    _fields_ = [("n_tiers", C.c_int32), ("n_ports_total", C.c_int32), ("n_levels", C.c_int32),
+                ("reserved", C.c_int32), ("kernel_launches", C.c_int64), ("stencil_launches", C.c_int64),
+                ("pcg_iters_max", C.c_int32), ("pcg_iters_sum", C.c_int32), ("rhs_iterations", C.c_int64),
+                ("worst_rel_residual", C.c_double), ("ms_upload", C.c_double), ("ms_stencil", C.c_double),
+                ("ms_dense", C.c_double), ("ms_total", C.c_double), ("stencil_bytes", C.c_double),
+                ("class_ms", C.c_double * 8), ("class_bytes", C.c_double * 8),
+                ("class_launches", C.c_int64 * 8)]
+
+
+EXPORTS = ("pdn_create", "pdn_reff", "pdn_reff_host", "pdn_destroy", "pdn_strerror", "pdn_last_error",
+           "pdn_get_stats", "pdn_port_count", "pdn_get_port_matrix")
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """dlopen libpdn.so (built in-tree by __graft_entry__.build()); fails loudly if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} not found: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                           "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    lib.pdn_create.restype = C.c_int
+    lib.pdn_create.argtypes = [C.POINTER(C.c_void_p), C.c_int32, C.POINTER(PdnTier), C.c_int32, C.POINTER(PdnTsv),
+                               C.c_int32, C.POINTER(PdnSite), C.c_int32, C.POINTER(PdnSite), C.POINTER(PdnOpts)]
+    for name in ("pdn_reff", "pdn_reff_host"):
+        f = getattr(lib, name)
+        f.restype = C.c_int
+        f.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.pdn_destroy.restype = None
+    lib.pdn_destroy.argtypes = [C.c_void_p]
+    lib.pdn_strerror.restype = C.c_char_p
+    lib.pdn_strerror.argtypes = [C.c_int]
+    lib.pdn_last_error.restype = C.c_char_p
+    lib.pdn_last_error.argtypes = []
+    lib.pdn_get_stats.restype = C.c_int
+    lib.pdn_get_stats.argtypes = [C.c_void_p, C.POINTER(PdnStats)]
+    lib.pdn_port_count.restype = C.c_int32
+    lib.pdn_port_count.argtypes = [C.c_void_p, C.c_int32]
+    lib.pdn_get_port_matrix.restype = C.c_int
+    lib.pdn_get_port_matrix.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
+    _lib = lib
+    return lib
+
+
+class PdnError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        lib = load_library()
+        self.status = status
+        msg = lib.pdn_strerror(status).decode()
+        detail = lib.pdn_last_error().decode()
+        super().__init__(f"{where}: status {status} ({msg}){': ' + detail if detail else ''}")
+
+
+def _sites(arr) -> C.Array:
+    a = np.ascontiguousarray(arr, dtype=np.int32).reshape(-1, 2)
+    out = (PdnSite * max(len(a), 1))()
+    for k, (y, x) in enumerate(a):
+        out[k].y, out[k].x = int(y), int(x)
+    return out
+
+
+def _ptr(t) -> int:
+    """Address of a torch tensor (device or host) or a numpy array; must be contiguous FP64/int32."""
+    if isinstance(t, np.ndarray):
+        assert t.flags["C_CONTIGUOUS"]
+        return t.ctypes.data
+    assert t.is_contiguous()
+    return t.data_ptr()
+
+
+class Pdn:
+    """Owns one pdn_ctx.  `gx`, `gy`: per-tier (n, n) FP64 planes, torch CUDA tensors (device path)
+    or numpy / torch CPU arrays (host path: PDN_TIERS_ON_HOST is set and the library uploads)."""
+
+    def __init__(self, n, gx, gy, tsv_site, tsv_r, bumps, loads, rtol=0.0, max_iter=0, rhs_batch=0,
+                 nu=0, flags=0, stream=None):
+        lib = load_library()
+        d = len(gx)
+        on_host = isinstance(gx[0], np.ndarray) or (hasattr(gx[0], "is_cuda") and not gx[0].is_cuda)
+        tiers = (PdnTier * d)()
+        self._keep = (gx, gy)
+        for t in range(d):
+            assert tuple(gx[t].shape) == (n, n) and tuple(gy[t].shape) == (n, n)
+            tiers[t].n = n
+            tiers[t].gx = _ptr(gx[t])
+            tiers[t].gy = _ptr(gy[t])
+        ntsv = sum(len(s) for s in tsv_site)
+        tsvs = (PdnTsv * max(ntsv, 1))()
+        k = 0
+        for i, (s, r) in enumerate(zip(tsv_site, tsv_r)):
+            for (y, x), rr in zip(np.asarray(s).reshape(-1, 2), np.asarray(r, dtype=np.float64)):
+                tsvs[k].iface, tsvs[k].y, tsvs[k].x, tsvs[k].r_ohm = i, int(y), int(x), float(rr)
+                k += 1
+        self.m = len(np.asarray(bumps).reshape(-1, 2))
+        self.nl = len(np.asarray(loads).reshape(-1, 2))
+        opts = PdnOpts(rtol=rtol, max_iter=max_iter, rhs_batch=rhs_batch,
+                       cuda_stream=C.c_void_p(stream) if stream else None,
+                       flags=flags | (PDN_TIERS_ON_HOST if on_host else 0), nu=nu)
+        h = C.c_void_p()
+        st = lib.pdn_create(C.byref(h), d, tiers, ntsv, tsvs, self.m, _sites(bumps), self.nl, _sites(loads),
+                            C.byref(opts))
+        if st != PDN_OK:
+            raise PdnError(st, "pdn_create")
+        self._h = h
+        self._lib = lib
+
+    @classmethod
+    def from_network(cls, net, device=None, **kw):
+        """Convenience: a pdn_inputs.Network; device='cuda' uploads the planes with torch first."""
+        gx, gy = net.gx, net.gy
+        if device is not None:
+            import torch
+            gx = [torch.from_numpy(np.ascontiguousarray(g)).to(device) for g in gx]
+            gy = [torch.from_numpy(np.ascontiguousarray(g)).to(device) for g in gy]
+        return cls(net.n, gx, gy, net.tsv_site, net.tsv_r, net.bumps, net.loads, **kw)
+
+    def reff(self, out, bump_idx=None, load_idx=None):
+        """pdn_reff: `out` (and the index arrays) are torch CUDA tensors."""
+        npairs = out.numel()
+        st = self._lib.pdn_reff(self._h, npairs, _ptr(bump_idx) if bump_idx is not None else None,
+                                _ptr(load_idx) if load_idx is not None else None, _ptr(out))
+        if st != PDN_OK:
+            raise PdnError(st, "pdn_reff")
+        return out
+
+    def reff_host(self, out: np.ndarray, bump_idx=None, load_idx=None):
+        """pdn_reff_host: `out` / index arrays are numpy (or pinned torch CPU) buffers."""
+        npairs = out.size if isinstance(out, np.ndarray) else out.numel()
+        st = self._lib.pdn_reff_host(self._h, npairs, _ptr(bump_idx) if bump_idx is not None else None,
+                                     _ptr(load_idx) if load_idx is not None else None, _ptr(out))
+        if st != PDN_OK:
+            raise PdnError(st, "pdn_reff_host")
+        return out
+
+    def stats(self) -> dict:
+        s = PdnStats()
+        st = self._lib.pdn_get_stats(self._h, C.byref(s))
+        if st != PDN_OK:
+            raise PdnError(st, "pdn_get_stats")
+        out = {name: getattr(s, name) for name, _ in PdnStats._fields_ if not name.startswith("class_")}
+        for key in ("class_ms", "class_bytes", "class_launches"):
+            out[key] = {k: getattr(s, key)[i] for i, k in enumerate(KERNEL_CLASSES)}
+        return out
+
+    def port_matrix(self, tier: int) -> np.ndarray:
+        q = self._lib.pdn_port_count(self._h, tier)
+        out = np.empty((q, q))
+        st = self._lib.pdn_get_port_matrix(self._h, tier, out.ctypes.data)
+        if st != PDN_OK:
+            raise PdnError(st, "pdn_get_port_matrix")
+        return out
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.pdn_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,118 @@
+// S1c/S1d: right-hand-side construction, per-right-hand-side PCG scalars (device resident, no host
+// round trip for alpha/beta), and the port gather.  The solution vector x is never stored: only its
+// values at the port nodes (x_port += alpha * p[port]) and its mean are accumulated -- Z_t needs
+// nothing else.
+#pragma once
+#include "common.cuh"
+
+namespace pdn {
+
+// r[b] = e_{node[src0+b]} - 1/n2  (consistent right-hand side of the singular tier system)
+__global__ void k_init_rhs(double* __restrict__ r, size_t n2, const int* __restrict__ node, int src0, int B) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int b = blockIdx.y;
+    if (i >= n2) return;
+    const double m = -1.0 / (double)n2;
+    r[b * n2 + i] = (i == (size_t)node[src0 + b]) ? 1.0 + m : m;
+}
+
+__global__ void k_zero(double* __restrict__ a, size_t n) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) a[i] = 0.0;
+}
+
+__global__ void k_pcg_init(PcgScalars s, int B) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b == 0) *s.n_active = B;
+    if (b >= B) return;
+    s.rho[b] = 1.0; s.rz[b] = 0.0; s.pq[b] = 0.0; s.rr[b] = 0.0; s.sump[b] = 0.0;
+    s.alpha[b] = 0.0; s.beta[b] = 0.0; s.xmean[b] = 0.0; s.relres[b] = 1.0; s.active[b] = 1;
+}
+
+// After the V-cycle: beta = rz / rho_old (0 on the first iteration or when frozen); rho = rz.
+__global__ void k_scal_beta(PcgScalars s, int B, int first) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    const double rz = s.rz[b], rho_old = s.rho[b];
+    s.beta[b] = (first || !s.active[b] || !(rho_old > 0.0)) ? 0.0 : rz / rho_old;
+    s.rho[b] = rz;
+    s.rz[b] = 0.0;
+    s.pq[b] = 0.0;
+    s.sump[b] = 0.0;
+}
+
+// After q = L p: alpha = rho / pq (0 when frozen); xmean += alpha * sum(p) / n2.
+__global__ void k_scal_alpha(PcgScalars s, int B, double inv_n2) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b == 0) *s.n_active = 0;  // counted again by k_scal_check
+    if (b >= B) return;
+    const double pq = s.pq[b];
+    const double a = (s.active[b] && pq > 0.0) ? s.rho[b] / pq : 0.0;
+    s.alpha[b] = a;
+    s.xmean[b] = fma(a * inv_n2, s.sump[b], s.xmean[b]);
+    s.rr[b] = 0.0;
+}
+
+// After r -= alpha q: convergence test  ||r||^2 <= tol2 * ||b||^2  (||b||^2 = 1 - 1/n2).
+__global__ void k_scal_check(PcgScalars s, int B, double tol2, double bnorm2) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    if (s.active[b]) {
+        const double rr = s.rr[b];
+        s.relres[b] = sqrt(rr / bnorm2);
+        if (!(rr > tol2 * bnorm2)) s.active[b] = 0;  // also freezes on NaN
+        else atomicAdd(s.n_active, 1);
+    }
+}
+
+// x_port[b][k] += alpha[b] * p[b][node[k]],  k over the gather list (all ports of the tier for a
+// TSV-source batch; for a terminal batch ngather == 0 and only the source node itself is read).
+__global__ void k_xport(const double* __restrict__ p, size_t n2, const double* __restrict__ alpha,
+                        const int* __restrict__ node, int ngather, int src0, double* __restrict__ xport,
+                        double* __restrict__ xown, int B) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int b = blockIdx.y;
+    const double a = alpha[b];
+    if (ngather > 0) {
+        if (k < ngather) xport[(size_t)b * ngather + k] = fma(a, p[b * n2 + node[k]], xport[(size_t)b * ngather + k]);
+    } else if (k == 0) {
+        xown[b] = fma(a, p[b * n2 + node[src0 + b]], xown[b]);
+    }
+}
+
+// ZT[src0+b][k] = x_port[b][k] - mean(x_b)   /   zdiag[b] = x_own[b] - mean(x_b)
+__global__ void k_finish_tsv(const double* __restrict__ xport, const double* __restrict__ xmean, int ngather,
+                             double* __restrict__ zt_rows, int B) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int b = blockIdx.y;
+    if (k < ngather) zt_rows[(size_t)b * ngather + k] = xport[(size_t)b * ngather + k] - xmean[b];
+}
+
+__global__ void k_finish_term(const double* __restrict__ xown, const double* __restrict__ xmean,
+                              double* __restrict__ zdiag, int B) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < B) zdiag[b] = xown[b] - xmean[b];
+}
+
+// Meshes with n <= 4 are their own coarsest level: Z comes straight from the dense pseudo-inverse.
+__global__ void k_direct_small(const double* __restrict__ pinv, int nc, const int* __restrict__ node, int ntsv,
+                               int q, double* __restrict__ ZT, double* __restrict__ zdiag) {
+    const int j = blockIdx.x;
+    for (int k = threadIdx.x; k < q; k += blockDim.x) {
+        if (j < ntsv) ZT[(size_t)j * q + k] = pinv[node[j] * nc + node[k]];
+        else if (k == 0) zdiag[j - ntsv] = pinv[node[j] * nc + node[j]];
+    }
+}
+
+// r.z for the single-level case (coarsest level is level 0).
+__global__ void k_dot(const double* __restrict__ a, const double* __restrict__ c, size_t n2, double* __restrict__ acc) {
+    __shared__ double red[32];
+    const int b = blockIdx.y;
+    double s = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += (size_t)gridDim.x * blockDim.x)
+        s = fma(a[b * n2 + i], c[b * n2 + i], s);
+    s = block_sum(s, red);
+    if (threadIdx.x == 0) atomicAdd(acc + b, s);
+}
+
+}  // namespace pdn

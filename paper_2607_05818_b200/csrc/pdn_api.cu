@@ -1,0 +1,821 @@
+// C-ABI entry points (include/pdn.h) and host-side orchestration of the hot path:
+//   pdn_create = S0 (tier import + multigrid hierarchy) -> S1 (batched port reduction by MG-PCG)
+//                -> S2 (assemble C) -> S3 (factor once, substitute for m+n right-hand sides)
+//   pdn_reff   = S4 (pair evaluation) [+ S5 copy to host]
+// Everything numerical runs in the kernels of stencil.cuh / pcg.cuh / setup.cuh / dense.cuh /
+// port.cuh; the host code below only validates, allocates, sequences launches and reads back the
+// per-batch convergence counter.  There is no CPU fallback.
+#include "../../include/pdn.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <set>
+#include <string>
+#include <utility>
+#include <vector>
+
+#include "common.cuh"
+#include "dense.cuh"
+#include "pcg.cuh"
+#include "port.cuh"
+#include "setup.cuh"
+#include "stencil.cuh"
+
+using namespace pdn;
+
+namespace {
+
+thread_local std::string g_last_error;
+
+struct CudaFail {
+    cudaError_t e;
+    const char* what;
+};
+
+#define CK(call)                                                    \
+    do {                                                            \
+        cudaError_t e__ = (call);                                   \
+        if (e__ != cudaSuccess) throw CudaFail{e__, #call};         \
+    } while (0)
+
+struct StatusFail {
+    int status;
+    std::string msg;
+};
+
+// kernel classes for the per-class timers / byte model
+enum { KC_PQ = 0, KC_DOWN0, KC_UP0, KC_DOWNC, KC_UPC, KC_SMALL, KC_DENSE, KC_PAIR, KC_COUNT };
+
+struct DevBuf {  // RAII device allocation
+    void* p = nullptr;
+    size_t bytes = 0;
+    DevBuf() = default;
+    DevBuf(const DevBuf&) = delete;
+    DevBuf& operator=(const DevBuf&) = delete;
+    DevBuf(DevBuf&& o) noexcept : p(o.p), bytes(o.bytes) { o.p = nullptr; o.bytes = 0; }
+    DevBuf& operator=(DevBuf&& o) noexcept {
+        if (this != &o) { release(); p = o.p; bytes = o.bytes; o.p = nullptr; o.bytes = 0; }
+        return *this;
+    }
+    ~DevBuf() { release(); }
+    void release() { if (p) cudaFree(p); p = nullptr; bytes = 0; }
+    void alloc(size_t n) {
+        release();
+        if (n == 0) n = 8;
+        cudaError_t e = cudaMalloc(&p, n);
+        if (e != cudaSuccess) { p = nullptr; cudaGetLastError(); throw StatusFail{PDN_E_NOMEM, "cudaMalloc of " + std::to_string(n) + " bytes failed"}; }
+        bytes = n;
+    }
+    template <class T> T* as() const { return static_cast<T*>(p); }
+};
+
+struct TierPorts {
+    int ntsv = 0, nterm = 0, q = 0;   // TSV ports, terminal ports, total
+    std::vector<int> node;            // local node id of every port, port order of port.cuh
+    DevBuf d_node;                    // device copy
+    DevBuf ZT;                        // ntsv x q
+    DevBuf zdiag;                     // nterm
+};
+
+}  // namespace
+
+struct pdn_ctx {
+    int d = 0, n = 0, m = 0, nl = 0, p0 = 0;
+    std::vector<int> p;               // TSVs per interface
+    std::vector<std::vector<double>> rt;
+    cudaStream_t stream = nullptr;
+    pdn_opts opts{};
+    std::vector<TierPorts> tiers;
+    DevBuf A1, X0, u, w;              // operands of the pair kernel
+    pdn_stats stats{};
+    double class_ms[KC_COUNT] = {};
+    double class_bytes[KC_COUNT] = {};
+    int64_t class_launches[KC_COUNT] = {};
+    bool time_kernels = false;
+    std::vector<std::pair<int, std::pair<cudaEvent_t, cudaEvent_t>>> pending_events;
+    std::vector<cudaEvent_t> event_pool;
+};
+
+namespace {
+
+// ------------------------------------------------------------------------------------------------
+// launch bookkeeping: every kernel goes through Launcher::run so that launches are counted and,
+// with PDN_TIME_KERNELS, bracketed by CUDA events on the launching stream.
+struct Launcher {
+    pdn_ctx* c;
+    cudaStream_t s;
+    cudaEvent_t get_event() {
+        if (!c->event_pool.empty()) { cudaEvent_t e = c->event_pool.back(); c->event_pool.pop_back(); return e; }
+        cudaEvent_t e;
+        CK(cudaEventCreate(&e));
+        return e;
+    }
+    template <class F>
+    void run(int cls, double bytes, F&& f) {
+        cudaEvent_t a = nullptr, b = nullptr;
+        if (c->time_kernels) { a = get_event(); b = get_event(); CK(cudaEventRecord(a, s)); }
+        f();
+        CK(cudaGetLastError());
+        if (c->time_kernels) { CK(cudaEventRecord(b, s)); c->pending_events.push_back({cls, {a, b}}); }
+        c->class_launches[cls]++;
+        c->class_bytes[cls] += bytes;
+        c->stats.kernel_launches++;
+        if (cls <= KC_SMALL) c->stats.stencil_launches++;
+    }
+    void resolve() {  // call after a stream synchronise
+        for (auto& pe : c->pending_events) {
+            float ms = 0.f;
+            CK(cudaEventElapsedTime(&ms, pe.second.first, pe.second.second));
+            c->class_ms[pe.first] += ms;
+            c->event_pool.push_back(pe.second.first);
+            c->event_pool.push_back(pe.second.second);
+        }
+        c->pending_events.clear();
+    }
+};
+
+inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) / b); }
+
+// ------------------------------------------------------------------------------------------------
+// S0: multigrid hierarchy of one tier (buffers are allocated once and reused for every tier).
+struct Hierarchy {
+    int nlev = 0;
+    int ny[MAX_LEVELS], nx[MAX_LEVELS];
+    DevBuf gx[MAX_LEVELS], gy[MAX_LEVELS], dinv[MAX_LEVELS];
+    DevBuf pinv, flags, labels;  // flags: [0] bad value, [1] isolated node, [2] label changed, [3] label nonzero
+    Level lev[MAX_LEVELS];
+
+    void allocate(int n) {
+        nlev = 0;
+        int cur = n;
+        while (true) {
+            ny[nlev] = nx[nlev] = cur;
+            const size_t b = (size_t)cur * cur * sizeof(double);
+            gx[nlev].alloc(b); gy[nlev].alloc(b); dinv[nlev].alloc(b);
+            lev[nlev] = Level{cur, cur, gx[nlev].as<double>(), gy[nlev].as<double>(), dinv[nlev].as<double>()};
+            ++nlev;
+            if (cur <= COARSEST_MAX) break;
+            if (nlev >= MAX_LEVELS) throw StatusFail{PDN_E_ARG, "mesh too large for MAX_LEVELS"};
+            cur = (cur + 1) / 2;
+        }
+        pinv.alloc(16 * 16 * sizeof(double));
+        flags.alloc(4 * sizeof(int));
+        labels.alloc((size_t)n * n * sizeof(int));
+    }
+
+    // Import one tier (gx_src / gy_src are device pointers) and build all levels.  Returns PDN status.
+    int build(Launcher& L, const double* gx_src, const double* gy_src, bool check_connectivity) {
+        const int n = ny[0];
+        CK(cudaMemsetAsync(flags.p, 0, 4 * sizeof(int), L.s));
+        int* fl = flags.as<int>();
+        L.run(KC_SMALL, 0, [&] { k_import_planes<<<cdiv((size_t)n * n, 256), 256, 0, L.s>>>(gx_src, gy_src, n, gx[0].as<double>(), gy[0].as<double>(), fl); });
+        for (int l = 0; l < nlev; ++l) {
+            const size_t n2 = (size_t)ny[l] * nx[l];
+            L.run(KC_SMALL, 0, [&] { k_dinv<<<cdiv(n2, 256), 256, 0, L.s>>>(ny[l], nx[l], gx[l].as<double>(), gy[l].as<double>(), dinv[l].as<double>(), l == 0 ? fl + 1 : nullptr); });
+            if (l + 1 < nlev) {
+                const size_t c2 = (size_t)ny[l + 1] * nx[l + 1];
+                L.run(KC_SMALL, 0, [&] { k_coarsen<<<cdiv(c2, 256), 256, 0, L.s>>>(ny[l], nx[l], gx[l].as<double>(), gy[l].as<double>(), ny[l + 1], nx[l + 1], gx[l + 1].as<double>(), gy[l + 1].as<double>()); });
+            }
+        }
+        const int lc = nlev - 1;
+        L.run(KC_SMALL, 0, [&] { k_coarsest_pinv<<<1, 32, 0, L.s>>>(ny[lc], nx[lc], gx[lc].as<double>(), gy[lc].as<double>(), pinv.as<double>()); });
+        int h[4] = {0, 0, 0, 0};
+        CK(cudaMemcpyAsync(h, fl, 2 * sizeof(int), cudaMemcpyDeviceToHost, L.s));
+        CK(cudaStreamSynchronize(L.s));
+        if (h[0]) return PDN_E_ARG;
+        if (h[1] && n > 1) return PDN_E_DISCONNECTED;
+        if (check_connectivity) {
+            const size_t n2 = (size_t)n * n;
+            int* lab = labels.as<int>();
+            L.run(KC_SMALL, 0, [&] { k_label_init<<<cdiv(n2, 256), 256, 0, L.s>>>((int)n2, lab); });
+            for (int sweep = 0; sweep < 4 * n + 64; ++sweep) {
+                CK(cudaMemsetAsync(fl + 2, 0, sizeof(int), L.s));
+                for (int rep = 0; rep < 4; ++rep)
+                    L.run(KC_SMALL, 0, [&] { k_label_sweep<<<cdiv(n2, 256), 256, 0, L.s>>>(n, n, gx[0].as<double>(), gy[0].as<double>(), lab, fl + 2); });
+                CK(cudaMemcpyAsync(h + 2, fl + 2, sizeof(int), cudaMemcpyDeviceToHost, L.s));
+                CK(cudaStreamSynchronize(L.s));
+                if (!h[2]) break;
+            }
+            L.run(KC_SMALL, 0, [&] { k_label_check<<<cdiv(n2, 256), 256, 0, L.s>>>((int)n2, lab, fl + 3); });
+            CK(cudaMemcpyAsync(h + 3, fl + 3, sizeof(int), cudaMemcpyDeviceToHost, L.s));
+            CK(cudaStreamSynchronize(L.s));
+            if (h[3]) return PDN_E_DISCONNECTED;
+        }
+        return PDN_OK;
+    }
+};
+
+Cheb make_cheb(int nu, double ratio) {
+    Cheb c{};
+    c.nu = nu;
+    const double lmax = 2.0, lmin = lmax / ratio;
+    const double theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin), sigma = theta / delta;
+    double rho = 1.0 / sigma;
+    c.c1[0] = 0.0;
+    c.c2[0] = 1.0 / theta;
+    for (int k = 1; k < nu; ++k) {
+        const double rho_new = 1.0 / (2.0 * sigma - rho);
+        c.c1[k] = rho_new * rho;
+        c.c2[k] = 2.0 * rho_new / delta;
+        rho = rho_new;
+    }
+    return c;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S1 workspace of one batch of right-hand sides.
+struct Work {
+    int Bmax = 0, qmax = 0;
+    DevBuf r[2], z0[2], p[2], q;                     // level 0 (ping-pong pairs avoid in-place halo races)
+    DevBuf rl[MAX_LEVELS], za[MAX_LEVELS], zb[MAX_LEVELS];  // levels >= 1
+    DevBuf scal, xport, xown, iact;
+    PcgScalars s{};
+    int* h_nact = nullptr;                           // pinned
+    double* h_relres = nullptr;                      // pinned, Bmax
+
+    static size_t bytes_per_rhs(const Hierarchy& H) {
+        size_t b = 7 * (size_t)H.ny[0] * H.nx[0];
+        for (int l = 1; l < H.nlev; ++l) b += 3 * (size_t)H.ny[l] * H.nx[l];
+        return b * sizeof(double);
+    }
+    void allocate(const Hierarchy& H, int B, int qmax_) {
+        Bmax = B; qmax = qmax_;
+        const size_t v0 = (size_t)B * H.ny[0] * H.nx[0] * sizeof(double);
+        for (int i = 0; i < 2; ++i) { r[i].alloc(v0); z0[i].alloc(v0); p[i].alloc(v0); }
+        q.alloc(v0);
+        for (int l = 1; l < H.nlev; ++l) {
+            const size_t vl = (size_t)B * H.ny[l] * H.nx[l] * sizeof(double);
+            rl[l].alloc(vl); za[l].alloc(vl); zb[l].alloc(vl);
+        }
+        scal.alloc((size_t)9 * B * sizeof(double));
+        double* sp = scal.as<double>();
+        s.rho = sp; s.rz = sp + B; s.pq = sp + 2 * B; s.rr = sp + 3 * B; s.sump = sp + 4 * B;
+        s.alpha = sp + 5 * B; s.beta = sp + 6 * B; s.xmean = sp + 7 * B; s.relres = sp + 8 * B;
+        iact.alloc((size_t)(B + 1) * sizeof(int));
+        s.active = iact.as<int>();
+        s.n_active = iact.as<int>() + B;
+        xport.alloc((size_t)B * std::max(qmax, 1) * sizeof(double));
+        xown.alloc((size_t)B * sizeof(double));
+        CK(cudaMallocHost(&h_nact, sizeof(int)));
+        CK(cudaMallocHost(&h_relres, (size_t)B * sizeof(double)));
+    }
+    ~Work() {
+        if (h_nact) cudaFreeHost(h_nact);
+        if (h_relres) cudaFreeHost(h_relres);
+    }
+};
+
+constexpr int TI = 32;  // tile interior of the first-version stencil kernels
+
+template <int NU>
+void launch_down(Launcher& L, int cls, double bytes, const Level& lv, const Cheb& ch, int B, const double* r_in,
+                 const double* q, const double* alpha, double* r_out, double* z_out, double* rc, int cny, int cnx,
+                 double* rr_acc) {
+    constexpr int E = TI + 2 * NU;
+    const size_t smem = 3 * E * E * sizeof(double);
+    dim3 grid(cdiv(lv.nx, TI), cdiv(lv.ny, TI), B);
+    L.run(cls, bytes, [&] { k_down<TI, NU><<<grid, STENCIL_THREADS, smem, L.s>>>(lv, ch, r_in, q, alpha, r_out, z_out, rc, cny, cnx, rr_acc); });
+}
+
+template <int NU>
+void launch_up(Launcher& L, int cls, double bytes, const Level& lv, const Cheb& ch, int B, const double* r,
+               const double* z_in, const double* ec, int cny, int cnx, double* z_out, double* rz_acc) {
+    constexpr int E = TI + 2 * NU;
+    const size_t smem = 3 * E * E * sizeof(double);
+    dim3 grid(cdiv(lv.nx, TI), cdiv(lv.ny, TI), B);
+    L.run(cls, bytes, [&] { k_up<TI, NU><<<grid, STENCIL_THREADS, smem, L.s>>>(lv, ch, r, z_in, ec, cny, cnx, z_out, rz_acc); });
+}
+
+#define NU_DISPATCH(nu, CALL)                 \
+    switch (nu) {                             \
+        case 1: { constexpr int NU_ = 1; CALL; } break; \
+        case 2: { constexpr int NU_ = 2; CALL; } break; \
+        case 3: { constexpr int NU_ = 3; CALL; } break; \
+        default: { constexpr int NU_ = 4; CALL; } break; \
+    }
+
+// One multigrid V-cycle  z = M^-1 r  on a batch.  If q != nullptr the level-0 down stage first forms
+// r_out = r_in - alpha q (and ||r_out||^2).  The result z is written to W.z0[1]; r.z goes to s.rz.
+// `after_down0` runs right after the level-0 down stage was enqueued (the convergence check); if it
+// returns true the rest of the cycle is skipped.
+template <class F>
+void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Cheb& ch, int B, const double* r_in, const double* q,
+            double* r_out, F&& after_down0) {
+    const int nl = H.nlev;
+    const double* r_use = q ? r_out : r_in;  // the residual the rest of the cycle works with
+    if (nl == 1) {  // the mesh itself is the coarsest level
+        if (q) throw StatusFail{PDN_E_CUDA, "internal: fused update on a single-level hierarchy"};
+        const int nc = H.ny[0] * H.nx[0];
+        L.run(KC_SMALL, 0, [&] { k_coarse_pinv<<<cdiv((size_t)B * nc, 128), 128, 0, L.s>>>(H.pinv.as<double>(), nc, r_in, W.z0[1].as<double>(), B); });
+        L.run(KC_SMALL, 0, [&] { k_dot<<<dim3(1, B), 128, 0, L.s>>>(r_in, W.z0[1].as<double>(), (size_t)nc, W.s.rz); });
+        (void)after_down0();
+        return;
+    }
+    for (int l = 0; l + 1 < nl; ++l) {
+        const double V = (double)B * H.ny[l] * H.nx[l] * 8.0, Vc = (double)B * H.ny[l + 1] * H.nx[l + 1] * 8.0;
+        const double* rin = l == 0 ? r_in : W.rl[l].as<double>();
+        double* zout = l == 0 ? W.z0[0].as<double>() : W.za[l].as<double>();
+        const bool fused = (l == 0 && q);
+        const double bytes = (fused ? 4.0 : 2.0) * V + Vc;
+        NU_DISPATCH(ch.nu, (launch_down<NU_>(L, l == 0 ? KC_DOWN0 : KC_DOWNC, bytes, H.lev[l], ch, B, rin, fused ? q : nullptr,
+                                             W.s.alpha, fused ? r_out : nullptr, zout, W.rl[l + 1].as<double>(),
+                                             H.ny[l + 1], H.nx[l + 1], W.s.rr)));
+        if (l == 0 && after_down0()) return;  // converged (or out of iterations): skip the rest of the cycle
+    }
+    const int lc = nl - 1, nc = H.ny[lc] * H.nx[lc];
+    L.run(KC_SMALL, 0, [&] { k_coarse_pinv<<<cdiv((size_t)B * nc, 128), 128, 0, L.s>>>(H.pinv.as<double>(), nc, W.rl[lc].as<double>(), W.za[lc].as<double>(), B); });
+    for (int l = nl - 2; l >= 0; --l) {
+        const double V = (double)B * H.ny[l] * H.nx[l] * 8.0, Vc = (double)B * H.ny[l + 1] * H.nx[l + 1] * 8.0;
+        const double* rr = l == 0 ? r_use : W.rl[l].as<double>();
+        const double* zin = l == 0 ? W.z0[0].as<double>() : W.za[l].as<double>();
+        double* zout = l == 0 ? W.z0[1].as<double>() : W.zb[l].as<double>();
+        const double* ec = (l + 1 == lc) ? W.za[lc].as<double>() : W.zb[l + 1].as<double>();
+        NU_DISPATCH(ch.nu, (launch_up<NU_>(L, l == 0 ? KC_UP0 : KC_UPC, 3.0 * V + Vc, H.lev[l], ch, B, rr, zin, ec,
+                                           H.ny[l + 1], H.nx[l + 1], zout, l == 0 ? W.s.rz : nullptr)));
+    }
+}
+
+// Solve L_t x_b = e_{port src0+b} - 1/n^2 for b in [0, B) by multigrid-preconditioned CG and leave
+//   TSV-source batch     : ZT[src0+b][k] = x_b[port k] - mean(x_b)      for all ports k of the tier
+//   terminal-source batch: zdiag[src0+b-ntsv] = x_b[own node] - mean(x_b)
+int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts& T, const Cheb& ch, int src0, int B,
+                bool terminal, double rtol, int max_iter);
+
+int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts& T, const Cheb& ch, int src0, int B,
+                bool terminal, double rtol, int max_iter) {
+    const int n = H.ny[0];
+    const size_t n2 = (size_t)n * n;
+    const double V = (double)B * n2 * 8.0;
+    const int* node = T.d_node.as<int>();
+    const int ngather = terminal ? 0 : T.q;
+    int cur_r = 0, cur_p = 0;
+    L.run(KC_SMALL, 0, [&] { k_pcg_init<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B); });
+    L.run(KC_SMALL, V, [&] { k_init_rhs<<<dim3(cdiv(n2, 256), B), 256, 0, L.s>>>(W.r[0].as<double>(), n2, node, src0, B); });
+    if (terminal) CK(cudaMemsetAsync(W.xown.p, 0, (size_t)B * sizeof(double), L.s));
+    else CK(cudaMemsetAsync(W.xport.p, 0, (size_t)B * ngather * sizeof(double), L.s));
+    vcycle(L, H, W, ch, B, W.r[0].as<double>(), nullptr, nullptr, [] { return false; });
+    const double bnorm2 = 1.0 - 1.0 / (double)n2;
+    int it = 0, status = PDN_OK;
+    while (true) {
+        L.run(KC_SMALL, 0, [&] { k_scal_beta<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, it == 0); });
+        {
+            dim3 grid(cdiv(n, TI), cdiv(n, TI), B);
+            L.run(KC_PQ, 4.0 * V, [&] { k_pq<TI><<<grid, STENCIL_THREADS, 0, L.s>>>(H.lev[0], W.z0[1].as<double>(), W.p[cur_p].as<double>(), W.s.beta, W.p[cur_p ^ 1].as<double>(), W.q.as<double>(), W.s.pq, W.s.sump); });
+            cur_p ^= 1;
+        }
+        L.run(KC_SMALL, 0, [&] { k_scal_alpha<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, 1.0 / (double)n2); });
+        L.run(KC_SMALL, 0, [&] { k_xport<<<dim3(cdiv(std::max(ngather, 1), 128), B), 128, 0, L.s>>>(W.p[cur_p].as<double>(), n2, W.s.alpha, node, ngather, src0, W.xport.as<double>(), W.xown.as<double>(), B); });
+        ++it;
+        bool done = false;
+        auto check = [&] {
+            L.run(KC_SMALL, 0, [&] { k_scal_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, rtol * rtol, bnorm2); });
+            CK(cudaMemcpyAsync(W.h_nact, W.s.n_active, sizeof(int), cudaMemcpyDeviceToHost, L.s));
+            CK(cudaStreamSynchronize(L.s));
+            done = (*W.h_nact == 0);
+            return done || it >= max_iter;
+        };
+        vcycle(L, H, W, ch, B, W.r[cur_r].as<double>(), W.q.as<double>(), W.r[cur_r ^ 1].as<double>(), check);
+        cur_r ^= 1;
+        if (done) break;
+        if (it >= max_iter) { status = PDN_E_NOCONV; break; }
+    }
+    // results + statistics
+    if (terminal)
+        L.run(KC_SMALL, 0, [&] { k_finish_term<<<cdiv(B, 128), 128, 0, L.s>>>(W.xown.as<double>(), W.s.xmean, T.zdiag.as<double>() + (src0 - T.ntsv), B); });
+    else
+        L.run(KC_SMALL, 0, [&] { k_finish_tsv<<<dim3(cdiv(ngather, 128), B), 128, 0, L.s>>>(W.xport.as<double>(), W.s.xmean, ngather, T.ZT.as<double>() + (size_t)src0 * T.q, B); });
+    CK(cudaMemcpyAsync(W.h_relres, W.s.relres, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, L.s));
+    CK(cudaStreamSynchronize(L.s));
+    double worst = 0.0;
+    for (int b = 0; b < B; ++b) worst = std::max(worst, W.h_relres[b]);
+    c->stats.worst_rel_residual = std::max(c->stats.worst_rel_residual, worst);
+    c->stats.pcg_iters_max = std::max(c->stats.pcg_iters_max, it);
+    c->stats.pcg_iters_sum += it;
+    c->stats.rhs_iterations += (int64_t)it * B;
+    return status;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S3 host drivers of the dense kernels (row-major, in place).
+void gemm(Launcher& L, int M, int N, int K, double alpha, const double* A, int64_t sai, int64_t sak, const double* B,
+          int64_t sbk, int64_t sbj, double beta, double* C, int64_t ldc) {
+    if (M <= 0 || N <= 0) return;
+    dim3 grid(cdiv(N, GEMM_BN), cdiv(M, GEMM_BM));
+    L.run(KC_DENSE, 0, [&] { k_gemm<<<grid, 256, 0, L.s>>>(M, N, K, alpha, A, sai, sak, B, sbk, sbj, beta, C, ldc); });
+}
+
+// A (n x n, lda) <- its lower Cholesky factor (strict upper part of the diagonal panels zeroed).
+void potrf(Launcher& L, double* A, int64_t lda, int n, int* fail) {
+    for (int k0 = 0; k0 < n; k0 += DENSE_NB) {
+        const int nb = std::min(DENSE_NB, n - k0);
+        L.run(KC_DENSE, 0, [&] { k_potrf_diag<<<1, DENSE_NB * DENSE_NB, 0, L.s>>>(A, lda, k0, nb, fail); });
+        const int rest = n - k0 - nb;
+        if (rest <= 0) break;
+        L.run(KC_DENSE, 0, [&] { k_potrf_panel<<<cdiv(rest, 128), 128, 0, L.s>>>(A, lda, n, k0, nb); });
+        const double* P = A + (int64_t)(k0 + nb) * lda + k0;  // panel rows (rest x nb)
+        gemm(L, rest, rest, nb, -1.0, P, lda, 1, P, 1, lda, 1.0, A + (int64_t)(k0 + nb) * lda + k0 + nb, lda);
+    }
+}
+
+// Bm (n x nrhs, ldb) <- Lm^-1 Bm
+void trsm_fwd(Launcher& L, const double* Lm, int64_t lda, int n, double* Bm, int64_t ldb, int nrhs) {
+    for (int k0 = 0; k0 < n; k0 += DENSE_NB) {
+        const int nb = std::min(DENSE_NB, n - k0);
+        L.run(KC_DENSE, 0, [&] { k_trsm_fwd_diag<<<cdiv(nrhs, 128), 128, 0, L.s>>>(Lm, lda, k0, nb, Bm, ldb, nrhs); });
+        const int rest = n - k0 - nb;
+        if (rest > 0)
+            gemm(L, rest, nrhs, nb, -1.0, Lm + (int64_t)(k0 + nb) * lda + k0, lda, 1, Bm + (int64_t)k0 * ldb, ldb, 1, 1.0,
+                 Bm + (int64_t)(k0 + nb) * ldb, ldb);
+    }
+}
+
+// Bm (n x nrhs, ldb) <- Lm^-T Bm
+void trsm_bwd(Launcher& L, const double* Lm, int64_t lda, int n, double* Bm, int64_t ldb, int nrhs) {
+    const int nblk = (n + DENSE_NB - 1) / DENSE_NB;
+    for (int kb = nblk - 1; kb >= 0; --kb) {
+        const int k0 = kb * DENSE_NB, nb = std::min(DENSE_NB, n - k0);
+        L.run(KC_DENSE, 0, [&] { k_trsm_bwd_diag<<<cdiv(nrhs, 128), 128, 0, L.s>>>(Lm, lda, k0, nb, Bm, ldb, nrhs); });
+        if (k0 > 0)  // rows [0,k0) -= L[k0:k0+nb, 0:k0]^T X_k
+            gemm(L, k0, nrhs, nb, -1.0, Lm + (int64_t)k0 * lda, 1, lda, Bm + (int64_t)k0 * ldb, ldb, 1, 1.0, Bm, ldb);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// S2 + S3: assemble C = [K B; B^T 0] (block-tridiagonal SPD K), factor it once, substitute for the
+// m + n + (d-1) right-hand sides, eliminate the multipliers, and leave the pair-kernel operands.
+int recombine(pdn_ctx* c, Launcher& L) {
+    const int d = c->d, dm1 = d - 1, m = c->m, n = c->nl, mn = m + n, nrhs = mn + dm1;
+    std::vector<DevBuf> Kd(dm1), V(dm1), F(dm1), rt(dm1);
+    DevBuf G, Sinv, Y, fail;
+    for (int i = 0; i < dm1; ++i) {
+        const size_t pi = c->p[i];
+        Kd[i].alloc(pi * pi * sizeof(double));
+        F[i].alloc(pi * (size_t)nrhs * sizeof(double));
+        if (i > 0) V[i].alloc((size_t)c->p[i - 1] * pi * sizeof(double));
+        rt[i].alloc(pi * sizeof(double));
+        CK(cudaMemcpyAsync(rt[i].p, c->rt[i].data(), pi * sizeof(double), cudaMemcpyHostToDevice, L.s));
+    }
+    G.alloc((size_t)dm1 * nrhs * sizeof(double));
+    Sinv.alloc((size_t)2 * dm1 * dm1 * sizeof(double));
+    Y.alloc((size_t)dm1 * mn * sizeof(double));
+    fail.alloc(sizeof(int));
+    CK(cudaMemsetAsync(fail.p, 0, sizeof(int), L.s));
+    TierPorts& T0 = c->tiers[0];
+    TierPorts& Td = c->tiers[d - 1];
+    for (int i = 0; i < dm1; ++i) {
+        const int pi = c->p[i];
+        TierPorts& Ta = c->tiers[i];
+        TierPorts& Tb = c->tiers[i + 1];
+        const int oa = i > 0 ? c->p[i - 1] : 0;
+        L.run(KC_DENSE, 0, [&] { k_assemble_diag<<<dim3(cdiv(pi, 128), pi), 128, 0, L.s>>>(pi, Ta.ZT.as<double>(), Ta.q, oa, Tb.ZT.as<double>(), Tb.q, rt[i].as<double>(), Kd[i].as<double>()); });
+        if (i + 1 < dm1) {
+            const int pj = c->p[i + 1];
+            L.run(KC_DENSE, 0, [&] { k_assemble_coupling<<<dim3(cdiv(pj, 128), pi), 128, 0, L.s>>>(pi, pj, Tb.ZT.as<double>(), Tb.q, V[i + 1].as<double>()); });
+        }
+        L.run(KC_DENSE, 0, [&] { k_assemble_rhs<<<dim3(cdiv(nrhs, 128), pi), 128, 0, L.s>>>(i, dm1, pi, m, n, T0.ZT.as<double>(), T0.q, T0.ntsv, Td.ZT.as<double>(), Td.q, Td.ntsv, F[i].as<double>()); });
+    }
+    // block-tridiagonal Cholesky + forward substitution
+    for (int i = 0; i < dm1; ++i) {
+        const int pi = c->p[i];
+        if (i > 0) {
+            const int ph = c->p[i - 1];
+            trsm_fwd(L, Kd[i - 1].as<double>(), ph, ph, V[i].as<double>(), pi, pi);
+            gemm(L, pi, pi, ph, -1.0, V[i].as<double>(), 1, pi, V[i].as<double>(), pi, 1, 1.0, Kd[i].as<double>(), pi);
+            gemm(L, pi, nrhs, ph, -1.0, V[i].as<double>(), 1, pi, F[i - 1].as<double>(), nrhs, 1, 1.0, F[i].as<double>(), nrhs);
+        }
+        potrf(L, Kd[i].as<double>(), pi, pi, fail.as<int>());
+        trsm_fwd(L, Kd[i].as<double>(), pi, pi, F[i].as<double>(), nrhs, nrhs);
+    }
+    // backward substitution
+    for (int i = dm1 - 1; i >= 0; --i) {
+        const int pi = c->p[i];
+        if (i + 1 < dm1) {
+            const int pj = c->p[i + 1];
+            gemm(L, pi, nrhs, pj, -1.0, V[i + 1].as<double>(), pj, 1, F[i + 1].as<double>(), nrhs, 1, 1.0, F[i].as<double>(), nrhs);
+        }
+        trsm_bwd(L, Kd[i].as<double>(), pi, pi, F[i].as<double>(), nrhs, nrhs);
+    }
+    // multipliers (Schur complement on the d-1 constraints, Eq. 8) and TSV currents
+    for (int i = 0; i < dm1; ++i)
+        L.run(KC_DENSE, 0, [&] { k_colsum<<<cdiv(nrhs, 128), 128, 0, L.s>>>(c->p[i], nrhs, F[i].as<double>(), G.as<double>() + (size_t)i * nrhs); });
+    L.run(KC_DENSE, 0, [&] { k_multipliers<<<1, 256, 0, L.s>>>(dm1, mn, G.as<double>(), Sinv.as<double>(), Y.as<double>(), fail.as<int>()); });
+    for (int i = 0; i < dm1; i += std::max(dm1 - 1, 1))  // only the first and the last block row are read below
+        L.run(KC_DENSE, 0, [&] { k_currents<<<dim3(cdiv(mn, 128), c->p[i]), 128, 0, L.s>>>(c->p[i], dm1, mn, F[i].as<double>(), Y.as<double>()); });
+    // operands of S4
+    const int p0 = c->p[0], pd = c->p[dm1 - 1];
+    c->p0 = p0;
+    c->A1.alloc((size_t)m * p0 * sizeof(double));
+    c->X0.alloc((size_t)n * p0 * sizeof(double));
+    c->u.alloc((size_t)m * sizeof(double));
+    c->w.alloc((size_t)n * sizeof(double));
+    L.run(KC_DENSE, 0, [&] { k_terminal_consts<<<cdiv(m, 128), 128, 0, L.s>>>(p0, dm1, mn, m, 0, 0, T0.ZT.as<double>(), T0.q, T0.ntsv, 0, F[0].as<double>(), Y.as<double>(), T0.zdiag.as<double>(), c->u.as<double>()); });
+    L.run(KC_DENSE, 0, [&] { k_terminal_consts<<<cdiv(n, 128), 128, 0, L.s>>>(pd, dm1, mn, n, m, 1, Td.ZT.as<double>(), Td.q, Td.ntsv, 0, F[dm1 - 1].as<double>(), Y.as<double>(), Td.zdiag.as<double>(), c->w.as<double>()); });
+    L.run(KC_DENSE, 0, [&] { k_pack_pair_operands<<<dim3(cdiv(p0, 128), mn), 128, 0, L.s>>>(p0, m, n, dm1, T0.ZT.as<double>(), T0.q, T0.ntsv, F[0].as<double>(), c->A1.as<double>(), c->X0.as<double>()); });
+    int h_fail = 0;
+    CK(cudaMemcpyAsync(&h_fail, fail.p, sizeof(int), cudaMemcpyDeviceToHost, L.s));
+    CK(cudaStreamSynchronize(L.s));
+    return h_fail ? PDN_E_NUMERIC : PDN_OK;
+}
+
+}  // namespace
+
+// ================================================================================================
+// C ABI
+// ================================================================================================
+extern "C" {
+
+const char* pdn_strerror(int status) {
+    switch (status) {
+        case PDN_OK: return "ok";
+        case PDN_E_ARG: return "invalid argument";
+        case PDN_E_DISCONNECTED: return "a tier is not connected";
+        case PDN_E_NOCONV: return "port solve did not converge within max_iter";
+        case PDN_E_CUDA: return "CUDA error";
+        case PDN_E_NOMEM: return "out of memory";
+        case PDN_E_NUMERIC: return "port-level matrix not positive definite";
+        default: return "unknown status";
+    }
+}
+
+const char* pdn_last_error(void) { return g_last_error.c_str(); }
+
+void pdn_destroy(pdn_ctx* ctx) {
+    if (!ctx) return;
+    for (cudaEvent_t e : ctx->event_pool) cudaEventDestroy(e);
+    for (auto& pe : ctx->pending_events) { cudaEventDestroy(pe.second.first); cudaEventDestroy(pe.second.second); }
+    delete ctx;
+}
+
+static int fail_arg(const char* msg) {
+    g_last_error = msg;
+    return PDN_E_ARG;
+}
+
+int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_tsv, const pdn_tsv* tsvs,
+               int32_t n_bumps, const pdn_site* bumps, int32_t n_loads, const pdn_site* loads, const pdn_opts* opts) {
+    if (!out) return fail_arg("out is null");
+    *out = nullptr;
+    if (!tiers || !tsvs || !bumps || !loads) return fail_arg("null input array");
+    if (n_tiers < 2) return fail_arg("need at least 2 tiers");
+    if (n_tsv < 1 || n_bumps < 1 || n_loads < 1) return fail_arg("need at least one TSV, bump and load");
+    const int d = n_tiers, n = tiers[0].n;
+    if (n < 2) return fail_arg("mesh size n must be >= 2");
+    if ((int64_t)n * n > (int64_t)1 << 30) return fail_arg("mesh too large");
+    for (int t = 0; t < d; ++t) {
+        if (tiers[t].n != n) return fail_arg("all tiers must have the same n");
+        if (!tiers[t].gx || !tiers[t].gy) return fail_arg("null conductance plane");
+    }
+    pdn_opts o{};
+    if (opts) o = *opts;
+    if (!(o.rtol > 0.0)) o.rtol = 1e-9;
+    if (o.max_iter <= 0) o.max_iter = 200;
+    if (o.nu <= 0) o.nu = 3;
+    if (o.nu > 4) o.nu = 4;
+
+    pdn_ctx* c = new (std::nothrow) pdn_ctx();
+    if (!c) return PDN_E_NOMEM;
+    int status = PDN_OK;
+    try {
+        c->d = d; c->n = n; c->m = n_bumps; c->nl = n_loads; c->opts = o;
+        c->stream = (cudaStream_t)o.cuda_stream;
+        c->time_kernels = (o.flags & PDN_TIME_KERNELS) != 0;
+        // ---- host-side validation and port lists
+        c->p.assign(d - 1, 0);
+        c->rt.assign(d - 1, {});
+        std::vector<std::vector<int>> site(d - 1);
+        std::vector<std::set<int>> seen(d - 1);
+        for (int k = 0; k < n_tsv; ++k) {
+            const pdn_tsv& t = tsvs[k];
+            if (t.iface < 0 || t.iface >= d - 1) throw StatusFail{PDN_E_ARG, "TSV interface out of range"};
+            if (t.y < 0 || t.y >= n || t.x < 0 || t.x >= n) throw StatusFail{PDN_E_ARG, "TSV site out of range"};
+            if (!(t.r_ohm > 0.0) || !std::isfinite(t.r_ohm)) throw StatusFail{PDN_E_ARG, "TSV resistance must be positive and finite"};
+            const int id = t.y * n + t.x;
+            if (!seen[t.iface].insert(id).second) throw StatusFail{PDN_E_ARG, "duplicate TSV site inside one interface"};
+            site[t.iface].push_back(id);
+            c->rt[t.iface].push_back(t.r_ohm);
+        }
+        for (int i = 0; i < d - 1; ++i) {
+            c->p[i] = (int)site[i].size();
+            if (c->p[i] == 0) throw StatusFail{PDN_E_ARG, "an interface has no TSV"};
+        }
+        auto check_sites = [&](const pdn_site* s, int cnt, std::vector<int>& ids) {
+            for (int k = 0; k < cnt; ++k) {
+                if (s[k].y < 0 || s[k].y >= n || s[k].x < 0 || s[k].x >= n) throw StatusFail{PDN_E_ARG, "bump/load site out of range"};
+                ids.push_back(s[k].y * n + s[k].x);
+            }
+        };
+        std::vector<int> bump_id, load_id;
+        check_sites(bumps, n_bumps, bump_id);
+        check_sites(loads, n_loads, load_id);
+
+        Launcher L{c, c->stream};
+        cudaEvent_t ev[4];
+        for (auto& e : ev) CK(cudaEventCreate(&e));
+        CK(cudaEventRecord(ev[0], L.s));
+
+        c->tiers.resize(d);
+        int qmax = 0;
+        for (int t = 0; t < d; ++t) {
+            TierPorts& T = c->tiers[t];
+            if (t > 0) T.node.insert(T.node.end(), site[t - 1].begin(), site[t - 1].end());
+            if (t < d - 1) T.node.insert(T.node.end(), site[t].begin(), site[t].end());
+            T.ntsv = (int)T.node.size();
+            if (t == 0) T.node.insert(T.node.end(), bump_id.begin(), bump_id.end());
+            if (t == d - 1) T.node.insert(T.node.end(), load_id.begin(), load_id.end());
+            T.q = (int)T.node.size();
+            T.nterm = T.q - T.ntsv;
+            T.d_node.alloc((size_t)T.q * sizeof(int));
+            CK(cudaMemcpyAsync(T.d_node.p, T.node.data(), (size_t)T.q * sizeof(int), cudaMemcpyHostToDevice, L.s));
+            T.ZT.alloc((size_t)T.ntsv * T.q * sizeof(double));
+            T.zdiag.alloc((size_t)std::max(T.nterm, 1) * sizeof(double));
+            qmax = std::max(qmax, T.q);
+            c->stats.n_ports_total += T.q;
+        }
+        c->stats.n_tiers = d;
+
+        // ---- S0 + S1, tier by tier
+        Hierarchy H;
+        H.allocate(n);
+        c->stats.n_levels = H.nlev;
+        DevBuf stage;  // staging for host-resident planes
+        if (o.flags & PDN_TIERS_ON_HOST) stage.alloc((size_t)2 * n * n * sizeof(double));
+        int Bmax = qmax;
+        if (H.nlev > 1) {
+            size_t free_b = 0, total_b = 0;
+            CK(cudaMemGetInfo(&free_b, &total_b));
+            const size_t per = Work::bytes_per_rhs(H) + (size_t)qmax * 8 + 128;
+            const size_t fit = std::max<size_t>(1, (size_t)(0.6 * (double)free_b) / per);
+            Bmax = (int)std::min<size_t>({(size_t)qmax, fit, (size_t)1024});
+            if (o.rhs_batch > 0) Bmax = std::min(Bmax, o.rhs_batch);
+        }
+        Work W;
+        if (H.nlev > 1) W.allocate(H, Bmax, qmax);
+        const Cheb ch = make_cheb(o.nu, 6.0);
+        const double rtol_term = std::max(o.rtol, std::min(1e-5, std::sqrt(o.rtol) / 3.0));
+        float ms_up = 0.f;
+        for (int t = 0; t < d && status == PDN_OK; ++t) {
+            TierPorts& T = c->tiers[t];
+            const double *gx = tiers[t].gx, *gy = tiers[t].gy;
+            CK(cudaEventRecord(ev[1], L.s));
+            if (o.flags & PDN_TIERS_ON_HOST) {
+                double* sg = stage.as<double>();
+                CK(cudaMemcpyAsync(sg, gx, (size_t)n * n * sizeof(double), cudaMemcpyHostToDevice, L.s));
+                CK(cudaMemcpyAsync(sg + (size_t)n * n, gy, (size_t)n * n * sizeof(double), cudaMemcpyHostToDevice, L.s));
+                gx = sg; gy = sg + (size_t)n * n;
+            }
+            status = H.build(L, gx, gy, !(o.flags & PDN_SKIP_CONNECTIVITY_CHECK));
+            CK(cudaEventRecord(ev[2], L.s));
+            CK(cudaEventSynchronize(ev[2]));
+            float ms = 0.f;
+            CK(cudaEventElapsedTime(&ms, ev[1], ev[2]));
+            ms_up += ms;
+            if (status != PDN_OK) { g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status); break; }
+            if (H.nlev == 1) {
+                L.run(KC_SMALL, 0, [&] { k_direct_small<<<T.q, 64, 0, L.s>>>(H.pinv.as<double>(), n * n, T.d_node.as<int>(), T.ntsv, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
+                continue;
+            }
+            for (int s0 = 0; s0 < T.ntsv && status == PDN_OK; s0 += Bmax)
+                status = solve_batch(c, L, H, W, T, ch, s0, std::min(Bmax, T.ntsv - s0), false, o.rtol, o.max_iter);
+            for (int s0 = T.ntsv; s0 < T.q && status == PDN_OK; s0 += Bmax)
+                status = solve_batch(c, L, H, W, T, ch, s0, std::min(Bmax, T.q - s0), true, rtol_term, o.max_iter);
+            if (status != PDN_OK) g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status);
+        }
+        CK(cudaEventRecord(ev[2], L.s));
+        // ---- S2 + S3
+        if (status == PDN_OK) {
+            status = recombine(c, L);
+            if (status != PDN_OK) g_last_error = pdn_strerror(status);
+        }
+        CK(cudaEventRecord(ev[3], L.s));
+        CK(cudaStreamSynchronize(L.s));
+        L.resolve();
+        float ms_all = 0.f, ms_dense = 0.f, ms_s01 = 0.f;
+        CK(cudaEventElapsedTime(&ms_all, ev[0], ev[3]));
+        CK(cudaEventElapsedTime(&ms_dense, ev[2], ev[3]));
+        CK(cudaEventElapsedTime(&ms_s01, ev[0], ev[2]));
+        c->stats.ms_total = ms_all; c->stats.ms_dense = ms_dense; c->stats.ms_upload = ms_up;
+        c->stats.ms_stencil = ms_s01 - ms_up;
+        for (auto& e : ev) cudaEventDestroy(e);
+    } catch (const CudaFail& f) {
+        g_last_error = std::string(f.what) + ": " + cudaGetErrorString(f.e);
+        cudaGetLastError();
+        status = f.e == cudaErrorMemoryAllocation ? PDN_E_NOMEM : PDN_E_CUDA;
+    } catch (const StatusFail& f) {
+        g_last_error = f.msg;
+        status = f.status;
+    } catch (const std::bad_alloc&) {
+        g_last_error = "host allocation failed";
+        status = PDN_E_NOMEM;
+    }
+    if (status != PDN_OK) {
+        pdn_destroy(c);
+        return status;
+    }
+    *out = c;
+    return PDN_OK;
+}
+
+static int reff_device(pdn_ctx* ctx, int64_t n_pairs, const int32_t* bi, const int32_t* li, double* out) {
+    Launcher L{ctx, ctx->stream};
+    const int m = ctx->m, n = ctx->nl, p0 = ctx->p0;
+    if (!bi) {
+        dim3 grid(cdiv(n, 64), cdiv(m, 64));
+        L.run(KC_PAIR, (double)n_pairs * 8.0, [&] { k_pair_full<<<grid, 256, 0, L.s>>>(m, n, p0, ctx->A1.as<double>(), ctx->X0.as<double>(), ctx->u.as<double>(), ctx->w.as<double>(), out); });
+    } else {
+        L.run(KC_PAIR, (double)n_pairs * 8.0, [&] { k_pair_list<<<cdiv((size_t)n_pairs * 32, 256), 256, 0, L.s>>>(n_pairs, m, n, p0, bi, li, ctx->A1.as<double>(), ctx->X0.as<double>(), ctx->u.as<double>(), ctx->w.as<double>(), out); });
+    }
+    return PDN_OK;
+}
+
+int pdn_reff(pdn_ctx* ctx, int64_t n_pairs, const int32_t* bump_idx, const int32_t* load_idx, double* out) {
+    if (!ctx || !out || n_pairs < 0) return fail_arg("null context / output or negative n_pairs");
+    if ((bump_idx == nullptr) != (load_idx == nullptr)) return fail_arg("bump_idx and load_idx must both be given or both be NULL");
+    if (!bump_idx && n_pairs != (int64_t)ctx->m * ctx->nl) return fail_arg("full cross product needs n_pairs == n_bumps*n_loads");
+    if (n_pairs == 0) return PDN_OK;
+    try {
+        reff_device(ctx, n_pairs, bump_idx, load_idx, out);
+        CK(cudaStreamSynchronize(ctx->stream));
+        Launcher{ctx, ctx->stream}.resolve();
+    } catch (const CudaFail& f) {
+        g_last_error = std::string(f.what) + ": " + cudaGetErrorString(f.e);
+        cudaGetLastError();
+        return PDN_E_CUDA;
+    }
+    return PDN_OK;
+}
+
+int pdn_reff_host(pdn_ctx* ctx, int64_t n_pairs, const int32_t* bump_idx, const int32_t* load_idx, double* out) {
+    if (!ctx || !out || n_pairs < 0) return fail_arg("null context / output or negative n_pairs");
+    if ((bump_idx == nullptr) != (load_idx == nullptr)) return fail_arg("bump_idx and load_idx must both be given or both be NULL");
+    if (!bump_idx && n_pairs != (int64_t)ctx->m * ctx->nl) return fail_arg("full cross product needs n_pairs == n_bumps*n_loads");
+    if (n_pairs == 0) return PDN_OK;
+    try {
+        DevBuf dout, dbi, dli;
+        dout.alloc((size_t)n_pairs * sizeof(double));
+        if (bump_idx) {
+            dbi.alloc((size_t)n_pairs * sizeof(int32_t));
+            dli.alloc((size_t)n_pairs * sizeof(int32_t));
+            CK(cudaMemcpyAsync(dbi.p, bump_idx, (size_t)n_pairs * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream));
+            CK(cudaMemcpyAsync(dli.p, load_idx, (size_t)n_pairs * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream));
+        }
+        reff_device(ctx, n_pairs, bump_idx ? dbi.as<int32_t>() : nullptr, bump_idx ? dli.as<int32_t>() : nullptr, dout.as<double>());
+        CK(cudaMemcpyAsync(out, dout.p, (size_t)n_pairs * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaStreamSynchronize(ctx->stream));
+        Launcher{ctx, ctx->stream}.resolve();
+    } catch (const CudaFail& f) {
+        g_last_error = std::string(f.what) + ": " + cudaGetErrorString(f.e);
+        cudaGetLastError();
+        return PDN_E_CUDA;
+    } catch (const StatusFail& f) {
+        g_last_error = f.msg;
+        return f.status;
+    }
+    return PDN_OK;
+}
+
+int pdn_get_stats(const pdn_ctx* ctx, pdn_stats* out) {
+    if (!ctx || !out) return fail_arg("null argument");
+    *out = ctx->stats;
+    out->stencil_bytes = 0.0;
+    for (int k = 0; k < KC_COUNT; ++k) {
+        out->class_ms[k] = ctx->class_ms[k];
+        out->class_bytes[k] = ctx->class_bytes[k];
+        out->class_launches[k] = ctx->class_launches[k];
+        if (k <= KC_SMALL) out->stencil_bytes += ctx->class_bytes[k];
+    }
+    return PDN_OK;
+}
+
+int32_t pdn_port_count(const pdn_ctx* ctx, int32_t tier) {
+    if (!ctx || tier < 0 || tier >= ctx->d) return -1;
+    return ctx->tiers[tier].q;
+}
+
+int pdn_get_port_matrix(const pdn_ctx* ctx, int32_t tier, double* out) {
+    if (!ctx || !out || tier < 0 || tier >= ctx->d) return fail_arg("bad tier or null output");
+    const TierPorts& T = ctx->tiers[tier];
+    try {
+        std::vector<double> zt((size_t)T.ntsv * T.q), zd((size_t)T.nterm);
+        CK(cudaMemcpy(zt.data(), T.ZT.p, zt.size() * sizeof(double), cudaMemcpyDeviceToHost));
+        if (T.nterm) CK(cudaMemcpy(zd.data(), T.zdiag.p, zd.size() * sizeof(double), cudaMemcpyDeviceToHost));
+        const double qnan = std::nan("");
+        for (int j = 0; j < T.q; ++j)
+            for (int k = 0; k < T.q; ++k) {
+                double v = qnan;
+                if (j < T.ntsv && k < T.ntsv) v = 0.5 * (zt[(size_t)j * T.q + k] + zt[(size_t)k * T.q + j]);
+                else if (j < T.ntsv) v = zt[(size_t)j * T.q + k];
+                else if (k < T.ntsv) v = zt[(size_t)k * T.q + j];
+                else if (j == k) v = zd[j - T.ntsv];
+                out[(size_t)j * T.q + k] = v;
+            }
+    } catch (const CudaFail& f) {
+        g_last_error = std::string(f.what) + ": " + cudaGetErrorString(f.e);
+        return PDN_E_CUDA;
+    }
+    return PDN_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,202 @@
+// S2 (assembly of the reusable coefficient matrix, Eq. 18), the multiplier part of S3,
+// and S4 (pair evaluation, Eq. 22) in the build's Z-notation.
+//
+// Per tier t the port reduction leaves  ZT_t[j][k] = (L_t^+)[port j, port k]  for the TSV ports j
+// (rows, ntsv_t of them) against ALL ports k of the tier (q_t columns), and zdiag_t[s] = (L_t^+)[s,s]
+// for the terminal ports (bumps on tier 0, loads on tier d-1).  Port order of tier t:
+//   [lower ends of interface t-1] ++ [upper ends of interface t] ++ [terminals].
+#pragma once
+#include "common.cuh"
+
+namespace pdn {
+
+// Diagonal block K_ii = sym(Z_i[up_i,up_i]) + sym(Z_{i+1}[lo_i,lo_i]) + diag(Rt_i)      (p x p)
+//   ZTa = ZT_i (ld qa), up_i ports start at offset oa;  ZTb = ZT_{i+1} (ld qb), lo_i ports start at 0.
+__global__ void k_assemble_diag(int p, const double* __restrict__ ZTa, int64_t qa, int oa,
+                                const double* __restrict__ ZTb, int64_t qb, const double* __restrict__ rt,
+                                double* __restrict__ Kii) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y;
+    if (b >= p) return;
+    double v = 0.5 * (ZTa[(oa + a) * qa + oa + b] + ZTa[(oa + b) * qa + oa + a]) +
+               0.5 * (ZTb[a * qb + b] + ZTb[b * qb + a]);
+    if (a == b) v += rt[a];
+    Kii[(int64_t)a * p + b] = v;
+}
+
+// Coupling block K_{i,i+1} = -sym-part of Z_{i+1}[lo_i, up_{i+1}]          (p_i x p_{i+1})
+//   ZT = ZT_{i+1} (ld q); lo_i ports at offset 0, up_{i+1} ports at offset p_i.
+__global__ void k_assemble_coupling(int pi, int pj, const double* __restrict__ ZT, int64_t q, double* __restrict__ V) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y;
+    if (b >= pj) return;
+    V[(int64_t)a * pj + b] = -0.5 * (ZT[a * q + pi + b] + ZT[(pi + b) * q + a]);
+}
+
+// Right-hand-side block row i of F = [F^1 | F^d | B]  (p_i x nrhs, nrhs = m + n + d-1), Eq. (19)/(21):
+//   block 0   , cols [0, m)      : Z_0[up_0, bump]       = ZT0[a][ntsv0 + s]
+//   block d-2 , cols [m, m+n)    : Z_{d-1}[lo_{d-2}, load] = ZTd[a][ntsvd + l]   (lo ports at offset 0)
+//   block i   , col  m+n+i       : 1   (the constraint column 1_{p_i}, Eq. 11)
+__global__ void k_assemble_rhs(int i, int dm1, int p, int m, int n, const double* __restrict__ ZT0, int64_t q0,
+                               int ntsv0, const double* __restrict__ ZTd, int64_t qd, int ntsvd,
+                               double* __restrict__ F) {
+    const int nrhs = m + n + dm1;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y;
+    if (c >= nrhs) return;
+    double v = 0.0;
+    if (c < m) {
+        if (i == 0) v = ZT0[a * q0 + ntsv0 + c];
+    } else if (c < m + n) {
+        if (i == dm1 - 1) v = ZTd[a * qd + ntsvd + (c - m)];
+    } else if (c - m - n == i) {
+        v = 1.0;
+    }
+    F[(int64_t)a * nrhs + c] = v;
+}
+
+// G[i][c] = sum over the rows of block i of T_i[a][c]   (= B^T K^-1 F)
+__global__ void k_colsum(int p, int nrhs, const double* __restrict__ T, double* __restrict__ Grow) {
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= nrhs) return;
+    double s = 0.0;
+    for (int a = 0; a < p; ++a) s += T[(int64_t)a * nrhs + c];
+    Grow[c] = s;
+}
+
+// Multipliers: S = G[:, m+n:] ((d-1)^2, SPD);  Y[i][c] = sum_k Sinv[i][k] (G[k][c] - 1/2) for c < m+n.
+// One block; thread 0 inverts S by Gauss-Jordan (d-1 is the number of interfaces, small).
+__global__ void k_multipliers(int dm1, int mn, const double* __restrict__ G, double* __restrict__ Sinv,
+                              double* __restrict__ Y, int* __restrict__ fail) {
+    const int nrhs = mn + dm1;
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < dm1; ++i)
+            for (int j = 0; j < dm1; ++j) Sinv[i * dm1 + j] = (i == j) ? 1.0 : 0.0;
+        // work on a copy of S stored behind Sinv
+        double* S = Sinv + dm1 * dm1;
+        for (int i = 0; i < dm1; ++i)
+            for (int j = 0; j < dm1; ++j) S[i * dm1 + j] = G[(int64_t)i * nrhs + mn + j];
+        for (int k = 0; k < dm1; ++k) {
+            const double piv = S[k * dm1 + k];
+            if (!(piv > 0.0)) { *fail = 1; break; }
+            const double inv = 1.0 / piv;
+            for (int j = 0; j < dm1; ++j) { S[k * dm1 + j] *= inv; Sinv[k * dm1 + j] *= inv; }
+            for (int i = 0; i < dm1; ++i) {
+                if (i == k) continue;
+                const double f = S[i * dm1 + k];
+                if (f == 0.0) continue;
+                for (int j = 0; j < dm1; ++j) {
+                    S[i * dm1 + j] -= f * S[k * dm1 + j];
+                    Sinv[i * dm1 + j] -= f * Sinv[k * dm1 + j];
+                }
+            }
+        }
+    }
+    __syncthreads();
+    for (int c = threadIdx.x; c < mn; c += blockDim.x)
+        for (int i = 0; i < dm1; ++i) {
+            double s = 0.0;
+            for (int k = 0; k < dm1; ++k) s = fma(Sinv[i * dm1 + k], G[(int64_t)k * nrhs + c] - 0.5, s);
+            Y[(int64_t)i * mn + c] = s;
+        }
+}
+
+// TSV currents of block row i:  I[a][c] = T[a][c] - sum_k T[a][m+n+k] Y[k][c]   for c < m+n  (in place)
+__global__ void k_currents(int p, int dm1, int mn, double* __restrict__ T, const double* __restrict__ Y) {
+    const int nrhs = mn + dm1;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y;
+    if (c >= mn) return;
+    double v = T[(int64_t)a * nrhs + c];
+    for (int k = 0; k < dm1; ++k) v = fma(-T[(int64_t)a * nrhs + mn + k], Y[(int64_t)k * mn + c], v);
+    T[(int64_t)a * nrhs + c] = v;
+}
+
+// Terminal constants (one thread per terminal column c of the first / last block row):
+//   s = zdiag[c] - ( sum_a f[a][c] I[a][c] + 1/2 sum_k Y[k][col] )  [ - sum_k Y[k][col]  for loads ]
+// f[a][c] = ZT[a*q + ntsv + c] (original right-hand side), I = solved block row (ld nrhs, column col0 + c).
+__global__ void k_terminal_consts(int p, int dm1, int mn, int nterm, int col0, int is_load,
+                                  const double* __restrict__ ZT, int64_t q, int ntsv, int row_off,
+                                  const double* __restrict__ I, const double* __restrict__ Y,
+                                  const double* __restrict__ zdiag, double* __restrict__ out) {
+    const int nrhs = mn + dm1;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= nterm) return;
+    double s = 0.0;
+    for (int a = 0; a < p; ++a) s = fma(ZT[(int64_t)(row_off + a) * q + ntsv + c], I[(int64_t)a * nrhs + col0 + c], s);
+    double ys = 0.0;
+    for (int k = 0; k < dm1; ++k) ys += Y[(int64_t)k * mn + col0 + c];
+    out[c] = zdiag[c] - (s + 0.5 * ys) - (is_load ? ys : 0.0);
+}
+
+// Packed operands of the pair kernel:  A1[s][a] = Z_0[up_0 a, bump s]  (m x p0);
+//                                      X0[l][a] = I_{load l}[block 0, a]  (n x p0).
+__global__ void k_pack_pair_operands(int p0, int m, int n, int dm1, const double* __restrict__ ZT0, int64_t q0,
+                                     int ntsv0, const double* __restrict__ I0, double* __restrict__ A1,
+                                     double* __restrict__ X0) {
+    const int nrhs = m + n + dm1;
+    const int a = blockIdx.x * blockDim.x + threadIdx.x, row = blockIdx.y;
+    if (a >= p0) return;
+    if (row < m) A1[(int64_t)row * p0 + a] = ZT0[(int64_t)a * q0 + ntsv0 + row];
+    else X0[(int64_t)(row - m) * p0 + a] = I0[(int64_t)a * nrhs + m + (row - m)];
+}
+
+// S4, full cross product:  R[i][j] = u[i] + w[j] - 2 sum_a A1[i][a] X0[j][a].   64x64 tile / block.
+__global__ void __launch_bounds__(256)
+k_pair_full(int m, int n, int p0, const double* __restrict__ A1, const double* __restrict__ X0,
+            const double* __restrict__ u, const double* __restrict__ w, double* __restrict__ R) {
+    __shared__ double As[16][65];
+    __shared__ double Bs[16][65];
+    const int tid = threadIdx.x, tx = tid % 16, ty = tid / 16;
+    const int i0 = blockIdx.y * 64, j0 = blockIdx.x * 64;
+    double acc[4][4] = {};
+    for (int k0 = 0; k0 < p0; k0 += 16) {
+        for (int e = tid; e < 16 * 64; e += 256) {
+            const int kk = e % 16, ii = e / 16;
+            As[kk][ii] = (i0 + ii < m && k0 + kk < p0) ? A1[(int64_t)(i0 + ii) * p0 + k0 + kk] : 0.0;
+            Bs[kk][ii] = (j0 + ii < n && k0 + kk < p0) ? X0[(int64_t)(j0 + ii) * p0 + k0 + kk] : 0.0;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int kk = 0; kk < 16; ++kk) {
+            double a[4], b[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) a[r] = As[kk][ty * 4 + r];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) b[c] = Bs[kk][tx + 16 * c];
+#pragma unroll
+            for (int r = 0; r < 4; ++r)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) acc[r][c] = fma(a[r], b[c], acc[r][c]);
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int i = i0 + ty * 4 + r;
+        if (i >= m) continue;
+        const double ui = u[i];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int j = j0 + tx + 16 * c;
+            if (j < n) R[(int64_t)i * n + j] = ui + w[j] - 2.0 * acc[r][c];
+        }
+    }
+}
+
+// S4, pair list: one warp per pair.
+__global__ void k_pair_list(int64_t npairs, int m, int n, int p0, const int* __restrict__ bi,
+                            const int* __restrict__ li, const double* __restrict__ A1,
+                            const double* __restrict__ X0, const double* __restrict__ u,
+                            const double* __restrict__ w, double* __restrict__ R) {
+    const int64_t pair = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (pair >= npairs) return;
+    const int i = bi[pair], j = li[pair];
+    if (i < 0 || i >= m || j < 0 || j >= n) {
+        if (lane == 0) R[pair] = nan("");
+        return;
+    }
+    double s = 0.0;
+    for (int a = lane; a < p0; a += 32) s = fma(A1[(int64_t)i * p0 + a], X0[(int64_t)j * p0 + a], s);
+    s = warp_sum(s);
+    if (lane == 0) R[pair] = u[i] + w[j] - 2.0 * s;
+}
+
+}  // namespace pdn

@@ -1,0 +1,218 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle, element by element.
+
+Tolerance (BASELINE.json north_star): per pair |R_gpu - R_oracle| / R_oracle, max <= 1e-6 and
+mean <= 1e-8.  Workloads 1-2: the full cross product; workloads 3-5: the seeded 4096-pair sample.
+Expected values for the five workloads are the oracle's, stored under tests/golden/ by
+tests/golden/make_golden.py (which calls only oracle/); small cases run the oracle live.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import pdn_inputs as P
+
+pytestmark = pytest.mark.gpu
+
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+MAX_REL, MEAN_REL = 1e-6, 1e-8
+
+
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("CUDA device required for -m gpu tests (no CPU fallback exists)")
+    return torch
+
+
+def load_golden(cfg):
+    path = os.path.join(GOLDEN, f"cfg{cfg}_reff.txt")
+    if not os.path.exists(path):
+        pytest.skip(f"{path} not generated yet (tests/golden/make_golden.py {cfg})")
+    a = np.loadtxt(path, comments="#")
+    return a[:, 0].astype(np.int32), a[:, 1].astype(np.int32), a[:, 2]
+
+
+def check(got, want):
+    rel = np.abs(got - want) / want
+    assert np.all(np.isfinite(got))
+    assert rel.max() <= MAX_REL, f"max rel err {rel.max():.3e}"
+    assert rel.mean() <= MEAN_REL, f"mean rel err {rel.mean():.3e}"
+    return rel
+
+
+def gpu_all_pairs(net, **kw):
+    torch = torch_cuda()
+    from paper_2607_05818_b200 import Pdn
+    pdn = Pdn.from_network(net, device="cuda:0", **kw)
+    out = torch.empty(net.m * net.nl, dtype=torch.float64, device="cuda:0")
+    pdn.reff(out)
+    st = pdn.stats()
+    pdn.close()
+    return out.cpu().numpy().reshape(net.m, net.nl), st
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_workload_full_cross_product(cfg):
+    bi, li, want = load_golden(cfg)
+    net = P.make_config(cfg, seed=0)
+    got, st = gpu_all_pairs(net)
+    rel = check(got[bi, li], want)
+    print(f"cfg{cfg}: max {rel.max():.2e} mean {rel.mean():.2e} iters {st['pcg_iters_max']}")
+
+
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_workload_sampled_pairs(cfg):
+    """Full-size workloads in the launch configuration bench.py times; pair-list mode of pdn_reff."""
+    torch = torch_cuda()
+    from paper_2607_05818_b200 import Pdn
+    bi, li, want = load_golden(cfg)
+    net = P.make_config(cfg, seed=0)
+    sbi, sli = P.sample_pairs(net, 4096, seed=0, cfg=cfg)
+    assert np.array_equal(sbi, bi) and np.array_equal(sli, li)
+    pdn = Pdn.from_network(net, device="cuda:0")
+    out = torch.empty(bi.size, dtype=torch.float64, device="cuda:0")
+    pdn.reff(out, torch.from_numpy(bi).cuda(), torch.from_numpy(li).cuda())
+    rel = check(out.cpu().numpy(), want)
+    # the full cross product agrees with the gathered list
+    full = torch.empty(net.m * net.nl, dtype=torch.float64, device="cuda:0")
+    pdn.reff(full)
+    full = full.cpu().numpy().reshape(net.m, net.nl)
+    assert np.array_equal(full[bi, li], out.cpu().numpy())
+    st = pdn.stats()
+    pdn.close()
+    print(f"cfg{cfg}: max {rel.max():.2e} mean {rel.mean():.2e} iters {st['pcg_iters_max']} "
+          f"stencil {st['ms_stencil']:.0f} ms dense {st['ms_dense']:.1f} ms")
+
+
+@pytest.mark.parametrize("seed,d,n,p,m,nl,kw", [
+    (0, 2, 2, 1, 1, 1, {}),                 # smallest legal mesh (single level)
+    (1, 3, 3, 2, 2, 3, {}),
+    (2, 2, 4, 3, 4, 4, {}),                 # n = 4: the mesh is its own coarsest level
+    (3, 4, 5, 4, 3, 3, {}),                 # first two-level size, odd
+    (4, 3, 7, 5, 4, 6, dict(drop=0.1)),
+    (5, 2, 8, 6, 5, 5, dict(aniso=3.0)),
+    (6, 3, 13, 7, 6, 4, dict(drop=0.08, aniso=2.0)),   # odd sizes on every level: 13, 7, 4
+    (7, 2, 33, 9, 8, 8, {}),                # one node more than a tile: ragged tail
+    (8, 4, 40, 11, 5, 9, dict(drop=0.05)),
+    (9, 2, 70, 16, 6, 7, dict(aniso=0.25)), # several tiles + ragged tail
+    (10, 3, 100, 5, 3, 12, dict(drop=0.02, aniso=3.0)),
+])
+def test_random_stacks_against_live_oracle(seed, d, n, p, m, nl, kw):
+    from oracle.reff_oracle import Oracle
+    net = P.make_random(seed, d=d, n=n, p=p, m=m, nl=nl, **kw)
+    want = Oracle(net).reff_all()
+    got, _ = gpu_all_pairs(net, rtol=1e-10)
+    check(got, want)
+
+
+@pytest.mark.parametrize("nu", [1, 2, 3, 4])
+def test_every_smoother_depth(nu):
+    from oracle.reff_oracle import Oracle
+    net = P.make_random(20 + nu, d=2, n=45, p=6, m=4, nl=4, drop=0.03)
+    got, st = gpu_all_pairs(net, nu=nu, rtol=1e-10)
+    check(got, Oracle(net).reff_all())
+
+
+def test_small_rhs_batches_and_host_planes_give_same_answer():
+    torch = torch_cuda()
+    from paper_2607_05818_b200 import Pdn
+    net = P.make_config(1, seed=0)
+    ref, _ = gpu_all_pairs(net)
+    got, _ = gpu_all_pairs(net, rhs_batch=3)          # ragged batches: 16 = 5*3 + 1, 4 = 3 + 1
+    assert np.allclose(got, ref, rtol=1e-8, atol=0)
+    pdn = Pdn.from_network(net)                       # numpy planes => PDN_TIERS_ON_HOST
+    out = np.empty(net.m * net.nl)
+    pdn.reff_host(out)
+    assert np.allclose(out.reshape(net.m, net.nl), ref, rtol=1e-8, atol=0)
+    bi = np.array([3, 0, 2], dtype=np.int32)
+    li = np.array([15, 7, 0], dtype=np.int32)
+    out3 = np.empty(3)
+    pdn.reff_host(out3, bi, li)
+    assert np.array_equal(out3, out.reshape(net.m, net.nl)[bi, li])
+    pdn.close()
+
+
+def test_port_matrix_matches_wu_closed_form():
+    """S1 pin: on a uniform tier the intra-die R_jk = Z_jj + Z_kk - 2 Z_jk from the GPU port matrix
+    must equal PAPER.md:49 Eq. (3)."""
+    from closed_forms import wu_mesh_reff
+    from paper_2607_05818_b200 import Pdn
+    torch_cuda()
+    n, rx, ry = 24, 0.8, 1.7
+    sites = [np.array([[1, 2], [20, 5], [11, 11], [23, 23], [0, 17]])]
+    bumps = np.array([[3, 3], [9, 21]])
+    loads = np.array([[5, 5]])
+    net = P.make_uniform(2, n, rx, ry, rt=0.1, tsv_sites=sites, bumps=bumps, loads=loads)
+    pdn = Pdn.from_network(net, device="cuda:0", rtol=1e-11)
+    Z = pdn.port_matrix(0)
+    pdn.close()
+    pts = [tuple(s) for s in sites[0]] + [tuple(b) for b in bumps]
+    assert Z.shape == (7, 7)
+    for j in range(7):
+        for k in range(5):                      # column must be a TSV port (bump-bump entries are not computed)
+            if j == k:
+                continue
+            (y1, x1), (y2, x2) = pts[j], pts[k]
+            want = wu_mesh_reff(n, n, rx, ry, x1, y1, x2, y2)
+            got = Z[j, j] + Z[k, k] - 2 * Z[j, k]
+            assert got == pytest.approx(want, rel=1e-8)
+    assert np.isnan(Z[5, 6]) and np.isnan(Z[6, 5])
+
+
+def test_bump_on_tsv_site_and_shared_sites_between_interfaces():
+    from oracle.reff_oracle import Oracle
+    sites = [np.array([[2, 2], [5, 1]]), np.array([[2, 2], [0, 6]])]     # (2,2) used by both interfaces
+    net = P.make_random(31, d=3, n=9, p=2, m=2, nl=2)
+    net.tsv_site = [s.astype(np.int32) for s in sites]
+    net.bumps = np.array([[2, 2], [8, 8]], dtype=np.int32)              # bump 0 sits on a TSV site
+    net.loads = np.array([[0, 6], [4, 4]], dtype=np.int32)              # load 0 sits on a TSV site
+    got, _ = gpu_all_pairs(net, rtol=1e-10)
+    check(got, Oracle(net).reff_all())
+
+
+def test_out_of_range_pair_index_yields_nan():
+    torch = torch_cuda()
+    from paper_2607_05818_b200 import Pdn
+    net = P.make_config(1, seed=0)
+    pdn = Pdn.from_network(net, device="cuda:0")
+    bi = torch.tensor([0, 4, -1], dtype=torch.int32, device="cuda:0")
+    li = torch.tensor([0, 0, 3], dtype=torch.int32, device="cuda:0")
+    out = torch.zeros(3, dtype=torch.float64, device="cuda:0")
+    pdn.reff(out, bi, li)
+    o = out.cpu().numpy()
+    assert np.isfinite(o[0]) and np.isnan(o[1]) and np.isnan(o[2])
+    pdn.close()
+
+
+def test_error_statuses():
+    torch_cuda()
+    from paper_2607_05818_b200 import Pdn, PdnError
+    net = P.make_config(1, seed=0)
+
+    def expect(status, mutate):
+        bad = P.make_config(1, seed=0)
+        mutate(bad)
+        with pytest.raises(PdnError) as e:
+            Pdn.from_network(bad, device="cuda:0")
+        assert e.value.status == status
+
+    expect(1, lambda b: b.tsv_site.__setitem__(0, np.vstack([b.tsv_site[0][:-1], b.tsv_site[0][:1]])))  # duplicate
+    expect(1, lambda b: b.tsv_r.__setitem__(0, -b.tsv_r[0]))                                            # r <= 0
+    expect(1, lambda b: setattr(b, "bumps", np.array([[32, 0]], dtype=np.int32)))                       # out of range
+    expect(1, lambda b: b.gx[0].__setitem__((3, 3), -1.0))                                              # negative g
+    expect(1, lambda b: b.gy[1].__setitem__((3, 3), np.nan))
+
+    def cut(b):   # split tier 1 in two halves
+        b.gx[1][:, 15] = 0.0
+    expect(2, cut)
+    # isolated node
+    def isolate(b):
+        b.gx[0][4, 4] = b.gx[0][4, 3] = b.gy[0][4, 4] = b.gy[0][3, 4] = 0.0
+    expect(2, isolate)
+    # wrong n_pairs for the cross product
+    import torch
+    pdn = Pdn.from_network(net, device="cuda:0")
+    with pytest.raises(PdnError):
+        pdn.reff(torch.empty(5, dtype=torch.float64, device="cuda:0"))
+    pdn.close()
