@@ -1,0 +1,278 @@
+#!/usr/bin/env python
+"""Benchmark of the bump x load effective-resistance path (BASELINE.json metric: pairs/sec, FP64).
+
+One "step" = one pass of the whole hot path over one synthetic workload: pdn_create (S0 tier import,
+S1 batched port reduction, S2 assembly, S3 factor + substitution) + pdn_reff for the full bump x load
+cross product (S4) + pdn_destroy.  `value` times it with the conductance planes already resident in
+HBM and the result left on the device; `e2e` times the same through the host-buffer entry points
+(planes in pinned host memory, result copied back to the host) -- copies inside the timed region.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl reference]
+
+N > 1 (torchrun): every rank runs its own independent network of the same workload (seed = rank): the
+path has no cross-problem exchange, so this is weak scaling without a collective (multi-GPU).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import pdn_inputs as P  # noqa: E402
+
+METRIC = "bump-load R_eff pairs/sec (FP64)"
+UNIT = "pairs/s"
+
+
+def workload_name(cfg):
+    c = P.CONFIGS[cfg]
+    return (f"configs[{cfg - 1}]: {c['d']} tiers x {c['n']}^2 mesh, {c['p']} TSV/interface, "
+            f"{c['m']}x{c['nl']} pairs")
+
+
+# ----------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100", "-i", str(gpu_index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        rows = [l.split(", ") for l in open(self.f.name).read().strip().splitlines() if l.count(",") >= 8]
+        os.unlink(self.f.name)
+        if not rows:
+            return out
+        sm = [float(r[1]) for r in rows if r[1].replace(".", "").isdigit()]
+        out["sm_mhz"] = float(np.median(sm)) if sm else None
+        out["sm_max_mhz"] = float(rows[0][2]) if rows[0][2].replace(".", "").isdigit() else None
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        out["reasons"] = [n for k, n in enumerate(names) if any(r[5 + k].strip() == "Active" for r in rows)]
+        out["samples"] = len(rows)
+        return out
+
+
+# ----------------------------------------------------------------------------------------- oracle arm
+def oracle_sample(cfg, budget_s, max_pairs=4096):
+    """Times the oracle as it stands on a bounded sample of workload `cfg` (1 core: SuperLU is serial).
+    Returns (pairs_per_s of the per-pair solves, dict describing the sample)."""
+    from oracle.reff_oracle import Oracle
+    net = P.make_config(cfg, seed=0)
+    t0 = time.perf_counter()
+    o = Oracle(net)
+    t_factor = time.perf_counter() - t0
+    bi, li = P.sample_pairs(net, max_pairs, seed=0, cfg=cfg)
+    done = 0
+    t1 = time.perf_counter()
+    while done < max_pairs:
+        o.reff(int(bi[done]), int(li[done]))
+        done += 1
+        if time.perf_counter() - t1 > budget_s:
+            break
+    t_pairs = time.perf_counter() - t1
+    return done / t_pairs, dict(kind="oracle", cores=1, factor_s=round(t_factor, 2), pairs=done,
+                                pairs_s=round(t_pairs, 2),
+                                sample=f"sparse LU of the whole 3D system once ({t_factor:.1f} s, not counted in "
+                                       f"value) + {done} seeded pairs solved one at a time in {t_pairs:.1f} s")
+
+
+def run_reference(a):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = a.config
+    per_step = []
+    desc = None
+    for s in range(a.warmup + a.steps):
+        v, desc = oracle_sample(cfg, budget_s=max(2.0, 20.0 / (a.warmup + a.steps)), max_pairs=256)
+        if s >= a.warmup:
+            per_step.append(v)
+    value = float(np.mean(per_step))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps,
+            "warmup": a.warmup, "ms_per_step": 1e3 * desc["pairs"] / value, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(cfg)},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc["sample"]},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+# ----------------------------------------------------------------------------------------- CUDA arm
+def run_cuda(a):
+    import torch
+    import torch.distributed as dist
+    from paper_2607_05818_b200 import PDN_TIME_KERNELS, Pdn
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = a.config
+    net = P.make_config(cfg, seed=rank)          # one independent network per rank
+    npairs = net.m * net.nl
+    gx_d = [torch.from_numpy(g).to(dev) for g in net.gx]
+    gy_d = [torch.from_numpy(g).to(dev) for g in net.gy]
+    gx_h = [torch.from_numpy(g).pin_memory() for g in net.gx]
+    gy_h = [torch.from_numpy(g).pin_memory() for g in net.gy]
+    out_d = torch.empty(npairs, dtype=torch.float64, device=dev)
+    out_h = torch.empty(npairs, dtype=torch.float64).pin_memory()
+    args = (net.n,), (net.tsv_site, net.tsv_r, net.bumps, net.loads)
+
+    def step_device(flags=0):
+        pdn = Pdn(net.n, gx_d, gy_d, *args[1], flags=flags, rtol=a.rtol, nu=a.nu, rhs_batch=a.rhs_batch)
+        pdn.reff(out_d)
+        st = pdn.stats()
+        pdn.close()
+        return st
+
+    def step_host():
+        pdn = Pdn(net.n, gx_h, gy_h, *args[1], rtol=a.rtol, nu=a.nu, rhs_batch=a.rhs_batch)
+        pdn.reff_host(out_h)
+        pdn.close()
+
+    def timed(fn, steps):
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        res = [fn() for _ in range(steps)]
+        e1.record()
+        barrier()
+        ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+        return float(ms.item()), res
+
+    for _ in range(a.warmup):
+        step_device()
+    sampler = ClockSampler(local) if rank == 0 else None
+    ms, stats = timed(lambda: step_device(), a.steps)
+    clocks = sampler.stop() if sampler else None
+    value = world * npairs * a.steps / (ms * 1e-3)
+
+    if a.only_device:   # used under ncu: no extra legs, no JSON contract
+        if rank == 0:
+            print(json.dumps({"only_device": True, "value": value, "ms_per_step": ms / a.steps}))
+        return
+    # per-kernel-class device time (CUDA events on the launching stream around every launch)
+    ms_prof, pstats = timed(lambda: step_device(PDN_TIME_KERNELS), a.steps)
+    # end to end through the host-buffer entry points
+    step_host()
+    ms_e2e, _ = timed(step_host, a.steps)
+    e2e_value = world * npairs * a.steps / (ms_e2e * 1e-3)
+    h2d = sum(g.numel() * 8 for g in gx_h) * 2
+    d2h = npairs * 8
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peaks = {}
+    pk_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(pk_path):
+        peaks = json.load(open(pk_path))
+    peak = float(peaks.get("hbm_gbs", 6650.0))
+    peak_src = "measured (MEASURED_PEAKS.json, sustained copy)" if "hbm_gbs" in peaks else "fallback 6650 GB/s"
+    st = pstats[-1]
+    cls_ms = {k: sum(s["class_ms"][k] for s in pstats) for k in st["class_ms"]}
+    cls_by = {k: sum(s["class_bytes"][k] for s in pstats) for k in st["class_bytes"]}
+    cls_n = {k: sum(s["class_launches"][k] for s in pstats) for k in st["class_launches"]}
+    stencil_classes = ["pq", "down0", "up0", "down_coarse", "up_coarse"]
+    dom = max(stencil_classes, key=lambda k: cls_ms[k])
+    ach = cls_by[dom] / (cls_ms[dom] * 1e-3) / 1e9 if cls_ms[dom] > 0 else 0.0
+    tot_ms = sum(cls_ms[k] for k in stencil_classes)
+    tot_by = sum(cls_by[k] for k in stencil_classes)
+    phase = tot_by / (tot_ms * 1e-3) / 1e9 if tot_ms > 0 else 0.0
+    traffic = None
+    tr_path = os.path.join(ROOT, "profiles", "ncu_traffic.json")     # dram bytes per launch from the ncu capture
+    if os.path.exists(tr_path):
+        traffic = json.load(open(tr_path)).get(f"cfg{cfg}", {}).get(dom)
+
+    last = stats[-1]
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
+        "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "cfg": cfg, "pairs_per_step_per_gpu": npairs,
+                   "l2": "working set of every stencil launch exceeds the 126 MB L2 (no flush needed)"
+                         if cfg >= 3 else "working set fits L2: latency-bound case, HBM fraction not meaningful",
+                   "rtol": a.rtol or 1e-9, "nu": a.nu or 3,
+                   "pcg_iters_max": last["pcg_iters_max"], "rhs_iterations": last["rhs_iterations"],
+                   "ms_stencil": last["ms_stencil"], "ms_dense": last["ms_dense"], "ms_upload": last["ms_upload"]},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": ms_e2e / a.steps},
+        "gpu_launches": int(sum(s["kernel_launches"] for s in stats)),
+        "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
+                     "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
+                     "launches": int(cls_n[dom]), "avg_launch_ms": cls_ms[dom] / max(cls_n[dom], 1),
+                     "alg_bytes_per_launch": cls_by[dom] / max(cls_n[dom], 1),
+                     "stencil_phase": {"achieved": phase, "frac": phase / peak, "ms": tot_ms,
+                                       "share_of_step": tot_ms / ms_prof if ms_prof else None},
+                     "classes": {k: {"ms": cls_ms[k], "GBps": (cls_by[k] / (cls_ms[k] * 1e-3) / 1e9) if cls_ms[k] > 0 else 0.0,
+                                     "launches": int(cls_n[k])} for k in cls_ms}},
+    }
+    if not a.no_cpu_baseline:
+        v, desc = oracle_sample(cfg, budget_s=a.cpu_budget)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc["sample"]}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--rtol", type=float, default=0.0)
+    ap.add_argument("--nu", type=int, default=0)
+    ap.add_argument("--rhs-batch", type=int, default=0)
+    ap.add_argument("--cpu-budget", type=float, default=12.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--only-device", action="store_true", help="run only the device-resident steps (for ncu)")
+    a = ap.parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_cuda(a)
+
+
+if __name__ == "__main__":
+    main()

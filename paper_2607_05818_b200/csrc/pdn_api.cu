@@ -10,6 +10,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <set>
@@ -23,6 +24,7 @@
 #include "port.cuh"
 #include "setup.cuh"
 #include "stencil.cuh"
+#include "stencil2.cuh"
 
 using namespace pdn;
 
@@ -225,6 +227,22 @@ Cheb make_cheb(int nu, double ratio) {
     return c;
 }
 
+ChebR make_cheb_roots(int nu, double ratio) {
+    ChebR c{};
+    c.nu = nu;
+    const double lmax = 2.0, lmin = lmax / ratio;
+    const double theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin);
+    for (int k = 0; k < nu; ++k) c.w[k] = 1.0 / (theta + delta * std::cos(M_PI * (2 * k + 1) / (2.0 * nu)));
+    return c;
+}
+
+struct Smoother {  // both parametrisations of the same polynomial (v1 kernels use Cheb, v2 ChebR)
+    Cheb ch;
+    ChebR cr;
+    bool v1;
+    int G;
+};
+
 // ------------------------------------------------------------------------------------------------
 // S1 workspace of one batch of right-hand sides.
 struct Work {
@@ -289,6 +307,39 @@ void launch_up(Launcher& L, int cls, double bytes, const Level& lv, const Cheb& 
     L.run(cls, bytes, [&] { k_up<TI, NU><<<grid, STENCIL_THREADS, smem, L.s>>>(lv, ch, r, z_in, ec, cny, cnx, z_out, rz_acc); });
 }
 
+template <int NU>
+void launch_down2(Launcher& L, int cls, double bytes, const Level& lv, const ChebR& ch, int B, int G, const double* r_in,
+                  const double* q, const double* alpha, double* r_out, double* z_out, double* rc, int cny, int cnx,
+                  double* rr_acc) {
+    constexpr int IW = T2_EW - 2 * NU, IH = T2_EH - 2 * NU;
+    dim3 grid(cdiv(lv.nx, IW), cdiv(lv.ny, IH), cdiv(B, G));
+    constexpr size_t stage1 = (size_t)2 * T2_R * T2_THREADS * sizeof(double);  // two stages of one array
+    static bool attr_done = false;
+    if (!attr_done) {
+        CK(cudaFuncSetAttribute(k_down2<NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * stage1)));
+        CK(cudaFuncSetAttribute(k_down2<NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stage1));
+        attr_done = true;
+    }
+    if (q) L.run(cls, bytes, [&] { k_down2<NU, true><<<grid, T2_THREADS, 2 * stage1, L.s>>>(lv, ch, r_in, q, alpha, r_out, z_out, rc, cny, cnx, rr_acc, B, G); });
+    else L.run(cls, bytes, [&] { k_down2<NU, false><<<grid, T2_THREADS, stage1, L.s>>>(lv, ch, r_in, q, alpha, r_out, z_out, rc, cny, cnx, rr_acc, B, G); });
+}
+
+template <int NU>
+void launch_up2(Launcher& L, int cls, double bytes, const Level& lv, const ChebR& ch, int B, int G, const double* r,
+                const double* z_in, const double* ec, int cny, int cnx, double* z_out, double* rz_acc) {
+    constexpr int IW = T2_EW - 2 * NU, IH = T2_EH - 2 * NU;
+    dim3 grid(cdiv(lv.nx, IW), cdiv(lv.ny, IH), cdiv(B, G));
+    constexpr size_t stage3 = (size_t)2 * 3 * T2_R * T2_THREADS * sizeof(double);
+    static bool attr_done = false;
+    if (!attr_done) {
+        CK(cudaFuncSetAttribute(k_up2<NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stage3));
+        CK(cudaFuncSetAttribute(k_up2<NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stage3));
+        attr_done = true;
+    }
+    if (rz_acc) L.run(cls, bytes, [&] { k_up2<NU, true><<<grid, T2_THREADS, stage3, L.s>>>(lv, ch, r, z_in, ec, cny, cnx, z_out, rz_acc, B, G); });
+    else L.run(cls, bytes, [&] { k_up2<NU, false><<<grid, T2_THREADS, stage3, L.s>>>(lv, ch, r, z_in, ec, cny, cnx, z_out, rz_acc, B, G); });
+}
+
 #define NU_DISPATCH(nu, CALL)                 \
     switch (nu) {                             \
         case 1: { constexpr int NU_ = 1; CALL; } break; \
@@ -302,8 +353,9 @@ void launch_up(Launcher& L, int cls, double bytes, const Level& lv, const Cheb& 
 // `after_down0` runs right after the level-0 down stage was enqueued (the convergence check); if it
 // returns true the rest of the cycle is skipped.
 template <class F>
-void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Cheb& ch, int B, const double* r_in, const double* q,
+void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Smoother& sm, int B, const double* r_in, const double* q,
             double* r_out, F&& after_down0) {
+    const Cheb& ch = sm.ch;
     const int nl = H.nlev;
     const double* r_use = q ? r_out : r_in;  // the residual the rest of the cycle works with
     if (nl == 1) {  // the mesh itself is the coarsest level
@@ -320,9 +372,15 @@ void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Cheb& ch, int B, con
         double* zout = l == 0 ? W.z0[0].as<double>() : W.za[l].as<double>();
         const bool fused = (l == 0 && q);
         const double bytes = (fused ? 4.0 : 2.0) * V + Vc;
-        NU_DISPATCH(ch.nu, (launch_down<NU_>(L, l == 0 ? KC_DOWN0 : KC_DOWNC, bytes, H.lev[l], ch, B, rin, fused ? q : nullptr,
-                                             W.s.alpha, fused ? r_out : nullptr, zout, W.rl[l + 1].as<double>(),
-                                             H.ny[l + 1], H.nx[l + 1], W.s.rr)));
+        if (sm.v1) {
+            NU_DISPATCH(ch.nu, (launch_down<NU_>(L, l == 0 ? KC_DOWN0 : KC_DOWNC, bytes, H.lev[l], ch, B, rin, fused ? q : nullptr,
+                                                 W.s.alpha, fused ? r_out : nullptr, zout, W.rl[l + 1].as<double>(),
+                                                 H.ny[l + 1], H.nx[l + 1], W.s.rr)));
+        } else {
+            NU_DISPATCH(ch.nu, (launch_down2<NU_>(L, l == 0 ? KC_DOWN0 : KC_DOWNC, bytes, H.lev[l], sm.cr, B, sm.G, rin, fused ? q : nullptr,
+                                                  W.s.alpha, fused ? r_out : nullptr, zout, W.rl[l + 1].as<double>(),
+                                                  H.ny[l + 1], H.nx[l + 1], W.s.rr)));
+        }
         if (l == 0 && after_down0()) return;  // converged (or out of iterations): skip the rest of the cycle
     }
     const int lc = nl - 1, nc = H.ny[lc] * H.nx[lc];
@@ -333,18 +391,23 @@ void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Cheb& ch, int B, con
         const double* zin = l == 0 ? W.z0[0].as<double>() : W.za[l].as<double>();
         double* zout = l == 0 ? W.z0[1].as<double>() : W.zb[l].as<double>();
         const double* ec = (l + 1 == lc) ? W.za[lc].as<double>() : W.zb[l + 1].as<double>();
-        NU_DISPATCH(ch.nu, (launch_up<NU_>(L, l == 0 ? KC_UP0 : KC_UPC, 3.0 * V + Vc, H.lev[l], ch, B, rr, zin, ec,
-                                           H.ny[l + 1], H.nx[l + 1], zout, l == 0 ? W.s.rz : nullptr)));
+        if (sm.v1) {
+            NU_DISPATCH(ch.nu, (launch_up<NU_>(L, l == 0 ? KC_UP0 : KC_UPC, 3.0 * V + Vc, H.lev[l], ch, B, rr, zin, ec,
+                                               H.ny[l + 1], H.nx[l + 1], zout, l == 0 ? W.s.rz : nullptr)));
+        } else {
+            NU_DISPATCH(ch.nu, (launch_up2<NU_>(L, l == 0 ? KC_UP0 : KC_UPC, 3.0 * V + Vc, H.lev[l], sm.cr, B, sm.G, rr, zin, ec,
+                                                H.ny[l + 1], H.nx[l + 1], zout, l == 0 ? W.s.rz : nullptr)));
+        }
     }
 }
 
 // Solve L_t x_b = e_{port src0+b} - 1/n^2 for b in [0, B) by multigrid-preconditioned CG and leave
 //   TSV-source batch     : ZT[src0+b][k] = x_b[port k] - mean(x_b)      for all ports k of the tier
 //   terminal-source batch: zdiag[src0+b-ntsv] = x_b[own node] - mean(x_b)
-int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts& T, const Cheb& ch, int src0, int B,
+int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts& T, const Smoother& ch, int src0, int B,
                 bool terminal, double rtol, int max_iter);
 
-int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts& T, const Cheb& ch, int src0, int B,
+int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts& T, const Smoother& ch, int src0, int B,
                 bool terminal, double rtol, int max_iter) {
     const int n = H.ny[0];
     const size_t n2 = (size_t)n * n;
@@ -653,7 +716,8 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         }
         Work W;
         if (H.nlev > 1) W.allocate(H, Bmax, qmax);
-        const Cheb ch = make_cheb(o.nu, 6.0);
+        Smoother ch{make_cheb(o.nu, 6.0), make_cheb_roots(o.nu, 6.0), getenv("PDN_STENCIL_V1") != nullptr,
+                    getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 4};
         const double rtol_term = std::max(o.rtol, std::min(1e-5, std::sqrt(o.rtol) / 3.0));
         float ms_up = 0.f;
         for (int t = 0; t < d && status == PDN_OK; ++t) {
