@@ -99,7 +99,7 @@ typedef struct {
     int32_t rhs_batch;  /* right-hand sides solved concurrently per tier          (default: auto) */
     void *cuda_stream;  /* cudaStream_t to run on                                 (default: 0)    */
     int32_t flags;      /* PDN_* flags                                                             */
-    int32_t nu;         /* Chebyshev smoothing steps per multigrid level and side (default 3)     */
+    int32_t nu;         /* Chebyshev smoothing steps per multigrid level and side (1..6, default 4)*/
 } pdn_opts;
 
 /* Counters and timings of the last pdn_create (device-event milliseconds). */
@@ -139,6 +139,11 @@ int pdn_reff_host(pdn_ctx *ctx, int64_t n_pairs, const int32_t *bump_idx, const 
 
 /* NULL-safe; frees all device and host memory of ctx. */
 void pdn_destroy(pdn_ctx *ctx);
+
+/* Device blocks released by pdn_destroy are kept in a process-wide cache and reused by the next
+ * pdn_create (cudaMalloc / cudaFree of multi-GB workspaces cost tens of ms).  This returns them to
+ * the driver.  Safe to call at any time from the thread that owns the contexts. */
+void pdn_release_cache(void);
 
 /* Helpers. */
 const char *pdn_strerror(int status);

@@ -49,7 +49,7 @@ class PdnStats(C.Structure):
 
 
 EXPORTS = ("pdn_create", "pdn_reff", "pdn_reff_host", "pdn_destroy", "pdn_strerror", "pdn_last_error",
-           "pdn_get_stats", "pdn_port_count", "pdn_get_port_matrix")
+           "pdn_get_stats", "pdn_port_count", "pdn_get_port_matrix", "pdn_release_cache")
 
 _lib = None
 
@@ -76,6 +76,8 @@ def load_library() -> C.CDLL:
     lib.pdn_strerror.argtypes = [C.c_int]
     lib.pdn_last_error.restype = C.c_char_p
     lib.pdn_last_error.argtypes = []
+    lib.pdn_release_cache.restype = None
+    lib.pdn_release_cache.argtypes = []
     lib.pdn_get_stats.restype = C.c_int
     lib.pdn_get_stats.argtypes = [C.c_void_p, C.POINTER(PdnStats)]
     lib.pdn_port_count.restype = C.c_int32

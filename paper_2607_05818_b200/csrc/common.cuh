@@ -1,30 +1,42 @@
 // Shared device-side definitions of the PDN effective-resistance path (sm_100a only).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 namespace pdn {
 
-constexpr int MAX_NU = 8;       // max Chebyshev steps per side
+constexpr int MAX_NU = 8;       // max smoothing steps per side
 constexpr int MAX_LEVELS = 16;  // multigrid levels (n halves per level)
 constexpr int COARSEST_MAX = 4; // coarsest level has n <= 4 (<= 16 unknowns, dense pseudo-inverse)
 
 // One multigrid level of one tier: matrix-free 5-point stencil with per-edge conductances.
-//   gx[y*nx+x] joins (y,x)-(y,x+1), zero in the last column; gy[y*nx+x] joins (y,x)-(y+1,x), zero in
-//   the last row; dinv = 1 / (sum of the incident conductances) (0 for an isolated node).
+//
+// Every plane and every batched vector of a level is stored with a row pitch of `pitch` doubles
+// (nx rounded up to an even number), so that a thread's two adjacent columns are one aligned
+// 16-byte word and TMA row strides are multiples of 16 bytes.  Pad entries of planes are zero.
+//
+// The V-cycle works on the symmetrically scaled operator  A^ = S L S = I - N,  S = D^-1/2:
+//   s  = 1/sqrt(d), sd = sqrt(d)   (d = sum of the incident conductances; 0 for a node with d = 0)
+//   hE[y][x] = gx[y][x] * s[y][x] * s[y][x+1]      hS[y][x] = gy[y][x] * s[y][x] * s[y+1][x]
+// so that the Jacobi-preconditioned Richardson step z <- z + w D^-1 (r - L z) becomes, for y = z/s,
+// r^ = s r:   y <- (1-w) y + w (r^ + sum_nb h_nb y_nb)  -- no diagonal in the inner loop.
 struct Level {
-    int ny, nx;
-    const double* gx;
+    int ny, nx, pitch;
+    const double* gx;   // raw conductances (level 0: sanitised copy of the caller's planes)
     const double* gy;
-    const double* dinv;
+    const double* hE;
+    const double* hS;
+    const double* s;
+    const double* sd;
 };
 
-// Chebyshev polynomial smoother on D^-1 L with spectrum bound [2/ratio, 2] (lambda_max(D^-1 L) <= 2
-// for any graph Laplacian):  d_0 = c2[0] D^-1 res_0;  d_k = c1[k] d_{k-1} + c2[k] D^-1 res_k;  z += d_k.
-struct Cheb {
+// Richardson steps with the reciprocals of the Chebyshev nodes of [2/ratio, 2] as step lengths: the
+// same polynomial as nu Chebyshev semi-iteration steps on D^-1 L (lambda_max(D^-1 L) <= 2 for any
+// graph Laplacian), with no direction vector to carry.
+struct ChebR {
     int nu;
-    double c1[MAX_NU];
-    double c2[MAX_NU];
+    double w[MAX_NU];
 };
 
 // Per-right-hand-side PCG scalars of one batch (device arrays of length B).
@@ -61,6 +73,46 @@ __device__ __forceinline__ double block_sum(double v, double* scratch) {
         v = warp_sum(v);
     }
     return v;
+}
+
+// ---------------------------------------------------------------------------------------------
+// TMA (cp.async.bulk.tensor) + mbarrier wrappers.  Tiles with halos are fetched as 3D boxes
+// (x, y, right-hand side) of a tensor map; coordinates may be negative or run past the mesh:
+// out-of-bounds elements arrive as zeros, which is exactly the "no node, no conductance" padding
+// the sweeps need.
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+
+__device__ __forceinline__ void tma_load_3d(void* smem_dst, const CUtensorMap* map, int c0, int c1, int c2,
+                                            uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+        ::"r"(smem_u32(smem_dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+}
+
+__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
+    asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
 }
 
 }  // namespace pdn

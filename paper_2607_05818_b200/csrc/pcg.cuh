@@ -7,13 +7,15 @@
 
 namespace pdn {
 
-// r[b] = e_{node[src0+b]} - 1/n2  (consistent right-hand side of the singular tier system)
-__global__ void k_init_rhs(double* __restrict__ r, size_t n2, const int* __restrict__ node, int src0, int B) {
+// r[b] = e_{node[src0+b]} - 1/n2  (consistent right-hand side of the singular tier system) on the
+// pitched plane (plane = ny*pitch doubles; pad entries 0); node[] holds pitched offsets y*pitch + x.
+__global__ void k_init_rhs(double* __restrict__ r, int nx, int pitch, size_t plane, double inv_n2,
+                           const int* __restrict__ node, int src0, int B) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int b = blockIdx.y;
-    if (i >= n2) return;
-    const double m = -1.0 / (double)n2;
-    r[b * n2 + i] = (i == (size_t)node[src0 + b]) ? 1.0 + m : m;
+    if (i >= plane) return;
+    const double m = ((int)(i % pitch) < nx) ? -inv_n2 : 0.0;
+    r[b * plane + i] = (i == (size_t)node[src0 + b]) ? 1.0 + m : m;
 }
 
 __global__ void k_zero(double* __restrict__ a, size_t n) {
@@ -95,24 +97,27 @@ __global__ void k_finish_term(const double* __restrict__ xown, const double* __r
 }
 
 // Meshes with n <= 4 are their own coarsest level: Z comes straight from the dense pseudo-inverse.
-__global__ void k_direct_small(const double* __restrict__ pinv, int nc, const int* __restrict__ node, int ntsv,
-                               int q, double* __restrict__ ZT, double* __restrict__ zdiag) {
+__global__ void k_direct_small(const double* __restrict__ pinv, int nx, int pitch, int nc,
+                               const int* __restrict__ node, int ntsv, int q, double* __restrict__ ZT,
+                               double* __restrict__ zdiag) {
     const int j = blockIdx.x;
+    const int dj = (node[j] / pitch) * nx + node[j] % pitch;
     for (int k = threadIdx.x; k < q; k += blockDim.x) {
-        if (j < ntsv) ZT[(size_t)j * q + k] = pinv[node[j] * nc + node[k]];
-        else if (k == 0) zdiag[j - ntsv] = pinv[node[j] * nc + node[j]];
+        const int dk = (node[k] / pitch) * nx + node[k] % pitch;
+        if (j < ntsv) ZT[(size_t)j * q + k] = pinv[dj * nc + dk];
+        else if (k == 0) zdiag[j - ntsv] = pinv[dj * nc + dj];
     }
 }
 
-// r.z for the single-level case (coarsest level is level 0).
-__global__ void k_dot(const double* __restrict__ a, const double* __restrict__ c, size_t n2, double* __restrict__ acc) {
-    __shared__ double red[32];
-    const int b = blockIdx.y;
+// Coarsest level: e = pinv * r, one thread per (b, i); nc = ny*nx <= 16; vectors are pitched.
+__global__ void k_coarse_pinv(const double* __restrict__ pinv, int nx, int pitch, int nc, size_t plane,
+                              const double* __restrict__ r, double* __restrict__ e, int B) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= B * nc) return;
+    const int b = t / nc, i = t % nc;
     double s = 0.0;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += (size_t)gridDim.x * blockDim.x)
-        s = fma(a[b * n2 + i], c[b * n2 + i], s);
-    s = block_sum(s, red);
-    if (threadIdx.x == 0) atomicAdd(acc + b, s);
+    for (int j = 0; j < nc; ++j) s = fma(__ldg(pinv + i * nc + j), r[b * plane + (j / nx) * pitch + j % nx], s);
+    e[b * plane + (i / nx) * pitch + i % nx] = s;
 }
 
 }  // namespace pdn

@@ -2,9 +2,9 @@
 //   pdn_create = S0 (tier import + multigrid hierarchy) -> S1 (batched port reduction by MG-PCG)
 //                -> S2 (assemble C) -> S3 (factor once, substitute for m+n right-hand sides)
 //   pdn_reff   = S4 (pair evaluation) [+ S5 copy to host]
-// Everything numerical runs in the kernels of stencil.cuh / pcg.cuh / setup.cuh / dense.cuh /
-// port.cuh; the host code below only validates, allocates, sequences launches and reads back the
-// per-batch convergence counter.  There is no CPU fallback.
+// Everything numerical runs in the kernels of stencil3.cuh / pcg.cuh / setup.cuh / dense.cuh /
+// port.cuh; the host code below only validates, allocates, encodes TMA descriptors, sequences
+// launches and reads back the per-batch convergence counter.  There is no CPU fallback.
 #include "../../include/pdn.h"
 
 #include <algorithm>
@@ -12,6 +12,8 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
+#include <mutex>
 #include <new>
 #include <set>
 #include <string>
@@ -23,8 +25,7 @@
 #include "pcg.cuh"
 #include "port.cuh"
 #include "setup.cuh"
-#include "stencil.cuh"
-#include "stencil2.cuh"
+#include "stencil3.cuh"
 
 using namespace pdn;
 
@@ -51,7 +52,56 @@ struct StatusFail {
 // kernel classes for the per-class timers / byte model
 enum { KC_PQ = 0, KC_DOWN0, KC_UP0, KC_DOWNC, KC_UPC, KC_SMALL, KC_DENSE, KC_PAIR, KC_COUNT };
 
-struct DevBuf {  // RAII device allocation
+// ------------------------------------------------------------------------------------------------
+// Device memory: a process-wide cache of freed blocks.  pdn_create needs tens of GB of workspace;
+// cudaMalloc / cudaFree of blocks that size cost tens of milliseconds each, so released blocks are
+// kept and handed out again (best fit within 25 %).  pdn_release_cache() returns them to the driver;
+// an allocation failure does so automatically before giving up.
+struct DevPool {
+    std::mutex mu;
+    std::multimap<size_t, void*> free_blocks;
+    size_t cached = 0;
+
+    void* get(size_t n) {
+        {
+            std::lock_guard<std::mutex> g(mu);
+            auto it = free_blocks.lower_bound(n);
+            if (it != free_blocks.end() && it->first <= n + n / 4 + 4096) {
+                void* p = it->second;
+                cached -= it->first;
+                free_blocks.erase(it);
+                return p;
+            }
+        }
+        void* p = nullptr;
+        cudaError_t e = cudaMalloc(&p, n);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            trim();
+            e = cudaMalloc(&p, n);
+            if (e != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        }
+        return p;
+    }
+    void put(void* p, size_t n) {
+        std::lock_guard<std::mutex> g(mu);
+        free_blocks.emplace(n, p);
+        cached += n;
+    }
+    void trim() {
+        std::lock_guard<std::mutex> g(mu);
+        for (auto& kv : free_blocks) cudaFree(kv.second);
+        free_blocks.clear();
+        cached = 0;
+    }
+    size_t cached_bytes() {
+        std::lock_guard<std::mutex> g(mu);
+        return cached;
+    }
+};
+DevPool g_pool;
+
+struct DevBuf {  // RAII device allocation (block sizes are rounded up to 1 MiB classes above 1 MiB)
     void* p = nullptr;
     size_t bytes = 0;
     DevBuf() = default;
@@ -63,12 +113,12 @@ struct DevBuf {  // RAII device allocation
         return *this;
     }
     ~DevBuf() { release(); }
-    void release() { if (p) cudaFree(p); p = nullptr; bytes = 0; }
+    void release() { if (p) g_pool.put(p, bytes); p = nullptr; bytes = 0; }
     void alloc(size_t n) {
         release();
-        if (n == 0) n = 8;
-        cudaError_t e = cudaMalloc(&p, n);
-        if (e != cudaSuccess) { p = nullptr; cudaGetLastError(); throw StatusFail{PDN_E_NOMEM, "cudaMalloc of " + std::to_string(n) + " bytes failed"}; }
+        n = n < 256 ? 256 : (n + 255) & ~size_t(255);
+        p = g_pool.get(n);
+        if (!p) throw StatusFail{PDN_E_NOMEM, "cudaMalloc of " + std::to_string(n) + " bytes failed"};
         bytes = n;
     }
     template <class T> T* as() const { return static_cast<T*>(p); }
@@ -76,7 +126,7 @@ struct DevBuf {  // RAII device allocation
 
 struct TierPorts {
     int ntsv = 0, nterm = 0, q = 0;   // TSV ports, terminal ports, total
-    std::vector<int> node;            // local node id of every port, port order of port.cuh
+    std::vector<int> node;            // pitched offset y*pitch + x of every port, port order of port.cuh
     DevBuf d_node;                    // device copy
     DevBuf ZT;                        // ntsv x q
     DevBuf zdiag;                     // nterm
@@ -142,22 +192,69 @@ struct Launcher {
 inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) / b); }
 
 // ------------------------------------------------------------------------------------------------
+// TMA descriptors: a batched pitched vector v[B][ny][pitch] as a 3D tensor (x, y, b) of doubles whose
+// x extent is the true nx (so pad columns read as zeros) and a box of bx x by x 1.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres));
+        if (!p || qres != cudaDriverEntryPointSuccess) throw StatusFail{PDN_E_CUDA, "cuTensorMapEncodeTiled is not available"};
+        fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+CUtensorMap make_map(const void* base, int nx, int ny, int pitch, int B, int box_x, int box_y) {
+    CUtensorMap m;
+    const cuuint64_t dims[3] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)B};
+    const cuuint64_t strides[2] = {(cuuint64_t)pitch * 8, (cuuint64_t)pitch * ny * 8};
+    const cuuint32_t box[3] = {(cuuint32_t)box_x, (cuuint32_t)box_y, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    const CUresult r = encode_tiled_fn()(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), dims, strides,
+                                         box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                         CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) throw StatusFail{PDN_E_CUDA, "cuTensorMapEncodeTiled failed with code " + std::to_string((int)r)};
+    return m;
+}
+
+#ifndef PDN_T3_R
+#define PDN_T3_R 4
+#endif
+#ifndef PDN_T3_W
+#define PDN_T3_W 16
+#endif
+constexpr int T3_R = PDN_T3_R, T3_W = PDN_T3_W, T3_EH = T3_R * T3_W, T3_THREADS = 32 * T3_W;
+constexpr size_t T3_TILE_BYTES = (size_t)T3_EH * T3_EW * sizeof(double);
+
+inline int pitch_of(int nx) { return (nx + 1) & ~1; }
+
+// ------------------------------------------------------------------------------------------------
 // S0: multigrid hierarchy of one tier (buffers are allocated once and reused for every tier).
 struct Hierarchy {
     int nlev = 0;
-    int ny[MAX_LEVELS], nx[MAX_LEVELS];
-    DevBuf gx[MAX_LEVELS], gy[MAX_LEVELS], dinv[MAX_LEVELS];
+    int ny[MAX_LEVELS], nx[MAX_LEVELS], pitch[MAX_LEVELS];
+    DevBuf gx[MAX_LEVELS], gy[MAX_LEVELS], hE[MAX_LEVELS], hS[MAX_LEVELS], s[MAX_LEVELS], sd[MAX_LEVELS];
     DevBuf pinv, flags, labels;  // flags: [0] bad value, [1] isolated node, [2] label changed, [3] label nonzero
     Level lev[MAX_LEVELS];
+
+    size_t plane(int l) const { return (size_t)ny[l] * pitch[l]; }
 
     void allocate(int n) {
         nlev = 0;
         int cur = n;
         while (true) {
             ny[nlev] = nx[nlev] = cur;
-            const size_t b = (size_t)cur * cur * sizeof(double);
-            gx[nlev].alloc(b); gy[nlev].alloc(b); dinv[nlev].alloc(b);
-            lev[nlev] = Level{cur, cur, gx[nlev].as<double>(), gy[nlev].as<double>(), dinv[nlev].as<double>()};
+            pitch[nlev] = pitch_of(cur);
+            const size_t b = plane(nlev) * sizeof(double);
+            gx[nlev].alloc(b); gy[nlev].alloc(b); hE[nlev].alloc(b); hS[nlev].alloc(b); s[nlev].alloc(b); sd[nlev].alloc(b);
+            lev[nlev] = Level{cur, cur, pitch[nlev], gx[nlev].as<double>(), gy[nlev].as<double>(), hE[nlev].as<double>(),
+                              hS[nlev].as<double>(), s[nlev].as<double>(), sd[nlev].as<double>()};
             ++nlev;
             if (cur <= COARSEST_MAX) break;
             if (nlev >= MAX_LEVELS) throw StatusFail{PDN_E_ARG, "mesh too large for MAX_LEVELS"};
@@ -168,22 +265,21 @@ struct Hierarchy {
         labels.alloc((size_t)n * n * sizeof(int));
     }
 
-    // Import one tier (gx_src / gy_src are device pointers) and build all levels.  Returns PDN status.
+    // Import one tier (gx_src / gy_src are device pointers, dense n x n) and build all levels.
     int build(Launcher& L, const double* gx_src, const double* gy_src, bool check_connectivity) {
         const int n = ny[0];
         CK(cudaMemsetAsync(flags.p, 0, 4 * sizeof(int), L.s));
         int* fl = flags.as<int>();
-        L.run(KC_SMALL, 0, [&] { k_import_planes<<<cdiv((size_t)n * n, 256), 256, 0, L.s>>>(gx_src, gy_src, n, gx[0].as<double>(), gy[0].as<double>(), fl); });
+        L.run(KC_SMALL, 0, [&] { k_import_planes<<<cdiv(plane(0), 256), 256, 0, L.s>>>(gx_src, gy_src, n, pitch[0], gx[0].as<double>(), gy[0].as<double>(), fl); });
         for (int l = 0; l < nlev; ++l) {
-            const size_t n2 = (size_t)ny[l] * nx[l];
-            L.run(KC_SMALL, 0, [&] { k_dinv<<<cdiv(n2, 256), 256, 0, L.s>>>(ny[l], nx[l], gx[l].as<double>(), gy[l].as<double>(), dinv[l].as<double>(), l == 0 ? fl + 1 : nullptr); });
-            if (l + 1 < nlev) {
-                const size_t c2 = (size_t)ny[l + 1] * nx[l + 1];
-                L.run(KC_SMALL, 0, [&] { k_coarsen<<<cdiv(c2, 256), 256, 0, L.s>>>(ny[l], nx[l], gx[l].as<double>(), gy[l].as<double>(), ny[l + 1], nx[l + 1], gx[l + 1].as<double>(), gy[l + 1].as<double>()); });
-            }
+            const unsigned g = cdiv(plane(l), 256);
+            L.run(KC_SMALL, 0, [&] { k_scale_nodes<<<g, 256, 0, L.s>>>(ny[l], nx[l], pitch[l], gx[l].as<double>(), gy[l].as<double>(), s[l].as<double>(), sd[l].as<double>(), l == 0 ? fl + 1 : nullptr); });
+            L.run(KC_SMALL, 0, [&] { k_scale_edges<<<g, 256, 0, L.s>>>(ny[l], nx[l], pitch[l], gx[l].as<double>(), gy[l].as<double>(), s[l].as<double>(), hE[l].as<double>(), hS[l].as<double>()); });
+            if (l + 1 < nlev)
+                L.run(KC_SMALL, 0, [&] { k_coarsen<<<cdiv(plane(l + 1), 256), 256, 0, L.s>>>(ny[l], nx[l], pitch[l], gx[l].as<double>(), gy[l].as<double>(), ny[l + 1], nx[l + 1], pitch[l + 1], gx[l + 1].as<double>(), gy[l + 1].as<double>()); });
         }
         const int lc = nlev - 1;
-        L.run(KC_SMALL, 0, [&] { k_coarsest_pinv<<<1, 32, 0, L.s>>>(ny[lc], nx[lc], gx[lc].as<double>(), gy[lc].as<double>(), pinv.as<double>()); });
+        L.run(KC_SMALL, 0, [&] { k_coarsest_pinv<<<1, 32, 0, L.s>>>(ny[lc], nx[lc], pitch[lc], gx[lc].as<double>(), gy[lc].as<double>(), pinv.as<double>()); });
         int h[4] = {0, 0, 0, 0};
         CK(cudaMemcpyAsync(h, fl, 2 * sizeof(int), cudaMemcpyDeviceToHost, L.s));
         CK(cudaStreamSynchronize(L.s));
@@ -196,7 +292,7 @@ struct Hierarchy {
             for (int sweep = 0; sweep < 4 * n + 64; ++sweep) {
                 CK(cudaMemsetAsync(fl + 2, 0, sizeof(int), L.s));
                 for (int rep = 0; rep < 4; ++rep)
-                    L.run(KC_SMALL, 0, [&] { k_label_sweep<<<cdiv(n2, 256), 256, 0, L.s>>>(n, n, gx[0].as<double>(), gy[0].as<double>(), lab, fl + 2); });
+                    L.run(KC_SMALL, 0, [&] { k_label_sweep<<<cdiv(n2, 256), 256, 0, L.s>>>(n, n, pitch[0], gx[0].as<double>(), gy[0].as<double>(), lab, fl + 2); });
                 CK(cudaMemcpyAsync(h + 2, fl + 2, sizeof(int), cudaMemcpyDeviceToHost, L.s));
                 CK(cudaStreamSynchronize(L.s));
                 if (!h[2]) break;
@@ -210,23 +306,6 @@ struct Hierarchy {
     }
 };
 
-Cheb make_cheb(int nu, double ratio) {
-    Cheb c{};
-    c.nu = nu;
-    const double lmax = 2.0, lmin = lmax / ratio;
-    const double theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin), sigma = theta / delta;
-    double rho = 1.0 / sigma;
-    c.c1[0] = 0.0;
-    c.c2[0] = 1.0 / theta;
-    for (int k = 1; k < nu; ++k) {
-        const double rho_new = 1.0 / (2.0 * sigma - rho);
-        c.c1[k] = rho_new * rho;
-        c.c2[k] = 2.0 * rho_new / delta;
-        rho = rho_new;
-    }
-    return c;
-}
-
 ChebR make_cheb_roots(int nu, double ratio) {
     ChebR c{};
     c.nu = nu;
@@ -236,37 +315,42 @@ ChebR make_cheb_roots(int nu, double ratio) {
     return c;
 }
 
-struct Smoother {  // both parametrisations of the same polynomial (v1 kernels use Cheb, v2 ChebR)
-    Cheb ch;
+struct Smoother {
     ChebR cr;
-    bool v1;
-    int G;
+    int G;  // right-hand sides a block loops over (upper bound; fewer on levels with few tiles)
 };
 
 // ------------------------------------------------------------------------------------------------
-// S1 workspace of one batch of right-hand sides.
+// S1 workspace of one batch of right-hand sides, with the TMA descriptor of every vector.
 struct Work {
     int Bmax = 0, qmax = 0;
-    DevBuf r[2], z0[2], p[2], q;                     // level 0 (ping-pong pairs avoid in-place halo races)
-    DevBuf rl[MAX_LEVELS], za[MAX_LEVELS], zb[MAX_LEVELS];  // levels >= 1
+    DevBuf r[2], y0, z, p[2], q;                           // level 0 (ping-pong pairs: halos are read across blocks)
+    DevBuf rl[MAX_LEVELS], ya[MAX_LEVELS], zb[MAX_LEVELS];  // levels >= 1: residual, scaled iterate, correction
+    CUtensorMap m_r[2], m_y0, m_z, m_p[2], m_q;
+    CUtensorMap m_rl[MAX_LEVELS], m_ya[MAX_LEVELS], m_ec[MAX_LEVELS];  // m_ec[l]: zb[l] as the coarse box of level l-1
     DevBuf scal, xport, xown, iact;
     PcgScalars s{};
     int* h_nact = nullptr;                           // pinned
     double* h_relres = nullptr;                      // pinned, Bmax
 
     static size_t bytes_per_rhs(const Hierarchy& H) {
-        size_t b = 7 * (size_t)H.ny[0] * H.nx[0];
-        for (int l = 1; l < H.nlev; ++l) b += 3 * (size_t)H.ny[l] * H.nx[l];
+        size_t b = 7 * H.plane(0);
+        for (int l = 1; l < H.nlev; ++l) b += 3 * H.plane(l);
         return b * sizeof(double);
     }
     void allocate(const Hierarchy& H, int B, int qmax_) {
         Bmax = B; qmax = qmax_;
-        const size_t v0 = (size_t)B * H.ny[0] * H.nx[0] * sizeof(double);
-        for (int i = 0; i < 2; ++i) { r[i].alloc(v0); z0[i].alloc(v0); p[i].alloc(v0); }
-        q.alloc(v0);
+        const size_t v0 = (size_t)B * H.plane(0) * sizeof(double);
+        for (int i = 0; i < 2; ++i) { r[i].alloc(v0); p[i].alloc(v0); }
+        y0.alloc(v0); z.alloc(v0); q.alloc(v0);
+        auto fine = [&](const DevBuf& d, int l) { return make_map(d.p, H.nx[l], H.ny[l], H.pitch[l], B, T3_EW, T3_EH); };
+        for (int i = 0; i < 2; ++i) { m_r[i] = fine(r[i], 0); m_p[i] = fine(p[i], 0); }
+        m_y0 = fine(y0, 0); m_z = fine(z, 0); m_q = fine(q, 0);
         for (int l = 1; l < H.nlev; ++l) {
-            const size_t vl = (size_t)B * H.ny[l] * H.nx[l] * sizeof(double);
-            rl[l].alloc(vl); za[l].alloc(vl); zb[l].alloc(vl);
+            const size_t vl = (size_t)B * H.plane(l) * sizeof(double);
+            rl[l].alloc(vl); ya[l].alloc(vl); zb[l].alloc(vl);
+            m_rl[l] = fine(rl[l], l); m_ya[l] = fine(ya[l], l);
+            m_ec[l] = make_map(zb[l].p, H.nx[l], H.ny[l], H.pitch[l], B, T3_ECW, T3_EH / 2);
         }
         scal.alloc((size_t)9 * B * sizeof(double));
         double* sp = scal.as<double>();
@@ -286,58 +370,60 @@ struct Work {
     }
 };
 
-constexpr int TI = 32;  // tile interior of the first-version stencil kernels
-
-template <int NU>
-void launch_down(Launcher& L, int cls, double bytes, const Level& lv, const Cheb& ch, int B, const double* r_in,
-                 const double* q, const double* alpha, double* r_out, double* z_out, double* rc, int cny, int cnx,
-                 double* rr_acc) {
-    constexpr int E = TI + 2 * NU;
-    const size_t smem = 3 * E * E * sizeof(double);
-    dim3 grid(cdiv(lv.nx, TI), cdiv(lv.ny, TI), B);
-    L.run(cls, bytes, [&] { k_down<TI, NU><<<grid, STENCIL_THREADS, smem, L.s>>>(lv, ch, r_in, q, alpha, r_out, z_out, rc, cny, cnx, rr_acc); });
+// right-hand sides per block: as many as G allows while the grid still fills the GPU a few times over
+inline int rhs_per_block(int tiles, int B, int G) {
+    const long blocks_wanted = 148L * 4;
+    long g = ((long)tiles * B) / blocks_wanted;
+    return (int)std::max(1L, std::min<long>(G, g));
 }
 
 template <int NU>
-void launch_up(Launcher& L, int cls, double bytes, const Level& lv, const Cheb& ch, int B, const double* r,
-               const double* z_in, const double* ec, int cny, int cnx, double* z_out, double* rz_acc) {
-    constexpr int E = TI + 2 * NU;
-    const size_t smem = 3 * E * E * sizeof(double);
-    dim3 grid(cdiv(lv.nx, TI), cdiv(lv.ny, TI), B);
-    L.run(cls, bytes, [&] { k_up<TI, NU><<<grid, STENCIL_THREADS, smem, L.s>>>(lv, ch, r, z_in, ec, cny, cnx, z_out, rz_acc); });
-}
-
-template <int NU>
-void launch_down2(Launcher& L, int cls, double bytes, const Level& lv, const ChebR& ch, int B, int G, const double* r_in,
-                  const double* q, const double* alpha, double* r_out, double* z_out, double* rc, int cny, int cnx,
-                  double* rr_acc) {
-    constexpr int IW = T2_EW - 2 * NU, IH = T2_EH - 2 * NU;
-    dim3 grid(cdiv(lv.nx, IW), cdiv(lv.ny, IH), cdiv(B, G));
-    constexpr size_t stage1 = (size_t)2 * T2_R * T2_THREADS * sizeof(double);  // two stages of one array
+void launch_down3(Launcher& L, int cls, double bytes, const Level& lv, const Smoother& sm, int B, const CUtensorMap& m_r,
+                  const CUtensorMap* m_q, const double* alpha, double* r_out, double* y_out, double* rc, int cny,
+                  int cnx, int cpitch, double* rr_acc) {
+    constexpr int H = halo_of(NU), IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
+    const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
+    dim3 grid(tx, ty, cdiv(B, G));
+    constexpr size_t base = 4 * T3_TILE_BYTES + sizeof(Exch<T3_W>) + 128;
     static bool attr_done = false;
     if (!attr_done) {
-        CK(cudaFuncSetAttribute(k_down2<NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * stage1)));
-        CK(cudaFuncSetAttribute(k_down2<NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stage1));
+        CK(cudaFuncSetAttribute(k_down3<T3_R, T3_W, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(base + T3_TILE_BYTES)));
+        CK(cudaFuncSetAttribute(k_down3<T3_R, T3_W, NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)base));
         attr_done = true;
     }
-    if (q) L.run(cls, bytes, [&] { k_down2<NU, true><<<grid, T2_THREADS, 2 * stage1, L.s>>>(lv, ch, r_in, q, alpha, r_out, z_out, rc, cny, cnx, rr_acc, B, G); });
-    else L.run(cls, bytes, [&] { k_down2<NU, false><<<grid, T2_THREADS, stage1, L.s>>>(lv, ch, r_in, q, alpha, r_out, z_out, rc, cny, cnx, rr_acc, B, G); });
+    if (m_q) L.run(cls, bytes, [&] { k_down3<T3_R, T3_W, NU, true><<<grid, T3_THREADS, base + T3_TILE_BYTES, L.s>>>(m_r, *m_q, lv, sm.cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G); });
+    else L.run(cls, bytes, [&] { k_down3<T3_R, T3_W, NU, false><<<grid, T3_THREADS, base, L.s>>>(m_r, m_r, lv, sm.cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G); });
 }
 
 template <int NU>
-void launch_up2(Launcher& L, int cls, double bytes, const Level& lv, const ChebR& ch, int B, int G, const double* r,
-                const double* z_in, const double* ec, int cny, int cnx, double* z_out, double* rz_acc) {
-    constexpr int IW = T2_EW - 2 * NU, IH = T2_EH - 2 * NU;
-    dim3 grid(cdiv(lv.nx, IW), cdiv(lv.ny, IH), cdiv(B, G));
-    constexpr size_t stage3 = (size_t)2 * 3 * T2_R * T2_THREADS * sizeof(double);
+void launch_up3(Launcher& L, int cls, double bytes, const Level& lv, const Smoother& sm, int B, const CUtensorMap& m_r,
+                const CUtensorMap& m_y, const CUtensorMap& m_e, double* z_out, double* rz_acc) {
+    constexpr int H = halo_of(NU), IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
+    const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
+    dim3 grid(tx, ty, cdiv(B, G));
+    constexpr size_t smem = 5 * T3_TILE_BYTES + (size_t)(T3_EH / 2) * T3_ECW * sizeof(double) + sizeof(Exch<T3_W>) + 128;
     static bool attr_done = false;
     if (!attr_done) {
-        CK(cudaFuncSetAttribute(k_up2<NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stage3));
-        CK(cudaFuncSetAttribute(k_up2<NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stage3));
+        CK(cudaFuncSetAttribute(k_up3<T3_R, T3_W, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_up3<T3_R, T3_W, NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_done = true;
     }
-    if (rz_acc) L.run(cls, bytes, [&] { k_up2<NU, true><<<grid, T2_THREADS, stage3, L.s>>>(lv, ch, r, z_in, ec, cny, cnx, z_out, rz_acc, B, G); });
-    else L.run(cls, bytes, [&] { k_up2<NU, false><<<grid, T2_THREADS, stage3, L.s>>>(lv, ch, r, z_in, ec, cny, cnx, z_out, rz_acc, B, G); });
+    if (rz_acc) L.run(cls, bytes, [&] { k_up3<T3_R, T3_W, NU, true><<<grid, T3_THREADS, smem, L.s>>>(m_r, m_y, m_e, lv, sm.cr, z_out, rz_acc, B, G); });
+    else L.run(cls, bytes, [&] { k_up3<T3_R, T3_W, NU, false><<<grid, T3_THREADS, smem, L.s>>>(m_r, m_y, m_e, lv, sm.cr, z_out, rz_acc, B, G); });
+}
+
+void launch_pq3(Launcher& L, double bytes, const Level& lv, const Smoother& sm, int B, const CUtensorMap& m_z,
+                const CUtensorMap& m_p, const double* beta, double* p_new, double* q, double* pq_acc, double* sump_acc) {
+    constexpr int H = 2, IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
+    const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
+    dim3 grid(tx, ty, cdiv(B, G));
+    constexpr size_t smem = 3 * T3_TILE_BYTES + sizeof(Exch<T3_W>) + 128;
+    static bool attr_done = false;
+    if (!attr_done) {
+        CK(cudaFuncSetAttribute(k_pq3<T3_R, T3_W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done = true;
+    }
+    L.run(KC_PQ, bytes, [&] { k_pq3<T3_R, T3_W><<<grid, T3_THREADS, smem, L.s>>>(m_z, m_p, lv, beta, p_new, q, pq_acc, sump_acc, B, G); });
 }
 
 #define NU_DISPATCH(nu, CALL)                 \
@@ -345,92 +431,63 @@ void launch_up2(Launcher& L, int cls, double bytes, const Level& lv, const ChebR
         case 1: { constexpr int NU_ = 1; CALL; } break; \
         case 2: { constexpr int NU_ = 2; CALL; } break; \
         case 3: { constexpr int NU_ = 3; CALL; } break; \
-        default: { constexpr int NU_ = 4; CALL; } break; \
+        case 4: { constexpr int NU_ = 4; CALL; } break; \
+        case 5: { constexpr int NU_ = 5; CALL; } break; \
+        default: { constexpr int NU_ = 6; CALL; } break; \
     }
 
-// One multigrid V-cycle  z = M^-1 r  on a batch.  If q != nullptr the level-0 down stage first forms
-// r_out = r_in - alpha q (and ||r_out||^2).  The result z is written to W.z0[1]; r.z goes to s.rz.
-// `after_down0` runs right after the level-0 down stage was enqueued (the convergence check); if it
-// returns true the rest of the cycle is skipped.
+// One multigrid V-cycle  z = M^-1 r  on a batch; r is W.r[ri].  If fused, the level-0 down stage first
+// forms W.r[ri^1] = W.r[ri] - alpha q (and its squared norm) and the cycle works with that.  The result z
+// is written to W.z; r.z goes to s.rz.  `after_down0` runs right after the level-0 down stage was
+// enqueued (the convergence check); if it returns true the rest of the cycle is skipped.
 template <class F>
-void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Smoother& sm, int B, const double* r_in, const double* q,
-            double* r_out, F&& after_down0) {
-    const Cheb& ch = sm.ch;
-    const int nl = H.nlev;
-    const double* r_use = q ? r_out : r_in;  // the residual the rest of the cycle works with
-    if (nl == 1) {  // the mesh itself is the coarsest level
-        if (q) throw StatusFail{PDN_E_CUDA, "internal: fused update on a single-level hierarchy"};
-        const int nc = H.ny[0] * H.nx[0];
-        L.run(KC_SMALL, 0, [&] { k_coarse_pinv<<<cdiv((size_t)B * nc, 128), 128, 0, L.s>>>(H.pinv.as<double>(), nc, r_in, W.z0[1].as<double>(), B); });
-        L.run(KC_SMALL, 0, [&] { k_dot<<<dim3(1, B), 128, 0, L.s>>>(r_in, W.z0[1].as<double>(), (size_t)nc, W.s.rz); });
-        (void)after_down0();
-        return;
-    }
+void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Smoother& sm, int B, int ri, bool fused, F&& after_down0) {
+    const int nl = H.nlev, nu = sm.cr.nu;
+    const int ru = fused ? ri ^ 1 : ri;  // the residual the rest of the cycle works with
     for (int l = 0; l + 1 < nl; ++l) {
         const double V = (double)B * H.ny[l] * H.nx[l] * 8.0, Vc = (double)B * H.ny[l + 1] * H.nx[l + 1] * 8.0;
-        const double* rin = l == 0 ? r_in : W.rl[l].as<double>();
-        double* zout = l == 0 ? W.z0[0].as<double>() : W.za[l].as<double>();
-        const bool fused = (l == 0 && q);
-        const double bytes = (fused ? 4.0 : 2.0) * V + Vc;
-        if (sm.v1) {
-            NU_DISPATCH(ch.nu, (launch_down<NU_>(L, l == 0 ? KC_DOWN0 : KC_DOWNC, bytes, H.lev[l], ch, B, rin, fused ? q : nullptr,
-                                                 W.s.alpha, fused ? r_out : nullptr, zout, W.rl[l + 1].as<double>(),
-                                                 H.ny[l + 1], H.nx[l + 1], W.s.rr)));
-        } else {
-            NU_DISPATCH(ch.nu, (launch_down2<NU_>(L, l == 0 ? KC_DOWN0 : KC_DOWNC, bytes, H.lev[l], sm.cr, B, sm.G, rin, fused ? q : nullptr,
-                                                  W.s.alpha, fused ? r_out : nullptr, zout, W.rl[l + 1].as<double>(),
-                                                  H.ny[l + 1], H.nx[l + 1], W.s.rr)));
-        }
+        const bool f = (l == 0 && fused);
+        const double bytes = (f ? 4.0 : 2.0) * V + Vc;
+        NU_DISPATCH(nu, (launch_down3<NU_>(L, l == 0 ? KC_DOWN0 : KC_DOWNC, bytes, H.lev[l], sm, B, l == 0 ? W.m_r[ri] : W.m_rl[l],
+                                           f ? &W.m_q : nullptr, W.s.alpha, f ? W.r[ri ^ 1].as<double>() : nullptr,
+                                           l == 0 ? W.y0.as<double>() : W.ya[l].as<double>(), W.rl[l + 1].as<double>(),
+                                           H.ny[l + 1], H.nx[l + 1], H.pitch[l + 1], W.s.rr)));
         if (l == 0 && after_down0()) return;  // converged (or out of iterations): skip the rest of the cycle
     }
     const int lc = nl - 1, nc = H.ny[lc] * H.nx[lc];
-    L.run(KC_SMALL, 0, [&] { k_coarse_pinv<<<cdiv((size_t)B * nc, 128), 128, 0, L.s>>>(H.pinv.as<double>(), nc, W.rl[lc].as<double>(), W.za[lc].as<double>(), B); });
+    L.run(KC_SMALL, 0, [&] { k_coarse_pinv<<<cdiv((size_t)B * nc, 128), 128, 0, L.s>>>(H.pinv.as<double>(), H.nx[lc], H.pitch[lc], nc, H.plane(lc), W.rl[lc].as<double>(), W.zb[lc].as<double>(), B); });
     for (int l = nl - 2; l >= 0; --l) {
         const double V = (double)B * H.ny[l] * H.nx[l] * 8.0, Vc = (double)B * H.ny[l + 1] * H.nx[l + 1] * 8.0;
-        const double* rr = l == 0 ? r_use : W.rl[l].as<double>();
-        const double* zin = l == 0 ? W.z0[0].as<double>() : W.za[l].as<double>();
-        double* zout = l == 0 ? W.z0[1].as<double>() : W.zb[l].as<double>();
-        const double* ec = (l + 1 == lc) ? W.za[lc].as<double>() : W.zb[l + 1].as<double>();
-        if (sm.v1) {
-            NU_DISPATCH(ch.nu, (launch_up<NU_>(L, l == 0 ? KC_UP0 : KC_UPC, 3.0 * V + Vc, H.lev[l], ch, B, rr, zin, ec,
-                                               H.ny[l + 1], H.nx[l + 1], zout, l == 0 ? W.s.rz : nullptr)));
-        } else {
-            NU_DISPATCH(ch.nu, (launch_up2<NU_>(L, l == 0 ? KC_UP0 : KC_UPC, 3.0 * V + Vc, H.lev[l], sm.cr, B, sm.G, rr, zin, ec,
-                                                H.ny[l + 1], H.nx[l + 1], zout, l == 0 ? W.s.rz : nullptr)));
-        }
+        NU_DISPATCH(nu, (launch_up3<NU_>(L, l == 0 ? KC_UP0 : KC_UPC, 3.0 * V + Vc, H.lev[l], sm, B, l == 0 ? W.m_r[ru] : W.m_rl[l],
+                                         l == 0 ? W.m_y0 : W.m_ya[l], W.m_ec[l + 1],
+                                         l == 0 ? W.z.as<double>() : W.zb[l].as<double>(), l == 0 ? W.s.rz : nullptr)));
     }
 }
 
 // Solve L_t x_b = e_{port src0+b} - 1/n^2 for b in [0, B) by multigrid-preconditioned CG and leave
 //   TSV-source batch     : ZT[src0+b][k] = x_b[port k] - mean(x_b)      for all ports k of the tier
 //   terminal-source batch: zdiag[src0+b-ntsv] = x_b[own node] - mean(x_b)
-int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts& T, const Smoother& ch, int src0, int B,
-                bool terminal, double rtol, int max_iter);
-
-int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts& T, const Smoother& ch, int src0, int B,
+int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts& T, const Smoother& sm, int src0, int B,
                 bool terminal, double rtol, int max_iter) {
     const int n = H.ny[0];
-    const size_t n2 = (size_t)n * n;
+    const size_t n2 = (size_t)n * n, plane = H.plane(0);
     const double V = (double)B * n2 * 8.0;
     const int* node = T.d_node.as<int>();
     const int ngather = terminal ? 0 : T.q;
     int cur_r = 0, cur_p = 0;
     L.run(KC_SMALL, 0, [&] { k_pcg_init<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B); });
-    L.run(KC_SMALL, V, [&] { k_init_rhs<<<dim3(cdiv(n2, 256), B), 256, 0, L.s>>>(W.r[0].as<double>(), n2, node, src0, B); });
+    L.run(KC_SMALL, V, [&] { k_init_rhs<<<dim3(cdiv(plane, 256), B), 256, 0, L.s>>>(W.r[0].as<double>(), n, H.pitch[0], plane, 1.0 / (double)n2, node, src0, B); });
     if (terminal) CK(cudaMemsetAsync(W.xown.p, 0, (size_t)B * sizeof(double), L.s));
     else CK(cudaMemsetAsync(W.xport.p, 0, (size_t)B * ngather * sizeof(double), L.s));
-    vcycle(L, H, W, ch, B, W.r[0].as<double>(), nullptr, nullptr, [] { return false; });
+    vcycle(L, H, W, sm, B, 0, false, [] { return false; });
     const double bnorm2 = 1.0 - 1.0 / (double)n2;
     int it = 0, status = PDN_OK;
     while (true) {
         L.run(KC_SMALL, 0, [&] { k_scal_beta<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, it == 0); });
-        {
-            dim3 grid(cdiv(n, TI), cdiv(n, TI), B);
-            L.run(KC_PQ, 4.0 * V, [&] { k_pq<TI><<<grid, STENCIL_THREADS, 0, L.s>>>(H.lev[0], W.z0[1].as<double>(), W.p[cur_p].as<double>(), W.s.beta, W.p[cur_p ^ 1].as<double>(), W.q.as<double>(), W.s.pq, W.s.sump); });
-            cur_p ^= 1;
-        }
+        launch_pq3(L, 4.0 * V, H.lev[0], sm, B, W.m_z, W.m_p[cur_p], W.s.beta, W.p[cur_p ^ 1].as<double>(), W.q.as<double>(), W.s.pq, W.s.sump);
+        cur_p ^= 1;
         L.run(KC_SMALL, 0, [&] { k_scal_alpha<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, 1.0 / (double)n2); });
-        L.run(KC_SMALL, 0, [&] { k_xport<<<dim3(cdiv(std::max(ngather, 1), 128), B), 128, 0, L.s>>>(W.p[cur_p].as<double>(), n2, W.s.alpha, node, ngather, src0, W.xport.as<double>(), W.xown.as<double>(), B); });
+        L.run(KC_SMALL, 0, [&] { k_xport<<<dim3(cdiv(std::max(ngather, 1), 128), B), 128, 0, L.s>>>(W.p[cur_p].as<double>(), plane, W.s.alpha, node, ngather, src0, W.xport.as<double>(), W.xown.as<double>(), B); });
         ++it;
         bool done = false;
         auto check = [&] {
@@ -440,7 +497,7 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
             done = (*W.h_nact == 0);
             return done || it >= max_iter;
         };
-        vcycle(L, H, W, ch, B, W.r[cur_r].as<double>(), W.q.as<double>(), W.r[cur_r ^ 1].as<double>(), check);
+        vcycle(L, H, W, sm, B, cur_r, true, check);
         cur_r ^= 1;
         if (done) break;
         if (it >= max_iter) { status = PDN_E_NOCONV; break; }
@@ -461,6 +518,7 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     return status;
 }
 
+// ------------------------------------------------------------------------------------------------
 // ------------------------------------------------------------------------------------------------
 // S3 host drivers of the dense kernels (row-major, in place).
 void gemm(Launcher& L, int M, int N, int K, double alpha, const double* A, int64_t sai, int64_t sak, const double* B,
@@ -635,8 +693,8 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
     if (opts) o = *opts;
     if (!(o.rtol > 0.0)) o.rtol = 1e-9;
     if (o.max_iter <= 0) o.max_iter = 200;
-    if (o.nu <= 0) o.nu = 3;
-    if (o.nu > 4) o.nu = 4;
+    if (o.nu <= 0) o.nu = 4;
+    if (o.nu > 6) o.nu = 6;
 
     pdn_ctx* c = new (std::nothrow) pdn_ctx();
     if (!c) return PDN_E_NOMEM;
@@ -655,7 +713,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
             if (t.iface < 0 || t.iface >= d - 1) throw StatusFail{PDN_E_ARG, "TSV interface out of range"};
             if (t.y < 0 || t.y >= n || t.x < 0 || t.x >= n) throw StatusFail{PDN_E_ARG, "TSV site out of range"};
             if (!(t.r_ohm > 0.0) || !std::isfinite(t.r_ohm)) throw StatusFail{PDN_E_ARG, "TSV resistance must be positive and finite"};
-            const int id = t.y * n + t.x;
+            const int id = t.y * pitch_of(n) + t.x;  // pitched offset (port.cuh / pcg.cuh index vectors with it)
             if (!seen[t.iface].insert(id).second) throw StatusFail{PDN_E_ARG, "duplicate TSV site inside one interface"};
             site[t.iface].push_back(id);
             c->rt[t.iface].push_back(t.r_ohm);
@@ -667,7 +725,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         auto check_sites = [&](const pdn_site* s, int cnt, std::vector<int>& ids) {
             for (int k = 0; k < cnt; ++k) {
                 if (s[k].y < 0 || s[k].y >= n || s[k].x < 0 || s[k].x >= n) throw StatusFail{PDN_E_ARG, "bump/load site out of range"};
-                ids.push_back(s[k].y * n + s[k].x);
+                ids.push_back(s[k].y * pitch_of(n) + s[k].x);
             }
         };
         std::vector<int> bump_id, load_id;
@@ -709,6 +767,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         if (H.nlev > 1) {
             size_t free_b = 0, total_b = 0;
             CK(cudaMemGetInfo(&free_b, &total_b));
+            free_b += g_pool.cached_bytes();  // blocks kept by the pool are ours to reuse
             const size_t per = Work::bytes_per_rhs(H) + (size_t)qmax * 8 + 128;
             const size_t fit = std::max<size_t>(1, (size_t)(0.6 * (double)free_b) / per);
             Bmax = (int)std::min<size_t>({(size_t)qmax, fit, (size_t)1024});
@@ -716,8 +775,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         }
         Work W;
         if (H.nlev > 1) W.allocate(H, Bmax, qmax);
-        Smoother ch{make_cheb(o.nu, 6.0), make_cheb_roots(o.nu, 6.0), getenv("PDN_STENCIL_V1") != nullptr,
-                    getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 4};
+        Smoother ch{make_cheb_roots(o.nu, 6.0), getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 8};
         const double rtol_term = std::max(o.rtol, std::min(1e-5, std::sqrt(o.rtol) / 3.0));
         float ms_up = 0.f;
         for (int t = 0; t < d && status == PDN_OK; ++t) {
@@ -738,7 +796,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
             ms_up += ms;
             if (status != PDN_OK) { g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status); break; }
             if (H.nlev == 1) {
-                L.run(KC_SMALL, 0, [&] { k_direct_small<<<T.q, 64, 0, L.s>>>(H.pinv.as<double>(), n * n, T.d_node.as<int>(), T.ntsv, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
+                L.run(KC_SMALL, 0, [&] { k_direct_small<<<T.q, 64, 0, L.s>>>(H.pinv.as<double>(), n, H.pitch[0], n * n, T.d_node.as<int>(), T.ntsv, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
                 continue;
             }
             for (int s0 = 0; s0 < T.ntsv && status == PDN_OK; s0 += Bmax)
@@ -839,6 +897,8 @@ int pdn_reff_host(pdn_ctx* ctx, int64_t n_pairs, const int32_t* bump_idx, const 
     }
     return PDN_OK;
 }
+
+void pdn_release_cache(void) { g_pool.trim(); }
 
 int pdn_get_stats(const pdn_ctx* ctx, pdn_stats* out) {
     if (!ctx || !out) return fail_arg("null argument");

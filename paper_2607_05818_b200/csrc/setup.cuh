@@ -1,62 +1,85 @@
 // S0: tier representation -- sanitised copies of the conductance planes, the multigrid hierarchy
 // (2x2 aggregation, coarse conductance = 1/2 * sum of the two fine segments crossing the coarse
-// face), inverse diagonals, and the dense pseudo-inverse of the coarsest level.
+// face), the symmetric scaling of every level, and the dense pseudo-inverse of the coarsest level.
 #pragma once
 #include "common.cuh"
 
 namespace pdn {
 
-// Copy the caller's planes, zero the padding column / row, flag bad values (negative, NaN, inf).
-__global__ void k_import_planes(const double* __restrict__ gx_in, const double* __restrict__ gy_in, int n,
+// Copy the caller's dense n x n planes into pitched planes, zero the padding column / row, flag bad
+// values (negative, NaN, inf).
+__global__ void k_import_planes(const double* __restrict__ gx_in, const double* __restrict__ gy_in, int n, int pitch,
                                 double* __restrict__ gx, double* __restrict__ gy, int* __restrict__ bad) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n * n) return;
-    const int y = i / n, x = i % n;
-    double a = x < n - 1 ? gx_in[i] : 0.0;
-    double b = y < n - 1 ? gy_in[i] : 0.0;
-    if (!(a >= 0.0) || !(b >= 0.0) || isinf(a) || isinf(b)) {
-        atomicExch(bad, 1);
-        a = 0.0;
-        b = 0.0;
+    if (i >= n * pitch) return;
+    const int y = i / pitch, x = i % pitch;
+    double a = 0.0, b = 0.0;
+    if (x < n) {
+        a = x < n - 1 ? gx_in[y * n + x] : 0.0;
+        b = y < n - 1 ? gy_in[y * n + x] : 0.0;
+        if (!(a >= 0.0) || !(b >= 0.0) || isinf(a) || isinf(b)) {
+            atomicExch(bad, 1);
+            a = 0.0;
+            b = 0.0;
+        }
     }
     gx[i] = a;
     gy[i] = b;
 }
 
-// dinv = 1 / sum of incident conductances (0 if the node is isolated; flagged on the finest level).
-__global__ void k_dinv(int ny, int nx, const double* __restrict__ gx, const double* __restrict__ gy,
-                       double* __restrict__ dinv, int* __restrict__ isolated) {
+// s = 1/sqrt(d), sd = sqrt(d), d = sum of incident conductances (both 0 if the node is isolated;
+// flagged on the finest level).
+__global__ void k_scale_nodes(int ny, int nx, int pitch, const double* __restrict__ gx, const double* __restrict__ gy,
+                              double* __restrict__ s, double* __restrict__ sd, int* __restrict__ isolated) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= ny * nx) return;
-    const int y = i / nx, x = i % nx;
-    double d = gx[i] + gy[i];
-    if (x > 0) d += gx[i - 1];
-    if (y > 0) d += gy[i - nx];
-    if (d > 0.0) {
-        dinv[i] = 1.0 / d;
-    } else {
-        dinv[i] = 0.0;
-        if (isolated) atomicExch(isolated, 1);
+    if (i >= ny * pitch) return;
+    const int y = i / pitch, x = i % pitch;
+    double d = 0.0;
+    if (x < nx) {
+        d = gx[i] + gy[i];
+        if (x > 0) d += gx[i - 1];
+        if (y > 0) d += gy[i - pitch];
     }
+    if (d > 0.0) {
+        const double r = sqrt(d);
+        sd[i] = r;
+        s[i] = 1.0 / r;
+    } else {
+        sd[i] = 0.0;
+        s[i] = 0.0;
+        if (isolated && x < nx) atomicExch(isolated, 1);
+    }
+}
+
+// hE = gx s s_east, hS = gy s s_south  (symmetric scaling; zero where the segment is absent).
+__global__ void k_scale_edges(int ny, int nx, int pitch, const double* __restrict__ gx, const double* __restrict__ gy,
+                              const double* __restrict__ s, double* __restrict__ hE, double* __restrict__ hS) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= ny * pitch) return;
+    const int y = i / pitch, x = i % pitch;
+    hE[i] = (x + 1 < nx) ? gx[i] * s[i] * s[i + 1] : 0.0;
+    hS[i] = (x < nx && y + 1 < ny) ? gy[i] * s[i] * s[i + pitch] : 0.0;
 }
 
 // Coarse planes (cny x cnx, cn = ceil(n/2)) from fine planes (ny x nx).
 //   cgx[Y][X] = 1/2 (gx[2Y][2X+1] + gx[2Y+1][2X+1])   -- the fine x-segments leaving aggregate X to X+1
 //   cgy[Y][X] = 1/2 (gy[2Y+1][2X] + gy[2Y+1][2X+1])
-__global__ void k_coarsen(int ny, int nx, const double* __restrict__ gx, const double* __restrict__ gy, int cny,
-                          int cnx, double* __restrict__ cgx, double* __restrict__ cgy) {
+__global__ void k_coarsen(int ny, int nx, int pitch, const double* __restrict__ gx, const double* __restrict__ gy,
+                          int cny, int cnx, int cpitch, double* __restrict__ cgx, double* __restrict__ cgy) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= cny * cnx) return;
-    const int Y = i / cnx, X = i % cnx;
+    if (i >= cny * cpitch) return;
+    const int Y = i / cpitch, X = i % cpitch;
     double a = 0.0, b = 0.0;
     const int fx = 2 * X + 1, fy = 2 * Y + 1;
-    if (fx < nx - 1) {  // a segment from column fx to fx+1 exists only if fx+1 < nx
-        a += gx[(2 * Y) * nx + fx];
-        if (fy < ny) a += gx[fy * nx + fx];
-    }
-    if (fy < ny - 1) {
-        b += gy[fy * nx + 2 * X];
-        if (fx < nx) b += gy[fy * nx + fx];
+    if (X < cnx) {
+        if (fx < nx - 1) {  // a segment from column fx to fx+1 exists only if fx+1 < nx
+            a += gx[(2 * Y) * pitch + fx];
+            if (fy < ny) a += gx[fy * pitch + fx];
+        }
+        if (fy < ny - 1) {
+            b += gy[fy * pitch + 2 * X];
+            if (fx < nx) b += gy[fy * pitch + fx];
+        }
     }
     cgx[i] = 0.5 * a;
     cgy[i] = 0.5 * b;
@@ -64,8 +87,8 @@ __global__ void k_coarsen(int ny, int nx, const double* __restrict__ gx, const d
 
 // Dense pseudo-inverse of the coarsest Laplacian (nc = ny*nx <= 16 unknowns), one block, one thread:
 //   L^+ = (L + 11^T/nc)^-1 - 11^T/nc   (Gauss-Jordan on an SPD matrix, no pivoting needed).
-__global__ void k_coarsest_pinv(int ny, int nx, const double* __restrict__ gx, const double* __restrict__ gy,
-                                double* __restrict__ pinv) {
+__global__ void k_coarsest_pinv(int ny, int nx, int pitch, const double* __restrict__ gx,
+                                const double* __restrict__ gy, double* __restrict__ pinv) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     const int nc = ny * nx;
     double A[16][32];
@@ -75,11 +98,11 @@ __global__ void k_coarsest_pinv(int ny, int nx, const double* __restrict__ gx, c
         for (int x = 0; x < nx; ++x) {
             const int i = y * nx + x;
             if (x < nx - 1) {
-                const double g = gx[i];
+                const double g = gx[y * pitch + x];
                 A[i][i] += g; A[i + 1][i + 1] += g; A[i][i + 1] -= g; A[i + 1][i] -= g;
             }
             if (y < ny - 1) {
-                const double g = gy[i];
+                const double g = gy[y * pitch + x];
                 A[i][i] += g; A[i + nx][i + nx] += g; A[i][i + nx] -= g; A[i + nx][i] -= g;
             }
         }
@@ -105,17 +128,18 @@ __global__ void k_label_init(int n2, int* __restrict__ lab) {
     if (i < n2) lab[i] = i;
 }
 
-__global__ void k_label_sweep(int ny, int nx, const double* __restrict__ gx, const double* __restrict__ gy,
-                              int* __restrict__ lab, int* __restrict__ changed) {
+__global__ void k_label_sweep(int ny, int nx, int pitch, const double* __restrict__ gx,
+                              const double* __restrict__ gy, int* __restrict__ lab, int* __restrict__ changed) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= ny * nx) return;
     const int y = i / nx, x = i % nx;
+    const int g = y * pitch + x;
     int m = lab[i];
     const int m0 = m;
-    if (x < nx - 1 && gx[i] > 0.0) m = min(m, lab[i + 1]);
-    if (x > 0 && gx[i - 1] > 0.0) m = min(m, lab[i - 1]);
-    if (y < ny - 1 && gy[i] > 0.0) m = min(m, lab[i + nx]);
-    if (y > 0 && gy[i - nx] > 0.0) m = min(m, lab[i - nx]);
+    if (x < nx - 1 && gx[g] > 0.0) m = min(m, lab[i + 1]);
+    if (x > 0 && gx[g - 1] > 0.0) m = min(m, lab[i - 1]);
+    if (y < ny - 1 && gy[g] > 0.0) m = min(m, lab[i + nx]);
+    if (y > 0 && gy[g - pitch] > 0.0) m = min(m, lab[i - nx]);
     // pointer jumping: the label of my label is at least as small
     int mm = lab[m];
     while (mm < m) { m = mm; mm = lab[m]; }

@@ -1,0 +1,443 @@
+// S1: batched matrix-free multigrid-PCG kernels on the per-tier 2D 5-point stencil (sm_100a).
+//
+// Layout.  Every vector is a batch of pitched planes v[b][y][pitch] (b = right-hand side).
+//
+// Tiling.  A block of W warps owns an extended tile of 64 x (R*W) nodes: interior
+// (64-2H) x (R*W-2H) plus a halo of H nodes that is recomputed redundantly, so a whole multigrid
+// stage (all its sweeps) runs on chip with no exchange between blocks.  Lane l of warp w owns the
+// 2 x R patch of columns 2l, 2l+1 and rows R*w .. R*w+R-1:
+//   * the iterate and the stencil coefficients of the patch live in REGISTERS for the whole kernel;
+//     the coefficients are loaded once per block and reused for the G right-hand sides it loops over;
+//   * left / right neighbours come from the adjacent lanes by warp shuffles, the rows above / below
+//     the patch through a double-buffered shared-memory exchange (one barrier per sweep);
+//   * the tile + halo of every input vector is fetched by TMA (cp.async.bulk.tensor, 3D box
+//     64 x R*W x 1 of a (x, y, rhs) tensor map) into shared memory, completion on an mbarrier, the
+//     fetch of right-hand side b+1 overlapping the sweeps of b.  Out-of-mesh elements arrive as
+//     zeros, and the coefficients there are zero, so the sweeps need no boundary cases;
+//   * global stores are 16-byte (both columns of a patch row), interior only.
+//
+// Arithmetic.  All sweeps act on the symmetrically scaled system (common.cuh: Level):
+//   y <- (1-w) y + w (r^ + sum_nb h_nb y_nb),   r^ = s r,   z = s y.
+#pragma once
+#include "common.cuh"
+
+namespace pdn {
+
+constexpr unsigned FULL = 0xffffffffu;
+constexpr int T3_EW = 64;
+// The coarse correction of a tile is 32 coarse columns starting at x0/2, which may be odd; TMA wants the
+// innermost box coordinate 16-byte aligned, so the box starts at the even column below and is 34 wide.
+constexpr int T3_ECW = 34;
+
+template <int R>
+struct Patch {  // scaled coefficients of a 2 x R patch
+    double hE0[R], hE1[R];  // east of column 0 (= west of column 1), east of column 1
+    double hW0[R];          // west of column 0
+    double hS0[R], hS1[R];  // south of row i (= north of row i+1)
+    double hN0, hN1;        // north of row 0
+};
+
+template <int W>
+struct Exch {  // rows above / below every warp's patch, double buffered; slot 0 of bot and slot W of top stay 0
+    double2 top[2][W + 1][32];
+    double2 bot[2][W + 1][32];
+};
+
+__device__ __forceinline__ double2 ld2(const double* p) { return *reinterpret_cast<const double2*>(p); }
+__device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<double2*>(p) = v; }
+__device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
+
+template <int R, int W>
+__device__ __forceinline__ void exch_clear(Exch<W>& x) {
+    for (int i = threadIdx.x; i < 2 * 32; i += 32 * W) {
+        x.top[i >> 5][W][i & 31] = make_double2(0.0, 0.0);
+        x.bot[i >> 5][0][i & 31] = make_double2(0.0, 0.0);
+    }
+}
+
+// Coefficients of this thread's patch (zeros outside the mesh) and its slots of the s / sd tiles.
+template <int R>
+__device__ __forceinline__ void patch_init(Patch<R>& c, const Level& L, int gx, int gy0, double* sS, double* sSD,
+                                           int slot0) {
+    const bool xin = gx >= 0 && gx < L.pitch;  // gx is even, pitch is even: both columns are addressable
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+        const int gy = gy0 + i;
+        const bool in = xin && gy >= 0 && gy < L.ny;
+        const size_t gi = (size_t)gy * L.pitch + gx;
+        const double2 z2 = make_double2(0.0, 0.0);
+        const double2 e = in ? ldg2(L.hE + gi) : z2;
+        const double2 s = in ? ldg2(L.hS + gi) : z2;
+        c.hE0[i] = e.x; c.hE1[i] = e.y;
+        c.hS0[i] = s.x; c.hS1[i] = s.y;
+        c.hW0[i] = (in && gx > 0) ? __ldg(L.hE + gi - 1) : 0.0;
+        if (sS) st2(sS + slot0 + i * T3_EW, in ? ldg2(L.s + gi) : z2);
+        st2(sSD + slot0 + i * T3_EW, in ? ldg2(L.sd + gi) : z2);
+    }
+    const int gyn = gy0 - 1;
+    const double2 nn = (xin && gyn >= 0 && gyn < L.ny) ? ldg2(L.hS + (size_t)gyn * L.pitch + gx) : make_double2(0.0, 0.0);
+    c.hN0 = nn.x; c.hN1 = nn.y;
+}
+
+// t += sum over the four neighbours of h_nb * y_nb  (t comes in holding the additive term).
+// One barrier; `cur` flips.
+template <int R, int W>
+__device__ __forceinline__ void nb_sum(Exch<W>& x, int& cur, const Patch<R>& c, int warp, int lane,
+                                       const double (&y0)[R], const double (&y1)[R], double (&t0)[R],
+                                       double (&t1)[R]) {
+    x.top[cur][warp][lane] = make_double2(y0[0], y1[0]);
+    x.bot[cur][warp + 1][lane] = make_double2(y0[R - 1], y1[R - 1]);
+    __syncthreads();
+    const double2 up = x.bot[cur][warp][lane];
+    const double2 dn = x.top[cur][warp + 1][lane];
+    cur ^= 1;
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+        const double yl = __shfl_up_sync(FULL, y1[i], 1);    // right column of the lane to the left
+        const double yr = __shfl_down_sync(FULL, y0[i], 1);  // left column of the lane to the right
+        const double u0 = i == 0 ? up.x : y0[i - 1], u1 = i == 0 ? up.y : y1[i - 1];
+        const double d0 = i == R - 1 ? dn.x : y0[i + 1], d1 = i == R - 1 ? dn.y : y1[i + 1];
+        const double n0 = i == 0 ? c.hN0 : c.hS0[i - 1], n1 = i == 0 ? c.hN1 : c.hS1[i - 1];
+        double a = fma(c.hE0[i], y1[i], t0[i]);
+        a = fma(c.hW0[i], yl, a);
+        a = fma(c.hS0[i], d0, a);
+        t0[i] = fma(n0, u0, a);
+        double b = fma(c.hE1[i], yr, t1[i]);
+        b = fma(c.hE0[i], y0[i], b);
+        b = fma(c.hS1[i], d1, b);
+        t1[i] = fma(n1, u1, b);
+    }
+}
+
+template <int R, int W, int H>
+struct Geom {
+    static constexpr int EH = R * W, IW = T3_EW - 2 * H, IH = EH - 2 * H, TILE = EH * T3_EW, THREADS = 32 * W;
+    static constexpr int ETILE = (EH / 2) * T3_ECW;  // coarse-correction tile of the up stage
+    static constexpr uint32_t TILE_BYTES = TILE * sizeof(double), ETILE_BYTES = ETILE * sizeof(double);
+    static_assert(R % 2 == 0 && H % 2 == 0, "2x2 aggregates must not straddle patches");
+    static_assert(IW > 0 && IH > 0, "halo too deep for the tile");
+};
+
+__host__ __device__ constexpr int halo_of(int nu) { return (nu + 1) & ~1; }
+
+// ---------------------------------------------------------------------------------------------
+// Down stage of the V-cycle on one level (fused with the CG residual update on level 0):
+//   [r = r_in - alpha q ; rr += r.r]   y = S_nu(0, r^)   rc = R sd (r^ - A^ y)
+// y (the scaled iterate) is written to y_out for the up stage; R sums 2x2 aggregates.
+// grid = (tiles_x, tiles_y, ceil(B / G)); the block loops over G right-hand sides.
+template <int R, int W, int NU, bool FUSED>
+__global__ void __launch_bounds__(32 * W, 1)
+k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensorMap tm_q, Level L, ChebR ch,
+        const double* __restrict__ alpha, double* __restrict__ r_out, double* __restrict__ y_out,
+        double* __restrict__ rc, int cny, int cnx, int cpitch, double* __restrict__ rr_acc, int B, int G) {
+    constexpr int H = halo_of(NU);
+    using Gm = Geom<R, W, H>;
+    extern __shared__ __align__(128) double smem_dyn[];
+    double* rbuf = smem_dyn;              // 2 stages
+    double* qbuf = rbuf + 2 * Gm::TILE;             // 1 stage (consumed at the start of an iteration)
+    double* sS = qbuf + (FUSED ? Gm::TILE : 0);
+    double* sSD = sS + Gm::TILE;
+    Exch<W>& x = *reinterpret_cast<Exch<W>*>(sSD + Gm::TILE);
+    __shared__ uint64_t mbar[3];
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int x0 = blockIdx.x * Gm::IW - H, y0 = blockIdx.y * Gm::IH - H;
+    const int gx = x0 + 2 * lane, gy0 = y0 + R * warp;
+    const int slot0 = (R * warp) * T3_EW + 2 * lane;
+    Patch<R> c;
+    patch_init<R>(c, L, gx, gy0, sS, sSD, slot0);
+    exch_clear<R, W>(x);
+    const bool xint = 2 * lane >= H && 2 * lane < H + Gm::IW && gx < L.nx;
+    unsigned interior = 0;  // bit i: row i of the patch is an interior row of the tile and inside the mesh
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+        const int ey = R * warp + i;
+        if (xint && ey >= H && ey < H + Gm::IH && gy0 + i < L.ny) interior |= 1u << i;
+    }
+    const size_t plane = (size_t)L.ny * L.pitch, cplane = (size_t)cny * cpitch;
+    const size_t goff = (size_t)gy0 * L.pitch + gx;
+    const int b0 = blockIdx.z * G, nb = min(G, B - b0);
+    if (threadIdx.x == 0) {
+        mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); mbar_init(&mbar[2], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    auto fetch = [&](int j) {  // thread 0 only
+        mbar_expect_tx(&mbar[j & 1], Gm::TILE_BYTES);
+        tma_load_3d(rbuf + (j & 1) * Gm::TILE, &tm_r, x0, y0, b0 + j, &mbar[j & 1]);
+        if (FUSED) {
+            mbar_expect_tx(&mbar[2], Gm::TILE_BYTES);
+            tma_load_3d(qbuf, &tm_q, x0, y0, b0 + j, &mbar[2]);
+        }
+    };
+    if (threadIdx.x == 0) fetch(0);
+    int cur = 0;
+    for (int j = 0; j < nb; ++j) {
+        const int b = b0 + j;
+        double* rs = rbuf + (j & 1) * Gm::TILE + slot0;
+        mbar_wait(&mbar[j & 1], (j >> 1) & 1);
+        if (FUSED) mbar_wait(&mbar[2], j & 1);
+        const double al = FUSED ? alpha[b] : 0.0;
+        double y0r[R], y1r[R], rr = 0.0;
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            double2 r = ld2(rs + i * T3_EW);
+            if (FUSED) {
+                const double2 q = ld2(qbuf + slot0 + i * T3_EW);
+                r.x = fma(-al, q.x, r.x);
+                r.y = fma(-al, q.y, r.y);
+                if ((interior >> i) & 1) {
+                    st2(r_out + b * plane + goff + (size_t)i * L.pitch, r);
+                    rr = fma(r.x, r.x, rr);
+                    rr = fma(r.y, r.y, rr);
+                }
+            }
+            const double2 s = ld2(sS + slot0 + i * T3_EW);
+            r.x *= s.x; r.y *= s.y;
+            st2(rs + i * T3_EW, r);  // r^ stays in this thread's own slots of the stage buffer
+            y0r[i] = ch.w[0] * r.x;
+            y1r[i] = ch.w[0] * r.y;
+        }
+        fence_proxy_async();  // order these generic-proxy writes before the TMA write that reuses the stage
+        bool fetched = false;
+        auto after_first_barrier = [&] {
+            if (!fetched && threadIdx.x == 0 && j + 1 < nb) fetch(j + 1);
+            fetched = true;
+        };
+#pragma unroll
+        for (int k = 1; k < NU; ++k) {
+            double t0[R], t1[R];
+#pragma unroll
+            for (int i = 0; i < R; ++i) { const double2 r = ld2(rs + i * T3_EW); t0[i] = r.x; t1[i] = r.y; }
+            nb_sum<R, W>(x, cur, c, warp, lane, y0r, y1r, t0, t1);
+            after_first_barrier();
+            const double w = ch.w[k], a = 1.0 - w;
+#pragma unroll
+            for (int i = 0; i < R; ++i) {
+                y0r[i] = fma(w, t0[i], a * y0r[i]);
+                y1r[i] = fma(w, t1[i], a * y1r[i]);
+            }
+        }
+        double t0[R], t1[R];
+#pragma unroll
+        for (int i = 0; i < R; ++i) { const double2 r = ld2(rs + i * T3_EW); t0[i] = r.x; t1[i] = r.y; }
+        nb_sum<R, W>(x, cur, c, warp, lane, y0r, y1r, t0, t1);
+        after_first_barrier();
+        // residual of the unscaled system at the patch nodes, summed over 2x2 aggregates
+#pragma unroll
+        for (int i = 0; i < R; i += 2) {
+            const double2 sda = ld2(sSD + slot0 + i * T3_EW), sdb = ld2(sSD + slot0 + (i + 1) * T3_EW);
+            double v = sda.x * (t0[i] - y0r[i]);
+            v = fma(sda.y, t1[i] - y1r[i], v);
+            v = fma(sdb.x, t0[i + 1] - y0r[i + 1], v);
+            v = fma(sdb.y, t1[i + 1] - y1r[i + 1], v);
+            if ((interior >> i) & 1) {  // rows i and i+1 are interior together (H, R, y0 even)
+                st2(y_out + b * plane + goff + (size_t)i * L.pitch, make_double2(y0r[i], y1r[i]));
+                if ((interior >> (i + 1)) & 1)
+                    st2(y_out + b * plane + goff + (size_t)(i + 1) * L.pitch, make_double2(y0r[i + 1], y1r[i + 1]));
+                rc[b * cplane + (size_t)((gy0 + i) >> 1) * cpitch + (gx >> 1)] = v;
+            }
+        }
+        if (FUSED) {
+            rr = warp_sum(rr);
+            if (lane == 0) atomicAdd(rr_acc + b, rr);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Up stage:  y = y_in + sd P e_c ;  y = S_nu(y, r^) ;  z = s y ;  [rz += r.z]
+// P = piecewise-constant prolongation (fine (y,x) takes coarse (y/2, x/2)).
+template <int R, int W, int NU, bool DOT>
+__global__ void __launch_bounds__(32 * W, 1)
+k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensorMap tm_y,
+      const __grid_constant__ CUtensorMap tm_e, Level L, ChebR ch, double* __restrict__ z_out,
+      double* __restrict__ rz_acc, int B, int G) {
+    constexpr int H = halo_of(NU);
+    using Gm = Geom<R, W, H>;
+    extern __shared__ __align__(128) double smem_dyn[];
+    double* rbuf = smem_dyn;   // 2 stages
+    double* ybuf = rbuf + 2 * Gm::TILE;  // 1 stage
+    double* ebuf = ybuf + Gm::TILE;      // 1 stage, T3_ECW x EH/2
+    double* sS = ebuf + Gm::ETILE;
+    double* sSD = sS + Gm::TILE;
+    Exch<W>& x = *reinterpret_cast<Exch<W>*>(sSD + Gm::TILE);
+    __shared__ uint64_t mbar[3];
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int x0 = blockIdx.x * Gm::IW - H, y0 = blockIdx.y * Gm::IH - H;
+    const int gx = x0 + 2 * lane, gy0 = y0 + R * warp;
+    const int slot0 = (R * warp) * T3_EW + 2 * lane;
+    Patch<R> c;
+    patch_init<R>(c, L, gx, gy0, sS, sSD, slot0);
+    exch_clear<R, W>(x);
+    const bool xint = 2 * lane >= H && 2 * lane < H + Gm::IW && gx < L.nx;
+    unsigned interior = 0;
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+        const int ey = R * warp + i;
+        if (xint && ey >= H && ey < H + Gm::IH && gy0 + i < L.ny) interior |= 1u << i;
+    }
+    const size_t plane = (size_t)L.ny * L.pitch;
+    const size_t goff = (size_t)gy0 * L.pitch + gx;
+    const int b0 = blockIdx.z * G, nb = min(G, B - b0);
+    const int cx0 = (x0 >> 1) & ~1;                 // even coarse column at or below x0/2 (x0 is even)
+    const int eslot = (x0 >> 1) - cx0 + lane;       // this lane's coarse column inside the box
+    if (threadIdx.x == 0) {
+        mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); mbar_init(&mbar[2], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    auto fetch = [&](int j) {  // thread 0 only
+        mbar_expect_tx(&mbar[j & 1], Gm::TILE_BYTES);
+        tma_load_3d(rbuf + (j & 1) * Gm::TILE, &tm_r, x0, y0, b0 + j, &mbar[j & 1]);
+        mbar_expect_tx(&mbar[2], Gm::TILE_BYTES + Gm::ETILE_BYTES);
+        tma_load_3d(ybuf, &tm_y, x0, y0, b0 + j, &mbar[2]);
+        tma_load_3d(ebuf, &tm_e, cx0, y0 / 2, b0 + j, &mbar[2]);
+    };
+    if (threadIdx.x == 0) fetch(0);
+    int cur = 0;
+    for (int j = 0; j < nb; ++j) {
+        const int b = b0 + j;
+        double* rs = rbuf + (j & 1) * Gm::TILE + slot0;
+        mbar_wait(&mbar[j & 1], (j >> 1) & 1);
+        mbar_wait(&mbar[2], j & 1);
+        double y0r[R], y1r[R];
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            double2 r = ld2(rs + i * T3_EW);
+            const double2 s = ld2(sS + slot0 + i * T3_EW);
+            r.x *= s.x; r.y *= s.y;
+            st2(rs + i * T3_EW, r);
+            const double2 yin = ld2(ybuf + slot0 + i * T3_EW);
+            const double2 sd = ld2(sSD + slot0 + i * T3_EW);
+            const double e = ebuf[((R * warp + i) >> 1) * T3_ECW + eslot];
+            y0r[i] = fma(sd.x, e, yin.x);
+            y1r[i] = fma(sd.y, e, yin.y);
+        }
+        fence_proxy_async();
+#pragma unroll
+        for (int k = 0; k < NU; ++k) {
+            double t0[R], t1[R];
+#pragma unroll
+            for (int i = 0; i < R; ++i) { const double2 r = ld2(rs + i * T3_EW); t0[i] = r.x; t1[i] = r.y; }
+            nb_sum<R, W>(x, cur, c, warp, lane, y0r, y1r, t0, t1);
+            if (k == 0 && threadIdx.x == 0 && j + 1 < nb) fetch(j + 1);
+            const double w = ch.w[NU - 1 - k], a = 1.0 - w;
+#pragma unroll
+            for (int i = 0; i < R; ++i) {
+                y0r[i] = fma(w, t0[i], a * y0r[i]);
+                y1r[i] = fma(w, t1[i], a * y1r[i]);
+            }
+        }
+        double rz = 0.0;
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            if ((interior >> i) & 1) {
+                const double2 s = ld2(sS + slot0 + i * T3_EW);
+                st2(z_out + b * plane + goff + (size_t)i * L.pitch, make_double2(s.x * y0r[i], s.y * y1r[i]));
+                if (DOT) {
+                    const double2 r = ld2(rs + i * T3_EW);  // r.z = (sd r^).(s y) = r^.y
+                    rz = fma(r.x, y0r[i], rz);
+                    rz = fma(r.y, y1r[i], rz);
+                }
+            }
+        }
+        if (DOT) {
+            rz = warp_sum(rz);
+            if (lane == 0) atomicAdd(rz_acc + b, rz);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// CG direction update fused with the operator apply (level 0):
+//   p = z + beta p_old ;  q = L p = sd (p^ - N p^), p^ = sd p ;  pq += p.q ;  sump += sum(p)
+template <int R, int W>
+__global__ void __launch_bounds__(32 * W, 1)
+k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensorMap tm_p, Level L,
+      const double* __restrict__ beta, double* __restrict__ p_new, double* __restrict__ q,
+      double* __restrict__ pq_acc, double* __restrict__ sump_acc, int B, int G) {
+    constexpr int H = 2;  // one ring is needed; two keep the 16-byte column pairs aligned
+    using Gm = Geom<R, W, H>;
+    extern __shared__ __align__(128) double smem_dyn[];
+    double* zbuf = smem_dyn;
+    double* pbuf = zbuf + Gm::TILE;
+    double* sSD = pbuf + Gm::TILE;
+    Exch<W>& x = *reinterpret_cast<Exch<W>*>(sSD + Gm::TILE);
+    __shared__ uint64_t mbar;
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int x0 = blockIdx.x * Gm::IW - H, y0 = blockIdx.y * Gm::IH - H;
+    const int gx = x0 + 2 * lane, gy0 = y0 + R * warp;
+    const int slot0 = (R * warp) * T3_EW + 2 * lane;
+    Patch<R> c;
+    patch_init<R>(c, L, gx, gy0, nullptr, sSD, slot0);
+    exch_clear<R, W>(x);
+    const bool xint = 2 * lane >= H && 2 * lane < H + Gm::IW && gx < L.nx;
+    unsigned interior = 0;
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+        const int ey = R * warp + i;
+        if (xint && ey >= H && ey < H + Gm::IH && gy0 + i < L.ny) interior |= 1u << i;
+    }
+    const size_t plane = (size_t)L.ny * L.pitch;
+    const size_t goff = (size_t)gy0 * L.pitch + gx;
+    const int b0 = blockIdx.z * G, nb = min(G, B - b0);
+    if (threadIdx.x == 0) {
+        mbar_init(&mbar, 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    auto fetch = [&](int j) {  // thread 0 only
+        mbar_expect_tx(&mbar, 2 * Gm::TILE_BYTES);
+        tma_load_3d(zbuf, &tm_z, x0, y0, b0 + j, &mbar);
+        tma_load_3d(pbuf, &tm_p, x0, y0, b0 + j, &mbar);
+    };
+    if (threadIdx.x == 0) fetch(0);
+    int cur = 0;
+    for (int j = 0; j < nb; ++j) {
+        const int b = b0 + j;
+        mbar_wait(&mbar, j & 1);
+        const double bt = beta[b];
+        double y0r[R], y1r[R], t0[R], t1[R], sump = 0.0, pq = 0.0;
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            double2 p = ld2(zbuf + slot0 + i * T3_EW);
+            if (bt != 0.0) {  // beta = 0 on the first iteration: p_old is not initialised then
+                const double2 po = ld2(pbuf + slot0 + i * T3_EW);
+                p.x = fma(bt, po.x, p.x);
+                p.y = fma(bt, po.y, p.y);
+            }
+            if ((interior >> i) & 1) {
+                st2(p_new + b * plane + goff + (size_t)i * L.pitch, p);
+                sump += p.x + p.y;
+            }
+            const double2 sd = ld2(sSD + slot0 + i * T3_EW);
+            y0r[i] = sd.x * p.x;
+            y1r[i] = sd.y * p.y;
+            t0[i] = 0.0;
+            t1[i] = 0.0;
+        }
+        nb_sum<R, W>(x, cur, c, warp, lane, y0r, y1r, t0, t1);
+        if (threadIdx.x == 0 && j + 1 < nb) fetch(j + 1);
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            if ((interior >> i) & 1) {
+                const double2 sd = ld2(sSD + slot0 + i * T3_EW);
+                const double a0 = y0r[i] - t0[i], a1 = y1r[i] - t1[i];
+                st2(q + b * plane + goff + (size_t)i * L.pitch, make_double2(sd.x * a0, sd.y * a1));
+                pq = fma(y0r[i], a0, pq);  // p.q = p^.(p^ - N p^)
+                pq = fma(y1r[i], a1, pq);
+            }
+        }
+        pq = warp_sum(pq);
+        sump = warp_sum(sump);
+        if (lane == 0) {
+            atomicAdd(pq_acc + b, pq);
+            atomicAdd(sump_acc + b, sump);
+        }
+    }
+}
+
+}  // namespace pdn
