@@ -16,19 +16,23 @@ constexpr int COARSEST_MAX = 4; // coarsest level has n <= 4 (<= 16 unknowns, de
 // (nx rounded up to an even number), so that a thread's two adjacent columns are one aligned
 // 16-byte word and TMA row strides are multiples of 16 bytes.  Pad entries of planes are zero.
 //
-// The V-cycle works on the symmetrically scaled operator  A^ = S L S = I - N,  S = D^-1/2:
-//   s  = 1/sqrt(d), sd = sqrt(d)   (d = sum of the incident conductances; 0 for a node with d = 0)
-//   hE[y][x] = gx[y][x] * s[y][x] * s[y][x+1]      hS[y][x] = gy[y][x] * s[y][x] * s[y+1][x]
-// so that the Jacobi-preconditioned Richardson step z <- z + w D^-1 (r - L z) becomes, for y = z/s,
-// r^ = s r:   y <- (1-w) y + w (r^ + sum_nb h_nb y_nb)  -- no diagonal in the inner loop.
+// The V-cycle works on the symmetrically scaled operator  A^ = S L S ~ I - N  (S = D^-1/2), so that the
+// Jacobi-preconditioned Richardson step z <- z + w D^-1 (r - L z) becomes, for y = z/s, r^ = s r:
+//   y <- (1-w) y + w (r^ + sum_nb h_nb y_nb)      -- no diagonal in the inner loop.
+//   sc[y][x]  = (s, sd) = (1/sqrt(d), sqrt(d)) rounded to FP32 (d = sum of the incident conductances;
+//               (0, 0) for a node with d = 0).  The scaling is part of the PRECONDITIONER only: any
+//               positive diagonal works there, symmetry needs the same S on the way in (r^ = s r,
+//               rc = R sd res) and out (y += sd P e, z = s y), and FP32 entries halve the on-chip
+//               footprint.  All arithmetic with them is FP64.
+//   hE[y][x]  = gx[y][x] * s[y][x] * s[y][x+1],  hS[y][x] = gy[y][x] * s[y][x] * s[y+1][x]   (FP64).
+// The CG operator apply (k_pq3) uses the raw gx / gy.
 struct Level {
     int ny, nx, pitch;
     const double* gx;   // raw conductances (level 0: sanitised copy of the caller's planes)
     const double* gy;
     const double* hE;
     const double* hS;
-    const double* s;
-    const double* sd;
+    const float2* sc;
 };
 
 // Richardson steps with the reciprocals of the Chebyshev nodes of [2/ratio, 2] as step lengths: the

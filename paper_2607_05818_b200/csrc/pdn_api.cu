@@ -230,7 +230,7 @@ CUtensorMap make_map(const void* base, int nx, int ny, int pitch, int B, int box
 #define PDN_T3_W 16
 #endif
 constexpr int T3_R = PDN_T3_R, T3_W = PDN_T3_W, T3_EH = T3_R * T3_W, T3_THREADS = 32 * T3_W;
-constexpr size_t T3_TILE_BYTES = (size_t)T3_EH * T3_EW * sizeof(double);
+constexpr size_t T3_TILE_BYTES = (size_t)T3_EH * T3_EW * sizeof(double), T3_SC_BYTES = (size_t)T3_EH * 32 * sizeof(float4);
 
 inline int pitch_of(int nx) { return (nx + 1) & ~1; }
 
@@ -239,7 +239,7 @@ inline int pitch_of(int nx) { return (nx + 1) & ~1; }
 struct Hierarchy {
     int nlev = 0;
     int ny[MAX_LEVELS], nx[MAX_LEVELS], pitch[MAX_LEVELS];
-    DevBuf gx[MAX_LEVELS], gy[MAX_LEVELS], hE[MAX_LEVELS], hS[MAX_LEVELS], s[MAX_LEVELS], sd[MAX_LEVELS];
+    DevBuf gx[MAX_LEVELS], gy[MAX_LEVELS], hE[MAX_LEVELS], hS[MAX_LEVELS], sc[MAX_LEVELS];
     DevBuf pinv, flags, labels;  // flags: [0] bad value, [1] isolated node, [2] label changed, [3] label nonzero
     Level lev[MAX_LEVELS];
 
@@ -252,9 +252,9 @@ struct Hierarchy {
             ny[nlev] = nx[nlev] = cur;
             pitch[nlev] = pitch_of(cur);
             const size_t b = plane(nlev) * sizeof(double);
-            gx[nlev].alloc(b); gy[nlev].alloc(b); hE[nlev].alloc(b); hS[nlev].alloc(b); s[nlev].alloc(b); sd[nlev].alloc(b);
+            gx[nlev].alloc(b); gy[nlev].alloc(b); hE[nlev].alloc(b); hS[nlev].alloc(b); sc[nlev].alloc(b);
             lev[nlev] = Level{cur, cur, pitch[nlev], gx[nlev].as<double>(), gy[nlev].as<double>(), hE[nlev].as<double>(),
-                              hS[nlev].as<double>(), s[nlev].as<double>(), sd[nlev].as<double>()};
+                              hS[nlev].as<double>(), sc[nlev].as<float2>()};
             ++nlev;
             if (cur <= COARSEST_MAX) break;
             if (nlev >= MAX_LEVELS) throw StatusFail{PDN_E_ARG, "mesh too large for MAX_LEVELS"};
@@ -273,8 +273,8 @@ struct Hierarchy {
         L.run(KC_SMALL, 0, [&] { k_import_planes<<<cdiv(plane(0), 256), 256, 0, L.s>>>(gx_src, gy_src, n, pitch[0], gx[0].as<double>(), gy[0].as<double>(), fl); });
         for (int l = 0; l < nlev; ++l) {
             const unsigned g = cdiv(plane(l), 256);
-            L.run(KC_SMALL, 0, [&] { k_scale_nodes<<<g, 256, 0, L.s>>>(ny[l], nx[l], pitch[l], gx[l].as<double>(), gy[l].as<double>(), s[l].as<double>(), sd[l].as<double>(), l == 0 ? fl + 1 : nullptr); });
-            L.run(KC_SMALL, 0, [&] { k_scale_edges<<<g, 256, 0, L.s>>>(ny[l], nx[l], pitch[l], gx[l].as<double>(), gy[l].as<double>(), s[l].as<double>(), hE[l].as<double>(), hS[l].as<double>()); });
+            L.run(KC_SMALL, 0, [&] { k_scale_nodes<<<g, 256, 0, L.s>>>(ny[l], nx[l], pitch[l], gx[l].as<double>(), gy[l].as<double>(), sc[l].as<float2>(), l == 0 ? fl + 1 : nullptr); });
+            L.run(KC_SMALL, 0, [&] { k_scale_edges<<<g, 256, 0, L.s>>>(ny[l], nx[l], pitch[l], gx[l].as<double>(), gy[l].as<double>(), sc[l].as<float2>(), hE[l].as<double>(), hS[l].as<double>()); });
             if (l + 1 < nlev)
                 L.run(KC_SMALL, 0, [&] { k_coarsen<<<cdiv(plane(l + 1), 256), 256, 0, L.s>>>(ny[l], nx[l], pitch[l], gx[l].as<double>(), gy[l].as<double>(), ny[l + 1], nx[l + 1], pitch[l + 1], gx[l + 1].as<double>(), gy[l + 1].as<double>()); });
         }
@@ -384,14 +384,14 @@ void launch_down3(Launcher& L, int cls, double bytes, const Level& lv, const Smo
     constexpr int H = halo_of(NU), IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
     const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
     dim3 grid(tx, ty, cdiv(B, G));
-    constexpr size_t base = 4 * T3_TILE_BYTES + sizeof(Exch<T3_W>) + 128;
+    constexpr size_t base = 2 * T3_TILE_BYTES + T3_SC_BYTES + sizeof(Exch<T3_W>);
     static bool attr_done = false;
     if (!attr_done) {
-        CK(cudaFuncSetAttribute(k_down3<T3_R, T3_W, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(base + T3_TILE_BYTES)));
+        CK(cudaFuncSetAttribute(k_down3<T3_R, T3_W, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(base + 2 * T3_TILE_BYTES)));
         CK(cudaFuncSetAttribute(k_down3<T3_R, T3_W, NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)base));
         attr_done = true;
     }
-    if (m_q) L.run(cls, bytes, [&] { k_down3<T3_R, T3_W, NU, true><<<grid, T3_THREADS, base + T3_TILE_BYTES, L.s>>>(m_r, *m_q, lv, sm.cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G); });
+    if (m_q) L.run(cls, bytes, [&] { k_down3<T3_R, T3_W, NU, true><<<grid, T3_THREADS, base + 2 * T3_TILE_BYTES, L.s>>>(m_r, *m_q, lv, sm.cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G); });
     else L.run(cls, bytes, [&] { k_down3<T3_R, T3_W, NU, false><<<grid, T3_THREADS, base, L.s>>>(m_r, m_r, lv, sm.cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G); });
 }
 
@@ -401,7 +401,7 @@ void launch_up3(Launcher& L, int cls, double bytes, const Level& lv, const Smoot
     constexpr int H = halo_of(NU), IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
     const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
     dim3 grid(tx, ty, cdiv(B, G));
-    constexpr size_t smem = 5 * T3_TILE_BYTES + (size_t)(T3_EH / 2) * T3_ECW * sizeof(double) + sizeof(Exch<T3_W>) + 128;
+    constexpr size_t smem = 4 * T3_TILE_BYTES + (size_t)2 * (T3_EH / 2) * T3_ECW * sizeof(double) + T3_SC_BYTES + sizeof(Exch<T3_W>);
     static bool attr_done = false;
     if (!attr_done) {
         CK(cudaFuncSetAttribute(k_up3<T3_R, T3_W, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -417,7 +417,7 @@ void launch_pq3(Launcher& L, double bytes, const Level& lv, const Smoother& sm, 
     constexpr int H = 2, IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
     const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
     dim3 grid(tx, ty, cdiv(B, G));
-    constexpr size_t smem = 3 * T3_TILE_BYTES + sizeof(Exch<T3_W>) + 128;
+    constexpr size_t smem = 4 * T3_TILE_BYTES + sizeof(Exch<T3_W>);
     static bool attr_done = false;
     if (!attr_done) {
         CK(cudaFuncSetAttribute(k_pq3<T3_R, T3_W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

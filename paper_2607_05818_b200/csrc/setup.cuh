@@ -27,10 +27,10 @@ __global__ void k_import_planes(const double* __restrict__ gx_in, const double* 
     gy[i] = b;
 }
 
-// s = 1/sqrt(d), sd = sqrt(d), d = sum of incident conductances (both 0 if the node is isolated;
-// flagged on the finest level).
+// sc = (s, sd) = (1/sqrt(d), sqrt(d)) in FP32, d = sum of incident conductances ((0,0) if the node is
+// isolated; flagged on the finest level).
 __global__ void k_scale_nodes(int ny, int nx, int pitch, const double* __restrict__ gx, const double* __restrict__ gy,
-                              double* __restrict__ s, double* __restrict__ sd, int* __restrict__ isolated) {
+                              float2* __restrict__ sc, int* __restrict__ isolated) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= ny * pitch) return;
     const int y = i / pitch, x = i % pitch;
@@ -42,23 +42,23 @@ __global__ void k_scale_nodes(int ny, int nx, int pitch, const double* __restric
     }
     if (d > 0.0) {
         const double r = sqrt(d);
-        sd[i] = r;
-        s[i] = 1.0 / r;
+        sc[i] = make_float2((float)(1.0 / r), (float)r);
     } else {
-        sd[i] = 0.0;
-        s[i] = 0.0;
+        sc[i] = make_float2(0.f, 0.f);
         if (isolated && x < nx) atomicExch(isolated, 1);
     }
 }
 
-// hE = gx s s_east, hS = gy s s_south  (symmetric scaling; zero where the segment is absent).
+// hE = gx s s_east, hS = gy s s_south  (symmetric scaling with the FP32-rounded s, products in FP64;
+// zero where the segment is absent).
 __global__ void k_scale_edges(int ny, int nx, int pitch, const double* __restrict__ gx, const double* __restrict__ gy,
-                              const double* __restrict__ s, double* __restrict__ hE, double* __restrict__ hS) {
+                              const float2* __restrict__ sc, double* __restrict__ hE, double* __restrict__ hS) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= ny * pitch) return;
     const int y = i / pitch, x = i % pitch;
-    hE[i] = (x + 1 < nx) ? gx[i] * s[i] * s[i + 1] : 0.0;
-    hS[i] = (x < nx && y + 1 < ny) ? gy[i] * s[i] * s[i + pitch] : 0.0;
+    const double s = (double)sc[i].x;
+    hE[i] = (x + 1 < nx) ? gx[i] * s * (double)sc[i + 1].x : 0.0;
+    hS[i] = (x < nx && y + 1 < ny) ? gy[i] * s * (double)sc[i + pitch].x : 0.0;
 }
 
 // Coarse planes (cny x cnx, cn = ceil(n/2)) from fine planes (ny x nx).

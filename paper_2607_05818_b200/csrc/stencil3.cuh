@@ -16,8 +16,13 @@
 //     zeros, and the coefficients there are zero, so the sweeps need no boundary cases;
 //   * global stores are 16-byte (both columns of a patch row), interior only.
 //
-// Arithmetic.  All sweeps act on the symmetrically scaled system (common.cuh: Level):
-//   y <- (1-w) y + w (r^ + sum_nb h_nb y_nb),   r^ = s r,   z = s y.
+// Arithmetic.  The V-cycle sweeps act on the symmetrically scaled system (common.cuh: Level):
+//   y <- (1-w) y + w (r^ + sum_nb h_nb y_nb),   r^ = s r,   z = s y,
+// with r^ and y of the patch in registers; k_pq3 (the CG operator apply) uses the raw conductances.
+//
+// What bounds these kernels (ncu, profiles/): the shared-memory data pipe (128 B/clk/SM), which TMA
+// fills, LDS/STS and the warp shuffles all share -- so every input value crosses it exactly twice
+// (TMA write, one LDS), nothing is re-read per sweep, and the per-sweep traffic is the patch perimeter.
 #pragma once
 #include "common.cuh"
 
@@ -28,6 +33,7 @@ constexpr int T3_EW = 64;
 // The coarse correction of a tile is 32 coarse columns starting at x0/2, which may be odd; TMA wants the
 // innermost box coordinate 16-byte aligned, so the box starts at the even column below and is 34 wide.
 constexpr int T3_ECW = 34;
+
 
 template <int R>
 struct Patch {  // scaled coefficients of a 2 x R patch
@@ -55,10 +61,12 @@ __device__ __forceinline__ void exch_clear(Exch<W>& x) {
     }
 }
 
-// Coefficients of this thread's patch (zeros outside the mesh) and its slots of the s / sd tiles.
+// Coefficients of this thread's patch (zeros outside the mesh) and its slots of the scaling tile
+// sc[row][lane] = (s, sd) of column 0, (s, sd) of column 1.
 template <int R>
-__device__ __forceinline__ void patch_init(Patch<R>& c, const Level& L, int gx, int gy0, double* sS, double* sSD,
-                                           int slot0) {
+__device__ __forceinline__ void patch_init(Patch<R>& c, const double* __restrict__ pE, const double* __restrict__ pS,
+                                           const float2* __restrict__ psc, const Level& L, int gx, int gy0,
+                                           float4* sc_slot) {
     const bool xin = gx >= 0 && gx < L.pitch;  // gx is even, pitch is even: both columns are addressable
 #pragma unroll
     for (int i = 0; i < R; ++i) {
@@ -66,46 +74,67 @@ __device__ __forceinline__ void patch_init(Patch<R>& c, const Level& L, int gx, 
         const bool in = xin && gy >= 0 && gy < L.ny;
         const size_t gi = (size_t)gy * L.pitch + gx;
         const double2 z2 = make_double2(0.0, 0.0);
-        const double2 e = in ? ldg2(L.hE + gi) : z2;
-        const double2 s = in ? ldg2(L.hS + gi) : z2;
+        const double2 e = in ? ldg2(pE + gi) : z2;
+        const double2 s = in ? ldg2(pS + gi) : z2;
         c.hE0[i] = e.x; c.hE1[i] = e.y;
         c.hS0[i] = s.x; c.hS1[i] = s.y;
-        c.hW0[i] = (in && gx > 0) ? __ldg(L.hE + gi - 1) : 0.0;
-        if (sS) st2(sS + slot0 + i * T3_EW, in ? ldg2(L.s + gi) : z2);
-        st2(sSD + slot0 + i * T3_EW, in ? ldg2(L.sd + gi) : z2);
+        c.hW0[i] = (in && gx > 0) ? __ldg(pE + gi - 1) : 0.0;
+        if (psc) sc_slot[i * 32] = in ? __ldg(reinterpret_cast<const float4*>(psc + gi)) : make_float4(0.f, 0.f, 0.f, 0.f);
     }
     const int gyn = gy0 - 1;
-    const double2 nn = (xin && gyn >= 0 && gyn < L.ny) ? ldg2(L.hS + (size_t)gyn * L.pitch + gx) : make_double2(0.0, 0.0);
+    const double2 nn = (xin && gyn >= 0 && gyn < L.ny) ? ldg2(pS + (size_t)gyn * L.pitch + gx) : make_double2(0.0, 0.0);
     c.hN0 = nn.x; c.hN1 = nn.y;
 }
 
-// t += sum over the four neighbours of h_nb * y_nb  (t comes in holding the additive term).
-// One barrier; `cur` flips.
+// Publish the patch's first and last row, wait for everybody's, fetch the rows just above / below.
 template <int R, int W>
-__device__ __forceinline__ void nb_sum(Exch<W>& x, int& cur, const Patch<R>& c, int warp, int lane,
-                                       const double (&y0)[R], const double (&y1)[R], double (&t0)[R],
-                                       double (&t1)[R]) {
+__device__ __forceinline__ void exchange_rows(Exch<W>& x, int& cur, int warp, int lane, const double (&y0)[R],
+                                              const double (&y1)[R], double2& up, double2& dn) {
     x.top[cur][warp][lane] = make_double2(y0[0], y1[0]);
     x.bot[cur][warp + 1][lane] = make_double2(y0[R - 1], y1[R - 1]);
     __syncthreads();
-    const double2 up = x.bot[cur][warp][lane];
-    const double2 dn = x.top[cur][warp + 1][lane];
+    up = x.bot[cur][warp][lane];
+    dn = x.top[cur][warp + 1][lane];
     cur ^= 1;
+}
+
+// t = add + sum over the four neighbours of h_nb * y_nb for row i of the patch (old values: pu = row above).
+template <int R>
+__device__ __forceinline__ void row_sum(const Patch<R>& c, int i, const double (&y0)[R], const double (&y1)[R],
+                                        double pu0, double pu1, const double2& dn, double add0, double add1,
+                                        double& t0, double& t1) {
+    const double yl = __shfl_up_sync(FULL, y1[i], 1);    // right column of the lane to the left
+    const double yr = __shfl_down_sync(FULL, y0[i], 1);  // left column of the lane to the right
+    const double d0 = i == R - 1 ? dn.x : y0[i == R - 1 ? i : i + 1];
+    const double d1 = i == R - 1 ? dn.y : y1[i == R - 1 ? i : i + 1];
+    const double n0 = i == 0 ? c.hN0 : c.hS0[i == 0 ? 0 : i - 1], n1 = i == 0 ? c.hN1 : c.hS1[i == 0 ? 0 : i - 1];
+    double a = fma(c.hE0[i], y1[i], add0);
+    a = fma(c.hW0[i], yl, a);
+    a = fma(c.hS0[i], d0, a);
+    t0 = fma(n0, pu0, a);
+    double b = fma(c.hE1[i], yr, add1);
+    b = fma(c.hE0[i], y0[i], b);
+    b = fma(c.hS1[i], d1, b);
+    t1 = fma(n1, pu1, b);
+}
+
+// One Richardson step  y <- (1-w) y + w (r^ + N y)  on the patch, in place (rows are updated top to
+// bottom; the old value of the row above is carried in two registers).  One barrier.
+template <int R, int W>
+__device__ __forceinline__ void smooth_step(Exch<W>& x, int& cur, const Patch<R>& c, int warp, int lane,
+                                            double (&y0)[R], double (&y1)[R], const double (&rh0)[R],
+                                            const double (&rh1)[R], double w) {
+    double2 up, dn;
+    exchange_rows<R, W>(x, cur, warp, lane, y0, y1, up, dn);
+    const double a = 1.0 - w;
+    double pu0 = up.x, pu1 = up.y;
 #pragma unroll
     for (int i = 0; i < R; ++i) {
-        const double yl = __shfl_up_sync(FULL, y1[i], 1);    // right column of the lane to the left
-        const double yr = __shfl_down_sync(FULL, y0[i], 1);  // left column of the lane to the right
-        const double u0 = i == 0 ? up.x : y0[i - 1], u1 = i == 0 ? up.y : y1[i - 1];
-        const double d0 = i == R - 1 ? dn.x : y0[i + 1], d1 = i == R - 1 ? dn.y : y1[i + 1];
-        const double n0 = i == 0 ? c.hN0 : c.hS0[i - 1], n1 = i == 0 ? c.hN1 : c.hS1[i - 1];
-        double a = fma(c.hE0[i], y1[i], t0[i]);
-        a = fma(c.hW0[i], yl, a);
-        a = fma(c.hS0[i], d0, a);
-        t0[i] = fma(n0, u0, a);
-        double b = fma(c.hE1[i], yr, t1[i]);
-        b = fma(c.hE0[i], y0[i], b);
-        b = fma(c.hS1[i], d1, b);
-        t1[i] = fma(n1, u1, b);
+        double t0, t1;
+        row_sum<R>(c, i, y0, y1, pu0, pu1, dn, rh0[i], rh1[i], t0, t1);
+        pu0 = y0[i]; pu1 = y1[i];
+        y0[i] = fma(w, t0, a * y0[i]);
+        y1[i] = fma(w, t1, a * y1[i]);
     }
 }
 
@@ -120,11 +149,24 @@ struct Geom {
 
 __host__ __device__ constexpr int halo_of(int nu) { return (nu + 1) & ~1; }
 
+// bit i: row i of the patch is an interior row of the tile and inside the mesh (columns too)
+template <int R, int H, int IW, int IH>
+__device__ __forceinline__ unsigned interior_mask(const Level& L, int lane, int warp, int gx, int gy0) {
+    const bool xint = 2 * lane >= H && 2 * lane < H + IW && gx < L.nx;
+    unsigned m = 0;
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+        const int ey = R * warp + i;
+        if (xint && ey >= H && ey < H + IH && gy0 + i < L.ny) m |= 1u << i;
+    }
+    return m;
+}
+
 // ---------------------------------------------------------------------------------------------
 // Down stage of the V-cycle on one level (fused with the CG residual update on level 0):
 //   [r = r_in - alpha q ; rr += r.r]   y = S_nu(0, r^)   rc = R sd (r^ - A^ y)
 // y (the scaled iterate) is written to y_out for the up stage; R sums 2x2 aggregates.
-// grid = (tiles_x, tiles_y, ceil(B / G)); the block loops over G right-hand sides.
+// grid = (tiles_x, tiles_y, ceil(B / G)); the block loops over G right-hand sides, two TMA stages.
 template <int R, int W, int NU, bool FUSED>
 __global__ void __launch_bounds__(32 * W, 1)
 k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensorMap tm_q, Level L, ChebR ch,
@@ -133,57 +175,50 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
     constexpr int H = halo_of(NU);
     using Gm = Geom<R, W, H>;
     extern __shared__ __align__(128) double smem_dyn[];
-    double* rbuf = smem_dyn;              // 2 stages
-    double* qbuf = rbuf + 2 * Gm::TILE;             // 1 stage (consumed at the start of an iteration)
-    double* sS = qbuf + (FUSED ? Gm::TILE : 0);
-    double* sSD = sS + Gm::TILE;
-    Exch<W>& x = *reinterpret_cast<Exch<W>*>(sSD + Gm::TILE);
-    __shared__ uint64_t mbar[3];
+    double* rbuf = smem_dyn;                                   // 2 stages
+    double* qbuf = rbuf + 2 * Gm::TILE;                        // 2 stages (FUSED only)
+    float4* sc = reinterpret_cast<float4*>(qbuf + (FUSED ? 2 * Gm::TILE : 0));
+    Exch<W>& x = *reinterpret_cast<Exch<W>*>(sc + Gm::EH * 32);
+    __shared__ uint64_t mbar[2];
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int x0 = blockIdx.x * Gm::IW - H, y0 = blockIdx.y * Gm::IH - H;
     const int gx = x0 + 2 * lane, gy0 = y0 + R * warp;
     const int slot0 = (R * warp) * T3_EW + 2 * lane;
+    float4* sc_slot = sc + (R * warp) * 32 + lane;
     Patch<R> c;
-    patch_init<R>(c, L, gx, gy0, sS, sSD, slot0);
+    patch_init<R>(c, L.hE, L.hS, L.sc, L, gx, gy0, sc_slot);
     exch_clear<R, W>(x);
-    const bool xint = 2 * lane >= H && 2 * lane < H + Gm::IW && gx < L.nx;
-    unsigned interior = 0;  // bit i: row i of the patch is an interior row of the tile and inside the mesh
-#pragma unroll
-    for (int i = 0; i < R; ++i) {
-        const int ey = R * warp + i;
-        if (xint && ey >= H && ey < H + Gm::IH && gy0 + i < L.ny) interior |= 1u << i;
-    }
+    const unsigned interior = interior_mask<R, H, Gm::IW, Gm::IH>(L, lane, warp, gx, gy0);
     const size_t plane = (size_t)L.ny * L.pitch, cplane = (size_t)cny * cpitch;
     const size_t goff = (size_t)gy0 * L.pitch + gx;
     const int b0 = blockIdx.z * G, nb = min(G, B - b0);
     if (threadIdx.x == 0) {
-        mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); mbar_init(&mbar[2], 1);
+        mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1);
         mbar_fence_init();
     }
     __syncthreads();
     auto fetch = [&](int j) {  // thread 0 only
-        mbar_expect_tx(&mbar[j & 1], Gm::TILE_BYTES);
-        tma_load_3d(rbuf + (j & 1) * Gm::TILE, &tm_r, x0, y0, b0 + j, &mbar[j & 1]);
-        if (FUSED) {
-            mbar_expect_tx(&mbar[2], Gm::TILE_BYTES);
-            tma_load_3d(qbuf, &tm_q, x0, y0, b0 + j, &mbar[2]);
-        }
+        const int st = j & 1;
+        mbar_expect_tx(&mbar[st], (FUSED ? 2 : 1) * Gm::TILE_BYTES);
+        tma_load_3d(rbuf + st * Gm::TILE, &tm_r, x0, y0, b0 + j, &mbar[st]);
+        if (FUSED) tma_load_3d(qbuf + st * Gm::TILE, &tm_q, x0, y0, b0 + j, &mbar[st]);
     };
-    if (threadIdx.x == 0) fetch(0);
+    if (threadIdx.x == 0) {
+        fetch(0);
+        if (nb > 1) fetch(1);
+    }
     int cur = 0;
     for (int j = 0; j < nb; ++j) {
-        const int b = b0 + j;
-        double* rs = rbuf + (j & 1) * Gm::TILE + slot0;
-        mbar_wait(&mbar[j & 1], (j >> 1) & 1);
-        if (FUSED) mbar_wait(&mbar[2], j & 1);
+        const int b = b0 + j, st = j & 1;
+        mbar_wait(&mbar[st], (j >> 1) & 1);
         const double al = FUSED ? alpha[b] : 0.0;
-        double y0r[R], y1r[R], rr = 0.0;
+        double y0r[R], y1r[R], rh0[R], rh1[R], rr = 0.0;
 #pragma unroll
         for (int i = 0; i < R; ++i) {
-            double2 r = ld2(rs + i * T3_EW);
+            double2 r = ld2(rbuf + st * Gm::TILE + slot0 + i * T3_EW);
             if (FUSED) {
-                const double2 q = ld2(qbuf + slot0 + i * T3_EW);
+                const double2 q = ld2(qbuf + st * Gm::TILE + slot0 + i * T3_EW);
                 r.x = fma(-al, q.x, r.x);
                 r.y = fma(-al, q.y, r.y);
                 if ((interior >> i) & 1) {
@@ -192,45 +227,35 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
                     rr = fma(r.y, r.y, rr);
                 }
             }
-            const double2 s = ld2(sS + slot0 + i * T3_EW);
-            r.x *= s.x; r.y *= s.y;
-            st2(rs + i * T3_EW, r);  // r^ stays in this thread's own slots of the stage buffer
-            y0r[i] = ch.w[0] * r.x;
-            y1r[i] = ch.w[0] * r.y;
+            const float4 s4 = sc_slot[i * 32];
+            rh0[i] = (double)s4.x * r.x;
+            rh1[i] = (double)s4.z * r.y;
+            y0r[i] = ch.w[0] * rh0[i];
+            y1r[i] = ch.w[0] * rh1[i];
         }
-        fence_proxy_async();  // order these generic-proxy writes before the TMA write that reuses the stage
-        bool fetched = false;
-        auto after_first_barrier = [&] {
-            if (!fetched && threadIdx.x == 0 && j + 1 < nb) fetch(j + 1);
-            fetched = true;
-        };
+        // every sweep starts with a barrier; after the first one of this iteration all threads have
+        // consumed the stage, so thread 0 may refill it with right-hand side j+2
 #pragma unroll
         for (int k = 1; k < NU; ++k) {
-            double t0[R], t1[R];
-#pragma unroll
-            for (int i = 0; i < R; ++i) { const double2 r = ld2(rs + i * T3_EW); t0[i] = r.x; t1[i] = r.y; }
-            nb_sum<R, W>(x, cur, c, warp, lane, y0r, y1r, t0, t1);
-            after_first_barrier();
-            const double w = ch.w[k], a = 1.0 - w;
-#pragma unroll
-            for (int i = 0; i < R; ++i) {
-                y0r[i] = fma(w, t0[i], a * y0r[i]);
-                y1r[i] = fma(w, t1[i], a * y1r[i]);
-            }
+            smooth_step<R, W>(x, cur, c, warp, lane, y0r, y1r, rh0, rh1, ch.w[k]);
+            if (k == 1 && threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
         }
-        double t0[R], t1[R];
-#pragma unroll
-        for (int i = 0; i < R; ++i) { const double2 r = ld2(rs + i * T3_EW); t0[i] = r.x; t1[i] = r.y; }
-        nb_sum<R, W>(x, cur, c, warp, lane, y0r, y1r, t0, t1);
-        after_first_barrier();
+        double2 up, dn;
+        exchange_rows<R, W>(x, cur, warp, lane, y0r, y1r, up, dn);
+        if (NU == 1 && threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
         // residual of the unscaled system at the patch nodes, summed over 2x2 aggregates
+        double pu0 = up.x, pu1 = up.y;
 #pragma unroll
         for (int i = 0; i < R; i += 2) {
-            const double2 sda = ld2(sSD + slot0 + i * T3_EW), sdb = ld2(sSD + slot0 + (i + 1) * T3_EW);
-            double v = sda.x * (t0[i] - y0r[i]);
-            v = fma(sda.y, t1[i] - y1r[i], v);
-            v = fma(sdb.x, t0[i + 1] - y0r[i + 1], v);
-            v = fma(sdb.y, t1[i + 1] - y1r[i + 1], v);
+            double ta0, ta1, tb0, tb1;
+            row_sum<R>(c, i, y0r, y1r, pu0, pu1, dn, rh0[i], rh1[i], ta0, ta1);
+            row_sum<R>(c, i + 1, y0r, y1r, y0r[i], y1r[i], dn, rh0[i + 1], rh1[i + 1], tb0, tb1);
+            pu0 = y0r[i + 1]; pu1 = y1r[i + 1];
+            const float4 sa = sc_slot[i * 32], sb = sc_slot[(i + 1) * 32];
+            double v = (double)sa.y * (ta0 - y0r[i]);
+            v = fma((double)sa.w, ta1 - y1r[i], v);
+            v = fma((double)sb.y, tb0 - y0r[i + 1], v);
+            v = fma((double)sb.w, tb1 - y1r[i + 1], v);
             if ((interior >> i) & 1) {  // rows i and i+1 are interior together (H, R, y0 even)
                 st2(y_out + b * plane + goff + (size_t)i * L.pitch, make_double2(y0r[i], y1r[i]));
                 if ((interior >> (i + 1)) & 1)
@@ -256,90 +281,74 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
     constexpr int H = halo_of(NU);
     using Gm = Geom<R, W, H>;
     extern __shared__ __align__(128) double smem_dyn[];
-    double* rbuf = smem_dyn;   // 2 stages
-    double* ybuf = rbuf + 2 * Gm::TILE;  // 1 stage
-    double* ebuf = ybuf + Gm::TILE;      // 1 stage, T3_ECW x EH/2
-    double* sS = ebuf + Gm::ETILE;
-    double* sSD = sS + Gm::TILE;
-    Exch<W>& x = *reinterpret_cast<Exch<W>*>(sSD + Gm::TILE);
-    __shared__ uint64_t mbar[3];
+    double* rbuf = smem_dyn;             // 2 stages each
+    double* ybuf = rbuf + 2 * Gm::TILE;
+    double* ebuf = ybuf + 2 * Gm::TILE;  // T3_ECW x EH/2 per stage
+    float4* sc = reinterpret_cast<float4*>(ebuf + 2 * Gm::ETILE);
+    Exch<W>& x = *reinterpret_cast<Exch<W>*>(sc + Gm::EH * 32);
+    __shared__ uint64_t mbar[2];
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int x0 = blockIdx.x * Gm::IW - H, y0 = blockIdx.y * Gm::IH - H;
     const int gx = x0 + 2 * lane, gy0 = y0 + R * warp;
     const int slot0 = (R * warp) * T3_EW + 2 * lane;
+    float4* sc_slot = sc + (R * warp) * 32 + lane;
     Patch<R> c;
-    patch_init<R>(c, L, gx, gy0, sS, sSD, slot0);
+    patch_init<R>(c, L.hE, L.hS, L.sc, L, gx, gy0, sc_slot);
     exch_clear<R, W>(x);
-    const bool xint = 2 * lane >= H && 2 * lane < H + Gm::IW && gx < L.nx;
-    unsigned interior = 0;
-#pragma unroll
-    for (int i = 0; i < R; ++i) {
-        const int ey = R * warp + i;
-        if (xint && ey >= H && ey < H + Gm::IH && gy0 + i < L.ny) interior |= 1u << i;
-    }
+    const unsigned interior = interior_mask<R, H, Gm::IW, Gm::IH>(L, lane, warp, gx, gy0);
     const size_t plane = (size_t)L.ny * L.pitch;
     const size_t goff = (size_t)gy0 * L.pitch + gx;
     const int b0 = blockIdx.z * G, nb = min(G, B - b0);
     const int cx0 = (x0 >> 1) & ~1;                 // even coarse column at or below x0/2 (x0 is even)
     const int eslot = (x0 >> 1) - cx0 + lane;       // this lane's coarse column inside the box
     if (threadIdx.x == 0) {
-        mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); mbar_init(&mbar[2], 1);
+        mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1);
         mbar_fence_init();
     }
     __syncthreads();
     auto fetch = [&](int j) {  // thread 0 only
-        mbar_expect_tx(&mbar[j & 1], Gm::TILE_BYTES);
-        tma_load_3d(rbuf + (j & 1) * Gm::TILE, &tm_r, x0, y0, b0 + j, &mbar[j & 1]);
-        mbar_expect_tx(&mbar[2], Gm::TILE_BYTES + Gm::ETILE_BYTES);
-        tma_load_3d(ybuf, &tm_y, x0, y0, b0 + j, &mbar[2]);
-        tma_load_3d(ebuf, &tm_e, cx0, y0 / 2, b0 + j, &mbar[2]);
+        const int st = j & 1;
+        mbar_expect_tx(&mbar[st], 2 * Gm::TILE_BYTES + Gm::ETILE_BYTES);
+        tma_load_3d(rbuf + st * Gm::TILE, &tm_r, x0, y0, b0 + j, &mbar[st]);
+        tma_load_3d(ybuf + st * Gm::TILE, &tm_y, x0, y0, b0 + j, &mbar[st]);
+        tma_load_3d(ebuf + st * Gm::ETILE, &tm_e, cx0, y0 / 2, b0 + j, &mbar[st]);
     };
-    if (threadIdx.x == 0) fetch(0);
+    if (threadIdx.x == 0) {
+        fetch(0);
+        if (nb > 1) fetch(1);
+    }
     int cur = 0;
     for (int j = 0; j < nb; ++j) {
-        const int b = b0 + j;
-        double* rs = rbuf + (j & 1) * Gm::TILE + slot0;
-        mbar_wait(&mbar[j & 1], (j >> 1) & 1);
-        mbar_wait(&mbar[2], j & 1);
-        double y0r[R], y1r[R];
+        const int b = b0 + j, st = j & 1;
+        mbar_wait(&mbar[st], (j >> 1) & 1);
+        double y0r[R], y1r[R], rh0[R], rh1[R];
 #pragma unroll
         for (int i = 0; i < R; ++i) {
-            double2 r = ld2(rs + i * T3_EW);
-            const double2 s = ld2(sS + slot0 + i * T3_EW);
-            r.x *= s.x; r.y *= s.y;
-            st2(rs + i * T3_EW, r);
-            const double2 yin = ld2(ybuf + slot0 + i * T3_EW);
-            const double2 sd = ld2(sSD + slot0 + i * T3_EW);
-            const double e = ebuf[((R * warp + i) >> 1) * T3_ECW + eslot];
-            y0r[i] = fma(sd.x, e, yin.x);
-            y1r[i] = fma(sd.y, e, yin.y);
+            const double2 r = ld2(rbuf + st * Gm::TILE + slot0 + i * T3_EW);
+            const double2 yin = ld2(ybuf + st * Gm::TILE + slot0 + i * T3_EW);
+            const double e = ebuf[st * Gm::ETILE + ((R * warp + i) >> 1) * T3_ECW + eslot];
+            const float4 s4 = sc_slot[i * 32];
+            rh0[i] = (double)s4.x * r.x;
+            rh1[i] = (double)s4.z * r.y;
+            y0r[i] = fma((double)s4.y, e, yin.x);
+            y1r[i] = fma((double)s4.w, e, yin.y);
         }
-        fence_proxy_async();
 #pragma unroll
         for (int k = 0; k < NU; ++k) {
-            double t0[R], t1[R];
-#pragma unroll
-            for (int i = 0; i < R; ++i) { const double2 r = ld2(rs + i * T3_EW); t0[i] = r.x; t1[i] = r.y; }
-            nb_sum<R, W>(x, cur, c, warp, lane, y0r, y1r, t0, t1);
-            if (k == 0 && threadIdx.x == 0 && j + 1 < nb) fetch(j + 1);
-            const double w = ch.w[NU - 1 - k], a = 1.0 - w;
-#pragma unroll
-            for (int i = 0; i < R; ++i) {
-                y0r[i] = fma(w, t0[i], a * y0r[i]);
-                y1r[i] = fma(w, t1[i], a * y1r[i]);
-            }
+            smooth_step<R, W>(x, cur, c, warp, lane, y0r, y1r, rh0, rh1, ch.w[NU - 1 - k]);
+            if (k == 0 && threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
         }
         double rz = 0.0;
 #pragma unroll
         for (int i = 0; i < R; ++i) {
             if ((interior >> i) & 1) {
-                const double2 s = ld2(sS + slot0 + i * T3_EW);
-                st2(z_out + b * plane + goff + (size_t)i * L.pitch, make_double2(s.x * y0r[i], s.y * y1r[i]));
-                if (DOT) {
-                    const double2 r = ld2(rs + i * T3_EW);  // r.z = (sd r^).(s y) = r^.y
-                    rz = fma(r.x, y0r[i], rz);
-                    rz = fma(r.y, y1r[i], rz);
+                const float4 s4 = sc_slot[i * 32];
+                st2(z_out + b * plane + goff + (size_t)i * L.pitch,
+                    make_double2((double)s4.x * y0r[i], (double)s4.z * y1r[i]));
+                if (DOT) {  // r.z = r.(s y) = (s r).y = r^.y
+                    rz = fma(rh0[i], y0r[i], rz);
+                    rz = fma(rh1[i], y1r[i], rz);
                 }
             }
         }
@@ -351,8 +360,9 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
 }
 
 // ---------------------------------------------------------------------------------------------
-// CG direction update fused with the operator apply (level 0):
-//   p = z + beta p_old ;  q = L p = sd (p^ - N p^), p^ = sd p ;  pq += p.q ;  sump += sum(p)
+// CG direction update fused with the operator apply (level 0), on the UNSCALED operator (this is the
+// matrix CG solves with, so it uses the raw conductances):
+//   p = z + beta p_old ;  q = L p = d p - sum_nb g_nb p_nb ;  pq += p.q ;  sump += sum(p)
 template <int R, int W>
 __global__ void __launch_bounds__(32 * W, 1)
 k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensorMap tm_p, Level L,
@@ -361,51 +371,55 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
     constexpr int H = 2;  // one ring is needed; two keep the 16-byte column pairs aligned
     using Gm = Geom<R, W, H>;
     extern __shared__ __align__(128) double smem_dyn[];
-    double* zbuf = smem_dyn;
-    double* pbuf = zbuf + Gm::TILE;
-    double* sSD = pbuf + Gm::TILE;
-    Exch<W>& x = *reinterpret_cast<Exch<W>*>(sSD + Gm::TILE);
-    __shared__ uint64_t mbar;
+    double* zbuf = smem_dyn;             // 2 stages each
+    double* pbuf = zbuf + 2 * Gm::TILE;
+    Exch<W>& x = *reinterpret_cast<Exch<W>*>(pbuf + 2 * Gm::TILE);
+    __shared__ uint64_t mbar[2];
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int x0 = blockIdx.x * Gm::IW - H, y0 = blockIdx.y * Gm::IH - H;
     const int gx = x0 + 2 * lane, gy0 = y0 + R * warp;
     const int slot0 = (R * warp) * T3_EW + 2 * lane;
     Patch<R> c;
-    patch_init<R>(c, L, gx, gy0, nullptr, sSD, slot0);
-    exch_clear<R, W>(x);
-    const bool xint = 2 * lane >= H && 2 * lane < H + Gm::IW && gx < L.nx;
-    unsigned interior = 0;
+    patch_init<R>(c, L.gx, L.gy, nullptr, L, gx, gy0, nullptr);
+    double d0[R], d1[R];  // diagonal = sum of the incident conductances
 #pragma unroll
     for (int i = 0; i < R; ++i) {
-        const int ey = R * warp + i;
-        if (xint && ey >= H && ey < H + Gm::IH && gy0 + i < L.ny) interior |= 1u << i;
+        const double n0 = i == 0 ? c.hN0 : c.hS0[i == 0 ? 0 : i - 1], n1 = i == 0 ? c.hN1 : c.hS1[i == 0 ? 0 : i - 1];
+        d0[i] = (c.hE0[i] + c.hW0[i]) + (c.hS0[i] + n0);
+        d1[i] = (c.hE1[i] + c.hE0[i]) + (c.hS1[i] + n1);
     }
+    exch_clear<R, W>(x);
+    const unsigned interior = interior_mask<R, H, Gm::IW, Gm::IH>(L, lane, warp, gx, gy0);
     const size_t plane = (size_t)L.ny * L.pitch;
     const size_t goff = (size_t)gy0 * L.pitch + gx;
     const int b0 = blockIdx.z * G, nb = min(G, B - b0);
     if (threadIdx.x == 0) {
-        mbar_init(&mbar, 1);
+        mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1);
         mbar_fence_init();
     }
     __syncthreads();
     auto fetch = [&](int j) {  // thread 0 only
-        mbar_expect_tx(&mbar, 2 * Gm::TILE_BYTES);
-        tma_load_3d(zbuf, &tm_z, x0, y0, b0 + j, &mbar);
-        tma_load_3d(pbuf, &tm_p, x0, y0, b0 + j, &mbar);
+        const int st = j & 1;
+        mbar_expect_tx(&mbar[st], 2 * Gm::TILE_BYTES);
+        tma_load_3d(zbuf + st * Gm::TILE, &tm_z, x0, y0, b0 + j, &mbar[st]);
+        tma_load_3d(pbuf + st * Gm::TILE, &tm_p, x0, y0, b0 + j, &mbar[st]);
     };
-    if (threadIdx.x == 0) fetch(0);
+    if (threadIdx.x == 0) {
+        fetch(0);
+        if (nb > 1) fetch(1);
+    }
     int cur = 0;
     for (int j = 0; j < nb; ++j) {
-        const int b = b0 + j;
-        mbar_wait(&mbar, j & 1);
+        const int b = b0 + j, st = j & 1;
+        mbar_wait(&mbar[st], (j >> 1) & 1);
         const double bt = beta[b];
-        double y0r[R], y1r[R], t0[R], t1[R], sump = 0.0, pq = 0.0;
+        double p0[R], p1[R], sump = 0.0, pq = 0.0;
 #pragma unroll
         for (int i = 0; i < R; ++i) {
-            double2 p = ld2(zbuf + slot0 + i * T3_EW);
+            double2 p = ld2(zbuf + st * Gm::TILE + slot0 + i * T3_EW);
             if (bt != 0.0) {  // beta = 0 on the first iteration: p_old is not initialised then
-                const double2 po = ld2(pbuf + slot0 + i * T3_EW);
+                const double2 po = ld2(pbuf + st * Gm::TILE + slot0 + i * T3_EW);
                 p.x = fma(bt, po.x, p.x);
                 p.y = fma(bt, po.y, p.y);
             }
@@ -413,22 +427,23 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
                 st2(p_new + b * plane + goff + (size_t)i * L.pitch, p);
                 sump += p.x + p.y;
             }
-            const double2 sd = ld2(sSD + slot0 + i * T3_EW);
-            y0r[i] = sd.x * p.x;
-            y1r[i] = sd.y * p.y;
-            t0[i] = 0.0;
-            t1[i] = 0.0;
+            p0[i] = p.x;
+            p1[i] = p.y;
         }
-        nb_sum<R, W>(x, cur, c, warp, lane, y0r, y1r, t0, t1);
-        if (threadIdx.x == 0 && j + 1 < nb) fetch(j + 1);
+        double2 up, dn;
+        exchange_rows<R, W>(x, cur, warp, lane, p0, p1, up, dn);
+        if (threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
+        double pu0 = up.x, pu1 = up.y;
 #pragma unroll
         for (int i = 0; i < R; ++i) {
+            double t0, t1;
+            row_sum<R>(c, i, p0, p1, pu0, pu1, dn, 0.0, 0.0, t0, t1);
+            pu0 = p0[i]; pu1 = p1[i];
             if ((interior >> i) & 1) {
-                const double2 sd = ld2(sSD + slot0 + i * T3_EW);
-                const double a0 = y0r[i] - t0[i], a1 = y1r[i] - t1[i];
-                st2(q + b * plane + goff + (size_t)i * L.pitch, make_double2(sd.x * a0, sd.y * a1));
-                pq = fma(y0r[i], a0, pq);  // p.q = p^.(p^ - N p^)
-                pq = fma(y1r[i], a1, pq);
+                const double q0 = fma(d0[i], p0[i], -t0), q1 = fma(d1[i], p1[i], -t1);
+                st2(q + b * plane + goff + (size_t)i * L.pitch, make_double2(q0, q1));
+                pq = fma(p0[i], q0, pq);
+                pq = fma(p1[i], q1, pq);
             }
         }
         pq = warp_sum(pq);
