@@ -229,7 +229,15 @@ CUtensorMap make_map(const void* base, int nx, int ny, int pitch, int B, int box
 #ifndef PDN_T3_W
 #define PDN_T3_W 16
 #endif
+#ifndef PDN_PQ_R
+#define PDN_PQ_R 8
+#endif
+#ifndef PDN_PQ_W
+#define PDN_PQ_W 8
+#endif
 constexpr int T3_R = PDN_T3_R, T3_W = PDN_T3_W, T3_EH = T3_R * T3_W, T3_THREADS = 32 * T3_W;
+constexpr int PQ_R = PDN_PQ_R, PQ_W = PDN_PQ_W;  // the operator apply has one sweep and no r^: fatter patches pay
+static_assert(PQ_R * PQ_W == T3_EH, "all level-0 kernels share the TMA box height");
 constexpr size_t T3_TILE_BYTES = (size_t)T3_EH * T3_EW * sizeof(double), T3_SC_BYTES = (size_t)T3_EH * 32 * sizeof(float4);
 
 inline int pitch_of(int nx) { return (nx + 1) & ~1; }
@@ -417,13 +425,13 @@ void launch_pq3(Launcher& L, double bytes, const Level& lv, const Smoother& sm, 
     constexpr int H = 2, IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
     const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
     dim3 grid(tx, ty, cdiv(B, G));
-    constexpr size_t smem = 4 * T3_TILE_BYTES + sizeof(Exch<T3_W>);
+    constexpr size_t smem = 4 * T3_TILE_BYTES + sizeof(Exch<PQ_W>);
     static bool attr_done = false;
     if (!attr_done) {
-        CK(cudaFuncSetAttribute(k_pq3<T3_R, T3_W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_pq3<PQ_R, PQ_W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_done = true;
     }
-    L.run(KC_PQ, bytes, [&] { k_pq3<T3_R, T3_W><<<grid, T3_THREADS, smem, L.s>>>(m_z, m_p, lv, beta, p_new, q, pq_acc, sump_acc, B, G); });
+    L.run(KC_PQ, bytes, [&] { k_pq3<PQ_R, PQ_W><<<grid, 32 * PQ_W, smem, L.s>>>(m_z, m_p, lv, beta, p_new, q, pq_acc, sump_acc, B, G); });
 }
 
 #define NU_DISPATCH(nu, CALL)                 \
@@ -775,7 +783,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         }
         Work W;
         if (H.nlev > 1) W.allocate(H, Bmax, qmax);
-        Smoother ch{make_cheb_roots(o.nu, 6.0), getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 8};
+        Smoother ch{make_cheb_roots(o.nu, 6.0), getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 16};
         const double rtol_term = std::max(o.rtol, std::min(1e-5, std::sqrt(o.rtol) / 3.0));
         float ms_up = 0.f;
         for (int t = 0; t < d && status == PDN_OK; ++t) {

@@ -86,56 +86,95 @@ __device__ __forceinline__ void patch_init(Patch<R>& c, const double* __restrict
     c.hN0 = nn.x; c.hN1 = nn.y;
 }
 
-// Publish the patch's first and last row, wait for everybody's, fetch the rows just above / below.
-template <int R, int W>
-__device__ __forceinline__ void exchange_rows(Exch<W>& x, int& cur, int warp, int lane, const double (&y0)[R],
-                                              const double (&y1)[R], double2& up, double2& dn) {
-    x.top[cur][warp][lane] = make_double2(y0[0], y1[0]);
-    x.bot[cur][warp + 1][lane] = make_double2(y0[R - 1], y1[R - 1]);
-    __syncthreads();
-    up = x.bot[cur][warp][lane];
-    dn = x.top[cur][warp + 1][lane];
-    cur ^= 1;
-}
+// Split-phase exchange of patch boundary rows between the warps of a block.  `publish` stores the
+// patch's first and last row and ARRIVES on an mbarrier; the rows that need nothing from other warps
+// are computed next; `collect` waits for everybody's arrival and fetches the rows just above / below.
+// Buffers alternate between sweeps, the mbarrier phase flips once per sweep.
+template <int W>
+struct Xchg {
+    Exch<W>* x;
+    uint64_t* bar;
+    int cur;        // buffer of the current sweep
+    uint32_t phase; // parity the next collect waits for
+    int warp, lane;
+    __device__ __forceinline__ void publish(double a0, double a1, double b0, double b1) {
+        x->top[cur][warp][lane] = make_double2(a0, a1);
+        x->bot[cur][warp + 1][lane] = make_double2(b0, b1);
+        mbar_arrive(bar);
+    }
+    __device__ __forceinline__ void collect(double2& up, double2& dn) {
+        mbar_wait(bar, phase);
+        up = x->bot[cur][warp][lane];
+        dn = x->top[cur][warp + 1][lane];
+        cur ^= 1;
+        phase ^= 1;
+    }
+};
 
-// t = add + sum over the four neighbours of h_nb * y_nb for row i of the patch (old values: pu = row above).
+// t = add + sum over the four neighbours of h_nb * y_nb for row i of the patch, whose own values are
+// (c0, c1), with the rows above (u0, u1) and below (d0, d1) given explicitly.
 template <int R>
-__device__ __forceinline__ void row_sum(const Patch<R>& c, int i, const double (&y0)[R], const double (&y1)[R],
-                                        double pu0, double pu1, const double2& dn, double add0, double add1,
-                                        double& t0, double& t1) {
-    const double yl = __shfl_up_sync(FULL, y1[i], 1);    // right column of the lane to the left
-    const double yr = __shfl_down_sync(FULL, y0[i], 1);  // left column of the lane to the right
-    const double d0 = i == R - 1 ? dn.x : y0[i == R - 1 ? i : i + 1];
-    const double d1 = i == R - 1 ? dn.y : y1[i == R - 1 ? i : i + 1];
+__device__ __forceinline__ void row_sum(const Patch<R>& c, int i, double c0, double c1, double u0, double u1,
+                                        double d0, double d1, double add0, double add1, double& t0, double& t1) {
+    const double yl = __shfl_up_sync(FULL, c1, 1);    // right column of the lane to the left
+    const double yr = __shfl_down_sync(FULL, c0, 1);  // left column of the lane to the right
     const double n0 = i == 0 ? c.hN0 : c.hS0[i == 0 ? 0 : i - 1], n1 = i == 0 ? c.hN1 : c.hS1[i == 0 ? 0 : i - 1];
-    double a = fma(c.hE0[i], y1[i], add0);
+    double a = fma(c.hE0[i], c1, add0);
     a = fma(c.hW0[i], yl, a);
     a = fma(c.hS0[i], d0, a);
-    t0 = fma(n0, pu0, a);
+    t0 = fma(n0, u0, a);
     double b = fma(c.hE1[i], yr, add1);
-    b = fma(c.hE0[i], y0[i], b);
+    b = fma(c.hE0[i], c0, b);
     b = fma(c.hS1[i], d1, b);
-    t1 = fma(n1, pu1, b);
+    t1 = fma(n1, u1, b);
 }
 
-// One Richardson step  y <- (1-w) y + w (r^ + N y)  on the patch, in place (rows are updated top to
-// bottom; the old value of the row above is carried in two registers).  One barrier.
+// One Richardson step  y <- (1-w) y + w (r^ + N y)  on the patch, in place.  Rows 1..R-2 need only this
+// thread's (and, by shuffle, this warp's) values: they are updated between publish and collect, top to
+// bottom, the old value of the row above carried in registers; rows 0 and R-1 follow the collect.
 template <int R, int W>
-__device__ __forceinline__ void smooth_step(Exch<W>& x, int& cur, const Patch<R>& c, int warp, int lane,
-                                            double (&y0)[R], double (&y1)[R], const double (&rh0)[R],
-                                            const double (&rh1)[R], double w) {
-    double2 up, dn;
-    exchange_rows<R, W>(x, cur, warp, lane, y0, y1, up, dn);
+__device__ __forceinline__ void smooth_step(Xchg<W>& xc, const Patch<R>& c, double (&y0)[R], double (&y1)[R],
+                                            const double (&rh0)[R], const double (&rh1)[R], double w) {
+    static_assert(R >= 2, "patch needs two rows");
+    xc.publish(y0[0], y1[0], y0[R - 1], y1[R - 1]);
     const double a = 1.0 - w;
-    double pu0 = up.x, pu1 = up.y;
+    const double f0 = y0[0], f1 = y1[0];          // old first row
+    const double s0 = y0[R > 2 ? 1 : 0], s1 = y1[R > 2 ? 1 : 0];  // old second row (below neighbour of row 0)
+    const double l0 = y0[R - 1], l1 = y1[R - 1];  // old last row
+    double pu0 = f0, pu1 = f1;
 #pragma unroll
-    for (int i = 0; i < R; ++i) {
+    for (int i = 1; i < R - 1; ++i) {
         double t0, t1;
-        row_sum<R>(c, i, y0, y1, pu0, pu1, dn, rh0[i], rh1[i], t0, t1);
+        row_sum<R>(c, i, y0[i], y1[i], pu0, pu1, y0[i + 1], y1[i + 1], rh0[i], rh1[i], t0, t1);
         pu0 = y0[i]; pu1 = y1[i];
         y0[i] = fma(w, t0, a * y0[i]);
         y1[i] = fma(w, t1, a * y1[i]);
     }
+    // pu = old row R-2 (or the old first row if R == 2)
+    double2 up, dn;
+    xc.collect(up, dn);
+    double t0, t1, v0, v1;
+    row_sum<R>(c, 0, f0, f1, up.x, up.y, R > 2 ? s0 : l0, R > 2 ? s1 : l1, rh0[0], rh1[0], t0, t1);
+    row_sum<R>(c, R - 1, l0, l1, pu0, pu1, dn.x, dn.y, rh0[R - 1], rh1[R - 1], v0, v1);
+    y0[0] = fma(w, t0, a * f0);
+    y1[0] = fma(w, t1, a * f1);
+    y0[R - 1] = fma(w, v0, a * l0);
+    y1[R - 1] = fma(w, v1, a * l1);
+}
+
+// t = add + N y for every row of the patch (y unchanged): the residual / operator-apply variant.
+template <int R, int W>
+__device__ __forceinline__ void apply_step(Xchg<W>& xc, const Patch<R>& c, const double (&y0)[R], const double (&y1)[R],
+                                           const double (&a0)[R], const double (&a1)[R], double (&t0)[R],
+                                           double (&t1)[R]) {
+    xc.publish(y0[0], y1[0], y0[R - 1], y1[R - 1]);
+#pragma unroll
+    for (int i = 1; i < R - 1; ++i)
+        row_sum<R>(c, i, y0[i], y1[i], y0[i - 1], y1[i - 1], y0[i + 1], y1[i + 1], a0[i], a1[i], t0[i], t1[i]);
+    double2 up, dn;
+    xc.collect(up, dn);
+    row_sum<R>(c, 0, y0[0], y1[0], up.x, up.y, y0[1], y1[1], a0[0], a1[0], t0[0], t1[0]);
+    row_sum<R>(c, R - 1, y0[R - 1], y1[R - 1], y0[R - 2], y1[R - 2], dn.x, dn.y, a0[R - 1], a1[R - 1], t0[R - 1], t1[R - 1]);
 }
 
 template <int R, int W, int H>
@@ -179,7 +218,7 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
     double* qbuf = rbuf + 2 * Gm::TILE;                        // 2 stages (FUSED only)
     float4* sc = reinterpret_cast<float4*>(qbuf + (FUSED ? 2 * Gm::TILE : 0));
     Exch<W>& x = *reinterpret_cast<Exch<W>*>(sc + Gm::EH * 32);
-    __shared__ uint64_t mbar[2];
+    __shared__ uint64_t mbar[3];  // two TMA stages + the row-exchange barrier
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int x0 = blockIdx.x * Gm::IW - H, y0 = blockIdx.y * Gm::IH - H;
@@ -194,7 +233,7 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
     const size_t goff = (size_t)gy0 * L.pitch + gx;
     const int b0 = blockIdx.z * G, nb = min(G, B - b0);
     if (threadIdx.x == 0) {
-        mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1);
+        mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); mbar_init(&mbar[2], 32 * W);
         mbar_fence_init();
     }
     __syncthreads();
@@ -208,7 +247,7 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
         fetch(0);
         if (nb > 1) fetch(1);
     }
-    int cur = 0;
+    Xchg<W> xc{&x, &mbar[2], 0, 0u, warp, lane};
     for (int j = 0; j < nb; ++j) {
         const int b = b0 + j, st = j & 1;
         mbar_wait(&mbar[st], (j >> 1) & 1);
@@ -233,29 +272,24 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
             y0r[i] = ch.w[0] * rh0[i];
             y1r[i] = ch.w[0] * rh1[i];
         }
-        // every sweep starts with a barrier; after the first one of this iteration all threads have
-        // consumed the stage, so thread 0 may refill it with right-hand side j+2
+        // once thread 0 is past the first row exchange of this iteration every thread has arrived there,
+        // i.e. has consumed the stage: thread 0 may refill it with right-hand side j+2
 #pragma unroll
         for (int k = 1; k < NU; ++k) {
-            smooth_step<R, W>(x, cur, c, warp, lane, y0r, y1r, rh0, rh1, ch.w[k]);
+            smooth_step<R, W>(xc, c, y0r, y1r, rh0, rh1, ch.w[k]);
             if (k == 1 && threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
         }
-        double2 up, dn;
-        exchange_rows<R, W>(x, cur, warp, lane, y0r, y1r, up, dn);
+        double t0[R], t1[R];
+        apply_step<R, W>(xc, c, y0r, y1r, rh0, rh1, t0, t1);
         if (NU == 1 && threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
         // residual of the unscaled system at the patch nodes, summed over 2x2 aggregates
-        double pu0 = up.x, pu1 = up.y;
 #pragma unroll
         for (int i = 0; i < R; i += 2) {
-            double ta0, ta1, tb0, tb1;
-            row_sum<R>(c, i, y0r, y1r, pu0, pu1, dn, rh0[i], rh1[i], ta0, ta1);
-            row_sum<R>(c, i + 1, y0r, y1r, y0r[i], y1r[i], dn, rh0[i + 1], rh1[i + 1], tb0, tb1);
-            pu0 = y0r[i + 1]; pu1 = y1r[i + 1];
             const float4 sa = sc_slot[i * 32], sb = sc_slot[(i + 1) * 32];
-            double v = (double)sa.y * (ta0 - y0r[i]);
-            v = fma((double)sa.w, ta1 - y1r[i], v);
-            v = fma((double)sb.y, tb0 - y0r[i + 1], v);
-            v = fma((double)sb.w, tb1 - y1r[i + 1], v);
+            double v = (double)sa.y * (t0[i] - y0r[i]);
+            v = fma((double)sa.w, t1[i] - y1r[i], v);
+            v = fma((double)sb.y, t0[i + 1] - y0r[i + 1], v);
+            v = fma((double)sb.w, t1[i + 1] - y1r[i + 1], v);
             if ((interior >> i) & 1) {  // rows i and i+1 are interior together (H, R, y0 even)
                 st2(y_out + b * plane + goff + (size_t)i * L.pitch, make_double2(y0r[i], y1r[i]));
                 if ((interior >> (i + 1)) & 1)
@@ -286,7 +320,7 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
     double* ebuf = ybuf + 2 * Gm::TILE;  // T3_ECW x EH/2 per stage
     float4* sc = reinterpret_cast<float4*>(ebuf + 2 * Gm::ETILE);
     Exch<W>& x = *reinterpret_cast<Exch<W>*>(sc + Gm::EH * 32);
-    __shared__ uint64_t mbar[2];
+    __shared__ uint64_t mbar[3];  // two TMA stages + the row-exchange barrier
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int x0 = blockIdx.x * Gm::IW - H, y0 = blockIdx.y * Gm::IH - H;
@@ -303,7 +337,7 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
     const int cx0 = (x0 >> 1) & ~1;                 // even coarse column at or below x0/2 (x0 is even)
     const int eslot = (x0 >> 1) - cx0 + lane;       // this lane's coarse column inside the box
     if (threadIdx.x == 0) {
-        mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1);
+        mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); mbar_init(&mbar[2], 32 * W);
         mbar_fence_init();
     }
     __syncthreads();
@@ -318,7 +352,7 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
         fetch(0);
         if (nb > 1) fetch(1);
     }
-    int cur = 0;
+    Xchg<W> xc{&x, &mbar[2], 0, 0u, warp, lane};
     for (int j = 0; j < nb; ++j) {
         const int b = b0 + j, st = j & 1;
         mbar_wait(&mbar[st], (j >> 1) & 1);
@@ -336,7 +370,7 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
         }
 #pragma unroll
         for (int k = 0; k < NU; ++k) {
-            smooth_step<R, W>(x, cur, c, warp, lane, y0r, y1r, rh0, rh1, ch.w[NU - 1 - k]);
+            smooth_step<R, W>(xc, c, y0r, y1r, rh0, rh1, ch.w[NU - 1 - k]);
             if (k == 0 && threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
         }
         double rz = 0.0;
@@ -374,7 +408,7 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
     double* zbuf = smem_dyn;             // 2 stages each
     double* pbuf = zbuf + 2 * Gm::TILE;
     Exch<W>& x = *reinterpret_cast<Exch<W>*>(pbuf + 2 * Gm::TILE);
-    __shared__ uint64_t mbar[2];
+    __shared__ uint64_t mbar[3];  // two TMA stages + the row-exchange barrier
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int x0 = blockIdx.x * Gm::IW - H, y0 = blockIdx.y * Gm::IH - H;
@@ -382,6 +416,7 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
     const int slot0 = (R * warp) * T3_EW + 2 * lane;
     Patch<R> c;
     patch_init<R>(c, L.gx, L.gy, nullptr, L, gx, gy0, nullptr);
+    const double zero[R] = {};
     double d0[R], d1[R];  // diagonal = sum of the incident conductances
 #pragma unroll
     for (int i = 0; i < R; ++i) {
@@ -395,7 +430,7 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
     const size_t goff = (size_t)gy0 * L.pitch + gx;
     const int b0 = blockIdx.z * G, nb = min(G, B - b0);
     if (threadIdx.x == 0) {
-        mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1);
+        mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); mbar_init(&mbar[2], 32 * W);
         mbar_fence_init();
     }
     __syncthreads();
@@ -409,7 +444,7 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
         fetch(0);
         if (nb > 1) fetch(1);
     }
-    int cur = 0;
+    Xchg<W> xc{&x, &mbar[2], 0, 0u, warp, lane};
     for (int j = 0; j < nb; ++j) {
         const int b = b0 + j, st = j & 1;
         mbar_wait(&mbar[st], (j >> 1) & 1);
@@ -430,17 +465,13 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
             p0[i] = p.x;
             p1[i] = p.y;
         }
-        double2 up, dn;
-        exchange_rows<R, W>(x, cur, warp, lane, p0, p1, up, dn);
+        double t0[R], t1[R];
+        apply_step<R, W>(xc, c, p0, p1, zero, zero, t0, t1);
         if (threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
-        double pu0 = up.x, pu1 = up.y;
 #pragma unroll
         for (int i = 0; i < R; ++i) {
-            double t0, t1;
-            row_sum<R>(c, i, p0, p1, pu0, pu1, dn, 0.0, 0.0, t0, t1);
-            pu0 = p0[i]; pu1 = p1[i];
             if ((interior >> i) & 1) {
-                const double q0 = fma(d0[i], p0[i], -t0), q1 = fma(d1[i], p1[i], -t1);
+                const double q0 = fma(d0[i], p0[i], -t0[i]), q1 = fma(d1[i], p1[i], -t1[i]);
                 st2(q + b * plane + goff + (size_t)i * L.pitch, make_double2(q0, q1));
                 pq = fma(p0[i], q0, pq);
                 pq = fma(p1[i], q1, pq);
