@@ -224,16 +224,16 @@ CUtensorMap make_map(const void* base, int nx, int ny, int pitch, int B, int box
 }
 
 #ifndef PDN_T3_R
-#define PDN_T3_R 4
+#define PDN_T3_R 6
 #endif
 #ifndef PDN_T3_W
-#define PDN_T3_W 16
+#define PDN_T3_W 12
 #endif
 #ifndef PDN_PQ_R
-#define PDN_PQ_R 8
+#define PDN_PQ_R (PDN_T3_R * 2)
 #endif
 #ifndef PDN_PQ_W
-#define PDN_PQ_W 8
+#define PDN_PQ_W (PDN_T3_W / 2)
 #endif
 constexpr int T3_R = PDN_T3_R, T3_W = PDN_T3_W, T3_EH = T3_R * T3_W, T3_THREADS = 32 * T3_W;
 constexpr int PQ_R = PDN_PQ_R, PQ_W = PDN_PQ_W;  // the operator apply has one sweep and no r^: fatter patches pay
@@ -409,7 +409,7 @@ void launch_up3(Launcher& L, int cls, double bytes, const Level& lv, const Smoot
     constexpr int H = halo_of(NU), IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
     const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
     dim3 grid(tx, ty, cdiv(B, G));
-    constexpr size_t smem = 4 * T3_TILE_BYTES + (size_t)2 * (T3_EH / 2) * T3_ECW * sizeof(double) + T3_SC_BYTES + sizeof(Exch<T3_W>);
+    constexpr size_t smem = 4 * T3_TILE_BYTES + (size_t)2 * Geom<T3_R, T3_W, 2>::ETILE_BYTES + T3_SC_BYTES + sizeof(Exch<T3_W>);
     static bool attr_done = false;
     if (!attr_done) {
         CK(cudaFuncSetAttribute(k_up3<T3_R, T3_W, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

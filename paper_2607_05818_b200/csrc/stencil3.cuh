@@ -180,8 +180,9 @@ __device__ __forceinline__ void apply_step(Xchg<W>& xc, const Patch<R>& c, const
 template <int R, int W, int H>
 struct Geom {
     static constexpr int EH = R * W, IW = T3_EW - 2 * H, IH = EH - 2 * H, TILE = EH * T3_EW, THREADS = 32 * W;
-    static constexpr int ETILE = (EH / 2) * T3_ECW;  // coarse-correction tile of the up stage
+    static constexpr int ETILE = ((EH / 2) * T3_ECW + 15) & ~15;  // coarse-correction tile of the up stage (128-byte multiple)
     static constexpr uint32_t TILE_BYTES = TILE * sizeof(double), ETILE_BYTES = ETILE * sizeof(double);
+    static constexpr uint32_t EBOX_BYTES = (EH / 2) * T3_ECW * sizeof(double);  // what the TMA box delivers
     static_assert(R % 2 == 0 && H % 2 == 0, "2x2 aggregates must not straddle patches");
     static_assert(IW > 0 && IH > 0, "halo too deep for the tile");
 };
@@ -343,7 +344,7 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
     __syncthreads();
     auto fetch = [&](int j) {  // thread 0 only
         const int st = j & 1;
-        mbar_expect_tx(&mbar[st], 2 * Gm::TILE_BYTES + Gm::ETILE_BYTES);
+        mbar_expect_tx(&mbar[st], 2 * Gm::TILE_BYTES + Gm::EBOX_BYTES);
         tma_load_3d(rbuf + st * Gm::TILE, &tm_r, x0, y0, b0 + j, &mbar[st]);
         tma_load_3d(ybuf + st * Gm::TILE, &tm_y, x0, y0, b0 + j, &mbar[st]);
         tma_load_3d(ebuf + st * Gm::ETILE, &tm_e, cx0, y0 / 2, b0 + j, &mbar[st]);
