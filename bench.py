@@ -52,7 +52,7 @@ class ClockSampler:
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                       "-lms", "100", "-i", str(gpu_index)], stdout=self.f, stderr=subprocess.DEVNULL)
+                                       "-lms", "500", "-i", str(gpu_index)], stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
 
@@ -235,10 +235,17 @@ def run_cuda(a):
     tot_ms = sum(cls_ms[k] for k in stencil_classes)
     tot_by = sum(cls_by[k] for k in stencil_classes)
     phase = tot_by / (tot_ms * 1e-3) / 1e9 if tot_ms > 0 else 0.0
+    # DRAM traffic of the dominant kernel from the committed ncu capture (profiles/ncu_traffic.csv: bytes per
+    # right-hand side of one launch), scaled to this run's average right-hand sides per launch
     traffic = None
-    tr_path = os.path.join(ROOT, "profiles", "ncu_traffic.json")     # dram bytes per launch from the ncu capture
-    if os.path.exists(tr_path):
-        traffic = json.load(open(tr_path)).get(f"cfg{cfg}", {}).get(dom)
+    tr_path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    if os.path.exists(tr_path) and cls_n[dom] > 0:
+        import csv
+        for row in csv.DictReader(open(tr_path)):
+            if int(row["cfg"]) == cfg and row["class"] == dom:
+                per_rhs_alg = float(row["algorithmic_bytes_per_launch"]) / float(row["rhs_in_launch"])
+                rhs_per_launch = (cls_by[dom] / cls_n[dom]) / per_rhs_alg
+                traffic = float(row["dram_bytes_per_rhs"]) * rhs_per_launch
 
     last = stats[-1]
     # parity of what the timed steps produced, against the oracle's stored values (tests/golden, written by

@@ -783,7 +783,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         }
         Work W;
         if (H.nlev > 1) W.allocate(H, Bmax, qmax);
-        Smoother ch{make_cheb_roots(o.nu, 6.0), getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 16};
+        Smoother ch{make_cheb_roots(o.nu, 6.0), getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 32};
         const double rtol_term = std::max(o.rtol, std::min(1e-5, std::sqrt(o.rtol) / 3.0));
         float ms_up = 0.f;
         for (int t = 0; t < d && status == PDN_OK; ++t) {
