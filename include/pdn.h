@@ -94,7 +94,7 @@ typedef struct {
 
 /* Options; pass NULL for the defaults.  Zero / negative fields mean "default". */
 typedef struct {
-    double rtol;        /* port solves stop at ||r||_2 <= rtol * ||b||_2          (default 1e-9)  */
+    double rtol;        /* port solves stop at ||r||_2 <= rtol * ||b||_2          (default 1e-8)  */
     int32_t max_iter;   /* iteration cap per port solve                           (default 200)   */
     int32_t rhs_batch;  /* right-hand sides solved concurrently per tier          (default: auto) */
     void *cuda_stream;  /* cudaStream_t to run on                                 (default: 0)    */

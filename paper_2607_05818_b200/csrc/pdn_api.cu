@@ -699,7 +699,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
     }
     pdn_opts o{};
     if (opts) o = *opts;
-    if (!(o.rtol > 0.0)) o.rtol = 1e-9;
+    if (!(o.rtol > 0.0)) o.rtol = 1e-8;
     if (o.max_iter <= 0) o.max_iter = 200;
     if (o.nu <= 0) o.nu = 4;
     if (o.nu > 6) o.nu = 6;
