@@ -109,7 +109,7 @@ typedef struct {
     int64_t stencil_launches;    /* of which S1 (stencil phase) kernels                            */
     int32_t pcg_iters_max;       /* max PCG iterations over all port-solve batches                */
     int32_t pcg_iters_sum;       /* sum over batches of the batch's iteration count               */
-    int64_t rhs_iterations;      /* sum over batches of (iterations x right-hand sides)           */
+    int64_t rhs_iterations;      /* sum over iterations of the right-hand sides still iterating     */
     double worst_rel_residual;   /* max over all port solves of ||r|| / ||b|| at exit             */
     double ms_upload, ms_stencil, ms_dense, ms_total;
     double stencil_bytes;        /* algorithmic HBM bytes of the stencil phase (DESIGN.md model)  */

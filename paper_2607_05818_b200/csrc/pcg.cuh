@@ -75,6 +75,7 @@ __global__ void k_xport(const double* __restrict__ p, size_t n2, const double* _
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     const int b = blockIdx.y;
     const double a = alpha[b];
+    if (a == 0.0) return;  // frozen right-hand side: its p is no longer maintained
     if (ngather > 0) {
         if (k < ngather) xport[(size_t)b * ngather + k] = fma(a, p[b * n2 + node[k]], xport[(size_t)b * ngather + k]);
     } else if (k == 0) {

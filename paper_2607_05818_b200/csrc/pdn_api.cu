@@ -324,7 +324,8 @@ ChebR make_cheb_roots(int nu, double ratio) {
 }
 
 struct Smoother {
-    ChebR cr;
+    ChebR cr;   // level 0
+    ChebR crc;  // levels >= 1
     int G;  // right-hand sides a block loops over (upper bound; fewer on levels with few tiles)
 };
 
@@ -382,13 +383,13 @@ struct Work {
 inline int rhs_per_block(int tiles, int B, int G) {
     const long blocks_wanted = 148L * 4;
     long g = ((long)tiles * B) / blocks_wanted;
-    return (int)std::max(1L, std::min<long>(G, g));
+    return (int)std::max(1L, std::min<long>(std::min(G, T3_MAX_G), g));
 }
 
 template <int NU>
-void launch_down3(Launcher& L, int cls, double bytes, const Level& lv, const Smoother& sm, int B, const CUtensorMap& m_r,
+void launch_down3(Launcher& L, int cls, double bytes, const Level& lv, const Smoother& sm, const ChebR& cr, int B, const CUtensorMap& m_r,
                   const CUtensorMap* m_q, const double* alpha, double* r_out, double* y_out, double* rc, int cny,
-                  int cnx, int cpitch, double* rr_acc) {
+                  int cnx, int cpitch, double* rr_acc, const int* active) {
     constexpr int H = halo_of(NU), IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
     const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
     dim3 grid(tx, ty, cdiv(B, G));
@@ -399,13 +400,13 @@ void launch_down3(Launcher& L, int cls, double bytes, const Level& lv, const Smo
         CK(cudaFuncSetAttribute(k_down3<T3_R, T3_W, NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)base));
         attr_done = true;
     }
-    if (m_q) L.run(cls, bytes, [&] { k_down3<T3_R, T3_W, NU, true><<<grid, T3_THREADS, base + 2 * T3_TILE_BYTES, L.s>>>(m_r, *m_q, lv, sm.cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G); });
-    else L.run(cls, bytes, [&] { k_down3<T3_R, T3_W, NU, false><<<grid, T3_THREADS, base, L.s>>>(m_r, m_r, lv, sm.cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G); });
+    if (m_q) L.run(cls, bytes, [&] { k_down3<T3_R, T3_W, NU, true><<<grid, T3_THREADS, base + 2 * T3_TILE_BYTES, L.s>>>(m_r, *m_q, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
+    else L.run(cls, bytes, [&] { k_down3<T3_R, T3_W, NU, false><<<grid, T3_THREADS, base, L.s>>>(m_r, m_r, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
 }
 
 template <int NU>
-void launch_up3(Launcher& L, int cls, double bytes, const Level& lv, const Smoother& sm, int B, const CUtensorMap& m_r,
-                const CUtensorMap& m_y, const CUtensorMap& m_e, double* z_out, double* rz_acc) {
+void launch_up3(Launcher& L, int cls, double bytes, const Level& lv, const Smoother& sm, const ChebR& cr, int B, const CUtensorMap& m_r,
+                const CUtensorMap& m_y, const CUtensorMap& m_e, double* z_out, double* rz_acc, const int* active) {
     constexpr int H = halo_of(NU), IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
     const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
     dim3 grid(tx, ty, cdiv(B, G));
@@ -416,12 +417,13 @@ void launch_up3(Launcher& L, int cls, double bytes, const Level& lv, const Smoot
         CK(cudaFuncSetAttribute(k_up3<T3_R, T3_W, NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_done = true;
     }
-    if (rz_acc) L.run(cls, bytes, [&] { k_up3<T3_R, T3_W, NU, true><<<grid, T3_THREADS, smem, L.s>>>(m_r, m_y, m_e, lv, sm.cr, z_out, rz_acc, B, G); });
-    else L.run(cls, bytes, [&] { k_up3<T3_R, T3_W, NU, false><<<grid, T3_THREADS, smem, L.s>>>(m_r, m_y, m_e, lv, sm.cr, z_out, rz_acc, B, G); });
+    if (rz_acc) L.run(cls, bytes, [&] { k_up3<T3_R, T3_W, NU, true><<<grid, T3_THREADS, smem, L.s>>>(m_r, m_y, m_e, lv, cr, z_out, rz_acc, B, G, active); });
+    else L.run(cls, bytes, [&] { k_up3<T3_R, T3_W, NU, false><<<grid, T3_THREADS, smem, L.s>>>(m_r, m_y, m_e, lv, cr, z_out, rz_acc, B, G, active); });
 }
 
 void launch_pq3(Launcher& L, double bytes, const Level& lv, const Smoother& sm, int B, const CUtensorMap& m_z,
-                const CUtensorMap& m_p, const double* beta, double* p_new, double* q, double* pq_acc, double* sump_acc) {
+                const CUtensorMap& m_p, const double* beta, double* p_new, double* q, double* pq_acc, double* sump_acc,
+                const int* active) {
     constexpr int H = 2, IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
     const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
     dim3 grid(tx, ty, cdiv(B, G));
@@ -431,7 +433,7 @@ void launch_pq3(Launcher& L, double bytes, const Level& lv, const Smoother& sm, 
         CK(cudaFuncSetAttribute(k_pq3<PQ_R, PQ_W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_done = true;
     }
-    L.run(KC_PQ, bytes, [&] { k_pq3<PQ_R, PQ_W><<<grid, 32 * PQ_W, smem, L.s>>>(m_z, m_p, lv, beta, p_new, q, pq_acc, sump_acc, B, G); });
+    L.run(KC_PQ, bytes, [&] { k_pq3<PQ_R, PQ_W><<<grid, 32 * PQ_W, smem, L.s>>>(m_z, m_p, lv, beta, p_new, q, pq_acc, sump_acc, B, G, active); });
 }
 
 #define NU_DISPATCH(nu, CALL)                 \
@@ -448,27 +450,32 @@ void launch_pq3(Launcher& L, double bytes, const Level& lv, const Smoother& sm, 
 // forms W.r[ri^1] = W.r[ri] - alpha q (and its squared norm) and the cycle works with that.  The result z
 // is written to W.z; r.z goes to s.rz.  `after_down0` runs right after the level-0 down stage was
 // enqueued (the convergence check); if it returns true the rest of the cycle is skipped.
+// `nact` = right-hand sides of the batch still iterating (the kernels skip the others); it only enters the
+// algorithmic-byte accounting and is re-read after `after_down0`, which may lower it.
 template <class F>
-void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Smoother& sm, int B, int ri, bool fused, F&& after_down0) {
-    const int nl = H.nlev, nu = sm.cr.nu;
+void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Smoother& sm, int B, int ri, bool fused, const int& nact,
+            F&& after_down0) {
+    const int nl = H.nlev;
     const int ru = fused ? ri ^ 1 : ri;  // the residual the rest of the cycle works with
     for (int l = 0; l + 1 < nl; ++l) {
-        const double V = (double)B * H.ny[l] * H.nx[l] * 8.0, Vc = (double)B * H.ny[l + 1] * H.nx[l + 1] * 8.0;
+        const double V = (double)nact * H.ny[l] * H.nx[l] * 8.0, Vc = (double)nact * H.ny[l + 1] * H.nx[l + 1] * 8.0;
         const bool f = (l == 0 && fused);
         const double bytes = (f ? 4.0 : 2.0) * V + Vc;
-        NU_DISPATCH(nu, (launch_down3<NU_>(L, l == 0 ? KC_DOWN0 : KC_DOWNC, bytes, H.lev[l], sm, B, l == 0 ? W.m_r[ri] : W.m_rl[l],
+        const ChebR& cr = l == 0 ? sm.cr : sm.crc;
+        NU_DISPATCH(cr.nu, (launch_down3<NU_>(L, l == 0 ? KC_DOWN0 : KC_DOWNC, bytes, H.lev[l], sm, cr, B, l == 0 ? W.m_r[ri] : W.m_rl[l],
                                            f ? &W.m_q : nullptr, W.s.alpha, f ? W.r[ri ^ 1].as<double>() : nullptr,
                                            l == 0 ? W.y0.as<double>() : W.ya[l].as<double>(), W.rl[l + 1].as<double>(),
-                                           H.ny[l + 1], H.nx[l + 1], H.pitch[l + 1], W.s.rr)));
+                                           H.ny[l + 1], H.nx[l + 1], H.pitch[l + 1], W.s.rr, W.s.active)));
         if (l == 0 && after_down0()) return;  // converged (or out of iterations): skip the rest of the cycle
     }
     const int lc = nl - 1, nc = H.ny[lc] * H.nx[lc];
     L.run(KC_SMALL, 0, [&] { k_coarse_pinv<<<cdiv((size_t)B * nc, 128), 128, 0, L.s>>>(H.pinv.as<double>(), H.nx[lc], H.pitch[lc], nc, H.plane(lc), W.rl[lc].as<double>(), W.zb[lc].as<double>(), B); });
     for (int l = nl - 2; l >= 0; --l) {
-        const double V = (double)B * H.ny[l] * H.nx[l] * 8.0, Vc = (double)B * H.ny[l + 1] * H.nx[l + 1] * 8.0;
-        NU_DISPATCH(nu, (launch_up3<NU_>(L, l == 0 ? KC_UP0 : KC_UPC, 3.0 * V + Vc, H.lev[l], sm, B, l == 0 ? W.m_r[ru] : W.m_rl[l],
+        const double V = (double)nact * H.ny[l] * H.nx[l] * 8.0, Vc = (double)nact * H.ny[l + 1] * H.nx[l + 1] * 8.0;
+        const ChebR& cr = l == 0 ? sm.cr : sm.crc;
+        NU_DISPATCH(cr.nu, (launch_up3<NU_>(L, l == 0 ? KC_UP0 : KC_UPC, 3.0 * V + Vc, H.lev[l], sm, cr, B, l == 0 ? W.m_r[ru] : W.m_rl[l],
                                          l == 0 ? W.m_y0 : W.m_ya[l], W.m_ec[l + 1],
-                                         l == 0 ? W.z.as<double>() : W.zb[l].as<double>(), l == 0 ? W.s.rz : nullptr)));
+                                         l == 0 ? W.z.as<double>() : W.zb[l].as<double>(), l == 0 ? W.s.rz : nullptr, W.s.active)));
     }
 }
 
@@ -487,12 +494,14 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     L.run(KC_SMALL, V, [&] { k_init_rhs<<<dim3(cdiv(plane, 256), B), 256, 0, L.s>>>(W.r[0].as<double>(), n, H.pitch[0], plane, 1.0 / (double)n2, node, src0, B); });
     if (terminal) CK(cudaMemsetAsync(W.xown.p, 0, (size_t)B * sizeof(double), L.s));
     else CK(cudaMemsetAsync(W.xport.p, 0, (size_t)B * ngather * sizeof(double), L.s));
-    vcycle(L, H, W, sm, B, 0, false, [] { return false; });
+    int nact = B;  // right-hand sides still iterating
+    vcycle(L, H, W, sm, B, 0, false, nact, [] { return false; });
     const double bnorm2 = 1.0 - 1.0 / (double)n2;
     int it = 0, status = PDN_OK;
+    long active_sum = B;  // right-hand sides still iterating, summed over the iterations (first one: all)
     while (true) {
         L.run(KC_SMALL, 0, [&] { k_scal_beta<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, it == 0); });
-        launch_pq3(L, 4.0 * V, H.lev[0], sm, B, W.m_z, W.m_p[cur_p], W.s.beta, W.p[cur_p ^ 1].as<double>(), W.q.as<double>(), W.s.pq, W.s.sump);
+        launch_pq3(L, 4.0 * V * nact / B, H.lev[0], sm, B, W.m_z, W.m_p[cur_p], W.s.beta, W.p[cur_p ^ 1].as<double>(), W.q.as<double>(), W.s.pq, W.s.sump, W.s.active);
         cur_p ^= 1;
         L.run(KC_SMALL, 0, [&] { k_scal_alpha<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, 1.0 / (double)n2); });
         L.run(KC_SMALL, 0, [&] { k_xport<<<dim3(cdiv(std::max(ngather, 1), 128), B), 128, 0, L.s>>>(W.p[cur_p].as<double>(), plane, W.s.alpha, node, ngather, src0, W.xport.as<double>(), W.xown.as<double>(), B); });
@@ -502,10 +511,12 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
             L.run(KC_SMALL, 0, [&] { k_scal_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, rtol * rtol, bnorm2); });
             CK(cudaMemcpyAsync(W.h_nact, W.s.n_active, sizeof(int), cudaMemcpyDeviceToHost, L.s));
             CK(cudaStreamSynchronize(L.s));
-            done = (*W.h_nact == 0);
+            nact = *W.h_nact;
+            done = (nact == 0);
+            active_sum += nact;
             return done || it >= max_iter;
         };
-        vcycle(L, H, W, sm, B, cur_r, true, check);
+        vcycle(L, H, W, sm, B, cur_r, true, nact, check);
         cur_r ^= 1;
         if (done) break;
         if (it >= max_iter) { status = PDN_E_NOCONV; break; }
@@ -522,7 +533,10 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     c->stats.worst_rel_residual = std::max(c->stats.worst_rel_residual, worst);
     c->stats.pcg_iters_max = std::max(c->stats.pcg_iters_max, it);
     c->stats.pcg_iters_sum += it;
-    c->stats.rhs_iterations += (int64_t)it * B;
+    c->stats.rhs_iterations += active_sum;
+    if (getenv("PDN_DEBUG"))
+        fprintf(stderr, "[pdn] batch src0=%d B=%d %s: %d iterations, rhs-iterations %ld (of %ld without skipping), worst relres %.2e\n", src0, B,
+                terminal ? "terminal" : "tsv", it, active_sum, (long)it * B, worst);
     return status;
 }
 
@@ -783,7 +797,8 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         }
         Work W;
         if (H.nlev > 1) W.allocate(H, Bmax, qmax);
-        Smoother ch{make_cheb_roots(o.nu, 6.0), getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 32};
+        const int nu_c = getenv("PDN_NU_COARSE") ? std::min(6, std::max(1, atoi(getenv("PDN_NU_COARSE")))) : o.nu;
+        Smoother ch{make_cheb_roots(o.nu, 6.0), make_cheb_roots(nu_c, 6.0), getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 32};
         const double rtol_term = std::max(o.rtol, std::min(1e-5, std::sqrt(o.rtol) / 3.0));
         float ms_up = 0.f;
         for (int t = 0; t < d && status == PDN_OK; ++t) {

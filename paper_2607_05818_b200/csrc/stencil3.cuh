@@ -187,6 +187,29 @@ struct Geom {
     static_assert(IW > 0 && IH > 0, "halo too deep for the tile");
 };
 
+// The right-hand sides of [b0, b0 + nmax) that are still iterating (all of them if active == nullptr), in
+// order, for every thread of the block.  Converged right-hand sides are frozen: no kernel touches their
+// vectors again.  Call before the block's first __syncthreads.
+constexpr int T3_MAX_G = 64;
+struct ActiveList {
+    int b[T3_MAX_G];
+    int n;
+};
+__device__ __forceinline__ void active_list_build(ActiveList& al, const int* __restrict__ active, int b0, int nmax) {
+    if (threadIdx.x < 32) {
+        const int lane = threadIdx.x;
+        int cnt = 0;
+        for (int base = 0; base < nmax; base += 32) {
+            const int j = base + lane;
+            const bool a = j < nmax && (active == nullptr || active[b0 + j] != 0);
+            const unsigned m = __ballot_sync(FULL, a);
+            if (a) al.b[cnt + __popc(m & ((1u << lane) - 1u))] = b0 + j;
+            cnt += __popc(m);
+        }
+        if (lane == 0) al.n = cnt;
+    }
+}
+
 __host__ __device__ constexpr int halo_of(int nu) { return (nu + 1) & ~1; }
 
 // bit i: row i of the patch is an interior row of the tile and inside the mesh (columns too)
@@ -211,7 +234,7 @@ template <int R, int W, int NU, bool FUSED>
 __global__ void __launch_bounds__(32 * W, 1)
 k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensorMap tm_q, Level L, ChebR ch,
         const double* __restrict__ alpha, double* __restrict__ r_out, double* __restrict__ y_out,
-        double* __restrict__ rc, int cny, int cnx, int cpitch, double* __restrict__ rr_acc, int B, int G) {
+        double* __restrict__ rc, int cny, int cnx, int cpitch, double* __restrict__ rr_acc, int B, int G, const int* __restrict__ active) {
     constexpr int H = halo_of(NU);
     using Gm = Geom<R, W, H>;
     extern __shared__ __align__(128) double smem_dyn[];
@@ -232,17 +255,19 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
     const unsigned interior = interior_mask<R, H, Gm::IW, Gm::IH>(L, lane, warp, gx, gy0);
     const size_t plane = (size_t)L.ny * L.pitch, cplane = (size_t)cny * cpitch;
     const size_t goff = (size_t)gy0 * L.pitch + gx;
-    const int b0 = blockIdx.z * G, nb = min(G, B - b0);
+    __shared__ ActiveList al;
+    active_list_build(al, active, blockIdx.z * G, min(G, B - (int)blockIdx.z * G));
     if (threadIdx.x == 0) {
         mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); mbar_init(&mbar[2], 32 * W);
         mbar_fence_init();
     }
     __syncthreads();
+    const int nb = al.n;
     auto fetch = [&](int j) {  // thread 0 only
         const int st = j & 1;
         mbar_expect_tx(&mbar[st], (FUSED ? 2 : 1) * Gm::TILE_BYTES);
-        tma_load_3d(rbuf + st * Gm::TILE, &tm_r, x0, y0, b0 + j, &mbar[st]);
-        if (FUSED) tma_load_3d(qbuf + st * Gm::TILE, &tm_q, x0, y0, b0 + j, &mbar[st]);
+        tma_load_3d(rbuf + st * Gm::TILE, &tm_r, x0, y0, al.b[j], &mbar[st]);
+        if (FUSED) tma_load_3d(qbuf + st * Gm::TILE, &tm_q, x0, y0, al.b[j], &mbar[st]);
     };
     if (threadIdx.x == 0) {
         fetch(0);
@@ -250,7 +275,7 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
     }
     Xchg<W> xc{&x, &mbar[2], 0, 0u, warp, lane};
     for (int j = 0; j < nb; ++j) {
-        const int b = b0 + j, st = j & 1;
+        const int b = al.b[j], st = j & 1;
         mbar_wait(&mbar[st], (j >> 1) & 1);
         const double al = FUSED ? alpha[b] : 0.0;
         double y0r[R], y1r[R], rh0[R], rh1[R], rr = 0.0;
@@ -312,7 +337,7 @@ template <int R, int W, int NU, bool DOT>
 __global__ void __launch_bounds__(32 * W, 1)
 k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensorMap tm_y,
       const __grid_constant__ CUtensorMap tm_e, Level L, ChebR ch, double* __restrict__ z_out,
-      double* __restrict__ rz_acc, int B, int G) {
+      double* __restrict__ rz_acc, int B, int G, const int* __restrict__ active) {
     constexpr int H = halo_of(NU);
     using Gm = Geom<R, W, H>;
     extern __shared__ __align__(128) double smem_dyn[];
@@ -334,7 +359,8 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
     const unsigned interior = interior_mask<R, H, Gm::IW, Gm::IH>(L, lane, warp, gx, gy0);
     const size_t plane = (size_t)L.ny * L.pitch;
     const size_t goff = (size_t)gy0 * L.pitch + gx;
-    const int b0 = blockIdx.z * G, nb = min(G, B - b0);
+    __shared__ ActiveList al;
+    active_list_build(al, active, blockIdx.z * G, min(G, B - (int)blockIdx.z * G));
     const int cx0 = (x0 >> 1) & ~1;                 // even coarse column at or below x0/2 (x0 is even)
     const int eslot = (x0 >> 1) - cx0 + lane;       // this lane's coarse column inside the box
     if (threadIdx.x == 0) {
@@ -342,12 +368,13 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
         mbar_fence_init();
     }
     __syncthreads();
+    const int nb = al.n;
     auto fetch = [&](int j) {  // thread 0 only
         const int st = j & 1;
         mbar_expect_tx(&mbar[st], 2 * Gm::TILE_BYTES + Gm::EBOX_BYTES);
-        tma_load_3d(rbuf + st * Gm::TILE, &tm_r, x0, y0, b0 + j, &mbar[st]);
-        tma_load_3d(ybuf + st * Gm::TILE, &tm_y, x0, y0, b0 + j, &mbar[st]);
-        tma_load_3d(ebuf + st * Gm::ETILE, &tm_e, cx0, y0 / 2, b0 + j, &mbar[st]);
+        tma_load_3d(rbuf + st * Gm::TILE, &tm_r, x0, y0, al.b[j], &mbar[st]);
+        tma_load_3d(ybuf + st * Gm::TILE, &tm_y, x0, y0, al.b[j], &mbar[st]);
+        tma_load_3d(ebuf + st * Gm::ETILE, &tm_e, cx0, y0 / 2, al.b[j], &mbar[st]);
     };
     if (threadIdx.x == 0) {
         fetch(0);
@@ -355,7 +382,7 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
     }
     Xchg<W> xc{&x, &mbar[2], 0, 0u, warp, lane};
     for (int j = 0; j < nb; ++j) {
-        const int b = b0 + j, st = j & 1;
+        const int b = al.b[j], st = j & 1;
         mbar_wait(&mbar[st], (j >> 1) & 1);
         double y0r[R], y1r[R], rh0[R], rh1[R];
 #pragma unroll
@@ -402,7 +429,8 @@ template <int R, int W>
 __global__ void __launch_bounds__(32 * W, 1)
 k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensorMap tm_p, Level L,
       const double* __restrict__ beta, double* __restrict__ p_new, double* __restrict__ q,
-      double* __restrict__ pq_acc, double* __restrict__ sump_acc, int B, int G) {
+      double* __restrict__ pq_acc, double* __restrict__ sump_acc, int B, int G,
+      const int* __restrict__ active) {
     constexpr int H = 2;  // one ring is needed; two keep the 16-byte column pairs aligned
     using Gm = Geom<R, W, H>;
     extern __shared__ __align__(128) double smem_dyn[];
@@ -429,17 +457,19 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
     const unsigned interior = interior_mask<R, H, Gm::IW, Gm::IH>(L, lane, warp, gx, gy0);
     const size_t plane = (size_t)L.ny * L.pitch;
     const size_t goff = (size_t)gy0 * L.pitch + gx;
-    const int b0 = blockIdx.z * G, nb = min(G, B - b0);
+    __shared__ ActiveList al;
+    active_list_build(al, active, blockIdx.z * G, min(G, B - (int)blockIdx.z * G));
     if (threadIdx.x == 0) {
         mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); mbar_init(&mbar[2], 32 * W);
         mbar_fence_init();
     }
     __syncthreads();
+    const int nb = al.n;
     auto fetch = [&](int j) {  // thread 0 only
         const int st = j & 1;
         mbar_expect_tx(&mbar[st], 2 * Gm::TILE_BYTES);
-        tma_load_3d(zbuf + st * Gm::TILE, &tm_z, x0, y0, b0 + j, &mbar[st]);
-        tma_load_3d(pbuf + st * Gm::TILE, &tm_p, x0, y0, b0 + j, &mbar[st]);
+        tma_load_3d(zbuf + st * Gm::TILE, &tm_z, x0, y0, al.b[j], &mbar[st]);
+        tma_load_3d(pbuf + st * Gm::TILE, &tm_p, x0, y0, al.b[j], &mbar[st]);
     };
     if (threadIdx.x == 0) {
         fetch(0);
@@ -447,7 +477,7 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
     }
     Xchg<W> xc{&x, &mbar[2], 0, 0u, warp, lane};
     for (int j = 0; j < nb; ++j) {
-        const int b = b0 + j, st = j & 1;
+        const int b = al.b[j], st = j & 1;
         mbar_wait(&mbar[st], (j >> 1) & 1);
         const double bt = beta[b];
         double p0[R], p1[R], sump = 0.0, pq = 0.0;
