@@ -53,7 +53,9 @@ enum {
 enum {
     PDN_TIERS_ON_HOST = 1,  /* pdn_tier.gx / gy are HOST pointers (the library uploads them)            */
     PDN_SKIP_CONNECTIVITY_CHECK = 2,
-    PDN_TIME_KERNELS = 4    /* bracket every kernel launch with CUDA events (per-class timers in pdn_stats) */
+    PDN_TIME_KERNELS = 4,   /* bracket every kernel launch with CUDA events (per-class timers in pdn_stats) */
+    PDN_NO_UNIFORM_FAST_PATH = 8 /* solve uniform tiers numerically too (default: a tier whose x-segments are all
+                               equal and whose y-segments are all equal is reduced by the closed form, Eq. (3)) */
 };
 
 /* kernel classes of pdn_stats.class_* */
@@ -104,7 +106,7 @@ typedef struct {
 
 /* Counters and timings of the last pdn_create (device-event milliseconds). */
 typedef struct {
-    int32_t n_tiers, n_ports_total, n_levels, reserved;
+    int32_t n_tiers, n_ports_total, n_levels, n_uniform_tiers; /* tiers reduced by Eq. (3) */
     int64_t kernel_launches;     /* kernels launched by pdn_create so far (+ pdn_reff calls)      */
     int64_t stencil_launches;    /* of which S1 (stencil phase) kernels                            */
     int32_t pcg_iters_max;       /* max PCG iterations over all port-solve batches                */

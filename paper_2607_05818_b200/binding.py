@@ -18,6 +18,7 @@ PDN_OK = 0
 PDN_TIERS_ON_HOST = 1
 PDN_SKIP_CONNECTIVITY_CHECK = 2
 PDN_TIME_KERNELS = 4
+PDN_NO_UNIFORM_FAST_PATH = 8
 KERNEL_CLASSES = ("pq", "down0", "up0", "down_coarse", "up_coarse", "small", "dense", "pair")
 
 
@@ -40,7 +41,7 @@ class PdnOpts(C.Structure):
 
 class PdnStats(C.Structure):
     _fields_ = [("n_tiers", C.c_int32), ("n_ports_total", C.c_int32), ("n_levels", C.c_int32),
-                ("reserved", C.c_int32), ("kernel_launches", C.c_int64), ("stencil_launches", C.c_int64),
+                ("n_uniform_tiers", C.c_int32), ("kernel_launches", C.c_int64), ("stencil_launches", C.c_int64),
                 ("pcg_iters_max", C.c_int32), ("pcg_iters_sum", C.c_int32), ("rhs_iterations", C.c_int64),
                 ("worst_rel_residual", C.c_double), ("ms_upload", C.c_double), ("ms_stencil", C.c_double),
                 ("ms_dense", C.c_double), ("ms_total", C.c_double), ("stencil_bytes", C.c_double),

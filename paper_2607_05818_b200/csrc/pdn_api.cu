@@ -26,6 +26,7 @@
 #include "port.cuh"
 #include "setup.cuh"
 #include "stencil3.cuh"
+#include "uniform.cuh"
 
 using namespace pdn;
 
@@ -821,6 +822,33 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
             if (H.nlev == 1) {
                 L.run(KC_SMALL, 0, [&] { k_direct_small<<<T.q, 64, 0, L.s>>>(H.pinv.as<double>(), n, H.pitch[0], n * n, T.d_node.as<int>(), T.ntsv, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
                 continue;
+            }
+            if (!(o.flags & PDN_NO_UNIFORM_FAST_PATH)) {
+                // uniform tier: Eq. (3) of the paper as two dense contractions + a gather (uniform.cuh)
+                int* fl = H.flags.as<int>();
+                CK(cudaMemsetAsync(fl, 0, sizeof(int), L.s));
+                L.run(KC_SMALL, 0, [&] { k_uniform_check<<<cdiv(H.plane(0), 256), 256, 0, L.s>>>(n, H.pitch[0], H.gx[0].as<double>(), H.gy[0].as<double>(), fl); });
+                int h_flag = 1;
+                double g0[2] = {0.0, 0.0};
+                CK(cudaMemcpyAsync(&h_flag, fl, sizeof(int), cudaMemcpyDeviceToHost, L.s));
+                CK(cudaMemcpyAsync(&g0[0], H.gx[0].p, sizeof(double), cudaMemcpyDeviceToHost, L.s));
+                CK(cudaMemcpyAsync(&g0[1], H.gy[0].p, sizeof(double), cudaMemcpyDeviceToHost, L.s));
+                CK(cudaStreamSynchronize(L.s));
+                if (h_flag == 0 && g0[0] > 0.0 && g0[1] > 0.0) {
+                    const size_t nn = (size_t)n * n;
+                    DevBuf Cm, Wm, T1, Gt;
+                    Cm.alloc(2 * nn * sizeof(double)); Wm.alloc(nn * sizeof(double));
+                    T1.alloc(2 * nn * sizeof(double)); Gt.alloc(4 * nn * sizeof(double));
+                    L.run(KC_SMALL, 0, [&] { k_cos_matrix<<<cdiv(2 * nn, 256), 256, 0, L.s>>>(n, Cm.as<double>()); });
+                    L.run(KC_SMALL, 0, [&] { k_spectral_weights<<<cdiv(nn, 256), 256, 0, L.s>>>(n, g0[0], g0[1], Wm.as<double>()); });
+                    // T[a][s] = sum_b W[a][b] C[s][b]  (n x 2n);  G[t][s] = sum_a C[t][a] T[a][s]  (2n x 2n)
+                    gemm(L, n, 2 * n, n, 1.0, Wm.as<double>(), n, 1, Cm.as<double>(), 1, n, 0.0, T1.as<double>(), 2 * n);
+                    gemm(L, 2 * n, 2 * n, n, 1.0, Cm.as<double>(), n, 1, T1.as<double>(), 2 * n, 1, 0.0, Gt.as<double>(), 2 * n);
+                    L.run(KC_SMALL, 0, [&] { k_uniform_gather<<<dim3(cdiv(T.q, 128), T.ntsv + 1), 128, 0, L.s>>>(Gt.as<double>(), n, H.pitch[0], T.d_node.as<int>(), T.ntsv, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
+                    CK(cudaStreamSynchronize(L.s));  // the table buffers go back to the pool here
+                    c->stats.n_uniform_tiers++;
+                    continue;
+                }
             }
             for (int s0 = 0; s0 < T.ntsv && status == PDN_OK; s0 += Bmax)
                 status = solve_batch(c, L, H, W, T, ch, s0, std::min(Bmax, T.ntsv - s0), false, o.rtol, o.max_iter);

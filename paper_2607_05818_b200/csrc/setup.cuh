@@ -85,39 +85,46 @@ __global__ void k_coarsen(int ny, int nx, int pitch, const double* __restrict__ 
     cgy[i] = 0.5 * b;
 }
 
-// Dense pseudo-inverse of the coarsest Laplacian (nc = ny*nx <= 16 unknowns), one block, one thread:
+// Dense pseudo-inverse of the coarsest Laplacian (nc = ny*nx <= 16 unknowns), one warp, lane j owns
+// column j of the augmented matrix [L + 11^T/nc | I]:
 //   L^+ = (L + 11^T/nc)^-1 - 11^T/nc   (Gauss-Jordan on an SPD matrix, no pivoting needed).
 __global__ void k_coarsest_pinv(int ny, int nx, int pitch, const double* __restrict__ gx,
                                 const double* __restrict__ gy, double* __restrict__ pinv) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    const int nc = ny * nx;
-    double A[16][32];
-    for (int i = 0; i < nc; ++i)
-        for (int j = 0; j < 2 * nc; ++j) A[i][j] = (j < nc ? 1.0 / nc : (j - nc == i ? 1.0 : 0.0));
-    for (int y = 0; y < ny; ++y)
-        for (int x = 0; x < nx; ++x) {
-            const int i = y * nx + x;
-            if (x < nx - 1) {
-                const double g = gx[y * pitch + x];
-                A[i][i] += g; A[i + 1][i + 1] += g; A[i][i + 1] -= g; A[i + 1][i] -= g;
+    __shared__ double A[16][33];
+    const int nc = ny * nx, j = threadIdx.x;  // blockDim.x == 32 >= 2 nc
+    for (int i = 0; i < nc; ++i) A[i][j] = (j < nc ? 1.0 / nc : (j - nc == i ? 1.0 : 0.0));
+    __syncwarp();
+    if (j == 0) {
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) {
+                const int i = y * nx + x;
+                if (x < nx - 1) {
+                    const double g = gx[y * pitch + x];
+                    A[i][i] += g; A[i + 1][i + 1] += g; A[i][i + 1] -= g; A[i + 1][i] -= g;
+                }
+                if (y < ny - 1) {
+                    const double g = gy[y * pitch + x];
+                    A[i][i] += g; A[i + nx][i + nx] += g; A[i][i + nx] -= g; A[i + nx][i] -= g;
+                }
             }
-            if (y < ny - 1) {
-                const double g = gy[y * pitch + x];
-                A[i][i] += g; A[i + nx][i + nx] += g; A[i][i + nx] -= g; A[i + nx][i] -= g;
-            }
-        }
+    }
+    __syncwarp();
     for (int k = 0; k < nc; ++k) {
         const double inv = 1.0 / A[k][k];
-        for (int j = 0; j < 2 * nc; ++j) A[k][j] *= inv;
+        __syncwarp();
+        const double akj = A[k][j] * inv;
+        A[k][j] = akj;
+        __syncwarp();
         for (int i = 0; i < nc; ++i) {
             if (i == k) continue;
             const double f = A[i][k];
-            if (f != 0.0)
-                for (int j = 0; j < 2 * nc; ++j) A[i][j] -= f * A[k][j];
+            __syncwarp();
+            A[i][j] -= f * akj;
+            __syncwarp();
         }
     }
-    for (int i = 0; i < nc; ++i)
-        for (int j = 0; j < nc; ++j) pinv[i * nc + j] = A[i][nc + j] - 1.0 / nc;
+    if (j < nc)
+        for (int i = 0; i < nc; ++i) pinv[i * nc + j] = A[i][nc + j] - 1.0 / nc;
 }
 
 // Connectivity of one tier by label propagation: lab[i] = min over the component of the node ids.

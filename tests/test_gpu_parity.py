@@ -133,19 +133,22 @@ def test_small_rhs_batches_and_host_planes_give_same_answer():
     pdn.close()
 
 
-def test_port_matrix_matches_wu_closed_form():
+@pytest.mark.parametrize("fast_path", [True, False])
+def test_port_matrix_matches_wu_closed_form(fast_path):
     """S1 pin: on a uniform tier the intra-die R_jk = Z_jj + Z_kk - 2 Z_jk from the GPU port matrix
-    must equal PAPER.md:49 Eq. (3)."""
+    must equal PAPER.md:49 Eq. (3) -- both for the spectral fast path (uniform.cuh: Eq. 3 as two dense
+    contractions) and for the numerical multigrid-PCG path forced onto the same tier."""
     from closed_forms import wu_mesh_reff
-    from paper_2607_05818_b200 import Pdn
+    from paper_2607_05818_b200 import PDN_NO_UNIFORM_FAST_PATH, Pdn
     torch_cuda()
     n, rx, ry = 24, 0.8, 1.7
     sites = [np.array([[1, 2], [20, 5], [11, 11], [23, 23], [0, 17]])]
     bumps = np.array([[3, 3], [9, 21]])
     loads = np.array([[5, 5]])
     net = P.make_uniform(2, n, rx, ry, rt=0.1, tsv_sites=sites, bumps=bumps, loads=loads)
-    pdn = Pdn.from_network(net, device="cuda:0", rtol=1e-11)
+    pdn = Pdn.from_network(net, device="cuda:0", rtol=1e-11, flags=0 if fast_path else PDN_NO_UNIFORM_FAST_PATH)
     Z = pdn.port_matrix(0)
+    assert pdn.stats()["n_uniform_tiers"] == (2 if fast_path else 0)
     pdn.close()
     pts = [tuple(s) for s in sites[0]] + [tuple(b) for b in bumps]
     assert Z.shape == (7, 7)
@@ -156,8 +159,61 @@ def test_port_matrix_matches_wu_closed_form():
             (y1, x1), (y2, x2) = pts[j], pts[k]
             want = wu_mesh_reff(n, n, rx, ry, x1, y1, x2, y2)
             got = Z[j, j] + Z[k, k] - 2 * Z[j, k]
-            assert got == pytest.approx(want, rel=1e-8)
+            assert got == pytest.approx(want, rel=1e-11 if fast_path else 1e-8)
     assert np.isnan(Z[5, 6]) and np.isnan(Z[6, 5])
+
+
+@pytest.mark.parametrize("d,n,rx,ry", [(2, 45, 1.0, 1.0), (3, 64, 0.5, 2.0), (4, 130, 1.3, 0.4)])
+def test_uniform_stacks_fast_path_against_live_oracle(d, n, rx, ry):
+    """End to end on uniform tiers: the Eq. (3) fast path and the numerical path both match the oracle, and
+    each other; a stack with one jittered tier takes the fast path only on the uniform ones."""
+    from oracle.reff_oracle import Oracle
+    from paper_2607_05818_b200 import PDN_NO_UNIFORM_FAST_PATH
+    rng = np.random.default_rng([d, n])
+    sites = [P._distinct_sites(rng, n, 7) for _ in range(d - 1)]
+    net = P.make_uniform(d, n, rx, ry, rt=0.07, tsv_sites=sites, bumps=P._distinct_sites(rng, n, 5),
+                         loads=P._distinct_sites(rng, n, 6))
+    want = Oracle(net).reff_all()
+    fast, st = gpu_all_pairs(net)
+    assert st["n_uniform_tiers"] == d and st["pcg_iters_max"] == 0
+    rel = check(fast, want)
+    assert rel.max() < 1e-10                  # the closed form is exact up to rounding
+    slow, st2 = gpu_all_pairs(net, flags=PDN_NO_UNIFORM_FAST_PATH, rtol=1e-10)
+    assert st2["n_uniform_tiers"] == 0 and st2["pcg_iters_max"] > 0
+    check(slow, want)
+    net.gx[1], net.gy[1] = P._jitter_planes(rng, n, rx, ry)          # tier 1 no longer uniform
+    mixed, st3 = gpu_all_pairs(net, rtol=1e-10)
+    assert st3["n_uniform_tiers"] == d - 1
+    check(mixed, Oracle(net).reff_all())
+
+
+def test_port_matrix_of_a_nonuniform_tier_matches_the_dense_pseudo_inverse():
+    """S1 pin on general conductances: Z_t from the GPU = rows / columns of pinv(L_t) of the tier's Laplacian,
+    assembled here from the generator's planes (brute force, numpy)."""
+    from paper_2607_05818_b200 import Pdn
+    torch_cuda()
+    net = P.make_random(77, d=2, n=21, p=6, m=3, nl=4, drop=0.05, aniso=2.5)
+    n = net.n
+    pdn = Pdn.from_network(net, device="cuda:0", rtol=1e-12)
+    for t in range(2):
+        Lt = np.zeros((n * n, n * n))
+        for y in range(n):
+            for x in range(n):
+                i = y * n + x
+                if x < n - 1 and net.gx[t][y, x] > 0:
+                    g = net.gx[t][y, x]; Lt[i, i] += g; Lt[i + 1, i + 1] += g; Lt[i, i + 1] -= g; Lt[i + 1, i] -= g
+                if y < n - 1 and net.gy[t][y, x] > 0:
+                    g = net.gy[t][y, x]; Lt[i, i] += g; Lt[i + n, i + n] += g; Lt[i, i + n] -= g; Lt[i + n, i] -= g
+        Lp = np.linalg.pinv(Lt, hermitian=True)
+        term = net.bumps if t == 0 else net.loads
+        ports = [int(s[0]) * n + int(s[1]) for s in net.tsv_site[0]] + [int(s[0]) * n + int(s[1]) for s in term]
+        Z = pdn.port_matrix(t)
+        ntsv = len(net.tsv_site[0])
+        want = Lp[np.ix_(ports, ports)]
+        ok = ~np.isnan(Z)
+        assert ok[:ntsv, :].all() and ok[:, :ntsv].all() and np.diag(ok).all()
+        assert np.allclose(Z[ok], want[ok], rtol=0, atol=1e-9 * np.abs(want).max())
+    pdn.close()
 
 
 def test_bump_on_tsv_site_and_shared_sites_between_interfaces():
