@@ -161,6 +161,11 @@ def run_cuda(a):
 
     cfg = a.config
     net = P.make_config(cfg, seed=rank)          # one independent network per rank
+    if a.uniform:   # NEXT-1 variant: every tier gets its median segment conductances (same sites): Eq. (3) fast path
+        for t in range(net.d):
+            n_ = net.n
+            net.gx[t][:, : n_ - 1] = np.median(net.gx[t][:, : n_ - 1][net.gx[t][:, : n_ - 1] > 0])
+            net.gy[t][: n_ - 1, :] = np.median(net.gy[t][: n_ - 1, :][net.gy[t][: n_ - 1, :] > 0])
     npairs = net.m * net.nl
     gx_d = [torch.from_numpy(g).to(dev) for g in net.gx]
     gy_d = [torch.from_numpy(g).to(dev) for g in net.gy]
@@ -170,15 +175,17 @@ def run_cuda(a):
     out_h = torch.empty(npairs, dtype=torch.float64).pin_memory()
     args = (net.n,), (net.tsv_site, net.tsv_r, net.bumps, net.loads)
 
+    base_flags = 8 if a.no_fast_path else 0      # PDN_NO_UNIFORM_FAST_PATH
+
     def step_device(flags=0):
-        pdn = Pdn(net.n, gx_d, gy_d, *args[1], flags=flags, rtol=a.rtol, nu=a.nu, rhs_batch=a.rhs_batch)
+        pdn = Pdn(net.n, gx_d, gy_d, *args[1], flags=flags | base_flags, rtol=a.rtol, nu=a.nu, rhs_batch=a.rhs_batch)
         pdn.reff(out_d)
         st = pdn.stats()
         pdn.close()
         return st
 
     def step_host():
-        pdn = Pdn(net.n, gx_h, gy_h, *args[1], rtol=a.rtol, nu=a.nu, rhs_batch=a.rhs_batch)
+        pdn = Pdn(net.n, gx_h, gy_h, *args[1], flags=base_flags, rtol=a.rtol, nu=a.nu, rhs_batch=a.rhs_batch)
         pdn.reff_host(out_h)
         pdn.close()
 
@@ -252,7 +259,7 @@ def run_cuda(a):
     # tests/golden/make_golden.py from oracle/ only): max / mean relative error over the golden pairs
     parity = None
     gpath = os.path.join(ROOT, "tests", "golden", f"cfg{cfg}_reff.txt")
-    if os.path.exists(gpath):
+    if os.path.exists(gpath) and not a.uniform:
         g = np.loadtxt(gpath, comments="#")
         got = out_d.cpu().numpy().reshape(net.m, net.nl)[g[:, 0].astype(int), g[:, 1].astype(int)]
         rel = np.abs(got - g[:, 2]) / g[:, 2]
@@ -262,7 +269,8 @@ def run_cuda(a):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
         "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(cfg), "cfg": cfg, "pairs_per_step_per_gpu": npairs,
+        "config": {"workload": workload_name(cfg) + (" -- UNIFORM variant (median conductances)" if a.uniform else ""),
+                   "cfg": cfg, "pairs_per_step_per_gpu": npairs, "uniform_tiers": last["n_uniform_tiers"],
                    "l2": "working set of every stencil launch exceeds the 126 MB L2 (no flush needed)"
                          if cfg >= 3 else "working set fits L2: latency-bound case, HBM fraction not meaningful",
                    "rtol": a.rtol or 1e-8, "nu": a.nu or 4,
@@ -303,6 +311,8 @@ def main():
     ap.add_argument("--rhs-batch", type=int, default=0)
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--uniform", action="store_true", help="uniform-tier variant of the workload (Eq. 3 fast path)")
+    ap.add_argument("--no-fast-path", action="store_true", help="solve uniform tiers numerically too")
     ap.add_argument("--only-device", action="store_true", help="run only the device-resident steps (for ncu)")
     a = ap.parse_args()
     if a.impl == "reference":
