@@ -139,6 +139,15 @@ def run_reference(a):
 
 
 # ----------------------------------------------------------------------------------------- CUDA arm
+def max_over_ranks(ms, device, dist):
+    """Step time of the job = the slowest rank's device time (all-reduce MAX; gloo on CPU in the tests)."""
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def run_cuda(a):
     import torch
     import torch.distributed as dist
@@ -196,10 +205,7 @@ def run_cuda(a):
         res = [fn() for _ in range(steps)]
         e1.record()
         barrier()
-        ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-        return float(ms.item()), res
+        return max_over_ranks(e0.elapsed_time(e1), dev, dist if world > 1 else None), res
 
     for _ in range(a.warmup):
         step_device()
