@@ -98,12 +98,33 @@ class PdnError(RuntimeError):
         super().__init__(f"{where}: status {status} ({msg}){': ' + detail if detail else ''}")
 
 
-def _sites(arr) -> C.Array:
+_TSV_DTYPE = np.dtype([("iface", np.int32), ("y", np.int32), ("x", np.int32), ("r_ohm", np.float64)], align=True)
+_SITE_DTYPE = np.dtype([("y", np.int32), ("x", np.int32)], align=True)
+assert _TSV_DTYPE.itemsize == C.sizeof(PdnTsv) and _SITE_DTYPE.itemsize == C.sizeof(PdnSite)
+
+
+def _sites(arr) -> np.ndarray:
+    """(k, 2) rows (y, x) -> array of pdn_site (numpy structured array with the C layout)."""
     a = np.ascontiguousarray(arr, dtype=np.int32).reshape(-1, 2)
-    out = (PdnSite * max(len(a), 1))()
-    for k, (y, x) in enumerate(a):
-        out[k].y, out[k].x = int(y), int(x)
+    out = np.zeros(max(len(a), 1), dtype=_SITE_DTYPE)
+    out["y"][: len(a)] = a[:, 0]
+    out["x"][: len(a)] = a[:, 1]
     return out
+
+
+def _tsvs(tsv_site, tsv_r) -> tuple:
+    """Per-interface site / resistance lists -> (array of pdn_tsv, count)."""
+    n = sum(len(np.asarray(s).reshape(-1, 2)) for s in tsv_site)
+    out = np.zeros(max(n, 1), dtype=_TSV_DTYPE)
+    k = 0
+    for i, (s, r) in enumerate(zip(tsv_site, tsv_r)):
+        s = np.asarray(s, dtype=np.int32).reshape(-1, 2)
+        out["iface"][k:k + len(s)] = i
+        out["y"][k:k + len(s)] = s[:, 0]
+        out["x"][k:k + len(s)] = s[:, 1]
+        out["r_ohm"][k:k + len(s)] = np.asarray(r, dtype=np.float64)
+        k += len(s)
+    return out, n
 
 
 def _ptr(t) -> int:
@@ -131,21 +152,17 @@ class Pdn:
             tiers[t].n = n
             tiers[t].gx = _ptr(gx[t])
             tiers[t].gy = _ptr(gy[t])
-        ntsv = sum(len(s) for s in tsv_site)
-        tsvs = (PdnTsv * max(ntsv, 1))()
-        k = 0
-        for i, (s, r) in enumerate(zip(tsv_site, tsv_r)):
-            for (y, x), rr in zip(np.asarray(s).reshape(-1, 2), np.asarray(r, dtype=np.float64)):
-                tsvs[k].iface, tsvs[k].y, tsvs[k].x, tsvs[k].r_ohm = i, int(y), int(x), float(rr)
-                k += 1
+        tsvs, ntsv = _tsvs(tsv_site, tsv_r)
         self.m = len(np.asarray(bumps).reshape(-1, 2))
         self.nl = len(np.asarray(loads).reshape(-1, 2))
         opts = PdnOpts(rtol=rtol, max_iter=max_iter, rhs_batch=rhs_batch,
                        cuda_stream=C.c_void_p(stream) if stream else None,
                        flags=flags | (PDN_TIERS_ON_HOST if on_host else 0), nu=nu)
         h = C.c_void_p()
-        st = lib.pdn_create(C.byref(h), d, tiers, ntsv, tsvs, self.m, _sites(bumps), self.nl, _sites(loads),
-                            C.byref(opts))
+        b_arr, l_arr = _sites(bumps), _sites(loads)
+        st = lib.pdn_create(C.byref(h), d, tiers, ntsv, tsvs.ctypes.data_as(C.POINTER(PdnTsv)), self.m,
+                            b_arr.ctypes.data_as(C.POINTER(PdnSite)), self.nl,
+                            l_arr.ctypes.data_as(C.POINTER(PdnSite)), C.byref(opts))
         if st != PDN_OK:
             raise PdnError(st, "pdn_create")
         self._h = h

@@ -286,17 +286,21 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
                 const double2 q = ld2(qbuf + st * Gm::TILE + slot0 + i * T3_EW);
                 r.x = fma(-al, q.x, r.x);
                 r.y = fma(-al, q.y, r.y);
-                if ((interior >> i) & 1) {
-                    st2(r_out + b * plane + goff + (size_t)i * L.pitch, r);
-                    rr = fma(r.x, r.x, rr);
-                    rr = fma(r.y, r.y, rr);
-                }
+                const bool in = (interior >> i) & 1;
+                if (in) st2(r_out + b * plane + goff + (size_t)i * L.pitch, r);
+                const double mx = in ? r.x : 0.0, my = in ? r.y : 0.0;
+                rr = fma(mx, mx, rr);
+                rr = fma(my, my, rr);
             }
             const float4 s4 = sc_slot[i * 32];
             rh0[i] = (double)s4.x * r.x;
             rh1[i] = (double)s4.z * r.y;
             y0r[i] = ch.w[0] * rh0[i];
             y1r[i] = ch.w[0] * rh1[i];
+        }
+        if (FUSED) {  // ||r||^2: the shuffle chain overlaps the sweeps that follow
+            rr = warp_sum(rr);
+            if (lane == 0) atomicAdd(rr_acc + b, rr);
         }
         // once thread 0 is past the first row exchange of this iteration every thread has arrived there,
         // i.e. has consumed the stage: thread 0 may refill it with right-hand side j+2
@@ -322,10 +326,6 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
                     st2(y_out + b * plane + goff + (size_t)(i + 1) * L.pitch, make_double2(y0r[i + 1], y1r[i + 1]));
                 rc[b * cplane + (size_t)((gy0 + i) >> 1) * cpitch + (gx >> 1)] = v;
             }
-        }
-        if (FUSED) {
-            rr = warp_sum(rr);
-            if (lane == 0) atomicAdd(rr_acc + b, rr);
         }
     }
 }
@@ -381,6 +381,8 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
         if (nb > 1) fetch(1);
     }
     Xchg<W> xc{&x, &mbar[2], 0, 0u, warp, lane};
+    double rz_pend = 0.0;  // r.z partial of the previous right-hand side: reduced while the next one sweeps
+    int b_pend = -1;
     for (int j = 0; j < nb; ++j) {
         const int b = al.b[j], st = j & 1;
         mbar_wait(&mbar[st], (j >> 1) & 1);
@@ -396,6 +398,10 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
             y0r[i] = fma((double)s4.y, e, yin.x);
             y1r[i] = fma((double)s4.w, e, yin.y);
         }
+        if (DOT && b_pend >= 0) {
+            rz_pend = warp_sum(rz_pend);
+            if (lane == 0) atomicAdd(rz_acc + b_pend, rz_pend);
+        }
 #pragma unroll
         for (int k = 0; k < NU; ++k) {
             smooth_step<R, W>(xc, c, y0r, y1r, rh0, rh1, ch.w[NU - 1 - k]);
@@ -404,20 +410,21 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
         double rz = 0.0;
 #pragma unroll
         for (int i = 0; i < R; ++i) {
-            if ((interior >> i) & 1) {
-                const float4 s4 = sc_slot[i * 32];
-                st2(z_out + b * plane + goff + (size_t)i * L.pitch,
-                    make_double2((double)s4.x * y0r[i], (double)s4.z * y1r[i]));
-                if (DOT) {  // r.z = r.(s y) = (s r).y = r^.y
-                    rz = fma(rh0[i], y0r[i], rz);
-                    rz = fma(rh1[i], y1r[i], rz);
-                }
+            const bool in = (interior >> i) & 1;
+            const float4 s4 = sc_slot[i * 32];
+            if (in) st2(z_out + b * plane + goff + (size_t)i * L.pitch,
+                        make_double2((double)s4.x * y0r[i], (double)s4.z * y1r[i]));
+            if (DOT) {  // r.z = r.(s y) = (s r).y = r^.y
+                rz = fma(in ? rh0[i] : 0.0, y0r[i], rz);
+                rz = fma(in ? rh1[i] : 0.0, y1r[i], rz);
             }
         }
-        if (DOT) {
-            rz = warp_sum(rz);
-            if (lane == 0) atomicAdd(rz_acc + b, rz);
-        }
+        rz_pend = rz;
+        b_pend = b;
+    }
+    if (DOT && b_pend >= 0) {
+        rz_pend = warp_sum(rz_pend);
+        if (lane == 0) atomicAdd(rz_acc + b_pend, rz_pend);
     }
 }
 
@@ -476,6 +483,16 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
         if (nb > 1) fetch(1);
     }
     Xchg<W> xc{&x, &mbar[2], 0, 0u, warp, lane};
+    double pq_pend = 0.0, sump_pend = 0.0;  // partials of the previous right-hand side, reduced one iteration later
+    int b_pend = -1;
+    auto flush = [&] {
+        pq_pend = warp_sum(pq_pend);
+        sump_pend = warp_sum(sump_pend);
+        if (lane == 0) {
+            atomicAdd(pq_acc + b_pend, pq_pend);
+            atomicAdd(sump_acc + b_pend, sump_pend);
+        }
+    };
     for (int j = 0; j < nb; ++j) {
         const int b = al.b[j], st = j & 1;
         mbar_wait(&mbar[st], (j >> 1) & 1);
@@ -489,32 +506,29 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
                 p.x = fma(bt, po.x, p.x);
                 p.y = fma(bt, po.y, p.y);
             }
-            if ((interior >> i) & 1) {
-                st2(p_new + b * plane + goff + (size_t)i * L.pitch, p);
-                sump += p.x + p.y;
-            }
+            const bool in = (interior >> i) & 1;
+            if (in) st2(p_new + b * plane + goff + (size_t)i * L.pitch, p);
+            sump += in ? p.x + p.y : 0.0;
             p0[i] = p.x;
             p1[i] = p.y;
         }
+        if (b_pend >= 0) flush();
         double t0[R], t1[R];
         apply_step<R, W>(xc, c, p0, p1, zero, zero, t0, t1);
         if (threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
 #pragma unroll
         for (int i = 0; i < R; ++i) {
-            if ((interior >> i) & 1) {
-                const double q0 = fma(d0[i], p0[i], -t0[i]), q1 = fma(d1[i], p1[i], -t1[i]);
-                st2(q + b * plane + goff + (size_t)i * L.pitch, make_double2(q0, q1));
-                pq = fma(p0[i], q0, pq);
-                pq = fma(p1[i], q1, pq);
-            }
+            const bool in = (interior >> i) & 1;
+            const double q0 = fma(d0[i], p0[i], -t0[i]), q1 = fma(d1[i], p1[i], -t1[i]);
+            if (in) st2(q + b * plane + goff + (size_t)i * L.pitch, make_double2(q0, q1));
+            pq = fma(in ? p0[i] : 0.0, q0, pq);
+            pq = fma(in ? p1[i] : 0.0, q1, pq);
         }
-        pq = warp_sum(pq);
-        sump = warp_sum(sump);
-        if (lane == 0) {
-            atomicAdd(pq_acc + b, pq);
-            atomicAdd(sump_acc + b, sump);
-        }
+        pq_pend = pq;
+        sump_pend = sump;
+        b_pend = b;
     }
+    if (b_pend >= 0) flush();
 }
 
 }  // namespace pdn

@@ -266,6 +266,10 @@ def test_error_statuses():
     def isolate(b):
         b.gx[0][4, 4] = b.gx[0][4, 3] = b.gy[0][4, 4] = b.gy[0][3, 4] = 0.0
     expect(2, isolate)
+    # iteration cap reached
+    with pytest.raises(PdnError) as e:
+        Pdn.from_network(net, device="cuda:0", max_iter=1)
+    assert e.value.status == 3
     # wrong n_pairs for the cross product
     import torch
     pdn = Pdn.from_network(net, device="cuda:0")
