@@ -102,6 +102,7 @@ typedef struct {
     void *cuda_stream;  /* cudaStream_t to run on                                 (default: 0)    */
     int32_t flags;      /* PDN_* flags                                                             */
     int32_t nu;         /* Chebyshev smoothing steps per multigrid level and side (1..6, default 4)*/
+    double cheb_ratio;  /* smoothing interval [2/ratio, 2] of D^-1 L (default: 3 + the tier's anisotropy)  */
 } pdn_opts;
 
 /* Counters and timings of the last pdn_create (device-event milliseconds). */

@@ -36,7 +36,7 @@ class PdnSite(C.Structure):
 
 class PdnOpts(C.Structure):
     _fields_ = [("rtol", C.c_double), ("max_iter", C.c_int32), ("rhs_batch", C.c_int32),
-                ("cuda_stream", C.c_void_p), ("flags", C.c_int32), ("nu", C.c_int32)]
+                ("cuda_stream", C.c_void_p), ("flags", C.c_int32), ("nu", C.c_int32), ("cheb_ratio", C.c_double)]
 
 
 class PdnStats(C.Structure):
@@ -141,7 +141,7 @@ class Pdn:
     or numpy / torch CPU arrays (host path: PDN_TIERS_ON_HOST is set and the library uploads)."""
 
     def __init__(self, n, gx, gy, tsv_site, tsv_r, bumps, loads, rtol=0.0, max_iter=0, rhs_batch=0,
-                 nu=0, flags=0, stream=None):
+                 nu=0, flags=0, stream=None, cheb_ratio=0.0):
         lib = load_library()
         d = len(gx)
         on_host = isinstance(gx[0], np.ndarray) or (hasattr(gx[0], "is_cuda") and not gx[0].is_cuda)
@@ -157,7 +157,7 @@ class Pdn:
         self.nl = len(np.asarray(loads).reshape(-1, 2))
         opts = PdnOpts(rtol=rtol, max_iter=max_iter, rhs_batch=rhs_batch,
                        cuda_stream=C.c_void_p(stream) if stream else None,
-                       flags=flags | (PDN_TIERS_ON_HOST if on_host else 0), nu=nu)
+                       flags=flags | (PDN_TIERS_ON_HOST if on_host else 0), nu=nu, cheb_ratio=cheb_ratio)
         h = C.c_void_p()
         b_arr, l_arr = _sites(bumps), _sites(loads)
         st = lib.pdn_create(C.byref(h), d, tiers, ntsv, tsvs.ctypes.data_as(C.POINTER(PdnTsv)), self.m,

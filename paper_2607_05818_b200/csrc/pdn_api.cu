@@ -249,7 +249,8 @@ struct Hierarchy {
     int nlev = 0;
     int ny[MAX_LEVELS], nx[MAX_LEVELS], pitch[MAX_LEVELS];
     DevBuf gx[MAX_LEVELS], gy[MAX_LEVELS], hE[MAX_LEVELS], hS[MAX_LEVELS], sc[MAX_LEVELS];
-    DevBuf pinv, flags, labels;  // flags: [0] bad value, [1] isolated node, [2] label changed, [3] label nonzero
+    DevBuf pinv, flags, labels, sums;  // flags: [0] bad value, [1] isolated node, [2] label changed, [3] label nonzero
+    double anisotropy = 1.0;           // max(mean gx / mean gy, mean gy / mean gx) of the tier built last
     Level lev[MAX_LEVELS];
 
     size_t plane(int l) const { return (size_t)ny[l] * pitch[l]; }
@@ -271,6 +272,7 @@ struct Hierarchy {
         }
         pinv.alloc(16 * 16 * sizeof(double));
         flags.alloc(4 * sizeof(int));
+        sums.alloc(2 * sizeof(double));
         labels.alloc((size_t)n * n * sizeof(int));
     }
 
@@ -289,9 +291,14 @@ struct Hierarchy {
         }
         const int lc = nlev - 1;
         L.run(KC_SMALL, 0, [&] { k_coarsest_pinv<<<1, 32, 0, L.s>>>(ny[lc], nx[lc], pitch[lc], gx[lc].as<double>(), gy[lc].as<double>(), pinv.as<double>()); });
+        CK(cudaMemsetAsync(sums.p, 0, 2 * sizeof(double), L.s));
+        L.run(KC_SMALL, 0, [&] { k_plane_sums<<<std::min(1024u, cdiv(plane(0), 256)), 256, 0, L.s>>>((int)plane(0), gx[0].as<double>(), gy[0].as<double>(), sums.as<double>()); });
         int h[4] = {0, 0, 0, 0};
+        double hs[2] = {1.0, 1.0};
         CK(cudaMemcpyAsync(h, fl, 2 * sizeof(int), cudaMemcpyDeviceToHost, L.s));
+        CK(cudaMemcpyAsync(hs, sums.p, 2 * sizeof(double), cudaMemcpyDeviceToHost, L.s));
         CK(cudaStreamSynchronize(L.s));
+        anisotropy = (hs[0] > 0.0 && hs[1] > 0.0) ? std::max(hs[0] / hs[1], hs[1] / hs[0]) : 1.0;
         if (h[0]) return PDN_E_ARG;
         if (h[1] && n > 1) return PDN_E_DISCONNECTED;
         if (check_connectivity) {
@@ -798,8 +805,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         }
         Work W;
         if (H.nlev > 1) W.allocate(H, Bmax, qmax);
-        const int nu_c = getenv("PDN_NU_COARSE") ? std::min(6, std::max(1, atoi(getenv("PDN_NU_COARSE")))) : o.nu;
-        Smoother ch{make_cheb_roots(o.nu, 6.0), make_cheb_roots(nu_c, 6.0), getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 32};
+        const int G = getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 32;
         const double rtol_term = std::max(o.rtol, std::min(1e-5, std::sqrt(o.rtol) / 3.0));
         float ms_up = 0.f;
         for (int t = 0; t < d && status == PDN_OK; ++t) {
@@ -819,6 +825,11 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
             CK(cudaEventElapsedTime(&ms, ev[1], ev[2]));
             ms_up += ms;
             if (status != PDN_OK) { g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status); break; }
+            // Smoothing interval [2/ratio, 2] of the Chebyshev polynomial.  With 2x2 aggregation the coarse grid
+            // takes fewer modes off the smoother the more anisotropic the tier is, so the interval widens with
+            // the anisotropy a: ratio = 3 + a (measured: a = 1 -> 4, a = 3 -> 6).
+            const double ratio = o.cheb_ratio > 1.0 ? o.cheb_ratio : std::min(10.0, 3.0 + H.anisotropy);
+            const Smoother ch{make_cheb_roots(o.nu, ratio), make_cheb_roots(o.nu, ratio), G};
             if (H.nlev == 1) {
                 L.run(KC_SMALL, 0, [&] { k_direct_small<<<T.q, 64, 0, L.s>>>(H.pinv.as<double>(), n, H.pitch[0], n * n, T.d_node.as<int>(), T.ntsv, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
                 continue;

@@ -27,6 +27,22 @@ __global__ void k_import_planes(const double* __restrict__ gx_in, const double* 
     gy[i] = b;
 }
 
+// sums[0] += sum of the x-conductances, sums[1] += sum of the y-conductances (the tier's anisotropy, which
+// picks the smoothing interval of the Chebyshev polynomial; pdn_api.cu).
+__global__ void k_plane_sums(int n_elems, const double* __restrict__ gx, const double* __restrict__ gy,
+                             double* __restrict__ sums) {
+    __shared__ double red[32];
+    double a = 0.0, b = 0.0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_elems; i += gridDim.x * blockDim.x) {
+        a += gx[i];
+        b += gy[i];
+    }
+    a = block_sum(a, red);
+    if (threadIdx.x == 0) atomicAdd(sums, a);
+    b = block_sum(b, red);
+    if (threadIdx.x == 0) atomicAdd(sums + 1, b);
+}
+
 // sc = (s, sd) = (1/sqrt(d), sqrt(d)) in FP32, d = sum of incident conductances ((0,0) if the node is
 // isolated; flagged on the finest level).
 __global__ void k_scale_nodes(int ny, int nx, int pitch, const double* __restrict__ gx, const double* __restrict__ gy,
