@@ -67,6 +67,40 @@ __global__ void k_scal_check(PcgScalars s, int B, double tol2, double bnorm2) {
     }
 }
 
+// Residual update alone, without the V-cycle's down stage -- launched when the batch is expected to converge
+// in this iteration, so that the smoothing of a cycle nobody needs is not run:
+//   r_out = r_in - alpha q ;  rr += ||r_out||^2      for the right-hand sides still iterating.
+// grid = (chunks of the plane, B); 16-byte accesses; plane (= ny*pitch) is even.
+constexpr int RESID_THREADS = 256, RESID_PER_THREAD = 4;  // double2 per thread
+__global__ void __launch_bounds__(RESID_THREADS)
+k_resid_update(const double* __restrict__ r_in, const double* __restrict__ q, const double* __restrict__ alpha,
+               const int* __restrict__ active, double* __restrict__ r_out, double* __restrict__ rr_acc, size_t plane) {
+    __shared__ double red[32];
+    const int b = blockIdx.y;
+    if (!active[b]) return;
+    const double al = alpha[b];
+    const size_t n2 = plane / 2, base = (size_t)blockIdx.x * RESID_THREADS * RESID_PER_THREAD + threadIdx.x;
+    const double2* r2 = reinterpret_cast<const double2*>(r_in + b * plane);
+    const double2* q2 = reinterpret_cast<const double2*>(q + b * plane);
+    double2* o2 = reinterpret_cast<double2*>(r_out + b * plane);
+    double rr = 0.0;
+#pragma unroll
+    for (int k = 0; k < RESID_PER_THREAD; ++k) {
+        const size_t i = base + (size_t)k * RESID_THREADS;
+        if (i < n2) {
+            double2 r = r2[i];
+            const double2 qq = q2[i];
+            r.x = fma(-al, qq.x, r.x);
+            r.y = fma(-al, qq.y, r.y);
+            o2[i] = r;
+            rr = fma(r.x, r.x, rr);
+            rr = fma(r.y, r.y, rr);
+        }
+    }
+    rr = block_sum(rr, red);
+    if (threadIdx.x == 0) atomicAdd(rr_acc + b, rr);
+}
+
 // x_port[b][k] += alpha[b] * p[b][node[k]],  k over the gather list (all ports of the tier for a
 // TSV-source batch; for a terminal batch ngather == 0 and only the source node itself is read).
 __global__ void k_xport(const double* __restrict__ p, size_t n2, const double* __restrict__ alpha,

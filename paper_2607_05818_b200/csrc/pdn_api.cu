@@ -102,6 +102,23 @@ struct DevPool {
 };
 DevPool g_pool;
 
+// Pinned host scratch for the per-iteration read-backs: one grow-only block per thread, kept for the life of
+// the process (cudaMallocHost / cudaFreeHost stall for hundreds of ms now and then).
+struct PinnedScratch {
+    void* p = nullptr;
+    size_t bytes = 0;
+    void* get(size_t n) {
+        if (n > bytes) {
+            if (p) cudaFreeHost(p);
+            p = nullptr; bytes = 0;
+            if (cudaMallocHost(&p, n) != cudaSuccess) { cudaGetLastError(); p = nullptr; return nullptr; }
+            bytes = n;
+        }
+        return p;
+    }
+};
+thread_local PinnedScratch g_pinned;
+
 struct DevBuf {  // RAII device allocation (block sizes are rounded up to 1 MiB classes above 1 MiB)
     void* p = nullptr;
     size_t bytes = 0;
@@ -347,7 +364,7 @@ struct Work {
     CUtensorMap m_rl[MAX_LEVELS], m_ya[MAX_LEVELS], m_ec[MAX_LEVELS];  // m_ec[l]: zb[l] as the coarse box of level l-1
     DevBuf scal, xport, xown, iact;
     PcgScalars s{};
-    int* h_nact = nullptr;                           // pinned
+    int* h_nact = nullptr;                           // pinned (g_pinned: not owned)
     double* h_relres = nullptr;                      // pinned, Bmax
 
     static size_t bytes_per_rhs(const Hierarchy& H) {
@@ -378,12 +395,10 @@ struct Work {
         s.n_active = iact.as<int>() + B;
         xport.alloc((size_t)B * std::max(qmax, 1) * sizeof(double));
         xown.alloc((size_t)B * sizeof(double));
-        CK(cudaMallocHost(&h_nact, sizeof(int)));
-        CK(cudaMallocHost(&h_relres, (size_t)B * sizeof(double)));
-    }
-    ~Work() {
-        if (h_nact) cudaFreeHost(h_nact);
-        if (h_relres) cudaFreeHost(h_relres);
+        char* hp = static_cast<char*>(g_pinned.get(64 + (size_t)B * sizeof(double)));
+        if (!hp) throw StatusFail{PDN_E_NOMEM, "pinned host allocation failed"};
+        h_nact = reinterpret_cast<int*>(hp);
+        h_relres = reinterpret_cast<double*>(hp + 64);
     }
 };
 
@@ -507,6 +522,7 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     const double bnorm2 = 1.0 - 1.0 / (double)n2;
     int it = 0, status = PDN_OK;
     long active_sum = B;  // right-hand sides still iterating, summed over the iterations (first one: all)
+    double rel_prev = 1.0, rel_cur = 1.0;  // max relative residual over the batch after the last two iterations
     while (true) {
         L.run(KC_SMALL, 0, [&] { k_scal_beta<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, it == 0); });
         launch_pq3(L, 4.0 * V * nact / B, H.lev[0], sm, B, W.m_z, W.m_p[cur_p], W.s.beta, W.p[cur_p ^ 1].as<double>(), W.q.as<double>(), W.s.pq, W.s.sump, W.s.active);
@@ -518,14 +534,28 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
         auto check = [&] {
             L.run(KC_SMALL, 0, [&] { k_scal_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, rtol * rtol, bnorm2); });
             CK(cudaMemcpyAsync(W.h_nact, W.s.n_active, sizeof(int), cudaMemcpyDeviceToHost, L.s));
+            CK(cudaMemcpyAsync(W.h_relres, W.s.relres, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, L.s));
             CK(cudaStreamSynchronize(L.s));
             nact = *W.h_nact;
             done = (nact == 0);
             active_sum += nact;
+            rel_prev = rel_cur;
+            rel_cur = 0.0;
+            for (int b = 0; b < B; ++b) rel_cur = std::max(rel_cur, W.h_relres[b]);
             return done || it >= max_iter;
         };
-        vcycle(L, H, W, sm, B, cur_r, true, nact, check);
-        cur_r ^= 1;
+        // CG residuals contract roughly geometrically: if the next one is expected below the tolerance, update the
+        // residual alone first (3 V of traffic) and run the V-cycle only if that expectation was wrong
+        const bool expect_done = rel_prev > 0.0 && rel_cur * (rel_cur / rel_prev) <= rtol;
+        if (expect_done) {
+            const size_t chunk = (size_t)RESID_THREADS * RESID_PER_THREAD * 2;
+            L.run(KC_SMALL, 3.0 * V * nact / B, [&] { k_resid_update<<<dim3(cdiv(plane, chunk), B), RESID_THREADS, 0, L.s>>>(W.r[cur_r].as<double>(), W.q.as<double>(), W.s.alpha, W.s.active, W.r[cur_r ^ 1].as<double>(), W.s.rr, plane); });
+            cur_r ^= 1;
+            if (!check()) vcycle(L, H, W, sm, B, cur_r, false, nact, [] { return false; });
+        } else {
+            vcycle(L, H, W, sm, B, cur_r, true, nact, check);
+            cur_r ^= 1;
+        }
         if (done) break;
         if (it >= max_iter) { status = PDN_E_NOCONV; break; }
     }
