@@ -64,6 +64,90 @@ k_gemm(int M, int N, int K, double alpha, const double* __restrict__ A, int64_t 
     }
 }
 
+// Same contraction on the FP64 tensor cores (DMMA, mma.sync m8n8k4): 128x128 block tile, 8 warps in a 2x4
+// grid, each accumulating a 64x32 tile as 8x4 m8n8 fragments; K is walked in steps of 16 through shared memory
+// (k-major tiles padded by 8 so that the four k-rows of a fragment load fall in two conflict-free wavefronts),
+// the next tile's global loads overlapping the current tile's MMAs in registers.  Any strides, any sizes.
+constexpr int DG_BM = 128, DG_BN = 128, DG_BK = 16, DG_PAD = 8, DG_THREADS = 256;
+
+__device__ __forceinline__ void dmma_m8n8k4(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+__global__ void __launch_bounds__(DG_THREADS)
+k_gemm_dmma(int M, int N, int K, double alpha, const double* __restrict__ A, int64_t sai, int64_t sak,
+            const double* __restrict__ B, int64_t sbk, int64_t sbj, double beta, double* __restrict__ C, int64_t ldc) {
+    __shared__ double As[DG_BK][DG_BM + DG_PAD];
+    __shared__ double Bs[DG_BK][DG_BN + DG_PAD];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wm = (warp >> 2) * 64, wn = (warp & 3) * 32;  // warp tile origin inside the block tile
+    const int i0 = blockIdx.y * DG_BM, j0 = blockIdx.x * DG_BN;
+    constexpr int PER = DG_BK * DG_BM / DG_THREADS;  // 8 elements of each operand per thread and k-tile
+    double ra[PER], rb[PER];
+    auto load_tile = [&](int k0) {
+#pragma unroll
+        for (int e = 0; e < PER; ++e) {
+            const int idx = tid + e * DG_THREADS;
+            int kk, ii;
+            if (sak == 1) { kk = idx % DG_BK; ii = idx / DG_BK; } else { ii = idx % DG_BM; kk = idx / DG_BM; }
+            const int gi = i0 + ii, gk = k0 + kk;
+            ra[e] = (gi < M && gk < K) ? A[gi * sai + gk * sak] : 0.0;
+            int kb, jj;
+            if (sbk == 1) { kb = idx % DG_BK; jj = idx / DG_BK; } else { jj = idx % DG_BN; kb = idx / DG_BN; }
+            const int gj = j0 + jj, gkb = k0 + kb;
+            rb[e] = (gj < N && gkb < K) ? B[gkb * sbk + gj * sbj] : 0.0;
+        }
+    };
+    auto store_tile = [&] {
+#pragma unroll
+        for (int e = 0; e < PER; ++e) {
+            const int idx = tid + e * DG_THREADS;
+            int kk, ii;
+            if (sak == 1) { kk = idx % DG_BK; ii = idx / DG_BK; } else { ii = idx % DG_BM; kk = idx / DG_BM; }
+            As[kk][ii] = ra[e];
+            int kb, jj;
+            if (sbk == 1) { kb = idx % DG_BK; jj = idx / DG_BK; } else { jj = idx % DG_BN; kb = idx / DG_BN; }
+            Bs[kb][jj] = rb[e];
+        }
+    };
+    double acc[8][4][2] = {};
+    const int fr = lane >> 2, fk = lane & 3;  // fragment row / column index, k index
+    load_tile(0);
+    for (int k0 = 0; k0 < K; k0 += DG_BK) {
+        __syncthreads();  // everybody is done with the previous tile
+        store_tile();
+        __syncthreads();
+        if (k0 + DG_BK < K) load_tile(k0 + DG_BK);
+#pragma unroll
+        for (int ks = 0; ks < DG_BK; ks += 4) {
+            double a[8], b[4];
+#pragma unroll
+            for (int mi = 0; mi < 8; ++mi) a[mi] = As[ks + fk][wm + mi * 8 + fr];
+#pragma unroll
+            for (int ni = 0; ni < 4; ++ni) b[ni] = Bs[ks + fk][wn + ni * 8 + fr];
+#pragma unroll
+            for (int mi = 0; mi < 8; ++mi)
+#pragma unroll
+                for (int ni = 0; ni < 4; ++ni) dmma_m8n8k4(acc[mi][ni][0], acc[mi][ni][1], a[mi], b[ni]);
+        }
+    }
+#pragma unroll
+    for (int mi = 0; mi < 8; ++mi) {
+        const int gi = i0 + wm + mi * 8 + fr;
+        if (gi >= M) continue;
+#pragma unroll
+        for (int ni = 0; ni < 4; ++ni)
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int gj = j0 + wn + ni * 8 + 2 * fk + h;
+                if (gj >= N) continue;
+                double* p = C + gi * ldc + gj;
+                *p = (beta == 0.0) ? alpha * acc[mi][ni][h] : fma(alpha, acc[mi][ni][h], beta * *p);
+            }
+    }
+}
+
 // Unblocked Cholesky of the nb x nb diagonal block at A[k0,k0] (nb <= DENSE_NB), lower triangle; one
 // block of DENSE_NB*DENSE_NB threads.  *fail is set if a pivot is not positive.
 __global__ void k_potrf_diag(double* __restrict__ A, int64_t lda, int k0, int nb, int* __restrict__ fail) {

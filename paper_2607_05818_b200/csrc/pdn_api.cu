@@ -584,6 +584,11 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
 void gemm(Launcher& L, int M, int N, int K, double alpha, const double* A, int64_t sai, int64_t sak, const double* B,
           int64_t sbk, int64_t sbj, double beta, double* C, int64_t ldc) {
     if (M <= 0 || N <= 0) return;
+    if (M >= 96 && N >= 96 && K >= 16) {  // large enough for the 128x128 tensor-core tiles to pay
+        dim3 grid(cdiv(N, DG_BN), cdiv(M, DG_BM));
+        L.run(KC_DENSE, 0, [&] { k_gemm_dmma<<<grid, DG_THREADS, 0, L.s>>>(M, N, K, alpha, A, sai, sak, B, sbk, sbj, beta, C, ldc); });
+        return;
+    }
     dim3 grid(cdiv(N, GEMM_BN), cdiv(M, GEMM_BM));
     L.run(KC_DENSE, 0, [&] { k_gemm<<<grid, 256, 0, L.s>>>(M, N, K, alpha, A, sai, sak, B, sbk, sbj, beta, C, ldc); });
 }
