@@ -1,6 +1,6 @@
 // S3: dense FP64 building blocks for the port-level system ("one decomposition",
 // PAPER.md:202 substitution for the m+n right-hand sides): generic-stride GEMM, blocked Cholesky,
-// blocked triangular solves with many right-hand sides.  All matrices row-major with a leading
+// blocked forward triangular solve (used to invert the diagonal Cholesky factors).  All matrices row-major with a leading
 // dimension; every kernel is bounds-checked (arbitrary sizes).
 #pragma once
 #include "common.cuh"
@@ -148,6 +148,11 @@ k_gemm_dmma(int M, int N, int K, double alpha, const double* __restrict__ A, int
     }
 }
 
+__global__ void k_set_identity(int n, double* __restrict__ A) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < (size_t)n * n) A[i] = (i / n == i % n) ? 1.0 : 0.0;
+}
+
 // Unblocked Cholesky of the nb x nb diagonal block at A[k0,k0] (nb <= DENSE_NB), lower triangle; one
 // block of DENSE_NB*DENSE_NB threads.  *fail is set if a pivot is not positive.
 __global__ void k_potrf_diag(double* __restrict__ A, int64_t lda, int k0, int nb, int* __restrict__ fail) {
@@ -197,23 +202,6 @@ __global__ void k_trsm_fwd_diag(const double* __restrict__ L, int64_t lda, int k
     for (int j = 0; j < nb; ++j) {
         double s = Bm[(k0 + j) * ldb + c];
         for (int l = 0; l < j; ++l) s = fma(-S[j][l], x[l], s);
-        x[j] = s / S[j][j];
-        Bm[(k0 + j) * ldb + c] = x[j];
-    }
-}
-
-// Backward panel solve: rows k0..k0+nb of X <- L_kk^-T B_k.
-__global__ void k_trsm_bwd_diag(const double* __restrict__ L, int64_t lda, int k0, int nb, double* __restrict__ Bm,
-                                int64_t ldb, int nrhs) {
-    __shared__ double S[DENSE_NB][DENSE_NB + 1];
-    for (int e = threadIdx.x; e < nb * nb; e += blockDim.x) S[e / nb][e % nb] = L[(k0 + e / nb) * lda + k0 + e % nb];
-    __syncthreads();
-    const int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= nrhs) return;
-    double x[DENSE_NB];
-    for (int j = nb - 1; j >= 0; --j) {
-        double s = Bm[(k0 + j) * ldb + c];
-        for (int l = j + 1; l < nb; ++l) s = fma(-S[l][j], x[l], s);
         x[j] = s / S[j][j];
         Bm[(k0 + j) * ldb + c] = x[j];
     }

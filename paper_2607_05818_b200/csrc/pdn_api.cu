@@ -618,17 +618,6 @@ void trsm_fwd(Launcher& L, const double* Lm, int64_t lda, int n, double* Bm, int
     }
 }
 
-// Bm (n x nrhs, ldb) <- Lm^-T Bm
-void trsm_bwd(Launcher& L, const double* Lm, int64_t lda, int n, double* Bm, int64_t ldb, int nrhs) {
-    const int nblk = (n + DENSE_NB - 1) / DENSE_NB;
-    for (int kb = nblk - 1; kb >= 0; --kb) {
-        const int k0 = kb * DENSE_NB, nb = std::min(DENSE_NB, n - k0);
-        L.run(KC_DENSE, 0, [&] { k_trsm_bwd_diag<<<cdiv(nrhs, 128), 128, 0, L.s>>>(Lm, lda, k0, nb, Bm, ldb, nrhs); });
-        if (k0 > 0)  // rows [0,k0) -= L[k0:k0+nb, 0:k0]^T X_k
-            gemm(L, k0, nrhs, nb, -1.0, Lm + (int64_t)k0 * lda, 1, lda, Bm + (int64_t)k0 * ldb, ldb, 1, 1.0, Bm, ldb);
-    }
-}
-
 // ------------------------------------------------------------------------------------------------
 // S2 + S3: assemble C = [K B; B^T 0] (block-tridiagonal SPD K), factor it once, substitute for the
 // m + n + (d-1) right-hand sides, eliminate the multipliers, and leave the pair-kernel operands.
@@ -663,17 +652,34 @@ int recombine(pdn_ctx* c, Launcher& L) {
         }
         L.run(KC_DENSE, 0, [&] { k_assemble_rhs<<<dim3(cdiv(nrhs, 128), pi), 128, 0, L.s>>>(i, dm1, pi, m, n, T0.ZT.as<double>(), T0.q, T0.ntsv, Td.ZT.as<double>(), Td.q, Td.ntsv, F[i].as<double>()); });
     }
-    // block-tridiagonal Cholesky + forward substitution
+    // block-tridiagonal Cholesky + forward substitution.  Every diagonal factor L_i (p_i x p_i, cond ~ 1e2) is
+    // inverted once by a p_i-column triangular solve; all substitutions for the m + n + d-1 right-hand sides
+    // are then K = p_i contractions on the FP64 tensor cores instead of 32-wide panel solves.
+    std::vector<DevBuf> Li(dm1);
+    DevBuf tmp;
+    {
+        size_t tmax = 0;
+        for (int i = 0; i < dm1; ++i) tmax = std::max(tmax, (size_t)c->p[i] * std::max(nrhs, c->p[i]));
+        for (int i = 1; i < dm1; ++i) tmax = std::max(tmax, (size_t)c->p[i - 1] * c->p[i]);
+        tmp.alloc(tmax * sizeof(double));
+    }
     for (int i = 0; i < dm1; ++i) {
         const int pi = c->p[i];
         if (i > 0) {
             const int ph = c->p[i - 1];
-            trsm_fwd(L, Kd[i - 1].as<double>(), ph, ph, V[i].as<double>(), pi, pi);
+            // V_i <- L_{i-1}^-1 V_i
+            gemm(L, ph, pi, ph, 1.0, Li[i - 1].as<double>(), ph, 1, V[i].as<double>(), pi, 1, 0.0, tmp.as<double>(), pi);
+            CK(cudaMemcpyAsync(V[i].p, tmp.p, (size_t)ph * pi * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
             gemm(L, pi, pi, ph, -1.0, V[i].as<double>(), 1, pi, V[i].as<double>(), pi, 1, 1.0, Kd[i].as<double>(), pi);
             gemm(L, pi, nrhs, ph, -1.0, V[i].as<double>(), 1, pi, F[i - 1].as<double>(), nrhs, 1, 1.0, F[i].as<double>(), nrhs);
         }
         potrf(L, Kd[i].as<double>(), pi, pi, fail.as<int>());
-        trsm_fwd(L, Kd[i].as<double>(), pi, pi, F[i].as<double>(), nrhs, nrhs);
+        Li[i].alloc((size_t)pi * pi * sizeof(double));
+        L.run(KC_DENSE, 0, [&] { k_set_identity<<<cdiv((size_t)pi * pi, 256), 256, 0, L.s>>>(pi, Li[i].as<double>()); });
+        trsm_fwd(L, Kd[i].as<double>(), pi, pi, Li[i].as<double>(), pi, pi);
+        // F_i <- L_i^-1 F_i
+        gemm(L, pi, nrhs, pi, 1.0, Li[i].as<double>(), pi, 1, F[i].as<double>(), nrhs, 1, 0.0, tmp.as<double>(), nrhs);
+        CK(cudaMemcpyAsync(F[i].p, tmp.p, (size_t)pi * nrhs * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
     }
     // backward substitution
     for (int i = dm1 - 1; i >= 0; --i) {
@@ -682,7 +688,9 @@ int recombine(pdn_ctx* c, Launcher& L) {
             const int pj = c->p[i + 1];
             gemm(L, pi, nrhs, pj, -1.0, V[i + 1].as<double>(), pj, 1, F[i + 1].as<double>(), nrhs, 1, 1.0, F[i].as<double>(), nrhs);
         }
-        trsm_bwd(L, Kd[i].as<double>(), pi, pi, F[i].as<double>(), nrhs, nrhs);
+        // F_i <- L_i^-T F_i
+        gemm(L, pi, nrhs, pi, 1.0, Li[i].as<double>(), 1, pi, F[i].as<double>(), nrhs, 1, 0.0, tmp.as<double>(), nrhs);
+        CK(cudaMemcpyAsync(F[i].p, tmp.p, (size_t)pi * nrhs * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
     }
     // multipliers (Schur complement on the d-1 constraints, Eq. 8) and TSV currents
     for (int i = 0; i < dm1; ++i)
