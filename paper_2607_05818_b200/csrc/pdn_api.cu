@@ -253,7 +253,15 @@ CUtensorMap make_map(const void* base, int nx, int ny, int pitch, int B, int box
 #ifndef PDN_PQ_W
 #define PDN_PQ_W (PDN_T3_W / 2)
 #endif
+#ifndef PDN_DN_R
+#define PDN_DN_R PDN_T3_R
+#endif
+#ifndef PDN_DN_W
+#define PDN_DN_W PDN_T3_W
+#endif
 constexpr int T3_R = PDN_T3_R, T3_W = PDN_T3_W, T3_EH = T3_R * T3_W, T3_THREADS = 32 * T3_W;
+constexpr int DN_R = PDN_DN_R, DN_W = PDN_DN_W;  // patch shape of the down stage (same tile height)
+static_assert(DN_R * DN_W == T3_EH, "all stencil kernels share the TMA box height");
 constexpr int PQ_R = PDN_PQ_R, PQ_W = PDN_PQ_W;  // the operator apply has one sweep and no r^: fatter patches pay
 static_assert(PQ_R * PQ_W == T3_EH, "all level-0 kernels share the TMA box height");
 constexpr size_t T3_TILE_BYTES = (size_t)T3_EH * T3_EW * sizeof(double), T3_SC_BYTES = (size_t)T3_EH * 32 * sizeof(float4);
@@ -416,15 +424,15 @@ void launch_down3(Launcher& L, int cls, double bytes, const Level& lv, const Smo
     constexpr int H = halo_of(NU), IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
     const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
     dim3 grid(tx, ty, cdiv(B, G));
-    constexpr size_t base = 2 * T3_TILE_BYTES + T3_SC_BYTES + sizeof(Exch<T3_W>);
+    constexpr size_t base = 2 * T3_TILE_BYTES + T3_SC_BYTES + sizeof(Exch<DN_W>);
     static bool attr_done = false;
     if (!attr_done) {
-        CK(cudaFuncSetAttribute(k_down3<T3_R, T3_W, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(base + 2 * T3_TILE_BYTES)));
-        CK(cudaFuncSetAttribute(k_down3<T3_R, T3_W, NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)base));
+        CK(cudaFuncSetAttribute(k_down3<DN_R, DN_W, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(base + 2 * T3_TILE_BYTES)));
+        CK(cudaFuncSetAttribute(k_down3<DN_R, DN_W, NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)base));
         attr_done = true;
     }
-    if (m_q) L.run(cls, bytes, [&] { k_down3<T3_R, T3_W, NU, true><<<grid, T3_THREADS, base + 2 * T3_TILE_BYTES, L.s>>>(m_r, *m_q, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
-    else L.run(cls, bytes, [&] { k_down3<T3_R, T3_W, NU, false><<<grid, T3_THREADS, base, L.s>>>(m_r, m_r, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
+    if (m_q) L.run(cls, bytes, [&] { k_down3<DN_R, DN_W, NU, true><<<grid, 32 * DN_W, base + 2 * T3_TILE_BYTES, L.s>>>(m_r, *m_q, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
+    else L.run(cls, bytes, [&] { k_down3<DN_R, DN_W, NU, false><<<grid, 32 * DN_W, base, L.s>>>(m_r, m_r, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
 }
 
 template <int NU>
