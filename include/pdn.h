@@ -116,6 +116,8 @@ typedef struct {
     double worst_rel_residual;   /* max over all port solves of ||r|| / ||b|| at exit             */
     double ms_upload, ms_stencil, ms_dense, ms_total;
     double stencil_bytes;        /* algorithmic HBM bytes of the stencil phase (DESIGN.md model)  */
+    double ms_update_stencil, ms_update_dense; /* last pdn_update_tsvs: port solves + remap / S2 + S3     */
+    int64_t update_solves;       /* port solves the last pdn_update_tsvs needed                   */
     double class_ms[8];          /* device ms per kernel class (only with PDN_TIME_KERNELS)       */
     double class_bytes[8];       /* algorithmic bytes moved per kernel class                      */
     int64_t class_launches[8];   /* launches per kernel class                                     */
@@ -139,6 +141,14 @@ int pdn_reff(pdn_ctx *ctx, int64_t n_pairs, const int32_t *bump_idx, const int32
 /* Same with HOST index arrays (or NULL, NULL) and a HOST output buffer (S4 + S5: PAPER.md:218,
  * "transferred back to the CPU host"). */
 int pdn_reff_host(pdn_ctx *ctx, int64_t n_pairs, const int32_t *bump_idx, const int32_t *load_idx, double *out);
+
+/* TSV re-planning (the paper's design-space use case): replaces the TSV set of ctx by
+ * the given list (HOST array, same rules as in pdn_create) and brings ctx up to date for pdn_reff.  The list is
+ * diffed against the current one per interface by site: kept sites cost nothing (their resistance may change),
+ * removed sites cost nothing, every added site costs one port solve on each of its two tiers; the port-level
+ * system is then re-assembled and re-factored.  If the call fails (PDN_E_ARG leaves ctx untouched; any other
+ * status may leave it half updated) the context must be destroyed. */
+int pdn_update_tsvs(pdn_ctx *ctx, int32_t n_tsv, const pdn_tsv *tsvs);
 
 /* NULL-safe; frees all device and host memory of ctx. */
 void pdn_destroy(pdn_ctx *ctx);

@@ -45,12 +45,13 @@ class PdnStats(C.Structure):
                 ("pcg_iters_max", C.c_int32), ("pcg_iters_sum", C.c_int32), ("rhs_iterations", C.c_int64),
                 ("worst_rel_residual", C.c_double), ("ms_upload", C.c_double), ("ms_stencil", C.c_double),
                 ("ms_dense", C.c_double), ("ms_total", C.c_double), ("stencil_bytes", C.c_double),
+                ("ms_update_stencil", C.c_double), ("ms_update_dense", C.c_double), ("update_solves", C.c_int64),
                 ("class_ms", C.c_double * 8), ("class_bytes", C.c_double * 8),
                 ("class_launches", C.c_int64 * 8)]
 
 
 EXPORTS = ("pdn_create", "pdn_reff", "pdn_reff_host", "pdn_destroy", "pdn_strerror", "pdn_last_error",
-           "pdn_get_stats", "pdn_port_count", "pdn_get_port_matrix", "pdn_release_cache")
+           "pdn_get_stats", "pdn_port_count", "pdn_get_port_matrix", "pdn_release_cache", "pdn_update_tsvs")
 
 _lib = None
 
@@ -77,6 +78,8 @@ def load_library() -> C.CDLL:
     lib.pdn_strerror.argtypes = [C.c_int]
     lib.pdn_last_error.restype = C.c_char_p
     lib.pdn_last_error.argtypes = []
+    lib.pdn_update_tsvs.restype = C.c_int
+    lib.pdn_update_tsvs.argtypes = [C.c_void_p, C.c_int32, C.POINTER(PdnTsv)]
     lib.pdn_release_cache.restype = None
     lib.pdn_release_cache.argtypes = []
     lib.pdn_get_stats.restype = C.c_int
@@ -195,6 +198,13 @@ class Pdn:
         if st != PDN_OK:
             raise PdnError(st, "pdn_reff_host")
         return out
+
+    def update_tsvs(self, tsv_site, tsv_r):
+        """pdn_update_tsvs: re-plan the TSVs (per-interface site / resistance lists, as in the constructor)."""
+        tsvs, ntsv = _tsvs(tsv_site, tsv_r)
+        st = self._lib.pdn_update_tsvs(self._h, ntsv, tsvs.ctypes.data_as(C.POINTER(PdnTsv)))
+        if st != PDN_OK:
+            raise PdnError(st, "pdn_update_tsvs")
 
     def stats(self) -> dict:
         s = PdnStats()

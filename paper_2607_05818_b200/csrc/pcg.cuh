@@ -7,15 +7,16 @@
 
 namespace pdn {
 
-// r[b] = e_{node[src0+b]} - 1/n2  (consistent right-hand side of the singular tier system) on the
-// pitched plane (plane = ny*pitch doubles; pad entries 0); node[] holds pitched offsets y*pitch + x.
+// r[b] = e_{node[src[b]]} - 1/n2  (consistent right-hand side of the singular tier system) on the
+// pitched plane (plane = ny*pitch doubles; pad entries 0); node[] holds pitched offsets y*pitch + x of the
+// tier's ports, src[b] is the port index right-hand side b is the source of.
 __global__ void k_init_rhs(double* __restrict__ r, int nx, int pitch, size_t plane, double inv_n2,
-                           const int* __restrict__ node, int src0, int B) {
+                           const int* __restrict__ node, const int* __restrict__ src, int B) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int b = blockIdx.y;
     if (i >= plane) return;
     const double m = ((int)(i % pitch) < nx) ? -inv_n2 : 0.0;
-    r[b * plane + i] = (i == (size_t)node[src0 + b]) ? 1.0 + m : m;
+    r[b * plane + i] = (i == (size_t)node[src[b]]) ? 1.0 + m : m;
 }
 
 __global__ void k_zero(double* __restrict__ a, size_t n) {
@@ -104,8 +105,8 @@ k_resid_update(const double* __restrict__ r_in, const double* __restrict__ q, co
 // x_port[b][k] += alpha[b] * p[b][node[k]],  k over the gather list (all ports of the tier for a
 // TSV-source batch; for a terminal batch ngather == 0 and only the source node itself is read).
 __global__ void k_xport(const double* __restrict__ p, size_t n2, const double* __restrict__ alpha,
-                        const int* __restrict__ node, int ngather, int src0, double* __restrict__ xport,
-                        double* __restrict__ xown, int B) {
+                        const int* __restrict__ node, int ngather, const int* __restrict__ src,
+                        double* __restrict__ xport, double* __restrict__ xown, int B) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     const int b = blockIdx.y;
     const double a = alpha[b];
@@ -113,22 +114,41 @@ __global__ void k_xport(const double* __restrict__ p, size_t n2, const double* _
     if (ngather > 0) {
         if (k < ngather) xport[(size_t)b * ngather + k] = fma(a, p[b * n2 + node[k]], xport[(size_t)b * ngather + k]);
     } else if (k == 0) {
-        xown[b] = fma(a, p[b * n2 + node[src0 + b]], xown[b]);
+        xown[b] = fma(a, p[b * n2 + node[src[b]]], xown[b]);
     }
 }
 
-// ZT[src0+b][k] = x_port[b][k] - mean(x_b)   /   zdiag[b] = x_own[b] - mean(x_b)
+// ZT[src[b]][k] = x_port[b][k] - mean(x_b)   /   zdiag[src[b] - ntsv] = x_own[b] - mean(x_b)
 __global__ void k_finish_tsv(const double* __restrict__ xport, const double* __restrict__ xmean, int ngather,
-                             double* __restrict__ zt_rows, int B) {
+                             const int* __restrict__ src, double* __restrict__ ZT, int B) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     const int b = blockIdx.y;
-    if (k < ngather) zt_rows[(size_t)b * ngather + k] = xport[(size_t)b * ngather + k] - xmean[b];
+    if (k < ngather) ZT[(size_t)src[b] * ngather + k] = xport[(size_t)b * ngather + k] - xmean[b];
 }
 
 __global__ void k_finish_term(const double* __restrict__ xown, const double* __restrict__ xmean,
-                              double* __restrict__ zdiag, int B) {
+                              const int* __restrict__ src, int ntsv, double* __restrict__ zdiag, int B) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b < B) zdiag[b] = xown[b] - xmean[b];
+    if (b < B) zdiag[src[b] - ntsv] = xown[b] - xmean[b];
+}
+
+// TSV re-planning (pdn_update_tsvs): copy the kept entries of a tier's port matrix into its new layout.
+//   ZTn[rmap[j]][cmap[k]] = ZTo[j][k]   for old TSV rows j and old ports k whose maps are >= 0
+__global__ void k_remap_zt(const double* __restrict__ ZTo, int ntsv_o, int q_o, const int* __restrict__ rmap,
+                           const int* __restrict__ cmap, double* __restrict__ ZTn, int q_n) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (k >= q_o || j >= ntsv_o) return;
+    const int jn = rmap[j], kn = cmap[k];
+    if (jn >= 0 && kn >= 0) ZTn[(size_t)jn * q_n + kn] = ZTo[(size_t)j * q_o + k];
+}
+
+// ... and fill the columns of the added TSV ports in the kept rows by symmetry: Z[j][s] = Z[s][j].
+__global__ void k_mirror_added(double* __restrict__ ZT, int ntsv, int q, const int* __restrict__ added, int n_added,
+                               const unsigned char* __restrict__ is_added) {
+    const int a = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (a >= n_added || j >= ntsv || is_added[j]) return;
+    const int s = added[a];
+    ZT[(size_t)j * q + s] = ZT[(size_t)s * q + j];
 }
 
 // Meshes with n <= 4 are their own coarsest level: Z comes straight from the dense pseudo-inverse.

@@ -148,6 +148,7 @@ struct TierPorts {
     DevBuf d_node;                    // device copy
     DevBuf ZT;                        // ntsv x q
     DevBuf zdiag;                     // nterm
+    DevBuf gx0, gy0;                  // sanitised pitched level-0 planes, kept for pdn_update_tsvs
 };
 
 }  // namespace
@@ -156,6 +157,8 @@ struct pdn_ctx {
     int d = 0, n = 0, m = 0, nl = 0, p0 = 0;
     std::vector<int> p;               // TSVs per interface
     std::vector<std::vector<double>> rt;
+    std::vector<std::vector<int>> site;   // per interface: pitched offsets of the TSV sites, in list order
+    std::vector<int> bump_id, load_id;    // pitched offsets of the terminals
     cudaStream_t stream = nullptr;
     pdn_opts opts{};
     std::vector<TierPorts> tiers;
@@ -301,12 +304,19 @@ struct Hierarchy {
         labels.alloc((size_t)n * n * sizeof(int));
     }
 
-    // Import one tier (gx_src / gy_src are device pointers, dense n x n) and build all levels.
-    int build(Launcher& L, const double* gx_src, const double* gy_src, bool check_connectivity) {
+    // Import one tier (gx_src / gy_src are device pointers: dense n x n planes of the caller, or -- `retained` --
+    // the sanitised pitched level-0 planes a context kept from its creation) and build all levels.
+    int build(Launcher& L, const double* gx_src, const double* gy_src, bool check_connectivity, bool retained = false) {
         const int n = ny[0];
         CK(cudaMemsetAsync(flags.p, 0, 4 * sizeof(int), L.s));
         int* fl = flags.as<int>();
-        L.run(KC_SMALL, 0, [&] { k_import_planes<<<cdiv(plane(0), 256), 256, 0, L.s>>>(gx_src, gy_src, n, pitch[0], gx[0].as<double>(), gy[0].as<double>(), fl); });
+        if (retained) {
+            CK(cudaMemcpyAsync(gx[0].p, gx_src, plane(0) * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
+            CK(cudaMemcpyAsync(gy[0].p, gy_src, plane(0) * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
+            check_connectivity = false;
+        } else {
+            L.run(KC_SMALL, 0, [&] { k_import_planes<<<cdiv(plane(0), 256), 256, 0, L.s>>>(gx_src, gy_src, n, pitch[0], gx[0].as<double>(), gy[0].as<double>(), fl); });
+        }
         for (int l = 0; l < nlev; ++l) {
             const unsigned g = cdiv(plane(l), 256);
             L.run(KC_SMALL, 0, [&] { k_scale_nodes<<<g, 256, 0, L.s>>>(ny[l], nx[l], pitch[l], gx[l].as<double>(), gy[l].as<double>(), sc[l].as<float2>(), l == 0 ? fl + 1 : nullptr); });
@@ -370,7 +380,7 @@ struct Work {
     DevBuf rl[MAX_LEVELS], ya[MAX_LEVELS], zb[MAX_LEVELS];  // levels >= 1: residual, scaled iterate, correction
     CUtensorMap m_r[2], m_y0, m_z, m_p[2], m_q;
     CUtensorMap m_rl[MAX_LEVELS], m_ya[MAX_LEVELS], m_ec[MAX_LEVELS];  // m_ec[l]: zb[l] as the coarse box of level l-1
-    DevBuf scal, xport, xown, iact;
+    DevBuf scal, xport, xown, iact, src;  // src: port index each right-hand side of the batch is the source of
     PcgScalars s{};
     int* h_nact = nullptr;                           // pinned (g_pinned: not owned)
     double* h_relres = nullptr;                      // pinned, Bmax
@@ -403,6 +413,7 @@ struct Work {
         s.n_active = iact.as<int>() + B;
         xport.alloc((size_t)B * std::max(qmax, 1) * sizeof(double));
         xown.alloc((size_t)B * sizeof(double));
+        src.alloc((size_t)B * sizeof(int));
         char* hp = static_cast<char*>(g_pinned.get(64 + (size_t)B * sizeof(double)));
         if (!hp) throw StatusFail{PDN_E_NOMEM, "pinned host allocation failed"};
         h_nact = reinterpret_cast<int*>(hp);
@@ -510,11 +521,14 @@ void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Smoother& sm, int B,
     }
 }
 
-// Solve L_t x_b = e_{port src0+b} - 1/n^2 for b in [0, B) by multigrid-preconditioned CG and leave
-//   TSV-source batch     : ZT[src0+b][k] = x_b[port k] - mean(x_b)      for all ports k of the tier
-//   terminal-source batch: zdiag[src0+b-ntsv] = x_b[own node] - mean(x_b)
-int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts& T, const Smoother& sm, int src0, int B,
-                bool terminal, double rtol, int max_iter) {
+// Solve L_t x_b = e_{port src[b]} - 1/n^2 for b in [0, B) by multigrid-preconditioned CG and leave
+//   TSV-source batch     : ZT[src[b]][k] = x_b[port k] - mean(x_b)      for all ports k of the tier
+//   terminal-source batch: zdiag[src[b]-ntsv] = x_b[own node] - mean(x_b)
+int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts& T, const Smoother& sm, const int* src_ports,
+                int B, bool terminal, double rtol, int max_iter) {
+    const int src0 = src_ports[0];
+    CK(cudaMemcpyAsync(W.src.p, src_ports, (size_t)B * sizeof(int), cudaMemcpyHostToDevice, L.s));
+    const int* src = W.src.as<int>();
     const int n = H.ny[0];
     const size_t n2 = (size_t)n * n, plane = H.plane(0);
     const double V = (double)B * n2 * 8.0;
@@ -522,7 +536,7 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     const int ngather = terminal ? 0 : T.q;
     int cur_r = 0, cur_p = 0;
     L.run(KC_SMALL, 0, [&] { k_pcg_init<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B); });
-    L.run(KC_SMALL, V, [&] { k_init_rhs<<<dim3(cdiv(plane, 256), B), 256, 0, L.s>>>(W.r[0].as<double>(), n, H.pitch[0], plane, 1.0 / (double)n2, node, src0, B); });
+    L.run(KC_SMALL, V, [&] { k_init_rhs<<<dim3(cdiv(plane, 256), B), 256, 0, L.s>>>(W.r[0].as<double>(), n, H.pitch[0], plane, 1.0 / (double)n2, node, src, B); });
     if (terminal) CK(cudaMemsetAsync(W.xown.p, 0, (size_t)B * sizeof(double), L.s));
     else CK(cudaMemsetAsync(W.xport.p, 0, (size_t)B * ngather * sizeof(double), L.s));
     int nact = B;  // right-hand sides still iterating
@@ -536,7 +550,7 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
         launch_pq3(L, 4.0 * V * nact / B, H.lev[0], sm, B, W.m_z, W.m_p[cur_p], W.s.beta, W.p[cur_p ^ 1].as<double>(), W.q.as<double>(), W.s.pq, W.s.sump, W.s.active);
         cur_p ^= 1;
         L.run(KC_SMALL, 0, [&] { k_scal_alpha<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, 1.0 / (double)n2); });
-        L.run(KC_SMALL, 0, [&] { k_xport<<<dim3(cdiv(std::max(ngather, 1), 128), B), 128, 0, L.s>>>(W.p[cur_p].as<double>(), plane, W.s.alpha, node, ngather, src0, W.xport.as<double>(), W.xown.as<double>(), B); });
+        L.run(KC_SMALL, 0, [&] { k_xport<<<dim3(cdiv(std::max(ngather, 1), 128), B), 128, 0, L.s>>>(W.p[cur_p].as<double>(), plane, W.s.alpha, node, ngather, src, W.xport.as<double>(), W.xown.as<double>(), B); });
         ++it;
         bool done = false;
         auto check = [&] {
@@ -569,9 +583,9 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     }
     // results + statistics
     if (terminal)
-        L.run(KC_SMALL, 0, [&] { k_finish_term<<<cdiv(B, 128), 128, 0, L.s>>>(W.xown.as<double>(), W.s.xmean, T.zdiag.as<double>() + (src0 - T.ntsv), B); });
+        L.run(KC_SMALL, 0, [&] { k_finish_term<<<cdiv(B, 128), 128, 0, L.s>>>(W.xown.as<double>(), W.s.xmean, src, T.ntsv, T.zdiag.as<double>(), B); });
     else
-        L.run(KC_SMALL, 0, [&] { k_finish_tsv<<<dim3(cdiv(ngather, 128), B), 128, 0, L.s>>>(W.xport.as<double>(), W.s.xmean, ngather, T.ZT.as<double>() + (size_t)src0 * T.q, B); });
+        L.run(KC_SMALL, 0, [&] { k_finish_tsv<<<dim3(cdiv(ngather, 128), B), 128, 0, L.s>>>(W.xport.as<double>(), W.s.xmean, ngather, src, T.ZT.as<double>(), B); });
     CK(cudaMemcpyAsync(W.h_relres, W.s.relres, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, L.s));
     CK(cudaStreamSynchronize(L.s));
     double worst = 0.0;
@@ -722,6 +736,109 @@ int recombine(pdn_ctx* c, Launcher& L) {
     return h_fail ? PDN_E_NUMERIC : PDN_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Host-side pieces shared by pdn_create and pdn_update_tsvs.
+
+// Validates a TSV list and splits it per interface (sites as pitched offsets y*pitch + x, in list order).
+void parse_tsvs(int d, int n, int n_tsv, const pdn_tsv* tsvs, std::vector<std::vector<int>>& site,
+                std::vector<std::vector<double>>& rt) {
+    site.assign(d - 1, {});
+    rt.assign(d - 1, {});
+    std::vector<std::set<int>> seen(d - 1);
+    for (int k = 0; k < n_tsv; ++k) {
+        const pdn_tsv& t = tsvs[k];
+        if (t.iface < 0 || t.iface >= d - 1) throw StatusFail{PDN_E_ARG, "TSV interface out of range"};
+        if (t.y < 0 || t.y >= n || t.x < 0 || t.x >= n) throw StatusFail{PDN_E_ARG, "TSV site out of range"};
+        if (!(t.r_ohm > 0.0) || !std::isfinite(t.r_ohm)) throw StatusFail{PDN_E_ARG, "TSV resistance must be positive and finite"};
+        const int id = t.y * pitch_of(n) + t.x;  // pitched offset (port.cuh / pcg.cuh index vectors with it)
+        if (!seen[t.iface].insert(id).second) throw StatusFail{PDN_E_ARG, "duplicate TSV site inside one interface"};
+        site[t.iface].push_back(id);
+        rt[t.iface].push_back(t.r_ohm);
+    }
+    for (int i = 0; i < d - 1; ++i)
+        if (site[i].empty()) throw StatusFail{PDN_E_ARG, "an interface has no TSV"};
+}
+
+// Port list of tier t:  [lower ends of interface t-1] ++ [upper ends of interface t] ++ [terminals].
+void tier_port_list(const pdn_ctx* c, int t, const std::vector<std::vector<int>>& site, std::vector<int>& node, int& ntsv) {
+    node.clear();
+    if (t > 0) node.insert(node.end(), site[t - 1].begin(), site[t - 1].end());
+    if (t < c->d - 1) node.insert(node.end(), site[t].begin(), site[t].end());
+    ntsv = (int)node.size();
+    if (t == 0) node.insert(node.end(), c->bump_id.begin(), c->bump_id.end());
+    if (t == c->d - 1) node.insert(node.end(), c->load_id.begin(), c->load_id.end());
+}
+
+// Right-hand sides per batch: what fits in 60 % of the free device memory (pool blocks count as free).
+int pick_batch(const Hierarchy& H, int want, const pdn_opts& o) {
+    if (H.nlev <= 1) return std::max(want, 1);
+    size_t free_b = 0, total_b = 0;
+    CK(cudaMemGetInfo(&free_b, &total_b));
+    free_b += g_pool.cached_bytes();
+    const size_t per = Work::bytes_per_rhs(H) + (size_t)want * 8 + 128;
+    const size_t fit = std::max<size_t>(1, (size_t)(0.6 * (double)free_b) / per);
+    int B = (int)std::min<size_t>({(size_t)std::max(want, 1), fit, (size_t)1024});
+    if (o.rhs_batch > 0) B = std::min(B, o.rhs_batch);
+    return B;
+}
+
+// S1 of one tier whose hierarchy H has just been built: fills rows `tsv_src` of ZT (each against all ports of
+// the tier) and, if `terminals`, zdiag.  Meshes with n <= 4 and uniform tiers (Eq. 3) are reduced whole.
+int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPorts& T, const std::vector<int>& tsv_src,
+                bool terminals) {
+    const pdn_opts& o = c->opts;
+    const int n = c->n;
+    if (H.nlev == 1) {
+        L.run(KC_SMALL, 0, [&] { k_direct_small<<<T.q, 64, 0, L.s>>>(H.pinv.as<double>(), n, H.pitch[0], n * n, T.d_node.as<int>(), T.ntsv, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
+        return PDN_OK;
+    }
+    if (!(o.flags & PDN_NO_UNIFORM_FAST_PATH)) {
+        // uniform tier: Eq. (3) of the paper as two dense contractions + a gather (uniform.cuh)
+        int* fl = H.flags.as<int>();
+        CK(cudaMemsetAsync(fl, 0, sizeof(int), L.s));
+        L.run(KC_SMALL, 0, [&] { k_uniform_check<<<cdiv(H.plane(0), 256), 256, 0, L.s>>>(n, H.pitch[0], H.gx[0].as<double>(), H.gy[0].as<double>(), fl); });
+        int h_flag = 1;
+        double g0[2] = {0.0, 0.0};
+        CK(cudaMemcpyAsync(&h_flag, fl, sizeof(int), cudaMemcpyDeviceToHost, L.s));
+        CK(cudaMemcpyAsync(&g0[0], H.gx[0].p, sizeof(double), cudaMemcpyDeviceToHost, L.s));
+        CK(cudaMemcpyAsync(&g0[1], H.gy[0].p, sizeof(double), cudaMemcpyDeviceToHost, L.s));
+        CK(cudaStreamSynchronize(L.s));
+        if (h_flag == 0 && g0[0] > 0.0 && g0[1] > 0.0) {
+            const size_t nn = (size_t)n * n;
+            DevBuf Cm, Wm, T1, Gt;
+            Cm.alloc(2 * nn * sizeof(double)); Wm.alloc(nn * sizeof(double));
+            T1.alloc(2 * nn * sizeof(double)); Gt.alloc(4 * nn * sizeof(double));
+            L.run(KC_SMALL, 0, [&] { k_cos_matrix<<<cdiv(2 * nn, 256), 256, 0, L.s>>>(n, Cm.as<double>()); });
+            L.run(KC_SMALL, 0, [&] { k_spectral_weights<<<cdiv(nn, 256), 256, 0, L.s>>>(n, g0[0], g0[1], Wm.as<double>()); });
+            // T[a][s] = sum_b W[a][b] C[s][b]  (n x 2n);  G[t][s] = sum_a C[t][a] T[a][s]  (2n x 2n)
+            gemm(L, n, 2 * n, n, 1.0, Wm.as<double>(), n, 1, Cm.as<double>(), 1, n, 0.0, T1.as<double>(), 2 * n);
+            gemm(L, 2 * n, 2 * n, n, 1.0, Cm.as<double>(), n, 1, T1.as<double>(), 2 * n, 1, 0.0, Gt.as<double>(), 2 * n);
+            L.run(KC_SMALL, 0, [&] { k_uniform_gather<<<dim3(cdiv(T.q, 128), T.ntsv + 1), 128, 0, L.s>>>(Gt.as<double>(), n, H.pitch[0], T.d_node.as<int>(), T.ntsv, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
+            CK(cudaStreamSynchronize(L.s));  // the table buffers go back to the pool here
+            c->stats.n_uniform_tiers++;
+            return PDN_OK;
+        }
+    }
+    // Smoothing interval [2/ratio, 2] of the Chebyshev polynomial.  With 2x2 aggregation the coarse grid
+    // takes fewer modes off the smoother the more anisotropic the tier is, so the interval widens with
+    // the anisotropy a: ratio = 3 + a (measured: a = 1 -> 4, a = 3 -> 6).
+    const double ratio = o.cheb_ratio > 1.0 ? o.cheb_ratio : std::min(10.0, 3.0 + H.anisotropy);
+    const int G = getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 32;
+    const Smoother ch{make_cheb_roots(o.nu, ratio), make_cheb_roots(o.nu, ratio), G};
+    // bump / load sources deliver only their own diagonal, whose CG error is the square of the energy-norm error
+    const double rtol_term = std::max(o.rtol, std::min(1e-5, std::sqrt(o.rtol) / 3.0));
+    int status = PDN_OK;
+    for (size_t s0 = 0; s0 < tsv_src.size() && status == PDN_OK; s0 += Bmax)
+        status = solve_batch(c, L, H, W, T, ch, tsv_src.data() + s0, (int)std::min<size_t>(Bmax, tsv_src.size() - s0), false, o.rtol, o.max_iter);
+    if (terminals) {
+        std::vector<int> term(T.nterm);
+        for (int k = 0; k < T.nterm; ++k) term[k] = T.ntsv + k;
+        for (size_t s0 = 0; s0 < term.size() && status == PDN_OK; s0 += Bmax)
+            status = solve_batch(c, L, H, W, T, ch, term.data() + s0, (int)std::min<size_t>(Bmax, term.size() - s0), true, rtol_term, o.max_iter);
+    }
+    return status;
+}
+
 }  // namespace
 
 // ================================================================================================
@@ -785,33 +902,17 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         c->stream = (cudaStream_t)o.cuda_stream;
         c->time_kernels = (o.flags & PDN_TIME_KERNELS) != 0;
         // ---- host-side validation and port lists
+        parse_tsvs(d, n, n_tsv, tsvs, c->site, c->rt);
         c->p.assign(d - 1, 0);
-        c->rt.assign(d - 1, {});
-        std::vector<std::vector<int>> site(d - 1);
-        std::vector<std::set<int>> seen(d - 1);
-        for (int k = 0; k < n_tsv; ++k) {
-            const pdn_tsv& t = tsvs[k];
-            if (t.iface < 0 || t.iface >= d - 1) throw StatusFail{PDN_E_ARG, "TSV interface out of range"};
-            if (t.y < 0 || t.y >= n || t.x < 0 || t.x >= n) throw StatusFail{PDN_E_ARG, "TSV site out of range"};
-            if (!(t.r_ohm > 0.0) || !std::isfinite(t.r_ohm)) throw StatusFail{PDN_E_ARG, "TSV resistance must be positive and finite"};
-            const int id = t.y * pitch_of(n) + t.x;  // pitched offset (port.cuh / pcg.cuh index vectors with it)
-            if (!seen[t.iface].insert(id).second) throw StatusFail{PDN_E_ARG, "duplicate TSV site inside one interface"};
-            site[t.iface].push_back(id);
-            c->rt[t.iface].push_back(t.r_ohm);
-        }
-        for (int i = 0; i < d - 1; ++i) {
-            c->p[i] = (int)site[i].size();
-            if (c->p[i] == 0) throw StatusFail{PDN_E_ARG, "an interface has no TSV"};
-        }
+        for (int i = 0; i < d - 1; ++i) c->p[i] = (int)c->site[i].size();
         auto check_sites = [&](const pdn_site* s, int cnt, std::vector<int>& ids) {
             for (int k = 0; k < cnt; ++k) {
                 if (s[k].y < 0 || s[k].y >= n || s[k].x < 0 || s[k].x >= n) throw StatusFail{PDN_E_ARG, "bump/load site out of range"};
                 ids.push_back(s[k].y * pitch_of(n) + s[k].x);
             }
         };
-        std::vector<int> bump_id, load_id;
-        check_sites(bumps, n_bumps, bump_id);
-        check_sites(loads, n_loads, load_id);
+        check_sites(bumps, n_bumps, c->bump_id);
+        check_sites(loads, n_loads, c->load_id);
 
         Launcher L{c, c->stream};
         cudaEvent_t ev[4];
@@ -822,11 +923,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         int qmax = 0;
         for (int t = 0; t < d; ++t) {
             TierPorts& T = c->tiers[t];
-            if (t > 0) T.node.insert(T.node.end(), site[t - 1].begin(), site[t - 1].end());
-            if (t < d - 1) T.node.insert(T.node.end(), site[t].begin(), site[t].end());
-            T.ntsv = (int)T.node.size();
-            if (t == 0) T.node.insert(T.node.end(), bump_id.begin(), bump_id.end());
-            if (t == d - 1) T.node.insert(T.node.end(), load_id.begin(), load_id.end());
+            tier_port_list(c, t, c->site, T.node, T.ntsv);
             T.q = (int)T.node.size();
             T.nterm = T.q - T.ntsv;
             T.d_node.alloc((size_t)T.q * sizeof(int));
@@ -844,20 +941,9 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         c->stats.n_levels = H.nlev;
         DevBuf stage;  // staging for host-resident planes
         if (o.flags & PDN_TIERS_ON_HOST) stage.alloc((size_t)2 * n * n * sizeof(double));
-        int Bmax = qmax;
-        if (H.nlev > 1) {
-            size_t free_b = 0, total_b = 0;
-            CK(cudaMemGetInfo(&free_b, &total_b));
-            free_b += g_pool.cached_bytes();  // blocks kept by the pool are ours to reuse
-            const size_t per = Work::bytes_per_rhs(H) + (size_t)qmax * 8 + 128;
-            const size_t fit = std::max<size_t>(1, (size_t)(0.6 * (double)free_b) / per);
-            Bmax = (int)std::min<size_t>({(size_t)qmax, fit, (size_t)1024});
-            if (o.rhs_batch > 0) Bmax = std::min(Bmax, o.rhs_batch);
-        }
+        const int Bmax = pick_batch(H, qmax, o);
         Work W;
         if (H.nlev > 1) W.allocate(H, Bmax, qmax);
-        const int G = getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 32;
-        const double rtol_term = std::max(o.rtol, std::min(1e-5, std::sqrt(o.rtol) / 3.0));
         float ms_up = 0.f;
         for (int t = 0; t < d && status == PDN_OK; ++t) {
             TierPorts& T = c->tiers[t];
@@ -870,52 +956,21 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
                 gx = sg; gy = sg + (size_t)n * n;
             }
             status = H.build(L, gx, gy, !(o.flags & PDN_SKIP_CONNECTIVITY_CHECK));
+            if (status == PDN_OK) {  // keep the sanitised planes: pdn_update_tsvs rebuilds the hierarchy from them
+                T.gx0.alloc(H.plane(0) * sizeof(double));
+                T.gy0.alloc(H.plane(0) * sizeof(double));
+                CK(cudaMemcpyAsync(T.gx0.p, H.gx[0].p, H.plane(0) * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
+                CK(cudaMemcpyAsync(T.gy0.p, H.gy[0].p, H.plane(0) * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
+            }
             CK(cudaEventRecord(ev[2], L.s));
             CK(cudaEventSynchronize(ev[2]));
             float ms = 0.f;
             CK(cudaEventElapsedTime(&ms, ev[1], ev[2]));
             ms_up += ms;
             if (status != PDN_OK) { g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status); break; }
-            // Smoothing interval [2/ratio, 2] of the Chebyshev polynomial.  With 2x2 aggregation the coarse grid
-            // takes fewer modes off the smoother the more anisotropic the tier is, so the interval widens with
-            // the anisotropy a: ratio = 3 + a (measured: a = 1 -> 4, a = 3 -> 6).
-            const double ratio = o.cheb_ratio > 1.0 ? o.cheb_ratio : std::min(10.0, 3.0 + H.anisotropy);
-            const Smoother ch{make_cheb_roots(o.nu, ratio), make_cheb_roots(o.nu, ratio), G};
-            if (H.nlev == 1) {
-                L.run(KC_SMALL, 0, [&] { k_direct_small<<<T.q, 64, 0, L.s>>>(H.pinv.as<double>(), n, H.pitch[0], n * n, T.d_node.as<int>(), T.ntsv, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
-                continue;
-            }
-            if (!(o.flags & PDN_NO_UNIFORM_FAST_PATH)) {
-                // uniform tier: Eq. (3) of the paper as two dense contractions + a gather (uniform.cuh)
-                int* fl = H.flags.as<int>();
-                CK(cudaMemsetAsync(fl, 0, sizeof(int), L.s));
-                L.run(KC_SMALL, 0, [&] { k_uniform_check<<<cdiv(H.plane(0), 256), 256, 0, L.s>>>(n, H.pitch[0], H.gx[0].as<double>(), H.gy[0].as<double>(), fl); });
-                int h_flag = 1;
-                double g0[2] = {0.0, 0.0};
-                CK(cudaMemcpyAsync(&h_flag, fl, sizeof(int), cudaMemcpyDeviceToHost, L.s));
-                CK(cudaMemcpyAsync(&g0[0], H.gx[0].p, sizeof(double), cudaMemcpyDeviceToHost, L.s));
-                CK(cudaMemcpyAsync(&g0[1], H.gy[0].p, sizeof(double), cudaMemcpyDeviceToHost, L.s));
-                CK(cudaStreamSynchronize(L.s));
-                if (h_flag == 0 && g0[0] > 0.0 && g0[1] > 0.0) {
-                    const size_t nn = (size_t)n * n;
-                    DevBuf Cm, Wm, T1, Gt;
-                    Cm.alloc(2 * nn * sizeof(double)); Wm.alloc(nn * sizeof(double));
-                    T1.alloc(2 * nn * sizeof(double)); Gt.alloc(4 * nn * sizeof(double));
-                    L.run(KC_SMALL, 0, [&] { k_cos_matrix<<<cdiv(2 * nn, 256), 256, 0, L.s>>>(n, Cm.as<double>()); });
-                    L.run(KC_SMALL, 0, [&] { k_spectral_weights<<<cdiv(nn, 256), 256, 0, L.s>>>(n, g0[0], g0[1], Wm.as<double>()); });
-                    // T[a][s] = sum_b W[a][b] C[s][b]  (n x 2n);  G[t][s] = sum_a C[t][a] T[a][s]  (2n x 2n)
-                    gemm(L, n, 2 * n, n, 1.0, Wm.as<double>(), n, 1, Cm.as<double>(), 1, n, 0.0, T1.as<double>(), 2 * n);
-                    gemm(L, 2 * n, 2 * n, n, 1.0, Cm.as<double>(), n, 1, T1.as<double>(), 2 * n, 1, 0.0, Gt.as<double>(), 2 * n);
-                    L.run(KC_SMALL, 0, [&] { k_uniform_gather<<<dim3(cdiv(T.q, 128), T.ntsv + 1), 128, 0, L.s>>>(Gt.as<double>(), n, H.pitch[0], T.d_node.as<int>(), T.ntsv, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
-                    CK(cudaStreamSynchronize(L.s));  // the table buffers go back to the pool here
-                    c->stats.n_uniform_tiers++;
-                    continue;
-                }
-            }
-            for (int s0 = 0; s0 < T.ntsv && status == PDN_OK; s0 += Bmax)
-                status = solve_batch(c, L, H, W, T, ch, s0, std::min(Bmax, T.ntsv - s0), false, o.rtol, o.max_iter);
-            for (int s0 = T.ntsv; s0 < T.q && status == PDN_OK; s0 += Bmax)
-                status = solve_batch(c, L, H, W, T, ch, s0, std::min(Bmax, T.q - s0), true, rtol_term, o.max_iter);
+            std::vector<int> all_tsv(T.ntsv);
+            for (int k = 0; k < T.ntsv; ++k) all_tsv[k] = k;
+            status = reduce_tier(c, L, H, W, Bmax, T, all_tsv, true);
             if (status != PDN_OK) g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status);
         }
         CK(cudaEventRecord(ev[2], L.s));
@@ -951,6 +1006,119 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
     }
     *out = c;
     return PDN_OK;
+}
+
+// NEXT-2: TSV re-planning.  The new TSV list is diffed against the current one per interface
+// by site.  A kept site keeps its rows / columns of the tier port matrices (its resistance may change freely:
+// it only enters K); a removed site drops them; an added site costs ONE port solve on each of its two tiers,
+// whose solution gives the new row and -- by symmetry of L^+ -- the new column.  C is then re-assembled and
+// re-factored (milliseconds).
+int pdn_update_tsvs(pdn_ctx* ctx, int32_t n_tsv, const pdn_tsv* tsvs) {
+    if (!ctx || !tsvs || n_tsv < 1) return fail_arg("null context / TSV list or empty list");
+    pdn_ctx* c = ctx;
+    const int d = c->d, n = c->n;
+    int status = PDN_OK;
+    try {
+        std::vector<std::vector<int>> nsite;
+        std::vector<std::vector<double>> nrt;
+        parse_tsvs(d, n, n_tsv, tsvs, nsite, nrt);
+        Launcher L{c, c->stream};
+        cudaEvent_t ev[3];
+        for (auto& e : ev) CK(cudaEventCreate(&e));
+        CK(cudaEventRecord(ev[0], L.s));
+        // old index -> new index per interface (-1 = removed)
+        std::vector<std::vector<int>> o2n(d - 1);
+        for (int i = 0; i < d - 1; ++i) {
+            std::map<int, int> where;
+            for (size_t k = 0; k < nsite[i].size(); ++k) where[nsite[i][k]] = (int)k;
+            o2n[i].assign(c->site[i].size(), -1);
+            for (size_t k = 0; k < c->site[i].size(); ++k) {
+                auto it = where.find(c->site[i][k]);
+                if (it != where.end()) o2n[i][k] = it->second;
+            }
+        }
+        Hierarchy H;
+        bool h_ready = false;
+        int64_t new_solves = 0;
+        for (int t = 0; t < d && status == PDN_OK; ++t) {
+            TierPorts& T = c->tiers[t];
+            std::vector<int> node_n;
+            int ntsv_n = 0;
+            tier_port_list(c, t, nsite, node_n, ntsv_n);
+            if (node_n == T.node) continue;  // same sites in the same order: Z_t is unchanged
+            const int q_o = T.q, ntsv_o = T.ntsv, q_n = (int)node_n.size();
+            const int plo_o = t > 0 ? (int)c->site[t - 1].size() : 0, plo_n = t > 0 ? (int)nsite[t - 1].size() : 0;
+            std::vector<int> cmap(q_o, -1);
+            std::vector<unsigned char> is_added(std::max(ntsv_n, 1), 1);
+            for (int k = 0; k < ntsv_o; ++k) {
+                int kn = -1;
+                if (k < plo_o) kn = o2n[t - 1][k];
+                else { const int m = o2n[t][k - plo_o]; kn = m < 0 ? -1 : plo_n + m; }
+                cmap[k] = kn;
+                if (kn >= 0) is_added[kn] = 0;
+            }
+            for (int k = ntsv_o; k < q_o; ++k) cmap[k] = ntsv_n + (k - ntsv_o);  // terminals keep their order
+            std::vector<int> added;
+            for (int k = 0; k < ntsv_n; ++k) if (is_added[k]) added.push_back(k);
+            DevBuf d_cmap, d_added, d_isadd, ZTn;
+            d_cmap.alloc((size_t)q_o * sizeof(int));
+            CK(cudaMemcpyAsync(d_cmap.p, cmap.data(), (size_t)q_o * sizeof(int), cudaMemcpyHostToDevice, L.s));
+            ZTn.alloc((size_t)ntsv_n * q_n * sizeof(double));
+            CK(cudaMemsetAsync(ZTn.p, 0, (size_t)ntsv_n * q_n * sizeof(double), L.s));
+            L.run(KC_SMALL, 0, [&] { k_remap_zt<<<dim3(cdiv(q_o, 128), ntsv_o), 128, 0, L.s>>>(T.ZT.as<double>(), ntsv_o, q_o, d_cmap.as<int>(), d_cmap.as<int>(), ZTn.as<double>(), q_n); });
+            CK(cudaStreamSynchronize(L.s));  // cmap (host vector) and the old ZT are released below
+            T.ZT = std::move(ZTn);
+            T.node = node_n; T.ntsv = ntsv_n; T.q = q_n; T.nterm = q_n - ntsv_n;
+            T.d_node.alloc((size_t)q_n * sizeof(int));
+            CK(cudaMemcpyAsync(T.d_node.p, T.node.data(), (size_t)q_n * sizeof(int), cudaMemcpyHostToDevice, L.s));
+            if (!added.empty()) {
+                if (!h_ready) { H.allocate(n); h_ready = true; }
+                status = H.build(L, T.gx0.as<double>(), T.gy0.as<double>(), false, true);
+                if (status != PDN_OK) break;
+                const int Bmax = pick_batch(H, (int)added.size(), c->opts);
+                Work W;
+                if (H.nlev > 1) W.allocate(H, Bmax, q_n);
+                status = reduce_tier(c, L, H, W, Bmax, T, added, false);
+                if (status != PDN_OK) { g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status); break; }
+                new_solves += (int64_t)added.size();
+                d_added.alloc(added.size() * sizeof(int));
+                d_isadd.alloc((size_t)ntsv_n);
+                CK(cudaMemcpyAsync(d_added.p, added.data(), added.size() * sizeof(int), cudaMemcpyHostToDevice, L.s));
+                CK(cudaMemcpyAsync(d_isadd.p, is_added.data(), (size_t)ntsv_n, cudaMemcpyHostToDevice, L.s));
+                L.run(KC_SMALL, 0, [&] { k_mirror_added<<<dim3(cdiv(added.size(), 128), ntsv_n), 128, 0, L.s>>>(T.ZT.as<double>(), ntsv_n, q_n, d_added.as<int>(), (int)added.size(), d_isadd.as<unsigned char>()); });
+                CK(cudaStreamSynchronize(L.s));
+            }
+        }
+        CK(cudaEventRecord(ev[1], L.s));
+        if (status == PDN_OK) {
+            c->site = nsite;
+            c->rt = nrt;
+            c->stats.n_ports_total = 0;
+            for (int i = 0; i < d - 1; ++i) c->p[i] = (int)nsite[i].size();
+            for (int t = 0; t < d; ++t) c->stats.n_ports_total += c->tiers[t].q;
+            status = recombine(c, L);
+            if (status != PDN_OK) g_last_error = pdn_strerror(status);
+        }
+        CK(cudaEventRecord(ev[2], L.s));
+        CK(cudaStreamSynchronize(L.s));
+        L.resolve();
+        float ms_s1 = 0.f, ms_dense = 0.f;
+        CK(cudaEventElapsedTime(&ms_s1, ev[0], ev[1]));
+        CK(cudaEventElapsedTime(&ms_dense, ev[1], ev[2]));
+        c->stats.ms_update_stencil = ms_s1; c->stats.ms_update_dense = ms_dense; c->stats.update_solves = new_solves;
+        for (auto& e : ev) cudaEventDestroy(e);
+    } catch (const CudaFail& f) {
+        g_last_error = std::string(f.what) + ": " + cudaGetErrorString(f.e);
+        cudaGetLastError();
+        status = f.e == cudaErrorMemoryAllocation ? PDN_E_NOMEM : PDN_E_CUDA;
+    } catch (const StatusFail& f) {
+        g_last_error = f.msg;
+        status = f.status;
+    } catch (const std::bad_alloc&) {
+        g_last_error = "host allocation failed";
+        status = PDN_E_NOMEM;
+    }
+    return status;
 }
 
 static int reff_device(pdn_ctx* ctx, int64_t n_pairs, const int32_t* bi, const int32_t* li, double* out) {

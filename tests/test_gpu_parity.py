@@ -216,6 +216,80 @@ def test_port_matrix_of_a_nonuniform_tier_matches_the_dense_pseudo_inverse():
     pdn.close()
 
 
+@pytest.mark.parametrize("seed,d,n,p,kw", [
+    (41, 2, 37, 9, {}),
+    (42, 3, 70, 12, dict(drop=0.03, aniso=2.0)),
+    (43, 4, 24, 6, {}),
+])
+def test_tsv_replanning_matches_a_fresh_context_and_the_oracle(seed, d, n, p, kw):
+    """pdn_update_tsvs (NEXT-2): remove, add, move TSVs and change resistances; the updated context must give
+    what a context created on the new network gives, and both must match the oracle of the new network."""
+    from oracle.reff_oracle import Oracle
+    from paper_2607_05818_b200 import Pdn
+    torch = torch_cuda()
+    net = P.make_random(seed, d=d, n=n, p=p, m=5, nl=6, **kw)
+    rng = np.random.default_rng(seed)
+    pdn = Pdn.from_network(net, device="cuda:0", rtol=1e-10)
+
+    def reff(obj):
+        out = torch.empty(net.m * net.nl, dtype=torch.float64, device="cuda:0")
+        obj.reff(out)
+        return out.cpu().numpy().reshape(net.m, net.nl)
+
+    before = reff(pdn)
+    for step in range(3):
+        for i in range(d - 1):
+            s, r = net.tsv_site[i].copy(), net.tsv_r[i].copy()
+            if step == 0:      # drop two sites, add three new ones in the middle of the list, rescale one resistance
+                keep = np.ones(len(s), bool); keep[rng.choice(len(s), 2, replace=False)] = False
+                s, r = s[keep], r[keep]
+                new = [x for x in P._distinct_sites(rng, n, 8).tolist() if x not in s.tolist()][:3]
+                s = np.vstack([s[:2], np.array(new, dtype=np.int32), s[2:]]); r = np.concatenate([r[:2], rng.uniform(0.02, 0.2, 3), r[2:]])
+                r[0] *= 3.0
+            elif step == 1:    # permute the list and change every resistance: no new solves
+                perm = rng.permutation(len(s)); s, r = s[perm], r[perm] * rng.uniform(0.5, 2.0, len(s))
+            else:              # interface 0 only: replace everything but one site
+                if i == 0:
+                    new = [x for x in P._distinct_sites(rng, n, 10).tolist() if x not in s.tolist()][:4]
+                    s = np.vstack([s[:1], np.array(new, dtype=np.int32)]); r = np.concatenate([r[:1], rng.uniform(0.02, 0.2, 4)])
+            net.tsv_site[i], net.tsv_r[i] = np.ascontiguousarray(s, dtype=np.int32), r
+        pdn.update_tsvs(net.tsv_site, net.tsv_r)
+        st = pdn.stats()
+        if step == 1:
+            assert st["update_solves"] == 0
+        got = reff(pdn)
+        fresh, _ = gpu_all_pairs(net, rtol=1e-10)
+        assert np.allclose(got, fresh, rtol=1e-8, atol=0)
+        check(got, Oracle(net).reff_all())
+    assert not np.allclose(got, before, rtol=1e-3)
+    # a bad list is refused and leaves the context usable
+    from paper_2607_05818_b200 import PdnError
+    with pytest.raises(PdnError):
+        pdn.update_tsvs([s[:0] for s in net.tsv_site], [r[:0] for r in net.tsv_r])
+    assert np.allclose(reff(pdn), got, rtol=1e-12, atol=0)
+    pdn.close()
+
+
+def test_tsv_replanning_on_uniform_and_tiny_tiers():
+    from oracle.reff_oracle import Oracle
+    from paper_2607_05818_b200 import Pdn
+    torch = torch_cuda()
+    for n in (4, 30):                      # n = 4: the mesh is its own coarsest level; n = 30: Eq. (3) fast path
+        rng = np.random.default_rng(n)
+        net = P.make_uniform(3, n, 0.7, 1.9, rt=0.05, tsv_sites=[P._distinct_sites(rng, n, 3) for _ in range(2)],
+                             bumps=P._distinct_sites(rng, n, 3), loads=P._distinct_sites(rng, n, 2))
+        pdn = Pdn.from_network(net, device="cuda:0")
+        net.tsv_site[1] = np.vstack([net.tsv_site[1][1:], [[n - 1, 0]]]).astype(np.int32)
+        if [n - 1, 0] in net.tsv_site[1][:-1].tolist():
+            net.tsv_site[1] = net.tsv_site[1][:-1]
+        net.tsv_r[1] = np.full(len(net.tsv_site[1]), 0.11)
+        pdn.update_tsvs(net.tsv_site, net.tsv_r)
+        out = torch.empty(net.m * net.nl, dtype=torch.float64, device="cuda:0")
+        pdn.reff(out)
+        check(out.cpu().numpy().reshape(net.m, net.nl), Oracle(net).reff_all())
+        pdn.close()
+
+
 def test_bump_on_tsv_site_and_shared_sites_between_interfaces():
     from oracle.reff_oracle import Oracle
     sites = [np.array([[2, 2], [5, 1]]), np.array([[2, 2], [0, 6]])]     # (2,2) used by both interfaces
