@@ -296,6 +296,35 @@ def run_cuda(a):
                      "classes": {k: {"ms": cls_ms[k], "GBps": (cls_by[k] / (cls_ms[k] * 1e-3) / 1e9) if cls_ms[k] > 0 else 0.0,
                                      "launches": int(cls_n[k])} for k in cls_ms}},
     }
+    if a.replan > 0:   # NEXT-2: move K TSVs per interface, time the update against a full re-creation
+        rng = np.random.default_rng([cfg, a.replan])
+        sites = [s_.copy() for s_ in net.tsv_site]
+        for i in range(net.d - 1):
+            taken = {tuple(x) for x in sites[i].tolist()}
+            k = 0
+            while k < min(a.replan, len(sites[i])):
+                cand = (int(rng.integers(0, net.n)), int(rng.integers(0, net.n)))
+                if cand not in taken:
+                    taken.add(cand)
+                    sites[i][k] = cand
+                    k += 1
+        pdn = Pdn(net.n, gx_d, gy_d, *args[1], flags=base_flags, rtol=a.rtol, nu=a.nu, rhs_batch=a.rhs_batch)
+        cur = [net.tsv_site, sites]
+        times = []
+        for rep in range(a.warmup + a.steps):      # alternate between the two plans
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            pdn.update_tsvs(cur[(rep + 1) % 2], net.tsv_r)
+            pdn.reff(out_d)
+            torch.cuda.synchronize()
+            if rep >= a.warmup:
+                times.append(time.perf_counter() - t0)
+        stu = pdn.stats()
+        pdn.close()
+        line["replan"] = {"tsvs_moved_per_interface": a.replan, "ms_per_update": 1e3 * float(np.mean(times)),
+                          "port_solves_per_update": int(stu["update_solves"]), "ms_solves": stu["ms_update_stencil"],
+                          "ms_refactor": stu["ms_update_dense"], "ms_full_step": ms / a.steps,
+                          "pairs_per_s": npairs / float(np.mean(times))}
     if not a.no_cpu_baseline:
         ot = OracleTimer(cfg)
         n, t = ot.sample(a.cpu_budget)
@@ -319,6 +348,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--uniform", action="store_true", help="uniform-tier variant of the workload (Eq. 3 fast path)")
     ap.add_argument("--no-fast-path", action="store_true", help="solve uniform tiers numerically too")
+    ap.add_argument("--replan", type=int, default=0, metavar="K",
+                    help="also time pdn_update_tsvs after moving K TSVs of every interface to new sites (NEXT-2)")
     ap.add_argument("--only-device", action="store_true", help="run only the device-resident steps (for ncu)")
     a = ap.parse_args()
     if a.impl == "reference":
