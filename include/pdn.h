@@ -54,6 +54,9 @@ enum {
     PDN_TIERS_ON_HOST = 1,  /* pdn_tier.gx / gy are HOST pointers (the library uploads them)            */
     PDN_SKIP_CONNECTIVITY_CHECK = 2,
     PDN_TIME_KERNELS = 4,   /* bracket every kernel launch with CUDA events (per-class timers in pdn_stats) */
+    PDN_TERMINAL_PAIRS = 16, /* also keep the bump-source / load-source rows of the port matrices (full tolerance,
+                               gathered at every port): needed by pdn_reff_same_side and pdn_load_voltages; costs
+                               about as much again as the bump / load part of pdn_create                        */
     PDN_NO_UNIFORM_FAST_PATH = 8 /* solve uniform tiers numerically too (default: a tier whose x-segments are all
                                equal and whose y-segments are all equal is reduced by the closed form, Eq. (3)) */
 };
@@ -150,6 +153,16 @@ int pdn_reff_host(pdn_ctx *ctx, int64_t n_pairs, const int32_t *bump_idx, const 
  * status may leave it half updated) the context must be destroyed. */
 int pdn_update_tsvs(pdn_ctx *ctx, int32_t n_tsv, const pdn_tsv *tsvs);
 
+/* Same-side pairs (context created with PDN_TERMINAL_PAIRS).  side 0: bumps, side 1: loads.  out: DEVICE fp64,
+ * nt*nt values (nt = n_bumps or n_loads), out[i*nt + j] = R_eff between terminals i and j of that side in the
+ * whole 3D network (0 on the diagonal). */
+int pdn_reff_same_side(pdn_ctx *ctx, int32_t side, double *out);
+
+/* Eq. (4): bump `bump` (index into the create-time list) is held at v_bump, load k draws
+ * i_load[k] (DEVICE, n_loads values, amperes); v_out[j] (DEVICE, n_loads values) receives the voltage of load j,
+ *   v_j = v_bump - 1/2 sum_k i_load[k] (R_{b,j} + R_{b,k} - R_{j,k}).   Needs PDN_TERMINAL_PAIRS. */
+int pdn_load_voltages(pdn_ctx *ctx, int32_t bump, const double *i_load, double v_bump, double *v_out);
+
 /* NULL-safe; frees all device and host memory of ctx. */
 void pdn_destroy(pdn_ctx *ctx);
 
@@ -167,8 +180,8 @@ int pdn_get_stats(const pdn_ctx *ctx, pdn_stats *out);
  * out (HOST, q*q doubles, row-major) receives Z_t = L_t^+ restricted to ports(t), where
  * ports(t) = [lower ends of interface t-1] ++ [upper ends of interface t] ++ [bumps if t = 0]
  * ++ [loads if t = d-1].  The intra-die effective resistance is R_jk = Z_jj + Z_kk - 2 Z_jk.
- * Entries between two bump/load ports other than the diagonal are not computed (NaN): the method
- * never needs them. */
+ * Entries between two bump/load ports other than the diagonal are not computed (NaN) unless the context was
+ * created with PDN_TERMINAL_PAIRS: the bump x load method never needs them. */
 int32_t pdn_port_count(const pdn_ctx *ctx, int32_t tier);
 int pdn_get_port_matrix(const pdn_ctx *ctx, int32_t tier, double *out);
 

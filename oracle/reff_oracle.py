@@ -23,11 +23,14 @@ forward/backward substitution, serial, ONE PAIR AT A TIME):
   4. per pair: rhs = e_b - e_l (grounded row dropped), v = solve(rhs), ONE step of iterative
      refinement (r = rhs - Gg v ; v += solve(r)), R = v_b - v_l  (v of the grounded node is 0).
   5. tiny graphs: `reff_dense_pinv` evaluates Eq. (2) literally with numpy.linalg.pinv.
+  6. `node_voltages` / `load_voltages`: the operating point behind Eq. (4) from KCL directly
+     (G v = i with the bump as the reference), for the same-side / voltage extension of the path.
 
 Pins (tests/test_oracle_pins.py, all independent of this file's arithmetic): series / parallel
 chains, n-segment line = n*r, 2x2 grid (3r/4 adjacent, r diagonal), Wu's closed form Eq. (3)
 PAPER.md:49 on uniform meshes, the separable 3D product-graph closed form, Foster's theorem,
-symmetry, triangle inequality, scaling, Rayleigh monotonicity, brute-force pinv on tiny graphs.
+symmetry, triangle inequality, scaling, Rayleigh monotonicity, brute-force pinv on tiny graphs; for the
+voltages: the series-chain closed form and the identity of Eq. (4) itself.
 """
 from __future__ import annotations
 
@@ -122,6 +125,36 @@ class Oracle:
         va = v[a] if a != g else 0.0
         vb = v[b] if b != g else 0.0
         return float(va - vb)
+
+    def node_voltages(self, src: int, v_src: float, sinks, currents) -> np.ndarray:
+        """Voltages at the `sinks` when node `src` is held at `v_src` and sink k draws `currents[k]` amperes out
+        of the network (which enter at `src`): the DC operating point the paper's Eq. (4)
+        expresses through effective resistances.  Computed here from its definition -- KCL, G v = i, one
+        grounded solve + one refinement step -- without any effective resistance."""
+        g = self.nn - 1
+        sinks = np.asarray(sinks, dtype=np.int64)
+        currents = np.asarray(currents, dtype=np.float64)
+        inj = np.zeros(self.nn)
+        np.add.at(inj, sinks, -currents)
+        inj[src] += currents.sum()
+        rhs = inj[:g]
+        v = self.lu.solve(rhs)
+        v += self.lu.solve(rhs - self.Gg @ v)
+        full = np.append(v, 0.0)                      # the grounded node sits at 0
+        return v_src + (full[sinks] - full[src])
+
+    def load_voltages(self, bump_idx: int, currents, v_bump: float) -> np.ndarray:
+        """Voltage of every load when bump `bump_idx` is the only supply (at v_bump) and load k draws currents[k]."""
+        return self.node_voltages(int(self.bump_id[bump_idx]), v_bump, self.load_id, currents)
+
+    def reff_same_side(self, side: int) -> np.ndarray:
+        """R_eff between all pairs of bumps (side 0) or loads (side 1), one pair at a time (Eq. 2)."""
+        ids = self.bump_id if side == 0 else self.load_id
+        out = np.zeros((ids.size, ids.size))
+        for i in range(ids.size):
+            for j in range(i + 1, ids.size):
+                out[i, j] = out[j, i] = self.reff_nodes(int(ids[i]), int(ids[j]))
+        return out
 
     def reff(self, bump_idx: int, load_idx: int) -> float:
         return self.reff_nodes(int(self.bump_id[bump_idx]), int(self.load_id[load_idx]))

@@ -19,6 +19,7 @@ PDN_TIERS_ON_HOST = 1
 PDN_SKIP_CONNECTIVITY_CHECK = 2
 PDN_TIME_KERNELS = 4
 PDN_NO_UNIFORM_FAST_PATH = 8
+PDN_TERMINAL_PAIRS = 16
 KERNEL_CLASSES = ("pq", "down0", "up0", "down_coarse", "up_coarse", "small", "dense", "pair")
 
 
@@ -51,7 +52,7 @@ class PdnStats(C.Structure):
 
 
 EXPORTS = ("pdn_create", "pdn_reff", "pdn_reff_host", "pdn_destroy", "pdn_strerror", "pdn_last_error",
-           "pdn_get_stats", "pdn_port_count", "pdn_get_port_matrix", "pdn_release_cache", "pdn_update_tsvs")
+           "pdn_get_stats", "pdn_port_count", "pdn_get_port_matrix", "pdn_release_cache", "pdn_update_tsvs", "pdn_reff_same_side", "pdn_load_voltages")
 
 _lib = None
 
@@ -80,6 +81,10 @@ def load_library() -> C.CDLL:
     lib.pdn_last_error.argtypes = []
     lib.pdn_update_tsvs.restype = C.c_int
     lib.pdn_update_tsvs.argtypes = [C.c_void_p, C.c_int32, C.POINTER(PdnTsv)]
+    lib.pdn_reff_same_side.restype = C.c_int
+    lib.pdn_reff_same_side.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
+    lib.pdn_load_voltages.restype = C.c_int
+    lib.pdn_load_voltages.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_double, C.c_void_p]
     lib.pdn_release_cache.restype = None
     lib.pdn_release_cache.argtypes = []
     lib.pdn_get_stats.restype = C.c_int
@@ -205,6 +210,20 @@ class Pdn:
         st = self._lib.pdn_update_tsvs(self._h, ntsv, tsvs.ctypes.data_as(C.POINTER(PdnTsv)))
         if st != PDN_OK:
             raise PdnError(st, "pdn_update_tsvs")
+
+    def reff_same_side(self, side: int, out):
+        """pdn_reff_same_side: `out` is a torch CUDA tensor of nt*nt doubles (side 0: bumps, 1: loads)."""
+        st = self._lib.pdn_reff_same_side(self._h, side, _ptr(out))
+        if st != PDN_OK:
+            raise PdnError(st, "pdn_reff_same_side")
+        return out
+
+    def load_voltages(self, bump: int, i_load, v_bump: float, v_out):
+        """pdn_load_voltages (Eq. 4): `i_load`, `v_out` are torch CUDA tensors of n_loads doubles."""
+        st = self._lib.pdn_load_voltages(self._h, bump, _ptr(i_load), float(v_bump), _ptr(v_out))
+        if st != PDN_OK:
+            raise PdnError(st, "pdn_load_voltages")
+        return v_out
 
     def stats(self) -> dict:
         s = PdnStats()

@@ -153,15 +153,21 @@ __global__ void k_mirror_added(double* __restrict__ ZT, int ntsv, int q, const i
 
 // Meshes with n <= 4 are their own coarsest level: Z comes straight from the dense pseudo-inverse.
 __global__ void k_direct_small(const double* __restrict__ pinv, int nx, int pitch, int nc,
-                               const int* __restrict__ node, int ntsv, int q, double* __restrict__ ZT,
+                               const int* __restrict__ node, int ntsv, int nrows, int q, double* __restrict__ ZT,
                                double* __restrict__ zdiag) {
     const int j = blockIdx.x;
     const int dj = (node[j] / pitch) * nx + node[j] % pitch;
     for (int k = threadIdx.x; k < q; k += blockDim.x) {
         const int dk = (node[k] / pitch) * nx + node[k] % pitch;
-        if (j < ntsv) ZT[(size_t)j * q + k] = pinv[dj * nc + dk];
-        else if (k == 0) zdiag[j - ntsv] = pinv[dj * nc + dj];
+        if (j < nrows) ZT[(size_t)j * q + k] = pinv[dj * nc + dk];
+        if (j >= ntsv && k == 0) zdiag[j - ntsv] = pinv[dj * nc + dj];
     }
+}
+
+// zdiag[s] = ZT[ntsv+s][ntsv+s] when the terminal rows are kept (PDN_TERMINAL_PAIRS)
+__global__ void k_zdiag_from_rows(const double* __restrict__ ZT, int q, int ntsv, int nterm, double* __restrict__ zdiag) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < nterm) zdiag[s] = ZT[(size_t)(ntsv + s) * q + ntsv + s];
 }
 
 // Coarsest level: e = pinv * r, one thread per (b, i); nc = ny*nx <= 16; vectors are pitched.

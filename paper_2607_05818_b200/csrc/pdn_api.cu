@@ -144,9 +144,10 @@ struct DevBuf {  // RAII device allocation (block sizes are rounded up to 1 MiB 
 
 struct TierPorts {
     int ntsv = 0, nterm = 0, q = 0;   // TSV ports, terminal ports, total
+    int nrows = 0;                    // rows of ZT: ntsv, or q when the terminal rows are kept (PDN_TERMINAL_PAIRS)
     std::vector<int> node;            // pitched offset y*pitch + x of every port, port order of port.cuh
     DevBuf d_node;                    // device copy
-    DevBuf ZT;                        // ntsv x q
+    DevBuf ZT;                        // nrows x q
     DevBuf zdiag;                     // nterm
     DevBuf gx0, gy0;                  // sanitised pitched level-0 planes, kept for pdn_update_tsvs
 };
@@ -163,6 +164,8 @@ struct pdn_ctx {
     pdn_opts opts{};
     std::vector<TierPorts> tiers;
     DevBuf A1, X0, u, w;              // operands of the pair kernel
+    struct Side { DevBuf A, X, ys, t; int p = 0; } side[2];  // same-side pairs: [0] bumps, [1] loads (PDN_TERMINAL_PAIRS)
+    bool terminal_pairs = false;
     pdn_stats stats{};
     double class_ms[KC_COUNT] = {};
     double class_bytes[KC_COUNT] = {};
@@ -730,6 +733,19 @@ int recombine(pdn_ctx* c, Launcher& L) {
     L.run(KC_DENSE, 0, [&] { k_terminal_consts<<<cdiv(m, 128), 128, 0, L.s>>>(p0, dm1, mn, m, 0, 0, T0.ZT.as<double>(), T0.q, T0.ntsv, 0, F[0].as<double>(), Y.as<double>(), T0.zdiag.as<double>(), c->u.as<double>()); });
     L.run(KC_DENSE, 0, [&] { k_terminal_consts<<<cdiv(n, 128), 128, 0, L.s>>>(pd, dm1, mn, n, m, 1, Td.ZT.as<double>(), Td.q, Td.ntsv, 0, F[dm1 - 1].as<double>(), Y.as<double>(), Td.zdiag.as<double>(), c->w.as<double>()); });
     L.run(KC_DENSE, 0, [&] { k_pack_pair_operands<<<dim3(cdiv(p0, 128), mn), 128, 0, L.s>>>(p0, m, n, dm1, T0.ZT.as<double>(), T0.q, T0.ntsv, F[0].as<double>(), c->A1.as<double>(), c->X0.as<double>()); });
+    if (c->terminal_pairs) {  // operands of the same-side pair kernel (port.cuh: k_pair_same)
+        struct { pdn_ctx::Side& S; TierPorts& T; int p, nt, col0; double* I; } sides[2] = {
+            {c->side[0], T0, p0, m, 0, F[0].as<double>()}, {c->side[1], Td, pd, n, m, F[dm1 - 1].as<double>()}};
+        for (auto& sd : sides) {
+            sd.S.p = sd.p;
+            sd.S.A.alloc((size_t)sd.nt * sd.p * sizeof(double));
+            sd.S.X.alloc((size_t)sd.nt * sd.p * sizeof(double));
+            sd.S.ys.alloc((size_t)sd.nt * sizeof(double));
+            sd.S.t.alloc((size_t)sd.nt * sizeof(double));
+            L.run(KC_DENSE, 0, [&] { k_pack_side<<<dim3(cdiv(sd.p, 128), sd.nt), 128, 0, L.s>>>(sd.p, sd.nt, sd.col0, nrhs, sd.T.ZT.as<double>(), sd.T.q, sd.T.ntsv, sd.I, sd.S.A.as<double>(), sd.S.X.as<double>()); });
+            L.run(KC_DENSE, 0, [&] { k_side_consts<<<cdiv(sd.nt, 128), 128, 0, L.s>>>(sd.p, sd.nt, sd.col0, dm1, mn, sd.S.A.as<double>(), sd.S.X.as<double>(), Y.as<double>(), sd.T.zdiag.as<double>(), sd.S.ys.as<double>(), sd.S.t.as<double>()); });
+        }
+    }
     int h_fail = 0;
     CK(cudaMemcpyAsync(&h_fail, fail.p, sizeof(int), cudaMemcpyDeviceToHost, L.s));
     CK(cudaStreamSynchronize(L.s));
@@ -789,7 +805,7 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
     const pdn_opts& o = c->opts;
     const int n = c->n;
     if (H.nlev == 1) {
-        L.run(KC_SMALL, 0, [&] { k_direct_small<<<T.q, 64, 0, L.s>>>(H.pinv.as<double>(), n, H.pitch[0], n * n, T.d_node.as<int>(), T.ntsv, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
+        L.run(KC_SMALL, 0, [&] { k_direct_small<<<T.q, 64, 0, L.s>>>(H.pinv.as<double>(), n, H.pitch[0], n * n, T.d_node.as<int>(), T.ntsv, T.nrows, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
         return PDN_OK;
     }
     if (!(o.flags & PDN_NO_UNIFORM_FAST_PATH)) {
@@ -813,7 +829,7 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
             // T[a][s] = sum_b W[a][b] C[s][b]  (n x 2n);  G[t][s] = sum_a C[t][a] T[a][s]  (2n x 2n)
             gemm(L, n, 2 * n, n, 1.0, Wm.as<double>(), n, 1, Cm.as<double>(), 1, n, 0.0, T1.as<double>(), 2 * n);
             gemm(L, 2 * n, 2 * n, n, 1.0, Cm.as<double>(), n, 1, T1.as<double>(), 2 * n, 1, 0.0, Gt.as<double>(), 2 * n);
-            L.run(KC_SMALL, 0, [&] { k_uniform_gather<<<dim3(cdiv(T.q, 128), T.ntsv + 1), 128, 0, L.s>>>(Gt.as<double>(), n, H.pitch[0], T.d_node.as<int>(), T.ntsv, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
+            L.run(KC_SMALL, 0, [&] { k_uniform_gather<<<dim3(cdiv(T.q, 128), T.nrows + 1), 128, 0, L.s>>>(Gt.as<double>(), n, H.pitch[0], T.d_node.as<int>(), T.ntsv, T.nrows, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
             CK(cudaStreamSynchronize(L.s));  // the table buffers go back to the pool here
             c->stats.n_uniform_tiers++;
             return PDN_OK;
@@ -830,11 +846,16 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
     int status = PDN_OK;
     for (size_t s0 = 0; s0 < tsv_src.size() && status == PDN_OK; s0 += Bmax)
         status = solve_batch(c, L, H, W, T, ch, tsv_src.data() + s0, (int)std::min<size_t>(Bmax, tsv_src.size() - s0), false, o.rtol, o.max_iter);
-    if (terminals) {
+    if (terminals && T.nterm > 0) {
         std::vector<int> term(T.nterm);
         for (int k = 0; k < T.nterm; ++k) term[k] = T.ntsv + k;
+        // with the terminal rows kept they are ordinary rows of ZT: full tolerance, gathered at every port
+        const bool rows = c->terminal_pairs;
         for (size_t s0 = 0; s0 < term.size() && status == PDN_OK; s0 += Bmax)
-            status = solve_batch(c, L, H, W, T, ch, term.data() + s0, (int)std::min<size_t>(Bmax, term.size() - s0), true, rtol_term, o.max_iter);
+            status = solve_batch(c, L, H, W, T, ch, term.data() + s0, (int)std::min<size_t>(Bmax, term.size() - s0), !rows,
+                                 rows ? o.rtol : rtol_term, o.max_iter);
+        if (rows && status == PDN_OK)
+            L.run(KC_SMALL, 0, [&] { k_zdiag_from_rows<<<cdiv(T.nterm, 128), 128, 0, L.s>>>(T.ZT.as<double>(), T.q, T.ntsv, T.nterm, T.zdiag.as<double>()); });
     }
     return status;
 }
@@ -901,6 +922,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         c->d = d; c->n = n; c->m = n_bumps; c->nl = n_loads; c->opts = o;
         c->stream = (cudaStream_t)o.cuda_stream;
         c->time_kernels = (o.flags & PDN_TIME_KERNELS) != 0;
+        c->terminal_pairs = (o.flags & PDN_TERMINAL_PAIRS) != 0;
         // ---- host-side validation and port lists
         parse_tsvs(d, n, n_tsv, tsvs, c->site, c->rt);
         c->p.assign(d - 1, 0);
@@ -928,7 +950,8 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
             T.nterm = T.q - T.ntsv;
             T.d_node.alloc((size_t)T.q * sizeof(int));
             CK(cudaMemcpyAsync(T.d_node.p, T.node.data(), (size_t)T.q * sizeof(int), cudaMemcpyHostToDevice, L.s));
-            T.ZT.alloc((size_t)T.ntsv * T.q * sizeof(double));
+            T.nrows = (c->terminal_pairs && T.nterm > 0) ? T.q : T.ntsv;
+            T.ZT.alloc((size_t)T.nrows * T.q * sizeof(double));
             T.zdiag.alloc((size_t)std::max(T.nterm, 1) * sizeof(double));
             qmax = std::max(qmax, T.q);
             c->stats.n_ports_total += T.q;
@@ -1047,9 +1070,11 @@ int pdn_update_tsvs(pdn_ctx* ctx, int32_t n_tsv, const pdn_tsv* tsvs) {
             tier_port_list(c, t, nsite, node_n, ntsv_n);
             if (node_n == T.node) continue;  // same sites in the same order: Z_t is unchanged
             const int q_o = T.q, ntsv_o = T.ntsv, q_n = (int)node_n.size();
+            const int rows_o = T.nrows, rows_n = (c->terminal_pairs && q_n > ntsv_n) ? q_n : ntsv_n;
             const int plo_o = t > 0 ? (int)c->site[t - 1].size() : 0, plo_n = t > 0 ? (int)nsite[t - 1].size() : 0;
             std::vector<int> cmap(q_o, -1);
-            std::vector<unsigned char> is_added(std::max(ntsv_n, 1), 1);
+            std::vector<unsigned char> is_added(std::max(rows_n, 1), 0);
+            for (int k = 0; k < ntsv_n; ++k) is_added[k] = 1;
             for (int k = 0; k < ntsv_o; ++k) {
                 int kn = -1;
                 if (k < plo_o) kn = o2n[t - 1][k];
@@ -1063,12 +1088,12 @@ int pdn_update_tsvs(pdn_ctx* ctx, int32_t n_tsv, const pdn_tsv* tsvs) {
             DevBuf d_cmap, d_added, d_isadd, ZTn;
             d_cmap.alloc((size_t)q_o * sizeof(int));
             CK(cudaMemcpyAsync(d_cmap.p, cmap.data(), (size_t)q_o * sizeof(int), cudaMemcpyHostToDevice, L.s));
-            ZTn.alloc((size_t)ntsv_n * q_n * sizeof(double));
-            CK(cudaMemsetAsync(ZTn.p, 0, (size_t)ntsv_n * q_n * sizeof(double), L.s));
-            L.run(KC_SMALL, 0, [&] { k_remap_zt<<<dim3(cdiv(q_o, 128), ntsv_o), 128, 0, L.s>>>(T.ZT.as<double>(), ntsv_o, q_o, d_cmap.as<int>(), d_cmap.as<int>(), ZTn.as<double>(), q_n); });
+            ZTn.alloc((size_t)rows_n * q_n * sizeof(double));
+            CK(cudaMemsetAsync(ZTn.p, 0, (size_t)rows_n * q_n * sizeof(double), L.s));
+            L.run(KC_SMALL, 0, [&] { k_remap_zt<<<dim3(cdiv(q_o, 128), rows_o), 128, 0, L.s>>>(T.ZT.as<double>(), rows_o, q_o, d_cmap.as<int>(), d_cmap.as<int>(), ZTn.as<double>(), q_n); });
             CK(cudaStreamSynchronize(L.s));  // cmap (host vector) and the old ZT are released below
             T.ZT = std::move(ZTn);
-            T.node = node_n; T.ntsv = ntsv_n; T.q = q_n; T.nterm = q_n - ntsv_n;
+            T.node = node_n; T.ntsv = ntsv_n; T.q = q_n; T.nterm = q_n - ntsv_n; T.nrows = rows_n;
             T.d_node.alloc((size_t)q_n * sizeof(int));
             CK(cudaMemcpyAsync(T.d_node.p, T.node.data(), (size_t)q_n * sizeof(int), cudaMemcpyHostToDevice, L.s));
             if (!added.empty()) {
@@ -1082,10 +1107,10 @@ int pdn_update_tsvs(pdn_ctx* ctx, int32_t n_tsv, const pdn_tsv* tsvs) {
                 if (status != PDN_OK) { g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status); break; }
                 new_solves += (int64_t)added.size();
                 d_added.alloc(added.size() * sizeof(int));
-                d_isadd.alloc((size_t)ntsv_n);
+                d_isadd.alloc((size_t)rows_n);
                 CK(cudaMemcpyAsync(d_added.p, added.data(), added.size() * sizeof(int), cudaMemcpyHostToDevice, L.s));
-                CK(cudaMemcpyAsync(d_isadd.p, is_added.data(), (size_t)ntsv_n, cudaMemcpyHostToDevice, L.s));
-                L.run(KC_SMALL, 0, [&] { k_mirror_added<<<dim3(cdiv(added.size(), 128), ntsv_n), 128, 0, L.s>>>(T.ZT.as<double>(), ntsv_n, q_n, d_added.as<int>(), (int)added.size(), d_isadd.as<unsigned char>()); });
+                CK(cudaMemcpyAsync(d_isadd.p, is_added.data(), (size_t)rows_n, cudaMemcpyHostToDevice, L.s));
+                L.run(KC_SMALL, 0, [&] { k_mirror_added<<<dim3(cdiv(added.size(), 128), rows_n), 128, 0, L.s>>>(T.ZT.as<double>(), rows_n, q_n, d_added.as<int>(), (int)added.size(), d_isadd.as<unsigned char>()); });
                 CK(cudaStreamSynchronize(L.s));
             }
         }
@@ -1181,6 +1206,64 @@ int pdn_reff_host(pdn_ctx* ctx, int64_t n_pairs, const int32_t* bump_idx, const 
 
 void pdn_release_cache(void) { g_pool.trim(); }
 
+// NEXT-3: R_eff between terminals of the same side (bump-bump or load-load), full nt x nt matrix on the device.
+int pdn_reff_same_side(pdn_ctx* ctx, int32_t side, double* out) {
+    if (!ctx || !out || (side != 0 && side != 1)) return fail_arg("null context / output or side not in {0, 1}");
+    if (!ctx->terminal_pairs) return fail_arg("the context was not created with PDN_TERMINAL_PAIRS");
+    try {
+        Launcher L{ctx, ctx->stream};
+        const pdn_ctx::Side& S = ctx->side[side];
+        const TierPorts& T = ctx->tiers[side == 0 ? 0 : ctx->d - 1];
+        const int nt = T.nterm;
+        dim3 grid(cdiv(nt, 64), cdiv(nt, 64));
+        L.run(KC_PAIR, (double)nt * nt * 8.0, [&] { k_pair_same<<<grid, 256, 0, L.s>>>(nt, S.p, S.A.as<double>(), S.X.as<double>(), S.ys.as<double>(), S.t.as<double>(), T.ZT.as<double>(), T.q, T.ntsv, out); });
+        CK(cudaStreamSynchronize(ctx->stream));
+        L.resolve();
+    } catch (const CudaFail& f) {
+        g_last_error = std::string(f.what) + ": " + cudaGetErrorString(f.e);
+        cudaGetLastError();
+        return PDN_E_CUDA;
+    }
+    return PDN_OK;
+}
+
+// NEXT-3: Eq. (4).
+int pdn_load_voltages(pdn_ctx* ctx, int32_t bump, const double* i_load, double v_bump, double* v_out) {
+    if (!ctx || !i_load || !v_out) return fail_arg("null argument");
+    if (!ctx->terminal_pairs) return fail_arg("the context was not created with PDN_TERMINAL_PAIRS");
+    if (bump < 0 || bump >= ctx->m) return fail_arg("bump index out of range");
+    try {
+        Launcher L{ctx, ctx->stream};
+        const int n = ctx->nl, m = ctx->m, p0 = ctx->p0;
+        DevBuf Rb, RLL, bi, li;
+        Rb.alloc((size_t)n * sizeof(double));
+        RLL.alloc((size_t)n * n * sizeof(double));
+        bi.alloc((size_t)n * sizeof(int));
+        li.alloc((size_t)n * sizeof(int));
+        std::vector<int> hb(n, bump), hl(n);
+        for (int k = 0; k < n; ++k) hl[k] = k;
+        CK(cudaMemcpyAsync(bi.p, hb.data(), (size_t)n * sizeof(int), cudaMemcpyHostToDevice, L.s));
+        CK(cudaMemcpyAsync(li.p, hl.data(), (size_t)n * sizeof(int), cudaMemcpyHostToDevice, L.s));
+        // R_b[k] = R_eff(bump, load k): one row of the bump x load matrix
+        L.run(KC_PAIR, (double)n * 8.0, [&] { k_pair_list<<<cdiv((size_t)n * 32, 256), 256, 0, L.s>>>(n, m, n, p0, bi.as<int>(), li.as<int>(), ctx->A1.as<double>(), ctx->X0.as<double>(), ctx->u.as<double>(), ctx->w.as<double>(), Rb.as<double>()); });
+        const pdn_ctx::Side& S = ctx->side[1];
+        const TierPorts& T = ctx->tiers[ctx->d - 1];
+        dim3 grid(cdiv(n, 64), cdiv(n, 64));
+        L.run(KC_PAIR, (double)n * n * 8.0, [&] { k_pair_same<<<grid, 256, 0, L.s>>>(n, S.p, S.A.as<double>(), S.X.as<double>(), S.ys.as<double>(), S.t.as<double>(), T.ZT.as<double>(), T.q, T.ntsv, RLL.as<double>()); });
+        L.run(KC_PAIR, (double)n * n * 8.0, [&] { k_load_voltages<<<cdiv((size_t)n * 32, 256), 256, 0, L.s>>>(n, Rb.as<double>(), RLL.as<double>(), i_load, v_bump, v_out); });
+        CK(cudaStreamSynchronize(ctx->stream));
+        L.resolve();
+    } catch (const CudaFail& f) {
+        g_last_error = std::string(f.what) + ": " + cudaGetErrorString(f.e);
+        cudaGetLastError();
+        return PDN_E_CUDA;
+    } catch (const StatusFail& f) {
+        g_last_error = f.msg;
+        return f.status;
+    }
+    return PDN_OK;
+}
+
 int pdn_get_stats(const pdn_ctx* ctx, pdn_stats* out) {
     if (!ctx || !out) return fail_arg("null argument");
     *out = ctx->stats;
@@ -1203,16 +1286,16 @@ int pdn_get_port_matrix(const pdn_ctx* ctx, int32_t tier, double* out) {
     if (!ctx || !out || tier < 0 || tier >= ctx->d) return fail_arg("bad tier or null output");
     const TierPorts& T = ctx->tiers[tier];
     try {
-        std::vector<double> zt((size_t)T.ntsv * T.q), zd((size_t)T.nterm);
+        std::vector<double> zt((size_t)T.nrows * T.q), zd((size_t)T.nterm);
         CK(cudaMemcpy(zt.data(), T.ZT.p, zt.size() * sizeof(double), cudaMemcpyDeviceToHost));
         if (T.nterm) CK(cudaMemcpy(zd.data(), T.zdiag.p, zd.size() * sizeof(double), cudaMemcpyDeviceToHost));
         const double qnan = std::nan("");
         for (int j = 0; j < T.q; ++j)
             for (int k = 0; k < T.q; ++k) {
                 double v = qnan;
-                if (j < T.ntsv && k < T.ntsv) v = 0.5 * (zt[(size_t)j * T.q + k] + zt[(size_t)k * T.q + j]);
-                else if (j < T.ntsv) v = zt[(size_t)j * T.q + k];
-                else if (k < T.ntsv) v = zt[(size_t)k * T.q + j];
+                if (j < T.nrows && k < T.nrows) v = 0.5 * (zt[(size_t)j * T.q + k] + zt[(size_t)k * T.q + j]);
+                else if (j < T.nrows) v = zt[(size_t)j * T.q + k];
+                else if (k < T.nrows) v = zt[(size_t)k * T.q + j];
                 else if (j == k) v = zd[j - T.ntsv];
                 out[(size_t)j * T.q + k] = v;
             }

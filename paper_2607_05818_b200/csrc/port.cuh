@@ -137,6 +137,92 @@ __global__ void k_pack_pair_operands(int p0, int m, int n, int dm1, const double
     else X0[(int64_t)(row - m) * p0 + a] = I0[(int64_t)a * nrhs + m + (row - m)];
 }
 
+// Same-side pairs (Eq. (4) PAPER.md:60-65 needs the load-load ones).  For two terminals
+// i, j of the same tier the unit current enters and leaves on that tier, b = b_i - b_j carries no net current
+// through any interface (the constraint entries cancel), and with x_i = C^-1 b_i (already solved for every
+// terminal in S3)
+//     R(i,j) = t_i + t_j - 2 ( Z[i,j] - b_i^T x_j ),   t_i = Z[i,i] - b_i^T x_i,
+//     b_i^T x_j = sum_a A[i][a] X[j][a] + ys[j],
+// A[i][a] = Z_t[tsv port a, terminal i] over the p ports of the adjacent interface, X[j][a] = that block of
+// the currents of x_j, ys[j] = 1/2 sum_k y_j[k].
+__global__ void k_pack_side(int p, int nt, int col0, int nrhs, const double* __restrict__ ZT, int64_t q, int ntsv,
+                            const double* __restrict__ Iblk, double* __restrict__ A, double* __restrict__ X) {
+    const int a = blockIdx.x * blockDim.x + threadIdx.x, s = blockIdx.y;
+    if (a >= p || s >= nt) return;
+    A[(int64_t)s * p + a] = ZT[(int64_t)a * q + ntsv + s];
+    X[(int64_t)s * p + a] = Iblk[(int64_t)a * nrhs + col0 + s];
+}
+
+__global__ void k_side_consts(int p, int nt, int col0, int dm1, int mn, const double* __restrict__ A,
+                              const double* __restrict__ X, const double* __restrict__ Y,
+                              const double* __restrict__ zdiag, double* __restrict__ ys, double* __restrict__ t) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= nt) return;
+    double dot = 0.0, y = 0.0;
+    for (int a = 0; a < p; ++a) dot = fma(A[(int64_t)s * p + a], X[(int64_t)s * p + a], dot);
+    for (int k = 0; k < dm1; ++k) y += Y[(int64_t)k * mn + col0 + s];
+    ys[s] = 0.5 * y;
+    t[s] = zdiag[s] - (dot + 0.5 * y);
+}
+
+// R[i][j] for all ordered pairs of the nt terminals of one side; 64x64 tile / block like k_pair_full.
+// ZTT = the terminal rows of the tier's port matrix (row ntsv+i, column ntsv+j), leading dimension q.
+__global__ void __launch_bounds__(256)
+k_pair_same(int nt, int p, const double* __restrict__ A, const double* __restrict__ X, const double* __restrict__ ys,
+            const double* __restrict__ t, const double* __restrict__ ZT, int64_t q, int ntsv, double* __restrict__ R) {
+    __shared__ double As[16][65];
+    __shared__ double Bs[16][65];
+    const int tid = threadIdx.x, tx = tid % 16, ty = tid / 16;
+    const int i0 = blockIdx.y * 64, j0 = blockIdx.x * 64;
+    double acc[4][4] = {};
+    for (int k0 = 0; k0 < p; k0 += 16) {
+        for (int e = tid; e < 16 * 64; e += 256) {
+            const int kk = e % 16, ii = e / 16;
+            As[kk][ii] = (i0 + ii < nt && k0 + kk < p) ? A[(int64_t)(i0 + ii) * p + k0 + kk] : 0.0;
+            Bs[kk][ii] = (j0 + ii < nt && k0 + kk < p) ? X[(int64_t)(j0 + ii) * p + k0 + kk] : 0.0;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int kk = 0; kk < 16; ++kk) {
+            double a[4], b[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) a[r] = As[kk][ty * 4 + r];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) b[c] = Bs[kk][tx + 16 * c];
+#pragma unroll
+            for (int r = 0; r < 4; ++r)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) acc[r][c] = fma(a[r], b[c], acc[r][c]);
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int i = i0 + ty * 4 + r;
+        if (i >= nt) continue;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int j = j0 + tx + 16 * c;
+            if (j >= nt) continue;
+            const double z = 0.5 * (ZT[(int64_t)(ntsv + i) * q + ntsv + j] + ZT[(int64_t)(ntsv + j) * q + ntsv + i]);
+            R[(int64_t)i * nt + j] = (i == j) ? 0.0 : (t[i] + t[j]) - 2.0 * (z - (acc[r][c] + ys[j]));
+        }
+    }
+}
+
+// Eq. (4): with bump b at v_bump and load k drawing I[k],
+//   v[j] = v_bump - 1/2 sum_k I[k] ( R_b[j] + R_b[k] - R_LL[j][k] )       one warp per load j
+__global__ void k_load_voltages(int n, const double* __restrict__ Rb, const double* __restrict__ RLL,
+                                const double* __restrict__ I, double v_bump, double* __restrict__ v) {
+    const int j = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (j >= n) return;
+    double s = 0.0;
+    const double rbj = Rb[j];
+    for (int k = lane; k < n; k += 32) s = fma(I[k], (rbj + Rb[k]) - RLL[(int64_t)j * n + k], s);
+    s = warp_sum(s);
+    if (lane == 0) v[j] = v_bump - 0.5 * s;
+}
+
 // S4, full cross product:  R[i][j] = u[i] + w[j] - 2 sum_a A1[i][a] X0[j][a].   64x64 tile / block.
 __global__ void __launch_bounds__(256)
 k_pair_full(int m, int n, int p0, const double* __restrict__ A1, const double* __restrict__ X0,

@@ -65,14 +65,15 @@ __device__ __forceinline__ double uniform_pinv_entry(const double* __restrict__ 
     return 0.25 * ((G[dx * ld + dy] + G[sx * ld + sy]) + (G[dx * ld + sy] + G[sx * ld + dy]));
 }
 
-// ZT[j][k] = L^+[port j, port k] for the TSV ports j < ntsv against all ports k < q (grid.y = j);
-// zdiag[s] = L^+[s, s] for the terminal ports.  node[] holds pitched offsets y*pitch + x; G is indexed [x][y].
+// ZT[j][k] = L^+[port j, port k] for the rows j < nrows (the TSV ports; all ports with PDN_TERMINAL_PAIRS)
+// against all ports k < q (grid.y = nrows + 1); zdiag[s] = L^+[s, s] for the terminal ports.  node[] holds
+// pitched offsets y*pitch + x; G is indexed [x][y].
 __global__ void k_uniform_gather(const double* __restrict__ G, int n, int pitch, const int* __restrict__ node, int ntsv,
-                                 int q, double* __restrict__ ZT, double* __restrict__ zdiag) {
+                                 int nrows, int q, double* __restrict__ ZT, double* __restrict__ zdiag) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
     if (k >= q) return;
-    if (j < ntsv) ZT[(size_t)j * q + k] = uniform_pinv_entry(G, n, pitch, node[j], node[k]);
-    else if (j == ntsv && k >= ntsv) zdiag[k - ntsv] = uniform_pinv_entry(G, n, pitch, node[k], node[k]);
+    if (j < nrows) ZT[(size_t)j * q + k] = uniform_pinv_entry(G, n, pitch, node[j], node[k]);
+    else if (k >= ntsv) zdiag[k - ntsv] = uniform_pinv_entry(G, n, pitch, node[k], node[k]);
 }
 
 }  // namespace pdn

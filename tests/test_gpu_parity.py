@@ -290,6 +290,64 @@ def test_tsv_replanning_on_uniform_and_tiny_tiers():
         pdn.close()
 
 
+@pytest.mark.parametrize("seed,d,n,p,kw", [
+    (51, 2, 33, 5, {}),
+    (52, 3, 64, 8, dict(drop=0.04, aniso=0.4)),
+    (53, 2, 4, 2, {}),                        # single-level mesh: direct path
+])
+def test_same_side_pairs_and_eq4_voltages_against_the_oracle(seed, d, n, p, kw):
+    """NEXT-3: bump-bump / load-load effective resistances and the load voltages of Eq. (4),
+    against the oracle (per-pair solves for R, a KCL solve for the voltages); the bump x load result of a
+    PDN_TERMINAL_PAIRS context equals the default one; TSV re-planning keeps working on it."""
+    from oracle.reff_oracle import Oracle
+    from paper_2607_05818_b200 import PDN_TERMINAL_PAIRS, Pdn
+    torch = torch_cuda()
+    net = P.make_random(seed, d=d, n=n, p=p, m=4, nl=7, **kw)
+    o = Oracle(net)
+    pdn = Pdn.from_network(net, device="cuda:0", rtol=1e-10, flags=PDN_TERMINAL_PAIRS)
+    for side, nt in ((0, net.m), (1, net.nl)):
+        out = torch.empty(nt * nt, dtype=torch.float64, device="cuda:0")
+        pdn.reff_same_side(side, out)
+        got, want = out.cpu().numpy().reshape(nt, nt), o.reff_same_side(side)
+        off = ~np.eye(nt, dtype=bool)
+        assert np.all(np.diag(got) == 0.0)
+        assert np.allclose(got, got.T, rtol=1e-8, atol=0)
+        rel = np.abs(got[off] - want[off]) / want[off]
+        assert rel.max() <= MAX_REL and rel.mean() <= MEAN_REL
+    cur = torch.tensor(np.random.default_rng(seed).uniform(0.0, 1.5, net.nl), dtype=torch.float64, device="cuda:0")
+    v = torch.empty(net.nl, dtype=torch.float64, device="cuda:0")
+    for b in range(net.m):
+        pdn.load_voltages(b, cur, 0.8, v)
+        want = o.load_voltages(b, cur.cpu().numpy(), 0.8)
+        assert np.allclose(v.cpu().numpy(), want, rtol=0, atol=1e-8 * np.abs(0.8 - want).max())
+    full = torch.empty(net.m * net.nl, dtype=torch.float64, device="cuda:0")
+    pdn.reff(full)
+    ref, _ = gpu_all_pairs(net, rtol=1e-10)
+    assert np.allclose(full.cpu().numpy().reshape(net.m, net.nl), ref, rtol=1e-8, atol=0)
+    Z = pdn.port_matrix(0)
+    assert not np.isnan(Z).any()              # terminal-terminal entries exist now
+    if n > 4:                                 # re-plan on a context that keeps the terminal rows
+        rng = np.random.default_rng(seed)
+        new = [x for x in P._distinct_sites(rng, n, 6).tolist() if x not in net.tsv_site[0].tolist()][:2]
+        net.tsv_site[0] = np.vstack([net.tsv_site[0][1:], np.array(new, dtype=np.int32)]).astype(np.int32)
+        net.tsv_r[0] = np.concatenate([net.tsv_r[0][1:], [0.07, 0.09]])
+        pdn.update_tsvs(net.tsv_site, net.tsv_r)
+        o2 = Oracle(net)
+        out = torch.empty(net.nl * net.nl, dtype=torch.float64, device="cuda:0")
+        pdn.reff_same_side(1, out)
+        got, want = out.cpu().numpy().reshape(net.nl, net.nl), o2.reff_same_side(1)
+        off = ~np.eye(net.nl, dtype=bool)
+        assert (np.abs(got[off] - want[off]) / want[off]).max() <= MAX_REL
+        pdn.reff(full)
+        check(full.cpu().numpy().reshape(net.m, net.nl), o2.reff_all())
+    pdn.close()
+    plain = Pdn.from_network(net, device="cuda:0")
+    from paper_2607_05818_b200 import PdnError
+    with pytest.raises(PdnError):
+        plain.reff_same_side(1, torch.empty(net.nl * net.nl, dtype=torch.float64, device="cuda:0"))
+    plain.close()
+
+
 def test_bump_on_tsv_site_and_shared_sites_between_interfaces():
     from oracle.reff_oracle import Oracle
     sites = [np.array([[2, 2], [5, 1]]), np.array([[2, 2], [0, 6]])]     # (2,2) used by both interfaces

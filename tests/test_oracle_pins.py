@@ -234,3 +234,42 @@ def test_forked_sampler_equals_serial():
     o = Oracle(net)
     bi, li = P.sample_pairs(net, 40, cfg=1)
     assert np.array_equal(reff_pairs_forked(o, bi, li, 2), o.reff_pairs(bi, li))
+
+
+# ----------------------------------------------------------------------------------------- Eq. (4) voltages
+def test_node_voltages_on_a_series_chain_closed_form():
+    """Chain 0-1-...-n of r-ohm segments, node 0 held at v0, node k draws I_k: the segment (j-1, j) carries the
+    current of all loads at or beyond j, so v_j = v0 - r * sum_{s=1..j} sum_{k>=s} I_k."""
+    from oracle.reff_oracle import Oracle
+    n, r, v0 = 9, 0.37, 1.2
+    u = np.arange(n); v = np.arange(1, n + 1)
+    o = Oracle.from_edges(n + 1, u, v, np.full(n, 1.0 / r))
+    sinks = np.array([2, 5, 9, 7])
+    cur = np.array([0.3, 1.1, 0.05, 0.7])
+    got = o.node_voltages(0, v0, sinks, cur)
+    full_i = np.zeros(n + 1); full_i[sinks] = cur
+    want = []
+    for j in sinks:
+        drop = sum(r * full_i[s:].sum() for s in range(1, j + 1))
+        want.append(v0 - drop)
+    assert np.allclose(got, want, rtol=1e-12, atol=0)
+
+
+def test_eq4_identity_between_voltages_and_effective_resistances():
+    """PAPER.md:60-65, Eq. (4): v_j = v_b - 1/2 sum_k I_k (R_bj + R_bk - R_jk).  The left side comes from KCL
+    (node_voltages), the right side from per-pair effective resistances: two independent routes in the oracle."""
+    from oracle.reff_oracle import Oracle
+    net = P.make_random(5, d=3, n=6, p=3, m=2, nl=5, drop=0.05)
+    o = Oracle(net)
+    cur = np.array([0.2, 0.9, 0.0, 1.3, 0.4])
+    RLL = o.reff_same_side(1)
+    for b in range(net.m):
+        Rb = np.array([o.reff(b, k) for k in range(net.nl)])
+        want = 0.9 - 0.5 * ((Rb[:, None] + Rb[None, :] - RLL) * cur[None, :]).sum(axis=1)
+        assert np.allclose(o.load_voltages(b, cur, 0.9), want, rtol=1e-11, atol=1e-13)
+    # same-side resistances against the dense pseudo-inverse
+    from oracle.reff_oracle import laplacian, node_ids
+    Gp = np.linalg.pinv(laplacian(net).toarray(), hermitian=True)
+    _, l = node_ids(net)
+    dg = np.diag(Gp)
+    assert np.allclose(RLL, dg[l][:, None] + dg[l][None, :] - 2 * Gp[np.ix_(l, l)], rtol=1e-9, atol=1e-12)
