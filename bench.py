@@ -325,6 +325,39 @@ def run_cuda(a):
                           "port_solves_per_update": int(stu["update_solves"]), "ms_solves": stu["ms_update_stencil"],
                           "ms_refactor": stu["ms_update_dense"], "ms_full_step": ms / a.steps,
                           "pairs_per_s": npairs / float(np.mean(times))}
+    if a.eq4:   # NEXT-3: same-side pairs and Eq. (4) voltages
+        nl = net.nl
+        rll = torch.empty(nl * nl, dtype=torch.float64, device=dev)
+        cur = torch.rand(nl, dtype=torch.float64, device=dev)
+        vout = torch.empty(nl, dtype=torch.float64, device=dev)
+
+        def ev_ms(fn, reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(reps):
+                fn()
+            e1.record()
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1) / reps
+
+        t_create = []
+        pdn = None
+        for rep in range(a.warmup + a.steps):
+            if pdn is not None:
+                pdn.close()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            pdn = Pdn(net.n, gx_d, gy_d, *args[1], flags=base_flags | 16, rtol=a.rtol, nu=a.nu, rhs_batch=a.rhs_batch)
+            torch.cuda.synchronize()
+            if rep >= a.warmup:
+                t_create.append(time.perf_counter() - t0)
+        ms_ll = ev_ms(lambda: pdn.reff_same_side(1, rll), 5)
+        ms_v = ev_ms(lambda: pdn.load_voltages(0, cur, 1.0, vout), 5)
+        pdn.close()
+        line["eq4"] = {"ms_create_with_terminal_pairs": 1e3 * float(np.mean(t_create)), "ms_create_default": ms / a.steps,
+                       "load_load_pairs": nl * nl, "ms_load_load": ms_ll, "load_load_pairs_per_s": nl * nl / (ms_ll * 1e-3),
+                       "ms_voltages_one_bump": ms_v}
     if not a.no_cpu_baseline:
         ot = OracleTimer(cfg)
         n, t = ot.sample(a.cpu_budget)
@@ -350,6 +383,8 @@ def main():
     ap.add_argument("--no-fast-path", action="store_true", help="solve uniform tiers numerically too")
     ap.add_argument("--replan", type=int, default=0, metavar="K",
                     help="also time pdn_update_tsvs after moving K TSVs of every interface to new sites (NEXT-2)")
+    ap.add_argument("--eq4", action="store_true",
+                    help="also time the NEXT-3 leg: context with PDN_TERMINAL_PAIRS, load-load R_eff, Eq. (4) voltages")
     ap.add_argument("--only-device", action="store_true", help="run only the device-resident steps (for ncu)")
     a = ap.parse_args()
     if a.impl == "reference":
