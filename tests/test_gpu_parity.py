@@ -348,6 +348,40 @@ def test_same_side_pairs_and_eq4_voltages_against_the_oracle(seed, d, n, p, kw):
     plain.close()
 
 
+@pytest.mark.parametrize("fast_path", [True, False])
+def test_recombination_pins_series_law_and_separable_product_graph(fast_path):
+    """S2-S3 pins that do not go through the oracle:
+    (i) one TSV per interface => R = sum_t R^t(entry, exit) + sum Rt with every R^t from Eq. (3) (PAPER.md:49);
+    (ii) identical uniform tiers with a TSV at EVERY node are the product graph P_n x P_n x P_d, whose two-point
+    resistance has a closed DCT form (tests/closed_forms.py)."""
+    from closed_forms import product_graph_reff, wu_mesh_reff
+    from paper_2607_05818_b200 import PDN_NO_UNIFORM_FAST_PATH
+    flags = 0 if fast_path else PDN_NO_UNIFORM_FAST_PATH
+    # (i) series law, 3 tiers of 17 x 17, anisotropic
+    n, rx, ry, rt = 17, 0.9, 2.3, 0.31
+    sites = [np.array([[3, 12]]), np.array([[15, 1]])]
+    bumps, loads = np.array([[0, 0], [8, 9]]), np.array([[16, 16], [2, 5], [15, 1]])
+    net = P.make_uniform(3, n, rx, ry, rt=rt, tsv_sites=sites, bumps=bumps, loads=loads)
+    got, _ = gpu_all_pairs(net, rtol=1e-11, flags=flags)
+
+    def R2d(a, b):
+        return 0.0 if tuple(a) == tuple(b) else wu_mesh_reff(n, n, rx, ry, a[1], a[0], b[1], b[0])
+    for i, b in enumerate(bumps):
+        for j, l in enumerate(loads):
+            want = R2d(b, sites[0][0]) + rt + R2d(sites[0][0], sites[1][0]) + rt + R2d(sites[1][0], l)
+            assert got[i, j] == pytest.approx(want, rel=1e-8)
+    # (ii) product graph, 3 tiers of 6 x 6, TSV at every node
+    n, d, rx, ry, rt = 6, 3, 1.2, 0.7, 0.45
+    every = np.array([[y, x] for y in range(n) for x in range(n)])
+    bumps, loads = np.array([[0, 0], [2, 3]]), np.array([[5, 5], [2, 3], [0, 4]])
+    net = P.make_uniform(d, n, rx, ry, rt=rt, tsv_sites=[every] * (d - 1), bumps=bumps, loads=loads)
+    got, _ = gpu_all_pairs(net, rtol=1e-11, flags=flags)
+    for i, b in enumerate(bumps):
+        for j, l in enumerate(loads):
+            want = product_graph_reff(n, n, d, rx, ry, rt, (b[1], b[0], 0), (l[1], l[0], d - 1))
+            assert got[i, j] == pytest.approx(want, rel=1e-8)
+
+
 def test_bump_on_tsv_site_and_shared_sites_between_interfaces():
     from oracle.reff_oracle import Oracle
     sites = [np.array([[2, 2], [5, 1]]), np.array([[2, 2], [0, 6]])]     # (2,2) used by both interfaces
