@@ -19,11 +19,6 @@ __global__ void k_init_rhs(double* __restrict__ r, int nx, int pitch, size_t pla
     r[b * plane + i] = (i == (size_t)node[src[b]]) ? 1.0 + m : m;
 }
 
-__global__ void k_zero(double* __restrict__ a, size_t n) {
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) a[i] = 0.0;
-}
-
 __global__ void k_pcg_init(PcgScalars s, int B) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b == 0) *s.n_active = B;

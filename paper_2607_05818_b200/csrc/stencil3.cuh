@@ -9,11 +9,13 @@
 //   * the iterate and the stencil coefficients of the patch live in REGISTERS for the whole kernel;
 //     the coefficients are loaded once per block and reused for the G right-hand sides it loops over;
 //   * left / right neighbours come from the adjacent lanes by warp shuffles, the rows above / below
-//     the patch through a double-buffered shared-memory exchange (one barrier per sweep);
+//     the patch through a double-buffered shared-memory exchange with a split-phase mbarrier
+//     (publish + arrive, update the rows that need no other warp, wait, update the boundary rows);
 //   * the tile + halo of every input vector is fetched by TMA (cp.async.bulk.tensor, 3D box
-//     64 x R*W x 1 of a (x, y, rhs) tensor map) into shared memory, completion on an mbarrier, the
-//     fetch of right-hand side b+1 overlapping the sweeps of b.  Out-of-mesh elements arrive as
-//     zeros, and the coefficients there are zero, so the sweeps need no boundary cases;
+//     64 x R*W x 1 of a (x, y, rhs) tensor map) into shared memory, two stages, completion on an
+//     mbarrier, the fetch of right-hand side j+2 overlapping the sweeps of j and j+1.  Out-of-mesh
+//     elements arrive as zeros, and the coefficients there are zero: no boundary cases in the sweeps;
+//   * converged right-hand sides are skipped (ActiveList);
 //   * global stores are 16-byte (both columns of a patch row), interior only.
 //
 // Arithmetic.  The V-cycle sweeps act on the symmetrically scaled system (common.cuh: Level):
