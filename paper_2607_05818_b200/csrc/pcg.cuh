@@ -12,11 +12,18 @@ namespace pdn {
 // tier's ports, src[b] is the port index right-hand side b is the source of.
 __global__ void k_init_rhs(double* __restrict__ r, int nx, int pitch, size_t plane, double inv_n2,
                            const int* __restrict__ node, const int* __restrict__ src, int B) {
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    // two adjacent columns (one 16-byte store) per thread and step; pitch and plane are even
     const int b = blockIdx.y;
-    if (i >= plane) return;
-    const double m = ((int)(i % pitch) < nx) ? -inv_n2 : 0.0;
-    r[b * plane + i] = (i == (size_t)node[src[b]]) ? 1.0 + m : m;
+    const size_t hot = (size_t)node[src[b]];
+    double2* r2 = reinterpret_cast<double2*>(r + b * plane);
+    for (size_t i2 = (size_t)blockIdx.x * blockDim.x + threadIdx.x; 2 * i2 < plane; i2 += (size_t)gridDim.x * blockDim.x) {
+        const size_t i = 2 * i2;
+        const int x = (int)(i % pitch);
+        double2 v = make_double2(x < nx ? -inv_n2 : 0.0, x + 1 < nx ? -inv_n2 : 0.0);
+        if (i == hot) v.x += 1.0;
+        if (i + 1 == hot) v.y += 1.0;
+        r2[i2] = v;
+    }
 }
 
 __global__ void k_pcg_init(PcgScalars s, int B) {

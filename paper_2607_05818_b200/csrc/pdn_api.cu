@@ -539,7 +539,7 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     const int ngather = terminal ? 0 : T.q;
     int cur_r = 0, cur_p = 0;
     L.run(KC_SMALL, 0, [&] { k_pcg_init<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B); });
-    L.run(KC_SMALL, V, [&] { k_init_rhs<<<dim3(cdiv(plane, 256), B), 256, 0, L.s>>>(W.r[0].as<double>(), n, H.pitch[0], plane, 1.0 / (double)n2, node, src, B); });
+    L.run(KC_SMALL, V, [&] { k_init_rhs<<<dim3(std::min(1024u, cdiv(plane / 2, 256)), B), 256, 0, L.s>>>(W.r[0].as<double>(), n, H.pitch[0], plane, 1.0 / (double)n2, node, src, B); });
     if (terminal) CK(cudaMemsetAsync(W.xown.p, 0, (size_t)B * sizeof(double), L.s));
     else CK(cudaMemsetAsync(W.xport.p, 0, (size_t)B * ngather * sizeof(double), L.s));
     int nact = B;  // right-hand sides still iterating
