@@ -54,3 +54,29 @@ def test_pure_status_helpers():
     lib = pkg.load_library()
     assert lib.pdn_strerror(0) == b"ok" and b"connected" in lib.pdn_strerror(2)
     lib.pdn_destroy(None)                # NULL-safe
+
+
+def test_argument_validation_runs_on_the_host_before_any_device_work():
+    """pdn_create rejects malformed inputs with PDN_E_ARG on the host (no device needed): too few tiers, a TSV
+    outside the mesh or on an interface that does not exist, a non-positive resistance, a duplicate site inside
+    one interface, an interface without TSVs, a terminal outside the mesh."""
+    import numpy as np
+    import pdn_inputs as P
+    from paper_2607_05818_b200 import Pdn, PdnError
+
+    def status_of(mutate):
+        net = P.make_config(1)
+        mutate(net)
+        with pytest.raises(PdnError) as e:
+            Pdn(net.n, net.gx, net.gy, net.tsv_site, net.tsv_r, net.bumps, net.loads)
+        return e.value.status
+
+    def one_tier(net):
+        net.gx, net.gy, net.tsv_site, net.tsv_r = net.gx[:1], net.gy[:1], net.tsv_site[:0], net.tsv_r[:0]
+    assert status_of(one_tier) == 1
+    assert status_of(lambda n: n.tsv_site[0].__setitem__(0, [32, 0])) == 1
+    assert status_of(lambda n: n.tsv_r[0].__setitem__(3, 0.0)) == 1
+    assert status_of(lambda n: n.tsv_r[0].__setitem__(3, float("inf"))) == 1
+    assert status_of(lambda n: n.tsv_site[0].__setitem__(1, n.tsv_site[0][0])) == 1
+    assert status_of(lambda n: (n.tsv_site.__setitem__(0, n.tsv_site[0][:0]), n.tsv_r.__setitem__(0, n.tsv_r[0][:0]))) == 1
+    assert status_of(lambda n: setattr(n, "loads", np.array([[0, -1]], dtype=np.int32))) == 1
