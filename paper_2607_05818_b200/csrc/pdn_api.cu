@@ -26,6 +26,7 @@
 #include "port.cuh"
 #include "setup.cuh"
 #include "stencil3.cuh"
+#include "tail.cuh"
 #include "uniform.cuh"
 
 using namespace pdn;
@@ -285,6 +286,13 @@ struct Hierarchy {
     Level lev[MAX_LEVELS];
 
     size_t plane(int l) const { return (size_t)ny[l] * pitch[l]; }
+    // levels tail0() .. nlev-1 are small enough for the fused shared-memory tail kernel (tail.cuh);
+    // tail0() == nlev-1 means only the dense coarsest level is left for it
+    int tail0() const {
+        int l = nlev - 1;
+        while (l > 0 && std::max(ny[l - 1], nx[l - 1]) <= TAIL_MAX_N && nlev - (l - 1) <= TAIL_MAX_LEVELS) --l;
+        return l;
+    }
 
     void allocate(int n) {
         nlev = 0;
@@ -491,6 +499,24 @@ void launch_pq3(Launcher& L, double bytes, const Level& lv, const Smoother& sm, 
         default: { constexpr int NU_ = 6; CALL; } break; \
     }
 
+// The coarse tail of the cycle (levels l0 .. nlev-1) in one kernel: z_out = M_tail^-1 r_in on level l0.
+void launch_tail(Launcher& L, const Hierarchy& H, const Smoother& sm, int l0, int B, const double* r_in, double* z_out,
+                 const int* active, double bytes) {
+    TailParams P{};
+    P.nlev = H.nlev - l0;
+    for (int l = l0; l < H.nlev; ++l) P.lev[l - l0] = H.lev[l];
+    P.pinv = H.pinv.as<double>();
+    P.ch = sm.crc;
+    const size_t smem = tail_smem_doubles(P) * sizeof(double);
+    static size_t attr_smem = 0;
+    if (smem > attr_smem) {
+        CK(cudaFuncSetAttribute(k_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_smem = smem;
+    }
+    const int G = std::max(1, std::min(sm.G, B / (148 * 2)));
+    L.run(KC_DOWNC, bytes, [&] { k_tail<<<cdiv(B, G), TAIL_THREADS, smem, L.s>>>(P, r_in, z_out, H.plane(l0), B, G, active); });
+}
+
 // One multigrid V-cycle  z = M^-1 r  on a batch; r is W.r[ri].  If fused, the level-0 down stage first
 // forms W.r[ri^1] = W.r[ri] - alpha q (and its squared norm) and the cycle works with that.  The result z
 // is written to W.z; r.z goes to s.rz.  `after_down0` runs right after the level-0 down stage was
@@ -500,9 +526,21 @@ void launch_pq3(Launcher& L, double bytes, const Level& lv, const Smoother& sm, 
 template <class F>
 void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Smoother& sm, int B, int ri, bool fused, const int& nact,
             F&& after_down0) {
-    const int nl = H.nlev;
+    const int nl = H.nlev, lt = H.tail0();
     const int ru = fused ? ri ^ 1 : ri;  // the residual the rest of the cycle works with
-    for (int l = 0; l + 1 < nl; ++l) {
+    if (lt == 0) {  // the mesh itself is a tail level: residual update, whole cycle in one kernel, r.z
+        const size_t plane = H.plane(0);
+        const double V = (double)nact * H.ny[0] * H.nx[0] * 8.0;
+        if (fused) {
+            const size_t chunk = (size_t)RESID_THREADS * RESID_PER_THREAD * 2;
+            L.run(KC_DOWN0, 3.0 * V, [&] { k_resid_update<<<dim3(cdiv(plane, chunk), B), RESID_THREADS, 0, L.s>>>(W.r[ri].as<double>(), W.q.as<double>(), W.s.alpha, W.s.active, W.r[ru].as<double>(), W.s.rr, plane); });
+        }
+        if (after_down0()) return;
+        launch_tail(L, H, sm, 0, B, W.r[ru].as<double>(), W.z.as<double>(), W.s.active, 2.0 * V);
+        L.run(KC_UP0, 2.0 * V, [&] { k_dot_planes<<<dim3(std::min(64u, cdiv(plane, 256)), B), 256, 0, L.s>>>(W.r[ru].as<double>(), W.z.as<double>(), plane, W.s.active, W.s.rz); });
+        return;
+    }
+    for (int l = 0; l < lt; ++l) {
         const double V = (double)nact * H.ny[l] * H.nx[l] * 8.0, Vc = (double)nact * H.ny[l + 1] * H.nx[l + 1] * 8.0;
         const bool f = (l == 0 && fused);
         const double bytes = (f ? 4.0 : 2.0) * V + Vc;
@@ -513,9 +551,13 @@ void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Smoother& sm, int B,
                                            H.ny[l + 1], H.nx[l + 1], H.pitch[l + 1], W.s.rr, W.s.active)));
         if (l == 0 && after_down0()) return;  // converged (or out of iterations): skip the rest of the cycle
     }
-    const int lc = nl - 1, nc = H.ny[lc] * H.nx[lc];
-    L.run(KC_SMALL, 0, [&] { k_coarse_pinv<<<cdiv((size_t)B * nc, 128), 128, 0, L.s>>>(H.pinv.as<double>(), H.nx[lc], H.pitch[lc], nc, H.plane(lc), W.rl[lc].as<double>(), W.zb[lc].as<double>(), B); });
-    for (int l = nl - 2; l >= 0; --l) {
+    if (lt == nl - 1) {
+        const int nc = H.ny[lt] * H.nx[lt];
+        L.run(KC_SMALL, 0, [&] { k_coarse_pinv<<<cdiv((size_t)B * nc, 128), 128, 0, L.s>>>(H.pinv.as<double>(), H.nx[lt], H.pitch[lt], nc, H.plane(lt), W.rl[lt].as<double>(), W.zb[lt].as<double>(), B); });
+    } else {
+        launch_tail(L, H, sm, lt, B, W.rl[lt].as<double>(), W.zb[lt].as<double>(), W.s.active, 2.0 * nact * H.ny[lt] * H.nx[lt] * 8.0);
+    }
+    for (int l = lt - 1; l >= 0; --l) {
         const double V = (double)nact * H.ny[l] * H.nx[l] * 8.0, Vc = (double)nact * H.ny[l + 1] * H.nx[l + 1] * 8.0;
         const ChebR& cr = l == 0 ? sm.cr : sm.crc;
         NU_DISPATCH(cr.nu, (launch_up3<NU_>(L, l == 0 ? KC_UP0 : KC_UPC, 3.0 * V + Vc, H.lev[l], sm, cr, B, l == 0 ? W.m_r[ru] : W.m_rl[l],
