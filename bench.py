@@ -207,9 +207,9 @@ def run_cuda(a):
         barrier()
         return max_over_ranks(e0.elapsed_time(e1), dev, dist if world > 1 else None), res
 
+    sampler = ClockSampler(local) if rank == 0 else None   # started before the warm-up: its spawn is not timed
     for _ in range(a.warmup):
         step_device()
-    sampler = ClockSampler(local) if rank == 0 else None
     ms, stats = timed(lambda: step_device(), a.steps)
     clocks = sampler.stop() if sampler else None
     value = world * npairs * a.steps / (ms * 1e-3)
