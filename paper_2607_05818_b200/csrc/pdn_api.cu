@@ -590,6 +590,7 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     int it = 0, status = PDN_OK;
     long active_sum = B;  // right-hand sides still iterating, summed over the iterations (first one: all)
     double rel_prev = 1.0, rel_cur = 1.0;  // max relative residual over the batch after the last two iterations
+    int skipped = 0;                       // consecutive iterations whose outcome the host did not read
     while (true) {
         L.run(KC_SMALL, 0, [&] { k_scal_beta<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, it == 0); });
         launch_pq3(L, 4.0 * V * nact / B, H.lev[0], sm, B, W.m_z, W.m_p[cur_p], W.s.beta, W.p[cur_p ^ 1].as<double>(), W.q.as<double>(), W.s.pq, W.s.sump, W.s.active);
@@ -620,7 +621,8 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
         // does not wait for the outcome at all: the device still freezes what converged (k_scal_check), the
         // next iteration is enqueued behind it, and the prediction is carried forward.  Iteration 1 is always read.
         const bool cheap = 13.3 * V < 2.0e9;  // under ~0.5 ms of HBM traffic
-        if (cheap && it >= 2 && it < max_iter && predicted > 30.0 * rtol) {
+        if (cheap && it >= 2 && it < max_iter && predicted > 30.0 * rtol && skipped < 2) {  // at most two in a row
+            ++skipped;
             vcycle(L, H, W, sm, B, cur_r, true, nact, [&] {
                 L.run(KC_SMALL, 0, [&] { k_scal_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, rtol * rtol, bnorm2); });
                 return false;
@@ -631,6 +633,7 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
             rel_cur = predicted;
             continue;
         }
+        skipped = 0;
         if (expect_done) {
             const size_t chunk = (size_t)RESID_THREADS * RESID_PER_THREAD * 2;
             L.run(KC_SMALL, 3.0 * V * nact / B, [&] { k_resid_update<<<dim3(cdiv(plane, chunk), B), RESID_THREADS, 0, L.s>>>(W.r[cur_r].as<double>(), W.q.as<double>(), W.s.alpha, W.s.active, W.r[cur_r ^ 1].as<double>(), W.s.rr, plane); });

@@ -106,6 +106,16 @@ def test_random_stacks_against_live_oracle(seed, d, n, p, m, nl, kw):
     check(got, want)
 
 
+def test_strongly_heterogeneous_conductances_converge_and_match():
+    """Four decades of segment resistance and 10 % removed segments: far from the BASELINE workloads, but the
+    solver must still converge (well below the iteration cap) and match the oracle."""
+    from oracle.reff_oracle import Oracle
+    net = P.make_random(7, d=2, n=150, p=10, m=4, nl=5, r_lo=0.01, r_hi=100.0, drop=0.1)
+    got, st = gpu_all_pairs(net)
+    assert st["pcg_iters_max"] < 120
+    check(got, Oracle(net).reff_all())
+
+
 @pytest.mark.parametrize("nu", [1, 2, 3, 4])
 def test_every_smoother_depth(nu):
     from oracle.reff_oracle import Oracle
