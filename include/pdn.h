@@ -19,7 +19,10 @@
  *
  * Conventions.  0-based.  Tier 0 is the top tier (bumps; the paper's die_1), tier d-1 the bottom
  * tier (loads; die_d).  Tier t is an n x n node mesh, node (y, x), local id y*n + x.  Interface i
- * (0 <= i < d-1) joins tier i and tier i+1.  All floating point is IEEE FP64.  Every entry point
+ * (0 <= i < d-1) joins tier i and tier i+1.  All arithmetic is IEEE FP64 (the diagonal scaling
+ * inside the multigrid preconditioner uses FP32-representable factors, applied in FP64; the operator,
+ * the residuals and every result are FP64).  A tier whose x-segments are all equal and whose
+ * y-segments are all equal is reduced by the closed form, Eq. (3).  Every entry point
  * is thread-compatible (one thread per context at a time), never throws, and returns a status
  * (0 = PDN_OK).  There is NO CPU fallback: without a CUDA device every compute call fails with
  * PDN_E_CUDA.
