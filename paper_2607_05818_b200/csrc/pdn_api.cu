@@ -902,7 +902,12 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
     // the anisotropy a: ratio = 3 + a (measured: a = 1 -> 4, a = 3 -> 6).
     const double ratio = o.cheb_ratio > 1.0 ? o.cheb_ratio : std::min(10.0, 3.0 + H.anisotropy);
     const int G = getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 32;
-    const Smoother ch{make_cheb_roots(o.nu, ratio), make_cheb_roots(o.nu, ratio), G};
+    // On near-isotropic tiers the coarse levels get by with one step less on a wider interval (measured: same
+    // iteration counts at configs 3 and 5, one level-visit cheaper); anisotropic tiers keep nu steps everywhere.
+    const bool iso = H.anisotropy < 1.5 && o.nu >= 3 && !(o.cheb_ratio > 1.0);
+    const int nu_c = iso ? o.nu - 1 : o.nu;
+    const double ratio_c = iso ? 2.0 * ratio : ratio;
+    const Smoother ch{make_cheb_roots(o.nu, ratio), make_cheb_roots(nu_c, ratio_c), G};
     // bump / load sources deliver only their own diagonal, whose CG error is the square of the energy-norm error
     const double rtol_term = std::max(o.rtol, std::min(1e-5, std::sqrt(o.rtol) / 3.0));
     int status = PDN_OK;
