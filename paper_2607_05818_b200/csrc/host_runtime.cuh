@@ -1,0 +1,223 @@
+// Host-side runtime of libpdn: error plumbing, the device-memory pool and RAII buffers, the context, launch
+// bookkeeping (counts, per-class CUDA-event timers) and TMA descriptor encoding.  Included by pdn_api.cu only.
+#pragma once
+
+using namespace pdn;
+
+namespace {
+
+thread_local std::string g_last_error;
+
+struct CudaFail {
+    cudaError_t e;
+    const char* what;
+};
+
+#define CK(call)                                                    \
+    do {                                                            \
+        cudaError_t e__ = (call);                                   \
+        if (e__ != cudaSuccess) throw CudaFail{e__, #call};         \
+    } while (0)
+
+struct StatusFail {
+    int status;
+    std::string msg;
+};
+
+// kernel classes for the per-class timers / byte model
+enum { KC_PQ = 0, KC_DOWN0, KC_UP0, KC_DOWNC, KC_UPC, KC_SMALL, KC_DENSE, KC_PAIR, KC_COUNT };
+
+// ------------------------------------------------------------------------------------------------
+// Device memory: a process-wide cache of freed blocks.  pdn_create needs tens of GB of workspace;
+// cudaMalloc / cudaFree of blocks that size cost tens of milliseconds each, so released blocks are
+// kept and handed out again (best fit within 25 %).  pdn_release_cache() returns them to the driver;
+// an allocation failure does so automatically before giving up.
+struct DevPool {
+    std::mutex mu;
+    std::multimap<size_t, void*> free_blocks;
+    size_t cached = 0;
+
+    void* get(size_t n) {
+        {
+            std::lock_guard<std::mutex> g(mu);
+            auto it = free_blocks.lower_bound(n);
+            if (it != free_blocks.end() && it->first <= n + n / 4 + 4096) {
+                void* p = it->second;
+                cached -= it->first;
+                free_blocks.erase(it);
+                return p;
+            }
+        }
+        void* p = nullptr;
+        cudaError_t e = cudaMalloc(&p, n);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            trim();
+            e = cudaMalloc(&p, n);
+            if (e != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        }
+        return p;
+    }
+    void put(void* p, size_t n) {
+        std::lock_guard<std::mutex> g(mu);
+        free_blocks.emplace(n, p);
+        cached += n;
+    }
+    void trim() {
+        std::lock_guard<std::mutex> g(mu);
+        for (auto& kv : free_blocks) cudaFree(kv.second);
+        free_blocks.clear();
+        cached = 0;
+    }
+    size_t cached_bytes() {
+        std::lock_guard<std::mutex> g(mu);
+        return cached;
+    }
+};
+DevPool g_pool;
+
+// Pinned host scratch for the per-iteration read-backs: one grow-only block per thread, kept for the life of
+// the process (cudaMallocHost / cudaFreeHost stall for hundreds of ms now and then).
+struct PinnedScratch {
+    void* p = nullptr;
+    size_t bytes = 0;
+    void* get(size_t n) {
+        if (n > bytes) {
+            if (p) cudaFreeHost(p);
+            p = nullptr; bytes = 0;
+            if (cudaMallocHost(&p, n) != cudaSuccess) { cudaGetLastError(); p = nullptr; return nullptr; }
+            bytes = n;
+        }
+        return p;
+    }
+};
+thread_local PinnedScratch g_pinned;
+
+struct DevBuf {  // RAII device allocation (block sizes are rounded up to 1 MiB classes above 1 MiB)
+    void* p = nullptr;
+    size_t bytes = 0;
+    DevBuf() = default;
+    DevBuf(const DevBuf&) = delete;
+    DevBuf& operator=(const DevBuf&) = delete;
+    DevBuf(DevBuf&& o) noexcept : p(o.p), bytes(o.bytes) { o.p = nullptr; o.bytes = 0; }
+    DevBuf& operator=(DevBuf&& o) noexcept {
+        if (this != &o) { release(); p = o.p; bytes = o.bytes; o.p = nullptr; o.bytes = 0; }
+        return *this;
+    }
+    ~DevBuf() { release(); }
+    void release() { if (p) g_pool.put(p, bytes); p = nullptr; bytes = 0; }
+    void alloc(size_t n) {
+        release();
+        n = n < 256 ? 256 : (n + 255) & ~size_t(255);
+        p = g_pool.get(n);
+        if (!p) throw StatusFail{PDN_E_NOMEM, "cudaMalloc of " + std::to_string(n) + " bytes failed"};
+        bytes = n;
+    }
+    template <class T> T* as() const { return static_cast<T*>(p); }
+};
+
+struct TierPorts {
+    int ntsv = 0, nterm = 0, q = 0;   // TSV ports, terminal ports, total
+    int nrows = 0;                    // rows of ZT: ntsv, or q when the terminal rows are kept (PDN_TERMINAL_PAIRS)
+    std::vector<int> node;            // pitched offset y*pitch + x of every port, port order of port.cuh
+    DevBuf d_node;                    // device copy
+    DevBuf ZT;                        // nrows x q
+    DevBuf zdiag;                     // nterm
+    DevBuf gx0, gy0;                  // sanitised pitched level-0 planes, kept for pdn_update_tsvs
+};
+
+}  // namespace
+
+struct pdn_ctx {
+    int d = 0, n = 0, m = 0, nl = 0, p0 = 0;
+    std::vector<int> p;               // TSVs per interface
+    std::vector<std::vector<double>> rt;
+    std::vector<std::vector<int>> site;   // per interface: pitched offsets of the TSV sites, in list order
+    std::vector<int> bump_id, load_id;    // pitched offsets of the terminals
+    cudaStream_t stream = nullptr;
+    pdn_opts opts{};
+    std::vector<TierPorts> tiers;
+    DevBuf A1, X0, u, w;              // operands of the pair kernel
+    struct Side { DevBuf A, X, ys, t; int p = 0; } side[2];  // same-side pairs: [0] bumps, [1] loads (PDN_TERMINAL_PAIRS)
+    bool terminal_pairs = false;
+    pdn_stats stats{};
+    double class_ms[KC_COUNT] = {};
+    double class_bytes[KC_COUNT] = {};
+    int64_t class_launches[KC_COUNT] = {};
+    bool time_kernels = false;
+    std::vector<std::pair<int, std::pair<cudaEvent_t, cudaEvent_t>>> pending_events;
+    std::vector<cudaEvent_t> event_pool;
+};
+
+namespace {
+
+// ------------------------------------------------------------------------------------------------
+// launch bookkeeping: every kernel goes through Launcher::run so that launches are counted and,
+// with PDN_TIME_KERNELS, bracketed by CUDA events on the launching stream.
+struct Launcher {
+    pdn_ctx* c;
+    cudaStream_t s;
+    cudaEvent_t get_event() {
+        if (!c->event_pool.empty()) { cudaEvent_t e = c->event_pool.back(); c->event_pool.pop_back(); return e; }
+        cudaEvent_t e;
+        CK(cudaEventCreate(&e));
+        return e;
+    }
+    template <class F>
+    void run(int cls, double bytes, F&& f) {
+        cudaEvent_t a = nullptr, b = nullptr;
+        if (c->time_kernels) { a = get_event(); b = get_event(); CK(cudaEventRecord(a, s)); }
+        f();
+        CK(cudaGetLastError());
+        if (c->time_kernels) { CK(cudaEventRecord(b, s)); c->pending_events.push_back({cls, {a, b}}); }
+        c->class_launches[cls]++;
+        c->class_bytes[cls] += bytes;
+        c->stats.kernel_launches++;
+        if (cls <= KC_SMALL) c->stats.stencil_launches++;
+    }
+    void resolve() {  // call after a stream synchronise
+        for (auto& pe : c->pending_events) {
+            float ms = 0.f;
+            CK(cudaEventElapsedTime(&ms, pe.second.first, pe.second.second));
+            c->class_ms[pe.first] += ms;
+            c->event_pool.push_back(pe.second.first);
+            c->event_pool.push_back(pe.second.second);
+        }
+        c->pending_events.clear();
+    }
+};
+
+inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) / b); }
+
+// ------------------------------------------------------------------------------------------------
+// TMA descriptors: a batched pitched vector v[B][ny][pitch] as a 3D tensor (x, y, b) of doubles whose
+// x extent is the true nx (so pad columns read as zeros) and a box of bx x by x 1.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres));
+        if (!p || qres != cudaDriverEntryPointSuccess) throw StatusFail{PDN_E_CUDA, "cuTensorMapEncodeTiled is not available"};
+        fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+CUtensorMap make_map(const void* base, int nx, int ny, int pitch, int B, int box_x, int box_y) {
+    CUtensorMap m;
+    const cuuint64_t dims[3] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)B};
+    const cuuint64_t strides[2] = {(cuuint64_t)pitch * 8, (cuuint64_t)pitch * ny * 8};
+    const cuuint32_t box[3] = {(cuuint32_t)box_x, (cuuint32_t)box_y, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    const CUresult r = encode_tiled_fn()(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), dims, strides,
+                                         box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                         CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) throw StatusFail{PDN_E_CUDA, "cuTensorMapEncodeTiled failed with code " + std::to_string((int)r)};
+    return m;
+}
+}  // namespace

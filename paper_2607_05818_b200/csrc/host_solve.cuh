@@ -1,0 +1,425 @@
+// Host-side orchestration of S0 + S1: multigrid hierarchy of a tier, batch workspace with its TMA descriptors,
+// kernel launchers, the V-cycle and the batched PCG loop.  Included by pdn_api.cu only (after host_runtime.cuh).
+#pragma once
+
+namespace {
+
+
+#ifndef PDN_T3_R
+#define PDN_T3_R 6
+#endif
+#ifndef PDN_T3_W
+#define PDN_T3_W 12
+#endif
+#ifndef PDN_PQ_R
+#define PDN_PQ_R (PDN_T3_R * 2)
+#endif
+#ifndef PDN_PQ_W
+#define PDN_PQ_W (PDN_T3_W / 2)
+#endif
+#ifndef PDN_DN_R
+#define PDN_DN_R PDN_T3_R
+#endif
+#ifndef PDN_DN_W
+#define PDN_DN_W PDN_T3_W
+#endif
+constexpr int T3_R = PDN_T3_R, T3_W = PDN_T3_W, T3_EH = T3_R * T3_W, T3_THREADS = 32 * T3_W;
+constexpr int DN_R = PDN_DN_R, DN_W = PDN_DN_W;  // patch shape of the down stage (same tile height)
+static_assert(DN_R * DN_W == T3_EH, "all stencil kernels share the TMA box height");
+constexpr int PQ_R = PDN_PQ_R, PQ_W = PDN_PQ_W;  // the operator apply has one sweep and no r^: fatter patches pay
+static_assert(PQ_R * PQ_W == T3_EH, "all level-0 kernels share the TMA box height");
+constexpr size_t T3_TILE_BYTES = (size_t)T3_EH * T3_EW * sizeof(double), T3_SC_BYTES = (size_t)T3_EH * 32 * sizeof(float4);
+
+inline int pitch_of(int nx) { return (nx + 1) & ~1; }
+
+// ------------------------------------------------------------------------------------------------
+// S0: multigrid hierarchy of one tier (buffers are allocated once and reused for every tier).
+struct Hierarchy {
+    int nlev = 0;
+    int ny[MAX_LEVELS], nx[MAX_LEVELS], pitch[MAX_LEVELS];
+    DevBuf gx[MAX_LEVELS], gy[MAX_LEVELS], hE[MAX_LEVELS], hS[MAX_LEVELS], sc[MAX_LEVELS];
+    DevBuf pinv, flags, labels, sums;  // flags: [0] bad value, [1] isolated node, [2] label changed, [3] label nonzero
+    double anisotropy = 1.0;           // max(mean gx / mean gy, mean gy / mean gx) of the tier built last
+    Level lev[MAX_LEVELS];
+
+    size_t plane(int l) const { return (size_t)ny[l] * pitch[l]; }
+    // levels tail0() .. nlev-1 are small enough for the fused shared-memory tail kernel (tail.cuh);
+    // tail0() == nlev-1 means only the dense coarsest level is left for it
+    int tail0() const {
+        int l = nlev - 1;
+        while (l > 0 && std::max(ny[l - 1], nx[l - 1]) <= TAIL_MAX_N && nlev - (l - 1) <= TAIL_MAX_LEVELS) --l;
+        return l;
+    }
+
+    void allocate(int n) {
+        nlev = 0;
+        int cur = n;
+        while (true) {
+            ny[nlev] = nx[nlev] = cur;
+            pitch[nlev] = pitch_of(cur);
+            const size_t b = plane(nlev) * sizeof(double);
+            gx[nlev].alloc(b); gy[nlev].alloc(b); hE[nlev].alloc(b); hS[nlev].alloc(b); sc[nlev].alloc(b);
+            lev[nlev] = Level{cur, cur, pitch[nlev], gx[nlev].as<double>(), gy[nlev].as<double>(), hE[nlev].as<double>(),
+                              hS[nlev].as<double>(), sc[nlev].as<float2>()};
+            ++nlev;
+            if (cur <= COARSEST_MAX) break;
+            if (nlev >= MAX_LEVELS) throw StatusFail{PDN_E_ARG, "mesh too large for MAX_LEVELS"};
+            cur = (cur + 1) / 2;
+        }
+        pinv.alloc(16 * 16 * sizeof(double));
+        flags.alloc(4 * sizeof(int));
+        sums.alloc(2 * sizeof(double));
+        labels.alloc((size_t)n * n * sizeof(int));
+    }
+
+    // Import one tier (gx_src / gy_src are device pointers: dense n x n planes of the caller, or -- `retained` --
+    // the sanitised pitched level-0 planes a context kept from its creation) and build all levels.
+    int build(Launcher& L, const double* gx_src, const double* gy_src, bool check_connectivity, bool retained = false) {
+        const int n = ny[0];
+        CK(cudaMemsetAsync(flags.p, 0, 4 * sizeof(int), L.s));
+        int* fl = flags.as<int>();
+        if (retained) {
+            CK(cudaMemcpyAsync(gx[0].p, gx_src, plane(0) * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
+            CK(cudaMemcpyAsync(gy[0].p, gy_src, plane(0) * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
+            check_connectivity = false;
+        } else {
+            L.run(KC_SMALL, 0, [&] { k_import_planes<<<cdiv(plane(0), 256), 256, 0, L.s>>>(gx_src, gy_src, n, pitch[0], gx[0].as<double>(), gy[0].as<double>(), fl); });
+        }
+        for (int l = 0; l < nlev; ++l) {
+            const unsigned g = cdiv(plane(l), 256);
+            L.run(KC_SMALL, 0, [&] { k_scale_nodes<<<g, 256, 0, L.s>>>(ny[l], nx[l], pitch[l], gx[l].as<double>(), gy[l].as<double>(), sc[l].as<float2>(), l == 0 ? fl + 1 : nullptr); });
+            L.run(KC_SMALL, 0, [&] { k_scale_edges<<<g, 256, 0, L.s>>>(ny[l], nx[l], pitch[l], gx[l].as<double>(), gy[l].as<double>(), sc[l].as<float2>(), hE[l].as<double>(), hS[l].as<double>()); });
+            if (l + 1 < nlev)
+                L.run(KC_SMALL, 0, [&] { k_coarsen<<<cdiv(plane(l + 1), 256), 256, 0, L.s>>>(ny[l], nx[l], pitch[l], gx[l].as<double>(), gy[l].as<double>(), ny[l + 1], nx[l + 1], pitch[l + 1], gx[l + 1].as<double>(), gy[l + 1].as<double>()); });
+        }
+        const int lc = nlev - 1;
+        L.run(KC_SMALL, 0, [&] { k_coarsest_pinv<<<1, 32, 0, L.s>>>(ny[lc], nx[lc], pitch[lc], gx[lc].as<double>(), gy[lc].as<double>(), pinv.as<double>()); });
+        CK(cudaMemsetAsync(sums.p, 0, 2 * sizeof(double), L.s));
+        L.run(KC_SMALL, 0, [&] { k_plane_sums<<<std::min(1024u, cdiv(plane(0), 256)), 256, 0, L.s>>>((int)plane(0), gx[0].as<double>(), gy[0].as<double>(), sums.as<double>()); });
+        int h[4] = {0, 0, 0, 0};
+        double hs[2] = {1.0, 1.0};
+        CK(cudaMemcpyAsync(h, fl, 2 * sizeof(int), cudaMemcpyDeviceToHost, L.s));
+        CK(cudaMemcpyAsync(hs, sums.p, 2 * sizeof(double), cudaMemcpyDeviceToHost, L.s));
+        CK(cudaStreamSynchronize(L.s));
+        anisotropy = (hs[0] > 0.0 && hs[1] > 0.0) ? std::max(hs[0] / hs[1], hs[1] / hs[0]) : 1.0;
+        if (h[0]) return PDN_E_ARG;
+        if (h[1] && n > 1) return PDN_E_DISCONNECTED;
+        if (check_connectivity) {
+            const size_t n2 = (size_t)n * n;
+            int* lab = labels.as<int>();
+            L.run(KC_SMALL, 0, [&] { k_label_init<<<cdiv(n2, 256), 256, 0, L.s>>>((int)n2, lab); });
+            for (int sweep = 0; sweep < 4 * n + 64; ++sweep) {
+                CK(cudaMemsetAsync(fl + 2, 0, sizeof(int), L.s));
+                for (int rep = 0; rep < 4; ++rep)
+                    L.run(KC_SMALL, 0, [&] { k_label_sweep<<<cdiv(n2, 256), 256, 0, L.s>>>(n, n, pitch[0], gx[0].as<double>(), gy[0].as<double>(), lab, fl + 2); });
+                CK(cudaMemcpyAsync(h + 2, fl + 2, sizeof(int), cudaMemcpyDeviceToHost, L.s));
+                CK(cudaStreamSynchronize(L.s));
+                if (!h[2]) break;
+            }
+            L.run(KC_SMALL, 0, [&] { k_label_check<<<cdiv(n2, 256), 256, 0, L.s>>>((int)n2, lab, fl + 3); });
+            CK(cudaMemcpyAsync(h + 3, fl + 3, sizeof(int), cudaMemcpyDeviceToHost, L.s));
+            CK(cudaStreamSynchronize(L.s));
+            if (h[3]) return PDN_E_DISCONNECTED;
+        }
+        return PDN_OK;
+    }
+};
+
+ChebR make_cheb_roots(int nu, double ratio) {
+    ChebR c{};
+    c.nu = nu;
+    const double lmax = 2.0, lmin = lmax / ratio;
+    const double theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin);
+    for (int k = 0; k < nu; ++k) c.w[k] = 1.0 / (theta + delta * std::cos(M_PI * (2 * k + 1) / (2.0 * nu)));
+    return c;
+}
+
+struct Smoother {
+    ChebR cr;   // level 0
+    ChebR crc;  // levels >= 1
+    int G;  // right-hand sides a block loops over (upper bound; fewer on levels with few tiles)
+};
+
+// ------------------------------------------------------------------------------------------------
+// S1 workspace of one batch of right-hand sides, with the TMA descriptor of every vector.
+struct Work {
+    int Bmax = 0, qmax = 0;
+    DevBuf r[2], y0, z, p[2], q;                           // level 0 (ping-pong pairs: halos are read across blocks)
+    DevBuf rl[MAX_LEVELS], ya[MAX_LEVELS], zb[MAX_LEVELS];  // levels >= 1: residual, scaled iterate, correction
+    CUtensorMap m_r[2], m_y0, m_z, m_p[2], m_q;
+    CUtensorMap m_rl[MAX_LEVELS], m_ya[MAX_LEVELS], m_ec[MAX_LEVELS];  // m_ec[l]: zb[l] as the coarse box of level l-1
+    DevBuf scal, xport, xown, iact, src;  // src: port index each right-hand side of the batch is the source of
+    PcgScalars s{};
+    int* h_nact = nullptr;                           // pinned (g_pinned: not owned)
+    double* h_relres = nullptr;                      // pinned, Bmax
+
+    static size_t bytes_per_rhs(const Hierarchy& H) {
+        size_t b = 7 * H.plane(0);
+        for (int l = 1; l < H.nlev; ++l) b += 3 * H.plane(l);
+        return b * sizeof(double);
+    }
+    void allocate(const Hierarchy& H, int B, int qmax_) {
+        Bmax = B; qmax = qmax_;
+        const size_t v0 = (size_t)B * H.plane(0) * sizeof(double);
+        for (int i = 0; i < 2; ++i) { r[i].alloc(v0); p[i].alloc(v0); }
+        y0.alloc(v0); z.alloc(v0); q.alloc(v0);
+        auto fine = [&](const DevBuf& d, int l) { return make_map(d.p, H.nx[l], H.ny[l], H.pitch[l], B, T3_EW, T3_EH); };
+        for (int i = 0; i < 2; ++i) { m_r[i] = fine(r[i], 0); m_p[i] = fine(p[i], 0); }
+        m_y0 = fine(y0, 0); m_z = fine(z, 0); m_q = fine(q, 0);
+        for (int l = 1; l < H.nlev; ++l) {
+            const size_t vl = (size_t)B * H.plane(l) * sizeof(double);
+            rl[l].alloc(vl); ya[l].alloc(vl); zb[l].alloc(vl);
+            m_rl[l] = fine(rl[l], l); m_ya[l] = fine(ya[l], l);
+            m_ec[l] = make_map(zb[l].p, H.nx[l], H.ny[l], H.pitch[l], B, T3_ECW, T3_EH / 2);
+        }
+        scal.alloc((size_t)9 * B * sizeof(double));
+        double* sp = scal.as<double>();
+        s.rho = sp; s.rz = sp + B; s.pq = sp + 2 * B; s.rr = sp + 3 * B; s.sump = sp + 4 * B;
+        s.alpha = sp + 5 * B; s.beta = sp + 6 * B; s.xmean = sp + 7 * B; s.relres = sp + 8 * B;
+        iact.alloc((size_t)(B + 1) * sizeof(int));
+        s.active = iact.as<int>();
+        s.n_active = iact.as<int>() + B;
+        xport.alloc((size_t)B * std::max(qmax, 1) * sizeof(double));
+        xown.alloc((size_t)B * sizeof(double));
+        src.alloc((size_t)B * sizeof(int));
+        char* hp = static_cast<char*>(g_pinned.get(64 + (size_t)B * sizeof(double)));
+        if (!hp) throw StatusFail{PDN_E_NOMEM, "pinned host allocation failed"};
+        h_nact = reinterpret_cast<int*>(hp);
+        h_relres = reinterpret_cast<double*>(hp + 64);
+    }
+};
+
+// right-hand sides per block: as many as G allows while the grid still fills the GPU a few times over
+inline int rhs_per_block(int tiles, int B, int G) {
+    const long blocks_wanted = 148L * 4;
+    long g = ((long)tiles * B) / blocks_wanted;
+    return (int)std::max(1L, std::min<long>(std::min(G, T3_MAX_G), g));
+}
+
+template <int NU>
+void launch_down3(Launcher& L, int cls, double bytes, const Level& lv, const Smoother& sm, const ChebR& cr, int B, const CUtensorMap& m_r,
+                  const CUtensorMap* m_q, const double* alpha, double* r_out, double* y_out, double* rc, int cny,
+                  int cnx, int cpitch, double* rr_acc, const int* active) {
+    constexpr int H = halo_of(NU), IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
+    const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
+    dim3 grid(tx, ty, cdiv(B, G));
+    constexpr size_t base = 2 * T3_TILE_BYTES + T3_SC_BYTES + sizeof(Exch<DN_W>);
+    static bool attr_done = false;
+    if (!attr_done) {
+        CK(cudaFuncSetAttribute(k_down3<DN_R, DN_W, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(base + 2 * T3_TILE_BYTES)));
+        CK(cudaFuncSetAttribute(k_down3<DN_R, DN_W, NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)base));
+        attr_done = true;
+    }
+    if (m_q) L.run(cls, bytes, [&] { k_down3<DN_R, DN_W, NU, true><<<grid, 32 * DN_W, base + 2 * T3_TILE_BYTES, L.s>>>(m_r, *m_q, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
+    else L.run(cls, bytes, [&] { k_down3<DN_R, DN_W, NU, false><<<grid, 32 * DN_W, base, L.s>>>(m_r, m_r, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
+}
+
+template <int NU>
+void launch_up3(Launcher& L, int cls, double bytes, const Level& lv, const Smoother& sm, const ChebR& cr, int B, const CUtensorMap& m_r,
+                const CUtensorMap& m_y, const CUtensorMap& m_e, double* z_out, double* rz_acc, const int* active) {
+    constexpr int H = halo_of(NU), IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
+    const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
+    dim3 grid(tx, ty, cdiv(B, G));
+    constexpr size_t smem = 4 * T3_TILE_BYTES + (size_t)2 * Geom<T3_R, T3_W, 2>::ETILE_BYTES + T3_SC_BYTES + sizeof(Exch<T3_W>);
+    static bool attr_done = false;
+    if (!attr_done) {
+        CK(cudaFuncSetAttribute(k_up3<T3_R, T3_W, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_up3<T3_R, T3_W, NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done = true;
+    }
+    if (rz_acc) L.run(cls, bytes, [&] { k_up3<T3_R, T3_W, NU, true><<<grid, T3_THREADS, smem, L.s>>>(m_r, m_y, m_e, lv, cr, z_out, rz_acc, B, G, active); });
+    else L.run(cls, bytes, [&] { k_up3<T3_R, T3_W, NU, false><<<grid, T3_THREADS, smem, L.s>>>(m_r, m_y, m_e, lv, cr, z_out, rz_acc, B, G, active); });
+}
+
+void launch_pq3(Launcher& L, double bytes, const Level& lv, const Smoother& sm, int B, const CUtensorMap& m_z,
+                const CUtensorMap& m_p, const double* beta, double* p_new, double* q, double* pq_acc, double* sump_acc,
+                const int* active) {
+    constexpr int H = 2, IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
+    const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
+    dim3 grid(tx, ty, cdiv(B, G));
+    constexpr size_t smem = 4 * T3_TILE_BYTES + sizeof(Exch<PQ_W>);
+    static bool attr_done = false;
+    if (!attr_done) {
+        CK(cudaFuncSetAttribute(k_pq3<PQ_R, PQ_W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done = true;
+    }
+    L.run(KC_PQ, bytes, [&] { k_pq3<PQ_R, PQ_W><<<grid, 32 * PQ_W, smem, L.s>>>(m_z, m_p, lv, beta, p_new, q, pq_acc, sump_acc, B, G, active); });
+}
+
+#define NU_DISPATCH(nu, CALL)                 \
+    switch (nu) {                             \
+        case 1: { constexpr int NU_ = 1; CALL; } break; \
+        case 2: { constexpr int NU_ = 2; CALL; } break; \
+        case 3: { constexpr int NU_ = 3; CALL; } break; \
+        case 4: { constexpr int NU_ = 4; CALL; } break; \
+        case 5: { constexpr int NU_ = 5; CALL; } break; \
+        default: { constexpr int NU_ = 6; CALL; } break; \
+    }
+
+// The coarse tail of the cycle (levels l0 .. nlev-1) in one kernel: z_out = M_tail^-1 r_in on level l0.
+void launch_tail(Launcher& L, const Hierarchy& H, const Smoother& sm, int l0, int B, const double* r_in, double* z_out,
+                 const int* active, double bytes) {
+    TailParams P{};
+    P.nlev = H.nlev - l0;
+    for (int l = l0; l < H.nlev; ++l) P.lev[l - l0] = H.lev[l];
+    P.pinv = H.pinv.as<double>();
+    P.ch = sm.crc;
+    const size_t smem = tail_smem_doubles(P) * sizeof(double);
+    static size_t attr_smem = 0;
+    if (smem > attr_smem) {
+        CK(cudaFuncSetAttribute(k_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_smem = smem;
+    }
+    const int G = std::max(1, std::min(sm.G, B / (148 * 2)));
+    L.run(KC_DOWNC, bytes, [&] { k_tail<<<cdiv(B, G), TAIL_THREADS, smem, L.s>>>(P, r_in, z_out, H.plane(l0), B, G, active); });
+}
+
+// One multigrid V-cycle  z = M^-1 r  on a batch; r is W.r[ri].  If fused, the level-0 down stage first
+// forms W.r[ri^1] = W.r[ri] - alpha q (and its squared norm) and the cycle works with that.  The result z
+// is written to W.z; r.z goes to s.rz.  `after_down0` runs right after the level-0 down stage was
+// enqueued (the convergence check); if it returns true the rest of the cycle is skipped.
+// `nact` = right-hand sides of the batch still iterating (the kernels skip the others); it only enters the
+// algorithmic-byte accounting and is re-read after `after_down0`, which may lower it.
+template <class F>
+void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Smoother& sm, int B, int ri, bool fused, const int& nact,
+            F&& after_down0) {
+    const int nl = H.nlev, lt = H.tail0();
+    const int ru = fused ? ri ^ 1 : ri;  // the residual the rest of the cycle works with
+    if (lt == 0) {  // the mesh itself is a tail level: residual update, whole cycle in one kernel, r.z
+        const size_t plane = H.plane(0);
+        const double V = (double)nact * H.ny[0] * H.nx[0] * 8.0;
+        if (fused) {
+            const size_t chunk = (size_t)RESID_THREADS * RESID_PER_THREAD * 2;
+            L.run(KC_DOWN0, 3.0 * V, [&] { k_resid_update<<<dim3(cdiv(plane, chunk), B), RESID_THREADS, 0, L.s>>>(W.r[ri].as<double>(), W.q.as<double>(), W.s.alpha, W.s.active, W.r[ru].as<double>(), W.s.rr, plane); });
+        }
+        if (after_down0()) return;
+        launch_tail(L, H, sm, 0, B, W.r[ru].as<double>(), W.z.as<double>(), W.s.active, 2.0 * V);
+        L.run(KC_UP0, 2.0 * V, [&] { k_dot_planes<<<dim3(std::min(64u, cdiv(plane, 256)), B), 256, 0, L.s>>>(W.r[ru].as<double>(), W.z.as<double>(), plane, W.s.active, W.s.rz); });
+        return;
+    }
+    for (int l = 0; l < lt; ++l) {
+        const double V = (double)nact * H.ny[l] * H.nx[l] * 8.0, Vc = (double)nact * H.ny[l + 1] * H.nx[l + 1] * 8.0;
+        const bool f = (l == 0 && fused);
+        const double bytes = (f ? 4.0 : 2.0) * V + Vc;
+        const ChebR& cr = l == 0 ? sm.cr : sm.crc;
+        NU_DISPATCH(cr.nu, (launch_down3<NU_>(L, l == 0 ? KC_DOWN0 : KC_DOWNC, bytes, H.lev[l], sm, cr, B, l == 0 ? W.m_r[ri] : W.m_rl[l],
+                                           f ? &W.m_q : nullptr, W.s.alpha, f ? W.r[ri ^ 1].as<double>() : nullptr,
+                                           l == 0 ? W.y0.as<double>() : W.ya[l].as<double>(), W.rl[l + 1].as<double>(),
+                                           H.ny[l + 1], H.nx[l + 1], H.pitch[l + 1], W.s.rr, W.s.active)));
+        if (l == 0 && after_down0()) return;  // converged (or out of iterations): skip the rest of the cycle
+    }
+    if (lt == nl - 1) {
+        const int nc = H.ny[lt] * H.nx[lt];
+        L.run(KC_SMALL, 0, [&] { k_coarse_pinv<<<cdiv((size_t)B * nc, 128), 128, 0, L.s>>>(H.pinv.as<double>(), H.nx[lt], H.pitch[lt], nc, H.plane(lt), W.rl[lt].as<double>(), W.zb[lt].as<double>(), B); });
+    } else {
+        launch_tail(L, H, sm, lt, B, W.rl[lt].as<double>(), W.zb[lt].as<double>(), W.s.active, 2.0 * nact * H.ny[lt] * H.nx[lt] * 8.0);
+    }
+    for (int l = lt - 1; l >= 0; --l) {
+        const double V = (double)nact * H.ny[l] * H.nx[l] * 8.0, Vc = (double)nact * H.ny[l + 1] * H.nx[l + 1] * 8.0;
+        const ChebR& cr = l == 0 ? sm.cr : sm.crc;
+        NU_DISPATCH(cr.nu, (launch_up3<NU_>(L, l == 0 ? KC_UP0 : KC_UPC, 3.0 * V + Vc, H.lev[l], sm, cr, B, l == 0 ? W.m_r[ru] : W.m_rl[l],
+                                         l == 0 ? W.m_y0 : W.m_ya[l], W.m_ec[l + 1],
+                                         l == 0 ? W.z.as<double>() : W.zb[l].as<double>(), l == 0 ? W.s.rz : nullptr, W.s.active)));
+    }
+}
+
+// Solve L_t x_b = e_{port src[b]} - 1/n^2 for b in [0, B) by multigrid-preconditioned CG and leave
+//   TSV-source batch     : ZT[src[b]][k] = x_b[port k] - mean(x_b)      for all ports k of the tier
+//   terminal-source batch: zdiag[src[b]-ntsv] = x_b[own node] - mean(x_b)
+int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts& T, const Smoother& sm, const int* src_ports,
+                int B, bool terminal, double rtol, int max_iter) {
+    const int src0 = src_ports[0];
+    CK(cudaMemcpyAsync(W.src.p, src_ports, (size_t)B * sizeof(int), cudaMemcpyHostToDevice, L.s));
+    const int* src = W.src.as<int>();
+    const int n = H.ny[0];
+    const size_t n2 = (size_t)n * n, plane = H.plane(0);
+    const double V = (double)B * n2 * 8.0;
+    const int* node = T.d_node.as<int>();
+    const int ngather = terminal ? 0 : T.q;
+    int cur_r = 0, cur_p = 0;
+    L.run(KC_SMALL, 0, [&] { k_pcg_init<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B); });
+    L.run(KC_SMALL, V, [&] { k_init_rhs<<<dim3(std::min(1024u, cdiv(plane / 2, 256)), B), 256, 0, L.s>>>(W.r[0].as<double>(), n, H.pitch[0], plane, 1.0 / (double)n2, node, src, B); });
+    if (terminal) CK(cudaMemsetAsync(W.xown.p, 0, (size_t)B * sizeof(double), L.s));
+    else CK(cudaMemsetAsync(W.xport.p, 0, (size_t)B * ngather * sizeof(double), L.s));
+    int nact = B;  // right-hand sides still iterating
+    vcycle(L, H, W, sm, B, 0, false, nact, [] { return false; });
+    const double bnorm2 = 1.0 - 1.0 / (double)n2;
+    int it = 0, status = PDN_OK;
+    long active_sum = B;  // right-hand sides still iterating, summed over the iterations (first one: all)
+    double rel_prev = 1.0, rel_cur = 1.0;  // max relative residual over the batch after the last two iterations
+    int skipped = 0;                       // consecutive iterations whose outcome the host did not read
+    while (true) {
+        L.run(KC_SMALL, 0, [&] { k_scal_beta<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, it == 0); });
+        launch_pq3(L, 4.0 * V * nact / B, H.lev[0], sm, B, W.m_z, W.m_p[cur_p], W.s.beta, W.p[cur_p ^ 1].as<double>(), W.q.as<double>(), W.s.pq, W.s.sump, W.s.active);
+        cur_p ^= 1;
+        L.run(KC_SMALL, 0, [&] { k_scal_alpha<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, 1.0 / (double)n2); });
+        L.run(KC_SMALL, 0, [&] { k_xport<<<dim3(cdiv(std::max(ngather, 1), 128), B), 128, 0, L.s>>>(W.p[cur_p].as<double>(), plane, W.s.alpha, node, ngather, src, W.xport.as<double>(), W.xown.as<double>(), B); });
+        ++it;
+        bool done = false;
+        auto check = [&] {
+            L.run(KC_SMALL, 0, [&] { k_scal_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, rtol * rtol, bnorm2); });
+            CK(cudaMemcpyAsync(W.h_nact, W.s.n_active, sizeof(int), cudaMemcpyDeviceToHost, L.s));
+            CK(cudaMemcpyAsync(W.h_relres, W.s.relres, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, L.s));
+            CK(cudaStreamSynchronize(L.s));
+            nact = *W.h_nact;
+            done = (nact == 0);
+            active_sum += nact;
+            rel_prev = rel_cur;
+            rel_cur = 0.0;
+            for (int b = 0; b < B; ++b) rel_cur = std::max(rel_cur, W.h_relres[b]);
+            if (getenv("PDN_DEBUG")) fprintf(stderr, "[pdn]   it %d: max relres %.3e, active %d\n", it, rel_cur, nact);
+            return done || it >= max_iter;
+        };
+        // CG residuals contract roughly geometrically: if the next one is expected below the tolerance, update the
+        // residual alone first (3 V of traffic) and run the V-cycle only if that expectation was wrong
+        const double predicted = rel_prev > 0.0 ? rel_cur * (rel_cur / rel_prev) : 1.0;
+        const bool expect_done = predicted <= rtol;
+        // ... and if it is expected far above it while an iteration is short (small meshes / batches), the host
+        // does not wait for the outcome at all: the device still freezes what converged (k_scal_check), the
+        // next iteration is enqueued behind it, and the prediction is carried forward.  Iteration 1 is always read.
+        const bool cheap = 13.3 * V < 2.0e9;  // under ~0.5 ms of HBM traffic
+        if (cheap && it >= 2 && it < max_iter && predicted > 30.0 * rtol && skipped < 2) {  // at most two in a row
+            ++skipped;
+            vcycle(L, H, W, sm, B, cur_r, true, nact, [&] {
+                L.run(KC_SMALL, 0, [&] { k_scal_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, rtol * rtol, bnorm2); });
+                return false;
+            });
+            cur_r ^= 1;
+            active_sum += nact;
+            rel_prev = rel_cur;
+            rel_cur = predicted;
+            continue;
+        }
+        skipped = 0;
+        if (expect_done) {
+            const size_t chunk = (size_t)RESID_THREADS * RESID_PER_THREAD * 2;
+            L.run(KC_SMALL, 3.0 * V * nact / B, [&] { k_resid_update<<<dim3(cdiv(plane, chunk), B), RESID_THREADS, 0, L.s>>>(W.r[cur_r].as<double>(), W.q.as<double>(), W.s.alpha, W.s.active, W.r[cur_r ^ 1].as<double>(), W.s.rr, plane); });
+            cur_r ^= 1;
+            if (!check()) vcycle(L, H, W, sm, B, cur_r, false, nact, [] { return false; });
+        } else {
+            vcycle(L, H, W, sm, B, cur_r, true, nact, check);
+            cur_r ^= 1;
+        }
+        if (done) break;
+        if (it >= max_iter) { status = PDN_E_NOCONV; break; }
+    }
+    // results + statistics
+    if (terminal)
+        L.run(KC_SMALL, 0, [&] { k_finish_term<<<cdiv(B, 128), 128, 0, L.s>>>(W.xown.as<double>(), W.s.xmean, src, T.ntsv, T.zdiag.as<double>(), B); });
+    else
+        L.run(KC_SMALL, 0, [&] { k_finish_tsv<<<dim3(cdiv(ngather, 128), B), 128, 0, L.s>>>(W.xport.as<double>(), W.s.xmean, ngather, src, T.ZT.as<double>(), B); });
+    CK(cudaMemcpyAsync(W.h_relres, W.s.relres, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, L.s));
+    CK(cudaStreamSynchronize(L.s));
+    double worst = 0.0;
+    for (int b = 0; b < B; ++b) worst = std::max(worst, W.h_relres[b]);
+    c->stats.worst_rel_residual = std::max(c->stats.worst_rel_residual, worst);
+    c->stats.pcg_iters_max = std::max(c->stats.pcg_iters_max, it);
+    c->stats.pcg_iters_sum += it;
+    c->stats.rhs_iterations += active_sum;
+    if (getenv("PDN_DEBUG"))
+        fprintf(stderr, "[pdn] batch src0=%d B=%d %s: %d iterations, rhs-iterations %ld (of %ld without skipping), worst relres %.2e\n", src0, B,
+                terminal ? "terminal" : "tsv", it, active_sum, (long)it * B, worst);
+    return status;
+}
+
+}  // namespace
