@@ -403,6 +403,28 @@ def test_bump_on_tsv_site_and_shared_sites_between_interfaces():
     check(got, Oracle(net).reff_all())
 
 
+def test_two_host_threads_with_their_own_contexts():
+    """The library is thread-compatible: contexts created and used concurrently from two host threads (shared
+    device-memory pool, per-thread pinned scratch) give the same results as one after the other."""
+    import threading
+    nets = [P.make_random(61 + k, d=2 + k, n=40 + 9 * k, p=6, m=3, nl=4) for k in range(2)]
+    ref = [gpu_all_pairs(net, rtol=1e-10)[0] for net in nets]
+    got, err = [None, None], []
+
+    def work(k):
+        try:
+            for _ in range(4):
+                got[k] = gpu_all_pairs(nets[k], rtol=1e-10)[0]
+        except Exception as e:      # noqa: BLE001
+            err.append(e)
+    th = [threading.Thread(target=work, args=(k,)) for k in range(2)]
+    [t.start() for t in th]
+    [t.join() for t in th]
+    assert not err, err
+    for k in range(2):
+        assert np.allclose(got[k], ref[k], rtol=1e-9, atol=0)
+
+
 def test_out_of_range_pair_index_yields_nan():
     torch = torch_cuda()
     from paper_2607_05818_b200 import Pdn
