@@ -169,7 +169,8 @@ def run_cuda(a):
         torch.cuda.synchronize()
 
     cfg = a.config
-    net = P.make_config(cfg, seed=rank)          # one independent network per rank
+    sharded = a.shard and world > 1
+    net = P.make_config(cfg, seed=0 if sharded else rank)   # one independent network per rank, or one for all
     if a.uniform:   # NEXT-1 variant: every tier gets its median segment conductances (same sites): Eq. (3) fast path
         for t in range(net.d):
             n_ = net.n
@@ -186,15 +187,22 @@ def run_cuda(a):
 
     base_flags = 8 if a.no_fast_path else 0      # PDN_NO_UNIFORM_FAST_PATH
 
+    shard_kw = dict(shard_rank=rank, shard_world=world) if sharded else {}
+
     def step_device(flags=0):
-        pdn = Pdn(net.n, gx_d, gy_d, *args[1], flags=flags | base_flags, rtol=a.rtol, nu=a.nu, rhs_batch=a.rhs_batch)
+        pdn = Pdn(net.n, gx_d, gy_d, *args[1], flags=flags | base_flags, rtol=a.rtol, nu=a.nu, rhs_batch=a.rhs_batch,
+                  **shard_kw)
+        if sharded:
+            pdn.exchange_and_finish(dist, world)
         pdn.reff(out_d)
         st = pdn.stats()
         pdn.close()
         return st
 
     def step_host():
-        pdn = Pdn(net.n, gx_h, gy_h, *args[1], flags=base_flags, rtol=a.rtol, nu=a.nu, rhs_batch=a.rhs_batch)
+        pdn = Pdn(net.n, gx_h, gy_h, *args[1], flags=base_flags, rtol=a.rtol, nu=a.nu, rhs_batch=a.rhs_batch, **shard_kw)
+        if sharded:
+            pdn.exchange_and_finish(dist, world)
         pdn.reff_host(out_h)
         pdn.close()
 
@@ -212,7 +220,8 @@ def run_cuda(a):
         step_device()
     ms, stats = timed(lambda: step_device(), a.steps)
     clocks = sampler.stop() if sampler else None
-    value = world * npairs * a.steps / (ms * 1e-3)
+    jobs = 1 if sharded else world               # networks solved per step by the whole job
+    value = jobs * npairs * a.steps / (ms * 1e-3)
 
     if a.only_device:   # used under ncu: no extra legs, no JSON contract
         if rank == 0:
@@ -223,7 +232,7 @@ def run_cuda(a):
     # end to end through the host-buffer entry points
     step_host()
     ms_e2e, _ = timed(step_host, a.steps)
-    e2e_value = world * npairs * a.steps / (ms_e2e * 1e-3)
+    e2e_value = jobs * npairs * a.steps / (ms_e2e * 1e-3)
     h2d = sum(g.numel() * 8 for g in gx_h) * 2
     d2h = npairs * 8
 
@@ -273,7 +282,8 @@ def run_cuda(a):
                   "tolerance": {"max_rel": 1e-6, "mean_rel": 1e-8}, "expected": f"tests/golden/cfg{cfg}_reff.txt (oracle)"}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
-        "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "strong" if sharded else "weak",
+        "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(cfg) + (" -- UNIFORM variant (median conductances)" if a.uniform else ""),
                    "cfg": cfg, "pairs_per_step_per_gpu": npairs, "uniform_tiers": last["n_uniform_tiers"],
@@ -385,6 +395,9 @@ def main():
                     help="also time pdn_update_tsvs after moving K TSVs of every interface to new sites (NEXT-2)")
     ap.add_argument("--eq4", action="store_true",
                     help="also time the NEXT-3 leg: context with PDN_TERMINAL_PAIRS, load-load R_eff, Eq. (4) voltages")
+    ap.add_argument("--shard", action="store_true",
+                    help="N > 1: ONE network, its port solves sharded over the ranks (NEXT-4, strong scaling) instead "
+                         "of one independent network per rank")
     ap.add_argument("--only-device", action="store_true", help="run only the device-resident steps (for ncu)")
     a = ap.parse_args()
     if a.impl == "reference":

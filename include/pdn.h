@@ -109,6 +109,8 @@ typedef struct {
     int32_t flags;      /* PDN_* flags                                                             */
     int32_t nu;         /* Chebyshev smoothing steps per multigrid level and side (1..6, default 4)*/
     double cheb_ratio;  /* smoothing interval [2/ratio, 2] of D^-1 L (default: 3 + the tier's anisotropy)  */
+    int32_t shard_rank; /* NEXT-4: this process solves slice shard_rank of shard_world of every tier's port     */
+    int32_t shard_world;/* solves and leaves the context OPEN (see pdn_shard_slice / pdn_finish); 0 or 1 = off  */
 } pdn_opts;
 
 /* Counters and timings of the last pdn_create (device-event milliseconds). */
@@ -165,6 +167,22 @@ int pdn_reff_same_side(pdn_ctx *ctx, int32_t side, double *out);
  * i_load[k] (DEVICE, n_loads values, amperes); v_out[j] (DEVICE, n_loads values) receives the voltage of load j,
  *   v_j = v_bump - 1/2 sum_k i_load[k] (R_{b,j} + R_{b,k} - R_{j,k}).   Needs PDN_TERMINAL_PAIRS. */
 int pdn_load_voltages(pdn_ctx *ctx, int32_t bump, const double *i_load, double v_bump, double *v_out);
+
+/* NEXT-4: one network sharded over several GPUs, one process per GPU.  The port solves of
+ * a tier are independent, so with opts->shard_world = W > 1 pdn_create (same arguments on every
+ * rank) imports all tiers but solves only slice opts->shard_rank of each tier's TSV sources and of its bump / load
+ * sources -- contiguous, rank r owning [floor(r k / W), floor((r+1) k / W)) of k sources -- and returns an OPEN
+ * context: pdn_reff & co. fail with PDN_E_ARG until pdn_finish.  The caller then makes every rank's rows present
+ * on every rank (one broadcast per rank and tier over NCCL / NVLink: rows [tsv0, tsv0+ntsv) of the port matrix are
+ * contiguous, ld doubles each; zdiag[term0 .. term0+nterm) likewise; with PDN_TERMINAL_PAIRS also rows
+ * [ntsv_total+term0, ...)) and calls pdn_finish, which runs S2-S3 (replicated: milliseconds).
+ * pdn_shard_slice: the slice of `rank` in `tier` (all zeros for a tier every rank reduced whole: uniform tiers,
+ * meshes with n <= 4).  pdn_shard_buffers: DEVICE pointers of the tier's port matrix (ld = its leading dimension =
+ * port count; ntsv_total = its number of TSV ports) and of zdiag. */
+int pdn_shard_slice(const pdn_ctx *ctx, int32_t tier, int32_t rank, int32_t *tsv0, int32_t *ntsv, int32_t *term0,
+                    int32_t *nterm);
+int pdn_shard_buffers(pdn_ctx *ctx, int32_t tier, double **zt, int64_t *ld, int32_t *ntsv_total, double **zdiag);
+int pdn_finish(pdn_ctx *ctx);
 
 /* NULL-safe; frees all device and host memory of ctx. */
 void pdn_destroy(pdn_ctx *ctx);

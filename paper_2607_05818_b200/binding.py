@@ -37,7 +37,8 @@ class PdnSite(C.Structure):
 
 class PdnOpts(C.Structure):
     _fields_ = [("rtol", C.c_double), ("max_iter", C.c_int32), ("rhs_batch", C.c_int32),
-                ("cuda_stream", C.c_void_p), ("flags", C.c_int32), ("nu", C.c_int32), ("cheb_ratio", C.c_double)]
+                ("cuda_stream", C.c_void_p), ("flags", C.c_int32), ("nu", C.c_int32), ("cheb_ratio", C.c_double),
+                ("shard_rank", C.c_int32), ("shard_world", C.c_int32)]
 
 
 class PdnStats(C.Structure):
@@ -52,7 +53,7 @@ class PdnStats(C.Structure):
 
 
 EXPORTS = ("pdn_create", "pdn_reff", "pdn_reff_host", "pdn_destroy", "pdn_strerror", "pdn_last_error",
-           "pdn_get_stats", "pdn_port_count", "pdn_get_port_matrix", "pdn_release_cache", "pdn_update_tsvs", "pdn_reff_same_side", "pdn_load_voltages")
+           "pdn_get_stats", "pdn_port_count", "pdn_get_port_matrix", "pdn_release_cache", "pdn_update_tsvs", "pdn_reff_same_side", "pdn_load_voltages", "pdn_shard_slice", "pdn_shard_buffers", "pdn_finish")
 
 _lib = None
 
@@ -85,6 +86,13 @@ def load_library() -> C.CDLL:
     lib.pdn_reff_same_side.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
     lib.pdn_load_voltages.restype = C.c_int
     lib.pdn_load_voltages.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_double, C.c_void_p]
+    lib.pdn_shard_slice.restype = C.c_int
+    lib.pdn_shard_slice.argtypes = [C.c_void_p, C.c_int32, C.c_int32] + [C.POINTER(C.c_int32)] * 4
+    lib.pdn_shard_buffers.restype = C.c_int
+    lib.pdn_shard_buffers.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_int64),
+                                      C.POINTER(C.c_int32), C.POINTER(C.c_void_p)]
+    lib.pdn_finish.restype = C.c_int
+    lib.pdn_finish.argtypes = [C.c_void_p]
     lib.pdn_release_cache.restype = None
     lib.pdn_release_cache.argtypes = []
     lib.pdn_get_stats.restype = C.c_int
@@ -144,12 +152,29 @@ def _ptr(t) -> int:
     return t.data_ptr()
 
 
+class _CudaArray:
+    """Minimal __cuda_array_interface__ carrier so that torch can alias library-owned device memory."""
+
+    def __init__(self, ptr: int, n: int):
+        self.__cuda_array_interface__ = {"shape": (n,), "typestr": "<f8", "data": (ptr, False), "version": 2}
+
+
+def _device_view(ptr: int, n: int):
+    import torch
+    return torch.as_tensor(_CudaArray(ptr, n), device="cuda")
+
+
+def shard_bounds(k: int, world: int):
+    """Rank r owns [floor(r k / world), floor((r+1) k / world)) of k sources (the rule pdn_create applies)."""
+    return [(r * k // world, (r + 1) * k // world) for r in range(world)]
+
+
 class Pdn:
     """Owns one pdn_ctx.  `gx`, `gy`: per-tier (n, n) FP64 planes, torch CUDA tensors (device path)
     or numpy / torch CPU arrays (host path: PDN_TIERS_ON_HOST is set and the library uploads)."""
 
     def __init__(self, n, gx, gy, tsv_site, tsv_r, bumps, loads, rtol=0.0, max_iter=0, rhs_batch=0,
-                 nu=0, flags=0, stream=None, cheb_ratio=0.0):
+                 nu=0, flags=0, stream=None, cheb_ratio=0.0, shard_rank=0, shard_world=0):
         lib = load_library()
         d = len(gx)
         on_host = isinstance(gx[0], np.ndarray) or (hasattr(gx[0], "is_cuda") and not gx[0].is_cuda)
@@ -165,7 +190,9 @@ class Pdn:
         self.nl = len(np.asarray(loads).reshape(-1, 2))
         opts = PdnOpts(rtol=rtol, max_iter=max_iter, rhs_batch=rhs_batch,
                        cuda_stream=C.c_void_p(stream) if stream else None,
-                       flags=flags | (PDN_TIERS_ON_HOST if on_host else 0), nu=nu, cheb_ratio=cheb_ratio)
+                       flags=flags | (PDN_TIERS_ON_HOST if on_host else 0), nu=nu, cheb_ratio=cheb_ratio,
+                       shard_rank=shard_rank, shard_world=shard_world)
+        self.d = d
         h = C.c_void_p()
         b_arr, l_arr = _sites(bumps), _sites(loads)
         st = lib.pdn_create(C.byref(h), d, tiers, ntsv, tsvs.ctypes.data_as(C.POINTER(PdnTsv)), self.m,
@@ -175,6 +202,7 @@ class Pdn:
             raise PdnError(st, "pdn_create")
         self._h = h
         self._lib = lib
+        self._terminal_rows = bool(flags & PDN_TERMINAL_PAIRS)
 
     @classmethod
     def from_network(cls, net, device=None, **kw):
@@ -224,6 +252,42 @@ class Pdn:
         if st != PDN_OK:
             raise PdnError(st, "pdn_load_voltages")
         return v_out
+
+    # ---- NEXT-4: one network sharded over several GPUs (argument marshalling + the exchange plumbing only)
+    def shard_pieces(self, rank: int):
+        """The device pieces rank `rank` owns, as (tier, torch CUDA tensor view) pairs: its rows of every tier's
+        port matrix and its slice of zdiag.  The views alias library memory (no copy)."""
+        import torch
+        out = []
+        for t in range(self.d):
+            v = [C.c_int32() for _ in range(4)]
+            st = self._lib.pdn_shard_slice(self._h, t, rank, *[C.byref(x) for x in v])
+            if st != PDN_OK:
+                raise PdnError(st, "pdn_shard_slice")
+            tsv0, ntsv, term0, nterm = [x.value for x in v]
+            zt, ld, ntot, zd = C.c_void_p(), C.c_int64(), C.c_int32(), C.c_void_p()
+            st = self._lib.pdn_shard_buffers(self._h, t, C.byref(zt), C.byref(ld), C.byref(ntot), C.byref(zd))
+            if st != PDN_OK:
+                raise PdnError(st, "pdn_shard_buffers")
+            if ntsv:
+                out.append((t, _device_view(zt.value + 8 * tsv0 * ld.value, ntsv * ld.value)))
+            if nterm:
+                out.append((t, _device_view(zd.value + 8 * term0, nterm)))
+                if self._terminal_rows:
+                    out.append((t, _device_view(zt.value + 8 * (ntot.value + term0) * ld.value, nterm * ld.value)))
+        return out
+
+    def exchange_and_finish(self, dist, world: int):
+        """Every rank broadcasts its pieces (torch.distributed, NCCL over NVLink on GPUs), then S2-S3 run."""
+        for r in range(world):
+            for _, piece in self.shard_pieces(r):
+                dist.broadcast(piece, src=r)
+        self.finish()
+
+    def finish(self):
+        st = self._lib.pdn_finish(self._h)
+        if st != PDN_OK:
+            raise PdnError(st, "pdn_finish")
 
     def stats(self) -> dict:
         s = PdnStats()

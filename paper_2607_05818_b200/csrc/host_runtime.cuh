@@ -124,6 +124,7 @@ struct TierPorts {
     DevBuf ZT;                        // nrows x q
     DevBuf zdiag;                     // nterm
     DevBuf gx0, gy0;                  // sanitised pitched level-0 planes, kept for pdn_update_tsvs
+    bool whole = false;               // reduced whole on this rank (uniform tier, n <= 4): nothing to exchange
 };
 
 }  // namespace
@@ -140,6 +141,8 @@ struct pdn_ctx {
     DevBuf A1, X0, u, w;              // operands of the pair kernel
     struct Side { DevBuf A, X, ys, t; int p = 0; } side[2];  // same-side pairs: [0] bumps, [1] loads (PDN_TERMINAL_PAIRS)
     bool terminal_pairs = false;
+    int shard_rank = 0, shard_world = 1;  // NEXT-4
+    bool open = false;                    // sharded context whose rows have not been completed / S2-S3 not run
     pdn_stats stats{};
     double class_ms[KC_COUNT] = {};
     double class_bytes[KC_COUNT] = {};

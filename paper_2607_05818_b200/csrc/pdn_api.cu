@@ -85,11 +85,13 @@ int pick_batch(const Hierarchy& H, int want, const pdn_opts& o) {
 // S1 of one tier whose hierarchy H has just been built: fills rows `tsv_src` of ZT (each against all ports of
 // the tier) and, if `terminals`, zdiag.  Meshes with n <= 4 and uniform tiers (Eq. 3) are reduced whole.
 int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPorts& T, const std::vector<int>& tsv_src,
-                bool terminals) {
+                const std::vector<int>& term) {  // term: port indices (>= ntsv) of the terminal sources to solve
+    T.whole = false;
     const pdn_opts& o = c->opts;
     const int n = c->n;
     if (H.nlev == 1) {
         L.run(KC_SMALL, 0, [&] { k_direct_small<<<T.q, 64, 0, L.s>>>(H.pinv.as<double>(), n, H.pitch[0], n * n, T.d_node.as<int>(), T.ntsv, T.nrows, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
+        T.whole = true;
         return PDN_OK;
     }
     if (!(o.flags & PDN_NO_UNIFORM_FAST_PATH)) {
@@ -116,6 +118,7 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
             L.run(KC_SMALL, 0, [&] { k_uniform_gather<<<dim3(cdiv(T.q, 128), T.nrows + 1), 128, 0, L.s>>>(Gt.as<double>(), n, H.pitch[0], T.d_node.as<int>(), T.ntsv, T.nrows, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
             CK(cudaStreamSynchronize(L.s));  // the table buffers go back to the pool here
             c->stats.n_uniform_tiers++;
+            T.whole = true;
             return PDN_OK;
         }
     }
@@ -135,15 +138,13 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
     int status = PDN_OK;
     for (size_t s0 = 0; s0 < tsv_src.size() && status == PDN_OK; s0 += Bmax)
         status = solve_batch(c, L, H, W, T, ch, tsv_src.data() + s0, (int)std::min<size_t>(Bmax, tsv_src.size() - s0), false, o.rtol, o.max_iter);
-    if (terminals && T.nterm > 0) {
-        std::vector<int> term(T.nterm);
-        for (int k = 0; k < T.nterm; ++k) term[k] = T.ntsv + k;
+    if (!term.empty()) {
         // with the terminal rows kept they are ordinary rows of ZT: full tolerance, gathered at every port
         const bool rows = c->terminal_pairs;
         for (size_t s0 = 0; s0 < term.size() && status == PDN_OK; s0 += Bmax)
             status = solve_batch(c, L, H, W, T, ch, term.data() + s0, (int)std::min<size_t>(Bmax, term.size() - s0), !rows,
                                  rows ? o.rtol : rtol_term, o.max_iter);
-        if (rows && status == PDN_OK)
+        if (rows && status == PDN_OK && !c->open)  // (an open, sharded context does this in pdn_finish)
             L.run(KC_SMALL, 0, [&] { k_zdiag_from_rows<<<cdiv(T.nterm, 128), 128, 0, L.s>>>(T.ZT.as<double>(), T.q, T.ntsv, T.nterm, T.zdiag.as<double>()); });
     }
     return status;
@@ -212,6 +213,10 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         c->stream = (cudaStream_t)o.cuda_stream;
         c->time_kernels = (o.flags & PDN_TIME_KERNELS) != 0;
         c->terminal_pairs = (o.flags & PDN_TERMINAL_PAIRS) != 0;
+        if (o.shard_world > 1) {
+            if (o.shard_rank < 0 || o.shard_rank >= o.shard_world) throw StatusFail{PDN_E_ARG, "shard_rank out of range"};
+            c->shard_world = o.shard_world; c->shard_rank = o.shard_rank; c->open = true;
+        }
         // ---- host-side validation and port lists
         parse_tsvs(d, n, n_tsv, tsvs, c->site, c->rt);
         c->p.assign(d - 1, 0);
@@ -280,14 +285,17 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
             CK(cudaEventElapsedTime(&ms, ev[1], ev[2]));
             ms_up += ms;
             if (status != PDN_OK) { g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status); break; }
-            std::vector<int> all_tsv(T.ntsv);
-            for (int k = 0; k < T.ntsv; ++k) all_tsv[k] = k;
-            status = reduce_tier(c, L, H, W, Bmax, T, all_tsv, true);
+            // this rank's contiguous slice of the TSV sources and of the terminal sources (everything if unsharded)
+            const int W_ = c->shard_world, r_ = c->shard_rank;
+            std::vector<int> tsv_src, term_src;
+            for (int k = (int)((int64_t)r_ * T.ntsv / W_); k < (int)((int64_t)(r_ + 1) * T.ntsv / W_); ++k) tsv_src.push_back(k);
+            for (int k = (int)((int64_t)r_ * T.nterm / W_); k < (int)((int64_t)(r_ + 1) * T.nterm / W_); ++k) term_src.push_back(T.ntsv + k);
+            status = reduce_tier(c, L, H, W, Bmax, T, tsv_src, term_src);
             if (status != PDN_OK) g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status);
         }
         CK(cudaEventRecord(ev[2], L.s));
-        // ---- S2 + S3
-        if (status == PDN_OK) {
+        // ---- S2 + S3 (a sharded context stays open until its rows are complete: pdn_finish)
+        if (status == PDN_OK && !c->open) {
             status = recombine(c, L);
             if (status != PDN_OK) g_last_error = pdn_strerror(status);
         }
@@ -327,6 +335,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
 // re-factored (milliseconds).
 int pdn_update_tsvs(pdn_ctx* ctx, int32_t n_tsv, const pdn_tsv* tsvs) {
     if (!ctx || !tsvs || n_tsv < 1) return fail_arg("null context / TSV list or empty list");
+    if (ctx->open || ctx->shard_world > 1) return fail_arg("TSV re-planning is not available on a sharded context");
     pdn_ctx* c = ctx;
     const int d = c->d, n = c->n;
     int status = PDN_OK;
@@ -392,7 +401,7 @@ int pdn_update_tsvs(pdn_ctx* ctx, int32_t n_tsv, const pdn_tsv* tsvs) {
                 const int Bmax = pick_batch(H, (int)added.size(), c->opts);
                 Work W;
                 if (H.nlev > 1) W.allocate(H, Bmax, q_n);
-                status = reduce_tier(c, L, H, W, Bmax, T, added, false);
+                status = reduce_tier(c, L, H, W, Bmax, T, added, {});
                 if (status != PDN_OK) { g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status); break; }
                 new_solves += (int64_t)added.size();
                 d_added.alloc(added.size() * sizeof(int));
@@ -449,6 +458,7 @@ static int reff_device(pdn_ctx* ctx, int64_t n_pairs, const int32_t* bi, const i
 
 int pdn_reff(pdn_ctx* ctx, int64_t n_pairs, const int32_t* bump_idx, const int32_t* load_idx, double* out) {
     if (!ctx || !out || n_pairs < 0) return fail_arg("null context / output or negative n_pairs");
+    if (ctx->open) return fail_arg("sharded context is still open: exchange the rows and call pdn_finish first");
     if ((bump_idx == nullptr) != (load_idx == nullptr)) return fail_arg("bump_idx and load_idx must both be given or both be NULL");
     if (!bump_idx && n_pairs != (int64_t)ctx->m * ctx->nl) return fail_arg("full cross product needs n_pairs == n_bumps*n_loads");
     if (n_pairs == 0) return PDN_OK;
@@ -466,6 +476,7 @@ int pdn_reff(pdn_ctx* ctx, int64_t n_pairs, const int32_t* bump_idx, const int32
 
 int pdn_reff_host(pdn_ctx* ctx, int64_t n_pairs, const int32_t* bump_idx, const int32_t* load_idx, double* out) {
     if (!ctx || !out || n_pairs < 0) return fail_arg("null context / output or negative n_pairs");
+    if (ctx->open) return fail_arg("sharded context is still open: exchange the rows and call pdn_finish first");
     if ((bump_idx == nullptr) != (load_idx == nullptr)) return fail_arg("bump_idx and load_idx must both be given or both be NULL");
     if (!bump_idx && n_pairs != (int64_t)ctx->m * ctx->nl) return fail_arg("full cross product needs n_pairs == n_bumps*n_loads");
     if (n_pairs == 0) return PDN_OK;
@@ -499,6 +510,7 @@ void pdn_release_cache(void) { g_pool.trim(); }
 int pdn_reff_same_side(pdn_ctx* ctx, int32_t side, double* out) {
     if (!ctx || !out || (side != 0 && side != 1)) return fail_arg("null context / output or side not in {0, 1}");
     if (!ctx->terminal_pairs) return fail_arg("the context was not created with PDN_TERMINAL_PAIRS");
+    if (ctx->open) return fail_arg("sharded context is still open: exchange the rows and call pdn_finish first");
     try {
         Launcher L{ctx, ctx->stream};
         const pdn_ctx::Side& S = ctx->side[side];
@@ -520,6 +532,7 @@ int pdn_reff_same_side(pdn_ctx* ctx, int32_t side, double* out) {
 int pdn_load_voltages(pdn_ctx* ctx, int32_t bump, const double* i_load, double v_bump, double* v_out) {
     if (!ctx || !i_load || !v_out) return fail_arg("null argument");
     if (!ctx->terminal_pairs) return fail_arg("the context was not created with PDN_TERMINAL_PAIRS");
+    if (ctx->open) return fail_arg("sharded context is still open: exchange the rows and call pdn_finish first");
     if (bump < 0 || bump >= ctx->m) return fail_arg("bump index out of range");
     try {
         Launcher L{ctx, ctx->stream};
@@ -551,6 +564,63 @@ int pdn_load_voltages(pdn_ctx* ctx, int32_t bump, const double* i_load, double v
         return f.status;
     }
     return PDN_OK;
+}
+
+int pdn_shard_slice(const pdn_ctx* ctx, int32_t tier, int32_t rank, int32_t* tsv0, int32_t* ntsv, int32_t* term0,
+                    int32_t* nterm) {
+    if (!ctx || !tsv0 || !ntsv || !term0 || !nterm || tier < 0 || tier >= ctx->d || rank < 0 || rank >= ctx->shard_world)
+        return fail_arg("bad tier / rank or null output");
+    const TierPorts& T = ctx->tiers[tier];
+    const int64_t W_ = ctx->shard_world;
+    *tsv0 = *ntsv = *term0 = *nterm = 0;
+    if (T.whole || W_ <= 1) return PDN_OK;
+    *tsv0 = (int32_t)(rank * (int64_t)T.ntsv / W_);
+    *ntsv = (int32_t)((rank + 1) * (int64_t)T.ntsv / W_) - *tsv0;
+    *term0 = (int32_t)(rank * (int64_t)T.nterm / W_);
+    *nterm = (int32_t)((rank + 1) * (int64_t)T.nterm / W_) - *term0;
+    return PDN_OK;
+}
+
+int pdn_shard_buffers(pdn_ctx* ctx, int32_t tier, double** zt, int64_t* ld, int32_t* ntsv_total, double** zdiag) {
+    if (!ctx || !zt || !ld || !ntsv_total || !zdiag || tier < 0 || tier >= ctx->d) return fail_arg("bad tier or null output");
+    TierPorts& T = ctx->tiers[tier];
+    *zt = T.ZT.as<double>(); *ld = T.q; *ntsv_total = T.ntsv; *zdiag = T.zdiag.as<double>();
+    return PDN_OK;
+}
+
+int pdn_finish(pdn_ctx* ctx) {
+    if (!ctx) return fail_arg("null context");
+    if (!ctx->open) return PDN_OK;
+    int status = PDN_OK;
+    try {
+        Launcher L{ctx, ctx->stream};
+        cudaEvent_t ev[2];
+        for (auto& e : ev) CK(cudaEventCreate(&e));
+        CK(cudaEventRecord(ev[0], L.s));
+        if (ctx->terminal_pairs)
+            for (TierPorts& T : ctx->tiers)
+                if (T.nterm > 0 && !T.whole)
+                    L.run(KC_SMALL, 0, [&] { k_zdiag_from_rows<<<cdiv(T.nterm, 128), 128, 0, L.s>>>(T.ZT.as<double>(), T.q, T.ntsv, T.nterm, T.zdiag.as<double>()); });
+        status = recombine(ctx, L);
+        if (status != PDN_OK) g_last_error = pdn_strerror(status);
+        CK(cudaEventRecord(ev[1], L.s));
+        CK(cudaStreamSynchronize(L.s));
+        L.resolve();
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, ev[0], ev[1]));
+        ctx->stats.ms_dense = ms;
+        ctx->stats.ms_total += ms;
+        for (auto& e : ev) cudaEventDestroy(e);
+        if (status == PDN_OK) ctx->open = false;
+    } catch (const CudaFail& f) {
+        g_last_error = std::string(f.what) + ": " + cudaGetErrorString(f.e);
+        cudaGetLastError();
+        status = f.e == cudaErrorMemoryAllocation ? PDN_E_NOMEM : PDN_E_CUDA;
+    } catch (const StatusFail& f) {
+        g_last_error = f.msg;
+        status = f.status;
+    }
+    return status;
 }
 
 int pdn_get_stats(const pdn_ctx* ctx, pdn_stats* out) {

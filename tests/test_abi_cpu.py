@@ -34,7 +34,7 @@ def test_library_builds_loads_and_exports_every_declared_symbol():
 def test_struct_sizes_match_the_header_layout():
     from paper_2607_05818_b200 import binding as b
     assert ctypes.sizeof(b.PdnTier) == 24 and ctypes.sizeof(b.PdnTsv) == 24 and ctypes.sizeof(b.PdnSite) == 8
-    assert ctypes.sizeof(b.PdnOpts) == 40
+    assert ctypes.sizeof(b.PdnOpts) == 48
     assert ctypes.sizeof(b.PdnStats) == 16 + 16 + 8 + 8 + 8 + 4 * 8 + 8 + 24 + 3 * 64
 
 

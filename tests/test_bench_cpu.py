@@ -61,3 +61,36 @@ def test_max_over_ranks_and_per_rank_networks_gloo_world2(tmp_path):
              "127.0.0.1", "--master-port", "29542", str(w)], env=env)
     assert r.returncode == 0, r.stderr[-2000:]
     assert r.stdout.count("ok") == 2
+
+
+_SHARD_WORKER = r"""
+import os, sys, torch, torch.distributed as dist
+sys.path.insert(0, os.getcwd())
+from paper_2607_05818_b200 import shard_bounds
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+# the exchange Pdn.exchange_and_finish does, on CPU tensors: rank r owns rows shard_bounds(k, world)[r] of a k x q
+# matrix; after one broadcast per rank every rank holds the whole matrix
+k, q = 11, 5
+full = torch.arange(k * q, dtype=torch.float64).reshape(k, q)
+mine = torch.full((k, q), float("nan"), dtype=torch.float64)
+lo, hi = shard_bounds(k, world)[rank]
+mine[lo:hi] = full[lo:hi]
+for r, (a, b) in enumerate(shard_bounds(k, world)):
+    piece = mine[a:b].reshape(-1)          # contiguous view, as the row slices of the port matrix are
+    dist.broadcast(piece, src=r)
+assert torch.equal(mine, full)
+assert shard_bounds(10, 4) == [(0, 2), (2, 5), (5, 7), (7, 10)] and shard_bounds(3, 2) == [(0, 1), (1, 3)]
+dist.destroy_process_group()
+print("ok", rank)
+"""
+
+
+def test_shard_bounds_and_row_exchange_gloo_world2(tmp_path):
+    w = tmp_path / "shard_worker.py"
+    w.write_text(_SHARD_WORKER)
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1")
+    r = run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
+             "127.0.0.1", "--master-port", "29543", str(w)], env=env)
+    assert r.returncode == 0, r.stderr[-2000:]
+    assert r.stdout.count("ok") == 2

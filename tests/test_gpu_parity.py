@@ -403,6 +403,47 @@ def test_bump_on_tsv_site_and_shared_sites_between_interfaces():
     check(got, Oracle(net).reff_all())
 
 
+@pytest.mark.parametrize("world,flags_name", [(2, None), (3, "PDN_TERMINAL_PAIRS")])
+def test_sharded_port_solves_emulated_on_one_gpu(world, flags_name):
+    """NEXT-4: `world` open contexts in one process play the ranks of a sharded run: each solves its slice of
+    every tier's sources, the rows are exchanged (here: device copies between the contexts' buffers -- what a
+    broadcast per rank does across GPUs), pdn_finish runs S2-S3 everywhere; every rank then equals the
+    unsharded result and the oracle."""
+    from oracle.reff_oracle import Oracle
+    import paper_2607_05818_b200 as pkg
+    from paper_2607_05818_b200 import Pdn, PdnError
+    torch = torch_cuda()
+    flags = getattr(pkg, flags_name) if flags_name else 0
+    net = P.make_random(71, d=3, n=47, p=7, m=5, nl=6, drop=0.03)
+    net.gx[1], net.gy[1] = P._planes(net.n, np.full((net.n, net.n), 0.8), np.full((net.n, net.n), 1.3))  # a uniform tier
+    ref, _ = gpu_all_pairs(net, rtol=1e-10, flags=flags)
+    ranks = [Pdn.from_network(net, device="cuda:0", rtol=1e-10, flags=flags, shard_rank=r, shard_world=world)
+             for r in range(world)]
+    out = torch.empty(net.m * net.nl, dtype=torch.float64, device="cuda:0")
+    with pytest.raises(PdnError):
+        ranks[0].reff(out)                      # still open
+    for src in range(world):                    # "broadcast" of rank src's pieces to everybody else
+        pieces = [r.shard_pieces(src) for r in ranks]
+        for k, (_, mine) in enumerate(pieces[src]):
+            for dst in range(world):
+                if dst != src:
+                    assert pieces[dst][k][1].numel() == mine.numel()
+                    pieces[dst][k][1].copy_(mine)
+    for r in ranks:
+        r.finish()
+        r.reff(out)
+        got = out.cpu().numpy().reshape(net.m, net.nl)
+        assert np.allclose(got, ref, rtol=1e-9, atol=0)
+        check(got, Oracle(net).reff_all())
+        if flags:
+            ll = torch.empty(net.nl * net.nl, dtype=torch.float64, device="cuda:0")
+            r.reff_same_side(1, ll)
+            want = Oracle(net).reff_same_side(1)
+            off = ~np.eye(net.nl, dtype=bool)
+            assert (np.abs(ll.cpu().numpy().reshape(net.nl, net.nl)[off] - want[off]) / want[off]).max() <= MAX_REL
+        r.close()
+
+
 def test_two_host_threads_with_their_own_contexts():
     """The library is thread-compatible: contexts created and used concurrently from two host threads (shared
     device-memory pool, per-thread pinned scratch) give the same results as one after the other."""
