@@ -335,6 +335,27 @@ def run_cuda(a):
                           "port_solves_per_update": int(stu["update_solves"]), "ms_solves": stu["ms_update_stencil"],
                           "ms_refactor": stu["ms_update_dense"], "ms_full_step": ms / a.steps,
                           "pairs_per_s": npairs / float(np.mean(times))}
+    if a.emulate_shards > 1:   # NEXT-4: per-rank compute of a sharded run, measured on this one GPU
+        emu = {}
+        w_ = 2
+        while w_ <= a.emulate_shards:
+            ts = []
+            for rep in range(a.warmup + a.steps):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                pdn = Pdn(net.n, gx_d, gy_d, *args[1], flags=base_flags, rtol=a.rtol, nu=a.nu, rhs_batch=a.rhs_batch,
+                          shard_rank=rep % w_, shard_world=w_)
+                torch.cuda.synchronize()
+                t1 = time.perf_counter()
+                pieces = sum(v.numel() * 8 for _, v in pdn.shard_pieces(rep % w_))
+                pdn.close()           # (pdn_finish needs every rank's rows: S2-S3 time is the unsharded run's ms_dense)
+                if rep >= a.warmup:
+                    ts.append((t1 - t0, pieces))
+            emu[str(w_)] = {"ms_rank_solves": 1e3 * float(np.mean([t[0] for t in ts])),
+                            "ms_s2_s3_replicated": last["ms_dense"],
+                            "bytes_rank_broadcasts": int(np.mean([t[1] for t in ts]))}
+            w_ *= 2
+        line["shard_emulation"] = {"ms_full_step_1gpu": ms / a.steps, "per_world": emu}
     if a.eq4:   # NEXT-3: same-side pairs and Eq. (4) voltages
         nl = net.nl
         rll = torch.empty(nl * nl, dtype=torch.float64, device=dev)
@@ -398,6 +419,9 @@ def main():
     ap.add_argument("--shard", action="store_true",
                     help="N > 1: ONE network, its port solves sharded over the ranks (NEXT-4, strong scaling) instead "
                          "of one independent network per rank")
+    ap.add_argument("--emulate-shards", type=int, default=0, metavar="W",
+                    help="1 GPU: also time what ONE rank of a W-rank sharded run computes (its slice of the port solves + "
+                         "S2-S3), for W = 2, 4, ... <= W; the row exchange is not included (NEXT-4 estimate)")
     ap.add_argument("--only-device", action="store_true", help="run only the device-resident steps (for ncu)")
     a = ap.parse_args()
     if a.impl == "reference":
