@@ -389,6 +389,37 @@ def run_cuda(a):
         line["eq4"] = {"ms_create_with_terminal_pairs": 1e3 * float(np.mean(t_create)), "ms_create_default": ms / a.steps,
                        "load_load_pairs": nl * nl, "ms_load_load": ms_ll, "load_load_pairs_per_s": nl * nl / (ms_ll * 1e-3),
                        "ms_voltages_one_bump": ms_v}
+    if a.nodes > 0:   # NEXT-3: arbitrary-tier endpoints (pdn_reff_nodes) and an R_eff map (Fig. 6(d))
+        rng = np.random.default_rng(12345)
+        k = a.nodes
+        nodes = np.stack([rng.integers(0, net.d, k), rng.integers(0, net.n, k), rng.integers(0, net.n, k)], axis=1).astype(np.int32)
+        out_n = torch.empty(k * k, dtype=torch.float64, device=dev)
+        pdn = Pdn(net.n, gx_d, gy_d, *args[1], flags=base_flags, rtol=a.rtol, nu=a.nu, rhs_batch=a.rhs_batch)
+        tn, tm = [], []
+        stride = max(1, net.n // 32)
+        for rep in range(a.warmup + a.steps):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            pdn.reff_nodes(nodes, out_n)
+            torch.cuda.synchronize()
+            t1 = time.perf_counter()
+            rmap = pdn.reff_map((0, int(net.bumps[0][0]), int(net.bumps[0][1])), net.d - 1, stride)
+            t2 = time.perf_counter()
+            if rep >= a.warmup:
+                tn.append(t1 - t0)
+                tm.append(t2 - t1)
+        pdn.close()
+        line["nodes"] = {"probes": k, "pairs": k * k, "ms_reff_nodes": 1e3 * float(np.mean(tn)),
+                         "pairs_per_s": k * k / float(np.mean(tn)), "map_points": int(rmap.size),
+                         "ms_reff_map": 1e3 * float(np.mean(tm)), "ms_create": ms / a.steps}
+        if a.nodes_check > 0:   # a few pairs against the oracle (factors the whole 3D system on the host: minutes)
+            from oracle.reff_oracle import Oracle
+            o = Oracle(net)
+            got = out_n.cpu().numpy().reshape(k, k)
+            gid = nodes[:, 0].astype(np.int64) * net.n * net.n + nodes[:, 1] * net.n + nodes[:, 2]
+            pa, pb = rng.integers(0, k, a.nodes_check), rng.integers(0, k, a.nodes_check)
+            rel = [abs(got[i, j] / o.reff_nodes(int(gid[i]), int(gid[j])) - 1.0) for i, j in zip(pa, pb) if gid[i] != gid[j]]
+            line["nodes"]["parity"] = {"pairs_checked": len(rel), "max_rel_err": float(np.max(rel)), "mean_rel_err": float(np.mean(rel))}
     if not a.no_cpu_baseline:
         ot = OracleTimer(cfg)
         n, t = ot.sample(a.cpu_budget)
@@ -416,6 +447,9 @@ def main():
                     help="also time pdn_update_tsvs after moving K TSVs of every interface to new sites (NEXT-2)")
     ap.add_argument("--eq4", action="store_true",
                     help="also time the NEXT-3 leg: context with PDN_TERMINAL_PAIRS, load-load R_eff, Eq. (4) voltages")
+    ap.add_argument("--nodes", type=int, default=0, metavar="K",
+                    help="also time pdn_reff_nodes on K random probes over all tiers and an R_eff map of the bottom tier (NEXT-3)")
+    ap.add_argument("--nodes-check", type=int, default=0, metavar="J", help="with --nodes: check J of the pairs against the oracle")
     ap.add_argument("--shard", action="store_true",
                     help="N > 1: ONE network, its port solves sharded over the ranks (NEXT-4, strong scaling) instead "
                          "of one independent network per rank")

@@ -168,6 +168,18 @@ int pdn_reff_same_side(pdn_ctx *ctx, int32_t side, double *out);
  *   v_j = v_bump - 1/2 sum_k i_load[k] (R_{b,j} + R_{b,k} - R_{j,k}).   Needs PDN_TERMINAL_PAIRS. */
 int pdn_load_voltages(pdn_ctx *ctx, int32_t bump, const double *i_load, double v_bump, double *v_out);
 
+/* Arbitrary-tier endpoints: R_eff in the whole 3D network between ANY nodes, on any
+ * tier, of an existing context (any flags).  nodes: HOST array of n_nodes probes (duplicates allowed).  out:
+ * DEVICE fp64, n_nodes*n_nodes values, out[a*n_nodes + b] = R_eff(node a, node b), 0 on the diagonal.
+ * Cost: one port solve per probe on its own tier (full tolerance, gathered at the tier's TSV ends and at the
+ * other probes of that tier), then one substitution with the factor of C kept since pdn_create / the last
+ * pdn_update_tsvs (Eq. (18)-(22) PAPER.md:179-204 with the source / sink on arbitrary tiers; DESIGN.md
+ * section 1).  The context is not changed.  Not available on a sharded context (PDN_E_ARG). */
+typedef struct pdn_node {
+    int32_t tier, y, x;
+} pdn_node;
+int pdn_reff_nodes(pdn_ctx *ctx, int32_t n_nodes, const pdn_node *nodes, double *out);
+
 /* NEXT-4: one network sharded over several GPUs, one process per GPU.  The port solves of
  * a tier are independent, so with opts->shard_world = W > 1 pdn_create (same arguments on every
  * rank) imports all tiers but solves only slice opts->shard_rank of each tier's TSV sources and of its bump / load

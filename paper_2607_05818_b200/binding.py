@@ -53,7 +53,7 @@ class PdnStats(C.Structure):
 
 
 EXPORTS = ("pdn_create", "pdn_reff", "pdn_reff_host", "pdn_destroy", "pdn_strerror", "pdn_last_error",
-           "pdn_get_stats", "pdn_port_count", "pdn_get_port_matrix", "pdn_release_cache", "pdn_update_tsvs", "pdn_reff_same_side", "pdn_load_voltages", "pdn_shard_slice", "pdn_shard_buffers", "pdn_finish")
+           "pdn_get_stats", "pdn_port_count", "pdn_get_port_matrix", "pdn_release_cache", "pdn_update_tsvs", "pdn_reff_same_side", "pdn_load_voltages", "pdn_reff_nodes", "pdn_shard_slice", "pdn_shard_buffers", "pdn_finish")
 
 _lib = None
 
@@ -86,6 +86,8 @@ def load_library() -> C.CDLL:
     lib.pdn_reff_same_side.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
     lib.pdn_load_voltages.restype = C.c_int
     lib.pdn_load_voltages.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_double, C.c_void_p]
+    lib.pdn_reff_nodes.restype = C.c_int
+    lib.pdn_reff_nodes.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
     lib.pdn_shard_slice.restype = C.c_int
     lib.pdn_shard_slice.argtypes = [C.c_void_p, C.c_int32, C.c_int32] + [C.POINTER(C.c_int32)] * 4
     lib.pdn_shard_buffers.restype = C.c_int
@@ -193,6 +195,7 @@ class Pdn:
                        flags=flags | (PDN_TIERS_ON_HOST if on_host else 0), nu=nu, cheb_ratio=cheb_ratio,
                        shard_rank=shard_rank, shard_world=shard_world)
         self.d = d
+        self.n = n
         h = C.c_void_p()
         b_arr, l_arr = _sites(bumps), _sites(loads)
         st = lib.pdn_create(C.byref(h), d, tiers, ntsv, tsvs.ctypes.data_as(C.POINTER(PdnTsv)), self.m,
@@ -252,6 +255,29 @@ class Pdn:
         if st != PDN_OK:
             raise PdnError(st, "pdn_load_voltages")
         return v_out
+
+    def reff_nodes(self, nodes, out):
+        """pdn_reff_nodes: `nodes` is an (k, 3) integer array of (tier, y, x) probes on the host, `out` a torch CUDA
+        tensor of k*k doubles that receives R_eff between every two of them."""
+        nd = np.ascontiguousarray(np.asarray(nodes, dtype=np.int32).reshape(-1, 3))
+        st = self._lib.pdn_reff_nodes(self._h, int(nd.shape[0]), nd.ctypes.data, _ptr(out))
+        if st != PDN_OK:
+            raise PdnError(st, "pdn_reff_nodes")
+        return out
+
+    def reff_map(self, src, tier: int, stride: int = 1):
+        """R_eff map (Fig. 6(d) of the paper): effective resistance from the node `src` = (tier, y, x)
+        to every `stride`-th node (rows and columns 0, stride, 2*stride, ...) of tier `tier`, as a 2-D numpy array.
+        One pdn_reff_nodes call with the source and the grid nodes as probes; only marshalling and slicing here."""
+        import torch
+        ys = np.arange(0, self.n, stride, dtype=np.int32)
+        yy, xx = np.meshgrid(ys, ys, indexing="ij")
+        nodes = np.vstack([np.asarray(src, dtype=np.int32).reshape(1, 3),
+                           np.stack([np.full(yy.size, tier, dtype=np.int32), yy.ravel(), xx.ravel()], axis=1)])
+        k = nodes.shape[0]
+        out = torch.empty(k * k, dtype=torch.float64, device="cuda")
+        self.reff_nodes(nodes, out)
+        return out[1:k].cpu().numpy().reshape(ys.size, ys.size)
 
     # ---- NEXT-4: one network sharded over several GPUs (argument marshalling + the exchange plumbing only)
     def shard_pieces(self, rank: int):

@@ -45,12 +45,47 @@ void trsm_fwd(Launcher& L, const double* Lm, int64_t lda, int n, double* Bm, int
 }
 
 // ------------------------------------------------------------------------------------------------
+// F_i <- (K^-1 F)_i for the block rows F_i (p_i x nrhs) of any right-hand-side set, with the factor kept in the
+// context (c->Li[i] = L_i^-1, c->Vf[i] = L_{i-1}^-1 K_{i-1,i}): forward then backward block substitution, every
+// step a contraction on the FP64 tensor cores.
+void block_substitute(pdn_ctx* c, Launcher& L, std::vector<DevBuf>& F, int nrhs) {
+    const int dm1 = c->d - 1;
+    DevBuf tmp;
+    size_t tmax = 0;
+    for (int i = 0; i < dm1; ++i) tmax = std::max(tmax, (size_t)c->p[i] * nrhs);
+    tmp.alloc(tmax * sizeof(double));
+    for (int i = 0; i < dm1; ++i) {
+        const int pi = c->p[i];
+        if (i > 0) gemm(L, pi, nrhs, c->p[i - 1], -1.0, c->Vf[i].as<double>(), 1, pi, F[i - 1].as<double>(), nrhs, 1, 1.0, F[i].as<double>(), nrhs);
+        // F_i <- L_i^-1 F_i
+        gemm(L, pi, nrhs, pi, 1.0, c->Li[i].as<double>(), pi, 1, F[i].as<double>(), nrhs, 1, 0.0, tmp.as<double>(), nrhs);
+        CK(cudaMemcpyAsync(F[i].p, tmp.p, (size_t)pi * nrhs * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
+    }
+    for (int i = dm1 - 1; i >= 0; --i) {
+        const int pi = c->p[i];
+        if (i + 1 < dm1) {
+            const int pj = c->p[i + 1];
+            gemm(L, pi, nrhs, pj, -1.0, c->Vf[i + 1].as<double>(), pj, 1, F[i + 1].as<double>(), nrhs, 1, 1.0, F[i].as<double>(), nrhs);
+        }
+        // F_i <- L_i^-T F_i
+        gemm(L, pi, nrhs, pi, 1.0, c->Li[i].as<double>(), 1, pi, F[i].as<double>(), nrhs, 1, 0.0, tmp.as<double>(), nrhs);
+        CK(cudaMemcpyAsync(F[i].p, tmp.p, (size_t)pi * nrhs * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
+    }
+    CK(cudaStreamSynchronize(L.s));  // tmp goes back to the pool here
+}
+
 // S2 + S3: assemble C = [K B; B^T 0] (block-tridiagonal SPD K), factor it once, substitute for the
-// m + n + (d-1) right-hand sides, eliminate the multipliers, and leave the pair-kernel operands.
+// m + n + (d-1) right-hand sides, eliminate the multipliers, and leave the pair-kernel operands.  The factor
+// (L_i^-1, the transformed couplings, K^-1 B and S^-1) stays in the context for pdn_reff_nodes.
 int recombine(pdn_ctx* c, Launcher& L) {
     const int d = c->d, dm1 = d - 1, m = c->m, n = c->nl, mn = m + n, nrhs = mn + dm1;
-    std::vector<DevBuf> Kd(dm1), V(dm1), F(dm1), rt(dm1);
-    DevBuf G, Sinv, Y, fail;
+    std::vector<DevBuf> Kd(dm1), F(dm1), rt(dm1);
+    std::vector<DevBuf>& V = c->Vf;
+    std::vector<DevBuf>& Li = c->Li;
+    V.clear(); V.resize(dm1);
+    Li.clear(); Li.resize(dm1);
+    DevBuf G, Y, fail;
+    DevBuf& Sinv = c->Sinv;
     for (int i = 0; i < dm1; ++i) {
         const size_t pi = c->p[i];
         Kd[i].alloc(pi * pi * sizeof(double));
@@ -78,45 +113,37 @@ int recombine(pdn_ctx* c, Launcher& L) {
         }
         L.run(KC_DENSE, 0, [&] { k_assemble_rhs<<<dim3(cdiv(nrhs, 128), pi), 128, 0, L.s>>>(i, dm1, pi, m, n, T0.ZT.as<double>(), T0.q, T0.ntsv, Td.ZT.as<double>(), Td.q, Td.ntsv, F[i].as<double>()); });
     }
-    // block-tridiagonal Cholesky + forward substitution.  Every diagonal factor L_i (p_i x p_i, cond ~ 1e2) is
-    // inverted once by a p_i-column triangular solve; all substitutions for the m + n + d-1 right-hand sides
-    // are then K = p_i contractions on the FP64 tensor cores instead of 32-wide panel solves.
-    std::vector<DevBuf> Li(dm1);
-    DevBuf tmp;
+    // block-tridiagonal Cholesky.  Every diagonal factor L_i (p_i x p_i, cond ~ 1e2) is inverted once by a
+    // p_i-column triangular solve; all substitutions are then K = p_i contractions on the FP64 tensor cores
+    // instead of 32-wide panel solves.
     {
-        size_t tmax = 0;
-        for (int i = 0; i < dm1; ++i) tmax = std::max(tmax, (size_t)c->p[i] * std::max(nrhs, c->p[i]));
+        DevBuf tmp;
+        size_t tmax = 1;
         for (int i = 1; i < dm1; ++i) tmax = std::max(tmax, (size_t)c->p[i - 1] * c->p[i]);
         tmp.alloc(tmax * sizeof(double));
+        for (int i = 0; i < dm1; ++i) {
+            const int pi = c->p[i];
+            if (i > 0) {
+                const int ph = c->p[i - 1];
+                // V_i <- L_{i-1}^-1 V_i
+                gemm(L, ph, pi, ph, 1.0, Li[i - 1].as<double>(), ph, 1, V[i].as<double>(), pi, 1, 0.0, tmp.as<double>(), pi);
+                CK(cudaMemcpyAsync(V[i].p, tmp.p, (size_t)ph * pi * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
+                gemm(L, pi, pi, ph, -1.0, V[i].as<double>(), 1, pi, V[i].as<double>(), pi, 1, 1.0, Kd[i].as<double>(), pi);
+            }
+            potrf(L, Kd[i].as<double>(), pi, pi, fail.as<int>());
+            Li[i].alloc((size_t)pi * pi * sizeof(double));
+            L.run(KC_DENSE, 0, [&] { k_set_identity<<<cdiv((size_t)pi * pi, 256), 256, 0, L.s>>>(pi, Li[i].as<double>()); });
+            trsm_fwd(L, Kd[i].as<double>(), pi, pi, Li[i].as<double>(), pi, pi);
+        }
+        CK(cudaStreamSynchronize(L.s));
     }
+    block_substitute(c, L, F, nrhs);
+    // keep K^-1 B (the last d-1 columns) for later right-hand sides
+    c->KB.clear(); c->KB.resize(dm1);
     for (int i = 0; i < dm1; ++i) {
-        const int pi = c->p[i];
-        if (i > 0) {
-            const int ph = c->p[i - 1];
-            // V_i <- L_{i-1}^-1 V_i
-            gemm(L, ph, pi, ph, 1.0, Li[i - 1].as<double>(), ph, 1, V[i].as<double>(), pi, 1, 0.0, tmp.as<double>(), pi);
-            CK(cudaMemcpyAsync(V[i].p, tmp.p, (size_t)ph * pi * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
-            gemm(L, pi, pi, ph, -1.0, V[i].as<double>(), 1, pi, V[i].as<double>(), pi, 1, 1.0, Kd[i].as<double>(), pi);
-            gemm(L, pi, nrhs, ph, -1.0, V[i].as<double>(), 1, pi, F[i - 1].as<double>(), nrhs, 1, 1.0, F[i].as<double>(), nrhs);
-        }
-        potrf(L, Kd[i].as<double>(), pi, pi, fail.as<int>());
-        Li[i].alloc((size_t)pi * pi * sizeof(double));
-        L.run(KC_DENSE, 0, [&] { k_set_identity<<<cdiv((size_t)pi * pi, 256), 256, 0, L.s>>>(pi, Li[i].as<double>()); });
-        trsm_fwd(L, Kd[i].as<double>(), pi, pi, Li[i].as<double>(), pi, pi);
-        // F_i <- L_i^-1 F_i
-        gemm(L, pi, nrhs, pi, 1.0, Li[i].as<double>(), pi, 1, F[i].as<double>(), nrhs, 1, 0.0, tmp.as<double>(), nrhs);
-        CK(cudaMemcpyAsync(F[i].p, tmp.p, (size_t)pi * nrhs * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
-    }
-    // backward substitution
-    for (int i = dm1 - 1; i >= 0; --i) {
-        const int pi = c->p[i];
-        if (i + 1 < dm1) {
-            const int pj = c->p[i + 1];
-            gemm(L, pi, nrhs, pj, -1.0, V[i + 1].as<double>(), pj, 1, F[i + 1].as<double>(), nrhs, 1, 1.0, F[i].as<double>(), nrhs);
-        }
-        // F_i <- L_i^-T F_i
-        gemm(L, pi, nrhs, pi, 1.0, Li[i].as<double>(), 1, pi, F[i].as<double>(), nrhs, 1, 0.0, tmp.as<double>(), nrhs);
-        CK(cudaMemcpyAsync(F[i].p, tmp.p, (size_t)pi * nrhs * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
+        c->KB[i].alloc((size_t)c->p[i] * dm1 * sizeof(double));
+        CK(cudaMemcpy2DAsync(c->KB[i].p, (size_t)dm1 * sizeof(double), F[i].as<double>() + mn, (size_t)nrhs * sizeof(double),
+                             (size_t)dm1 * sizeof(double), (size_t)c->p[i], cudaMemcpyDeviceToDevice, L.s));
     }
     // multipliers (Schur complement on the d-1 constraints, Eq. 8) and TSV currents
     for (int i = 0; i < dm1; ++i)

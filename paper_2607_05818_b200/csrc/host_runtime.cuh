@@ -140,6 +140,8 @@ struct pdn_ctx {
     std::vector<TierPorts> tiers;
     DevBuf A1, X0, u, w;              // operands of the pair kernel
     struct Side { DevBuf A, X, ys, t; int p = 0; } side[2];  // same-side pairs: [0] bumps, [1] loads (PDN_TERMINAL_PAIRS)
+    std::vector<DevBuf> Li, Vf, KB;   // factor of C kept for pdn_reff_nodes: L_i^-1, L_{i-1}^-1 K_{i-1,i}, (K^-1 B)_i
+    DevBuf Sinv;                      // inverse of the Schur complement B^T K^-1 B ((d-1)^2)
     bool terminal_pairs = false;
     int shard_rank = 0, shard_world = 1;  // NEXT-4
     bool open = false;                    // sharded context whose rows have not been completed / S2-S3 not run

@@ -566,6 +566,107 @@ int pdn_load_voltages(pdn_ctx* ctx, int32_t bump, const double* i_load, double v
     return PDN_OK;
 }
 
+// NEXT-3: arbitrary-tier endpoints (port.cuh "Arbitrary-tier endpoints" has the algebra).
+int pdn_reff_nodes(pdn_ctx* ctx, int32_t n_nodes, const pdn_node* nodes, double* out) {
+    if (!ctx || !nodes || !out || n_nodes < 1) return fail_arg("null context / node list / output or empty list");
+    if (ctx->open || ctx->shard_world > 1) return fail_arg("pdn_reff_nodes is not available on a sharded context");
+    pdn_ctx* c = ctx;
+    const int d = c->d, n = c->n, dm1 = d - 1, np = n_nodes;
+    for (int a = 0; a < np; ++a) {
+        if (nodes[a].tier < 0 || nodes[a].tier >= d) return fail_arg("probe tier out of range");
+        if (nodes[a].y < 0 || nodes[a].y >= n || nodes[a].x < 0 || nodes[a].x >= n) return fail_arg("probe site out of range");
+    }
+    int status = PDN_OK;
+    const pdn_stats stats0 = c->stats;  // the solve statistics describe pdn_create / pdn_update_tsvs only
+    try {
+        Launcher L{c, c->stream};
+        std::vector<DevBuf> F(dm1), X(dm1);
+        DevBuf M, G, Cs, mu, d_tier;
+        for (int i = 0; i < dm1; ++i) {
+            F[i].alloc((size_t)c->p[i] * np * sizeof(double));
+            X[i].alloc((size_t)c->p[i] * np * sizeof(double));
+            CK(cudaMemsetAsync(F[i].p, 0, (size_t)c->p[i] * np * sizeof(double), L.s));
+        }
+        M.alloc((size_t)np * np * sizeof(double));
+        CK(cudaMemsetAsync(M.p, 0, (size_t)np * np * sizeof(double), L.s));
+        std::vector<int> h_tier(np);
+        for (int a = 0; a < np; ++a) h_tier[a] = nodes[a].tier;
+        d_tier.alloc((size_t)np * sizeof(int));
+        CK(cudaMemcpyAsync(d_tier.p, h_tier.data(), (size_t)np * sizeof(int), cudaMemcpyHostToDevice, L.s));
+        // ---- one port solve per probe, tier by tier
+        Hierarchy H;
+        bool h_ready = false;
+        for (int t = 0; t < d && status == PDN_OK; ++t) {
+            std::vector<int> probe;
+            for (int a = 0; a < np; ++a) if (nodes[a].tier == t) probe.push_back(a);
+            if (probe.empty()) continue;
+            const TierPorts& T = c->tiers[t];
+            const int k = (int)probe.size();
+            TierPorts Tp;
+            Tp.node.assign(T.node.begin(), T.node.begin() + T.ntsv);
+            for (int a : probe) Tp.node.push_back(nodes[a].y * pitch_of(n) + nodes[a].x);
+            Tp.ntsv = T.ntsv; Tp.nterm = k; Tp.q = T.ntsv + k; Tp.nrows = Tp.q;
+            Tp.d_node.alloc((size_t)Tp.q * sizeof(int));
+            CK(cudaMemcpyAsync(Tp.d_node.p, Tp.node.data(), (size_t)Tp.q * sizeof(int), cudaMemcpyHostToDevice, L.s));
+            Tp.ZT.alloc((size_t)Tp.q * Tp.q * sizeof(double));
+            Tp.zdiag.alloc((size_t)k * sizeof(double));
+            if (!h_ready) { H.allocate(n); h_ready = true; }
+            status = H.build(L, T.gx0.as<double>(), T.gy0.as<double>(), false, true);
+            if (status != PDN_OK) break;
+            const int Bmax = pick_batch(H, k, c->opts);
+            Work W;
+            if (H.nlev > 1) W.allocate(H, Bmax, Tp.q);
+            std::vector<int> src(k);
+            for (int j = 0; j < k; ++j) src[j] = T.ntsv + j;
+            status = reduce_tier(c, L, H, W, Bmax, Tp, src, {});
+            if (status != PDN_OK) { g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status); break; }
+            DevBuf d_probe;
+            d_probe.alloc((size_t)k * sizeof(int));
+            CK(cudaMemcpyAsync(d_probe.p, probe.data(), (size_t)k * sizeof(int), cudaMemcpyHostToDevice, L.s));
+            const int plo = t > 0 ? c->p[t - 1] : 0;
+            double* Fup = t < dm1 ? F[t].as<double>() : nullptr;
+            double* Flo = t > 0 ? F[t - 1].as<double>() : nullptr;
+            L.run(KC_DENSE, 0, [&] { k_probe_scatter<<<dim3(cdiv(Tp.q, 128), k), 128, 0, L.s>>>(k, T.ntsv, plo, np, d_probe.as<int>(), Tp.ZT.as<double>(), Fup, Flo, M.as<double>()); });
+            CK(cudaStreamSynchronize(L.s));  // probe (host vector) and the tier's buffers are released here
+        }
+        if (status == PDN_OK) {
+            // ---- X = currents of C^-1 [F; Cs];  M -= F^T X + Cs^T mu
+            for (int i = 0; i < dm1; ++i) CK(cudaMemcpyAsync(X[i].p, F[i].p, (size_t)c->p[i] * np * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
+            block_substitute(c, L, X, np);
+            G.alloc((size_t)dm1 * np * sizeof(double));
+            Cs.alloc((size_t)dm1 * np * sizeof(double));
+            mu.alloc((size_t)dm1 * np * sizeof(double));
+            for (int i = 0; i < dm1; ++i)
+                L.run(KC_DENSE, 0, [&] { k_colsum<<<cdiv(np, 128), 128, 0, L.s>>>(c->p[i], np, X[i].as<double>(), G.as<double>() + (size_t)i * np); });
+            L.run(KC_DENSE, 0, [&] { k_probe_multipliers<<<cdiv(np, 128), 128, 0, L.s>>>(dm1, np, G.as<double>(), c->Sinv.as<double>(), d_tier.as<int>(), Cs.as<double>(), mu.as<double>()); });
+            for (int i = 0; i < dm1; ++i) {
+                const int pi = c->p[i];
+                gemm(L, pi, np, dm1, -1.0, c->KB[i].as<double>(), dm1, 1, mu.as<double>(), np, 1, 1.0, X[i].as<double>(), np);
+                gemm(L, np, np, pi, -1.0, F[i].as<double>(), 1, np, X[i].as<double>(), np, 1, 1.0, M.as<double>(), np);
+            }
+            gemm(L, np, np, dm1, -1.0, Cs.as<double>(), 1, np, mu.as<double>(), np, 1, 1.0, M.as<double>(), np);
+            L.run(KC_PAIR, (double)np * np * 8.0, [&] { k_probe_pairs<<<dim3(cdiv(np, 128), np), 128, 0, L.s>>>(np, M.as<double>(), out); });
+        }
+        CK(cudaStreamSynchronize(L.s));
+        L.resolve();
+    } catch (const CudaFail& f) {
+        g_last_error = std::string(f.what) + ": " + cudaGetErrorString(f.e);
+        cudaGetLastError();
+        status = f.e == cudaErrorMemoryAllocation ? PDN_E_NOMEM : PDN_E_CUDA;
+    } catch (const StatusFail& f) {
+        g_last_error = f.msg;
+        status = f.status;
+    } catch (const std::bad_alloc&) {
+        g_last_error = "host allocation failed";
+        status = PDN_E_NOMEM;
+    }
+    const int64_t launches = c->stats.kernel_launches, stencil_launches = c->stats.stencil_launches;
+    c->stats = stats0;
+    c->stats.kernel_launches = launches;
+    c->stats.stencil_launches = stencil_launches;
+    return status;
+}
+
 int pdn_shard_slice(const pdn_ctx* ctx, int32_t tier, int32_t rank, int32_t* tsv0, int32_t* ntsv, int32_t* term0,
                     int32_t* nterm) {
     if (!ctx || !tsv0 || !ntsv || !term0 || !nterm || tier < 0 || tier >= ctx->d || rank < 0 || rank >= ctx->shard_world)

@@ -210,6 +210,55 @@ k_pair_same(int nt, int p, const double* __restrict__ A, const double* __restric
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Arbitrary-tier endpoints (pdn_reff_nodes).  A unit current entering at probe a (tier t_a) is the right-hand
+// side  b_a = [f_a; c_a]  of C:  f_a = +Z_t[up_t, a] in block row t (t < d-1), -Z_t[lo_{t-1}, a] in block row
+// t-1 (t > 0), zero elsewhere (the KVL rows of Eq. (9)/(16) with the source on tier t), and  c_a[i] = 1 for
+// the interfaces i >= t_a below it (the KCL rows, Eq. (11)).  With
+//     M = Zloc - [F; Cs]^T C^-1 [F; Cs],     Zloc[a][b] = Z_t[a, b] if t_a = t_b else 0,
+// the effective resistance of any pair is  R(a,b) = M_aa + M_bb - M_ab - M_ba  (a constant shift of every c_a,
+// e.g. the 1/2 of Eq. (19)/(21), cancels in the difference).
+//
+// Scatter of one tier's probe rows.  Zp = port matrix of [tsv ports of the tier] ++ [its k probes] (ld q =
+// ntsv + k, probe rows ntsv..q-1 valid); probe[j] = column of probe j in the n_nodes-wide arrays; plo = number
+// of lower ends (interface t-1) heading the port list.  Fup / Flo = block rows t / t-1 of F (null if absent).
+__global__ void k_probe_scatter(int k, int ntsv, int plo, int np, const int* __restrict__ probe,
+                                const double* __restrict__ Zp, double* __restrict__ Fup, double* __restrict__ Flo,
+                                double* __restrict__ M) {
+    const int col = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, q = ntsv + k;
+    if (col >= q) return;
+    const double* row = Zp + (int64_t)(ntsv + j) * q;
+    const int a = probe[j];
+    if (col < plo) {
+        if (Flo) Flo[(int64_t)col * np + a] = -row[col];
+    } else if (col < ntsv) {
+        if (Fup) Fup[(int64_t)(col - plo) * np + a] = row[col];
+    } else {
+        const int j2 = col - ntsv;
+        M[(int64_t)a * np + probe[j2]] = 0.5 * (row[col] + Zp[(int64_t)(ntsv + j2) * q + ntsv + j]);
+    }
+}
+
+// Multipliers of the probe right-hand sides:  Cs[i][a] = (tier[a] <= i),  mu[i][a] = sum_k Sinv[i][k] (G[k][a] - Cs[k][a])
+__global__ void k_probe_multipliers(int dm1, int np, const double* __restrict__ G, const double* __restrict__ Sinv,
+                                    const int* __restrict__ tier, double* __restrict__ Cs, double* __restrict__ mu) {
+    const int a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= np) return;
+    const int t = tier[a];
+    for (int i = 0; i < dm1; ++i) {
+        double s = 0.0;
+        for (int k = 0; k < dm1; ++k) s = fma(Sinv[i * dm1 + k], G[(int64_t)k * np + a] - (t <= k ? 1.0 : 0.0), s);
+        mu[(int64_t)i * np + a] = s;
+        Cs[(int64_t)i * np + a] = t <= i ? 1.0 : 0.0;
+    }
+}
+
+__global__ void k_probe_pairs(int np, const double* __restrict__ M, double* __restrict__ R) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y;
+    if (b >= np) return;
+    R[(int64_t)a * np + b] = a == b ? 0.0 : (M[(int64_t)a * np + a] + M[(int64_t)b * np + b]) - (M[(int64_t)a * np + b] + M[(int64_t)b * np + a]);
+}
+
 // Eq. (4): with bump b at v_bump and load k drawing I[k],
 //   v[j] = v_bump - 1/2 sum_k I[k] ( R_b[j] + R_b[k] - R_LL[j][k] )       one warp per load j
 __global__ void k_load_voltages(int n, const double* __restrict__ Rb, const double* __restrict__ RLL,

@@ -301,6 +301,84 @@ def test_tsv_replanning_on_uniform_and_tiny_tiers():
 
 
 @pytest.mark.parametrize("seed,d,n,p,kw", [
+    (61, 2, 33, 5, {}),
+    (62, 4, 48, 7, dict(drop=0.04, aniso=0.4)),
+    (63, 3, 4, 2, {}),                        # single-level mesh: direct path
+    (64, 3, 40, 6, dict(uniform=True)),       # uniform tiers: Eq. (3) table
+])
+def test_arbitrary_tier_endpoints_against_the_oracle(seed, d, n, p, kw):
+    """NEXT-3: R_eff between probes on ANY tiers (same tier, adjacent tiers, top-to-bottom, a probe on a TSV site,
+    a bump, a load, a duplicate) against the oracle's per-pair solves of the whole 3D system; the bump x load block
+    of the probe result equals pdn_reff; still right after TSV re-planning (the kept factor is replaced)."""
+    from oracle.reff_oracle import Oracle
+    from paper_2607_05818_b200 import Pdn
+    torch = torch_cuda()
+    kw = dict(kw)
+    if kw.pop("uniform", False):
+        rng = np.random.default_rng(seed)
+        net = P.make_uniform(d, n, 0.9, 1.4, rt=0.1, tsv_sites=[P._distinct_sites(rng, n, p) for _ in range(d - 1)],
+                             bumps=P._distinct_sites(rng, n, 3), loads=P._distinct_sites(rng, n, 4))
+    else:
+        net = P.make_random(seed, d=d, n=n, p=p, m=3, nl=4, **kw)
+    rng = np.random.default_rng(seed + 1000)
+    nodes = [(int(rng.integers(d)), int(rng.integers(n)), int(rng.integers(n))) for _ in range(9)]
+    nodes += [(0, *map(int, net.tsv_site[0][1])), (1, *map(int, net.tsv_site[0][1]))]      # both ends of one TSV
+    nodes += [(0, *map(int, net.bumps[0])), (d - 1, *map(int, net.loads[2])), nodes[0]]    # a bump, a load, a duplicate
+    nodes = np.array(nodes, dtype=np.int32)
+    k = len(nodes)
+    gid = nodes[:, 0].astype(np.int64) * n * n + nodes[:, 1] * n + nodes[:, 2]
+    pdn = Pdn.from_network(net, device="cuda:0", rtol=1e-10)
+
+    def check(o):
+        out = torch.empty(k * k, dtype=torch.float64, device="cuda:0")
+        pdn.reff_nodes(nodes, out)
+        got = out.cpu().numpy().reshape(k, k)
+        want = np.array([[o.reff_nodes(int(a), int(b)) for b in gid] for a in gid])
+        assert np.all(np.diag(got) == 0.0)
+        nz = want > 0
+        rel = np.abs(got[nz] - want[nz]) / want[nz]
+        assert rel.max() <= MAX_REL and rel.mean() <= MEAN_REL, (rel.max(), rel.mean())
+        assert np.abs(got[~nz]).max() <= 1e-9 * want.max()       # duplicates: cancellation of equal terms
+        full = torch.empty(net.m * net.nl, dtype=torch.float64, device="cuda:0")
+        pdn.reff(full)
+        assert abs(got[k - 3, k - 2] / full.cpu().numpy().reshape(net.m, net.nl)[0, 2] - 1.0) <= 1e-8
+
+    check(Oracle(net))
+    if n > 4:
+        rng = np.random.default_rng(seed + 7)
+        new = [x for x in P._distinct_sites(rng, n, 6).tolist() if x not in net.tsv_site[0].tolist()][:2]
+        net.tsv_site[0] = np.vstack([net.tsv_site[0][:-1], np.array(new, dtype=np.int32)]).astype(np.int32)
+        net.tsv_r[0] = np.concatenate([net.tsv_r[0][:-1], [0.07, 0.09]])
+        pdn.update_tsvs(net.tsv_site, net.tsv_r)
+        check(Oracle(net))
+    with pytest.raises(Exception):
+        pdn.reff_nodes(np.array([[d, 0, 0]], dtype=np.int32), torch.empty(1, dtype=torch.float64, device="cuda:0"))
+    pdn.close()
+
+
+def test_reff_map_over_a_whole_tier_against_the_oracle():
+    """NEXT-3 / Fig. 6(d): the R_eff map from a bump to EVERY node of the bottom tier (stride 1) and to a
+    sub-grid of a middle tier, against per-node solves of the oracle."""
+    from oracle.reff_oracle import Oracle
+    from paper_2607_05818_b200 import Pdn
+    torch_cuda()
+    d, n = 3, 20
+    net = P.make_random(71, d=d, n=n, p=6, m=2, nl=3, drop=0.03)
+    o = Oracle(net)
+    pdn = Pdn.from_network(net, device="cuda:0", rtol=1e-10)
+    src = (0, int(net.bumps[1][0]), int(net.bumps[1][1]))
+    a = src[1] * n + src[2]
+    for tier, stride in ((d - 1, 1), (1, 3)):
+        got = pdn.reff_map(src, tier, stride)
+        ys = np.arange(0, n, stride)
+        want = np.array([[o.reff_nodes(a, tier * n * n + int(y) * n + int(x)) for x in ys] for y in ys])
+        assert got.shape == want.shape
+        rel = np.abs(got - want) / want
+        assert rel.max() <= MAX_REL and rel.mean() <= MEAN_REL, (rel.max(), rel.mean())
+    pdn.close()
+
+
+@pytest.mark.parametrize("seed,d,n,p,kw", [
     (51, 2, 33, 5, {}),
     (52, 3, 64, 8, dict(drop=0.04, aniso=0.4)),
     (53, 2, 4, 2, {}),                        # single-level mesh: direct path
