@@ -174,7 +174,8 @@ int pdn_load_voltages(pdn_ctx *ctx, int32_t bump, const double *i_load, double v
  * Cost: one port solve per probe on its own tier (full tolerance, gathered at the tier's TSV ends and at the
  * other probes of that tier), then one substitution with the factor of C kept since pdn_create / the last
  * pdn_update_tsvs (Eq. (18)-(22) PAPER.md:179-204 with the source / sink on arbitrary tiers; DESIGN.md
- * section 1).  The context is not changed.  Not available on a sharded context (PDN_E_ARG). */
+ * section 1).  The context is not changed.  On a sharded context (after pdn_finish) every rank that calls it
+ * does all the probe solves itself. */
 typedef struct pdn_node {
     int32_t tier, y, x;
 } pdn_node;

@@ -569,7 +569,7 @@ int pdn_load_voltages(pdn_ctx* ctx, int32_t bump, const double* i_load, double v
 // NEXT-3: arbitrary-tier endpoints (port.cuh "Arbitrary-tier endpoints" has the algebra).
 int pdn_reff_nodes(pdn_ctx* ctx, int32_t n_nodes, const pdn_node* nodes, double* out) {
     if (!ctx || !nodes || !out || n_nodes < 1) return fail_arg("null context / node list / output or empty list");
-    if (ctx->open || ctx->shard_world > 1) return fail_arg("pdn_reff_nodes is not available on a sharded context");
+    if (ctx->open) return fail_arg("sharded context is still open: exchange the rows and call pdn_finish first");
     pdn_ctx* c = ctx;
     const int d = c->d, n = c->n, dm1 = d - 1, np = n_nodes;
     for (int a = 0; a < np; ++a) {

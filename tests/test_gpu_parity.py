@@ -356,6 +356,30 @@ def test_arbitrary_tier_endpoints_against_the_oracle(seed, d, n, p, kw):
     pdn.close()
 
 
+@pytest.mark.parametrize("n", [1500, 2047])
+@pytest.mark.parametrize("fast_path", [True, False])
+def test_large_ragged_meshes_match_wu_closed_form(n, fast_path):
+    """Sizes beyond BASELINE's and not powers of two (ragged tiles on every level, odd coarse meshes), ports in
+    three corners: the intra-die R_jk from the GPU port matrix against Eq. (3), for the numerical path
+    and for the spectral table."""
+    from closed_forms import wu_mesh_reff
+    from paper_2607_05818_b200 import PDN_NO_UNIFORM_FAST_PATH, Pdn
+    torch_cuda()
+    rng = np.random.default_rng(n)
+    sites = [P._distinct_sites(rng, n, 6)]
+    sites[0][0], sites[0][1], sites[0][2] = (0, 0), (n - 1, n - 1), (n - 1, 0)
+    net = P.make_uniform(2, n, 0.8, 1.7, rt=0.1, tsv_sites=sites, bumps=np.array([[3, 3]]), loads=np.array([[5, 5]]))
+    pdn = Pdn.from_network(net, device="cuda:0", rtol=1e-10, flags=0 if fast_path else PDN_NO_UNIFORM_FAST_PATH)
+    Z = pdn.port_matrix(0)
+    assert pdn.stats()["n_uniform_tiers"] == (2 if fast_path else 0)
+    pdn.close()
+    for j in range(6):
+        for k in range(j + 1, 6):
+            (y1, x1), (y2, x2) = sites[0][j], sites[0][k]
+            want = wu_mesh_reff(n, n, 0.8, 1.7, x1, y1, x2, y2)
+            assert abs((Z[j, j] + Z[k, k] - 2 * Z[j, k]) / want - 1.0) <= 1e-9
+
+
 def test_reff_map_over_a_whole_tier_against_the_oracle():
     """NEXT-3 / Fig. 6(d): the R_eff map from a bump to EVERY node of the bottom tier (stride 1) and to a
     sub-grid of a middle tier, against per-node solves of the oracle."""
@@ -468,6 +492,18 @@ def test_recombination_pins_series_law_and_separable_product_graph(fast_path):
         for j, l in enumerate(loads):
             want = product_graph_reff(n, n, d, rx, ry, rt, (b[1], b[0], 0), (l[1], l[0], d - 1))
             assert got[i, j] == pytest.approx(want, rel=1e-8)
+    # (iii) the same product graph, endpoints on ANY tier (pdn_reff_nodes): middle-middle, top-middle, same column
+    torch = torch_cuda()
+    from paper_2607_05818_b200 import Pdn
+    nodes = np.array([[1, 2, 3], [1, 5, 0], [0, 2, 3], [2, 2, 3], [0, 0, 0], [2, 5, 5], [1, 0, 4]], dtype=np.int32)
+    pdn = Pdn.from_network(net, device="cuda:0", rtol=1e-11, flags=flags)
+    out = torch.empty(len(nodes) ** 2, dtype=torch.float64, device="cuda:0")
+    got = pdn.reff_nodes(nodes, out).cpu().numpy().reshape(len(nodes), len(nodes))
+    pdn.close()
+    for i, (ta, ya, xa) in enumerate(nodes):
+        for j, (tb, yb, xb) in enumerate(nodes):
+            if i != j:
+                assert got[i, j] == pytest.approx(product_graph_reff(n, n, d, rx, ry, rt, (xa, ya, ta), (xb, yb, tb)), rel=1e-8)
 
 
 def test_bump_on_tsv_site_and_shared_sites_between_interfaces():
@@ -519,6 +555,14 @@ def test_sharded_port_solves_emulated_on_one_gpu(world, flags_name):
             want = Oracle(net).reff_same_side(1)
             off = ~np.eye(net.nl, dtype=bool)
             assert (np.abs(ll.cpu().numpy().reshape(net.nl, net.nl)[off] - want[off]) / want[off]).max() <= MAX_REL
+        nodes = np.array([[1, 3, 40], [0, 20, 20], [2, 46, 0]], dtype=np.int32)     # probes on a finished sharded context
+        rn = torch.empty(9, dtype=torch.float64, device="cuda:0")
+        r.reff_nodes(nodes, rn)
+        o = Oracle(net)
+        gid = nodes[:, 0].astype(np.int64) * net.n ** 2 + nodes[:, 1] * net.n + nodes[:, 2]
+        for a_ in range(3):
+            for b_ in range(a_ + 1, 3):
+                assert abs(rn[3 * a_ + b_].item() / o.reff_nodes(int(gid[a_]), int(gid[b_])) - 1.0) <= MAX_REL
         r.close()
 
 
