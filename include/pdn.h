@@ -107,8 +107,10 @@ typedef struct {
     int32_t rhs_batch;  /* right-hand sides solved concurrently per tier          (default: auto) */
     void *cuda_stream;  /* cudaStream_t to run on                                 (default: 0)    */
     int32_t flags;      /* PDN_* flags                                                             */
-    int32_t nu;         /* Chebyshev smoothing steps per multigrid level and side (1..6, default 4)*/
-    double cheb_ratio;  /* smoothing interval [2/ratio, 2] of D^-1 L (default: 3 + the tier's anisotropy)  */
+    int32_t nu;         /* Chebyshev smoothing steps per multigrid level and side (1..6; default 4, and 6 on
+                           tiers whose anisotropy mean g_x / mean g_y (or its inverse) is >= 6)             */
+    double cheb_ratio;  /* smoothing interval [2/ratio, 2] of D^-1 L (default: 3 + the tier's anisotropy a,
+                           2 (1 + a) for a >= 6)                                                             */
     int32_t shard_rank; /* NEXT-4: this process solves slice shard_rank of shard_world of every tier's port     */
     int32_t shard_world;/* solves and leaves the context OPEN (see pdn_shard_slice / pdn_finish); 0 or 1 = off  */
 } pdn_opts;

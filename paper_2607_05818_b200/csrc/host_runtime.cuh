@@ -143,6 +143,7 @@ struct pdn_ctx {
     std::vector<DevBuf> Li, Vf, KB;   // factor of C kept for pdn_reff_nodes: L_i^-1, L_{i-1}^-1 K_{i-1,i}, (K^-1 B)_i
     DevBuf Sinv;                      // inverse of the Schur complement B^T K^-1 B ((d-1)^2)
     bool terminal_pairs = false;
+    bool nu_auto = true;                  // opts.nu was left at its default: strongly anisotropic tiers may deepen it
     int shard_rank = 0, shard_world = 1;  // NEXT-4
     bool open = false;                    // sharded context whose rows have not been completed / S2-S3 not run
     pdn_stats stats{};

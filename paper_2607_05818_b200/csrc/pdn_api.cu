@@ -125,14 +125,20 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
     // Smoothing interval [2/ratio, 2] of the Chebyshev polynomial.  With 2x2 aggregation the coarse grid
     // takes fewer modes off the smoother the more anisotropic the tier is, so the interval widens with
     // the anisotropy a: ratio = 3 + a (measured: a = 1 -> 4, a = 3 -> 6).
-    const double ratio = o.cheb_ratio > 1.0 ? o.cheb_ratio : std::min(10.0, 3.0 + H.anisotropy);
+    // Strongly anisotropic tiers (a >= 6) leave modes that are smooth along the strong direction and oscillatory
+    // across it, with eigenvalues down to ~2/(1+a) of D^-1 L, to the smoother: the interval becomes [1/(1+a), 2]
+    // and, unless the caller fixed nu, the smoother gets the deepest polynomial the kernels have (measured at
+    // 512^2: a = 10 / 30 / 100 need 9 / 12 / 40 iterations this way against 16 / 62 / 146 with the rule above).
+    const bool strong = H.anisotropy >= 6.0;
+    const int nu = (strong && c->nu_auto) ? 6 : o.nu;
+    const double ratio = o.cheb_ratio > 1.0 ? o.cheb_ratio : strong ? 2.0 * (1.0 + H.anisotropy) : 3.0 + H.anisotropy;
     const int G = getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 32;
     // On near-isotropic tiers the coarse levels get by with one step less on a wider interval (measured: same
     // iteration counts at configs 3 and 5, one level-visit cheaper); anisotropic tiers keep nu steps everywhere.
-    const bool iso = H.anisotropy < 1.5 && o.nu >= 3 && !(o.cheb_ratio > 1.0);
-    const int nu_c = iso ? o.nu - 1 : o.nu;
+    const bool iso = H.anisotropy < 1.5 && nu >= 3 && !(o.cheb_ratio > 1.0);
+    const int nu_c = iso ? nu - 1 : nu;
     const double ratio_c = iso ? 2.0 * ratio : ratio;
-    const Smoother ch{make_cheb_roots(o.nu, ratio), make_cheb_roots(nu_c, ratio_c), G};
+    const Smoother ch{make_cheb_roots(nu, ratio), make_cheb_roots(nu_c, ratio_c), G};
     // bump / load sources deliver only their own diagonal, whose CG error is the square of the energy-norm error
     const double rtol_term = std::max(o.rtol, std::min(1e-5, std::sqrt(o.rtol) / 3.0));
     int status = PDN_OK;
@@ -202,6 +208,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
     if (opts) o = *opts;
     if (!(o.rtol > 0.0)) o.rtol = 1e-8;
     if (o.max_iter <= 0) o.max_iter = 200;
+    const bool nu_auto = o.nu <= 0;
     if (o.nu <= 0) o.nu = 4;
     if (o.nu > 6) o.nu = 6;
 
@@ -213,6 +220,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         c->stream = (cudaStream_t)o.cuda_stream;
         c->time_kernels = (o.flags & PDN_TIME_KERNELS) != 0;
         c->terminal_pairs = (o.flags & PDN_TERMINAL_PAIRS) != 0;
+        c->nu_auto = nu_auto;
         if (o.shard_world > 1) {
             if (o.shard_rank < 0 || o.shard_rank >= o.shard_world) throw StatusFail{PDN_E_ARG, "shard_rank out of range"};
             c->shard_world = o.shard_world; c->shard_rank = o.shard_rank; c->open = true;

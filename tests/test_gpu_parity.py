@@ -380,6 +380,22 @@ def test_large_ragged_meshes_match_wu_closed_form(n, fast_path):
             assert abs((Z[j, j] + Z[k, k] - 2 * Z[j, k]) / want - 1.0) <= 1e-9
 
 
+@pytest.mark.parametrize("aniso", [40.0, 1.0 / 40.0])
+def test_strongly_anisotropic_tiers_converge_and_match_the_oracle(aniso):
+    """Tiers whose x- and y-segments differ 40-fold (either way): the smoother widens its interval and deepens its
+    polynomial by itself (pdn_api.cu: reduce_tier), the solves stay far from max_iter and the result is the oracle's."""
+    from oracle.reff_oracle import Oracle
+    from paper_2607_05818_b200 import Pdn
+    torch = torch_cuda()
+    net = P.make_random(81, d=3, n=150, p=9, m=4, nl=5, aniso=aniso)
+    pdn = Pdn.from_network(net, device="cuda:0")
+    out = torch.empty(net.m * net.nl, dtype=torch.float64, device="cuda:0")
+    pdn.reff(out)
+    assert pdn.stats()["pcg_iters_max"] <= 30
+    pdn.close()
+    check(out.cpu().numpy().reshape(net.m, net.nl), Oracle(net).reff_all())
+
+
 def test_reff_map_over_a_whole_tier_against_the_oracle():
     """NEXT-3 / Fig. 6(d): the R_eff map from a bump to EVERY node of the bottom tier (stride 1) and to a
     sub-grid of a middle tier, against per-node solves of the oracle."""
