@@ -24,8 +24,10 @@
  * the residuals and every result are FP64).  A tier whose x-segments are all equal and whose
  * y-segments are all equal is reduced by the closed form, Eq. (3).  Every entry point
  * is thread-compatible (one thread per context at a time), never throws, and returns a status
- * (0 = PDN_OK).  There is NO CPU fallback: without a CUDA device every compute call fails with
- * PDN_E_CUDA.
+ * (0 = PDN_OK).  A context lives on the CUDA device that is current when pdn_create is called; later
+ * calls on it must be made with that device current (PDN_E_ARG otherwise).  A process may hold contexts
+ * on several devices; freed device memory is cached per device (pdn_release_cache).  There is NO CPU
+ * fallback: without a CUDA device every compute call fails with PDN_E_CUDA.
  */
 #ifndef PDN_H_
 #define PDN_H_

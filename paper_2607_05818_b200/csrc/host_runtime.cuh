@@ -33,18 +33,25 @@ enum { KC_PQ = 0, KC_DOWN0, KC_UP0, KC_DOWNC, KC_UPC, KC_SMALL, KC_DENSE, KC_PAI
 // kept and handed out again (best fit within 25 %).  pdn_release_cache() returns them to the driver;
 // an allocation failure does so automatically before giving up.
 struct DevPool {
+    static constexpr int MAX_DEV = 64;
     std::mutex mu;
-    std::multimap<size_t, void*> free_blocks;
-    size_t cached = 0;
+    std::multimap<size_t, void*> free_blocks[MAX_DEV];  // per device: a block only ever goes back to its own device
+    size_t cached[MAX_DEV] = {};
 
-    void* get(size_t n) {
+    static int current_device() {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        return dev & (MAX_DEV - 1);
+    }
+    void* get(size_t n, int dev) {
         {
             std::lock_guard<std::mutex> g(mu);
-            auto it = free_blocks.lower_bound(n);
-            if (it != free_blocks.end() && it->first <= n + n / 4 + 4096) {
+            auto& fb = free_blocks[dev];
+            auto it = fb.lower_bound(n);
+            if (it != fb.end() && it->first <= n + n / 4 + 4096) {
                 void* p = it->second;
-                cached -= it->first;
-                free_blocks.erase(it);
+                cached[dev] -= it->first;
+                fb.erase(it);
                 return p;
             }
         }
@@ -58,20 +65,22 @@ struct DevPool {
         }
         return p;
     }
-    void put(void* p, size_t n) {
+    void put(void* p, size_t n, int dev) {
         std::lock_guard<std::mutex> g(mu);
-        free_blocks.emplace(n, p);
-        cached += n;
+        free_blocks[dev].emplace(n, p);
+        cached[dev] += n;
     }
     void trim() {
         std::lock_guard<std::mutex> g(mu);
-        for (auto& kv : free_blocks) cudaFree(kv.second);
-        free_blocks.clear();
-        cached = 0;
+        for (int d = 0; d < MAX_DEV; ++d) {
+            for (auto& kv : free_blocks[d]) cudaFree(kv.second);
+            free_blocks[d].clear();
+            cached[d] = 0;
+        }
     }
-    size_t cached_bytes() {
+    size_t cached_bytes(int dev) {
         std::lock_guard<std::mutex> g(mu);
-        return cached;
+        return cached[dev];
     }
 };
 DevPool g_pool;
@@ -93,23 +102,25 @@ struct PinnedScratch {
 };
 thread_local PinnedScratch g_pinned;
 
-struct DevBuf {  // RAII device allocation (block sizes are rounded up to 1 MiB classes above 1 MiB)
+struct DevBuf {  // RAII device allocation on the device that is current at alloc()
     void* p = nullptr;
     size_t bytes = 0;
+    int dev = 0;
     DevBuf() = default;
     DevBuf(const DevBuf&) = delete;
     DevBuf& operator=(const DevBuf&) = delete;
-    DevBuf(DevBuf&& o) noexcept : p(o.p), bytes(o.bytes) { o.p = nullptr; o.bytes = 0; }
+    DevBuf(DevBuf&& o) noexcept : p(o.p), bytes(o.bytes), dev(o.dev) { o.p = nullptr; o.bytes = 0; }
     DevBuf& operator=(DevBuf&& o) noexcept {
-        if (this != &o) { release(); p = o.p; bytes = o.bytes; o.p = nullptr; o.bytes = 0; }
+        if (this != &o) { release(); p = o.p; bytes = o.bytes; dev = o.dev; o.p = nullptr; o.bytes = 0; }
         return *this;
     }
     ~DevBuf() { release(); }
-    void release() { if (p) g_pool.put(p, bytes); p = nullptr; bytes = 0; }
+    void release() { if (p) g_pool.put(p, bytes, dev); p = nullptr; bytes = 0; }
     void alloc(size_t n) {
         release();
         n = n < 256 ? 256 : (n + 255) & ~size_t(255);
-        p = g_pool.get(n);
+        dev = DevPool::current_device();
+        p = g_pool.get(n, dev);
         if (!p) throw StatusFail{PDN_E_NOMEM, "cudaMalloc of " + std::to_string(n) + " bytes failed"};
         bytes = n;
     }
@@ -131,6 +142,7 @@ struct TierPorts {
 
 struct pdn_ctx {
     int d = 0, n = 0, m = 0, nl = 0, p0 = 0;
+    int device = 0;                   // the CUDA device the context lives on (current at pdn_create)
     std::vector<int> p;               // TSVs per interface
     std::vector<std::vector<double>> rt;
     std::vector<std::vector<int>> site;   // per interface: pitched offsets of the TSV sites, in list order
@@ -192,6 +204,16 @@ struct Launcher {
         c->pending_events.clear();
     }
 };
+
+// Runs `set` once per device (kernel attributes are per device); the bit is published after the attributes are
+// in place, so a second host thread either sees it set or sets the same attributes again (harmless).
+template <class F>
+inline void once_per_device(std::atomic<uint64_t>& mask, F&& set) {
+    const uint64_t bit = 1ull << DevPool::current_device();
+    if (mask.load(std::memory_order_acquire) & bit) return;
+    set();
+    mask.fetch_or(bit, std::memory_order_release);
+}
 
 inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) / b); }
 

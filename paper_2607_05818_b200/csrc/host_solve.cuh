@@ -204,12 +204,11 @@ void launch_down3(Launcher& L, int cls, double bytes, const Level& lv, const Smo
     const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
     dim3 grid(tx, ty, cdiv(B, G));
     constexpr size_t base = 2 * T3_TILE_BYTES + T3_SC_BYTES + sizeof(Exch<DN_W>);
-    static bool attr_done = false;
-    if (!attr_done) {
+    static std::atomic<uint64_t> attr_done{0};
+    once_per_device(attr_done, [&] {
         CK(cudaFuncSetAttribute(k_down3<DN_R, DN_W, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(base + 2 * T3_TILE_BYTES)));
         CK(cudaFuncSetAttribute(k_down3<DN_R, DN_W, NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)base));
-        attr_done = true;
-    }
+    });
     if (m_q) L.run(cls, bytes, [&] { k_down3<DN_R, DN_W, NU, true><<<grid, 32 * DN_W, base + 2 * T3_TILE_BYTES, L.s>>>(m_r, *m_q, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
     else L.run(cls, bytes, [&] { k_down3<DN_R, DN_W, NU, false><<<grid, 32 * DN_W, base, L.s>>>(m_r, m_r, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
 }
@@ -221,12 +220,11 @@ void launch_up3(Launcher& L, int cls, double bytes, const Level& lv, const Smoot
     const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
     dim3 grid(tx, ty, cdiv(B, G));
     constexpr size_t smem = 4 * T3_TILE_BYTES + (size_t)2 * Geom<T3_R, T3_W, 2>::ETILE_BYTES + T3_SC_BYTES + sizeof(Exch<T3_W>);
-    static bool attr_done = false;
-    if (!attr_done) {
+    static std::atomic<uint64_t> attr_done{0};
+    once_per_device(attr_done, [&] {
         CK(cudaFuncSetAttribute(k_up3<T3_R, T3_W, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         CK(cudaFuncSetAttribute(k_up3<T3_R, T3_W, NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
-    }
+    });
     if (rz_acc) L.run(cls, bytes, [&] { k_up3<T3_R, T3_W, NU, true><<<grid, T3_THREADS, smem, L.s>>>(m_r, m_y, m_e, lv, cr, z_out, rz_acc, B, G, active); });
     else L.run(cls, bytes, [&] { k_up3<T3_R, T3_W, NU, false><<<grid, T3_THREADS, smem, L.s>>>(m_r, m_y, m_e, lv, cr, z_out, rz_acc, B, G, active); });
 }
@@ -238,11 +236,10 @@ void launch_pq3(Launcher& L, double bytes, const Level& lv, const Smoother& sm, 
     const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
     dim3 grid(tx, ty, cdiv(B, G));
     constexpr size_t smem = 4 * T3_TILE_BYTES + sizeof(Exch<PQ_W>);
-    static bool attr_done = false;
-    if (!attr_done) {
+    static std::atomic<uint64_t> attr_done{0};
+    once_per_device(attr_done, [&] {
         CK(cudaFuncSetAttribute(k_pq3<PQ_R, PQ_W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
-    }
+    });
     L.run(KC_PQ, bytes, [&] { k_pq3<PQ_R, PQ_W><<<grid, 32 * PQ_W, smem, L.s>>>(m_z, m_p, lv, beta, p_new, q, pq_acc, sump_acc, B, G, active); });
 }
 
@@ -265,11 +262,15 @@ void launch_tail(Launcher& L, const Hierarchy& H, const Smoother& sm, int l0, in
     P.pinv = H.pinv.as<double>();
     P.ch = sm.crc;
     const size_t smem = tail_smem_doubles(P) * sizeof(double);
-    static size_t attr_smem = 0;
-    if (smem > attr_smem) {
-        CK(cudaFuncSetAttribute(k_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_smem = smem;
-    }
+    static std::atomic<uint64_t> attr_done{0};
+    once_per_device(attr_done, [&] {  // the most the device allows, so that any hierarchy's tail fits
+        int dev = 0, optin = 0;
+        cudaFuncAttributes fa{};
+        CK(cudaGetDevice(&dev));
+        CK(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+        CK(cudaFuncGetAttributes(&fa, k_tail));
+        CK(cudaFuncSetAttribute(k_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa.sharedSizeBytes));
+    });
     const int G = std::max(1, std::min(sm.G, B / (148 * 2)));
     L.run(KC_DOWNC, bytes, [&] { k_tail<<<cdiv(B, G), TAIL_THREADS, smem, L.s>>>(P, r_in, z_out, H.plane(l0), B, G, active); });
 }

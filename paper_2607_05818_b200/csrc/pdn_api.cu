@@ -10,6 +10,7 @@
 #include "../../include/pdn.h"
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -74,7 +75,7 @@ int pick_batch(const Hierarchy& H, int want, const pdn_opts& o) {
     if (H.nlev <= 1) return std::max(want, 1);
     size_t free_b = 0, total_b = 0;
     CK(cudaMemGetInfo(&free_b, &total_b));
-    free_b += g_pool.cached_bytes();
+    free_b += g_pool.cached_bytes(DevPool::current_device());
     const size_t per = Work::bytes_per_rhs(H) + (size_t)want * 8 + 128;
     const size_t fit = std::max<size_t>(1, (size_t)(0.6 * (double)free_b) / per);
     int B = (int)std::min<size_t>({(size_t)std::max(want, 1), fit, (size_t)1024});
@@ -190,6 +191,14 @@ static int fail_arg(const char* msg) {
     return PDN_E_ARG;
 }
 
+// A context lives on the device that was current at pdn_create; every later call must be made with it current.
+static bool wrong_device(const pdn_ctx* c) {
+    int dev = -1;
+    return cudaGetDevice(&dev) != cudaSuccess || dev != c->device;
+}
+#define PDN_CHECK_DEVICE(ctx) \
+    do { if (wrong_device(ctx)) return fail_arg("the context's CUDA device is not the current device"); } while (0)
+
 int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_tsv, const pdn_tsv* tsvs,
                int32_t n_bumps, const pdn_site* bumps, int32_t n_loads, const pdn_site* loads, const pdn_opts* opts) {
     if (!out) return fail_arg("out is null");
@@ -238,6 +247,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         check_sites(bumps, n_bumps, c->bump_id);
         check_sites(loads, n_loads, c->load_id);
 
+        CK(cudaGetDevice(&c->device));
         Launcher L{c, c->stream};
         cudaEvent_t ev[4];
         for (auto& e : ev) CK(cudaEventCreate(&e));
@@ -343,6 +353,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
 // re-factored (milliseconds).
 int pdn_update_tsvs(pdn_ctx* ctx, int32_t n_tsv, const pdn_tsv* tsvs) {
     if (!ctx || !tsvs || n_tsv < 1) return fail_arg("null context / TSV list or empty list");
+    PDN_CHECK_DEVICE(ctx);
     if (ctx->open || ctx->shard_world > 1) return fail_arg("TSV re-planning is not available on a sharded context");
     pdn_ctx* c = ctx;
     const int d = c->d, n = c->n;
@@ -466,6 +477,7 @@ static int reff_device(pdn_ctx* ctx, int64_t n_pairs, const int32_t* bi, const i
 
 int pdn_reff(pdn_ctx* ctx, int64_t n_pairs, const int32_t* bump_idx, const int32_t* load_idx, double* out) {
     if (!ctx || !out || n_pairs < 0) return fail_arg("null context / output or negative n_pairs");
+    PDN_CHECK_DEVICE(ctx);
     if (ctx->open) return fail_arg("sharded context is still open: exchange the rows and call pdn_finish first");
     if ((bump_idx == nullptr) != (load_idx == nullptr)) return fail_arg("bump_idx and load_idx must both be given or both be NULL");
     if (!bump_idx && n_pairs != (int64_t)ctx->m * ctx->nl) return fail_arg("full cross product needs n_pairs == n_bumps*n_loads");
@@ -484,6 +496,7 @@ int pdn_reff(pdn_ctx* ctx, int64_t n_pairs, const int32_t* bump_idx, const int32
 
 int pdn_reff_host(pdn_ctx* ctx, int64_t n_pairs, const int32_t* bump_idx, const int32_t* load_idx, double* out) {
     if (!ctx || !out || n_pairs < 0) return fail_arg("null context / output or negative n_pairs");
+    PDN_CHECK_DEVICE(ctx);
     if (ctx->open) return fail_arg("sharded context is still open: exchange the rows and call pdn_finish first");
     if ((bump_idx == nullptr) != (load_idx == nullptr)) return fail_arg("bump_idx and load_idx must both be given or both be NULL");
     if (!bump_idx && n_pairs != (int64_t)ctx->m * ctx->nl) return fail_arg("full cross product needs n_pairs == n_bumps*n_loads");
@@ -517,6 +530,7 @@ void pdn_release_cache(void) { g_pool.trim(); }
 // NEXT-3: R_eff between terminals of the same side (bump-bump or load-load), full nt x nt matrix on the device.
 int pdn_reff_same_side(pdn_ctx* ctx, int32_t side, double* out) {
     if (!ctx || !out || (side != 0 && side != 1)) return fail_arg("null context / output or side not in {0, 1}");
+    PDN_CHECK_DEVICE(ctx);
     if (!ctx->terminal_pairs) return fail_arg("the context was not created with PDN_TERMINAL_PAIRS");
     if (ctx->open) return fail_arg("sharded context is still open: exchange the rows and call pdn_finish first");
     try {
@@ -539,6 +553,7 @@ int pdn_reff_same_side(pdn_ctx* ctx, int32_t side, double* out) {
 // NEXT-3: Eq. (4).
 int pdn_load_voltages(pdn_ctx* ctx, int32_t bump, const double* i_load, double v_bump, double* v_out) {
     if (!ctx || !i_load || !v_out) return fail_arg("null argument");
+    PDN_CHECK_DEVICE(ctx);
     if (!ctx->terminal_pairs) return fail_arg("the context was not created with PDN_TERMINAL_PAIRS");
     if (ctx->open) return fail_arg("sharded context is still open: exchange the rows and call pdn_finish first");
     if (bump < 0 || bump >= ctx->m) return fail_arg("bump index out of range");
@@ -577,6 +592,7 @@ int pdn_load_voltages(pdn_ctx* ctx, int32_t bump, const double* i_load, double v
 // NEXT-3: arbitrary-tier endpoints (port.cuh "Arbitrary-tier endpoints" has the algebra).
 int pdn_reff_nodes(pdn_ctx* ctx, int32_t n_nodes, const pdn_node* nodes, double* out) {
     if (!ctx || !nodes || !out || n_nodes < 1) return fail_arg("null context / node list / output or empty list");
+    PDN_CHECK_DEVICE(ctx);
     if (ctx->open) return fail_arg("sharded context is still open: exchange the rows and call pdn_finish first");
     pdn_ctx* c = ctx;
     const int d = c->d, n = c->n, dm1 = d - 1, np = n_nodes;
@@ -699,6 +715,7 @@ int pdn_shard_buffers(pdn_ctx* ctx, int32_t tier, double** zt, int64_t* ld, int3
 
 int pdn_finish(pdn_ctx* ctx) {
     if (!ctx) return fail_arg("null context");
+    PDN_CHECK_DEVICE(ctx);
     if (!ctx->open) return PDN_OK;
     int status = PDN_OK;
     try {
