@@ -104,7 +104,9 @@ typedef struct {
 
 /* Options; pass NULL for the defaults.  Zero / negative fields mean "default". */
 typedef struct {
-    double rtol;        /* port solves stop at ||r||_2 <= rtol * ||b||_2          (default 1e-8)  */
+    double rtol;        /* port solves stop at ||r||_2 <= rtol * ||b||_2          (default 1e-8);
+                           bump / load sources, of which only the diagonal entry is used (its error is
+                           quadratic in the residual), stop at min(1e-5, sqrt(rtol)/3, 1000 rtol)        */
     int32_t max_iter;   /* iteration cap per port solve                           (default 200)   */
     int32_t rhs_batch;  /* right-hand sides solved concurrently per tier          (default: auto) */
     void *cuda_stream;  /* cudaStream_t to run on                                 (default: 0)    */

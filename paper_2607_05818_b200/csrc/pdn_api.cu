@@ -141,7 +141,9 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
     const double ratio_c = iso ? 2.0 * ratio : ratio;
     const Smoother ch{make_cheb_roots(nu, ratio), make_cheb_roots(nu_c, ratio_c), G};
     // bump / load sources deliver only their own diagonal, whose CG error is the square of the energy-norm error
-    const double rtol_term = std::max(o.rtol, std::min(1e-5, std::sqrt(o.rtol) / 3.0));
+    // (times the condition number of the preconditioned operator, which is why a caller who tightens rtol below
+    // the default also gets tighter terminal solves: at most 1000 rtol)
+    const double rtol_term = std::max(o.rtol, std::min({1e-5, std::sqrt(o.rtol) / 3.0, 1e3 * o.rtol}));
     int status = PDN_OK;
     for (size_t s0 = 0; s0 < tsv_src.size() && status == PDN_OK; s0 += Bmax)
         status = solve_batch(c, L, H, W, T, ch, tsv_src.data() + s0, (int)std::min<size_t>(Bmax, tsv_src.size() - s0), false, o.rtol, o.max_iter);
