@@ -582,6 +582,65 @@ def test_sharded_port_solves_emulated_on_one_gpu(world, flags_name):
         r.close()
 
 
+@pytest.mark.parametrize("block", [0, 1, 2])
+def test_randomised_stacks_through_every_entry_point(block):
+    """Seeded fuzz, 12 stacks per block: random d, n (1-level meshes, one node more / less than a tile, odd sizes),
+    port counts, anisotropy (up to 12), removed segments, a uniform tier now and then, random flags, batch sizes and
+    smoother depths, device or host planes -- pdn_reff, pdn_reff_nodes on random probes, then a TSV re-plan followed by
+    pdn_reff (and the load-load pairs when the context keeps them), all against the oracle."""
+    from oracle.reff_oracle import Oracle
+    from paper_2607_05818_b200 import PDN_NO_UNIFORM_FAST_PATH, PDN_TERMINAL_PAIRS, Pdn
+    torch = torch_cuda()
+
+    def rel_err(got, want):
+        nz = want > 0
+        assert np.abs(got[~nz]).max(initial=0.0) <= 1e-9 * max(want.max(), 1.0)
+        return np.abs(got[nz] / want[nz] - 1.0).max(initial=0.0)
+
+    for it in range(12):
+        seed = 7000 + 100 * block + it
+        rng = np.random.default_rng(seed)
+        d, n = int(rng.integers(2, 6)), int(rng.choice([2, 3, 4, 5, 7, 9, 16, 17, 31, 33, 56, 57, 65, 90, 113]))
+        p = int(rng.integers(1, min(n * n, 12) + 1))
+        m, nl = int(rng.integers(1, min(n * n, 6) + 1)), int(rng.integers(1, min(n * n, 7) + 1))
+        aniso = float(rng.choice([1.0, 1.0, 0.3, 3.0, 12.0]))
+        drop = float(rng.choice([0.0, 0.0, 0.03, 0.1])) if n >= 5 else 0.0
+        net = P.make_random(seed, d=d, n=n, p=p, m=m, nl=nl, aniso=aniso, drop=drop)
+        if rng.random() < 0.25:
+            t = int(rng.integers(d))
+            net.gx[t], net.gy[t] = P._planes(n, np.full((n, n), 0.7), np.full((n, n), 1.9))
+        flags = (PDN_TERMINAL_PAIRS if rng.random() < 0.4 else 0) | (PDN_NO_UNIFORM_FAST_PATH if rng.random() < 0.3 else 0)
+        kw = dict(rtol=1e-10, flags=flags, rhs_batch=int(rng.choice([0, 0, 1, 3, 7])), nu=int(rng.choice([0, 0, 2, 3, 5, 6])))
+        what = f"seed {seed}: d={d} n={n} p={p} m={m} nl={nl} aniso={aniso} drop={drop} {kw}"
+        pdn = Pdn.from_network(net, device="cuda:0" if rng.random() < 0.7 else None, **kw)
+        o = Oracle(net)
+        out = torch.empty(m * nl, dtype=torch.float64, device="cuda:0")
+        pdn.reff(out)
+        assert rel_err(out.cpu().numpy().reshape(m, nl), o.reff_all()) <= 1e-8, what
+        k = int(rng.integers(1, 8))
+        nodes = np.stack([rng.integers(0, d, k), rng.integers(0, n, k), rng.integers(0, n, k)], axis=1).astype(np.int32)
+        rn = torch.empty(k * k, dtype=torch.float64, device="cuda:0")
+        pdn.reff_nodes(nodes, rn)
+        gid = nodes[:, 0].astype(np.int64) * n * n + nodes[:, 1] * n + nodes[:, 2]
+        want = np.array([[o.reff_nodes(int(a), int(b)) for b in gid] for a in gid])
+        assert rel_err(rn.cpu().numpy().reshape(k, k), want) <= 1e-8, what
+        if n * n > p + 1:
+            new = [x for x in P._distinct_sites(np.random.default_rng(seed + 5), n, min(n * n, p + 3)).tolist()
+                   if x not in net.tsv_site[0].tolist()][:1]
+            keep = slice(1, None) if p > 1 else slice(None)
+            net.tsv_site[0] = np.vstack([net.tsv_site[0][keep], np.array(new, dtype=np.int32).reshape(-1, 2)]).astype(np.int32)
+            net.tsv_r[0] = np.concatenate([net.tsv_r[0][keep], [0.11] * len(new)])
+            pdn.update_tsvs(net.tsv_site, net.tsv_r)
+            o = Oracle(net)
+            pdn.reff(out)
+            assert rel_err(out.cpu().numpy().reshape(m, nl), o.reff_all()) <= 1e-8, what
+            if flags & PDN_TERMINAL_PAIRS:
+                ll = torch.empty(nl * nl, dtype=torch.float64, device="cuda:0")
+                pdn.reff_same_side(1, ll)
+                assert rel_err(ll.cpu().numpy().reshape(nl, nl), o.reff_same_side(1)) <= 1e-8, what
+        pdn.close()
+
+
 def test_two_host_threads_with_their_own_contexts():
     """The library is thread-compatible: contexts created and used concurrently from two host threads (shared
     device-memory pool, per-thread pinned scratch) give the same results as one after the other."""
