@@ -301,6 +301,9 @@ def run_cuda(a):
                      "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
                      "launches": int(cls_n[dom]), "avg_launch_ms": cls_ms[dom] / max(cls_n[dom], 1),
                      "alg_bytes_per_launch": cls_by[dom] / max(cls_n[dom], 1),
+                     "timing": "CUDA events around every launch on the launching stream, in a repeat of the same "
+                               f"{a.steps} steps right after the timed region (so that `value` carries no event overhead)",
+                     "ms_per_step_in_that_pass": ms_prof / a.steps,
                      "stencil_phase": {"achieved": phase, "frac": phase / peak, "ms": tot_ms,
                                        "share_of_step": tot_ms / ms_prof if ms_prof else None},
                      "classes": {k: {"ms": cls_ms[k], "GBps": (cls_by[k] / (cls_ms[k] * 1e-3) / 1e9) if cls_ms[k] > 0 else 0.0,
