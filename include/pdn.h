@@ -63,7 +63,8 @@ enum {
                                gathered at every port): needed by pdn_reff_same_side and pdn_load_voltages; costs
                                about as much again as the bump / load part of pdn_create                        */
     PDN_NO_UNIFORM_FAST_PATH = 8 /* solve uniform tiers numerically too (default: a tier whose x-segments are all
-                               equal and whose y-segments are all equal is reduced by the closed form, Eq. (3)) */
+                               equal and whose y-segments are all equal is reduced by the closed form, Eq. (3),
+                               when it has enough ports for the 12 n^3-flop table to be cheaper than the solves) */
 };
 
 /* kernel classes of pdn_stats.class_* */

@@ -95,7 +95,14 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
         T.whole = true;
         return PDN_OK;
     }
-    if (!(o.flags & PDN_NO_UNIFORM_FAST_PATH)) {
+    // The spectral table of a uniform tier costs 12 n^3 flops whatever the port count; q port solves cost about
+    // 8 iterations x 14 passes over a vector each.  With few ports on a very large mesh the solves are cheaper
+    // (measured: n = 16384, 7 ports: 0.9 s against 4.7 s), so the table is used only where this model says it pays
+    // (FP64 tensor-core rate of the two contractions: ~3 TF/s at n = 1024, saturating near 22 TF/s).
+    const double nn = (double)n * n;
+    const double t_table = 1e-4 + 12.0 * nn * n / std::min(22e12, 3e12 * n / 1024.0);
+    const double t_solves = 5e-4 + (double)T.q * 112.0 * 8.0 * nn / 4e12;
+    if (!(o.flags & PDN_NO_UNIFORM_FAST_PATH) && t_table <= t_solves) {
         // uniform tier: Eq. (3) of the paper as two dense contractions + a gather (uniform.cuh)
         int* fl = H.flags.as<int>();
         CK(cudaMemsetAsync(fl, 0, sizeof(int), L.s));

@@ -369,6 +369,10 @@ def test_large_ragged_meshes_match_wu_closed_form(n, fast_path):
     sites = [P._distinct_sites(rng, n, 6)]
     sites[0][0], sites[0][1], sites[0][2] = (0, 0), (n - 1, n - 1), (n - 1, 0)
     net = P.make_uniform(2, n, 0.8, 1.7, rt=0.1, tsv_sites=sites, bumps=np.array([[3, 3]]), loads=np.array([[5, 5]]))
+    if fast_path:      # enough ports for the table to pay on a mesh this size (with 6 the library solves instead)
+        extra = [s for s in P._distinct_sites(rng, n, 300).tolist() if s not in sites[0].tolist()]
+        sites[0] = np.vstack([sites[0], np.array(extra, dtype=np.int32)])
+        net = P.make_uniform(2, n, 0.8, 1.7, rt=0.1, tsv_sites=sites, bumps=np.array([[3, 3]]), loads=np.array([[5, 5]]))
     pdn = Pdn.from_network(net, device="cuda:0", rtol=1e-10, flags=0 if fast_path else PDN_NO_UNIFORM_FAST_PATH)
     Z = pdn.port_matrix(0)
     assert pdn.stats()["n_uniform_tiers"] == (2 if fast_path else 0)
