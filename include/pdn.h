@@ -140,7 +140,11 @@ typedef struct {
 
 /* S0-S3.  tiers: HOST array of n_tiers descriptors (all tiers must have the same n).  tsvs, bumps,
  * loads: HOST arrays, copied.  On success *out owns all device memory it needs for pdn_reff.
- * Work is ordered on opts->cuda_stream; the call returns after that work completed. */
+ * Work is ordered on opts->cuda_stream; the call returns after that work completed.
+ * n_tiers >= 2 needs at least one TSV on every interface.  n_tiers == 1 is the degenerate 2-D PDN (bumps and
+ * loads on the one mesh, n_tsv == 0, tsvs may be NULL): R_eff is then Eq. (2) on that mesh, by the same port
+ * solves and no recombination; pdn_update_tsvs, pdn_reff_same_side, pdn_load_voltages and pdn_reff_nodes need
+ * n_tiers >= 2. */
 int pdn_create(pdn_ctx **out, int32_t n_tiers, const pdn_tier *tiers,
                int32_t n_tsv, const pdn_tsv *tsvs,
                int32_t n_bumps, const pdn_site *bumps,

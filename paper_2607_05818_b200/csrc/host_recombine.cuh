@@ -74,10 +74,26 @@ void block_substitute(pdn_ctx* c, Launcher& L, std::vector<DevBuf>& F, int nrhs)
     CK(cudaStreamSynchronize(L.s));  // tmp goes back to the pool here
 }
 
+// d = 1: the pair-kernel operands straight from the tier's port matrix (port.cuh: k_single_tier_operands).
+int single_tier_operands(pdn_ctx* c, Launcher& L) {
+    const int m = c->m, n = c->nl;
+    TierPorts& T = c->tiers[0];
+    c->p0 = m;
+    c->A1.alloc((size_t)m * m * sizeof(double));
+    c->X0.alloc((size_t)n * m * sizeof(double));
+    c->u.alloc((size_t)m * sizeof(double));
+    c->w.alloc((size_t)n * sizeof(double));
+    L.run(KC_DENSE, 0, [&] { k_set_identity<<<cdiv((size_t)m * m, 256), 256, 0, L.s>>>(m, c->A1.as<double>()); });
+    L.run(KC_DENSE, 0, [&] { k_single_tier_operands<<<dim3(cdiv(m, 128), n + 1), 128, 0, L.s>>>(m, n, T.ZT.as<double>(), T.q, T.zdiag.as<double>(), c->X0.as<double>(), c->u.as<double>(), c->w.as<double>()); });
+    CK(cudaStreamSynchronize(L.s));
+    return PDN_OK;
+}
+
 // S2 + S3: assemble C = [K B; B^T 0] (block-tridiagonal SPD K), factor it once, substitute for the
 // m + n + (d-1) right-hand sides, eliminate the multipliers, and leave the pair-kernel operands.  The factor
 // (L_i^-1, the transformed couplings, K^-1 B and S^-1) stays in the context for pdn_reff_nodes.
 int recombine(pdn_ctx* c, Launcher& L) {
+    if (c->d == 1) return single_tier_operands(c, L);
     const int d = c->d, dm1 = d - 1, m = c->m, n = c->nl, mn = m + n, nrhs = mn + dm1;
     std::vector<DevBuf> Kd(dm1), F(dm1), rt(dm1);
     std::vector<DevBuf>& V = c->Vf;

@@ -67,6 +67,7 @@ void tier_port_list(const pdn_ctx* c, int t, const std::vector<std::vector<int>>
     if (t < c->d - 1) node.insert(node.end(), site[t].begin(), site[t].end());
     ntsv = (int)node.size();
     if (t == 0) node.insert(node.end(), c->bump_id.begin(), c->bump_id.end());
+    if (c->d == 1) ntsv = (int)node.size();  // single tier: the bumps are the row sources, the loads the terminals
     if (t == c->d - 1) node.insert(node.end(), c->load_id.begin(), c->load_id.end());
 }
 
@@ -212,9 +213,10 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
                int32_t n_bumps, const pdn_site* bumps, int32_t n_loads, const pdn_site* loads, const pdn_opts* opts) {
     if (!out) return fail_arg("out is null");
     *out = nullptr;
-    if (!tiers || !tsvs || !bumps || !loads) return fail_arg("null input array");
-    if (n_tiers < 2) return fail_arg("need at least 2 tiers");
-    if (n_tsv < 1 || n_bumps < 1 || n_loads < 1) return fail_arg("need at least one TSV, bump and load");
+    if (!tiers || !bumps || !loads || (!tsvs && n_tsv > 0)) return fail_arg("null input array");
+    if (n_tiers < 1) return fail_arg("need at least 1 tier");
+    if (n_tiers == 1 ? n_tsv != 0 : n_tsv < 1) return fail_arg("need at least one TSV per interface (and none for a single tier)");
+    if (n_bumps < 1 || n_loads < 1) return fail_arg("need at least one bump and one load");
     const int d = n_tiers, n = tiers[0].n;
     if (n < 2) return fail_arg("mesh size n must be >= 2");
     if ((int64_t)n * n > (int64_t)1 << 30) return fail_arg("mesh too large");
@@ -240,6 +242,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         c->terminal_pairs = (o.flags & PDN_TERMINAL_PAIRS) != 0;
         c->nu_auto = nu_auto;
         if (o.shard_world > 1) {
+            if (d == 1) throw StatusFail{PDN_E_ARG, "sharding needs at least 2 tiers"};
             if (o.shard_rank < 0 || o.shard_rank >= o.shard_world) throw StatusFail{PDN_E_ARG, "shard_rank out of range"};
             c->shard_world = o.shard_world; c->shard_rank = o.shard_rank; c->open = true;
         }
@@ -364,6 +367,7 @@ int pdn_update_tsvs(pdn_ctx* ctx, int32_t n_tsv, const pdn_tsv* tsvs) {
     if (!ctx || !tsvs || n_tsv < 1) return fail_arg("null context / TSV list or empty list");
     PDN_CHECK_DEVICE(ctx);
     if (ctx->open || ctx->shard_world > 1) return fail_arg("TSV re-planning is not available on a sharded context");
+    if (ctx->d < 2) return fail_arg("a single-tier context has no TSVs");
     pdn_ctx* c = ctx;
     const int d = c->d, n = c->n;
     int status = PDN_OK;
@@ -542,6 +546,7 @@ int pdn_reff_same_side(pdn_ctx* ctx, int32_t side, double* out) {
     PDN_CHECK_DEVICE(ctx);
     if (!ctx->terminal_pairs) return fail_arg("the context was not created with PDN_TERMINAL_PAIRS");
     if (ctx->open) return fail_arg("sharded context is still open: exchange the rows and call pdn_finish first");
+    if (ctx->d < 2) return fail_arg("same-side pairs need at least 2 tiers (on one tier list the nodes as bumps and loads)");
     try {
         Launcher L{ctx, ctx->stream};
         const pdn_ctx::Side& S = ctx->side[side];
@@ -566,6 +571,7 @@ int pdn_load_voltages(pdn_ctx* ctx, int32_t bump, const double* i_load, double v
     if (!ctx->terminal_pairs) return fail_arg("the context was not created with PDN_TERMINAL_PAIRS");
     if (ctx->open) return fail_arg("sharded context is still open: exchange the rows and call pdn_finish first");
     if (bump < 0 || bump >= ctx->m) return fail_arg("bump index out of range");
+    if (ctx->d < 2) return fail_arg("pdn_load_voltages needs at least 2 tiers");
     try {
         Launcher L{ctx, ctx->stream};
         const int n = ctx->nl, m = ctx->m, p0 = ctx->p0;
@@ -603,6 +609,7 @@ int pdn_reff_nodes(pdn_ctx* ctx, int32_t n_nodes, const pdn_node* nodes, double*
     if (!ctx || !nodes || !out || n_nodes < 1) return fail_arg("null context / node list / output or empty list");
     PDN_CHECK_DEVICE(ctx);
     if (ctx->open) return fail_arg("sharded context is still open: exchange the rows and call pdn_finish first");
+    if (ctx->d < 2) return fail_arg("pdn_reff_nodes needs at least 2 tiers (on one tier list the nodes as bumps and loads)");
     pdn_ctx* c = ctx;
     const int d = c->d, n = c->n, dm1 = d - 1, np = n_nodes;
     for (int a = 0; a < np; ++a) {

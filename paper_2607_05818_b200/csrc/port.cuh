@@ -272,6 +272,20 @@ __global__ void k_load_voltages(int n, const double* __restrict__ Rb, const doub
     if (lane == 0) v[j] = v_bump - 0.5 * s;
 }
 
+// Single tier (d = 1, a 2-D PDN: no TSVs, nothing to recombine).  The bumps are the row sources of the tier's port
+// matrix (ports = [bumps] ++ [loads], ntsv = m), and R(i,j) = Z[b_i,b_i] + Z[l_j,l_j] - 2 Z[b_i,l_j] is Eq. (2) on
+// the one mesh.  Written as operands of the pair kernels:  A1 = I (m x m, set by the caller),
+// X0[j][a] = Z[b_a, l_j],  u[i] = Z[b_i, b_i],  w[j] = zdiag[j].
+__global__ void k_single_tier_operands(int m, int n, const double* __restrict__ ZT, int64_t q,
+                                       const double* __restrict__ zdiag, double* __restrict__ X0,
+                                       double* __restrict__ u, double* __restrict__ w) {
+    const int a = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (a >= m) return;
+    if (j < n) X0[(int64_t)j * m + a] = ZT[(int64_t)a * q + m + j];
+    else u[a] = ZT[(int64_t)a * q + a];
+    if (j < n && a == 0) w[j] = zdiag[j];
+}
+
 // S4, full cross product:  R[i][j] = u[i] + w[j] - 2 sum_a A1[i][a] X0[j][a].   64x64 tile / block.
 __global__ void __launch_bounds__(256)
 k_pair_full(int m, int n, int p0, const double* __restrict__ A1, const double* __restrict__ X0,

@@ -57,7 +57,7 @@ def test_pure_status_helpers():
 
 
 def test_argument_validation_runs_on_the_host_before_any_device_work():
-    """pdn_create rejects malformed inputs with PDN_E_ARG on the host (no device needed): too few tiers, a TSV
+    """pdn_create rejects malformed inputs with PDN_E_ARG on the host (no device needed): TSVs on a single tier, a TSV
     outside the mesh or on an interface that does not exist, a non-positive resistance, a duplicate site inside
     one interface, an interface without TSVs, a terminal outside the mesh."""
     import numpy as np
@@ -71,9 +71,9 @@ def test_argument_validation_runs_on_the_host_before_any_device_work():
             Pdn(net.n, net.gx, net.gy, net.tsv_site, net.tsv_r, net.bumps, net.loads)
         return e.value.status
 
-    def one_tier(net):
-        net.gx, net.gy, net.tsv_site, net.tsv_r = net.gx[:1], net.gy[:1], net.tsv_site[:0], net.tsv_r[:0]
-    assert status_of(one_tier) == 1
+    def one_tier_with_tsvs(net):                 # a single tier is a 2-D PDN: it has no interface for a TSV
+        net.gx, net.gy = net.gx[:1], net.gy[:1]
+    assert status_of(one_tier_with_tsvs) == 1
     assert status_of(lambda n: n.tsv_site[0].__setitem__(0, [32, 0])) == 1
     assert status_of(lambda n: n.tsv_r[0].__setitem__(3, 0.0)) == 1
     assert status_of(lambda n: n.tsv_r[0].__setitem__(3, float("inf"))) == 1

@@ -645,6 +645,47 @@ def test_randomised_stacks_through_every_entry_point(block):
         pdn.close()
 
 
+@pytest.mark.parametrize("n,kw", [(4, {}), (37, dict(drop=0.05, aniso=2.0)), (130, {}), (64, dict(uniform=True))])
+def test_single_tier_is_the_2d_case(n, kw):
+    """Degenerate stack: ONE tier, no TSVs -- R_eff between bumps and loads of the same mesh (Eq. 2 on a 2-D PDN), against
+    the oracle and, on the uniform mesh, against Eq. (3) PAPER.md:49 directly; a bump that is also a load gives 0."""
+    from closed_forms import wu_mesh_reff
+    from oracle.reff_oracle import Oracle
+    from paper_2607_05818_b200 import Pdn, PdnError
+    torch = torch_cuda()
+    kw = dict(kw)
+    if kw.pop("uniform", False):
+        rng = np.random.default_rng(n)
+        net = P.make_uniform(1, n, 0.6, 1.1, tsv_sites=[], bumps=P._distinct_sites(rng, n, 40), loads=P._distinct_sites(rng, n, 45))
+    else:
+        net = P.make_random(91, d=1, n=n, p=1, m=3, nl=5, **kw)
+    net.loads[1] = net.bumps[0]                      # the same node on both lists
+    pdn = Pdn.from_network(net, device="cuda:0", rtol=1e-10)
+    out = torch.empty(net.m * net.nl, dtype=torch.float64, device="cuda:0")
+    pdn.reff(out)
+    got = out.cpu().numpy().reshape(net.m, net.nl)
+    want = Oracle(net).reff_all()
+    assert abs(got[0, 1]) <= 1e-12 * want.max()
+    nz = want > 0
+    rel = np.abs(got[nz] / want[nz] - 1.0)
+    assert rel.max() <= MAX_REL and rel.mean() <= MEAN_REL
+    if net.name.startswith("uniform") or "uniform" in net.name:
+        assert pdn.stats()["n_uniform_tiers"] == 1
+    if n == 64:
+        for i in range(0, net.m, 7):
+            for j in range(2, net.nl, 9):
+                (y1, x1), (y2, x2) = net.bumps[i], net.loads[j]
+                assert got[i, j] == pytest.approx(wu_mesh_reff(n, n, 0.6, 1.1, x1, y1, x2, y2), rel=1e-9)
+    bi = torch.tensor([2, 0], dtype=torch.int32, device="cuda:0")
+    li = torch.tensor([4, 3], dtype=torch.int32, device="cuda:0")
+    o2 = torch.empty(2, dtype=torch.float64, device="cuda:0")
+    pdn.reff(o2, bi, li)
+    assert np.allclose(o2.cpu().numpy(), got[[2, 0], [4, 3]], rtol=1e-12, atol=0)
+    with pytest.raises(PdnError):
+        pdn.reff_nodes(np.array([[0, 0, 0], [0, 1, 1]], dtype=np.int32), torch.empty(4, dtype=torch.float64, device="cuda:0"))
+    pdn.close()
+
+
 def test_two_host_threads_with_their_own_contexts():
     """The library is thread-compatible: contexts created and used concurrently from two host threads (shared
     device-memory pool, per-thread pinned scratch) give the same results as one after the other."""
