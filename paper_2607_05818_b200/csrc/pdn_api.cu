@@ -540,6 +540,12 @@ int pdn_reff_host(pdn_ctx* ctx, int64_t n_pairs, const int32_t* bump_idx, const 
 
 void pdn_release_cache(void) { g_pool.trim(); }
 
+#ifdef PDN_PHASE_CLOCKS
+int pdn_debug_phase_clocks(long long* out) {  // scratch instrumentation, not part of the ABI
+    return (int)cudaMemcpyFromSymbol(out, pdn::g_phase_clk, sizeof(long long) * 64 * 8);
+}
+#endif
+
 // NEXT-3: R_eff between terminals of the same side (bump-bump or load-load), full nt x nt matrix on the device.
 int pdn_reff_same_side(pdn_ctx* ctx, int32_t side, double* out) {
     if (!ctx || !out || (side != 0 && side != 1)) return fail_arg("null context / output or side not in {0, 1}");

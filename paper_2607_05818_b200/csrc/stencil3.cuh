@@ -63,12 +63,13 @@ __device__ __forceinline__ void exch_clear(Exch<W>& x) {
     }
 }
 
-// Coefficients of this thread's patch (zeros outside the mesh) and its slots of the scaling tile
-// sc[row][lane] = (s, sd) of column 0, (s, sd) of column 1.
+// Coefficients of this thread's patch (zeros outside the mesh) and its slots of the scaling tile: two float2
+// planes, s_slot[row*32] = s of columns 0, 1 and s_slot[SD_OFF + row*32] = sd of columns 0, 1, so that a stage
+// that needs only one of the two reads 8 bytes per lane, not 16.
 template <int R>
 __device__ __forceinline__ void patch_init(Patch<R>& c, const double* __restrict__ pE, const double* __restrict__ pS,
                                            const float2* __restrict__ psc, const Level& L, int gx, int gy0,
-                                           float4* sc_slot) {
+                                           float2* s_slot, int sd_off) {
     const bool xin = gx >= 0 && gx < L.pitch;  // gx is even, pitch is even: both columns are addressable
 #pragma unroll
     for (int i = 0; i < R; ++i) {
@@ -81,7 +82,11 @@ __device__ __forceinline__ void patch_init(Patch<R>& c, const double* __restrict
         c.hE0[i] = e.x; c.hE1[i] = e.y;
         c.hS0[i] = s.x; c.hS1[i] = s.y;
         c.hW0[i] = (in && gx > 0) ? __ldg(pE + gi - 1) : 0.0;
-        if (psc) sc_slot[i * 32] = in ? __ldg(reinterpret_cast<const float4*>(psc + gi)) : make_float4(0.f, 0.f, 0.f, 0.f);
+        if (psc) {
+            const float4 v = in ? __ldg(reinterpret_cast<const float4*>(psc + gi)) : make_float4(0.f, 0.f, 0.f, 0.f);
+            s_slot[i * 32] = make_float2(v.x, v.z);
+            s_slot[sd_off + i * 32] = make_float2(v.y, v.w);
+        }
     }
     const int gyn = gy0 - 1;
     const double2 nn = (xin && gyn >= 0 && gyn < L.ny) ? ldg2(pS + (size_t)gyn * L.pitch + gx) : make_double2(0.0, 0.0);
@@ -192,12 +197,25 @@ struct Geom {
 // The right-hand sides of [b0, b0 + nmax) that are still iterating (all of them if active == nullptr), in
 // order, for every thread of the block.  Converged right-hand sides are frozen: no kernel touches their
 // vectors again.  Call before the block's first __syncthreads.
-constexpr int T3_MAX_G = 64;
+constexpr int T3_MAX_G = 32;
+#ifdef PDN_PHASE_CLOCKS
+__device__ long long g_phase_clk[64 * 8];
+#define PHASE_CLK(j, k)                                                                                   \
+    do {                                                                                                  \
+        if (FUSED && blockIdx.x == 5 && blockIdx.y == 5 && blockIdx.z == 0 && threadIdx.x == 5 * 32 && (j) < 64) \
+            g_phase_clk[(j) * 8 + (k)] = clock64();                                                       \
+    } while (0)
+#else
+#define PHASE_CLK(j, k) do { } while (0)
+#endif
+
 struct ActiveList {
     int b[T3_MAX_G];
-    int n;
+    double s[T3_MAX_G];  // the per-right-hand-side scalar of the kernel (alpha / beta), staged once per block so that
+    int n;               // the loop over right-hand sides has no dependent global load in front of its first FMA
 };
-__device__ __forceinline__ void active_list_build(ActiveList& al, const int* __restrict__ active, int b0, int nmax) {
+__device__ __forceinline__ void active_list_build(ActiveList& al, const int* __restrict__ active, int b0, int nmax,
+                                                  const double* __restrict__ scal = nullptr) {
     if (threadIdx.x < 32) {
         const int lane = threadIdx.x;
         int cnt = 0;
@@ -205,7 +223,11 @@ __device__ __forceinline__ void active_list_build(ActiveList& al, const int* __r
             const int j = base + lane;
             const bool a = j < nmax && (active == nullptr || active[b0 + j] != 0);
             const unsigned m = __ballot_sync(FULL, a);
-            if (a) al.b[cnt + __popc(m & ((1u << lane) - 1u))] = b0 + j;
+            if (a) {
+                const int slot = cnt + __popc(m & ((1u << lane) - 1u));
+                al.b[slot] = b0 + j;
+                al.s[slot] = scal ? scal[b0 + j] : 0.0;
+            }
             cnt += __popc(m);
         }
         if (lane == 0) al.n = cnt;
@@ -242,23 +264,24 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
     extern __shared__ __align__(128) double smem_dyn[];
     double* rbuf = smem_dyn;                                   // 2 stages
     double* qbuf = rbuf + 2 * Gm::TILE;                        // 2 stages (FUSED only)
-    float4* sc = reinterpret_cast<float4*>(qbuf + (FUSED ? 2 * Gm::TILE : 0));
-    Exch<W>& x = *reinterpret_cast<Exch<W>*>(sc + Gm::EH * 32);
+    float2* sc = reinterpret_cast<float2*>(qbuf + (FUSED ? 2 * Gm::TILE : 0));
+    constexpr int SD_OFF = Gm::EH * 32;
+    Exch<W>& x = *reinterpret_cast<Exch<W>*>(sc + 2 * SD_OFF);
     __shared__ uint64_t mbar[3];  // two TMA stages + the row-exchange barrier
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int x0 = blockIdx.x * Gm::IW - H, y0 = blockIdx.y * Gm::IH - H;
     const int gx = x0 + 2 * lane, gy0 = y0 + R * warp;
     const int slot0 = (R * warp) * T3_EW + 2 * lane;
-    float4* sc_slot = sc + (R * warp) * 32 + lane;
+    float2* sc_slot = sc + (R * warp) * 32 + lane;
     Patch<R> c;
-    patch_init<R>(c, L.hE, L.hS, L.sc, L, gx, gy0, sc_slot);
+    patch_init<R>(c, L.hE, L.hS, L.sc, L, gx, gy0, sc_slot, SD_OFF);
     exch_clear<R, W>(x);
     const unsigned interior = interior_mask<R, H, Gm::IW, Gm::IH>(L, lane, warp, gx, gy0);
     const size_t plane = (size_t)L.ny * L.pitch, cplane = (size_t)cny * cpitch;
     const size_t goff = (size_t)gy0 * L.pitch + gx;
     __shared__ ActiveList al;
-    active_list_build(al, active, blockIdx.z * G, min(G, B - (int)blockIdx.z * G));
+    active_list_build(al, active, blockIdx.z * G, min(G, B - (int)blockIdx.z * G), FUSED ? alpha : nullptr);
     if (threadIdx.x == 0) {
         mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); mbar_init(&mbar[2], 32 * W);
         mbar_fence_init();
@@ -278,25 +301,27 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
     Xchg<W> xc{&x, &mbar[2], 0, 0u, warp, lane};
     for (int j = 0; j < nb; ++j) {
         const int b = al.b[j], st = j & 1;
+        PHASE_CLK(j, 0);
         mbar_wait(&mbar[st], (j >> 1) & 1);
-        const double al = FUSED ? alpha[b] : 0.0;
+        PHASE_CLK(j, 1);
+        const double alj = FUSED ? al.s[j] : 0.0;
         double y0r[R], y1r[R], rh0[R], rh1[R], rr = 0.0;
 #pragma unroll
         for (int i = 0; i < R; ++i) {
             double2 r = ld2(rbuf + st * Gm::TILE + slot0 + i * T3_EW);
             if (FUSED) {
                 const double2 q = ld2(qbuf + st * Gm::TILE + slot0 + i * T3_EW);
-                r.x = fma(-al, q.x, r.x);
-                r.y = fma(-al, q.y, r.y);
+                r.x = fma(-alj, q.x, r.x);
+                r.y = fma(-alj, q.y, r.y);
                 const bool in = (interior >> i) & 1;
                 if (in) st2(r_out + b * plane + goff + (size_t)i * L.pitch, r);
                 const double mx = in ? r.x : 0.0, my = in ? r.y : 0.0;
                 rr = fma(mx, mx, rr);
                 rr = fma(my, my, rr);
             }
-            const float4 s4 = sc_slot[i * 32];
-            rh0[i] = (double)s4.x * r.x;
-            rh1[i] = (double)s4.z * r.y;
+            const float2 s2 = sc_slot[i * 32];
+            rh0[i] = (double)s2.x * r.x;
+            rh1[i] = (double)s2.y * r.y;
             y0r[i] = ch.w[0] * rh0[i];
             y1r[i] = ch.w[0] * rh1[i];
         }
@@ -304,6 +329,7 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
             rr = warp_sum(rr);
             if (lane == 0) atomicAdd(rr_acc + b, rr);
         }
+        PHASE_CLK(j, 2);
         // once thread 0 is past the first row exchange of this iteration every thread has arrived there,
         // i.e. has consumed the stage: thread 0 may refill it with right-hand side j+2
 #pragma unroll
@@ -311,17 +337,19 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
             smooth_step<R, W>(xc, c, y0r, y1r, rh0, rh1, ch.w[k]);
             if (k == 1 && threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
         }
+        PHASE_CLK(j, 3);
         double t0[R], t1[R];
         apply_step<R, W>(xc, c, y0r, y1r, rh0, rh1, t0, t1);
+        PHASE_CLK(j, 4);
         if (NU == 1 && threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
         // residual of the unscaled system at the patch nodes, summed over 2x2 aggregates
 #pragma unroll
         for (int i = 0; i < R; i += 2) {
-            const float4 sa = sc_slot[i * 32], sb = sc_slot[(i + 1) * 32];
-            double v = (double)sa.y * (t0[i] - y0r[i]);
-            v = fma((double)sa.w, t1[i] - y1r[i], v);
-            v = fma((double)sb.y, t0[i + 1] - y0r[i + 1], v);
-            v = fma((double)sb.w, t1[i + 1] - y1r[i + 1], v);
+            const float2 sa = sc_slot[SD_OFF + i * 32], sb = sc_slot[SD_OFF + (i + 1) * 32];
+            double v = (double)sa.x * (t0[i] - y0r[i]);
+            v = fma((double)sa.y, t1[i] - y1r[i], v);
+            v = fma((double)sb.x, t0[i + 1] - y0r[i + 1], v);
+            v = fma((double)sb.y, t1[i + 1] - y1r[i + 1], v);
             if ((interior >> i) & 1) {  // rows i and i+1 are interior together (H, R, y0 even)
                 st2(y_out + b * plane + goff + (size_t)i * L.pitch, make_double2(y0r[i], y1r[i]));
                 if ((interior >> (i + 1)) & 1)
@@ -329,6 +357,7 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
                 rc[b * cplane + (size_t)((gy0 + i) >> 1) * cpitch + (gx >> 1)] = v;
             }
         }
+        PHASE_CLK(j, 5);
     }
 }
 
@@ -346,17 +375,18 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
     double* rbuf = smem_dyn;             // 2 stages each
     double* ybuf = rbuf + 2 * Gm::TILE;
     double* ebuf = ybuf + 2 * Gm::TILE;  // T3_ECW x EH/2 per stage
-    float4* sc = reinterpret_cast<float4*>(ebuf + 2 * Gm::ETILE);
-    Exch<W>& x = *reinterpret_cast<Exch<W>*>(sc + Gm::EH * 32);
+    float2* sc = reinterpret_cast<float2*>(ebuf + 2 * Gm::ETILE);
+    constexpr int SD_OFF = Gm::EH * 32;
+    Exch<W>& x = *reinterpret_cast<Exch<W>*>(sc + 2 * SD_OFF);
     __shared__ uint64_t mbar[3];  // two TMA stages + the row-exchange barrier
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int x0 = blockIdx.x * Gm::IW - H, y0 = blockIdx.y * Gm::IH - H;
     const int gx = x0 + 2 * lane, gy0 = y0 + R * warp;
     const int slot0 = (R * warp) * T3_EW + 2 * lane;
-    float4* sc_slot = sc + (R * warp) * 32 + lane;
+    float2* sc_slot = sc + (R * warp) * 32 + lane;
     Patch<R> c;
-    patch_init<R>(c, L.hE, L.hS, L.sc, L, gx, gy0, sc_slot);
+    patch_init<R>(c, L.hE, L.hS, L.sc, L, gx, gy0, sc_slot, SD_OFF);
     exch_clear<R, W>(x);
     const unsigned interior = interior_mask<R, H, Gm::IW, Gm::IH>(L, lane, warp, gx, gy0);
     const size_t plane = (size_t)L.ny * L.pitch;
@@ -389,16 +419,19 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
         const int b = al.b[j], st = j & 1;
         mbar_wait(&mbar[st], (j >> 1) & 1);
         double y0r[R], y1r[R], rh0[R], rh1[R];
+        double ec[R / 2];  // one coarse correction per pair of rows (R and H are even: rows 2k, 2k+1 share a coarse row)
+#pragma unroll
+        for (int k = 0; k < R / 2; ++k) ec[k] = ebuf[st * Gm::ETILE + ((R * warp) / 2 + k) * T3_ECW + eslot];
 #pragma unroll
         for (int i = 0; i < R; ++i) {
             const double2 r = ld2(rbuf + st * Gm::TILE + slot0 + i * T3_EW);
             const double2 yin = ld2(ybuf + st * Gm::TILE + slot0 + i * T3_EW);
-            const double e = ebuf[st * Gm::ETILE + ((R * warp + i) >> 1) * T3_ECW + eslot];
-            const float4 s4 = sc_slot[i * 32];
-            rh0[i] = (double)s4.x * r.x;
-            rh1[i] = (double)s4.z * r.y;
-            y0r[i] = fma((double)s4.y, e, yin.x);
-            y1r[i] = fma((double)s4.w, e, yin.y);
+            const double e = ec[i >> 1];
+            const float2 s2 = sc_slot[i * 32], d2 = sc_slot[SD_OFF + i * 32];
+            rh0[i] = (double)s2.x * r.x;
+            rh1[i] = (double)s2.y * r.y;
+            y0r[i] = fma((double)d2.x, e, yin.x);
+            y1r[i] = fma((double)d2.y, e, yin.y);
         }
         if (DOT && b_pend >= 0) {
             rz_pend = warp_sum(rz_pend);
@@ -413,9 +446,9 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
 #pragma unroll
         for (int i = 0; i < R; ++i) {
             const bool in = (interior >> i) & 1;
-            const float4 s4 = sc_slot[i * 32];
+            const float2 s2 = sc_slot[i * 32];
             if (in) st2(z_out + b * plane + goff + (size_t)i * L.pitch,
-                        make_double2((double)s4.x * y0r[i], (double)s4.z * y1r[i]));
+                        make_double2((double)s2.x * y0r[i], (double)s2.y * y1r[i]));
             if (DOT) {  // r.z = r.(s y) = (s r).y = r^.y
                 rz = fma(in ? rh0[i] : 0.0, y0r[i], rz);
                 rz = fma(in ? rh1[i] : 0.0, y1r[i], rz);
@@ -453,7 +486,7 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
     const int gx = x0 + 2 * lane, gy0 = y0 + R * warp;
     const int slot0 = (R * warp) * T3_EW + 2 * lane;
     Patch<R> c;
-    patch_init<R>(c, L.gx, L.gy, nullptr, L, gx, gy0, nullptr);
+    patch_init<R>(c, L.gx, L.gy, nullptr, L, gx, gy0, nullptr, 0);
     const double zero[R] = {};
     double d0[R], d1[R];  // diagonal = sum of the incident conductances
 #pragma unroll
@@ -467,7 +500,7 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
     const size_t plane = (size_t)L.ny * L.pitch;
     const size_t goff = (size_t)gy0 * L.pitch + gx;
     __shared__ ActiveList al;
-    active_list_build(al, active, blockIdx.z * G, min(G, B - (int)blockIdx.z * G));
+    active_list_build(al, active, blockIdx.z * G, min(G, B - (int)blockIdx.z * G), beta);
     if (threadIdx.x == 0) {
         mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); mbar_init(&mbar[2], 32 * W);
         mbar_fence_init();
@@ -498,7 +531,7 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
     for (int j = 0; j < nb; ++j) {
         const int b = al.b[j], st = j & 1;
         mbar_wait(&mbar[st], (j >> 1) & 1);
-        const double bt = beta[b];
+        const double bt = al.s[j];
         double p0[R], p1[R], sump = 0.0, pq = 0.0;
 #pragma unroll
         for (int i = 0; i < R; ++i) {
