@@ -53,7 +53,9 @@ class PdnStats(C.Structure):
 
 
 EXPORTS = ("pdn_create", "pdn_reff", "pdn_reff_host", "pdn_destroy", "pdn_strerror", "pdn_last_error",
-           "pdn_get_stats", "pdn_port_count", "pdn_get_port_matrix", "pdn_release_cache", "pdn_update_tsvs", "pdn_reff_same_side", "pdn_load_voltages", "pdn_reff_nodes", "pdn_shard_slice", "pdn_shard_buffers", "pdn_finish")
+           "pdn_get_stats", "pdn_port_count", "pdn_get_port_matrix", "pdn_release_cache", "pdn_update_tsvs",
+           "pdn_reff_same_side", "pdn_load_voltages", "pdn_reff_nodes", "pdn_shard_slice", "pdn_shard_buffers",
+           "pdn_finish")
 
 _lib = None
 
