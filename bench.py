@@ -185,7 +185,7 @@ def run_cuda(a):
     out_h = torch.empty(npairs, dtype=torch.float64).pin_memory()
     args = (net.n,), (net.tsv_site, net.tsv_r, net.bumps, net.loads)
 
-    base_flags = 8 if a.no_fast_path else 0      # PDN_NO_UNIFORM_FAST_PATH
+    base_flags = (8 if a.no_fast_path else 0) | (32 if a.precond_f32 else 0)  # PDN_NO_UNIFORM_FAST_PATH, PDN_PRECOND_F32
 
     shard_kw = dict(shard_rank=rank, shard_world=world) if sharded else {}
 
@@ -284,12 +284,12 @@ def run_cuda(a):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
         "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "strong" if sharded else "weak",
         "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
+        "dtype": "f64 (multigrid sweeps in f32 registers: --precond-f32)" if a.precond_f32 else "f64", "data": "synthetic",
         "config": {"workload": workload_name(cfg) + (" -- UNIFORM variant (median conductances)" if a.uniform else ""),
                    "cfg": cfg, "pairs_per_step_per_gpu": npairs, "uniform_tiers": last["n_uniform_tiers"],
                    "l2": "working set of every stencil launch exceeds the 126 MB L2 (no flush needed)"
                          if cfg >= 3 else "working set fits L2: latency-bound case, HBM fraction not meaningful",
-                   "rtol": a.rtol or 1e-8, "nu": a.nu or 4,
+                   "rtol": a.rtol or 1e-8, "nu": a.nu or 4, "preconditioner_sweeps": "f32" if a.precond_f32 else "f64",
                    "pcg_iters_max": last["pcg_iters_max"], "rhs_iterations": last["rhs_iterations"],
                    "ms_stencil": last["ms_stencil"], "ms_dense": last["ms_dense"], "ms_upload": last["ms_upload"]},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -446,6 +446,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--uniform", action="store_true", help="uniform-tier variant of the workload (Eq. 3 fast path)")
     ap.add_argument("--no-fast-path", action="store_true", help="solve uniform tiers numerically too")
+    ap.add_argument("--precond-f32", action="store_true",
+                    help="opt-in PDN_PRECOND_F32: multigrid sweeps in FP32 registers (CG, residuals, results stay FP64)")
     ap.add_argument("--replan", type=int, default=0, metavar="K",
                     help="also time pdn_update_tsvs after moving K TSVs of every interface to new sites (NEXT-2)")
     ap.add_argument("--eq4", action="store_true",

@@ -62,6 +62,12 @@ enum {
     PDN_TERMINAL_PAIRS = 16, /* also keep the bump-source / load-source rows of the port matrices (full tolerance,
                                gathered at every port): needed by pdn_reff_same_side and pdn_load_voltages; costs
                                about as much again as the bump / load part of pdn_create                        */
+    PDN_PRECOND_F32 = 32,   /* opt-in mixed precision: the sweeps of the multigrid preconditioner (V-cycle stages
+                               above the fused coarse tail) run in FP32 registers.  The CG operator, residuals,
+                               step lengths, solutions, port matrices and everything after S1 stay FP64, every
+                               vector in HBM stays FP64, and the solves still stop at the FP64 residual test, so
+                               the results meet the same tolerance; only the iteration count may change.
+                               Off by default: the default path computes in FP64 throughout                    */
     PDN_NO_UNIFORM_FAST_PATH = 8 /* solve uniform tiers numerically too (default: a tier whose x-segments are all
                                equal and whose y-segments are all equal is reduced by the closed form, Eq. (3),
                                when it has enough ports for the 12 n^3-flop table to be cheaper than the solves) */

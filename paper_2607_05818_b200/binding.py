@@ -20,6 +20,7 @@ PDN_SKIP_CONNECTIVITY_CHECK = 2
 PDN_TIME_KERNELS = 4
 PDN_NO_UNIFORM_FAST_PATH = 8
 PDN_TERMINAL_PAIRS = 16
+PDN_PRECOND_F32 = 32
 KERNEL_CLASSES = ("pq", "down0", "up0", "down_coarse", "up_coarse", "small", "dense", "pair")
 
 

@@ -138,6 +138,7 @@ struct Smoother {
     ChebR cr;   // level 0
     ChebR crc;  // levels >= 1
     int G;  // right-hand sides a block loops over (upper bound; fewer on levels with few tiles)
+    bool f32 = false;  // PDN_PRECOND_F32: the V-cycle stages above the tail sweep in FP32 registers
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -196,7 +197,7 @@ inline int rhs_per_block(int tiles, int B, int G) {
     return (int)std::max(1L, std::min<long>(std::min(G, T3_MAX_G), g));
 }
 
-template <int NU>
+template <int NU, class T>
 void launch_down3(Launcher& L, int cls, double bytes, const Level& lv, const Smoother& sm, const ChebR& cr, int B, const CUtensorMap& m_r,
                   const CUtensorMap* m_q, const double* alpha, double* r_out, double* y_out, double* rc, int cny,
                   int cnx, int cpitch, double* rr_acc, const int* active) {
@@ -206,14 +207,14 @@ void launch_down3(Launcher& L, int cls, double bytes, const Level& lv, const Smo
     constexpr size_t base = 2 * T3_TILE_BYTES + T3_SC_BYTES + sizeof(Exch<DN_W>);
     static std::atomic<uint64_t> attr_done{0};
     once_per_device(attr_done, [&] {
-        CK(cudaFuncSetAttribute(k_down3<DN_R, DN_W, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(base + 2 * T3_TILE_BYTES)));
-        CK(cudaFuncSetAttribute(k_down3<DN_R, DN_W, NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)base));
+        CK(cudaFuncSetAttribute(k_down3<DN_R, DN_W, NU, true, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(base + 2 * T3_TILE_BYTES)));
+        CK(cudaFuncSetAttribute(k_down3<DN_R, DN_W, NU, false, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)base));
     });
-    if (m_q) L.run(cls, bytes, [&] { k_down3<DN_R, DN_W, NU, true><<<grid, 32 * DN_W, base + 2 * T3_TILE_BYTES, L.s>>>(m_r, *m_q, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
-    else L.run(cls, bytes, [&] { k_down3<DN_R, DN_W, NU, false><<<grid, 32 * DN_W, base, L.s>>>(m_r, m_r, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
+    if (m_q) L.run(cls, bytes, [&] { k_down3<DN_R, DN_W, NU, true, T><<<grid, 32 * DN_W, base + 2 * T3_TILE_BYTES, L.s>>>(m_r, *m_q, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
+    else L.run(cls, bytes, [&] { k_down3<DN_R, DN_W, NU, false, T><<<grid, 32 * DN_W, base, L.s>>>(m_r, m_r, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
 }
 
-template <int NU>
+template <int NU, class T>
 void launch_up3(Launcher& L, int cls, double bytes, const Level& lv, const Smoother& sm, const ChebR& cr, int B, const CUtensorMap& m_r,
                 const CUtensorMap& m_y, const CUtensorMap& m_e, double* z_out, double* rz_acc, const int* active) {
     constexpr int H = halo_of(NU), IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
@@ -222,11 +223,11 @@ void launch_up3(Launcher& L, int cls, double bytes, const Level& lv, const Smoot
     constexpr size_t smem = 4 * T3_TILE_BYTES + (size_t)2 * Geom<T3_R, T3_W, 2>::ETILE_BYTES + T3_SC_BYTES + sizeof(Exch<T3_W>);
     static std::atomic<uint64_t> attr_done{0};
     once_per_device(attr_done, [&] {
-        CK(cudaFuncSetAttribute(k_up3<T3_R, T3_W, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(cudaFuncSetAttribute(k_up3<T3_R, T3_W, NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_up3<T3_R, T3_W, NU, true, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_up3<T3_R, T3_W, NU, false, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     });
-    if (rz_acc) L.run(cls, bytes, [&] { k_up3<T3_R, T3_W, NU, true><<<grid, T3_THREADS, smem, L.s>>>(m_r, m_y, m_e, lv, cr, z_out, rz_acc, B, G, active); });
-    else L.run(cls, bytes, [&] { k_up3<T3_R, T3_W, NU, false><<<grid, T3_THREADS, smem, L.s>>>(m_r, m_y, m_e, lv, cr, z_out, rz_acc, B, G, active); });
+    if (rz_acc) L.run(cls, bytes, [&] { k_up3<T3_R, T3_W, NU, true, T><<<grid, T3_THREADS, smem, L.s>>>(m_r, m_y, m_e, lv, cr, z_out, rz_acc, B, G, active); });
+    else L.run(cls, bytes, [&] { k_up3<T3_R, T3_W, NU, false, T><<<grid, T3_THREADS, smem, L.s>>>(m_r, m_y, m_e, lv, cr, z_out, rz_acc, B, G, active); });
 }
 
 void launch_pq3(Launcher& L, double bytes, const Level& lv, const Smoother& sm, int B, const CUtensorMap& m_z,
@@ -243,7 +244,9 @@ void launch_pq3(Launcher& L, double bytes, const Level& lv, const Smoother& sm, 
     L.run(KC_PQ, bytes, [&] { k_pq3<PQ_R, PQ_W><<<grid, 32 * PQ_W, smem, L.s>>>(m_z, m_p, lv, beta, p_new, q, pq_acc, sump_acc, B, G, active); });
 }
 
-#define NU_DISPATCH(nu, CALL)                 \
+#define NU_DISPATCH(nu, CALL0)                \
+    if (sm.f32) { using T_ = float; NU_DISPATCH_(nu, CALL0) } else { using T_ = double; NU_DISPATCH_(nu, CALL0) }
+#define NU_DISPATCH_(nu, CALL)                \
     switch (nu) {                             \
         case 1: { constexpr int NU_ = 1; CALL; } break; \
         case 2: { constexpr int NU_ = 2; CALL; } break; \
@@ -303,7 +306,7 @@ void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Smoother& sm, int B,
         const bool f = (l == 0 && fused);
         const double bytes = (f ? 4.0 : 2.0) * V + Vc;
         const ChebR& cr = l == 0 ? sm.cr : sm.crc;
-        NU_DISPATCH(cr.nu, (launch_down3<NU_>(L, l == 0 ? KC_DOWN0 : KC_DOWNC, bytes, H.lev[l], sm, cr, B, l == 0 ? W.m_r[ri] : W.m_rl[l],
+        NU_DISPATCH(cr.nu, (launch_down3<NU_, T_>(L, l == 0 ? KC_DOWN0 : KC_DOWNC, bytes, H.lev[l], sm, cr, B, l == 0 ? W.m_r[ri] : W.m_rl[l],
                                            f ? &W.m_q : nullptr, W.s.alpha, f ? W.r[ri ^ 1].as<double>() : nullptr,
                                            l == 0 ? W.y0.as<double>() : W.ya[l].as<double>(), W.rl[l + 1].as<double>(),
                                            H.ny[l + 1], H.nx[l + 1], H.pitch[l + 1], W.s.rr, W.s.active)));
@@ -318,7 +321,7 @@ void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Smoother& sm, int B,
     for (int l = lt - 1; l >= 0; --l) {
         const double V = (double)nact * H.ny[l] * H.nx[l] * 8.0, Vc = (double)nact * H.ny[l + 1] * H.nx[l + 1] * 8.0;
         const ChebR& cr = l == 0 ? sm.cr : sm.crc;
-        NU_DISPATCH(cr.nu, (launch_up3<NU_>(L, l == 0 ? KC_UP0 : KC_UPC, 3.0 * V + Vc, H.lev[l], sm, cr, B, l == 0 ? W.m_r[ru] : W.m_rl[l],
+        NU_DISPATCH(cr.nu, (launch_up3<NU_, T_>(L, l == 0 ? KC_UP0 : KC_UPC, 3.0 * V + Vc, H.lev[l], sm, cr, B, l == 0 ? W.m_r[ru] : W.m_rl[l],
                                          l == 0 ? W.m_y0 : W.m_ya[l], W.m_ec[l + 1],
                                          l == 0 ? W.z.as<double>() : W.zb[l].as<double>(), l == 0 ? W.s.rz : nullptr, W.s.active)));
     }

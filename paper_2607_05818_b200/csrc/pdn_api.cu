@@ -147,7 +147,8 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
     const bool iso = H.anisotropy < 1.5 && nu >= 3 && !(o.cheb_ratio > 1.0);
     const int nu_c = iso ? nu - 1 : nu;
     const double ratio_c = iso ? 2.0 * ratio : ratio;
-    const Smoother ch{make_cheb_roots(nu, ratio), make_cheb_roots(nu_c, ratio_c), G};
+    const bool f32 = (o.flags & PDN_PRECOND_F32) != 0;
+    const Smoother ch{make_cheb_roots(nu, ratio), make_cheb_roots(nu_c, ratio_c), G, f32};
     // bump / load sources deliver only their own diagonal, whose CG error is the square of the energy-norm error
     // (times the condition number of the preconditioned operator, which is why a caller who tightens rtol below
     // the default also gets tighter terminal solves: at most 1000 rtol)

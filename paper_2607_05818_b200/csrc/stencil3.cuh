@@ -37,37 +37,46 @@ constexpr int T3_EW = 64;
 constexpr int T3_ECW = 34;
 
 
-template <int R>
+// T = the type the sweeps compute in: double everywhere by default; float for the V-cycle stages of a context
+// created with PDN_PRECOND_F32 (the preconditioner only: the CG operator, residuals and solutions stay FP64).
+template <class T> struct Vec2;
+template <> struct Vec2<double> { using type = double2; };
+template <> struct Vec2<float> { using type = float2; };
+template <class T> __device__ __forceinline__ typename Vec2<T>::type mk2(T a, T b);
+template <> __device__ __forceinline__ double2 mk2<double>(double a, double b) { return make_double2(a, b); }
+template <> __device__ __forceinline__ float2 mk2<float>(float a, float b) { return make_float2(a, b); }
+
+template <int R, class T = double>
 struct Patch {  // scaled coefficients of a 2 x R patch
-    double hE0[R], hE1[R];  // east of column 0 (= west of column 1), east of column 1
-    double hW0[R];          // west of column 0
-    double hS0[R], hS1[R];  // south of row i (= north of row i+1)
-    double hN0, hN1;        // north of row 0
+    T hE0[R], hE1[R];  // east of column 0 (= west of column 1), east of column 1
+    T hW0[R];          // west of column 0
+    T hS0[R], hS1[R];  // south of row i (= north of row i+1)
+    T hN0, hN1;        // north of row 0
 };
 
-template <int W>
+template <int W, class T = double>
 struct Exch {  // rows above / below every warp's patch, double buffered; slot 0 of bot and slot W of top stay 0
-    double2 top[2][W + 1][32];
-    double2 bot[2][W + 1][32];
+    typename Vec2<T>::type top[2][W + 1][32];
+    typename Vec2<T>::type bot[2][W + 1][32];
 };
 
 __device__ __forceinline__ double2 ld2(const double* p) { return *reinterpret_cast<const double2*>(p); }
 __device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<double2*>(p) = v; }
 __device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
 
-template <int R, int W>
-__device__ __forceinline__ void exch_clear(Exch<W>& x) {
+template <int R, int W, class T>
+__device__ __forceinline__ void exch_clear(Exch<W, T>& x) {
     for (int i = threadIdx.x; i < 2 * 32; i += 32 * W) {
-        x.top[i >> 5][W][i & 31] = make_double2(0.0, 0.0);
-        x.bot[i >> 5][0][i & 31] = make_double2(0.0, 0.0);
+        x.top[i >> 5][W][i & 31] = mk2<T>(T(0), T(0));
+        x.bot[i >> 5][0][i & 31] = mk2<T>(T(0), T(0));
     }
 }
 
 // Coefficients of this thread's patch (zeros outside the mesh) and its slots of the scaling tile: two float2
 // planes, s_slot[row*32] = s of columns 0, 1 and s_slot[SD_OFF + row*32] = sd of columns 0, 1, so that a stage
 // that needs only one of the two reads 8 bytes per lane, not 16.
-template <int R>
-__device__ __forceinline__ void patch_init(Patch<R>& c, const double* __restrict__ pE, const double* __restrict__ pS,
+template <int R, class T>
+__device__ __forceinline__ void patch_init(Patch<R, T>& c, const double* __restrict__ pE, const double* __restrict__ pS,
                                            const float2* __restrict__ psc, const Level& L, int gx, int gy0,
                                            float2* s_slot, int sd_off) {
     const bool xin = gx >= 0 && gx < L.pitch;  // gx is even, pitch is even: both columns are addressable
@@ -79,9 +88,9 @@ __device__ __forceinline__ void patch_init(Patch<R>& c, const double* __restrict
         const double2 z2 = make_double2(0.0, 0.0);
         const double2 e = in ? ldg2(pE + gi) : z2;
         const double2 s = in ? ldg2(pS + gi) : z2;
-        c.hE0[i] = e.x; c.hE1[i] = e.y;
-        c.hS0[i] = s.x; c.hS1[i] = s.y;
-        c.hW0[i] = (in && gx > 0) ? __ldg(pE + gi - 1) : 0.0;
+        c.hE0[i] = (T)e.x; c.hE1[i] = (T)e.y;
+        c.hS0[i] = (T)s.x; c.hS1[i] = (T)s.y;
+        c.hW0[i] = (T)((in && gx > 0) ? __ldg(pE + gi - 1) : 0.0);
         if (psc) {
             const float4 v = in ? __ldg(reinterpret_cast<const float4*>(psc + gi)) : make_float4(0.f, 0.f, 0.f, 0.f);
             s_slot[i * 32] = make_float2(v.x, v.z);
@@ -90,26 +99,27 @@ __device__ __forceinline__ void patch_init(Patch<R>& c, const double* __restrict
     }
     const int gyn = gy0 - 1;
     const double2 nn = (xin && gyn >= 0 && gyn < L.ny) ? ldg2(pS + (size_t)gyn * L.pitch + gx) : make_double2(0.0, 0.0);
-    c.hN0 = nn.x; c.hN1 = nn.y;
+    c.hN0 = (T)nn.x; c.hN1 = (T)nn.y;
 }
 
 // Split-phase exchange of patch boundary rows between the warps of a block.  `publish` stores the
 // patch's first and last row and ARRIVES on an mbarrier; the rows that need nothing from other warps
 // are computed next; `collect` waits for everybody's arrival and fetches the rows just above / below.
 // Buffers alternate between sweeps, the mbarrier phase flips once per sweep.
-template <int W>
+template <int W, class T = double>
 struct Xchg {
-    Exch<W>* x;
+    using T2 = typename Vec2<T>::type;
+    Exch<W, T>* x;
     uint64_t* bar;
     int cur;        // buffer of the current sweep
     uint32_t phase; // parity the next collect waits for
     int warp, lane;
-    __device__ __forceinline__ void publish(double a0, double a1, double b0, double b1) {
-        x->top[cur][warp][lane] = make_double2(a0, a1);
-        x->bot[cur][warp + 1][lane] = make_double2(b0, b1);
+    __device__ __forceinline__ void publish(T a0, T a1, T b0, T b1) {
+        x->top[cur][warp][lane] = mk2<T>(a0, a1);
+        x->bot[cur][warp + 1][lane] = mk2<T>(b0, b1);
         mbar_arrive(bar);
     }
-    __device__ __forceinline__ void collect(double2& up, double2& dn) {
+    __device__ __forceinline__ void collect(T2& up, T2& dn) {
         mbar_wait(bar, phase);
         up = x->bot[cur][warp][lane];
         dn = x->top[cur][warp + 1][lane];
@@ -120,17 +130,17 @@ struct Xchg {
 
 // t = add + sum over the four neighbours of h_nb * y_nb for row i of the patch, whose own values are
 // (c0, c1), with the rows above (u0, u1) and below (d0, d1) given explicitly.
-template <int R>
-__device__ __forceinline__ void row_sum(const Patch<R>& c, int i, double c0, double c1, double u0, double u1,
-                                        double d0, double d1, double add0, double add1, double& t0, double& t1) {
-    const double yl = __shfl_up_sync(FULL, c1, 1);    // right column of the lane to the left
-    const double yr = __shfl_down_sync(FULL, c0, 1);  // left column of the lane to the right
-    const double n0 = i == 0 ? c.hN0 : c.hS0[i == 0 ? 0 : i - 1], n1 = i == 0 ? c.hN1 : c.hS1[i == 0 ? 0 : i - 1];
-    double a = fma(c.hE0[i], c1, add0);
+template <int R, class T>
+__device__ __forceinline__ void row_sum(const Patch<R, T>& c, int i, T c0, T c1, T u0, T u1,
+                                        T d0, T d1, T add0, T add1, T& t0, T& t1) {
+    const T yl = __shfl_up_sync(FULL, c1, 1);    // right column of the lane to the left
+    const T yr = __shfl_down_sync(FULL, c0, 1);  // left column of the lane to the right
+    const T n0 = i == 0 ? c.hN0 : c.hS0[i == 0 ? 0 : i - 1], n1 = i == 0 ? c.hN1 : c.hS1[i == 0 ? 0 : i - 1];
+    T a = fma(c.hE0[i], c1, add0);
     a = fma(c.hW0[i], yl, a);
     a = fma(c.hS0[i], d0, a);
     t0 = fma(n0, u0, a);
-    double b = fma(c.hE1[i], yr, add1);
+    T b = fma(c.hE1[i], yr, add1);
     b = fma(c.hE0[i], c0, b);
     b = fma(c.hS1[i], d1, b);
     t1 = fma(n1, u1, b);
@@ -139,30 +149,30 @@ __device__ __forceinline__ void row_sum(const Patch<R>& c, int i, double c0, dou
 // One Richardson step  y <- (1-w) y + w (r^ + N y)  on the patch, in place.  Rows 1..R-2 need only this
 // thread's (and, by shuffle, this warp's) values: they are updated between publish and collect, top to
 // bottom, the old value of the row above carried in registers; rows 0 and R-1 follow the collect.
-template <int R, int W>
-__device__ __forceinline__ void smooth_step(Xchg<W>& xc, const Patch<R>& c, double (&y0)[R], double (&y1)[R],
-                                            const double (&rh0)[R], const double (&rh1)[R], double w) {
+template <int R, int W, class T>
+__device__ __forceinline__ void smooth_step(Xchg<W, T>& xc, const Patch<R, T>& c, T (&y0)[R], T (&y1)[R],
+                                            const T (&rh0)[R], const T (&rh1)[R], T w) {
     static_assert(R >= 2, "patch needs two rows");
     xc.publish(y0[0], y1[0], y0[R - 1], y1[R - 1]);
-    const double a = 1.0 - w;
-    const double f0 = y0[0], f1 = y1[0];          // old first row
-    const double s0 = y0[R > 2 ? 1 : 0], s1 = y1[R > 2 ? 1 : 0];  // old second row (below neighbour of row 0)
-    const double l0 = y0[R - 1], l1 = y1[R - 1];  // old last row
-    double pu0 = f0, pu1 = f1;
+    const T a = T(1) - w;
+    const T f0 = y0[0], f1 = y1[0];          // old first row
+    const T s0 = y0[R > 2 ? 1 : 0], s1 = y1[R > 2 ? 1 : 0];  // old second row (below neighbour of row 0)
+    const T l0 = y0[R - 1], l1 = y1[R - 1];  // old last row
+    T pu0 = f0, pu1 = f1;
 #pragma unroll
     for (int i = 1; i < R - 1; ++i) {
-        double t0, t1;
-        row_sum<R>(c, i, y0[i], y1[i], pu0, pu1, y0[i + 1], y1[i + 1], rh0[i], rh1[i], t0, t1);
+        T t0, t1;
+        row_sum<R, T>(c, i, y0[i], y1[i], pu0, pu1, y0[i + 1], y1[i + 1], rh0[i], rh1[i], t0, t1);
         pu0 = y0[i]; pu1 = y1[i];
         y0[i] = fma(w, t0, a * y0[i]);
         y1[i] = fma(w, t1, a * y1[i]);
     }
     // pu = old row R-2 (or the old first row if R == 2)
-    double2 up, dn;
+    typename Vec2<T>::type up, dn;
     xc.collect(up, dn);
-    double t0, t1, v0, v1;
-    row_sum<R>(c, 0, f0, f1, up.x, up.y, R > 2 ? s0 : l0, R > 2 ? s1 : l1, rh0[0], rh1[0], t0, t1);
-    row_sum<R>(c, R - 1, l0, l1, pu0, pu1, dn.x, dn.y, rh0[R - 1], rh1[R - 1], v0, v1);
+    T t0, t1, v0, v1;
+    row_sum<R, T>(c, 0, f0, f1, up.x, up.y, R > 2 ? s0 : l0, R > 2 ? s1 : l1, rh0[0], rh1[0], t0, t1);
+    row_sum<R, T>(c, R - 1, l0, l1, pu0, pu1, dn.x, dn.y, rh0[R - 1], rh1[R - 1], v0, v1);
     y0[0] = fma(w, t0, a * f0);
     y1[0] = fma(w, t1, a * f1);
     y0[R - 1] = fma(w, v0, a * l0);
@@ -170,18 +180,18 @@ __device__ __forceinline__ void smooth_step(Xchg<W>& xc, const Patch<R>& c, doub
 }
 
 // t = add + N y for every row of the patch (y unchanged): the residual / operator-apply variant.
-template <int R, int W>
-__device__ __forceinline__ void apply_step(Xchg<W>& xc, const Patch<R>& c, const double (&y0)[R], const double (&y1)[R],
-                                           const double (&a0)[R], const double (&a1)[R], double (&t0)[R],
-                                           double (&t1)[R]) {
+template <int R, int W, class T>
+__device__ __forceinline__ void apply_step(Xchg<W, T>& xc, const Patch<R, T>& c, const T (&y0)[R], const T (&y1)[R],
+                                           const T (&a0)[R], const T (&a1)[R], T (&t0)[R],
+                                           T (&t1)[R]) {
     xc.publish(y0[0], y1[0], y0[R - 1], y1[R - 1]);
 #pragma unroll
     for (int i = 1; i < R - 1; ++i)
-        row_sum<R>(c, i, y0[i], y1[i], y0[i - 1], y1[i - 1], y0[i + 1], y1[i + 1], a0[i], a1[i], t0[i], t1[i]);
-    double2 up, dn;
+        row_sum<R, T>(c, i, y0[i], y1[i], y0[i - 1], y1[i - 1], y0[i + 1], y1[i + 1], a0[i], a1[i], t0[i], t1[i]);
+    typename Vec2<T>::type up, dn;
     xc.collect(up, dn);
-    row_sum<R>(c, 0, y0[0], y1[0], up.x, up.y, y0[1], y1[1], a0[0], a1[0], t0[0], t1[0]);
-    row_sum<R>(c, R - 1, y0[R - 1], y1[R - 1], y0[R - 2], y1[R - 2], dn.x, dn.y, a0[R - 1], a1[R - 1], t0[R - 1], t1[R - 1]);
+    row_sum<R, T>(c, 0, y0[0], y1[0], up.x, up.y, y0[1], y1[1], a0[0], a1[0], t0[0], t1[0]);
+    row_sum<R, T>(c, R - 1, y0[R - 1], y1[R - 1], y0[R - 2], y1[R - 2], dn.x, dn.y, a0[R - 1], a1[R - 1], t0[R - 1], t1[R - 1]);
 }
 
 template <int R, int W, int H>
@@ -254,7 +264,7 @@ __device__ __forceinline__ unsigned interior_mask(const Level& L, int lane, int 
 //   [r = r_in - alpha q ; rr += r.r]   y = S_nu(0, r^)   rc = R sd (r^ - A^ y)
 // y (the scaled iterate) is written to y_out for the up stage; R sums 2x2 aggregates.
 // grid = (tiles_x, tiles_y, ceil(B / G)); the block loops over G right-hand sides, two TMA stages.
-template <int R, int W, int NU, bool FUSED>
+template <int R, int W, int NU, bool FUSED, class T = double>
 __global__ void __launch_bounds__(32 * W, 1)
 k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensorMap tm_q, Level L, ChebR ch,
         const double* __restrict__ alpha, double* __restrict__ r_out, double* __restrict__ y_out,
@@ -266,7 +276,7 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
     double* qbuf = rbuf + 2 * Gm::TILE;                        // 2 stages (FUSED only)
     float2* sc = reinterpret_cast<float2*>(qbuf + (FUSED ? 2 * Gm::TILE : 0));
     constexpr int SD_OFF = Gm::EH * 32;
-    Exch<W>& x = *reinterpret_cast<Exch<W>*>(sc + 2 * SD_OFF);
+    Exch<W, T>& x = *reinterpret_cast<Exch<W, T>*>(sc + 2 * SD_OFF);
     __shared__ uint64_t mbar[3];  // two TMA stages + the row-exchange barrier
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -274,9 +284,9 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
     const int gx = x0 + 2 * lane, gy0 = y0 + R * warp;
     const int slot0 = (R * warp) * T3_EW + 2 * lane;
     float2* sc_slot = sc + (R * warp) * 32 + lane;
-    Patch<R> c;
-    patch_init<R>(c, L.hE, L.hS, L.sc, L, gx, gy0, sc_slot, SD_OFF);
-    exch_clear<R, W>(x);
+    Patch<R, T> c;
+    patch_init<R, T>(c, L.hE, L.hS, L.sc, L, gx, gy0, sc_slot, SD_OFF);
+    exch_clear<R, W, T>(x);
     const unsigned interior = interior_mask<R, H, Gm::IW, Gm::IH>(L, lane, warp, gx, gy0);
     const size_t plane = (size_t)L.ny * L.pitch, cplane = (size_t)cny * cpitch;
     const size_t goff = (size_t)gy0 * L.pitch + gx;
@@ -298,14 +308,15 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
         fetch(0);
         if (nb > 1) fetch(1);
     }
-    Xchg<W> xc{&x, &mbar[2], 0, 0u, warp, lane};
+    Xchg<W, T> xc{&x, &mbar[2], 0, 0u, warp, lane};
     for (int j = 0; j < nb; ++j) {
         const int b = al.b[j], st = j & 1;
         PHASE_CLK(j, 0);
         mbar_wait(&mbar[st], (j >> 1) & 1);
         PHASE_CLK(j, 1);
         const double alj = FUSED ? al.s[j] : 0.0;
-        double y0r[R], y1r[R], rh0[R], rh1[R], rr = 0.0;
+        T y0r[R], y1r[R], rh0[R], rh1[R];
+        double rr = 0.0;
 #pragma unroll
         for (int i = 0; i < R; ++i) {
             double2 r = ld2(rbuf + st * Gm::TILE + slot0 + i * T3_EW);
@@ -320,10 +331,10 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
                 rr = fma(my, my, rr);
             }
             const float2 s2 = sc_slot[i * 32];
-            rh0[i] = (double)s2.x * r.x;
-            rh1[i] = (double)s2.y * r.y;
-            y0r[i] = ch.w[0] * rh0[i];
-            y1r[i] = ch.w[0] * rh1[i];
+            rh0[i] = (T)s2.x * (T)r.x;
+            rh1[i] = (T)s2.y * (T)r.y;
+            y0r[i] = (T)ch.w[0] * rh0[i];
+            y1r[i] = (T)ch.w[0] * rh1[i];
         }
         if (FUSED) {  // ||r||^2: the shuffle chain overlaps the sweeps that follow
             rr = warp_sum(rr);
@@ -334,27 +345,27 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
         // i.e. has consumed the stage: thread 0 may refill it with right-hand side j+2
 #pragma unroll
         for (int k = 1; k < NU; ++k) {
-            smooth_step<R, W>(xc, c, y0r, y1r, rh0, rh1, ch.w[k]);
+            smooth_step<R, W, T>(xc, c, y0r, y1r, rh0, rh1, (T)ch.w[k]);
             if (k == 1 && threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
         }
         PHASE_CLK(j, 3);
-        double t0[R], t1[R];
-        apply_step<R, W>(xc, c, y0r, y1r, rh0, rh1, t0, t1);
+        T t0[R], t1[R];
+        apply_step<R, W, T>(xc, c, y0r, y1r, rh0, rh1, t0, t1);
         PHASE_CLK(j, 4);
         if (NU == 1 && threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
         // residual of the unscaled system at the patch nodes, summed over 2x2 aggregates
 #pragma unroll
         for (int i = 0; i < R; i += 2) {
             const float2 sa = sc_slot[SD_OFF + i * 32], sb = sc_slot[SD_OFF + (i + 1) * 32];
-            double v = (double)sa.x * (t0[i] - y0r[i]);
-            v = fma((double)sa.y, t1[i] - y1r[i], v);
-            v = fma((double)sb.x, t0[i + 1] - y0r[i + 1], v);
-            v = fma((double)sb.y, t1[i + 1] - y1r[i + 1], v);
+            T v = (T)sa.x * (t0[i] - y0r[i]);
+            v = fma((T)sa.y, t1[i] - y1r[i], v);
+            v = fma((T)sb.x, t0[i + 1] - y0r[i + 1], v);
+            v = fma((T)sb.y, t1[i + 1] - y1r[i + 1], v);
             if ((interior >> i) & 1) {  // rows i and i+1 are interior together (H, R, y0 even)
-                st2(y_out + b * plane + goff + (size_t)i * L.pitch, make_double2(y0r[i], y1r[i]));
+                st2(y_out + b * plane + goff + (size_t)i * L.pitch, make_double2((double)y0r[i], (double)y1r[i]));
                 if ((interior >> (i + 1)) & 1)
-                    st2(y_out + b * plane + goff + (size_t)(i + 1) * L.pitch, make_double2(y0r[i + 1], y1r[i + 1]));
-                rc[b * cplane + (size_t)((gy0 + i) >> 1) * cpitch + (gx >> 1)] = v;
+                    st2(y_out + b * plane + goff + (size_t)(i + 1) * L.pitch, make_double2((double)y0r[i + 1], (double)y1r[i + 1]));
+                rc[b * cplane + (size_t)((gy0 + i) >> 1) * cpitch + (gx >> 1)] = (double)v;
             }
         }
         PHASE_CLK(j, 5);
@@ -364,7 +375,7 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
 // ---------------------------------------------------------------------------------------------
 // Up stage:  y = y_in + sd P e_c ;  y = S_nu(y, r^) ;  z = s y ;  [rz += r.z]
 // P = piecewise-constant prolongation (fine (y,x) takes coarse (y/2, x/2)).
-template <int R, int W, int NU, bool DOT>
+template <int R, int W, int NU, bool DOT, class T = double>
 __global__ void __launch_bounds__(32 * W, 1)
 k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensorMap tm_y,
       const __grid_constant__ CUtensorMap tm_e, Level L, ChebR ch, double* __restrict__ z_out,
@@ -377,7 +388,7 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
     double* ebuf = ybuf + 2 * Gm::TILE;  // T3_ECW x EH/2 per stage
     float2* sc = reinterpret_cast<float2*>(ebuf + 2 * Gm::ETILE);
     constexpr int SD_OFF = Gm::EH * 32;
-    Exch<W>& x = *reinterpret_cast<Exch<W>*>(sc + 2 * SD_OFF);
+    Exch<W, T>& x = *reinterpret_cast<Exch<W, T>*>(sc + 2 * SD_OFF);
     __shared__ uint64_t mbar[3];  // two TMA stages + the row-exchange barrier
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -385,9 +396,9 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
     const int gx = x0 + 2 * lane, gy0 = y0 + R * warp;
     const int slot0 = (R * warp) * T3_EW + 2 * lane;
     float2* sc_slot = sc + (R * warp) * 32 + lane;
-    Patch<R> c;
-    patch_init<R>(c, L.hE, L.hS, L.sc, L, gx, gy0, sc_slot, SD_OFF);
-    exch_clear<R, W>(x);
+    Patch<R, T> c;
+    patch_init<R, T>(c, L.hE, L.hS, L.sc, L, gx, gy0, sc_slot, SD_OFF);
+    exch_clear<R, W, T>(x);
     const unsigned interior = interior_mask<R, H, Gm::IW, Gm::IH>(L, lane, warp, gx, gy0);
     const size_t plane = (size_t)L.ny * L.pitch;
     const size_t goff = (size_t)gy0 * L.pitch + gx;
@@ -412,26 +423,26 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
         fetch(0);
         if (nb > 1) fetch(1);
     }
-    Xchg<W> xc{&x, &mbar[2], 0, 0u, warp, lane};
+    Xchg<W, T> xc{&x, &mbar[2], 0, 0u, warp, lane};
     double rz_pend = 0.0;  // r.z partial of the previous right-hand side: reduced while the next one sweeps
     int b_pend = -1;
     for (int j = 0; j < nb; ++j) {
         const int b = al.b[j], st = j & 1;
         mbar_wait(&mbar[st], (j >> 1) & 1);
-        double y0r[R], y1r[R], rh0[R], rh1[R];
-        double ec[R / 2];  // one coarse correction per pair of rows (R and H are even: rows 2k, 2k+1 share a coarse row)
+        T y0r[R], y1r[R], rh0[R], rh1[R];
+        T ec[R / 2];  // one coarse correction per pair of rows (R and H are even: rows 2k, 2k+1 share a coarse row)
 #pragma unroll
-        for (int k = 0; k < R / 2; ++k) ec[k] = ebuf[st * Gm::ETILE + ((R * warp) / 2 + k) * T3_ECW + eslot];
+        for (int k = 0; k < R / 2; ++k) ec[k] = (T)ebuf[st * Gm::ETILE + ((R * warp) / 2 + k) * T3_ECW + eslot];
 #pragma unroll
         for (int i = 0; i < R; ++i) {
             const double2 r = ld2(rbuf + st * Gm::TILE + slot0 + i * T3_EW);
             const double2 yin = ld2(ybuf + st * Gm::TILE + slot0 + i * T3_EW);
-            const double e = ec[i >> 1];
+            const T e = ec[i >> 1];
             const float2 s2 = sc_slot[i * 32], d2 = sc_slot[SD_OFF + i * 32];
-            rh0[i] = (double)s2.x * r.x;
-            rh1[i] = (double)s2.y * r.y;
-            y0r[i] = fma((double)d2.x, e, yin.x);
-            y1r[i] = fma((double)d2.y, e, yin.y);
+            rh0[i] = (T)s2.x * (T)r.x;
+            rh1[i] = (T)s2.y * (T)r.y;
+            y0r[i] = fma((T)d2.x, e, (T)yin.x);
+            y1r[i] = fma((T)d2.y, e, (T)yin.y);
         }
         if (DOT && b_pend >= 0) {
             rz_pend = warp_sum(rz_pend);
@@ -439,7 +450,7 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
         }
 #pragma unroll
         for (int k = 0; k < NU; ++k) {
-            smooth_step<R, W>(xc, c, y0r, y1r, rh0, rh1, ch.w[NU - 1 - k]);
+            smooth_step<R, W, T>(xc, c, y0r, y1r, rh0, rh1, (T)ch.w[NU - 1 - k]);
             if (k == 0 && threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
         }
         double rz = 0.0;
@@ -448,10 +459,10 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
             const bool in = (interior >> i) & 1;
             const float2 s2 = sc_slot[i * 32];
             if (in) st2(z_out + b * plane + goff + (size_t)i * L.pitch,
-                        make_double2((double)s2.x * y0r[i], (double)s2.y * y1r[i]));
+                        make_double2((double)((T)s2.x * y0r[i]), (double)((T)s2.y * y1r[i])));
             if (DOT) {  // r.z = r.(s y) = (s r).y = r^.y
-                rz = fma(in ? rh0[i] : 0.0, y0r[i], rz);
-                rz = fma(in ? rh1[i] : 0.0, y1r[i], rz);
+                rz = fma(in ? (double)rh0[i] : 0.0, (double)y0r[i], rz);
+                rz = fma(in ? (double)rh1[i] : 0.0, (double)y1r[i], rz);
             }
         }
         rz_pend = rz;
@@ -486,7 +497,7 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
     const int gx = x0 + 2 * lane, gy0 = y0 + R * warp;
     const int slot0 = (R * warp) * T3_EW + 2 * lane;
     Patch<R> c;
-    patch_init<R>(c, L.gx, L.gy, nullptr, L, gx, gy0, nullptr, 0);
+    patch_init<R, double>(c, L.gx, L.gy, nullptr, L, gx, gy0, nullptr, 0);
     const double zero[R] = {};
     double d0[R], d1[R];  // diagonal = sum of the incident conductances
 #pragma unroll
@@ -495,7 +506,7 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
         d0[i] = (c.hE0[i] + c.hW0[i]) + (c.hS0[i] + n0);
         d1[i] = (c.hE1[i] + c.hE0[i]) + (c.hS1[i] + n1);
     }
-    exch_clear<R, W>(x);
+    exch_clear<R, W, double>(x);
     const unsigned interior = interior_mask<R, H, Gm::IW, Gm::IH>(L, lane, warp, gx, gy0);
     const size_t plane = (size_t)L.ny * L.pitch;
     const size_t goff = (size_t)gy0 * L.pitch + gx;
@@ -549,7 +560,7 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
         }
         if (b_pend >= 0) flush();
         double t0[R], t1[R];
-        apply_step<R, W>(xc, c, p0, p1, zero, zero, t0, t1);
+        apply_step<R, W, double>(xc, c, p0, p1, zero, zero, t0, t1);
         if (threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
 #pragma unroll
         for (int i = 0; i < R; ++i) {

@@ -61,6 +61,31 @@ def test_workload_full_cross_product(cfg):
     print(f"cfg{cfg}: max {rel.max():.2e} mean {rel.mean():.2e} iters {st['pcg_iters_max']}")
 
 
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
+def test_precond_f32_meets_the_same_tolerance(cfg):
+    """Opt-in PDN_PRECOND_F32 (multigrid sweeps in FP32 registers; CG operator, residuals, solutions FP64):
+    same tolerance against the oracle, at most two PCG iterations more than the FP64 preconditioner, and it
+    agrees with the default path far inside the tolerance."""
+    from paper_2607_05818_b200 import PDN_PRECOND_F32
+    bi, li, want = load_golden(cfg)
+    net = P.make_config(cfg, seed=0)
+    got32, st32 = gpu_all_pairs(net, flags=PDN_PRECOND_F32)
+    rel = check(got32[bi, li], want)
+    got64, st64 = gpu_all_pairs(net)
+    assert st32["pcg_iters_max"] <= st64["pcg_iters_max"] + 2
+    assert np.abs(got32 - got64).max() / got64.min() <= 1e-7
+    print(f"cfg{cfg} f32 preconditioner: max {rel.max():.2e} mean {rel.mean():.2e} iters {st32['pcg_iters_max']} (f64: {st64['pcg_iters_max']})")
+
+
+@pytest.mark.parametrize("seed,aniso", [(3, 1.0), (4, 3.0), (5, 40.0)])
+def test_precond_f32_random_stacks_against_live_oracle(seed, aniso):
+    from oracle.reff_oracle import Oracle
+    from paper_2607_05818_b200 import PDN_PRECOND_F32
+    net = P.make_random(seed, d=3, n=150, p=12, m=5, nl=7, drop=0.01, aniso=aniso)
+    got, _ = gpu_all_pairs(net, flags=PDN_PRECOND_F32, rtol=1e-10)
+    check(got, Oracle(net).reff_all())
+
+
 @pytest.mark.parametrize("cfg", [3, 4, 5])
 def test_workload_sampled_pairs(cfg):
     """Full-size workloads in the launch configuration bench.py times; pair-list mode of pdn_reff."""
