@@ -204,7 +204,7 @@ void launch_down3(Launcher& L, int cls, double bytes, const Level& lv, const Smo
     constexpr int H = halo_of(NU), IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
     const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
     dim3 grid(tx, ty, cdiv(B, G));
-    constexpr size_t base = 2 * T3_TILE_BYTES + T3_SC_BYTES + sizeof(Exch<DN_W>);
+    constexpr size_t base = 2 * T3_TILE_BYTES + T3_SC_BYTES + sizeof(Exch<DN_W, T>);
     static std::atomic<uint64_t> attr_done{0};
     once_per_device(attr_done, [&] {
         CK(cudaFuncSetAttribute(k_down3<DN_R, DN_W, NU, true, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(base + 2 * T3_TILE_BYTES)));
@@ -220,7 +220,7 @@ void launch_up3(Launcher& L, int cls, double bytes, const Level& lv, const Smoot
     constexpr int H = halo_of(NU), IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
     const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
     dim3 grid(tx, ty, cdiv(B, G));
-    constexpr size_t smem = 4 * T3_TILE_BYTES + (size_t)2 * Geom<T3_R, T3_W, 2>::ETILE_BYTES + T3_SC_BYTES + sizeof(Exch<T3_W>);
+    constexpr size_t smem = 4 * T3_TILE_BYTES + (size_t)2 * Geom<T3_R, T3_W, 2>::ETILE_BYTES + T3_SC_BYTES + sizeof(Exch<T3_W, T>);
     static std::atomic<uint64_t> attr_done{0};
     once_per_device(attr_done, [&] {
         CK(cudaFuncSetAttribute(k_up3<T3_R, T3_W, NU, true, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
