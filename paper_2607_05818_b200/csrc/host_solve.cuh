@@ -190,11 +190,26 @@ struct Work {
     }
 };
 
-// right-hand sides per block: as many as G allows while the grid still fills the GPU a few times over
+// Right-hand sides per block.  One block is resident per SM, so a launch of tiles * ceil(B / g) blocks runs in
+// ceil(blocks / SMs) waves, each as long as g right-hand sides plus the block's set-up (its coefficients: about
+// two right-hand sides' worth of loads).  Take the g <= G with the shortest launch by that count -- a grid just
+// over a multiple of the SM count (640 blocks at 512^2 with B = 256, g = 32) idles most SMs for a whole wave.
 inline int rhs_per_block(int tiles, int B, int G) {
-    const long blocks_wanted = 148L * 4;
-    long g = ((long)tiles * B) / blocks_wanted;
-    return (int)std::max(1L, std::min<long>(std::min(G, T3_MAX_G), g));
+    static const int sms = [] {
+        int dev = 0, n = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+        return n;
+    }();
+    constexpr double setup = 2.0;  // measured flat between 1 and 8 (configs 3, 4)
+    const int gmax = std::max(1, std::min(G, T3_MAX_G));
+    int best = 1;
+    double best_cost = 1e300;
+    for (int g = 1; g <= gmax; ++g) {
+        const long blocks = (long)tiles * cdiv(B, g);
+        const double cost = (double)((blocks + sms - 1) / sms) * (g + setup);
+        if (cost < best_cost) { best_cost = cost; best = g; }
+    }
+    return best;
 }
 
 template <int NU, class T>
