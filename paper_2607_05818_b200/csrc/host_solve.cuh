@@ -194,14 +194,14 @@ struct Work {
 // ceil(blocks / SMs) waves, each as long as g right-hand sides plus the block's set-up (its coefficients: about
 // two right-hand sides' worth of loads).  Take the g <= G with the shortest launch by that count -- a grid just
 // over a multiple of the SM count (640 blocks at 512^2 with B = 256, g = 32) idles most SMs for a whole wave.
-inline int rhs_per_block(int tiles, int B, int G) {
+inline int rhs_per_block(int tiles, int B, int G, int cap = T3_MAX_G) {
     static const int sms = [] {
         int dev = 0, n = 0;
         if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
         return n;
     }();
     constexpr double setup = 2.0;  // measured flat between 1 and 8 (configs 3, 4)
-    const int gmax = std::max(1, std::min(G, T3_MAX_G));
+    const int gmax = std::max(1, std::min(G, cap));
     int best = 1;
     double best_cost = 1e300;
     for (int g = 1; g <= gmax; ++g) {
@@ -249,7 +249,7 @@ void launch_pq3(Launcher& L, double bytes, const Level& lv, const Smoother& sm, 
                 const CUtensorMap& m_p, const double* beta, double* p_new, double* q, double* pq_acc, double* sump_acc,
                 const int* active) {
     constexpr int H = 2, IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
-    const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
+    const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G, T3_MAX_G_PQ);
     dim3 grid(tx, ty, cdiv(B, G));
     constexpr size_t smem = 4 * T3_TILE_BYTES + sizeof(Exch<PQ_W>);
     static std::atomic<uint64_t> attr_done{0};

@@ -141,7 +141,7 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
     const bool strong = H.anisotropy >= 6.0;
     const int nu = (strong && c->nu_auto) ? 6 : o.nu;
     const double ratio = o.cheb_ratio > 1.0 ? o.cheb_ratio : strong ? 2.0 * (1.0 + H.anisotropy) : 3.0 + H.anisotropy;
-    const int G = getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 32;
+    const int G = getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 64;
     // On near-isotropic tiers the coarse levels get by with one step less on a wider interval (measured: same
     // iteration counts at configs 3 and 5, one level-visit cheaper); anisotropic tiers keep nu steps everywhere.
     const bool iso = H.anisotropy < 1.5 && nu >= 3 && !(o.cheb_ratio > 1.0);
