@@ -305,7 +305,7 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
         tma_load_3d(rbuf + st * Gm::TILE, &tm_r, x0, y0, al.b[j], &mbar[st]);
         if (FUSED) tma_load_3d(qbuf + st * Gm::TILE, &tm_q, x0, y0, al.b[j], &mbar[st]);
     };
-    if (threadIdx.x == 0) {
+    if (threadIdx.x == 0 && nb > 0) {  // nb == 0: every right-hand side of the group has converged
         fetch(0);
         if (nb > 1) fetch(1);
     }
@@ -420,7 +420,7 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
         tma_load_3d(ybuf + st * Gm::TILE, &tm_y, x0, y0, al.b[j], &mbar[st]);
         tma_load_3d(ebuf + st * Gm::ETILE, &tm_e, cx0, y0 / 2, al.b[j], &mbar[st]);
     };
-    if (threadIdx.x == 0) {
+    if (threadIdx.x == 0 && nb > 0) {  // nb == 0: every right-hand side of the group has converged
         fetch(0);
         if (nb > 1) fetch(1);
     }
@@ -525,7 +525,7 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
         tma_load_3d(zbuf + st * Gm::TILE, &tm_z, x0, y0, al.b[j], &mbar[st]);
         tma_load_3d(pbuf + st * Gm::TILE, &tm_p, x0, y0, al.b[j], &mbar[st]);
     };
-    if (threadIdx.x == 0) {
+    if (threadIdx.x == 0 && nb > 0) {  // nb == 0: every right-hand side of the group has converged
         fetch(0);
         if (nb > 1) fetch(1);
     }
