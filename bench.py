@@ -9,9 +9,10 @@ HBM and the result left on the device; `e2e` times the same through the host-buf
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl reference]
 
-Default workload: configs[3] (4 tiers x 1024^2, 1,048,576 pairs) -- the largest workload whose oracle
-sample (one sparse LU of the whole 3D system, ~100 s on one core, plus a few pairs) still lets the default
-run end within a few minutes; configs[4] (8 x 1024^2, LU ~270 s) is `--config 5`.
+Default workload: configs[4] (8 tiers x 1024^2, 4,194,304 pairs) -- BASELINE.json's `metric` names no config,
+so the headline is the largest single-GPU one.  Its oracle sample costs one sparse LU of the whole 3D system
+(~4-5 min on one core, ~19 GB) plus a few pairs; `--config 4` (configs[3], LU ~1 min) and the others are
+measured the same way and recorded under profiles/.
 
 N > 1 (torchrun): every rank runs its own independent network of the same workload (seed = rank): the
 path has no cross-problem exchange, so this is weak scaling without a collective (multi-GPU).
@@ -258,13 +259,14 @@ def run_cuda(a):
     tot_by = sum(cls_by[k] for k in stencil_classes)
     phase = tot_by / (tot_ms * 1e-3) / 1e9 if tot_ms > 0 else 0.0
     # DRAM traffic of the dominant kernel from the committed ncu capture (profiles/ncu_traffic.csv: bytes per
-    # right-hand side of one launch), scaled to this run's average right-hand sides per launch
+    # right-hand side of one launch on a mesh of the same size), scaled to this run's average right-hand sides per
+    # launch -- NOT measured in this run (a run under ncu is never a bench value): `traffic_source` says so
     traffic = None
     tr_path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     if os.path.exists(tr_path) and cls_n[dom] > 0:
         import csv
         for row in csv.DictReader(open(tr_path)):
-            if int(row["cfg"]) == cfg and row["class"] == dom:
+            if int(row["n"]) == net.n and row["class"] == dom:
                 per_rhs_alg = float(row["algorithmic_bytes_per_launch"]) / float(row["rhs_in_launch"])
                 rhs_per_launch = (cls_by[dom] / cls_n[dom]) / per_rhs_alg
                 traffic = float(row["dram_bytes_per_rhs"]) * rhs_per_launch
@@ -298,7 +300,10 @@ def run_cuda(a):
         "parity": parity,
         "clocks": clocks,
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
-                     "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
+                     "frac": ach / peak, "traffic": traffic,
+                     "traffic_source": "ncu capture (profiles/ncu_traffic.csv), scaled by right-hand sides per launch; "
+                                       "not measured in this run" if traffic is not None else None,
+                     "peak_source": peak_src,
                      "launches": int(cls_n[dom]), "avg_launch_ms": cls_ms[dom] / max(cls_n[dom], 1),
                      "alg_bytes_per_launch": cls_by[dom] / max(cls_n[dom], 1),
                      "timing": "CUDA events around every launch on the launching stream, in a repeat of the same "
@@ -437,7 +442,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--rtol", type=float, default=0.0)
     ap.add_argument("--nu", type=int, default=0)
