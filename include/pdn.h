@@ -171,9 +171,18 @@ int pdn_reff_host(pdn_ctx *ctx, int64_t n_pairs, const int32_t *bump_idx, const 
  * the given list (HOST array, same rules as in pdn_create) and brings ctx up to date for pdn_reff.  The list is
  * diffed against the current one per interface by site: kept sites cost nothing (their resistance may change),
  * removed sites cost nothing, every added site costs one port solve on each of its two tiers; the port-level
- * system is then re-assembled and re-factored.  If the call fails (PDN_E_ARG leaves ctx untouched; any other
- * status may leave it half updated) the context must be destroyed. */
+ * system is then re-assembled and re-factored.  The update is staged: if a port solve fails (PDN_E_NOCONV,
+ * PDN_E_NOMEM, PDN_E_CUDA, PDN_E_NUMERIC from a solve) or the list is malformed (PDN_E_ARG), ctx is left exactly as it
+ * was and still answers for the OLD plan.  Only a failure of the final re-factorisation (PDN_E_NUMERIC from S3, or a
+ * CUDA / allocation error inside it) leaves no valid factor: ctx is then marked unusable, every later call on it
+ * returns PDN_E_ARG, and it must be destroyed. */
 int pdn_update_tsvs(pdn_ctx *ctx, int32_t n_tsv, const pdn_tsv *tsvs);
+
+/* Changes the stopping rule of the port solves that later calls on ctx run (pdn_update_tsvs, pdn_reff_nodes): the
+ * relative residual rtol and the iteration cap max_iter of pdn_opts; a value <= 0 keeps the current one.  Design-
+ * space sweeps may re-plan at a looser tolerance than the sign-off run.  Nothing already
+ * computed changes. */
+int pdn_set_solver_opts(pdn_ctx *ctx, double rtol, int32_t max_iter);
 
 /* Same-side pairs (context created with PDN_TERMINAL_PAIRS).  side 0: bumps, side 1: loads.  out: DEVICE fp64,
  * nt*nt values (nt = n_bumps or n_loads), out[i*nt + j] = R_eff between terminals i and j of that side in the

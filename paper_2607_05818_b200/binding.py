@@ -56,7 +56,7 @@ class PdnStats(C.Structure):
 EXPORTS = ("pdn_create", "pdn_reff", "pdn_reff_host", "pdn_destroy", "pdn_strerror", "pdn_last_error",
            "pdn_get_stats", "pdn_port_count", "pdn_get_port_matrix", "pdn_release_cache", "pdn_update_tsvs",
            "pdn_reff_same_side", "pdn_load_voltages", "pdn_reff_nodes", "pdn_shard_slice", "pdn_shard_buffers",
-           "pdn_finish")
+           "pdn_finish", "pdn_set_solver_opts")
 
 _lib = None
 
@@ -85,6 +85,8 @@ def load_library() -> C.CDLL:
     lib.pdn_last_error.argtypes = []
     lib.pdn_update_tsvs.restype = C.c_int
     lib.pdn_update_tsvs.argtypes = [C.c_void_p, C.c_int32, C.POINTER(PdnTsv)]
+    lib.pdn_set_solver_opts.restype = C.c_int
+    lib.pdn_set_solver_opts.argtypes = [C.c_void_p, C.c_double, C.c_int32]
     lib.pdn_reff_same_side.restype = C.c_int
     lib.pdn_reff_same_side.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
     lib.pdn_load_voltages.restype = C.c_int
@@ -148,13 +150,29 @@ def _tsvs(tsv_site, tsv_r) -> tuple:
     return out, n
 
 
-def _ptr(t) -> int:
-    """Address of a torch tensor (device or host) or a numpy array; must be contiguous FP64/int32."""
+def _ptr(t, kind: str, what: str, count=None) -> int:
+    """Address of a torch tensor (device or host) or a numpy array after checking what the C side assumes about
+    it: contiguous, dtype `kind` ("f8" = float64, "i4" = int32) and, if given, exactly `count` elements.  The
+    library reads / writes raw doubles and int32s: a float32 `out` or an int64 index tensor would be misread
+    silently, so they are refused here."""
     if isinstance(t, np.ndarray):
-        assert t.flags["C_CONTIGUOUS"]
-        return t.ctypes.data
-    assert t.is_contiguous()
-    return t.data_ptr()
+        ok_dtype = t.dtype == (np.float64 if kind == "f8" else np.int32)
+        contiguous, n, addr = t.flags["C_CONTIGUOUS"], t.size, t.ctypes.data
+    else:
+        import torch
+        ok_dtype = t.dtype == (torch.float64 if kind == "f8" else torch.int32)
+        contiguous, n, addr = t.is_contiguous(), t.numel(), t.data_ptr()
+    if not ok_dtype:
+        raise TypeError(f"{what} must be {'float64' if kind == 'f8' else 'int32'}, got {t.dtype}")
+    if not contiguous:
+        raise ValueError(f"{what} must be contiguous")
+    if count is not None and n != count:
+        raise ValueError(f"{what} must have {count} elements, got {n}")
+    return addr
+
+
+def _on_cuda(t) -> bool:
+    return bool(getattr(t, "is_cuda", False))
 
 
 class _CudaArray:
@@ -166,7 +184,7 @@ class _CudaArray:
 
 def _device_view(ptr: int, n: int):
     import torch
-    return torch.as_tensor(_CudaArray(ptr, n), device="cuda")
+    return torch.as_tensor(_CudaArray(ptr, n), device=f"cuda:{torch.cuda.current_device()}")
 
 
 def shard_bounds(k: int, world: int):
@@ -186,10 +204,13 @@ class Pdn:
         tiers = (PdnTier * d)()
         self._keep = (gx, gy)
         for t in range(d):
-            assert tuple(gx[t].shape) == (n, n) and tuple(gy[t].shape) == (n, n)
+            if tuple(gx[t].shape) != (n, n) or tuple(gy[t].shape) != (n, n):
+                raise ValueError(f"tier {t}: gx / gy must have shape ({n}, {n})")
+            if _on_cuda(gx[t]) == on_host or _on_cuda(gy[t]) == on_host:
+                raise ValueError("all conductance planes must live on the same side (all CUDA tensors or all host arrays)")
             tiers[t].n = n
-            tiers[t].gx = _ptr(gx[t])
-            tiers[t].gy = _ptr(gy[t])
+            tiers[t].gx = _ptr(gx[t], "f8", f"gx[{t}]")
+            tiers[t].gy = _ptr(gy[t], "f8", f"gy[{t}]")
         tsvs, ntsv = _tsvs(tsv_site, tsv_r)
         self.m = len(np.asarray(bumps).reshape(-1, 2))
         self.nl = len(np.asarray(loads).reshape(-1, 2))
@@ -209,6 +230,17 @@ class Pdn:
         self._h = h
         self._lib = lib
         self._terminal_rows = bool(flags & PDN_TERMINAL_PAIRS)
+        # the CUDA device the context lives on (the one current at pdn_create): buffers made here go there
+        self._device = None
+        if not on_host:
+            self._device = gx[0].device
+        else:
+            try:
+                import torch
+                if torch.cuda.is_available():
+                    self._device = torch.device("cuda", torch.cuda.current_device())
+            except ImportError:
+                pass
 
     @classmethod
     def from_network(cls, net, device=None, **kw):
@@ -220,20 +252,28 @@ class Pdn:
             gy = [torch.from_numpy(np.ascontiguousarray(g)).to(device) for g in gy]
         return cls(net.n, gx, gy, net.tsv_site, net.tsv_r, net.bumps, net.loads, **kw)
 
+    def _pair_args(self, out, bump_idx, load_idx, device: bool):
+        npairs = out.size if isinstance(out, np.ndarray) else out.numel()
+        if (bump_idx is None) != (load_idx is None):
+            raise ValueError("bump_idx and load_idx must both be given or both be None")
+        for t, what in ((out, "out"), (bump_idx, "bump_idx"), (load_idx, "load_idx")):
+            if t is not None and _on_cuda(t) != device:
+                raise ValueError(f"{what} must be a {'CUDA tensor' if device else 'host array'}")
+        if bump_idx is None and npairs != self.m * self.nl:
+            raise ValueError(f"the full cross product needs out of {self.m * self.nl} elements, got {npairs}")
+        return (npairs, _ptr(bump_idx, "i4", "bump_idx", npairs) if bump_idx is not None else None,
+                _ptr(load_idx, "i4", "load_idx", npairs) if load_idx is not None else None, _ptr(out, "f8", "out"))
+
     def reff(self, out, bump_idx=None, load_idx=None):
-        """pdn_reff: `out` (and the index arrays) are torch CUDA tensors."""
-        npairs = out.numel()
-        st = self._lib.pdn_reff(self._h, npairs, _ptr(bump_idx) if bump_idx is not None else None,
-                                _ptr(load_idx) if load_idx is not None else None, _ptr(out))
+        """pdn_reff: `out` (float64) and the index arrays (int32, one entry per pair) are torch CUDA tensors."""
+        st = self._lib.pdn_reff(self._h, *self._pair_args(out, bump_idx, load_idx, True))
         if st != PDN_OK:
             raise PdnError(st, "pdn_reff")
         return out
 
     def reff_host(self, out: np.ndarray, bump_idx=None, load_idx=None):
-        """pdn_reff_host: `out` / index arrays are numpy (or pinned torch CPU) buffers."""
-        npairs = out.size if isinstance(out, np.ndarray) else out.numel()
-        st = self._lib.pdn_reff_host(self._h, npairs, _ptr(bump_idx) if bump_idx is not None else None,
-                                     _ptr(load_idx) if load_idx is not None else None, _ptr(out))
+        """pdn_reff_host: `out` (float64) / index arrays (int32) are numpy (or pinned torch CPU) buffers."""
+        st = self._lib.pdn_reff_host(self._h, *self._pair_args(out, bump_idx, load_idx, False))
         if st != PDN_OK:
             raise PdnError(st, "pdn_reff_host")
         return out
@@ -243,18 +283,28 @@ class Pdn:
         tsvs, ntsv = _tsvs(tsv_site, tsv_r)
         st = self._lib.pdn_update_tsvs(self._h, ntsv, tsvs.ctypes.data_as(C.POINTER(PdnTsv)))
         if st != PDN_OK:
+            # A failure before the library's commit point leaves the context valid for the OLD plan; one after it
+            # poisons the context (every later call returns PDN_E_ARG).  Either way the caller is told.
             raise PdnError(st, "pdn_update_tsvs")
+
+    def set_solver_opts(self, rtol: float = 0.0, max_iter: int = 0):
+        """pdn_set_solver_opts: stopping rule of the port solves later calls run (0 keeps the current value)."""
+        st = self._lib.pdn_set_solver_opts(self._h, float(rtol), int(max_iter))
+        if st != PDN_OK:
+            raise PdnError(st, "pdn_set_solver_opts")
 
     def reff_same_side(self, side: int, out):
         """pdn_reff_same_side: `out` is a torch CUDA tensor of nt*nt doubles (side 0: bumps, 1: loads)."""
-        st = self._lib.pdn_reff_same_side(self._h, side, _ptr(out))
+        nt = self.m if side == 0 else self.nl
+        st = self._lib.pdn_reff_same_side(self._h, side, _ptr(out, "f8", "out", nt * nt))
         if st != PDN_OK:
             raise PdnError(st, "pdn_reff_same_side")
         return out
 
     def load_voltages(self, bump: int, i_load, v_bump: float, v_out):
         """pdn_load_voltages (Eq. 4): `i_load`, `v_out` are torch CUDA tensors of n_loads doubles."""
-        st = self._lib.pdn_load_voltages(self._h, bump, _ptr(i_load), float(v_bump), _ptr(v_out))
+        st = self._lib.pdn_load_voltages(self._h, bump, _ptr(i_load, "f8", "i_load", self.nl), float(v_bump),
+                                         _ptr(v_out, "f8", "v_out", self.nl))
         if st != PDN_OK:
             raise PdnError(st, "pdn_load_voltages")
         return v_out
@@ -263,7 +313,8 @@ class Pdn:
         """pdn_reff_nodes: `nodes` is an (k, 3) integer array of (tier, y, x) probes on the host, `out` a torch CUDA
         tensor of k*k doubles that receives R_eff between every two of them."""
         nd = np.ascontiguousarray(np.asarray(nodes, dtype=np.int32).reshape(-1, 3))
-        st = self._lib.pdn_reff_nodes(self._h, int(nd.shape[0]), nd.ctypes.data, _ptr(out))
+        k = int(nd.shape[0])
+        st = self._lib.pdn_reff_nodes(self._h, k, nd.ctypes.data, _ptr(out, "f8", "out", k * k))
         if st != PDN_OK:
             raise PdnError(st, "pdn_reff_nodes")
         return out
@@ -278,7 +329,7 @@ class Pdn:
         nodes = np.vstack([np.asarray(src, dtype=np.int32).reshape(1, 3),
                            np.stack([np.full(yy.size, tier, dtype=np.int32), yy.ravel(), xx.ravel()], axis=1)])
         k = nodes.shape[0]
-        out = torch.empty(k * k, dtype=torch.float64, device="cuda")
+        out = torch.empty(k * k, dtype=torch.float64, device=self._device)
         self.reff_nodes(nodes, out)
         return out[1:k].cpu().numpy().reshape(ys.size, ys.size)
 

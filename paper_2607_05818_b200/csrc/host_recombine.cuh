@@ -84,7 +84,7 @@ int single_tier_operands(pdn_ctx* c, Launcher& L) {
     c->u.alloc((size_t)m * sizeof(double));
     c->w.alloc((size_t)n * sizeof(double));
     L.run(KC_DENSE, 0, [&] { k_set_identity<<<cdiv((size_t)m * m, 256), 256, 0, L.s>>>(m, c->A1.as<double>()); });
-    L.run(KC_DENSE, 0, [&] { k_single_tier_operands<<<dim3(cdiv(m, 128), n + 1), 128, 0, L.s>>>(m, n, T.ZT.as<double>(), T.q, T.zdiag.as<double>(), c->X0.as<double>(), c->u.as<double>(), c->w.as<double>()); });
+    L.run(KC_DENSE, 0, [&] { k_single_tier_operands<<<dim3(cdiv(m, 128), grid_rows((size_t)n + 1)), 128, 0, L.s>>>(m, n, T.ZT.as<double>(), T.q, T.zdiag.as<double>(), c->X0.as<double>(), c->u.as<double>(), c->w.as<double>()); });
     CK(cudaStreamSynchronize(L.s));
     return PDN_OK;
 }
@@ -122,12 +122,12 @@ int recombine(pdn_ctx* c, Launcher& L) {
         TierPorts& Ta = c->tiers[i];
         TierPorts& Tb = c->tiers[i + 1];
         const int oa = i > 0 ? c->p[i - 1] : 0;
-        L.run(KC_DENSE, 0, [&] { k_assemble_diag<<<dim3(cdiv(pi, 128), pi), 128, 0, L.s>>>(pi, Ta.ZT.as<double>(), Ta.q, oa, Tb.ZT.as<double>(), Tb.q, rt[i].as<double>(), Kd[i].as<double>()); });
+        L.run(KC_DENSE, 0, [&] { k_assemble_diag<<<dim3(cdiv(pi, 128), grid_rows(pi)), 128, 0, L.s>>>(pi, Ta.ZT.as<double>(), Ta.q, oa, Tb.ZT.as<double>(), Tb.q, rt[i].as<double>(), Kd[i].as<double>()); });
         if (i + 1 < dm1) {
             const int pj = c->p[i + 1];
-            L.run(KC_DENSE, 0, [&] { k_assemble_coupling<<<dim3(cdiv(pj, 128), pi), 128, 0, L.s>>>(pi, pj, Tb.ZT.as<double>(), Tb.q, V[i + 1].as<double>()); });
+            L.run(KC_DENSE, 0, [&] { k_assemble_coupling<<<dim3(cdiv(pj, 128), grid_rows(pi)), 128, 0, L.s>>>(pi, pj, Tb.ZT.as<double>(), Tb.q, V[i + 1].as<double>()); });
         }
-        L.run(KC_DENSE, 0, [&] { k_assemble_rhs<<<dim3(cdiv(nrhs, 128), pi), 128, 0, L.s>>>(i, dm1, pi, m, n, T0.ZT.as<double>(), T0.q, T0.ntsv, Td.ZT.as<double>(), Td.q, Td.ntsv, F[i].as<double>()); });
+        L.run(KC_DENSE, 0, [&] { k_assemble_rhs<<<dim3(cdiv(nrhs, 128), grid_rows(pi)), 128, 0, L.s>>>(i, dm1, pi, m, n, T0.ZT.as<double>(), T0.q, T0.ntsv, Td.ZT.as<double>(), Td.q, Td.ntsv, F[i].as<double>()); });
     }
     // block-tridiagonal Cholesky.  Every diagonal factor L_i (p_i x p_i, cond ~ 1e2) is inverted once by a
     // p_i-column triangular solve; all substitutions are then K = p_i contractions on the FP64 tensor cores
@@ -166,7 +166,7 @@ int recombine(pdn_ctx* c, Launcher& L) {
         L.run(KC_DENSE, 0, [&] { k_colsum<<<cdiv(nrhs, 128), 128, 0, L.s>>>(c->p[i], nrhs, F[i].as<double>(), G.as<double>() + (size_t)i * nrhs); });
     L.run(KC_DENSE, 0, [&] { k_multipliers<<<1, 256, 0, L.s>>>(dm1, mn, G.as<double>(), Sinv.as<double>(), Y.as<double>(), fail.as<int>()); });
     for (int i = 0; i < dm1; i += std::max(dm1 - 1, 1))  // only the first and the last block row are read below
-        L.run(KC_DENSE, 0, [&] { k_currents<<<dim3(cdiv(mn, 128), c->p[i]), 128, 0, L.s>>>(c->p[i], dm1, mn, F[i].as<double>(), Y.as<double>()); });
+        L.run(KC_DENSE, 0, [&] { k_currents<<<dim3(cdiv(mn, 128), grid_rows(c->p[i])), 128, 0, L.s>>>(c->p[i], dm1, mn, F[i].as<double>(), Y.as<double>()); });
     // operands of S4
     const int p0 = c->p[0], pd = c->p[dm1 - 1];
     c->p0 = p0;
@@ -176,7 +176,7 @@ int recombine(pdn_ctx* c, Launcher& L) {
     c->w.alloc((size_t)n * sizeof(double));
     L.run(KC_DENSE, 0, [&] { k_terminal_consts<<<cdiv(m, 128), 128, 0, L.s>>>(p0, dm1, mn, m, 0, 0, T0.ZT.as<double>(), T0.q, T0.ntsv, 0, F[0].as<double>(), Y.as<double>(), T0.zdiag.as<double>(), c->u.as<double>()); });
     L.run(KC_DENSE, 0, [&] { k_terminal_consts<<<cdiv(n, 128), 128, 0, L.s>>>(pd, dm1, mn, n, m, 1, Td.ZT.as<double>(), Td.q, Td.ntsv, 0, F[dm1 - 1].as<double>(), Y.as<double>(), Td.zdiag.as<double>(), c->w.as<double>()); });
-    L.run(KC_DENSE, 0, [&] { k_pack_pair_operands<<<dim3(cdiv(p0, 128), mn), 128, 0, L.s>>>(p0, m, n, dm1, T0.ZT.as<double>(), T0.q, T0.ntsv, F[0].as<double>(), c->A1.as<double>(), c->X0.as<double>()); });
+    L.run(KC_DENSE, 0, [&] { k_pack_pair_operands<<<dim3(cdiv(p0, 128), grid_rows(mn)), 128, 0, L.s>>>(p0, m, n, dm1, T0.ZT.as<double>(), T0.q, T0.ntsv, F[0].as<double>(), c->A1.as<double>(), c->X0.as<double>()); });
     if (c->terminal_pairs) {  // operands of the same-side pair kernel (port.cuh: k_pair_same)
         struct { pdn_ctx::Side& S; TierPorts& T; int p, nt, col0; double* I; } sides[2] = {
             {c->side[0], T0, p0, m, 0, F[0].as<double>()}, {c->side[1], Td, pd, n, m, F[dm1 - 1].as<double>()}};
@@ -186,7 +186,7 @@ int recombine(pdn_ctx* c, Launcher& L) {
             sd.S.X.alloc((size_t)sd.nt * sd.p * sizeof(double));
             sd.S.ys.alloc((size_t)sd.nt * sizeof(double));
             sd.S.t.alloc((size_t)sd.nt * sizeof(double));
-            L.run(KC_DENSE, 0, [&] { k_pack_side<<<dim3(cdiv(sd.p, 128), sd.nt), 128, 0, L.s>>>(sd.p, sd.nt, sd.col0, nrhs, sd.T.ZT.as<double>(), sd.T.q, sd.T.ntsv, sd.I, sd.S.A.as<double>(), sd.S.X.as<double>()); });
+            L.run(KC_DENSE, 0, [&] { k_pack_side<<<dim3(cdiv(sd.p, 128), grid_rows(sd.nt)), 128, 0, L.s>>>(sd.p, sd.nt, sd.col0, nrhs, sd.T.ZT.as<double>(), sd.T.q, sd.T.ntsv, sd.I, sd.S.A.as<double>(), sd.S.X.as<double>()); });
             L.run(KC_DENSE, 0, [&] { k_side_consts<<<cdiv(sd.nt, 128), 128, 0, L.s>>>(sd.p, sd.nt, sd.col0, dm1, mn, sd.S.A.as<double>(), sd.S.X.as<double>(), Y.as<double>(), sd.T.zdiag.as<double>(), sd.S.ys.as<double>(), sd.S.t.as<double>()); });
         }
     }

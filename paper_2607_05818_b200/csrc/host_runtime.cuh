@@ -158,11 +158,13 @@ struct pdn_ctx {
     bool nu_auto = true;                  // opts.nu was left at its default: strongly anisotropic tiers may deepen it
     int shard_rank = 0, shard_world = 1;  // NEXT-4
     bool open = false;                    // sharded context whose rows have not been completed / S2-S3 not run
+    bool poisoned = false;                // pdn_update_tsvs failed after its commit point: only pdn_destroy is left
     pdn_stats stats{};
     double class_ms[KC_COUNT] = {};
     double class_bytes[KC_COUNT] = {};
     int64_t class_launches[KC_COUNT] = {};
     bool time_kernels = false;
+    bool debug = false;                   // PDN_DEBUG was set in the environment at pdn_create: iteration history on stderr
     std::vector<std::pair<int, std::pair<cudaEvent_t, cudaEvent_t>>> pending_events;
     std::vector<cudaEvent_t> event_pool;
 };
@@ -216,6 +218,8 @@ inline void once_per_device(std::atomic<uint64_t>& mask, F&& set) {
 }
 
 inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) / b); }
+// gridDim.y of the kernels that walk a problem dimension with `for (row = blockIdx.y; row < rows; row += gridDim.y)`
+inline unsigned grid_rows(size_t rows) { return (unsigned)std::min<size_t>(std::max<size_t>(rows, 1), 65535); }
 
 // ------------------------------------------------------------------------------------------------
 // TMA descriptors: a batched pitched vector v[B][ny][pitch] as a 3D tensor (x, y, b) of doubles whose

@@ -17,15 +17,7 @@ namespace {
 #ifndef PDN_PQ_W
 #define PDN_PQ_W (PDN_T3_W / 2)
 #endif
-#ifndef PDN_DN_R
-#define PDN_DN_R PDN_T3_R
-#endif
-#ifndef PDN_DN_W
-#define PDN_DN_W PDN_T3_W
-#endif
 constexpr int T3_R = PDN_T3_R, T3_W = PDN_T3_W, T3_EH = T3_R * T3_W, T3_THREADS = 32 * T3_W;
-constexpr int DN_R = PDN_DN_R, DN_W = PDN_DN_W;  // patch shape of the down stage (same tile height)
-static_assert(DN_R * DN_W == T3_EH, "all stencil kernels share the TMA box height");
 constexpr int PQ_R = PDN_PQ_R, PQ_W = PDN_PQ_W;  // the operator apply has one sweep and no r^: fatter patches pay
 static_assert(PQ_R * PQ_W == T3_EH, "all level-0 kernels share the TMA box height");
 constexpr size_t T3_TILE_BYTES = (size_t)T3_EH * T3_EW * sizeof(double), T3_SC_BYTES = (size_t)T3_EH * 32 * sizeof(float4);
@@ -219,14 +211,14 @@ void launch_down3(Launcher& L, int cls, double bytes, const Level& lv, const Smo
     constexpr int H = halo_of(NU), IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
     const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G);
     dim3 grid(tx, ty, cdiv(B, G));
-    constexpr size_t base = 2 * T3_TILE_BYTES + T3_SC_BYTES + sizeof(Exch<DN_W, T>);
+    constexpr size_t base = 2 * T3_TILE_BYTES + T3_SC_BYTES + sizeof(Exch<T3_W, T>);
     static std::atomic<uint64_t> attr_done{0};
     once_per_device(attr_done, [&] {
-        CK(cudaFuncSetAttribute(k_down3<DN_R, DN_W, NU, true, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(base + 2 * T3_TILE_BYTES)));
-        CK(cudaFuncSetAttribute(k_down3<DN_R, DN_W, NU, false, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)base));
+        CK(cudaFuncSetAttribute(k_down3<T3_R, T3_W, NU, true, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(base + 2 * T3_TILE_BYTES)));
+        CK(cudaFuncSetAttribute(k_down3<T3_R, T3_W, NU, false, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)base));
     });
-    if (m_q) L.run(cls, bytes, [&] { k_down3<DN_R, DN_W, NU, true, T><<<grid, 32 * DN_W, base + 2 * T3_TILE_BYTES, L.s>>>(m_r, *m_q, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
-    else L.run(cls, bytes, [&] { k_down3<DN_R, DN_W, NU, false, T><<<grid, 32 * DN_W, base, L.s>>>(m_r, m_r, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
+    if (m_q) L.run(cls, bytes, [&] { k_down3<T3_R, T3_W, NU, true, T><<<grid, 32 * T3_W, base + 2 * T3_TILE_BYTES, L.s>>>(m_r, *m_q, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
+    else L.run(cls, bytes, [&] { k_down3<T3_R, T3_W, NU, false, T><<<grid, 32 * T3_W, base, L.s>>>(m_r, m_r, lv, cr, alpha, r_out, y_out, rc, cny, cnx, cpitch, rr_acc, B, G, active); });
 }
 
 template <int NU, class T>
@@ -313,7 +305,7 @@ void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Smoother& sm, int B,
         }
         if (after_down0()) return;
         launch_tail(L, H, sm, 0, B, W.r[ru].as<double>(), W.z.as<double>(), W.s.active, 2.0 * V);
-        L.run(KC_UP0, 2.0 * V, [&] { k_dot_planes<<<dim3(std::min(64u, cdiv(plane, 256)), B), 256, 0, L.s>>>(W.r[ru].as<double>(), W.z.as<double>(), plane, W.s.active, W.s.rz); });
+        L.run(KC_UP0, 2.0 * V, [&] { k_dot_planes<<<dim3(std::min(64u, cdiv(plane, 256)), B), 256, 0, L.s>>>(W.r[ru].as<double>(), W.z.as<double>(), plane, H.nx[0], H.pitch[0], W.s.active, W.s.rz); });
         return;
     }
     for (int l = 0; l < lt; ++l) {
@@ -385,8 +377,8 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
             active_sum += nact;
             rel_prev = rel_cur;
             rel_cur = 0.0;
-            for (int b = 0; b < B; ++b) rel_cur = std::max(rel_cur, W.h_relres[b]);
-            if (getenv("PDN_DEBUG")) fprintf(stderr, "[pdn]   it %d: max relres %.3e, active %d\n", it, rel_cur, nact);
+            for (int b = 0; b < B; ++b) rel_cur = std::max(rel_cur, W.h_relres[b]);  // (a NaN is caught after the loop)
+            if (c->debug) fprintf(stderr, "[pdn]   it %d: max relres %.3e, active %d\n", it, rel_cur, nact);
             return done || it >= max_iter;
         };
         // CG residuals contract roughly geometrically: if the next one is expected below the tolerance, update the
@@ -430,12 +422,20 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     CK(cudaMemcpyAsync(W.h_relres, W.s.relres, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, L.s));
     CK(cudaStreamSynchronize(L.s));
     double worst = 0.0;
-    for (int b = 0; b < B; ++b) worst = std::max(worst, W.h_relres[b]);
+    bool nonfinite = false;  // a NaN / Inf residual froze its right-hand side (k_scal_check): that is a failure, not convergence
+    for (int b = 0; b < B; ++b) {
+        if (!std::isfinite(W.h_relres[b])) nonfinite = true;
+        else worst = std::max(worst, W.h_relres[b]);
+    }
+    if (nonfinite) {
+        g_last_error = "a port solve produced a non-finite residual";
+        status = PDN_E_NUMERIC;
+    }
     c->stats.worst_rel_residual = std::max(c->stats.worst_rel_residual, worst);
     c->stats.pcg_iters_max = std::max(c->stats.pcg_iters_max, it);
     c->stats.pcg_iters_sum += it;
     c->stats.rhs_iterations += active_sum;
-    if (getenv("PDN_DEBUG"))
+    if (c->debug)
         fprintf(stderr, "[pdn] batch src0=%d B=%d %s: %d iterations, rhs-iterations %ld (of %ld without skipping), worst relres %.2e\n", src0, B,
                 terminal ? "terminal" : "tsv", it, active_sum, (long)it * B, worst);
     return status;

@@ -138,19 +138,23 @@ __global__ void k_finish_term(const double* __restrict__ xown, const double* __r
 //   ZTn[rmap[j]][cmap[k]] = ZTo[j][k]   for old TSV rows j and old ports k whose maps are >= 0
 __global__ void k_remap_zt(const double* __restrict__ ZTo, int ntsv_o, int q_o, const int* __restrict__ rmap,
                            const int* __restrict__ cmap, double* __restrict__ ZTn, int q_n) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
-    if (k >= q_o || j >= ntsv_o) return;
-    const int jn = rmap[j], kn = cmap[k];
-    if (jn >= 0 && kn >= 0) ZTn[(size_t)jn * q_n + kn] = ZTo[(size_t)j * q_o + k];
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= q_o) return;
+    const int kn = cmap[k];
+    for (int j = blockIdx.y; j < ntsv_o; j += gridDim.y) {
+        const int jn = rmap[j];
+        if (jn >= 0 && kn >= 0) ZTn[(size_t)jn * q_n + kn] = ZTo[(size_t)j * q_o + k];
+    }
 }
 
 // ... and fill the columns of the added TSV ports in the kept rows by symmetry: Z[j][s] = Z[s][j].
 __global__ void k_mirror_added(double* __restrict__ ZT, int ntsv, int q, const int* __restrict__ added, int n_added,
                                const unsigned char* __restrict__ is_added) {
-    const int a = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
-    if (a >= n_added || j >= ntsv || is_added[j]) return;
+    const int a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= n_added) return;
     const int s = added[a];
-    ZT[(size_t)j * q + s] = ZT[(size_t)s * q + j];
+    for (int j = blockIdx.y; j < ntsv; j += gridDim.y)
+        if (!is_added[j]) ZT[(size_t)j * q + s] = ZT[(size_t)s * q + j];
 }
 
 // Meshes with n <= 4 are their own coarsest level: Z comes straight from the dense pseudo-inverse.

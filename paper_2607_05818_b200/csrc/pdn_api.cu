@@ -124,7 +124,7 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
             // T[a][s] = sum_b W[a][b] C[s][b]  (n x 2n);  G[t][s] = sum_a C[t][a] T[a][s]  (2n x 2n)
             gemm(L, n, 2 * n, n, 1.0, Wm.as<double>(), n, 1, Cm.as<double>(), 1, n, 0.0, T1.as<double>(), 2 * n);
             gemm(L, 2 * n, 2 * n, n, 1.0, Cm.as<double>(), n, 1, T1.as<double>(), 2 * n, 1, 0.0, Gt.as<double>(), 2 * n);
-            L.run(KC_SMALL, 0, [&] { k_uniform_gather<<<dim3(cdiv(T.q, 128), T.nrows + 1), 128, 0, L.s>>>(Gt.as<double>(), n, H.pitch[0], T.d_node.as<int>(), T.ntsv, T.nrows, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
+            L.run(KC_SMALL, 0, [&] { k_uniform_gather<<<dim3(cdiv(T.q, 128), grid_rows((size_t)T.nrows + 1)), 128, 0, L.s>>>(Gt.as<double>(), n, H.pitch[0], T.d_node.as<int>(), T.ntsv, T.nrows, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
             CK(cudaStreamSynchronize(L.s));  // the table buffers go back to the pool here
             c->stats.n_uniform_tiers++;
             T.whole = true;
@@ -141,7 +141,7 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
     const bool strong = H.anisotropy >= 6.0;
     const int nu = (strong && c->nu_auto) ? 6 : o.nu;
     const double ratio = o.cheb_ratio > 1.0 ? o.cheb_ratio : strong ? 2.0 * (1.0 + H.anisotropy) : 3.0 + H.anisotropy;
-    const int G = getenv("PDN_RHS_GROUP") ? std::max(1, atoi(getenv("PDN_RHS_GROUP"))) : 64;
+    const int G = T3_MAX_G;  // upper bound of the right-hand sides a stencil block loops over (rhs_per_block picks)
     // On near-isotropic tiers the coarse levels get by with one step less on a wider interval (measured: same
     // iteration counts at configs 3 and 5, one level-visit cheaper); anisotropic tiers keep nu steps everywhere.
     const bool iso = H.anisotropy < 1.5 && nu >= 3 && !(o.cheb_ratio > 1.0);
@@ -207,8 +207,11 @@ static bool wrong_device(const pdn_ctx* c) {
     int dev = -1;
     return cudaGetDevice(&dev) != cudaSuccess || dev != c->device;
 }
-#define PDN_CHECK_DEVICE(ctx) \
-    do { if (wrong_device(ctx)) return fail_arg("the context's CUDA device is not the current device"); } while (0)
+#define PDN_CHECK_DEVICE(ctx)                                                                                      \
+    do {                                                                                                           \
+        if ((ctx)->poisoned) return fail_arg("the context is unusable after a failed pdn_update_tsvs: destroy it"); \
+        if (wrong_device(ctx)) return fail_arg("the context's CUDA device is not the current device");             \
+    } while (0)
 
 int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_tsv, const pdn_tsv* tsvs,
                int32_t n_bumps, const pdn_site* bumps, int32_t n_loads, const pdn_site* loads, const pdn_opts* opts) {
@@ -240,6 +243,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         c->d = d; c->n = n; c->m = n_bumps; c->nl = n_loads; c->opts = o;
         c->stream = (cudaStream_t)o.cuda_stream;
         c->time_kernels = (o.flags & PDN_TIME_KERNELS) != 0;
+        c->debug = getenv("PDN_DEBUG") != nullptr;
         c->terminal_pairs = (o.flags & PDN_TERMINAL_PAIRS) != 0;
         c->nu_auto = nu_auto;
         if (o.shard_world > 1) {
@@ -372,6 +376,7 @@ int pdn_update_tsvs(pdn_ctx* ctx, int32_t n_tsv, const pdn_tsv* tsvs) {
     pdn_ctx* c = ctx;
     const int d = c->d, n = c->n;
     int status = PDN_OK;
+    bool committed = false;  // the staged tiers were swapped in: a failure after that point poisons the context
     try {
         std::vector<std::vector<int>> nsite;
         std::vector<std::vector<double>> nrt;
@@ -394,14 +399,20 @@ int pdn_update_tsvs(pdn_ctx* ctx, int32_t n_tsv, const pdn_tsv* tsvs) {
         Hierarchy H;
         bool h_ready = false;
         int64_t new_solves = 0;
+        // Every tier's new port list, port matrix and device copies are built in `staged` and swapped into the
+        // context only after ALL tiers succeeded: a failure on a later tier (PDN_E_NOCONV, PDN_E_NOMEM, ...) leaves
+        // the context exactly as it was, still valid for the old plan.
+        std::vector<TierPorts> staged(d);
+        std::vector<char> changed(d, 0);
         for (int t = 0; t < d && status == PDN_OK; ++t) {
-            TierPorts& T = c->tiers[t];
-            std::vector<int> node_n;
-            int ntsv_n = 0;
-            tier_port_list(c, t, nsite, node_n, ntsv_n);
-            if (node_n == T.node) continue;  // same sites in the same order: Z_t is unchanged
-            const int q_o = T.q, ntsv_o = T.ntsv, q_n = (int)node_n.size();
+            const TierPorts& T = c->tiers[t];
+            TierPorts& N = staged[t];
+            tier_port_list(c, t, nsite, N.node, N.ntsv);
+            if (N.node == T.node) continue;  // same sites in the same order: Z_t is unchanged
+            changed[t] = 1;
+            const int q_o = T.q, ntsv_o = T.ntsv, q_n = (int)N.node.size(), ntsv_n = N.ntsv;
             const int rows_o = T.nrows, rows_n = (c->terminal_pairs && q_n > ntsv_n) ? q_n : ntsv_n;
+            N.q = q_n; N.nterm = q_n - ntsv_n; N.nrows = rows_n;
             const int plo_o = t > 0 ? (int)c->site[t - 1].size() : 0, plo_n = t > 0 ? (int)nsite[t - 1].size() : 0;
             std::vector<int> cmap(q_o, -1);
             std::vector<unsigned char> is_added(std::max(rows_n, 1), 0);
@@ -416,17 +427,17 @@ int pdn_update_tsvs(pdn_ctx* ctx, int32_t n_tsv, const pdn_tsv* tsvs) {
             for (int k = ntsv_o; k < q_o; ++k) cmap[k] = ntsv_n + (k - ntsv_o);  // terminals keep their order
             std::vector<int> added;
             for (int k = 0; k < ntsv_n; ++k) if (is_added[k]) added.push_back(k);
-            DevBuf d_cmap, d_added, d_isadd, ZTn;
+            DevBuf d_cmap, d_added, d_isadd;
             d_cmap.alloc((size_t)q_o * sizeof(int));
             CK(cudaMemcpyAsync(d_cmap.p, cmap.data(), (size_t)q_o * sizeof(int), cudaMemcpyHostToDevice, L.s));
-            ZTn.alloc((size_t)rows_n * q_n * sizeof(double));
-            CK(cudaMemsetAsync(ZTn.p, 0, (size_t)rows_n * q_n * sizeof(double), L.s));
-            L.run(KC_SMALL, 0, [&] { k_remap_zt<<<dim3(cdiv(q_o, 128), rows_o), 128, 0, L.s>>>(T.ZT.as<double>(), rows_o, q_o, d_cmap.as<int>(), d_cmap.as<int>(), ZTn.as<double>(), q_n); });
-            CK(cudaStreamSynchronize(L.s));  // cmap (host vector) and the old ZT are released below
-            T.ZT = std::move(ZTn);
-            T.node = node_n; T.ntsv = ntsv_n; T.q = q_n; T.nterm = q_n - ntsv_n; T.nrows = rows_n;
-            T.d_node.alloc((size_t)q_n * sizeof(int));
-            CK(cudaMemcpyAsync(T.d_node.p, T.node.data(), (size_t)q_n * sizeof(int), cudaMemcpyHostToDevice, L.s));
+            N.ZT.alloc((size_t)rows_n * q_n * sizeof(double));
+            CK(cudaMemsetAsync(N.ZT.p, 0, (size_t)rows_n * q_n * sizeof(double), L.s));
+            L.run(KC_SMALL, 0, [&] { k_remap_zt<<<dim3(cdiv(q_o, 128), grid_rows(rows_o)), 128, 0, L.s>>>(T.ZT.as<double>(), rows_o, q_o, d_cmap.as<int>(), d_cmap.as<int>(), N.ZT.as<double>(), q_n); });
+            N.zdiag.alloc((size_t)std::max(N.nterm, 1) * sizeof(double));  // the terminals' diagonal does not depend on the TSV plan
+            if (N.nterm > 0) CK(cudaMemcpyAsync(N.zdiag.p, T.zdiag.p, (size_t)N.nterm * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
+            N.d_node.alloc((size_t)q_n * sizeof(int));
+            CK(cudaMemcpyAsync(N.d_node.p, N.node.data(), (size_t)q_n * sizeof(int), cudaMemcpyHostToDevice, L.s));
+            CK(cudaStreamSynchronize(L.s));  // cmap / node (host vectors) were read
             if (!added.empty()) {
                 if (!h_ready) { H.allocate(n); h_ready = true; }
                 status = H.build(L, T.gx0.as<double>(), T.gy0.as<double>(), false, true);
@@ -434,26 +445,38 @@ int pdn_update_tsvs(pdn_ctx* ctx, int32_t n_tsv, const pdn_tsv* tsvs) {
                 const int Bmax = pick_batch(H, (int)added.size(), c->opts);
                 Work W;
                 if (H.nlev > 1) W.allocate(H, Bmax, q_n);
-                status = reduce_tier(c, L, H, W, Bmax, T, added, {});
+                status = reduce_tier(c, L, H, W, Bmax, N, added, {});
                 if (status != PDN_OK) { g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status); break; }
                 new_solves += (int64_t)added.size();
                 d_added.alloc(added.size() * sizeof(int));
                 d_isadd.alloc((size_t)rows_n);
                 CK(cudaMemcpyAsync(d_added.p, added.data(), added.size() * sizeof(int), cudaMemcpyHostToDevice, L.s));
                 CK(cudaMemcpyAsync(d_isadd.p, is_added.data(), (size_t)rows_n, cudaMemcpyHostToDevice, L.s));
-                L.run(KC_SMALL, 0, [&] { k_mirror_added<<<dim3(cdiv(added.size(), 128), rows_n), 128, 0, L.s>>>(T.ZT.as<double>(), rows_n, q_n, d_added.as<int>(), (int)added.size(), d_isadd.as<unsigned char>()); });
+                L.run(KC_SMALL, 0, [&] { k_mirror_added<<<dim3(cdiv(added.size(), 128), grid_rows(rows_n)), 128, 0, L.s>>>(N.ZT.as<double>(), rows_n, q_n, d_added.as<int>(), (int)added.size(), d_isadd.as<unsigned char>()); });
                 CK(cudaStreamSynchronize(L.s));
             }
         }
         CK(cudaEventRecord(ev[1], L.s));
         if (status == PDN_OK) {
+            // ---- commit: from here on the context describes the new plan
+            committed = true;
+            for (int t = 0; t < d; ++t) {
+                if (!changed[t]) continue;
+                TierPorts& T = c->tiers[t];
+                TierPorts& N = staged[t];
+                T.node = std::move(N.node); T.ntsv = N.ntsv; T.nterm = N.nterm; T.q = N.q; T.nrows = N.nrows;
+                T.d_node = std::move(N.d_node); T.ZT = std::move(N.ZT); T.zdiag = std::move(N.zdiag);
+            }
             c->site = nsite;
             c->rt = nrt;
             c->stats.n_ports_total = 0;
             for (int i = 0; i < d - 1; ++i) c->p[i] = (int)nsite[i].size();
             for (int t = 0; t < d; ++t) c->stats.n_ports_total += c->tiers[t].q;
             status = recombine(c, L);
-            if (status != PDN_OK) g_last_error = pdn_strerror(status);
+            if (status != PDN_OK) {  // the old factor is gone and the new one is incomplete: nothing but pdn_destroy is left
+                g_last_error = std::string(pdn_strerror(status)) + " (the context is no longer usable: destroy it)";
+                c->poisoned = true;
+            }
         }
         CK(cudaEventRecord(ev[2], L.s));
         CK(cudaStreamSynchronize(L.s));
@@ -474,7 +497,18 @@ int pdn_update_tsvs(pdn_ctx* ctx, int32_t n_tsv, const pdn_tsv* tsvs) {
         g_last_error = "host allocation failed";
         status = PDN_E_NOMEM;
     }
+    if (status != PDN_OK && committed) c->poisoned = true;
     return status;
+}
+
+int pdn_set_solver_opts(pdn_ctx* ctx, double rtol, int32_t max_iter) {
+    if (!ctx) return fail_arg("null context");
+    if (rtol > 0.0) {
+        if (!std::isfinite(rtol) || rtol >= 1.0) return fail_arg("rtol must be in (0, 1)");
+        ctx->opts.rtol = rtol;
+    }
+    if (max_iter > 0) ctx->opts.max_iter = max_iter;
+    return PDN_OK;
 }
 
 static int reff_device(pdn_ctx* ctx, int64_t n_pairs, const int32_t* bi, const int32_t* li, double* out) {
@@ -540,12 +574,6 @@ int pdn_reff_host(pdn_ctx* ctx, int64_t n_pairs, const int32_t* bump_idx, const 
 }
 
 void pdn_release_cache(void) { g_pool.trim(); }
-
-#ifdef PDN_PHASE_CLOCKS
-int pdn_debug_phase_clocks(long long* out) {  // scratch instrumentation, not part of the ABI
-    return (int)cudaMemcpyFromSymbol(out, pdn::g_phase_clk, sizeof(long long) * 64 * 8);
-}
-#endif
 
 // NEXT-3: R_eff between terminals of the same side (bump-bump or load-load), full nt x nt matrix on the device.
 int pdn_reff_same_side(pdn_ctx* ctx, int32_t side, double* out) {
@@ -673,7 +701,7 @@ int pdn_reff_nodes(pdn_ctx* ctx, int32_t n_nodes, const pdn_node* nodes, double*
             const int plo = t > 0 ? c->p[t - 1] : 0;
             double* Fup = t < dm1 ? F[t].as<double>() : nullptr;
             double* Flo = t > 0 ? F[t - 1].as<double>() : nullptr;
-            L.run(KC_DENSE, 0, [&] { k_probe_scatter<<<dim3(cdiv(Tp.q, 128), k), 128, 0, L.s>>>(k, T.ntsv, plo, np, d_probe.as<int>(), Tp.ZT.as<double>(), Fup, Flo, M.as<double>()); });
+            L.run(KC_DENSE, 0, [&] { k_probe_scatter<<<dim3(cdiv(Tp.q, 128), grid_rows(k)), 128, 0, L.s>>>(k, T.ntsv, plo, np, d_probe.as<int>(), Tp.ZT.as<double>(), Fup, Flo, M.as<double>()); });
             CK(cudaStreamSynchronize(L.s));  // probe (host vector) and the tier's buffers are released here
         }
         if (status == PDN_OK) {
@@ -692,7 +720,7 @@ int pdn_reff_nodes(pdn_ctx* ctx, int32_t n_nodes, const pdn_node* nodes, double*
                 gemm(L, np, np, pi, -1.0, F[i].as<double>(), 1, np, X[i].as<double>(), np, 1, 1.0, M.as<double>(), np);
             }
             gemm(L, np, np, dm1, -1.0, Cs.as<double>(), 1, np, mu.as<double>(), np, 1, 1.0, M.as<double>(), np);
-            L.run(KC_PAIR, (double)np * np * 8.0, [&] { k_probe_pairs<<<dim3(cdiv(np, 128), np), 128, 0, L.s>>>(np, M.as<double>(), out); });
+            L.run(KC_PAIR, (double)np * np * 8.0, [&] { k_probe_pairs<<<dim3(cdiv(np, 128), grid_rows(np)), 128, 0, L.s>>>(np, M.as<double>(), out); });
         }
         CK(cudaStreamSynchronize(L.s));
         L.resolve();
@@ -792,6 +820,7 @@ int32_t pdn_port_count(const pdn_ctx* ctx, int32_t tier) {
 
 int pdn_get_port_matrix(const pdn_ctx* ctx, int32_t tier, double* out) {
     if (!ctx || !out || tier < 0 || tier >= ctx->d) return fail_arg("bad tier or null output");
+    if (ctx->poisoned) return fail_arg("the context is unusable after a failed pdn_update_tsvs: destroy it");
     const TierPorts& T = ctx->tiers[tier];
     try {
         std::vector<double> zt((size_t)T.nrows * T.q), zd((size_t)T.nterm);

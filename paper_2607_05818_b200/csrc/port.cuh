@@ -15,20 +15,22 @@ namespace pdn {
 __global__ void k_assemble_diag(int p, const double* __restrict__ ZTa, int64_t qa, int oa,
                                 const double* __restrict__ ZTb, int64_t qb, const double* __restrict__ rt,
                                 double* __restrict__ Kii) {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y;
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= p) return;
-    double v = 0.5 * (ZTa[(oa + a) * qa + oa + b] + ZTa[(oa + b) * qa + oa + a]) +
-               0.5 * (ZTb[a * qb + b] + ZTb[b * qb + a]);
-    if (a == b) v += rt[a];
-    Kii[(int64_t)a * p + b] = v;
+    for (int a = blockIdx.y; a < p; a += gridDim.y) {  // (rows walk gridDim.y, which is capped at 65535)
+        double v = 0.5 * (ZTa[(oa + a) * qa + oa + b] + ZTa[(oa + b) * qa + oa + a]) +
+                   0.5 * (ZTb[a * qb + b] + ZTb[b * qb + a]);
+        if (a == b) v += rt[a];
+        Kii[(int64_t)a * p + b] = v;
+    }
 }
 
 // Coupling block K_{i,i+1} = -sym-part of Z_{i+1}[lo_i, up_{i+1}]          (p_i x p_{i+1})
 //   ZT = ZT_{i+1} (ld q); lo_i ports at offset 0, up_{i+1} ports at offset p_i.
 __global__ void k_assemble_coupling(int pi, int pj, const double* __restrict__ ZT, int64_t q, double* __restrict__ V) {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y;
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= pj) return;
-    V[(int64_t)a * pj + b] = -0.5 * (ZT[a * q + pi + b] + ZT[(pi + b) * q + a]);
+    for (int a = blockIdx.y; a < pi; a += gridDim.y) V[(int64_t)a * pj + b] = -0.5 * (ZT[a * q + pi + b] + ZT[(pi + b) * q + a]);
 }
 
 // Right-hand-side block row i of F = [F^1 | F^d | B]  (p_i x nrhs, nrhs = m + n + d-1), Eq. (19)/(21):
@@ -39,17 +41,19 @@ __global__ void k_assemble_rhs(int i, int dm1, int p, int m, int n, const double
                                int ntsv0, const double* __restrict__ ZTd, int64_t qd, int ntsvd,
                                double* __restrict__ F) {
     const int nrhs = m + n + dm1;
-    const int c = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= nrhs) return;
-    double v = 0.0;
-    if (c < m) {
-        if (i == 0) v = ZT0[a * q0 + ntsv0 + c];
-    } else if (c < m + n) {
-        if (i == dm1 - 1) v = ZTd[a * qd + ntsvd + (c - m)];
-    } else if (c - m - n == i) {
-        v = 1.0;
+    for (int a = blockIdx.y; a < p; a += gridDim.y) {
+        double v = 0.0;
+        if (c < m) {
+            if (i == 0) v = ZT0[a * q0 + ntsv0 + c];
+        } else if (c < m + n) {
+            if (i == dm1 - 1) v = ZTd[a * qd + ntsvd + (c - m)];
+        } else if (c - m - n == i) {
+            v = 1.0;
+        }
+        F[(int64_t)a * nrhs + c] = v;
     }
-    F[(int64_t)a * nrhs + c] = v;
 }
 
 // G[i][c] = sum over the rows of block i of T_i[a][c]   (= B^T K^-1 F)
@@ -101,11 +105,13 @@ __global__ void k_multipliers(int dm1, int mn, const double* __restrict__ G, dou
 // TSV currents of block row i:  I[a][c] = T[a][c] - sum_k T[a][m+n+k] Y[k][c]   for c < m+n  (in place)
 __global__ void k_currents(int p, int dm1, int mn, double* __restrict__ T, const double* __restrict__ Y) {
     const int nrhs = mn + dm1;
-    const int c = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= mn) return;
-    double v = T[(int64_t)a * nrhs + c];
-    for (int k = 0; k < dm1; ++k) v = fma(-T[(int64_t)a * nrhs + mn + k], Y[(int64_t)k * mn + c], v);
-    T[(int64_t)a * nrhs + c] = v;
+    for (int a = blockIdx.y; a < p; a += gridDim.y) {
+        double v = T[(int64_t)a * nrhs + c];
+        for (int k = 0; k < dm1; ++k) v = fma(-T[(int64_t)a * nrhs + mn + k], Y[(int64_t)k * mn + c], v);
+        T[(int64_t)a * nrhs + c] = v;
+    }
 }
 
 // Terminal constants (one thread per terminal column c of the first / last block row):
@@ -131,10 +137,12 @@ __global__ void k_pack_pair_operands(int p0, int m, int n, int dm1, const double
                                      int ntsv0, const double* __restrict__ I0, double* __restrict__ A1,
                                      double* __restrict__ X0) {
     const int nrhs = m + n + dm1;
-    const int a = blockIdx.x * blockDim.x + threadIdx.x, row = blockIdx.y;
+    const int a = blockIdx.x * blockDim.x + threadIdx.x;
     if (a >= p0) return;
-    if (row < m) A1[(int64_t)row * p0 + a] = ZT0[(int64_t)a * q0 + ntsv0 + row];
-    else X0[(int64_t)(row - m) * p0 + a] = I0[(int64_t)a * nrhs + m + (row - m)];
+    for (int row = blockIdx.y; row < m + n; row += gridDim.y) {
+        if (row < m) A1[(int64_t)row * p0 + a] = ZT0[(int64_t)a * q0 + ntsv0 + row];
+        else X0[(int64_t)(row - m) * p0 + a] = I0[(int64_t)a * nrhs + m + (row - m)];
+    }
 }
 
 // Same-side pairs (Eq. (4) PAPER.md:60-65 needs the load-load ones).  For two terminals
@@ -147,10 +155,12 @@ __global__ void k_pack_pair_operands(int p0, int m, int n, int dm1, const double
 // the currents of x_j, ys[j] = 1/2 sum_k y_j[k].
 __global__ void k_pack_side(int p, int nt, int col0, int nrhs, const double* __restrict__ ZT, int64_t q, int ntsv,
                             const double* __restrict__ Iblk, double* __restrict__ A, double* __restrict__ X) {
-    const int a = blockIdx.x * blockDim.x + threadIdx.x, s = blockIdx.y;
-    if (a >= p || s >= nt) return;
-    A[(int64_t)s * p + a] = ZT[(int64_t)a * q + ntsv + s];
-    X[(int64_t)s * p + a] = Iblk[(int64_t)a * nrhs + col0 + s];
+    const int a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= p) return;
+    for (int s = blockIdx.y; s < nt; s += gridDim.y) {
+        A[(int64_t)s * p + a] = ZT[(int64_t)a * q + ntsv + s];
+        X[(int64_t)s * p + a] = Iblk[(int64_t)a * nrhs + col0 + s];
+    }
 }
 
 __global__ void k_side_consts(int p, int nt, int col0, int dm1, int mn, const double* __restrict__ A,
@@ -225,17 +235,19 @@ k_pair_same(int nt, int p, const double* __restrict__ A, const double* __restric
 __global__ void k_probe_scatter(int k, int ntsv, int plo, int np, const int* __restrict__ probe,
                                 const double* __restrict__ Zp, double* __restrict__ Fup, double* __restrict__ Flo,
                                 double* __restrict__ M) {
-    const int col = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, q = ntsv + k;
+    const int col = blockIdx.x * blockDim.x + threadIdx.x, q = ntsv + k;
     if (col >= q) return;
-    const double* row = Zp + (int64_t)(ntsv + j) * q;
-    const int a = probe[j];
-    if (col < plo) {
-        if (Flo) Flo[(int64_t)col * np + a] = -row[col];
-    } else if (col < ntsv) {
-        if (Fup) Fup[(int64_t)(col - plo) * np + a] = row[col];
-    } else {
-        const int j2 = col - ntsv;
-        M[(int64_t)a * np + probe[j2]] = 0.5 * (row[col] + Zp[(int64_t)(ntsv + j2) * q + ntsv + j]);
+    for (int j = blockIdx.y; j < k; j += gridDim.y) {
+        const double* row = Zp + (int64_t)(ntsv + j) * q;
+        const int a = probe[j];
+        if (col < plo) {
+            if (Flo) Flo[(int64_t)col * np + a] = -row[col];
+        } else if (col < ntsv) {
+            if (Fup) Fup[(int64_t)(col - plo) * np + a] = row[col];
+        } else {
+            const int j2 = col - ntsv;
+            M[(int64_t)a * np + probe[j2]] = 0.5 * (row[col] + Zp[(int64_t)(ntsv + j2) * q + ntsv + j]);
+        }
     }
 }
 
@@ -254,9 +266,10 @@ __global__ void k_probe_multipliers(int dm1, int np, const double* __restrict__ 
 }
 
 __global__ void k_probe_pairs(int np, const double* __restrict__ M, double* __restrict__ R) {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y;
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= np) return;
-    R[(int64_t)a * np + b] = a == b ? 0.0 : (M[(int64_t)a * np + a] + M[(int64_t)b * np + b]) - (M[(int64_t)a * np + b] + M[(int64_t)b * np + a]);
+    for (int a = blockIdx.y; a < np; a += gridDim.y)
+        R[(int64_t)a * np + b] = a == b ? 0.0 : (M[(int64_t)a * np + a] + M[(int64_t)b * np + b]) - (M[(int64_t)a * np + b] + M[(int64_t)b * np + a]);
 }
 
 // Eq. (4): with bump b at v_bump and load k drawing I[k],
@@ -279,11 +292,13 @@ __global__ void k_load_voltages(int n, const double* __restrict__ Rb, const doub
 __global__ void k_single_tier_operands(int m, int n, const double* __restrict__ ZT, int64_t q,
                                        const double* __restrict__ zdiag, double* __restrict__ X0,
                                        double* __restrict__ u, double* __restrict__ w) {
-    const int a = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    const int a = blockIdx.x * blockDim.x + threadIdx.x;
     if (a >= m) return;
-    if (j < n) X0[(int64_t)j * m + a] = ZT[(int64_t)a * q + m + j];
-    else u[a] = ZT[(int64_t)a * q + a];
-    if (j < n && a == 0) w[j] = zdiag[j];
+    for (int j = blockIdx.y; j <= n; j += gridDim.y) {
+        if (j < n) X0[(int64_t)j * m + a] = ZT[(int64_t)a * q + m + j];
+        else u[a] = ZT[(int64_t)a * q + a];
+        if (j < n && a == 0) w[j] = zdiag[j];
+    }
 }
 
 // S4, full cross product:  R[i][j] = u[i] + w[j] - 2 sum_a A1[i][a] X0[j][a].   64x64 tile / block.

@@ -209,16 +209,6 @@ struct Geom {
 // vectors again.  Call before the block's first __syncthreads.
 constexpr int T3_MAX_G = 64;     // V-cycle stages: a block's set-up (coefficients, scaling tile) is spread over up to 64
 constexpr int T3_MAX_G_PQ = 32;  // operator apply: lighter set-up; measured 2 % slower with 64
-#ifdef PDN_PHASE_CLOCKS
-__device__ long long g_phase_clk[64 * 8];
-#define PHASE_CLK(j, k)                                                                                   \
-    do {                                                                                                  \
-        if (FUSED && blockIdx.x == 5 && blockIdx.y == 5 && blockIdx.z == 0 && threadIdx.x == 5 * 32 && (j) < 64) \
-            g_phase_clk[(j) * 8 + (k)] = clock64();                                                       \
-    } while (0)
-#else
-#define PHASE_CLK(j, k) do { } while (0)
-#endif
 
 struct ActiveList {
     int b[T3_MAX_G];
@@ -312,9 +302,7 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
     Xchg<W, T> xc{&x, &mbar[2], 0, 0u, warp, lane};
     for (int j = 0; j < nb; ++j) {
         const int b = al.b[j], st = j & 1;
-        PHASE_CLK(j, 0);
         mbar_wait(&mbar[st], (j >> 1) & 1);
-        PHASE_CLK(j, 1);
         const double alj = FUSED ? al.s[j] : 0.0;
         T y0r[R], y1r[R], rh0[R], rh1[R];
         double rr = 0.0;
@@ -341,7 +329,6 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
             rr = warp_sum(rr);
             if (lane == 0) atomicAdd(rr_acc + b, rr);
         }
-        PHASE_CLK(j, 2);
         // once thread 0 is past the first row exchange of this iteration every thread has arrived there,
         // i.e. has consumed the stage: thread 0 may refill it with right-hand side j+2
 #pragma unroll
@@ -349,10 +336,8 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
             smooth_step<R, W, T>(xc, c, y0r, y1r, rh0, rh1, (T)ch.w[k]);
             if (k == 1 && threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
         }
-        PHASE_CLK(j, 3);
         T t0[R], t1[R];
         apply_step<R, W, T>(xc, c, y0r, y1r, rh0, rh1, t0, t1);
-        PHASE_CLK(j, 4);
         if (NU == 1 && threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
         // residual of the unscaled system at the patch nodes, summed over 2x2 aggregates
 #pragma unroll
@@ -369,7 +354,6 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
                 rc[b * cplane + (size_t)((gy0 + i) >> 1) * cpitch + (gx >> 1)] = (double)v;
             }
         }
-        PHASE_CLK(j, 5);
     }
 }
 

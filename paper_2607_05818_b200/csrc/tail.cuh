@@ -188,16 +188,18 @@ k_tail(TailParams P, const double* __restrict__ r_in, double* __restrict__ z_out
     }
 }
 
-// acc[b] += sum over the plane of a[b] * c[b]   (r.z on meshes whose level 0 is in the tail); grid.y = B
+// acc[b] += sum over the nodes of a[b] * c[b]   (r.z on meshes whose level 0 is in the tail); grid.y = B.
+// The pad column of an odd-width plane is skipped: k_tail never writes it, so it holds whatever the pool block
+// held before (possibly a NaN bit pattern).
 __global__ void __launch_bounds__(256)
-k_dot_planes(const double* __restrict__ a, const double* __restrict__ c, size_t plane, const int* __restrict__ active,
-             double* __restrict__ acc) {
+k_dot_planes(const double* __restrict__ a, const double* __restrict__ c, size_t plane, int nx, int pitch,
+             const int* __restrict__ active, double* __restrict__ acc) {
     __shared__ double red[32];
     const int b = blockIdx.y;
     if (active && !active[b]) return;
     double s = 0.0;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < plane; i += (size_t)gridDim.x * blockDim.x)
-        s = fma(a[b * plane + i], c[b * plane + i], s);
+        if ((int)(i % pitch) < nx) s = fma(a[b * plane + i], c[b * plane + i], s);
     s = block_sum(s, red);
     if (threadIdx.x == 0) atomicAdd(acc + b, s);
 }

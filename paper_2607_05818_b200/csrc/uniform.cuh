@@ -70,14 +70,16 @@ __device__ __forceinline__ double uniform_pinv_entry(const double* __restrict__ 
 }
 
 // ZT[j][k] = L^+[port j, port k] for the rows j < nrows (the TSV ports; all ports with PDN_TERMINAL_PAIRS)
-// against all ports k < q (grid.y = nrows + 1); zdiag[s] = L^+[s, s] for the terminal ports.  node[] holds
+// against all ports k < q (grid.y walks rows 0 .. nrows); zdiag[s] = L^+[s, s] for the terminal ports.  node[] holds
 // pitched offsets y*pitch + x; G is indexed [x][y].
 __global__ void k_uniform_gather(const double* __restrict__ G, int n, int pitch, const int* __restrict__ node, int ntsv,
                                  int nrows, int q, double* __restrict__ ZT, double* __restrict__ zdiag) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= q) return;
-    if (j < nrows) ZT[(size_t)j * q + k] = uniform_pinv_entry(G, n, pitch, node[j], node[k]);
-    else if (k >= ntsv) zdiag[k - ntsv] = uniform_pinv_entry(G, n, pitch, node[k], node[k]);
+    for (int j = blockIdx.y; j <= nrows; j += gridDim.y) {
+        if (j < nrows) ZT[(size_t)j * q + k] = uniform_pinv_entry(G, n, pitch, node[j], node[k]);
+        else if (k >= ntsv) zdiag[k - ntsv] = uniform_pinv_entry(G, n, pitch, node[k], node[k]);
+    }
 }
 
 }  // namespace pdn

@@ -123,11 +123,14 @@ def test_workload_sampled_pairs(cfg):
     (9, 2, 70, 16, 6, 7, dict(aniso=0.25)), # several tiles + ragged tail
     (10, 3, 100, 5, 3, 12, dict(drop=0.02, aniso=3.0)),
 ])
-def test_random_stacks_against_live_oracle(seed, d, n, p, m, nl, kw):
+@pytest.mark.parametrize("rtol", [None, 1e-10], ids=["default_rtol", "rtol1e-10"])
+def test_random_stacks_against_live_oracle(seed, d, n, p, m, nl, kw, rtol):
+    """`default_rtol`: no rtol argument at all -- the library's default stopping rule (rtol 1e-8 for TSV sources,
+    1e-5 for bump / load sources) must meet the north_star tolerance away from the five workloads too."""
     from oracle.reff_oracle import Oracle
     net = P.make_random(seed, d=d, n=n, p=p, m=m, nl=nl, **kw)
     want = Oracle(net).reff_all()
-    got, _ = gpu_all_pairs(net, rtol=1e-10)
+    got, _ = gpu_all_pairs(net, **({} if rtol is None else dict(rtol=rtol)))
     check(got, want)
 
 
@@ -141,11 +144,12 @@ def test_strongly_heterogeneous_conductances_converge_and_match():
     check(got, Oracle(net).reff_all())
 
 
+@pytest.mark.parametrize("rtol", [None, 1e-10], ids=["default_rtol", "rtol1e-10"])
 @pytest.mark.parametrize("nu", [1, 2, 3, 4])
-def test_every_smoother_depth(nu):
+def test_every_smoother_depth(nu, rtol):
     from oracle.reff_oracle import Oracle
     net = P.make_random(20 + nu, d=2, n=45, p=6, m=4, nl=4, drop=0.03)
-    got, st = gpu_all_pairs(net, nu=nu, rtol=1e-10)
+    got, st = gpu_all_pairs(net, nu=nu, **({} if rtol is None else dict(rtol=rtol)))
     check(got, Oracle(net).reff_all())
 
 
@@ -611,8 +615,9 @@ def test_sharded_port_solves_emulated_on_one_gpu(world, flags_name):
         r.close()
 
 
-@pytest.mark.parametrize("block", [0, 1, 2])
-def test_randomised_stacks_through_every_entry_point(block):
+@pytest.mark.parametrize("block,rtol", [(0, 1e-10), (1, 1e-10), (2, 1e-10), (3, None), (4, None)],
+                         ids=["b0", "b1", "b2", "b3_default_rtol", "b4_default_rtol"])
+def test_randomised_stacks_through_every_entry_point(block, rtol):
     """Seeded fuzz, 12 stacks per block: random d, n (1-level meshes, one node more / less than a tile, odd sizes),
     port counts, anisotropy (up to 12), removed segments, a uniform tier now and then, random flags, batch sizes and
     smoother depths, device or host planes -- pdn_reff, pdn_reff_nodes on random probes, then a TSV re-plan followed by
@@ -621,10 +626,17 @@ def test_randomised_stacks_through_every_entry_point(block):
     from paper_2607_05818_b200 import PDN_NO_UNIFORM_FAST_PATH, PDN_TERMINAL_PAIRS, Pdn
     torch = torch_cuda()
 
+    # rtol 1e-10: every single entry within 1e-8.  Default stopping rule (no rtol argument): the north_star bar
+    # itself, max <= 1e-6 and mean <= 1e-8 per result array, on stacks far from BASELINE's distributions
+    # (anisotropy 12, 10 % of the segments removed, smoother depth 2).
     def rel_err(got, want):
         nz = want > 0
         assert np.abs(got[~nz]).max(initial=0.0) <= 1e-9 * max(want.max(), 1.0)
-        return np.abs(got[nz] / want[nz] - 1.0).max(initial=0.0)
+        rel = np.abs(got[nz] / want[nz] - 1.0)
+        if rtol is None:
+            assert rel.mean() <= MEAN_REL if rel.size else True
+            return rel.max(initial=0.0) * (1e-8 / MAX_REL)      # so that "<= 1e-8" below reads "max <= 1e-6"
+        return rel.max(initial=0.0)
 
     for it in range(12):
         seed = 7000 + 100 * block + it
@@ -639,7 +651,9 @@ def test_randomised_stacks_through_every_entry_point(block):
             t = int(rng.integers(d))
             net.gx[t], net.gy[t] = P._planes(n, np.full((n, n), 0.7), np.full((n, n), 1.9))
         flags = (PDN_TERMINAL_PAIRS if rng.random() < 0.4 else 0) | (PDN_NO_UNIFORM_FAST_PATH if rng.random() < 0.3 else 0)
-        kw = dict(rtol=1e-10, flags=flags, rhs_batch=int(rng.choice([0, 0, 1, 3, 7])), nu=int(rng.choice([0, 0, 2, 3, 5, 6])))
+        kw = dict(flags=flags, rhs_batch=int(rng.choice([0, 0, 1, 3, 7])), nu=int(rng.choice([0, 0, 2, 3, 5, 6])))
+        if rtol is not None:
+            kw["rtol"] = rtol
         what = f"seed {seed}: d={d} n={n} p={p} m={m} nl={nl} aniso={aniso} drop={drop} {kw}"
         pdn = Pdn.from_network(net, device="cuda:0" if rng.random() < 0.7 else None, **kw)
         o = Oracle(net)
@@ -779,6 +793,185 @@ def test_error_statuses():
     # wrong n_pairs for the cross product
     import torch
     pdn = Pdn.from_network(net, device="cuda:0")
-    with pytest.raises(PdnError):
-        pdn.reff(torch.empty(5, dtype=torch.float64, device="cuda:0"))
+    five = torch.empty(5, dtype=torch.float64, device="cuda:0")
+    with pytest.raises(ValueError):
+        pdn.reff(five)                                     # refused by the binding ...
+    assert pdn._lib.pdn_reff(pdn._h, 5, None, None, five.data_ptr()) == 1   # ... and by the library itself (PDN_E_ARG)
     pdn.close()
+
+
+def test_binding_refuses_buffers_the_library_would_misread():
+    """The C side reads raw doubles / int32s: wrong dtypes, sizes or sides are refused before the call."""
+    torch = torch_cuda()
+    from paper_2607_05818_b200 import Pdn
+    net = P.make_config(1, seed=0)
+    with pytest.raises(TypeError):
+        Pdn(net.n, [g.astype(np.float32) for g in net.gx], net.gy, net.tsv_site, net.tsv_r, net.bumps, net.loads)
+    pdn = Pdn.from_network(net, device="cuda:0")
+    npairs = net.m * net.nl
+    with pytest.raises(TypeError):
+        pdn.reff(torch.empty(npairs, dtype=torch.float32, device="cuda:0"))
+    out3 = torch.empty(3, dtype=torch.float64, device="cuda:0")
+    with pytest.raises(TypeError):                         # torch's default integer dtype is int64
+        pdn.reff(out3, torch.tensor([0, 1, 2], device="cuda:0"), torch.tensor([0, 1, 2], device="cuda:0"))
+    i32 = torch.tensor([0, 1], dtype=torch.int32, device="cuda:0")
+    with pytest.raises(ValueError):                        # one index per pair
+        pdn.reff(out3, i32, i32)
+    with pytest.raises(ValueError):                        # a host buffer on the device entry point
+        pdn.reff(np.empty(npairs))
+    with pytest.raises(ValueError):
+        pdn.reff_host(torch.empty(npairs, dtype=torch.float64, device="cuda:0"))
+    with pytest.raises(ValueError):
+        pdn.reff_nodes(np.array([[0, 0, 0], [1, 1, 1]], dtype=np.int32), torch.empty(3, dtype=torch.float64, device="cuda:0"))
+    m = pdn.reff_map((0, 0, 0), 1, stride=16)              # allocates on the context's device
+    assert m.shape == (2, 2) and np.isfinite(m).all()
+    pdn.close()
+
+
+def test_permuting_the_bump_and_load_lists_permutes_the_output():
+    """S4 pin: R depends on the pair, not on where it sits in the create-time lists."""
+    net = P.make_random(11, d=3, n=40, p=7, m=6, nl=9, drop=0.02)
+    ref, _ = gpu_all_pairs(net, rtol=1e-11)
+    rng = np.random.default_rng(5)
+    pb, pl = rng.permutation(net.m), rng.permutation(net.nl)
+    net.bumps, net.loads = np.ascontiguousarray(net.bumps[pb]), np.ascontiguousarray(net.loads[pl])
+    got, _ = gpu_all_pairs(net, rtol=1e-11)
+    assert np.allclose(got, ref[np.ix_(pb, pl)], rtol=1e-9, atol=0)
+
+
+def test_pair_kernel_equals_per_pair_solves_of_c_from_the_port_matrices():
+    """S4 pin (Eq. (18)-(22) PAPER.md:179-204): the bilinear split R(i,j) = u_i + w_j - 2 b_i^T x_j
+    of the pair kernel against ONE naive solve per pair of the coupled system C x = b, C = [K B; B^T 0] built here
+    in numpy from the tier port matrices the library returns (pdn_get_port_matrix), R = Z_0[s,s] + Z_{d-1}[l,l] - b^T x
+    (reading G9).  Checks S2 (assembly), S3 (factor + substitution) and S4 without the oracle."""
+    torch_cuda()
+    from paper_2607_05818_b200 import Pdn
+    d, n, p, m, nl = 4, 14, 5, 3, 4
+    net = P.make_random(19, d=d, n=n, p=p, m=m, nl=nl, drop=0.03, aniso=1.7)
+    pdn = Pdn.from_network(net, device="cuda:0", rtol=1e-12)
+    Z = [pdn.port_matrix(t) for t in range(d)]
+    import torch
+    out = torch.empty(m * nl, dtype=torch.float64, device="cuda:0")
+    got = pdn.reff(out).cpu().numpy().reshape(m, nl)
+    pdn.close()
+    pc = [len(s) for s in net.tsv_site]
+    off = np.concatenate([[0], np.cumsum(pc)])
+    Pt = int(off[-1])
+    K = np.zeros((Pt, Pt))
+    B = np.zeros((Pt, d - 1))
+    for i in range(d - 1):
+        lo_prev = pc[i - 1] if i > 0 else 0               # ports of tier i: [lo_{i-1}] ++ [up_i] ++ terminals
+        up = slice(lo_prev, lo_prev + pc[i])
+        lo = slice(0, pc[i])                                # ports of tier i+1 start with lo_i
+        blk = slice(off[i], off[i + 1])
+        K[blk, blk] = Z[i][up, up] + Z[i + 1][lo, lo] + np.diag(net.tsv_r[i])
+        if i + 1 < d - 1:
+            nxt = slice(off[i + 1], off[i + 2])
+            cpl = -Z[i + 1][lo, pc[i]:pc[i] + pc[i + 1]]    # -Z_{i+1}[lo_i, up_{i+1}]
+            K[blk, nxt], K[nxt, blk] = cpl, cpl.T
+        B[blk, i] = 1.0
+    Cm = np.block([[K, B], [B.T, np.zeros((d - 1, d - 1))]])
+    nt0, ntd = pc[0], (pc[-1] if d > 1 else 0)              # TSV ports of tier 0 / of tier d-1 (its lo ends)
+    for i in range(m):
+        for j in range(nl):
+            b = np.zeros(Pt + d - 1)
+            b[off[0]:off[1]] += Z[0][:nt0, nt0 + i]                       # Z_0[up_0, bump i]
+            b[off[d - 2]:off[d - 1]] += Z[d - 1][:ntd, ntd + j]           # Z_{d-1}[lo_{d-2}, load j]
+            b[Pt:] = 1.0
+            x = np.linalg.solve(Cm, b)
+            want = Z[0][nt0 + i, nt0 + i] + Z[d - 1][ntd + j, ntd + j] - b @ x
+            assert got[i, j] == pytest.approx(want, rel=1e-9)
+
+
+def test_failed_replanning_leaves_the_context_as_it_was():
+    """pdn_update_tsvs is staged: tier 0's new port matrix is a pure remap (its interface only loses a site) and
+    succeeds, then the added sites of tier 1 fail (iteration cap of 1, set through pdn_set_solver_opts).  The context
+    must still answer for the OLD plan, bit for bit (reff, every port matrix), pdn_reff_nodes must still work, and the
+    same update must go through once the cap is restored."""
+    from oracle.reff_oracle import Oracle
+    from paper_2607_05818_b200 import Pdn, PdnError
+    torch = torch_cuda()
+    d, n = 4, 41
+    net = P.make_random(23, d=d, n=n, p=6, m=4, nl=5, drop=0.02)
+    pdn = Pdn.from_network(net, device="cuda:0", rtol=1e-10)
+    out = torch.empty(net.m * net.nl, dtype=torch.float64, device="cuda:0")
+    before = pdn.reff(out).cpu().numpy().copy()
+    z_before = [pdn.port_matrix(t) for t in range(d)]
+    rng = np.random.default_rng(3)
+    new_sites = [s.copy() for s in net.tsv_site]
+    new_r = [r.copy() for r in net.tsv_r]
+    new_sites[0], new_r[0] = new_sites[0][1:].copy(), new_r[0][1:].copy()   # interface 0 only LOSES a site: tier 0 needs no solve
+    for i in range(1, d - 1):                               # the others get a new site: tiers 1 .. d-1 need solves
+        cand = [x for x in P._distinct_sites(rng, n, 8).tolist() if x not in new_sites[i].tolist()][0]
+        new_sites[i] = np.vstack([new_sites[i][1:], [cand]]).astype(np.int32)
+        new_r[i] = np.concatenate([new_r[i][1:], [0.09]])
+    pdn.set_solver_opts(max_iter=1)
+    with pytest.raises(PdnError) as e:
+        pdn.update_tsvs(new_sites, new_r)
+    assert e.value.status == 3                              # PDN_E_NOCONV
+    assert np.array_equal(pdn.reff(out).cpu().numpy(), before)
+    for t in range(d):
+        zt = pdn.port_matrix(t)
+        assert zt.shape == z_before[t].shape and np.array_equal(np.nan_to_num(zt), np.nan_to_num(z_before[t]))
+    pdn.set_solver_opts(max_iter=200)
+    nodes = np.array([[0, 1, 2], [d - 1, 30, 7]], dtype=np.int32)
+    rn = pdn.reff_nodes(nodes, torch.empty(4, dtype=torch.float64, device="cuda:0")).cpu().numpy()
+    o_old = Oracle(net)
+    assert abs(rn[1] / o_old.reff_nodes(1 * n + 2, (d - 1) * n * n + 30 * n + 7) - 1.0) <= MAX_REL
+    pdn.update_tsvs(new_sites, new_r)                       # the same list now goes through
+    net.tsv_site, net.tsv_r = new_sites, new_r
+    check(pdn.reff(out).cpu().numpy().reshape(net.m, net.nl), Oracle(net).reff_all())
+    pdn.close()
+
+
+_SHARD_WORKER = r"""
+import os, sys
+import numpy as np
+import torch, torch.distributed as dist
+sys.path.insert(0, os.getcwd())
+import pdn_inputs as P
+from oracle.reff_oracle import Oracle
+from paper_2607_05818_b200 import Pdn, PDN_TERMINAL_PAIRS
+dist.init_process_group("gloo")                       # NCCL refuses two ranks on one device; gloo moves CUDA tensors
+rank, world = dist.get_rank(), dist.get_world_size()
+torch.cuda.set_device(0)
+net = P.make_random(71, d=3, n=47, p=7, m=5, nl=6, drop=0.03)       # the same network on every rank
+net.gx[1], net.gy[1] = P._planes(net.n, np.full((net.n, net.n), 0.8), np.full((net.n, net.n), 1.3))  # a uniform tier
+flags = PDN_TERMINAL_PAIRS if os.environ.get("SHARD_TERMINAL_PAIRS") == "1" else 0
+pdn = Pdn.from_network(net, device="cuda:0", rtol=1e-10, flags=flags, shard_rank=rank, shard_world=world)
+pdn.exchange_and_finish(dist, world)                  # the product path, unchanged: broadcasts of library memory
+out = torch.empty(net.m * net.nl, dtype=torch.float64, device="cuda:0")
+got = pdn.reff(out).cpu().numpy().reshape(net.m, net.nl)
+want = Oracle(net).reff_all()
+rel = np.abs(got - want) / want
+assert rel.max() <= 1e-6 and rel.mean() <= 1e-8, (rel.max(), rel.mean())
+ref = Pdn.from_network(net, device="cuda:0", rtol=1e-10, flags=flags)   # unsharded, same process
+full = ref.reff(torch.empty_like(out)).cpu().numpy().reshape(net.m, net.nl)
+assert np.allclose(got, full, rtol=1e-9, atol=0)
+every = [torch.zeros_like(out) for _ in range(world)]                   # every rank holds the same result
+dist.all_gather(every, out)
+assert all(torch.equal(e, every[0]) for e in every)
+pdn.close(); ref.close()
+dist.destroy_process_group()
+print("shard-ok", rank, f"{rel.max():.2e}")
+"""
+
+
+@pytest.mark.parametrize("terminal_pairs", [False, True])
+def test_sharded_exchange_runs_for_real_between_two_processes_on_one_gpu(tmp_path, terminal_pairs):
+    """NEXT-4: `Pdn.exchange_and_finish` -- pdn_shard_slice / pdn_shard_buffers views of library
+    memory under torch.distributed.broadcast -- executed unchanged by two ranks (torchrun, one process per rank, both on
+    cuda:0, backend gloo since NCCL will not place two ranks on one device); every rank must equal the oracle and the
+    unsharded context, and all ranks must hold bit-identical results."""
+    import subprocess
+    import sys
+    torch_cuda()
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    w = tmp_path / "shard_worker.py"
+    w.write_text(_SHARD_WORKER)
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", SHARD_TERMINAL_PAIRS="1" if terminal_pairs else "0")
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                        "--master-addr", "127.0.0.1", "--master-port", "29547" if terminal_pairs else "29546", str(w)],
+                       cwd=root, env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, (r.stdout[-2000:], r.stderr[-4000:])
+    assert r.stdout.count("shard-ok") == 2
