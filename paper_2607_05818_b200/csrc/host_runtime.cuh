@@ -102,6 +102,16 @@ struct PinnedScratch {
 };
 thread_local PinnedScratch g_pinned;
 
+// PDN_POISON=1 in the environment (read once): every device block handed out is first filled with 0xFF bytes --
+// NaN as a double or float, -1 as an int -- so that any read of memory the library did not write itself turns
+// up as a NaN in the results (PDN_E_NUMERIC / a failed parity test) instead of depending on what the block held
+// before.  A debugging aid (the pool recycles blocks, which hides such reads); compute-sanitizer's initcheck is
+// not available on every box.
+inline bool poison_enabled() {
+    static const bool on = [] { const char* e = getenv("PDN_POISON"); return e && e[0] && e[0] != '0'; }();
+    return on;
+}
+
 struct DevBuf {  // RAII device allocation on the device that is current at alloc()
     void* p = nullptr;
     size_t bytes = 0;
@@ -123,6 +133,7 @@ struct DevBuf {  // RAII device allocation on the device that is current at allo
         p = g_pool.get(n, dev);
         if (!p) throw StatusFail{PDN_E_NOMEM, "cudaMalloc of " + std::to_string(n) + " bytes failed"};
         bytes = n;
+        if (poison_enabled()) { CK(cudaMemset(p, 0xFF, n)); CK(cudaDeviceSynchronize()); }
     }
     template <class T> T* as() const { return static_cast<T*>(p); }
 };
