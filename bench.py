@@ -186,7 +186,8 @@ def run_cuda(a):
     out_h = torch.empty(npairs, dtype=torch.float64).pin_memory()
     args = (net.n,), (net.tsv_site, net.tsv_r, net.bumps, net.loads)
 
-    base_flags = (8 if a.no_fast_path else 0) | (32 if a.precond_f32 else 0)  # PDN_NO_UNIFORM_FAST_PATH, PDN_PRECOND_F32
+    # PDN_NO_UNIFORM_FAST_PATH, PDN_PRECOND_F32, PDN_NO_INITIAL_GUESS
+    base_flags = (8 if a.no_fast_path else 0) | (32 if a.precond_f32 else 0) | (64 if a.no_guess else 0)
 
     shard_kw = dict(shard_rank=rank, shard_world=world) if sharded else {}
 
@@ -293,6 +294,7 @@ def run_cuda(a):
                          if cfg >= 3 else "working set fits L2: latency-bound case, HBM fraction not meaningful",
                    "rtol": a.rtol or 1e-8, "nu": a.nu or 4, "preconditioner_sweeps": "f32" if a.precond_f32 else "f64",
                    "pcg_iters_max": last["pcg_iters_max"], "rhs_iterations": last["rhs_iterations"],
+                   "initial_guess_tiers": last["n_guess_tiers"],
                    "ms_stencil": last["ms_stencil"], "ms_dense": last["ms_dense"], "ms_upload": last["ms_upload"]},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": ms_e2e / a.steps},
@@ -451,6 +453,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--uniform", action="store_true", help="uniform-tier variant of the workload (Eq. 3 fast path)")
     ap.add_argument("--no-fast-path", action="store_true", help="solve uniform tiers numerically too")
+    ap.add_argument("--no-guess", action="store_true",
+                    help="PDN_NO_INITIAL_GUESS: start every port solve from x0 = 0 instead of the closed form of the mean mesh")
     ap.add_argument("--precond-f32", action="store_true",
                     help="opt-in PDN_PRECOND_F32: multigrid sweeps in FP32 registers (CG, residuals, results stay FP64)")
     ap.add_argument("--replan", type=int, default=0, metavar="K",

@@ -68,6 +68,10 @@ enum {
                                vector in HBM stays FP64, and the solves still stop at the FP64 residual test, so
                                the results meet the same tolerance; only the iteration count may change.
                                Off by default: the default path computes in FP64 throughout                    */
+    PDN_NO_INITIAL_GUESS = 64, /* start every port solve from x0 = 0 (default: on a mesh of n >= 192 whose segment
+                               conductances scatter around their mean -- coefficient of variation <= 0.5 -- the
+                               solves start from the closed form, Eq. (3), of the mean mesh; same stopping test,
+                               same accuracy, about one PCG iteration less)                                      */
     PDN_NO_UNIFORM_FAST_PATH = 8 /* solve uniform tiers numerically too (default: a tier whose x-segments are all
                                equal and whose y-segments are all equal is reduced by the closed form, Eq. (3),
                                when it has enough ports for the 12 n^3-flop table to be cheaper than the solves) */
@@ -142,6 +146,8 @@ typedef struct {
     double class_ms[8];          /* device ms per kernel class (only with PDN_TIME_KERNELS)       */
     double class_bytes[8];       /* algorithmic bytes moved per kernel class                      */
     int64_t class_launches[8];   /* launches per kernel class                                     */
+    int32_t n_guess_tiers;       /* tier reductions whose port solves started from the closed-form guess */
+    int32_t reserved_;
 } pdn_stats;
 
 /* S0-S3.  tiers: HOST array of n_tiers descriptors (all tiers must have the same n).  tsvs, bumps,

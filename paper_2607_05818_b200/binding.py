@@ -21,6 +21,7 @@ PDN_TIME_KERNELS = 4
 PDN_NO_UNIFORM_FAST_PATH = 8
 PDN_TERMINAL_PAIRS = 16
 PDN_PRECOND_F32 = 32
+PDN_NO_INITIAL_GUESS = 64
 KERNEL_CLASSES = ("pq", "down0", "up0", "down_coarse", "up_coarse", "small", "dense", "pair")
 
 
@@ -50,7 +51,7 @@ class PdnStats(C.Structure):
                 ("ms_dense", C.c_double), ("ms_total", C.c_double), ("stencil_bytes", C.c_double),
                 ("ms_update_stencil", C.c_double), ("ms_update_dense", C.c_double), ("update_solves", C.c_int64),
                 ("class_ms", C.c_double * 8), ("class_bytes", C.c_double * 8),
-                ("class_launches", C.c_int64 * 8)]
+                ("class_launches", C.c_int64 * 8), ("n_guess_tiers", C.c_int32), ("reserved_", C.c_int32)]
 
 
 EXPORTS = ("pdn_create", "pdn_reff", "pdn_reff_host", "pdn_destroy", "pdn_strerror", "pdn_last_error",

@@ -32,6 +32,8 @@ struct Hierarchy {
     DevBuf gx[MAX_LEVELS], gy[MAX_LEVELS], hE[MAX_LEVELS], hS[MAX_LEVELS], sc[MAX_LEVELS];
     DevBuf pinv, flags, labels, sums;  // flags: [0] bad value, [1] isolated node, [2] label changed, [3] label nonzero
     double anisotropy = 1.0;           // max(mean gx / mean gy, mean gy / mean gx) of the tier built last
+    double mean_gx = 1.0, mean_gy = 1.0;  // mean segment conductance per direction (absent segments count as 0)
+    double cv = 0.0;                   // larger of the two coefficients of variation of the segment conductances
     Level lev[MAX_LEVELS];
 
     size_t plane(int l) const { return (size_t)ny[l] * pitch[l]; }
@@ -60,7 +62,7 @@ struct Hierarchy {
         }
         pinv.alloc(16 * 16 * sizeof(double));
         flags.alloc(4 * sizeof(int));
-        sums.alloc(2 * sizeof(double));
+        sums.alloc(4 * sizeof(double));
         labels.alloc((size_t)n * n * sizeof(int));
     }
 
@@ -86,14 +88,18 @@ struct Hierarchy {
         }
         const int lc = nlev - 1;
         L.run(KC_SMALL, 0, [&] { k_coarsest_pinv<<<1, 32, 0, L.s>>>(ny[lc], nx[lc], pitch[lc], gx[lc].as<double>(), gy[lc].as<double>(), pinv.as<double>()); });
-        CK(cudaMemsetAsync(sums.p, 0, 2 * sizeof(double), L.s));
+        CK(cudaMemsetAsync(sums.p, 0, 4 * sizeof(double), L.s));
         L.run(KC_SMALL, 0, [&] { k_plane_sums<<<std::min(1024u, cdiv(plane(0), 256)), 256, 0, L.s>>>((int)plane(0), gx[0].as<double>(), gy[0].as<double>(), sums.as<double>()); });
         int h[4] = {0, 0, 0, 0};
-        double hs[2] = {1.0, 1.0};
+        double hs[4] = {1.0, 1.0, 1.0, 1.0};
         CK(cudaMemcpyAsync(h, fl, 2 * sizeof(int), cudaMemcpyDeviceToHost, L.s));
-        CK(cudaMemcpyAsync(hs, sums.p, 2 * sizeof(double), cudaMemcpyDeviceToHost, L.s));
+        CK(cudaMemcpyAsync(hs, sums.p, 4 * sizeof(double), cudaMemcpyDeviceToHost, L.s));
         CK(cudaStreamSynchronize(L.s));
         anisotropy = (hs[0] > 0.0 && hs[1] > 0.0) ? std::max(hs[0] / hs[1], hs[1] / hs[0]) : 1.0;
+        const double cnt = (double)n * std::max(n - 1, 1);   // segments per direction
+        mean_gx = hs[0] / cnt; mean_gy = hs[1] / cnt;
+        auto cvar = [&](double s1, double s2) { const double m = s1 / cnt; return m > 0.0 ? std::sqrt(std::max(s2 / cnt / (m * m) - 1.0, 0.0)) : 1e300; };
+        cv = std::max(cvar(hs[0], hs[2]), cvar(hs[1], hs[3]));
         if (h[0]) return PDN_E_ARG;
         if (h[1] && n > 1) return PDN_E_DISCONNECTED;
         if (check_connectivity) {
@@ -142,6 +148,8 @@ struct Work {
     CUtensorMap m_r[2], m_y0, m_z, m_p[2], m_q;
     CUtensorMap m_rl[MAX_LEVELS], m_ya[MAX_LEVELS], m_ec[MAX_LEVELS];  // m_ec[l]: zb[l] as the coarse box of level l-1
     DevBuf scal, xport, xown, iact, src;  // src: port index each right-hand side of the batch is the source of
+    double *g_rr0 = nullptr, *g_sumx = nullptr, *g_dot = nullptr;  // initial guess (guess.cuh): ||r0||^2, sum(x0), x0.r_k per right-hand side
+    int *g_keep = nullptr, *g_rbuf = nullptr;     // ... whether the guess is used; buffer of the last residual
     PcgScalars s{};
     int* h_nact = nullptr;                           // pinned (g_pinned: not owned)
     double* h_relres = nullptr;                      // pinned, Bmax
@@ -165,13 +173,16 @@ struct Work {
             m_rl[l] = fine(rl[l], l); m_ya[l] = fine(ya[l], l);
             m_ec[l] = make_map(zb[l].p, H.nx[l], H.ny[l], H.pitch[l], B, T3_ECW, T3_EH / 2);
         }
-        scal.alloc((size_t)9 * B * sizeof(double));
+        scal.alloc((size_t)12 * B * sizeof(double));
         double* sp = scal.as<double>();
         s.rho = sp; s.rz = sp + B; s.pq = sp + 2 * B; s.rr = sp + 3 * B; s.sump = sp + 4 * B;
         s.alpha = sp + 5 * B; s.beta = sp + 6 * B; s.xmean = sp + 7 * B; s.relres = sp + 8 * B;
-        iact.alloc((size_t)(B + 1) * sizeof(int));
+        g_rr0 = sp + 9 * B; g_sumx = sp + 10 * B; g_dot = sp + 11 * B;
+        iact.alloc((size_t)(3 * B + 1) * sizeof(int));
         s.active = iact.as<int>();
         s.n_active = iact.as<int>() + B;
+        g_keep = iact.as<int>() + B + 1;
+        g_rbuf = iact.as<int>() + 2 * B + 1;
         xport.alloc((size_t)B * std::max(qmax, 1) * sizeof(double));
         xown.alloc((size_t)B * sizeof(double));
         src.alloc((size_t)B * sizeof(int));
@@ -337,8 +348,9 @@ void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Smoother& sm, int B,
 // Solve L_t x_b = e_{port src[b]} - 1/n^2 for b in [0, B) by multigrid-preconditioned CG and leave
 //   TSV-source batch     : ZT[src[b]][k] = x_b[port k] - mean(x_b)      for all ports k of the tier
 //   terminal-source batch: zdiag[src[b]-ntsv] = x_b[own node] - mean(x_b)
+// `guess` (may be null): closed-form starting point x0 of every right-hand side (guess.cuh).
 int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts& T, const Smoother& sm, const int* src_ports,
-                int B, bool terminal, double rtol, int max_iter) {
+                int B, bool terminal, double rtol, int max_iter, const GuessTable* guess) {
     const int src0 = src_ports[0];
     CK(cudaMemcpyAsync(W.src.p, src_ports, (size_t)B * sizeof(int), cudaMemcpyHostToDevice, L.s));
     const int* src = W.src.as<int>();
@@ -348,13 +360,25 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     const int* node = T.d_node.as<int>();
     const int ngather = terminal ? 0 : T.q;
     int cur_r = 0, cur_p = 0;
+    const double bnorm2 = 1.0 - 1.0 / (double)n2;
     L.run(KC_SMALL, 0, [&] { k_pcg_init<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B); });
-    L.run(KC_SMALL, V, [&] { k_init_rhs<<<dim3(std::min(1024u, cdiv(plane / 2, 256)), B), 256, 0, L.s>>>(W.r[0].as<double>(), n, H.pitch[0], plane, 1.0 / (double)n2, node, src, B); });
-    if (terminal) CK(cudaMemsetAsync(W.xown.p, 0, (size_t)B * sizeof(double), L.s));
-    else CK(cudaMemsetAsync(W.xport.p, 0, (size_t)B * ngather * sizeof(double), L.s));
+    if (guess) {
+        // x0 = column `src` of the mean mesh's closed-form pseudo-inverse, r0 = b - L x0; right-hand sides it does not
+        // help (||r0|| > ||b|| / 2) are re-initialised with x0 = 0, r0 = b -- all on the device
+        CK(cudaMemsetAsync(W.g_rr0, 0, (size_t)2 * B * sizeof(double), L.s));  // g_rr0 and g_sumx are adjacent
+        const int tiles = cdiv(n, GUESS_TX) * cdiv(n, GUESS_TY);
+        const int GR = std::max(1, std::min(16, (int)((long)tiles * B / (148L * 8))));
+        L.run(KC_SMALL, V, [&] { k_guess_rhs<<<dim3(tiles, cdiv(B, GR)), GUESS_THREADS, 0, L.s>>>(*guess, H.lev[0], node, src, 1.0 / (double)n2, W.r[0].as<double>(), W.g_rr0, W.g_sumx, B, GR); });
+        L.run(KC_SMALL, 0, [&] { k_guess_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.g_rr0, bnorm2, W.g_keep, B); });
+        L.run(KC_SMALL, 0, [&] { k_init_rhs<<<dim3(std::min(1024u, cdiv(plane / 2, 256)), B), 256, 0, L.s>>>(W.r[0].as<double>(), n, H.pitch[0], plane, 1.0 / (double)n2, node, src, B, W.g_keep); });
+        L.run(KC_SMALL, 0, [&] { k_guess_ports<<<dim3(cdiv(std::max(ngather, 1), 128), B), 128, 0, L.s>>>(*guess, H.pitch[0], node, ngather, src, W.g_keep, W.g_sumx, 1.0 / (double)n2, W.xport.as<double>(), W.xown.as<double>(), W.s.xmean, B); });
+    } else {
+        L.run(KC_SMALL, V, [&] { k_init_rhs<<<dim3(std::min(1024u, cdiv(plane / 2, 256)), B), 256, 0, L.s>>>(W.r[0].as<double>(), n, H.pitch[0], plane, 1.0 / (double)n2, node, src, B); });
+        if (terminal) CK(cudaMemsetAsync(W.xown.p, 0, (size_t)B * sizeof(double), L.s));
+        else CK(cudaMemsetAsync(W.xport.p, 0, (size_t)B * ngather * sizeof(double), L.s));
+    }
     int nact = B;  // right-hand sides still iterating
     vcycle(L, H, W, sm, B, 0, false, nact, [] { return false; });
-    const double bnorm2 = 1.0 - 1.0 / (double)n2;
     int it = 0, status = PDN_OK;
     long active_sum = B;  // right-hand sides still iterating, summed over the iterations (first one: all)
     double rel_prev = 1.0, rel_cur = 1.0;  // max relative residual over the batch after the last two iterations
@@ -367,8 +391,9 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
         L.run(KC_SMALL, 0, [&] { k_xport<<<dim3(cdiv(std::max(ngather, 1), 128), B), 128, 0, L.s>>>(W.p[cur_p].as<double>(), plane, W.s.alpha, node, ngather, src, W.xport.as<double>(), W.xown.as<double>(), B); });
         ++it;
         bool done = false;
+        int r_new = cur_r ^ 1;  // the buffer this iteration's residual update writes
         auto check = [&] {
-            L.run(KC_SMALL, 0, [&] { k_scal_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, rtol * rtol, bnorm2); });
+            L.run(KC_SMALL, 0, [&] { k_scal_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, rtol * rtol, bnorm2, r_new, W.g_rbuf); });
             CK(cudaMemcpyAsync(W.h_nact, W.s.n_active, sizeof(int), cudaMemcpyDeviceToHost, L.s));
             CK(cudaMemcpyAsync(W.h_relres, W.s.relres, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, L.s));
             CK(cudaStreamSynchronize(L.s));
@@ -392,7 +417,7 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
         if (cheap && it >= 2 && it < max_iter && predicted > 30.0 * rtol && skipped < 2) {  // at most two in a row
             ++skipped;
             vcycle(L, H, W, sm, B, cur_r, true, nact, [&] {
-                L.run(KC_SMALL, 0, [&] { k_scal_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, rtol * rtol, bnorm2); });
+                L.run(KC_SMALL, 0, [&] { k_scal_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, rtol * rtol, bnorm2, r_new, W.g_rbuf); });
                 return false;
             });
             cur_r ^= 1;
@@ -415,8 +440,12 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
         if (it >= max_iter) { status = PDN_E_NOCONV; break; }
     }
     // results + statistics
+    if (terminal && guess) {  // second-order form of the diagonal from a non-zero starting point: + x0 . r_k (guess.cuh)
+        CK(cudaMemsetAsync(W.g_dot, 0, (size_t)B * sizeof(double), L.s));
+        L.run(KC_SMALL, V, [&] { k_guess_dot<<<dim3(cdiv(n, GDOT_T) * cdiv(n, GDOT_T), B), 256, 0, L.s>>>(*guess, n, n, H.pitch[0], plane, node, src, W.g_keep, W.r[0].as<double>(), W.r[1].as<double>(), W.g_rbuf, W.g_dot); });
+    }
     if (terminal)
-        L.run(KC_SMALL, 0, [&] { k_finish_term<<<cdiv(B, 128), 128, 0, L.s>>>(W.xown.as<double>(), W.s.xmean, src, T.ntsv, T.zdiag.as<double>(), B); });
+        L.run(KC_SMALL, 0, [&] { k_finish_term<<<cdiv(B, 128), 128, 0, L.s>>>(W.xown.as<double>(), W.s.xmean, src, T.ntsv, T.zdiag.as<double>(), B, guess ? W.g_dot : nullptr); });
     else
         L.run(KC_SMALL, 0, [&] { k_finish_tsv<<<dim3(cdiv(ngather, 128), B), 128, 0, L.s>>>(W.xport.as<double>(), W.s.xmean, ngather, src, T.ZT.as<double>(), B); });
     CK(cudaMemcpyAsync(W.h_relres, W.s.relres, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, L.s));

@@ -11,9 +11,11 @@ namespace pdn {
 // pitched plane (plane = ny*pitch doubles; pad entries 0); node[] holds pitched offsets y*pitch + x of the
 // tier's ports, src[b] is the port index right-hand side b is the source of.
 __global__ void k_init_rhs(double* __restrict__ r, int nx, int pitch, size_t plane, double inv_n2,
-                           const int* __restrict__ node, const int* __restrict__ src, int B) {
+                           const int* __restrict__ node, const int* __restrict__ src, int B,
+                           const int* __restrict__ skip = nullptr) {
     // two adjacent columns (one 16-byte store) per thread and step; pitch and plane are even
     const int b = blockIdx.y;
+    if (skip && skip[b]) return;  // (guess.cuh: this right-hand side starts from its closed-form guess)
     const size_t hot = (size_t)node[src[b]];
     double2* r2 = reinterpret_cast<double2*>(r + b * plane);
     for (size_t i2 = (size_t)blockIdx.x * blockDim.x + threadIdx.x; 2 * i2 < plane; i2 += (size_t)gridDim.x * blockDim.x) {
@@ -59,13 +61,16 @@ __global__ void k_scal_alpha(PcgScalars s, int B, double inv_n2) {
 }
 
 // After r -= alpha q: convergence test  ||r||^2 <= tol2 * ||b||^2  (||b||^2 = 1 - 1/n2).
-__global__ void k_scal_check(PcgScalars s, int B, double tol2, double bnorm2) {
+// rbuf_of[b] (optional) records which of the two residual buffers holds the last residual of a right-hand side
+// (`rbuf` = the buffer this iteration wrote; a frozen right-hand side is never written again).
+__global__ void k_scal_check(PcgScalars s, int B, double tol2, double bnorm2, int rbuf = 0, int* __restrict__ rbuf_of = nullptr) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= B) return;
     if (s.active[b]) {
         const double rr = s.rr[b];
         s.relres[b] = sqrt(rr / bnorm2);
-        if (!(rr > tol2 * bnorm2)) s.active[b] = 0;  // also freezes on NaN
+        if (rbuf_of) rbuf_of[b] = rbuf;
+        if (!(rr > tol2 * bnorm2)) s.active[b] = 0;  // also freezes on NaN (reported by the host: PDN_E_NUMERIC)
         else atomicAdd(s.n_active, 1);
     }
 }
@@ -128,10 +133,12 @@ __global__ void k_finish_tsv(const double* __restrict__ xport, const double* __r
     if (k < ngather) ZT[(size_t)src[b] * ngather + k] = xport[(size_t)b * ngather + k] - xmean[b];
 }
 
+// (+ extra[b], the second-order correction of a solve that started from a guess: guess.cuh)
 __global__ void k_finish_term(const double* __restrict__ xown, const double* __restrict__ xmean,
-                              const int* __restrict__ src, int ntsv, double* __restrict__ zdiag, int B) {
+                              const int* __restrict__ src, int ntsv, double* __restrict__ zdiag, int B,
+                              const double* __restrict__ extra = nullptr) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b < B) zdiag[src[b] - ntsv] = xown[b] - xmean[b];
+    if (b < B) zdiag[src[b] - ntsv] = (xown[b] - xmean[b]) + (extra ? extra[b] : 0.0);
 }
 
 // TSV re-planning (pdn_update_tsvs): copy the kept entries of a tier's port matrix into its new layout.

@@ -31,6 +31,7 @@
 #include "stencil3.cuh"
 #include "tail.cuh"
 #include "uniform.cuh"
+#include "guess.cuh"
 #include "host_runtime.cuh"
 #include "host_solve.cuh"
 #include "host_recombine.cuh"
@@ -84,10 +85,47 @@ int pick_batch(const Hierarchy& H, int want, const pdn_opts& o) {
     return B;
 }
 
+// Spectral tables of Eq. (3) (uniform.cuh) built during one call, keyed by mesh size and rho = g_x / g_y: tiers that
+// differ by a scale factor share a table (a uniform stack builds one table, not one per tier; the initial guess of
+// BASELINE's workloads builds one per call).
+struct SpectralTables {
+    struct Entry { int n; double rho; DevBuf G, Gf; };
+    std::vector<Entry> list;
+    Entry* find(int n, double rho, double rel_tol) {
+        for (Entry& e : list)
+            if (e.n == n && std::fabs(e.rho - rho) <= rel_tol * rho) return &e;
+        return nullptr;
+    }
+    Entry& build(Launcher& L, int n, double rho, bool want_float) {
+        const size_t nn = (size_t)n * n, n1 = (size_t)n + 1;
+        Entry e;
+        e.n = n; e.rho = rho;
+        e.G.alloc(n1 * n1 * sizeof(double));
+        DevBuf Cm, Wm, T1;
+        Cm.alloc(n1 * n * sizeof(double)); Wm.alloc(nn * sizeof(double)); T1.alloc(n * n1 * sizeof(double));
+        L.run(KC_SMALL, 0, [&] { k_cos_matrix<<<cdiv(n1 * n, 256), 256, 0, L.s>>>(n, Cm.as<double>()); });
+        L.run(KC_SMALL, 0, [&] { k_spectral_weights<<<cdiv(nn, 256), 256, 0, L.s>>>(n, rho, 1.0, Wm.as<double>()); });
+        // T[a][s] = sum_b W[a][b] C[s][b]  (n x (n+1));  G[t][s] = sum_a C[t][a] T[a][s]  ((n+1) x (n+1))
+        gemm(L, n, n + 1, n, 1.0, Wm.as<double>(), n, 1, Cm.as<double>(), 1, n, 0.0, T1.as<double>(), n + 1);
+        gemm(L, n + 1, n + 1, n, 1.0, Cm.as<double>(), n, 1, T1.as<double>(), n + 1, 1, 0.0, e.G.as<double>(), n + 1);
+        CK(cudaStreamSynchronize(L.s));  // the work buffers go back to the pool here
+        list.push_back(std::move(e));
+        Entry& r = list.back();
+        if (want_float) float_copy(L, r);
+        return r;
+    }
+    void float_copy(Launcher& L, Entry& e) {
+        if (e.Gf.p) return;
+        const size_t cnt = ((size_t)e.n + 1) * (e.n + 1);
+        e.Gf.alloc(cnt * sizeof(float));
+        L.run(KC_SMALL, 0, [&] { k_table_to_float<<<cdiv(cnt, 256), 256, 0, L.s>>>(cnt, e.G.as<double>(), e.Gf.as<float>()); });
+    }
+};
+
 // S1 of one tier whose hierarchy H has just been built: fills rows `tsv_src` of ZT (each against all ports of
 // the tier) and, if `terminals`, zdiag.  Meshes with n <= 4 and uniform tiers (Eq. 3) are reduced whole.
 int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPorts& T, const std::vector<int>& tsv_src,
-                const std::vector<int>& term) {  // term: port indices (>= ntsv) of the terminal sources to solve
+                const std::vector<int>& term, SpectralTables& tabs) {  // term: port indices (>= ntsv) of the terminal sources to solve
     T.whole = false;
     const pdn_opts& o = c->opts;
     const int n = c->n;
@@ -96,14 +134,14 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
         T.whole = true;
         return PDN_OK;
     }
-    // The spectral table of a uniform tier costs 12 n^3 flops whatever the port count; q port solves cost about
-    // 8 iterations x 14 passes over a vector each.  With few ports on a very large mesh the solves are cheaper
-    // (measured: n = 16384, 7 ports: 0.9 s against 4.7 s), so the table is used only where this model says it pays
+    // The spectral table of a uniform tier costs 4 n^3 flops whatever the port count; q port solves cost about
+    // 8 iterations x 14 passes over a vector each.  With few ports on a very large mesh the solves are cheaper,
+    // so the table is used only where this model says it pays -- or where an earlier tier of the call left one
     // (FP64 tensor-core rate of the two contractions: ~3 TF/s at n = 1024, saturating near 22 TF/s).
     const double nn = (double)n * n;
-    const double t_table = 1e-4 + 12.0 * nn * n / std::min(22e12, 3e12 * n / 1024.0);
+    const double t_table = 1e-4 + 4.0 * nn * n / std::min(22e12, 3e12 * n / 1024.0);
     const double t_solves = 5e-4 + (double)T.q * 112.0 * 8.0 * nn / 4e12;
-    if (!(o.flags & PDN_NO_UNIFORM_FAST_PATH) && t_table <= t_solves) {
+    if (!(o.flags & PDN_NO_UNIFORM_FAST_PATH) && H.cv <= 1e-6) {
         // uniform tier: Eq. (3) of the paper as two dense contractions + a gather (uniform.cuh)
         int* fl = H.flags.as<int>();
         CK(cudaMemsetAsync(fl, 0, sizeof(int), L.s));
@@ -115,20 +153,33 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
         CK(cudaMemcpyAsync(&g0[1], H.gy[0].p, sizeof(double), cudaMemcpyDeviceToHost, L.s));
         CK(cudaStreamSynchronize(L.s));
         if (h_flag == 0 && g0[0] > 0.0 && g0[1] > 0.0) {
-            const size_t nn = (size_t)n * n;
-            DevBuf Cm, Wm, T1, Gt;
-            Cm.alloc(2 * nn * sizeof(double)); Wm.alloc(nn * sizeof(double));
-            T1.alloc(2 * nn * sizeof(double)); Gt.alloc(4 * nn * sizeof(double));
-            L.run(KC_SMALL, 0, [&] { k_cos_matrix<<<cdiv(2 * nn, 256), 256, 0, L.s>>>(n, Cm.as<double>()); });
-            L.run(KC_SMALL, 0, [&] { k_spectral_weights<<<cdiv(nn, 256), 256, 0, L.s>>>(n, g0[0], g0[1], Wm.as<double>()); });
-            // T[a][s] = sum_b W[a][b] C[s][b]  (n x 2n);  G[t][s] = sum_a C[t][a] T[a][s]  (2n x 2n)
-            gemm(L, n, 2 * n, n, 1.0, Wm.as<double>(), n, 1, Cm.as<double>(), 1, n, 0.0, T1.as<double>(), 2 * n);
-            gemm(L, 2 * n, 2 * n, n, 1.0, Cm.as<double>(), n, 1, T1.as<double>(), 2 * n, 1, 0.0, Gt.as<double>(), 2 * n);
-            L.run(KC_SMALL, 0, [&] { k_uniform_gather<<<dim3(cdiv(T.q, 128), grid_rows((size_t)T.nrows + 1)), 128, 0, L.s>>>(Gt.as<double>(), n, H.pitch[0], T.d_node.as<int>(), T.ntsv, T.nrows, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
-            CK(cudaStreamSynchronize(L.s));  // the table buffers go back to the pool here
-            c->stats.n_uniform_tiers++;
-            T.whole = true;
-            return PDN_OK;
+            const double rho = g0[0] / g0[1];
+            SpectralTables::Entry* e = tabs.find(n, rho, 0.0);
+            if (!e && t_table <= t_solves) e = &tabs.build(L, n, rho, false);
+            if (e) {
+                L.run(KC_SMALL, 0, [&] { k_uniform_gather<<<dim3(cdiv(T.q, 128), grid_rows((size_t)T.nrows + 1)), 128, 0, L.s>>>(e->G.as<double>(), 1.0 / g0[1], n, H.pitch[0], T.d_node.as<int>(), T.ntsv, T.nrows, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
+                c->stats.n_uniform_tiers++;
+                T.whole = true;
+                return PDN_OK;
+            }
+        }
+    }
+    // Initial guess (guess.cuh): the closed form of the tier's MEAN mesh as the starting point of every port solve,
+    // where the tier is near enough to it (coefficient of variation of the segment conductances; a rejected guess
+    // costs one pass over the vector) and large enough for an iteration to be worth more than the extra launches.
+    // A table left by an earlier tier of the call with the same anisotropy (within 2 %) is reused: the guess need
+    // not be exact.  A new one is built only for enough right-hand sides to pay for its 4 n^3 flops.
+    GuessTable gtab{};
+    const GuessTable* guess = nullptr;
+    if (!(o.flags & PDN_NO_INITIAL_GUESS) && n >= 192 && H.cv <= 0.5 && H.mean_gx > 0.0 && H.mean_gy > 0.0) {
+        const double rho = H.mean_gx / H.mean_gy;
+        SpectralTables::Entry* e = tabs.find(n, rho, 0.02);
+        if (!e && (long)(tsv_src.size() + term.size()) >= n / 2) e = &tabs.build(L, n, rho, true);
+        if (e) {
+            tabs.float_copy(L, *e);
+            gtab = GuessTable{e->Gf.as<float>(), 1.0 / H.mean_gy, n};
+            guess = &gtab;
+            c->stats.n_guess_tiers++;
         }
     }
     // Smoothing interval [2/ratio, 2] of the Chebyshev polynomial.  With 2x2 aggregation the coarse grid
@@ -155,13 +206,13 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
     const double rtol_term = std::max(o.rtol, std::min({1e-5, std::sqrt(o.rtol) / 3.0, 1e3 * o.rtol}));
     int status = PDN_OK;
     for (size_t s0 = 0; s0 < tsv_src.size() && status == PDN_OK; s0 += Bmax)
-        status = solve_batch(c, L, H, W, T, ch, tsv_src.data() + s0, (int)std::min<size_t>(Bmax, tsv_src.size() - s0), false, o.rtol, o.max_iter);
+        status = solve_batch(c, L, H, W, T, ch, tsv_src.data() + s0, (int)std::min<size_t>(Bmax, tsv_src.size() - s0), false, o.rtol, o.max_iter, guess);
     if (!term.empty()) {
         // with the terminal rows kept they are ordinary rows of ZT: full tolerance, gathered at every port
         const bool rows = c->terminal_pairs;
         for (size_t s0 = 0; s0 < term.size() && status == PDN_OK; s0 += Bmax)
             status = solve_batch(c, L, H, W, T, ch, term.data() + s0, (int)std::min<size_t>(Bmax, term.size() - s0), !rows,
-                                 rows ? o.rtol : rtol_term, o.max_iter);
+                                 rows ? o.rtol : rtol_term, o.max_iter, guess);
         if (rows && status == PDN_OK && !c->open)  // (an open, sharded context does this in pdn_finish)
             L.run(KC_SMALL, 0, [&] { k_zdiag_from_rows<<<cdiv(T.nterm, 128), 128, 0, L.s>>>(T.ZT.as<double>(), T.q, T.ntsv, T.nterm, T.zdiag.as<double>()); });
     }
@@ -288,6 +339,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         c->stats.n_tiers = d;
 
         // ---- S0 + S1, tier by tier
+        SpectralTables tabs;
         Hierarchy H;
         H.allocate(n);
         c->stats.n_levels = H.nlev;
@@ -325,7 +377,7 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
             std::vector<int> tsv_src, term_src;
             for (int k = (int)((int64_t)r_ * T.ntsv / W_); k < (int)((int64_t)(r_ + 1) * T.ntsv / W_); ++k) tsv_src.push_back(k);
             for (int k = (int)((int64_t)r_ * T.nterm / W_); k < (int)((int64_t)(r_ + 1) * T.nterm / W_); ++k) term_src.push_back(T.ntsv + k);
-            status = reduce_tier(c, L, H, W, Bmax, T, tsv_src, term_src);
+            status = reduce_tier(c, L, H, W, Bmax, T, tsv_src, term_src, tabs);
             if (status != PDN_OK) g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status);
         }
         CK(cudaEventRecord(ev[2], L.s));
@@ -396,6 +448,7 @@ int pdn_update_tsvs(pdn_ctx* ctx, int32_t n_tsv, const pdn_tsv* tsvs) {
                 if (it != where.end()) o2n[i][k] = it->second;
             }
         }
+        SpectralTables tabs;
         Hierarchy H;
         bool h_ready = false;
         int64_t new_solves = 0;
@@ -445,7 +498,7 @@ int pdn_update_tsvs(pdn_ctx* ctx, int32_t n_tsv, const pdn_tsv* tsvs) {
                 const int Bmax = pick_batch(H, (int)added.size(), c->opts);
                 Work W;
                 if (H.nlev > 1) W.allocate(H, Bmax, q_n);
-                status = reduce_tier(c, L, H, W, Bmax, N, added, {});
+                status = reduce_tier(c, L, H, W, Bmax, N, added, {}, tabs);
                 if (status != PDN_OK) { g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status); break; }
                 new_solves += (int64_t)added.size();
                 d_added.alloc(added.size() * sizeof(int));
@@ -669,6 +722,7 @@ int pdn_reff_nodes(pdn_ctx* ctx, int32_t n_nodes, const pdn_node* nodes, double*
         d_tier.alloc((size_t)np * sizeof(int));
         CK(cudaMemcpyAsync(d_tier.p, h_tier.data(), (size_t)np * sizeof(int), cudaMemcpyHostToDevice, L.s));
         // ---- one port solve per probe, tier by tier
+        SpectralTables tabs;
         Hierarchy H;
         bool h_ready = false;
         for (int t = 0; t < d && status == PDN_OK; ++t) {
@@ -693,7 +747,7 @@ int pdn_reff_nodes(pdn_ctx* ctx, int32_t n_nodes, const pdn_node* nodes, double*
             if (H.nlev > 1) W.allocate(H, Bmax, Tp.q);
             std::vector<int> src(k);
             for (int j = 0; j < k; ++j) src[j] = T.ntsv + j;
-            status = reduce_tier(c, L, H, W, Bmax, Tp, src, {});
+            status = reduce_tier(c, L, H, W, Bmax, Tp, src, {}, tabs);
             if (status != PDN_OK) { g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status); break; }
             DevBuf d_probe;
             d_probe.alloc((size_t)k * sizeof(int));

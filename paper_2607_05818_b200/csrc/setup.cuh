@@ -28,19 +28,25 @@ __global__ void k_import_planes(const double* __restrict__ gx_in, const double* 
 }
 
 // sums[0] += sum of the x-conductances, sums[1] += sum of the y-conductances (the tier's anisotropy, which
-// picks the smoothing interval of the Chebyshev polynomial; pdn_api.cu).
+// picks the smoothing interval of the Chebyshev polynomial; pdn_api.cu), sums[2], sums[3] += the sums of their
+// squares (how far the tier is from its mean mesh: whether the closed-form initial guess is worth trying).
 __global__ void k_plane_sums(int n_elems, const double* __restrict__ gx, const double* __restrict__ gy,
                              double* __restrict__ sums) {
     __shared__ double red[32];
-    double a = 0.0, b = 0.0;
+    double a = 0.0, b = 0.0, a2 = 0.0, b2 = 0.0;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_elems; i += gridDim.x * blockDim.x) {
-        a += gx[i];
-        b += gy[i];
+        const double u = gx[i], v = gy[i];
+        a += u; b += v;
+        a2 = fma(u, u, a2); b2 = fma(v, v, b2);
     }
     a = block_sum(a, red);
     if (threadIdx.x == 0) atomicAdd(sums, a);
     b = block_sum(b, red);
     if (threadIdx.x == 0) atomicAdd(sums + 1, b);
+    a2 = block_sum(a2, red);
+    if (threadIdx.x == 0) atomicAdd(sums + 2, a2);
+    b2 = block_sum(b2, red);
+    if (threadIdx.x == 0) atomicAdd(sums + 3, b2);
 }
 
 // sc = (s, sd) = (1/sqrt(d), sqrt(d)) in FP32, d = sum of incident conductances ((0,0) if the node is

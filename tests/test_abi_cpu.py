@@ -35,7 +35,7 @@ def test_struct_sizes_match_the_header_layout():
     from paper_2607_05818_b200 import binding as b
     assert ctypes.sizeof(b.PdnTier) == 24 and ctypes.sizeof(b.PdnTsv) == 24 and ctypes.sizeof(b.PdnSite) == 8
     assert ctypes.sizeof(b.PdnOpts) == 48
-    assert ctypes.sizeof(b.PdnStats) == 16 + 16 + 8 + 8 + 8 + 4 * 8 + 8 + 24 + 3 * 64
+    assert ctypes.sizeof(b.PdnStats) == 16 + 16 + 8 + 8 + 8 + 4 * 8 + 8 + 24 + 3 * 64 + 8
 
 
 def test_compute_calls_fail_loudly_without_a_device():
