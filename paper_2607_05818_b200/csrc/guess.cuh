@@ -18,10 +18,36 @@
 namespace pdn {
 
 struct GuessTable {
-    const float* G;  // table of (rho, 1), (n+1) x (n+1)
-    double scale;    // 1 / mean g_y
+    const float* G;   // table of (rho, 1), (n+1) x (n+1)
+    const float2* P;  // the same values as pairs (G[t][s], G[t][s+1])
+    double scale;     // 1 / mean g_y
     int n;
 };
+
+// columns a, b = a +- 1 of table row t with one 8-byte load
+__device__ __forceinline__ void guess_pair(const GuessTable& t, int row, int a, int b, float& va, float& vb) {
+    const float2 v = __ldg(t.P + (size_t)row * (t.n + 1) + min(a, b));
+    va = a < b ? v.x : v.y;
+    vb = a < b ? v.y : v.x;
+}
+
+// x0 at the two nodes (y, x) and (y, x + 1): bit-identical to guess_x0 of each (same values, same association)
+__device__ __forceinline__ void guess_x0_pair(const GuessTable& t, int y, int x, int ys, int xs, double& v0, double& v1) {
+    const int n = t.n, dy = abs(y - ys);
+    int sy = y + ys + 1;
+    sy = sy <= n ? sy : 2 * n - sy;
+    const int dxa = abs(x - xs), dxb = abs(x + 1 - xs);
+    int sxa = x + xs + 1, sxb = x + xs + 2;
+    sxa = sxa <= n ? sxa : 2 * n - sxa;
+    sxb = sxb <= n ? sxb : 2 * n - sxb;
+    float ddA, ddB, dsA, dsB, sdA, sdB, ssA, ssB;  // G[dy][dx], G[dy][sx], G[sy][dx], G[sy][sx] at nodes A, B
+    guess_pair(t, dy, dxa, dxb, ddA, ddB);
+    guess_pair(t, dy, sxa, sxb, dsA, dsB);
+    guess_pair(t, sy, dxa, dxb, sdA, sdB);
+    guess_pair(t, sy, sxa, sxb, ssA, ssB);
+    v0 = t.scale * (0.25 * (((double)ddA + (double)ssA) + ((double)dsA + (double)sdA)));
+    v1 = t.scale * (0.25 * (((double)ddB + (double)ssB) + ((double)dsB + (double)sdB)));
+}
 
 __device__ __forceinline__ double guess_x0(const GuessTable& t, int y, int x, int ys, int xs) {
     return t.scale * spectral_entry<float>(t.G, t.n, y, x, ys, xs);
@@ -57,9 +83,18 @@ k_guess_rhs(GuessTable tab, Level L, const int* __restrict__ node, const int* __
     for (int b = blockIdx.y * GR; b < b_end; ++b, buf ^= 1) {
         const int so = node[src[b]], ys = so / L.pitch, xs = so % L.pitch;
         double* xt = xs0[buf];
-        for (int i = tid; i < XH * XW; i += GUESS_THREADS) {
-            const int y = ty0 + i / XW - 1, x = tx0 + i % XW - 1;
-            xt[i] = (y >= 0 && y < L.ny && x >= 0 && x < L.nx) ? guess_x0(tab, y, x, ys, xs) : 0.0;
+        for (int i = tid; i < XH * (XW / 2); i += GUESS_THREADS) {  // two neighbouring columns per step
+            const int ry = i / (XW / 2), rx = 2 * (i % (XW / 2)), y = ty0 + ry - 1, x = tx0 + rx - 1;
+            double v0 = 0.0, v1 = 0.0;
+            if (y >= 0 && y < L.ny) {
+                if (x >= 0 && x + 1 < L.nx) guess_x0_pair(tab, y, x, ys, xs, v0, v1);
+                else {
+                    if (x >= 0 && x < L.nx) v0 = guess_x0(tab, y, x, ys, xs);
+                    if (x + 1 >= 0 && x + 1 < L.nx) v1 = guess_x0(tab, y, x + 1, ys, xs);
+                }
+            }
+            xt[ry * XW + rx] = v0;
+            xt[ry * XW + rx + 1] = v1;
         }
         __syncthreads();  // (also orders the coefficient tiles on the first pass)
         double rr = 0.0, sx = 0.0;
@@ -104,9 +139,18 @@ k_guess_dot(GuessTable tab, int ny, int nx, int pitch, size_t plane, const int* 
     const double* r = (rbuf_of[b] ? rb : ra) + b * plane;
     const int so = node[src[b]], ys = so / pitch, xs = so % pitch;
     double s = 0.0;
-    for (int i = threadIdx.x; i < GDOT_T * GDOT_T; i += 256) {
-        const int y = ty0 + i / GDOT_T, x = tx0 + i % GDOT_T;
-        if (y < ny && x < nx) s = fma(guess_x0(tab, y, x, ys, xs), r[(size_t)y * pitch + x], s);
+    for (int i = threadIdx.x; i < GDOT_T * (GDOT_T / 2); i += 256) {  // two neighbouring columns per step
+        const int y = ty0 + i / (GDOT_T / 2), x = tx0 + 2 * (i % (GDOT_T / 2));
+        if (y >= ny || x >= nx) continue;
+        if (x + 1 < nx) {
+            double v0, v1;
+            guess_x0_pair(tab, y, x, ys, xs, v0, v1);
+            const double2 rv = *reinterpret_cast<const double2*>(r + (size_t)y * pitch + x);  // x and pitch are even
+            s = fma(v0, rv.x, s);
+            s = fma(v1, rv.y, s);
+        } else {
+            s = fma(guess_x0(tab, y, x, ys, xs), r[(size_t)y * pitch + x], s);
+        }
     }
     s = warp_sum(s);
     if ((threadIdx.x & 31) == 0) atomicAdd(dot + b, s);

@@ -250,7 +250,7 @@ void launch_up3(Launcher& L, int cls, double bytes, const Level& lv, const Smoot
 
 void launch_pq3(Launcher& L, double bytes, const Level& lv, const Smoother& sm, int B, const CUtensorMap& m_z,
                 const CUtensorMap& m_p, const double* beta, double* p_new, double* q, double* pq_acc, double* sump_acc,
-                const int* active) {
+                const int* active, bool first) {
     constexpr int H = 2, IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
     const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G, T3_MAX_G_PQ);
     dim3 grid(tx, ty, cdiv(B, G));
@@ -259,7 +259,7 @@ void launch_pq3(Launcher& L, double bytes, const Level& lv, const Smoother& sm, 
     once_per_device(attr_done, [&] {
         CK(cudaFuncSetAttribute(k_pq3<PQ_R, PQ_W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     });
-    L.run(KC_PQ, bytes, [&] { k_pq3<PQ_R, PQ_W><<<grid, 32 * PQ_W, smem, L.s>>>(m_z, m_p, lv, beta, p_new, q, pq_acc, sump_acc, B, G, active); });
+    L.run(KC_PQ, bytes, [&] { k_pq3<PQ_R, PQ_W><<<grid, 32 * PQ_W, smem, L.s>>>(m_z, m_p, lv, beta, p_new, q, pq_acc, sump_acc, B, G, active, first ? 1 : 0); });
 }
 
 #define NU_DISPATCH(nu, CALL0)                \
@@ -370,7 +370,8 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
         const int GR = std::max(1, std::min(16, (int)((long)tiles * B / (148L * 8))));
         L.run(KC_SMALL, V, [&] { k_guess_rhs<<<dim3(tiles, cdiv(B, GR)), GUESS_THREADS, 0, L.s>>>(*guess, H.lev[0], node, src, 1.0 / (double)n2, W.r[0].as<double>(), W.g_rr0, W.g_sumx, B, GR); });
         L.run(KC_SMALL, 0, [&] { k_guess_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.g_rr0, bnorm2, W.g_keep, B); });
-        L.run(KC_SMALL, 0, [&] { k_init_rhs<<<dim3(std::min(1024u, cdiv(plane / 2, 256)), B), 256, 0, L.s>>>(W.r[0].as<double>(), n, H.pitch[0], plane, 1.0 / (double)n2, node, src, B, W.g_keep); });
+        // (a small grid: nearly every block returns at once -- a rejected guess is the exception)
+        L.run(KC_SMALL, 0, [&] { k_init_rhs<<<dim3(std::min(32u, cdiv(plane / 2, 256)), B), 256, 0, L.s>>>(W.r[0].as<double>(), n, H.pitch[0], plane, 1.0 / (double)n2, node, src, B, W.g_keep); });
         L.run(KC_SMALL, 0, [&] { k_guess_ports<<<dim3(cdiv(std::max(ngather, 1), 128), B), 128, 0, L.s>>>(*guess, H.pitch[0], node, ngather, src, W.g_keep, W.g_sumx, 1.0 / (double)n2, W.xport.as<double>(), W.xown.as<double>(), W.s.xmean, B); });
     } else {
         L.run(KC_SMALL, V, [&] { k_init_rhs<<<dim3(std::min(1024u, cdiv(plane / 2, 256)), B), 256, 0, L.s>>>(W.r[0].as<double>(), n, H.pitch[0], plane, 1.0 / (double)n2, node, src, B); });
@@ -385,7 +386,7 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     int skipped = 0;                       // consecutive iterations whose outcome the host did not read
     while (true) {
         L.run(KC_SMALL, 0, [&] { k_scal_beta<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, it == 0); });
-        launch_pq3(L, 4.0 * V * nact / B, H.lev[0], sm, B, W.m_z, W.m_p[cur_p], W.s.beta, W.p[cur_p ^ 1].as<double>(), W.q.as<double>(), W.s.pq, W.s.sump, W.s.active);
+        launch_pq3(L, (it == 0 ? 3.0 : 4.0) * V * nact / B, H.lev[0], sm, B, W.m_z, W.m_p[cur_p], W.s.beta, W.p[cur_p ^ 1].as<double>(), W.q.as<double>(), W.s.pq, W.s.sump, W.s.active, it == 0);
         cur_p ^= 1;
         L.run(KC_SMALL, 0, [&] { k_scal_alpha<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, 1.0 / (double)n2); });
         L.run(KC_SMALL, 0, [&] { k_xport<<<dim3(cdiv(std::max(ngather, 1), 128), B), 128, 0, L.s>>>(W.p[cur_p].as<double>(), plane, W.s.alpha, node, ngather, src, W.xport.as<double>(), W.xown.as<double>(), B); });

@@ -468,7 +468,7 @@ __global__ void __launch_bounds__(32 * W, 1)
 k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensorMap tm_p, Level L,
       const double* __restrict__ beta, double* __restrict__ p_new, double* __restrict__ q,
       double* __restrict__ pq_acc, double* __restrict__ sump_acc, int B, int G,
-      const int* __restrict__ active) {
+      const int* __restrict__ active, int first) {  // first: beta = 0 for every right-hand side, p_old is not fetched
     constexpr int H = 2;  // one ring is needed; two keep the 16-byte column pairs aligned
     using Gm = Geom<R, W, H>;
     extern __shared__ __align__(128) double smem_dyn[];
@@ -505,9 +505,9 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
     const int nb = al.n;
     auto fetch = [&](int j) {  // thread 0 only
         const int st = j & 1;
-        mbar_expect_tx(&mbar[st], 2 * Gm::TILE_BYTES);
+        mbar_expect_tx(&mbar[st], (first ? 1 : 2) * Gm::TILE_BYTES);
         tma_load_3d(zbuf + st * Gm::TILE, &tm_z, x0, y0, al.b[j], &mbar[st]);
-        tma_load_3d(pbuf + st * Gm::TILE, &tm_p, x0, y0, al.b[j], &mbar[st]);
+        if (!first) tma_load_3d(pbuf + st * Gm::TILE, &tm_p, x0, y0, al.b[j], &mbar[st]);
     };
     if (threadIdx.x == 0 && nb > 0) {  // nb == 0: every right-hand side of the group has converged
         fetch(0);
@@ -532,7 +532,7 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
 #pragma unroll
         for (int i = 0; i < R; ++i) {
             double2 p = ld2(zbuf + st * Gm::TILE + slot0 + i * T3_EW);
-            if (bt != 0.0) {  // beta = 0 on the first iteration: p_old is not initialised then
+            if (!first && bt != 0.0) {  // beta = 0 on the first iteration: p_old is not initialised (nor fetched) then
                 const double2 po = ld2(pbuf + st * Gm::TILE + slot0 + i * T3_EW);
                 p.x = fma(bt, po.x, p.x);
                 p.y = fma(bt, po.y, p.y);
