@@ -47,9 +47,11 @@ struct ChebR {
 struct PcgScalars {
     double* rho;     // r.z of the current iteration
     double* rz;      // accumulator: r.z after the V-cycle
-    double* pq;      // accumulator: p.Lp
+    double* pq;      // accumulator: z.Lz of this iteration (k_pq3)
     double* rr;      // accumulator: ||r||^2
-    double* sump;    // accumulator: sum(p)
+    double* sump;    // accumulator: sum(z) of this iteration (k_pq3)
+    double* pap;     // p.Lp of the current direction, by recurrence: z.Lz - beta^2 p_old.Lp_old
+    double* psum;    // sum(p) of the current direction, by recurrence: sum(z) + beta sum(p_old)
     double* alpha;
     double* beta;
     double* xmean;   // mean of the (implicit) solution x = sum_k alpha_k p_k

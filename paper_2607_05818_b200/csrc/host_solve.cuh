@@ -143,11 +143,12 @@ struct Smoother {
 // S1 workspace of one batch of right-hand sides, with the TMA descriptor of every vector.
 struct Work {
     int Bmax = 0, qmax = 0;
-    DevBuf r[2], y0, z, p[2], q;                           // level 0 (ping-pong pairs: halos are read across blocks)
+    DevBuf r[2], y0, z, q;                                 // level 0 (r is a ping-pong pair: halos are read across blocks)
     DevBuf rl[MAX_LEVELS], ya[MAX_LEVELS], zb[MAX_LEVELS];  // levels >= 1: residual, scaled iterate, correction
-    CUtensorMap m_r[2], m_y0, m_z, m_p[2], m_q;
+    CUtensorMap m_r[2], m_y0, m_z, m_q;
     CUtensorMap m_rl[MAX_LEVELS], m_ya[MAX_LEVELS], m_ec[MAX_LEVELS];  // m_ec[l]: zb[l] as the coarse box of level l-1
-    DevBuf scal, xport, xown, iact, src;  // src: port index each right-hand side of the batch is the source of
+    DevBuf scal, xport, xown, pport, iact, src;  // pport: the search direction at the gathered nodes (+ B own nodes);
+                                                 // src: port index each right-hand side of the batch is the source of
     double *g_rr0 = nullptr, *g_sumx = nullptr, *g_dot = nullptr;  // initial guess (guess.cuh): ||r0||^2, sum(x0), x0.r_k per right-hand side
     int *g_keep = nullptr, *g_rbuf = nullptr;     // ... whether the guess is used; buffer of the last residual
     PcgScalars s{};
@@ -155,17 +156,17 @@ struct Work {
     double* h_relres = nullptr;                      // pinned, Bmax
 
     static size_t bytes_per_rhs(const Hierarchy& H) {
-        size_t b = 7 * H.plane(0);
+        size_t b = 5 * H.plane(0);
         for (int l = 1; l < H.nlev; ++l) b += 3 * H.plane(l);
         return b * sizeof(double);
     }
     void allocate(const Hierarchy& H, int B, int qmax_) {
         Bmax = B; qmax = qmax_;
         const size_t v0 = (size_t)B * H.plane(0) * sizeof(double);
-        for (int i = 0; i < 2; ++i) { r[i].alloc(v0); p[i].alloc(v0); }
+        for (int i = 0; i < 2; ++i) r[i].alloc(v0);
         y0.alloc(v0); z.alloc(v0); q.alloc(v0);
         auto fine = [&](const DevBuf& d, int l) { return make_map(d.p, H.nx[l], H.ny[l], H.pitch[l], B, T3_EW, T3_EH); };
-        for (int i = 0; i < 2; ++i) { m_r[i] = fine(r[i], 0); m_p[i] = fine(p[i], 0); }
+        for (int i = 0; i < 2; ++i) m_r[i] = fine(r[i], 0);
         m_y0 = fine(y0, 0); m_z = fine(z, 0); m_q = fine(q, 0);
         for (int l = 1; l < H.nlev; ++l) {
             const size_t vl = (size_t)B * H.plane(l) * sizeof(double);
@@ -173,11 +174,12 @@ struct Work {
             m_rl[l] = fine(rl[l], l); m_ya[l] = fine(ya[l], l);
             m_ec[l] = make_map(zb[l].p, H.nx[l], H.ny[l], H.pitch[l], B, T3_ECW, T3_EH / 2);
         }
-        scal.alloc((size_t)12 * B * sizeof(double));
+        scal.alloc((size_t)14 * B * sizeof(double));
         double* sp = scal.as<double>();
         s.rho = sp; s.rz = sp + B; s.pq = sp + 2 * B; s.rr = sp + 3 * B; s.sump = sp + 4 * B;
         s.alpha = sp + 5 * B; s.beta = sp + 6 * B; s.xmean = sp + 7 * B; s.relres = sp + 8 * B;
         g_rr0 = sp + 9 * B; g_sumx = sp + 10 * B; g_dot = sp + 11 * B;
+        s.pap = sp + 12 * B; s.psum = sp + 13 * B;
         iact.alloc((size_t)(3 * B + 1) * sizeof(int));
         s.active = iact.as<int>();
         s.n_active = iact.as<int>() + B;
@@ -185,6 +187,7 @@ struct Work {
         g_rbuf = iact.as<int>() + 2 * B + 1;
         xport.alloc((size_t)B * std::max(qmax, 1) * sizeof(double));
         xown.alloc((size_t)B * sizeof(double));
+        pport.alloc((size_t)B * (std::max(qmax, 1) + 1) * sizeof(double));
         src.alloc((size_t)B * sizeof(int));
         char* hp = static_cast<char*>(g_pinned.get(64 + (size_t)B * sizeof(double)));
         if (!hp) throw StatusFail{PDN_E_NOMEM, "pinned host allocation failed"};
@@ -249,17 +252,17 @@ void launch_up3(Launcher& L, int cls, double bytes, const Level& lv, const Smoot
 }
 
 void launch_pq3(Launcher& L, double bytes, const Level& lv, const Smoother& sm, int B, const CUtensorMap& m_z,
-                const CUtensorMap& m_p, const double* beta, double* p_new, double* q, double* pq_acc, double* sump_acc,
+                const CUtensorMap& m_q, const double* beta, double* q, double* zw_acc, double* sumz_acc,
                 const int* active, bool first) {
     constexpr int H = 2, IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
     const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G, T3_MAX_G_PQ);
     dim3 grid(tx, ty, cdiv(B, G));
-    constexpr size_t smem = 4 * T3_TILE_BYTES + sizeof(Exch<PQ_W>);
+    constexpr size_t smem = 5 * T3_TILE_BYTES + sizeof(Exch<PQ_W>);  // 2 z stages + 3 q slots
     static std::atomic<uint64_t> attr_done{0};
     once_per_device(attr_done, [&] {
         CK(cudaFuncSetAttribute(k_pq3<PQ_R, PQ_W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     });
-    L.run(KC_PQ, bytes, [&] { k_pq3<PQ_R, PQ_W><<<grid, 32 * PQ_W, smem, L.s>>>(m_z, m_p, lv, beta, p_new, q, pq_acc, sump_acc, B, G, active, first ? 1 : 0); });
+    L.run(KC_PQ, bytes, [&] { k_pq3<PQ_R, PQ_W><<<grid, 32 * PQ_W, smem, L.s>>>(m_z, m_q, lv, beta, q, zw_acc, sumz_acc, B, G, active, first ? 1 : 0); });
 }
 
 #define NU_DISPATCH(nu, CALL0)                \
@@ -359,7 +362,7 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     const double V = (double)B * n2 * 8.0;
     const int* node = T.d_node.as<int>();
     const int ngather = terminal ? 0 : T.q;
-    int cur_r = 0, cur_p = 0;
+    int cur_r = 0;
     const double bnorm2 = 1.0 - 1.0 / (double)n2;
     L.run(KC_SMALL, 0, [&] { k_pcg_init<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B); });
     if (guess) {
@@ -386,10 +389,9 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     int skipped = 0;                       // consecutive iterations whose outcome the host did not read
     while (true) {
         L.run(KC_SMALL, 0, [&] { k_scal_beta<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, it == 0); });
-        launch_pq3(L, (it == 0 ? 3.0 : 4.0) * V * nact / B, H.lev[0], sm, B, W.m_z, W.m_p[cur_p], W.s.beta, W.p[cur_p ^ 1].as<double>(), W.q.as<double>(), W.s.pq, W.s.sump, W.s.active, it == 0);
-        cur_p ^= 1;
+        launch_pq3(L, (it == 0 ? 2.0 : 3.0) * V * nact / B, H.lev[0], sm, B, W.m_z, W.m_q, W.s.beta, W.q.as<double>(), W.s.pq, W.s.sump, W.s.active, it == 0);
         L.run(KC_SMALL, 0, [&] { k_scal_alpha<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, 1.0 / (double)n2); });
-        L.run(KC_SMALL, 0, [&] { k_xport<<<dim3(cdiv(std::max(ngather, 1), 128), B), 128, 0, L.s>>>(W.p[cur_p].as<double>(), plane, W.s.alpha, node, ngather, src, W.xport.as<double>(), W.xown.as<double>(), B); });
+        L.run(KC_SMALL, 0, [&] { k_xport<<<dim3(cdiv(std::max(ngather, 1), 128), B), 128, 0, L.s>>>(W.z.as<double>(), plane, W.s.alpha, W.s.beta, node, ngather, src, W.pport.as<double>(), W.pport.as<double>() + (size_t)B * std::max(ngather, 1), W.xport.as<double>(), W.xown.as<double>(), B, it == 0 ? 1 : 0); });
         ++it;
         bool done = false;
         int r_new = cur_r ^ 1;  // the buffer this iteration's residual update writes

@@ -32,7 +32,7 @@ __global__ void k_pcg_init(PcgScalars s, int B) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b == 0) *s.n_active = B;
     if (b >= B) return;
-    s.rho[b] = 1.0; s.rz[b] = 0.0; s.pq[b] = 0.0; s.rr[b] = 0.0; s.sump[b] = 0.0;
+    s.rho[b] = 1.0; s.rz[b] = 0.0; s.pq[b] = 0.0; s.rr[b] = 0.0; s.sump[b] = 0.0; s.pap[b] = 0.0; s.psum[b] = 0.0;
     s.alpha[b] = 0.0; s.beta[b] = 0.0; s.xmean[b] = 0.0; s.relres[b] = 1.0; s.active[b] = 1;
 }
 
@@ -48,15 +48,23 @@ __global__ void k_scal_beta(PcgScalars s, int B, int first) {
     s.sump[b] = 0.0;
 }
 
-// After q = L p: alpha = rho / pq (0 when frozen); xmean += alpha * sum(p) / n2.
+// After w = L z, q = w + beta q_old (k_pq3).  The direction p = z + beta p_old is implicit:
+//   p.Lp   = z.Lz - beta^2 p_old.Lp_old     (p is L-conjugate to p_old, so z.Lp_old = -beta p_old.Lp_old)
+//   sum(p) = sum(z) + beta sum(p_old)
+// alpha = rho / p.Lp (0 when frozen); xmean += alpha * sum(p) / n2.
 __global__ void k_scal_alpha(PcgScalars s, int B, double inv_n2) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b == 0) *s.n_active = 0;  // counted again by k_scal_check
     if (b >= B) return;
-    const double pq = s.pq[b];
-    const double a = (s.active[b] && pq > 0.0) ? s.rho[b] / pq : 0.0;
+    if (!s.active[b]) { s.alpha[b] = 0.0; s.rr[b] = 0.0; return; }  // frozen: nothing of it is maintained any more
+    const double bt = s.beta[b];
+    const double pap = fma(-bt * bt, s.pap[b], s.pq[b]);
+    const double psum = fma(bt, s.psum[b], s.sump[b]);
+    s.pap[b] = pap;
+    s.psum[b] = psum;
+    const double a = pap > 0.0 ? s.rho[b] / pap : 0.0;
     s.alpha[b] = a;
-    s.xmean[b] = fma(a * inv_n2, s.sump[b], s.xmean[b]);
+    s.xmean[b] = fma(a * inv_n2, psum, s.xmean[b]);
     s.rr[b] = 0.0;
 }
 
@@ -109,19 +117,31 @@ k_resid_update(const double* __restrict__ r_in, const double* __restrict__ q, co
     if (threadIdx.x == 0) atomicAdd(rr_acc + b, rr);
 }
 
-// x_port[b][k] += alpha[b] * p[b][node[k]],  k over the gather list (all ports of the tier for a
-// TSV-source batch; for a terminal batch ngather == 0 and only the source node itself is read).
-__global__ void k_xport(const double* __restrict__ p, size_t n2, const double* __restrict__ alpha,
-                        const int* __restrict__ node, int ngather, const int* __restrict__ src,
-                        double* __restrict__ xport, double* __restrict__ xown, int B) {
+// The search direction exists only at the gathered nodes:  pp = z[b][node] + beta[b] * pp  (pp = z on the first
+// iteration), then  x_port[b][k] += alpha[b] * pp[b][k],  k over the gather list (all ports of the tier for a
+// TSV-source batch; for a terminal batch ngather == 0 and only the source node itself is kept, in pown / xown).
+__global__ void k_xport(const double* __restrict__ z, size_t n2, const double* __restrict__ alpha,
+                        const double* __restrict__ beta, const int* __restrict__ node, int ngather,
+                        const int* __restrict__ src, double* __restrict__ pport, double* __restrict__ pown,
+                        double* __restrict__ xport, double* __restrict__ xown, int B, int first) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     const int b = blockIdx.y;
     const double a = alpha[b];
-    if (a == 0.0) return;  // frozen right-hand side: its p is no longer maintained
+    if (a == 0.0) return;  // frozen right-hand side: its z is no longer maintained
+    const double bt = beta[b];
     if (ngather > 0) {
-        if (k < ngather) xport[(size_t)b * ngather + k] = fma(a, p[b * n2 + node[k]], xport[(size_t)b * ngather + k]);
+        if (k < ngather) {
+            const size_t i = (size_t)b * ngather + k;
+            const double zz = z[b * n2 + node[k]];
+            const double pp = first ? zz : fma(bt, pport[i], zz);
+            pport[i] = pp;
+            xport[i] = fma(a, pp, xport[i]);
+        }
     } else if (k == 0) {
-        xown[b] = fma(a, p[b * n2 + node[src[b]]], xown[b]);
+        const double zz = z[b * n2 + node[src[b]]];
+        const double pp = first ? zz : fma(bt, pown[b], zz);
+        pown[b] = pp;
+        xown[b] = fma(a, pp, xown[b]);
     }
 }
 

@@ -468,22 +468,32 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
 }
 
 // ---------------------------------------------------------------------------------------------
-// CG direction update fused with the operator apply (level 0), on the UNSCALED operator (this is the
-// matrix CG solves with, so it uses the raw conductances):
-//   p = z + beta p_old ;  q = L p = d p - sum_nb g_nb p_nb ;  pq += p.q ;  sump += sum(p)
+// Operator apply of the CG iteration (level 0), on the UNSCALED operator (this is the matrix CG solves with, so it
+// uses the raw conductances), with the direction kept implicit:
+//   w = L z = d z - sum_nb g_nb z_nb ;  q = w + beta q_old   (= L p for p = z + beta p_old, by linearity) ;
+//   zw += z.w ;  sumz += sum(z)
+// The search direction p itself is never stored: CG needs it only at the port nodes (x_port += alpha p[port]; pcg.cuh
+// keeps p[port] = z[port] + beta p_old[port]) and in the scalars p.Lp = z.w - beta^2 p_old.Lp_old (L-conjugacy of
+// consecutive directions) and sum(p) = sum(z) + beta sum(p_old) (k_scal_alpha).  That is one vector written and one
+// read per iteration less than the textbook update (3 V instead of 4 V).  q is updated in place: a block reads and
+// writes q only at its own interior nodes.
+// Shared memory: z tiles in two stages (refilled after the apply, as in the V-cycle kernels), q tiles in a ring of
+// three (a q tile is consumed at the END of its iteration, so its slot is refilled one iteration later, with the
+// right-hand side three ahead: the same two iterations of prefetch lead as z).
 template <int R, int W>
 __global__ void __launch_bounds__(32 * W, 1)
-k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensorMap tm_p, Level L,
-      const double* __restrict__ beta, double* __restrict__ p_new, double* __restrict__ q,
-      double* __restrict__ pq_acc, double* __restrict__ sump_acc, int B, int G,
-      const int* __restrict__ active, int first) {  // first: beta = 0 for every right-hand side, p_old is not fetched
+k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensorMap tm_q, Level L,
+      const double* __restrict__ beta, double* __restrict__ q, double* __restrict__ zw_acc,
+      double* __restrict__ sumz_acc, int B, int G, const int* __restrict__ active,
+      int first) {  // first: beta = 0 for every right-hand side, q_old is not fetched (it does not exist yet)
     constexpr int H = 2;  // one ring is needed; two keep the 16-byte column pairs aligned
     using Gm = Geom<R, W, H>;
     extern __shared__ __align__(128) double smem_dyn[];
-    double* zbuf = smem_dyn;             // 2 stages each
-    double* pbuf = zbuf + 2 * Gm::TILE;
-    Exch<W>& x = *reinterpret_cast<Exch<W>*>(pbuf + 2 * Gm::TILE);
-    __shared__ uint64_t mbar[3];  // two TMA stages + the row-exchange barrier
+    double* zbuf = smem_dyn;             // 2 stages
+    double* qbuf = zbuf + 2 * Gm::TILE;  // 3 slots
+    Exch<W>& x = *reinterpret_cast<Exch<W>*>(qbuf + 3 * Gm::TILE);
+    __shared__ uint64_t mbar[3];  // two z stages + the row-exchange barrier
+    __shared__ uint64_t mbq[3];   // the q ring
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int x0 = blockIdx.x * Gm::IW - H, y0 = blockIdx.y * Gm::IH - H;
@@ -507,64 +517,77 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
     active_list_build(al, active, blockIdx.z * G, min(G, B - (int)blockIdx.z * G), beta);
     if (threadIdx.x == 0) {
         mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); mbar_init(&mbar[2], 32 * W);
+        mbar_init(&mbq[0], 1); mbar_init(&mbq[1], 1); mbar_init(&mbq[2], 1);
         mbar_fence_init();
     }
     __syncthreads();
     const int nb = al.n;
-    auto fetch = [&](int j) {  // thread 0 only
+    auto fetch_z = [&](int j) {  // thread 0 only
         const int st = j & 1;
-        mbar_expect_tx(&mbar[st], (first ? 1 : 2) * Gm::TILE_BYTES);
+        mbar_expect_tx(&mbar[st], Gm::TILE_BYTES);
         tma_load_3d(zbuf + st * Gm::TILE, &tm_z, x0, y0, al.b[j], &mbar[st]);
-        if (!first) tma_load_3d(pbuf + st * Gm::TILE, &tm_p, x0, y0, al.b[j], &mbar[st]);
+    };
+    auto fetch_q = [&](int j) {  // thread 0 only
+        const int sq = j % 3;
+        mbar_expect_tx(&mbq[sq], Gm::TILE_BYTES);
+        tma_load_3d(qbuf + sq * Gm::TILE, &tm_q, x0, y0, al.b[j], &mbq[sq]);
     };
     if (threadIdx.x == 0 && nb > 0) {  // nb == 0: every right-hand side of the group has converged
-        fetch(0);
-        if (nb > 1) fetch(1);
+        fetch_z(0);
+        if (nb > 1) fetch_z(1);
+        if (!first)
+            for (int j = 0; j < 3 && j < nb; ++j) fetch_q(j);
     }
     Xchg<W> xc{&x, &mbar[2], 0, 0u, warp, lane};
-    double pq_pend = 0.0, sump_pend = 0.0;  // partials of the previous right-hand side, reduced one iteration later
+    double zw_pend = 0.0, sumz_pend = 0.0;  // partials of the previous right-hand side, reduced one iteration later
     int b_pend = -1;
     auto flush = [&] {
-        pq_pend = warp_sum(pq_pend);
-        sump_pend = warp_sum(sump_pend);
+        zw_pend = warp_sum(zw_pend);
+        sumz_pend = warp_sum(sumz_pend);
         if (lane == 0) {
-            atomicAdd(pq_acc + b_pend, pq_pend);
-            atomicAdd(sump_acc + b_pend, sump_pend);
+            atomicAdd(zw_acc + b_pend, zw_pend);
+            atomicAdd(sumz_acc + b_pend, sumz_pend);
         }
     };
     for (int j = 0; j < nb; ++j) {
-        const int b = al.b[j], st = j & 1;
+        const int b = al.b[j], st = j & 1, sq = j % 3;
         mbar_wait(&mbar[st], (j >> 1) & 1);
         const double bt = al.s[j];
-        double p0[R], p1[R], sump = 0.0, pq = 0.0;
+        double z0[R], z1[R], sumz = 0.0, zw = 0.0;
 #pragma unroll
         for (int i = 0; i < R; ++i) {
-            double2 p = ld2(zbuf + st * Gm::TILE + slot0 + i * T3_EW);
-            if (!first && bt != 0.0) {  // beta = 0 on the first iteration: p_old is not initialised (nor fetched) then
-                const double2 po = ld2(pbuf + st * Gm::TILE + slot0 + i * T3_EW);
-                p.x = fma(bt, po.x, p.x);
-                p.y = fma(bt, po.y, p.y);
-            }
-            const bool in = (interior >> i) & 1;
-            if (in) st2(p_new + b * plane + goff + (size_t)i * L.pitch, p);
-            sump += in ? p.x + p.y : 0.0;
-            p0[i] = p.x;
-            p1[i] = p.y;
+            const double2 zz = ld2(zbuf + st * Gm::TILE + slot0 + i * T3_EW);
+            sumz += ((interior >> i) & 1) ? zz.x + zz.y : 0.0;
+            z0[i] = zz.x;
+            z1[i] = zz.y;
         }
         if (b_pend >= 0) flush();
         double t0[R], t1[R];
-        apply_step<R, W, double>(xc, c, p0, p1, zero, zero, t0, t1);
-        if (threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
+        apply_step<R, W, double>(xc, c, z0, z1, zero, zero, t0, t1);
+        // past this exchange every thread has read its z tile of this iteration and its q tile of the previous one
+        if (threadIdx.x == 0 && j + 2 < nb) {
+            fetch_z(j + 2);
+            if (!first && j >= 1) fetch_q(j + 2);  // slot (j+2) % 3 = (j-1) % 3
+        }
+        if (!first) mbar_wait(&mbq[sq], (j / 3) & 1);
+        double* qp = q + b * plane + goff;
 #pragma unroll
         for (int i = 0; i < R; ++i) {
             const bool in = (interior >> i) & 1;
-            const double q0 = fma(d0[i], p0[i], -t0[i]), q1 = fma(d1[i], p1[i], -t1[i]);
-            if (in) st2(q + b * plane + goff + (size_t)i * L.pitch, make_double2(q0, q1));
-            pq = fma(in ? p0[i] : 0.0, q0, pq);
-            pq = fma(in ? p1[i] : 0.0, q1, pq);
+            const double w0 = fma(d0[i], z0[i], -t0[i]), w1 = fma(d1[i], z1[i], -t1[i]);
+            double q0 = w0, q1 = w1;
+            if (!first) {
+                const double2 qo = ld2(qbuf + sq * Gm::TILE + slot0 + i * T3_EW);
+                q0 = fma(bt, qo.x, w0);
+                q1 = fma(bt, qo.y, w1);
+            }
+            if (in) st2(qp, make_double2(q0, q1));
+            qp += L.pitch;
+            zw = fma(in ? z0[i] : 0.0, w0, zw);
+            zw = fma(in ? z1[i] : 0.0, w1, zw);
         }
-        pq_pend = pq;
-        sump_pend = sump;
+        zw_pend = zw;
+        sumz_pend = sumz;
         b_pend = b;
     }
     if (b_pend >= 0) flush();
