@@ -54,28 +54,47 @@ __device__ __forceinline__ double guess_x0(const GuessTable& t, int y, int x, in
 }
 
 // r0[b] = b - L x0 on the pitched plane, rr0[b] += ||r0||^2, sumx[b] += sum(x0).
-// grid = (tiles_x * tiles_y, ceil(B / GR)); block = GUESS_THREADS; a block keeps the raw conductances of its
-// GUESS_TY x GUESS_TX tile in shared memory and loops over GR right-hand sides; per right-hand side it tabulates x0
-// on the tile plus one ring (shared memory, double buffered: one __syncthreads per right-hand side) and applies
-// the 5-point operator.
+// grid = (tiles_x * tiles_y, ceil(B / GR)); block = GUESS_THREADS; a thread keeps the raw conductances of its four
+// nodes of the GUESS_TY x GUESS_TX tile in registers and loops over GR right-hand sides; per right-hand side the block
+// tabulates x0 on the tile plus one ring (shared memory, double buffered: one __syncthreads per right-hand side) and
+// applies the 5-point operator.  Everything that does not depend on the right-hand side (which table entries a
+// thread evaluates, its nodes, their coefficients) is set up once per block: the kernel is instruction-bound.
 constexpr int GUESS_TX = 64, GUESS_TY = 16, GUESS_THREADS = 256;
 __global__ void __launch_bounds__(GUESS_THREADS)
 k_guess_rhs(GuessTable tab, Level L, const int* __restrict__ node, const int* __restrict__ src, double inv_n2,
             double* __restrict__ r0, double* __restrict__ rr0, double* __restrict__ sumx, int B, int GR) {
-    constexpr int XW = GUESS_TX + 2, XH = GUESS_TY + 2;
-    __shared__ double xs0[2][XH * XW];
-    __shared__ double gE[GUESS_TY][GUESS_TX + 1];   // gE[y][x+1] = conductance (y, x)-(y, x+1); gE[y][0] = west of column 0
-    __shared__ double gS[GUESS_TY + 1][GUESS_TX];   // gS[y+1][x] = conductance (y, x)-(y+1, x); gS[0][x] = north of row 0
+    constexpr int XW = GUESS_TX + 2, XH = GUESS_TY + 2, NPAIR = XH * (XW / 2);
+    constexpr int PER = (NPAIR + GUESS_THREADS - 1) / GUESS_THREADS;       // pair entries of the ring tile per thread
+    constexpr int NODES = GUESS_TY * GUESS_TX / GUESS_THREADS;             // tile nodes per thread (same column)
+    static_assert(GUESS_THREADS % GUESS_TX == 0 && (GUESS_TY * GUESS_TX) % GUESS_THREADS == 0, "tile / block shape");
+    __shared__ __align__(16) double xs0[2][XH * XW];
     const int tiles_x = (L.nx + GUESS_TX - 1) / GUESS_TX;
     const int tx0 = (blockIdx.x % tiles_x) * GUESS_TX, ty0 = (blockIdx.x / tiles_x) * GUESS_TY;
     const int tid = threadIdx.x, lane = tid & 31;
-    for (int i = tid; i < GUESS_TY * (GUESS_TX + 1); i += GUESS_THREADS) {
-        const int y = ty0 + i / (GUESS_TX + 1), x = tx0 + i % (GUESS_TX + 1) - 1;
-        gE[i / (GUESS_TX + 1)][i % (GUESS_TX + 1)] = (y < L.ny && x >= 0 && x < L.nx) ? L.gx[(size_t)y * L.pitch + x] : 0.0;
+    // ---- per-thread constants of the tabulation: entry k covers ring-tile columns rx, rx+1 of ring-tile row ry
+    int ey[PER], ex[PER], eo[PER], ekind[PER];  // mesh row, mesh column of the first node, offset in xs0, 0 none / 1 pair / 2 singles
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+        const int i = tid + k * GUESS_THREADS, ry = i / (XW / 2), rx = 2 * (i % (XW / 2));
+        ey[k] = ty0 + ry - 1; ex[k] = tx0 + rx - 1; eo[k] = ry * XW + rx;
+        const bool row_ok = i < NPAIR && ey[k] >= 0 && ey[k] < L.ny;
+        ekind[k] = i >= NPAIR ? -1 : !row_ok ? 0 : (ex[k] >= 0 && ex[k] + 1 < L.nx) ? 1 : 2;
     }
-    for (int i = tid; i < (GUESS_TY + 1) * GUESS_TX; i += GUESS_THREADS) {
-        const int y = ty0 + i / GUESS_TX - 1, x = tx0 + i % GUESS_TX;
-        gS[i / GUESS_TX][i % GUESS_TX] = (y >= 0 && y < L.ny && x < L.nx) ? L.gy[(size_t)y * L.pitch + x] : 0.0;
+    // ---- per-thread constants of the operator: nodes (ly0 + k * step, lx), their four conductances
+    const int lx = tid % GUESS_TX, ly0 = tid / GUESS_TX, x = tx0 + lx;
+    constexpr int STEP = GUESS_THREADS / GUESS_TX;
+    double ge[NODES], gw[NODES], gs[NODES], gn[NODES];
+    int nkind[NODES];  // 0 outside the plane, 1 node, 2 pad column
+#pragma unroll
+    for (int k = 0; k < NODES; ++k) {
+        const int y = ty0 + ly0 + k * STEP;
+        nkind[k] = (y >= L.ny || x >= L.pitch) ? 0 : x >= L.nx ? 2 : 1;
+        const bool in = nkind[k] == 1;
+        const size_t o = (size_t)y * L.pitch + x;
+        ge[k] = in ? L.gx[o] : 0.0;                       // pad / last column of gx is zero
+        gw[k] = (in && x > 0) ? L.gx[o - 1] : 0.0;
+        gs[k] = in ? L.gy[o] : 0.0;                       // last row of gy is zero
+        gn[k] = (in && y > 0) ? L.gy[o - L.pitch] : 0.0;
     }
     const size_t plane = (size_t)L.ny * L.pitch;
     const int b_end = min(B, (int)(blockIdx.y + 1) * GR);
@@ -83,34 +102,34 @@ k_guess_rhs(GuessTable tab, Level L, const int* __restrict__ node, const int* __
     for (int b = blockIdx.y * GR; b < b_end; ++b, buf ^= 1) {
         const int so = node[src[b]], ys = so / L.pitch, xs = so % L.pitch;
         double* xt = xs0[buf];
-        for (int i = tid; i < XH * (XW / 2); i += GUESS_THREADS) {  // two neighbouring columns per step
-            const int ry = i / (XW / 2), rx = 2 * (i % (XW / 2)), y = ty0 + ry - 1, x = tx0 + rx - 1;
+#pragma unroll
+        for (int k = 0; k < PER; ++k) {
+            if (ekind[k] < 0) continue;
             double v0 = 0.0, v1 = 0.0;
-            if (y >= 0 && y < L.ny) {
-                if (x >= 0 && x + 1 < L.nx) guess_x0_pair(tab, y, x, ys, xs, v0, v1);
-                else {
-                    if (x >= 0 && x < L.nx) v0 = guess_x0(tab, y, x, ys, xs);
-                    if (x + 1 >= 0 && x + 1 < L.nx) v1 = guess_x0(tab, y, x + 1, ys, xs);
-                }
+            if (ekind[k] == 1) guess_x0_pair(tab, ey[k], ex[k], ys, xs, v0, v1);
+            else if (ekind[k] == 2) {
+                if (ex[k] >= 0 && ex[k] < L.nx) v0 = guess_x0(tab, ey[k], ex[k], ys, xs);
+                if (ex[k] + 1 >= 0 && ex[k] + 1 < L.nx) v1 = guess_x0(tab, ey[k], ex[k] + 1, ys, xs);
             }
-            xt[ry * XW + rx] = v0;
-            xt[ry * XW + rx + 1] = v1;
+            *reinterpret_cast<double2*>(xt + eo[k]) = make_double2(v0, v1);  // eo is even, XW is even
         }
-        __syncthreads();  // (also orders the coefficient tiles on the first pass)
+        __syncthreads();
         double rr = 0.0, sx = 0.0;
-        for (int i = tid; i < GUESS_TY * GUESS_TX; i += GUESS_THREADS) {
-            const int ly = i / GUESS_TX, lx = i % GUESS_TX, y = ty0 + ly, x = tx0 + lx;
-            if (y >= L.ny || x >= L.pitch) continue;
-            if (x >= L.nx) { r0[b * plane + (size_t)y * L.pitch + x] = 0.0; continue; }  // pad column of an odd-width plane
-            const double c = xt[(ly + 1) * XW + lx + 1];
-            const double e = gE[ly][lx + 1], w = gE[ly][lx], s = gS[ly + 1][lx], nn = gS[ly][lx];
+        double* rp = r0 + b * plane + (size_t)(ty0 + ly0) * L.pitch + x;
+#pragma unroll
+        for (int k = 0; k < NODES; ++k, rp += (size_t)STEP * L.pitch) {
+            if (nkind[k] == 0) continue;
+            if (nkind[k] == 2) { *rp = 0.0; continue; }  // pad column of an odd-width plane
+            const int ly = ly0 + k * STEP;
+            const double* xc = xt + (ly + 1) * XW + lx + 1;
+            const double c = xc[0];
             // (L x0)_i = sum over neighbours of g (x0_i - x0_nb); absent neighbours have g = 0
-            double lx0 = e * (c - xt[(ly + 1) * XW + lx + 2]);
-            lx0 = fma(w, c - xt[(ly + 1) * XW + lx], lx0);
-            lx0 = fma(s, c - xt[(ly + 2) * XW + lx + 1], lx0);
-            lx0 = fma(nn, c - xt[ly * XW + lx + 1], lx0);
-            const double r = ((y == ys && x == xs) ? 1.0 - inv_n2 : -inv_n2) - lx0;
-            r0[b * plane + (size_t)y * L.pitch + x] = r;
+            double lx0 = ge[k] * (c - xc[1]);
+            lx0 = fma(gw[k], c - xc[-1], lx0);
+            lx0 = fma(gs[k], c - xc[XW], lx0);
+            lx0 = fma(gn[k], c - xc[-XW], lx0);
+            const double r = ((ty0 + ly == ys && x == xs) ? 1.0 - inv_n2 : -inv_n2) - lx0;
+            *rp = r;
             rr = fma(r, r, rr);
             sx += c;
         }

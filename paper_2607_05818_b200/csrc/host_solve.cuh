@@ -368,7 +368,8 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     if (guess) {
         // x0 = column `src` of the mean mesh's closed-form pseudo-inverse, r0 = b - L x0; right-hand sides it does not
         // help (||r0|| > ||b|| / 2) are re-initialised with x0 = 0, r0 = b -- all on the device
-        CK(cudaMemsetAsync(W.g_rr0, 0, (size_t)2 * B * sizeof(double), L.s));  // g_rr0 and g_sumx are adjacent
+        CK(cudaMemsetAsync(W.g_rr0, 0, (size_t)B * sizeof(double), L.s));
+        CK(cudaMemsetAsync(W.g_sumx, 0, (size_t)B * sizeof(double), L.s));
         const int tiles = cdiv(n, GUESS_TX) * cdiv(n, GUESS_TY);
         const int GR = std::max(1, std::min(16, (int)((long)tiles * B / (148L * 8))));
         L.run(KC_SMALL, V, [&] { k_guess_rhs<<<dim3(tiles, cdiv(B, GR)), GUESS_THREADS, 0, L.s>>>(*guess, H.lev[0], node, src, 1.0 / (double)n2, W.r[0].as<double>(), W.g_rr0, W.g_sumx, B, GR); });
