@@ -24,6 +24,13 @@ struct GuessTable {
     int n;
 };
 
+// The four look-ups of Eq. (3) are summed in FP32, in one fixed order (explicitly rounded operations: no contraction),
+// and converted once: FP32 -> FP64 conversions run on the SM's conversion pipe, and four per node made it the busiest
+// unit of the guess kernels.  A guess needs no more than FP32; what matters is that every kernel gets the same bits.
+__device__ __forceinline__ float guess_sum4(float dd, float ss, float ds, float sd) {
+    return __fmul_rn(0.25f, __fadd_rn(__fadd_rn(dd, ss), __fadd_rn(ds, sd)));
+}
+
 // columns a, b = a +- 1 of table row t with one 8-byte load
 __device__ __forceinline__ void guess_pair(const GuessTable& t, int row, int a, int b, float& va, float& vb) {
     const float2 v = __ldg(t.P + (size_t)row * (t.n + 1) + min(a, b));
@@ -45,57 +52,83 @@ __device__ __forceinline__ void guess_x0_pair(const GuessTable& t, int y, int x,
     guess_pair(t, dy, sxa, sxb, dsA, dsB);
     guess_pair(t, sy, dxa, dxb, sdA, sdB);
     guess_pair(t, sy, sxa, sxb, ssA, ssB);
-    v0 = t.scale * (0.25 * (((double)ddA + (double)ssA) + ((double)dsA + (double)sdA)));
-    v1 = t.scale * (0.25 * (((double)ddB + (double)ssB) + ((double)dsB + (double)sdB)));
+    v0 = t.scale * (double)guess_sum4(ddA, ssA, dsA, sdA);
+    v1 = t.scale * (double)guess_sum4(ddB, ssB, dsB, sdB);
 }
 
 __device__ __forceinline__ double guess_x0(const GuessTable& t, int y, int x, int ys, int xs) {
-    return t.scale * spectral_entry<float>(t.G, t.n, y, x, ys, xs);
+    const int n = t.n, dx = abs(x - xs), dy = abs(y - ys);
+    int sx = x + xs + 1, sy = y + ys + 1;
+    sx = sx <= n ? sx : 2 * n - sx;
+    sy = sy <= n ? sy : 2 * n - sy;
+    const size_t ld = (size_t)n + 1;
+    return t.scale * (double)guess_sum4(__ldg(t.G + dy * ld + dx), __ldg(t.G + sy * ld + sx), __ldg(t.G + dy * ld + sx), __ldg(t.G + sy * ld + dx));
 }
 
 // r0[b] = b - L x0 on the pitched plane, rr0[b] += ||r0||^2, sumx[b] += sum(x0).
-// grid = (tiles_x * tiles_y, ceil(B / GR)); block = GUESS_THREADS; a thread keeps the raw conductances of its four
-// nodes of the GUESS_TY x GUESS_TX tile in registers and loops over GR right-hand sides; per right-hand side the block
-// tabulates x0 on the tile plus one ring (shared memory, double buffered: one __syncthreads per right-hand side) and
-// applies the 5-point operator.  Everything that does not depend on the right-hand side (which table entries a
-// thread evaluates, its nodes, their coefficients) is set up once per block: the kernel is instruction-bound.
+// grid = (tiles_x * tiles_y, ceil(B / GR)); block = GUESS_THREADS; a thread owns a 2 x 2 patch of the GUESS_TY x
+// GUESS_TX tile (its conductances in registers) and loops over GR right-hand sides; per right-hand side the block
+// tabulates x0 on the tile plus one ring (shared memory, double buffered: one __syncthreads per right-hand side;
+// mesh column j of the tile sits at index j + 2 of a 68-wide row, so that column pairs are 16-byte aligned) and
+// applies the 5-point operator with 16-byte shared loads and global stores.  Everything that does not depend on
+// the right-hand side is set up once per block.
 constexpr int GUESS_TX = 64, GUESS_TY = 16, GUESS_THREADS = 256;
 __global__ void __launch_bounds__(GUESS_THREADS)
 k_guess_rhs(GuessTable tab, Level L, const int* __restrict__ node, const int* __restrict__ src, double inv_n2,
             double* __restrict__ r0, double* __restrict__ rr0, double* __restrict__ sumx, int B, int GR) {
-    constexpr int XW = GUESS_TX + 2, XH = GUESS_TY + 2, NPAIR = XH * (XW / 2);
-    constexpr int PER = (NPAIR + GUESS_THREADS - 1) / GUESS_THREADS;       // pair entries of the ring tile per thread
-    constexpr int NODES = GUESS_TY * GUESS_TX / GUESS_THREADS;             // tile nodes per thread (same column)
-    static_assert(GUESS_THREADS % GUESS_TX == 0 && (GUESS_TY * GUESS_TX) % GUESS_THREADS == 0, "tile / block shape");
+    constexpr int XW = GUESS_TX + 4, XH = GUESS_TY + 2, EPR = GUESS_TX / 2 + 2, NENT = XH * EPR;  // entries per ring row: 32 pairs + 2 singles
+    constexpr int PER = (NENT + GUESS_THREADS - 1) / GUESS_THREADS;
+    static_assert((GUESS_TX / 2) * (GUESS_TY / 2) == GUESS_THREADS, "one 2 x 2 patch per thread");
     __shared__ __align__(16) double xs0[2][XH * XW];
+    __shared__ double part[2][2][GUESS_THREADS / 32];  // per-warp partial sums of the two reductions, double buffered
     const int tiles_x = (L.nx + GUESS_TX - 1) / GUESS_TX;
     const int tx0 = (blockIdx.x % tiles_x) * GUESS_TX, ty0 = (blockIdx.x / tiles_x) * GUESS_TY;
-    const int tid = threadIdx.x, lane = tid & 31;
-    // ---- per-thread constants of the tabulation: entry k covers ring-tile columns rx, rx+1 of ring-tile row ry
-    int ey[PER], ex[PER], eo[PER], ekind[PER];  // mesh row, mesh column of the first node, offset in xs0, 0 none / 1 pair / 2 singles
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // the block's partial sums of right-hand side b go out as ONE atomic per quantity (1024 blocks add to the same two
+    // words per right-hand side: per-warp atomics were the kernel's bottleneck), one iteration later: after the next
+    // __syncthreads the eight per-warp values are visible to threads 0 and 1
+    auto flush = [&](int bb, int pb) {
+        if (tid < 2) {
+            double v = 0.0;
+#pragma unroll
+            for (int w = 0; w < GUESS_THREADS / 32; ++w) v += part[pb][tid][w];
+            atomicAdd((tid == 0 ? rr0 : sumx) + bb, v);
+        }
+    };
+    // ---- per-thread constants of the tabulation
+    int ey[PER], ex[PER], eo[PER], ekind[PER];  // mesh row, first mesh column, offset in xs0; -1 nothing, 0 zeros, 1 pair, 2 first only, 3 single
 #pragma unroll
     for (int k = 0; k < PER; ++k) {
-        const int i = tid + k * GUESS_THREADS, ry = i / (XW / 2), rx = 2 * (i % (XW / 2));
-        ey[k] = ty0 + ry - 1; ex[k] = tx0 + rx - 1; eo[k] = ry * XW + rx;
-        const bool row_ok = i < NPAIR && ey[k] >= 0 && ey[k] < L.ny;
-        ekind[k] = i >= NPAIR ? -1 : !row_ok ? 0 : (ex[k] >= 0 && ex[k] + 1 < L.nx) ? 1 : 2;
+        const int i = tid + k * GUESS_THREADS, ry = i / EPR, e = i % EPR;
+        ey[k] = ty0 + ry - 1;
+        const bool row_ok = ey[k] >= 0 && ey[k] < L.ny;
+        if (e < GUESS_TX / 2) {  // columns 2e, 2e+1 of the tile
+            ex[k] = tx0 + 2 * e; eo[k] = ry * XW + 2 * e + 2;
+            ekind[k] = i >= NENT ? -1 : (!row_ok || ex[k] >= L.nx) ? 0 : ex[k] + 1 < L.nx ? 1 : 2;
+        } else {                 // ring column -1 (e == 32) or GUESS_TX (e == 33)
+            const int j = e == GUESS_TX / 2 ? -1 : GUESS_TX;
+            ex[k] = tx0 + j; eo[k] = ry * XW + j + 2;
+            ekind[k] = i >= NENT ? -1 : (row_ok && ex[k] >= 0 && ex[k] < L.nx) ? 3 : 4;  // 4: a single zero
+        }
     }
-    // ---- per-thread constants of the operator: nodes (ly0 + k * step, lx), their four conductances
-    const int lx = tid % GUESS_TX, ly0 = tid / GUESS_TX, x = tx0 + lx;
-    constexpr int STEP = GUESS_THREADS / GUESS_TX;
-    double ge[NODES], gw[NODES], gs[NODES], gn[NODES];
-    int nkind[NODES];  // 0 outside the plane, 1 node, 2 pad column
+    // ---- per-thread constants of the operator: patch rows 2 pr, 2 pr + 1, columns 2 pc, 2 pc + 1
+    const int pc = tid % (GUESS_TX / 2), pr = tid / (GUESS_TX / 2), x = tx0 + 2 * pc, y = ty0 + 2 * pr;
+    double ge[2][2], gw[2], gs[2][2], gn[2];  // east of both columns, west of column 0; south of both rows, north of row 0
+    bool in[2][2];
 #pragma unroll
-    for (int k = 0; k < NODES; ++k) {
-        const int y = ty0 + ly0 + k * STEP;
-        nkind[k] = (y >= L.ny || x >= L.pitch) ? 0 : x >= L.nx ? 2 : 1;
-        const bool in = nkind[k] == 1;
-        const size_t o = (size_t)y * L.pitch + x;
-        ge[k] = in ? L.gx[o] : 0.0;                       // pad / last column of gx is zero
-        gw[k] = (in && x > 0) ? L.gx[o - 1] : 0.0;
-        gs[k] = in ? L.gy[o] : 0.0;                       // last row of gy is zero
-        gn[k] = (in && y > 0) ? L.gy[o - L.pitch] : 0.0;
-    }
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            in[i][j] = y + i < L.ny && x + j < L.nx;
+            const size_t o = (size_t)(y + i) * L.pitch + x + j;
+            ge[i][j] = in[i][j] ? L.gx[o] : 0.0;   // (zero in the last column of the mesh)
+            gs[i][j] = in[i][j] ? L.gy[o] : 0.0;   // (zero in the last row)
+        }
+#pragma unroll
+    for (int i = 0; i < 2; ++i) gw[i] = (in[i][0] && x > 0) ? L.gx[(size_t)(y + i) * L.pitch + x - 1] : 0.0;
+#pragma unroll
+    for (int j = 0; j < 2; ++j) gn[j] = (in[0][j] && y > 0) ? L.gy[(size_t)(y - 1) * L.pitch + x + j] : 0.0;
+    const bool row_in[2] = {y < L.ny && x < L.pitch, y + 1 < L.ny && x < L.pitch};  // x even: both columns are addressable
     const size_t plane = (size_t)L.ny * L.pitch;
     const int b_end = min(B, (int)(blockIdx.y + 1) * GR);
     int buf = 0;
@@ -105,38 +138,45 @@ k_guess_rhs(GuessTable tab, Level L, const int* __restrict__ node, const int* __
 #pragma unroll
         for (int k = 0; k < PER; ++k) {
             if (ekind[k] < 0) continue;
+            if (ekind[k] >= 3) { xt[eo[k]] = ekind[k] == 3 ? guess_x0(tab, ey[k], ex[k], ys, xs) : 0.0; continue; }
             double v0 = 0.0, v1 = 0.0;
             if (ekind[k] == 1) guess_x0_pair(tab, ey[k], ex[k], ys, xs, v0, v1);
-            else if (ekind[k] == 2) {
-                if (ex[k] >= 0 && ex[k] < L.nx) v0 = guess_x0(tab, ey[k], ex[k], ys, xs);
-                if (ex[k] + 1 >= 0 && ex[k] + 1 < L.nx) v1 = guess_x0(tab, ey[k], ex[k] + 1, ys, xs);
-            }
-            *reinterpret_cast<double2*>(xt + eo[k]) = make_double2(v0, v1);  // eo is even, XW is even
+            else if (ekind[k] == 2) v0 = guess_x0(tab, ey[k], ex[k], ys, xs);
+            *reinterpret_cast<double2*>(xt + eo[k]) = make_double2(v0, v1);
         }
         __syncthreads();
-        double rr = 0.0, sx = 0.0;
-        double* rp = r0 + b * plane + (size_t)(ty0 + ly0) * L.pitch + x;
-#pragma unroll
-        for (int k = 0; k < NODES; ++k, rp += (size_t)STEP * L.pitch) {
-            if (nkind[k] == 0) continue;
-            if (nkind[k] == 2) { *rp = 0.0; continue; }  // pad column of an odd-width plane
-            const int ly = ly0 + k * STEP;
-            const double* xc = xt + (ly + 1) * XW + lx + 1;
-            const double c = xc[0];
-            // (L x0)_i = sum over neighbours of g (x0_i - x0_nb); absent neighbours have g = 0
-            double lx0 = ge[k] * (c - xc[1]);
-            lx0 = fma(gw[k], c - xc[-1], lx0);
-            lx0 = fma(gs[k], c - xc[XW], lx0);
-            lx0 = fma(gn[k], c - xc[-XW], lx0);
-            const double r = ((ty0 + ly == ys && x == xs) ? 1.0 - inv_n2 : -inv_n2) - lx0;
-            *rp = r;
-            rr = fma(r, r, rr);
-            sx += c;
-        }
+        if (b > (int)blockIdx.y * GR) flush(b - 1, buf ^ 1);
+        // rows 2 pr - 1 .. 2 pr + 2 of the ring tile (ring row = tile row + 1), columns 2 pc, 2 pc + 1 (+ the two beside them)
+        const double* xc = xt + (2 * pr) * XW + 2 * pc + 2;
+        const double2 up = *reinterpret_cast<const double2*>(xc), c0 = *reinterpret_cast<const double2*>(xc + XW),
+                      c1 = *reinterpret_cast<const double2*>(xc + 2 * XW), dn = *reinterpret_cast<const double2*>(xc + 3 * XW);
+        const double w0 = xc[XW - 1], e0 = xc[XW + 2], w1 = xc[2 * XW - 1], e1 = xc[2 * XW + 2];
+        // (L x0)_i = sum over neighbours of g (x0_i - x0_nb); absent neighbours have g = 0
+        double l00 = ge[0][0] * (c0.x - c0.y), l01 = ge[0][1] * (c0.y - e0);
+        l00 = fma(gw[0], c0.x - w0, l00);       l01 = fma(ge[0][0], c0.y - c0.x, l01);
+        l00 = fma(gs[0][0], c0.x - c1.x, l00);  l01 = fma(gs[0][1], c0.y - c1.y, l01);
+        l00 = fma(gn[0], c0.x - up.x, l00);     l01 = fma(gn[1], c0.y - up.y, l01);
+        double l10 = ge[1][0] * (c1.x - c1.y), l11 = ge[1][1] * (c1.y - e1);
+        l10 = fma(gw[1], c1.x - w1, l10);       l11 = fma(ge[1][0], c1.y - c1.x, l11);
+        l10 = fma(gs[1][0], c1.x - dn.x, l10);  l11 = fma(gs[1][1], c1.y - dn.y, l11);
+        l10 = fma(gs[0][0], c1.x - c0.x, l10);  l11 = fma(gs[0][1], c1.y - c0.y, l11);
+        const bool sy0 = y == ys, sy1 = y + 1 == ys, sx0 = x == xs, sx1 = x + 1 == xs;
+        // pad entries (the pad column of an odd-width plane) are written as zeros
+        const double r00 = in[0][0] ? ((sy0 && sx0) ? 1.0 - inv_n2 : -inv_n2) - l00 : 0.0;
+        const double r01 = in[0][1] ? ((sy0 && sx1) ? 1.0 - inv_n2 : -inv_n2) - l01 : 0.0;
+        const double r10 = in[1][0] ? ((sy1 && sx0) ? 1.0 - inv_n2 : -inv_n2) - l10 : 0.0;
+        const double r11 = in[1][1] ? ((sy1 && sx1) ? 1.0 - inv_n2 : -inv_n2) - l11 : 0.0;
+        double* rp = r0 + b * plane + (size_t)y * L.pitch + x;
+        if (row_in[0]) *reinterpret_cast<double2*>(rp) = make_double2(r00, r01);
+        if (row_in[1]) *reinterpret_cast<double2*>(rp + L.pitch) = make_double2(r10, r11);
+        double rr = fma(r00, r00, fma(r01, r01, fma(r10, r10, r11 * r11)));
+        double sx = (in[0][0] ? c0.x : 0.0) + (in[0][1] ? c0.y : 0.0) + (in[1][0] ? c1.x : 0.0) + (in[1][1] ? c1.y : 0.0);
         rr = warp_sum(rr);
         sx = warp_sum(sx);
-        if (lane == 0) { atomicAdd(rr0 + b, rr); atomicAdd(sumx + b, sx); }  // one atomic per warp and quantity
+        if (lane == 0) { part[buf][0][warp] = rr; part[buf][1][warp] = sx; }
     }
+    __syncthreads();
+    if (b_end > (int)blockIdx.y * GR) flush(b_end - 1, buf ^ 1);
 }
 
 // Terminal-source solves deliver ONE number, Z[s,s] = b^T L^+ b, and stop early because the CG error of b^T x_k is the
