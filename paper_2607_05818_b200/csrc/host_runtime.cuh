@@ -85,22 +85,35 @@ struct DevPool {
 };
 DevPool g_pool;
 
-// Pinned host scratch for the per-iteration read-backs: one grow-only block per thread, kept for the life of
-// the process (cudaMallocHost / cudaFreeHost stall for hundreds of ms now and then).
-struct PinnedScratch {
-    void* p = nullptr;
-    size_t bytes = 0;
-    void* get(size_t n) {
-        if (n > bytes) {
-            if (p) cudaFreeHost(p);
-            p = nullptr; bytes = 0;
-            if (cudaMallocHost(&p, n) != cudaSuccess) { cudaGetLastError(); p = nullptr; return nullptr; }
-            bytes = n;
+// Pinned host scratch for the per-iteration read-backs: blocks are kept for the life of the process and handed
+// from one workspace to the next (cudaMallocHost / cudaFreeHost stall for hundreds of ms now and then); a
+// workspace owns its block while it lives, so host threads solving tiers concurrently never share one.
+struct PinnedPool {
+    std::mutex mu;
+    std::vector<std::pair<size_t, void*>> free_blocks;
+    void* get(size_t n, size_t* got) {
+        {
+            std::lock_guard<std::mutex> g(mu);
+            for (size_t i = 0; i < free_blocks.size(); ++i)
+                if (free_blocks[i].first >= n) {
+                    void* p = free_blocks[i].second;
+                    *got = free_blocks[i].first;
+                    free_blocks.erase(free_blocks.begin() + i);
+                    return p;
+                }
         }
+        void* p = nullptr;
+        n = std::max<size_t>(n, 16384);
+        if (cudaMallocHost(&p, n) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        *got = n;
         return p;
     }
+    void put(void* p, size_t n) {
+        std::lock_guard<std::mutex> g(mu);
+        free_blocks.emplace_back(n, p);
+    }
 };
-thread_local PinnedScratch g_pinned;
+PinnedPool g_pinned;
 
 // PDN_POISON=1 in the environment (read once): every device block handed out is first filled with 0xFF bytes --
 // NaN as a double or float, -1 as an int -- so that any read of memory the library did not write itself turns
@@ -174,6 +187,7 @@ struct pdn_ctx {
     double class_ms[KC_COUNT] = {};
     double class_bytes[KC_COUNT] = {};
     int64_t class_launches[KC_COUNT] = {};
+    std::mutex mu;                        // guards the counters below when tiers are solved by several host threads
     bool time_kernels = false;
     bool debug = false;                   // PDN_DEBUG was set in the environment at pdn_create: iteration history on stderr
     std::vector<std::pair<int, std::pair<cudaEvent_t, cudaEvent_t>>> pending_events;
@@ -197,10 +211,15 @@ struct Launcher {
     template <class F>
     void run(int cls, double bytes, F&& f) {
         cudaEvent_t a = nullptr, b = nullptr;
-        if (c->time_kernels) { a = get_event(); b = get_event(); CK(cudaEventRecord(a, s)); }
+        if (c->time_kernels) {
+            { std::lock_guard<std::mutex> g(c->mu); a = get_event(); b = get_event(); }
+            CK(cudaEventRecord(a, s));
+        }
         f();
         CK(cudaGetLastError());
-        if (c->time_kernels) { CK(cudaEventRecord(b, s)); c->pending_events.push_back({cls, {a, b}}); }
+        if (c->time_kernels) CK(cudaEventRecord(b, s));
+        std::lock_guard<std::mutex> g(c->mu);
+        if (c->time_kernels) c->pending_events.push_back({cls, {a, b}});
         c->class_launches[cls]++;
         c->class_bytes[cls] += bytes;
         c->stats.kernel_launches++;

@@ -152,8 +152,14 @@ struct Work {
     double *g_rr0 = nullptr, *g_sumx = nullptr, *g_dot = nullptr;  // initial guess (guess.cuh): ||r0||^2, sum(x0), x0.r_k per right-hand side
     int *g_keep = nullptr, *g_rbuf = nullptr;     // ... whether the guess is used; buffer of the last residual
     PcgScalars s{};
-    int* h_nact = nullptr;                           // pinned (g_pinned: not owned)
+    int* h_nact = nullptr;                           // pinned (a block of g_pinned, owned while the workspace lives)
     double* h_relres = nullptr;                      // pinned, Bmax
+    void* h_block = nullptr;
+    size_t h_bytes = 0;
+    Work() = default;
+    Work(const Work&) = delete;
+    Work& operator=(const Work&) = delete;
+    ~Work() { if (h_block) g_pinned.put(h_block, h_bytes); }
 
     static size_t bytes_per_rhs(const Hierarchy& H) {
         size_t b = 5 * H.plane(0);
@@ -189,7 +195,9 @@ struct Work {
         xown.alloc((size_t)B * sizeof(double));
         pport.alloc((size_t)B * (std::max(qmax, 1) + 1) * sizeof(double));
         src.alloc((size_t)B * sizeof(int));
-        char* hp = static_cast<char*>(g_pinned.get(64 + (size_t)B * sizeof(double)));
+        if (h_block) { g_pinned.put(h_block, h_bytes); h_block = nullptr; }
+        h_block = g_pinned.get(64 + (size_t)B * sizeof(double), &h_bytes);
+        char* hp = static_cast<char*>(h_block);
         if (!hp) throw StatusFail{PDN_E_NOMEM, "pinned host allocation failed"};
         h_nact = reinterpret_cast<int*>(hp);
         h_relres = reinterpret_cast<double*>(hp + 64);
@@ -464,10 +472,13 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
         g_last_error = "a port solve produced a non-finite residual";
         status = PDN_E_NUMERIC;
     }
-    c->stats.worst_rel_residual = std::max(c->stats.worst_rel_residual, worst);
-    c->stats.pcg_iters_max = std::max(c->stats.pcg_iters_max, it);
-    c->stats.pcg_iters_sum += it;
-    c->stats.rhs_iterations += active_sum;
+    {
+        std::lock_guard<std::mutex> g(c->mu);
+        c->stats.worst_rel_residual = std::max(c->stats.worst_rel_residual, worst);
+        c->stats.pcg_iters_max = std::max(c->stats.pcg_iters_max, it);
+        c->stats.pcg_iters_sum += it;
+        c->stats.rhs_iterations += active_sum;
+    }
     if (c->debug)
         fprintf(stderr, "[pdn] batch src0=%d B=%d %s: %d iterations, rhs-iterations %ld (of %ld without skipping), worst relres %.2e\n", src0, B,
                 terminal ? "terminal" : "tsv", it, active_sum, (long)it * B, worst);

@@ -17,6 +17,7 @@
 #include <cstring>
 #include <map>
 #include <mutex>
+#include <thread>
 #include <new>
 #include <set>
 #include <string>
@@ -160,7 +161,7 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
             if (!e && t_table <= t_solves) e = &tabs.build(L, n, rho, false);
             if (e) {
                 L.run(KC_SMALL, 0, [&] { k_uniform_gather<<<dim3(cdiv(T.q, 128), grid_rows((size_t)T.nrows + 1)), 128, 0, L.s>>>(e->G.as<double>(), 1.0 / g0[1], n, H.pitch[0], T.d_node.as<int>(), T.ntsv, T.nrows, T.q, T.ZT.as<double>(), T.zdiag.as<double>()); });
-                c->stats.n_uniform_tiers++;
+                { std::lock_guard<std::mutex> g(c->mu); c->stats.n_uniform_tiers++; }
                 T.whole = true;
                 return PDN_OK;
             }
@@ -181,7 +182,7 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
             tabs.float_copy(L, *e);
             gtab = GuessTable{e->Gf.as<float>(), e->Gp.as<float2>(), 1.0 / H.mean_gy, n};
             guess = &gtab;
-            c->stats.n_guess_tiers++;
+            { std::lock_guard<std::mutex> g(c->mu); c->stats.n_guess_tiers++; }
         }
     }
     // Smoothing interval [2/ratio, 2] of the Chebyshev polynomial.  With 2x2 aggregation the coarse grid
@@ -340,48 +341,122 @@ int pdn_create(pdn_ctx** out, int32_t n_tiers, const pdn_tier* tiers, int32_t n_
         }
         c->stats.n_tiers = d;
 
-        // ---- S0 + S1, tier by tier
-        SpectralTables tabs;
-        Hierarchy H;
-        H.allocate(n);
-        c->stats.n_levels = H.nlev;
-        DevBuf stage;  // staging for host-resident planes
-        if (o.flags & PDN_TIERS_ON_HOST) stage.alloc((size_t)2 * n * n * sizeof(double));
-        const int Bmax = pick_batch(H, qmax, o);
-        Work W;
-        if (H.nlev > 1) W.allocate(H, Bmax, qmax);
+        // ---- S0 + S1, tier by tier.  One tier: import + hierarchy (S0), then its port solves (S1).
+        std::mutex msg_mu;
+        std::string first_msg;
         float ms_up = 0.f;
-        for (int t = 0; t < d && status == PDN_OK; ++t) {
+        auto run_tier = [&](int t, Launcher& TL, Hierarchy& H, Work& W, int Bmax, DevBuf& stage, SpectralTables& tabs,
+                            cudaEvent_t e0, cudaEvent_t e1) -> int {
             TierPorts& T = c->tiers[t];
             const double *gx = tiers[t].gx, *gy = tiers[t].gy;
-            CK(cudaEventRecord(ev[1], L.s));
+            CK(cudaEventRecord(e0, TL.s));
             if (o.flags & PDN_TIERS_ON_HOST) {
                 double* sg = stage.as<double>();
-                CK(cudaMemcpyAsync(sg, gx, (size_t)n * n * sizeof(double), cudaMemcpyHostToDevice, L.s));
-                CK(cudaMemcpyAsync(sg + (size_t)n * n, gy, (size_t)n * n * sizeof(double), cudaMemcpyHostToDevice, L.s));
+                CK(cudaMemcpyAsync(sg, gx, (size_t)n * n * sizeof(double), cudaMemcpyHostToDevice, TL.s));
+                CK(cudaMemcpyAsync(sg + (size_t)n * n, gy, (size_t)n * n * sizeof(double), cudaMemcpyHostToDevice, TL.s));
                 gx = sg; gy = sg + (size_t)n * n;
             }
-            status = H.build(L, gx, gy, !(o.flags & PDN_SKIP_CONNECTIVITY_CHECK));
-            if (status == PDN_OK) {  // keep the sanitised planes: pdn_update_tsvs rebuilds the hierarchy from them
+            int st = H.build(TL, gx, gy, !(o.flags & PDN_SKIP_CONNECTIVITY_CHECK));
+            if (st == PDN_OK) {  // keep the sanitised planes: pdn_update_tsvs rebuilds the hierarchy from them
                 T.gx0.alloc(H.plane(0) * sizeof(double));
                 T.gy0.alloc(H.plane(0) * sizeof(double));
-                CK(cudaMemcpyAsync(T.gx0.p, H.gx[0].p, H.plane(0) * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
-                CK(cudaMemcpyAsync(T.gy0.p, H.gy[0].p, H.plane(0) * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
+                CK(cudaMemcpyAsync(T.gx0.p, H.gx[0].p, H.plane(0) * sizeof(double), cudaMemcpyDeviceToDevice, TL.s));
+                CK(cudaMemcpyAsync(T.gy0.p, H.gy[0].p, H.plane(0) * sizeof(double), cudaMemcpyDeviceToDevice, TL.s));
             }
-            CK(cudaEventRecord(ev[2], L.s));
-            CK(cudaEventSynchronize(ev[2]));
+            CK(cudaEventRecord(e1, TL.s));
+            CK(cudaEventSynchronize(e1));
             float ms = 0.f;
-            CK(cudaEventElapsedTime(&ms, ev[1], ev[2]));
+            CK(cudaEventElapsedTime(&ms, e0, e1));
+            if (st == PDN_OK) {
+                // this rank's contiguous slice of the TSV sources and of the terminal sources (everything if unsharded)
+                const int W_ = c->shard_world, r_ = c->shard_rank;
+                std::vector<int> tsv_src, term_src;
+                for (int k = (int)((int64_t)r_ * T.ntsv / W_); k < (int)((int64_t)(r_ + 1) * T.ntsv / W_); ++k) tsv_src.push_back(k);
+                for (int k = (int)((int64_t)r_ * T.nterm / W_); k < (int)((int64_t)(r_ + 1) * T.nterm / W_); ++k) term_src.push_back(T.ntsv + k);
+                st = reduce_tier(c, TL, H, W, Bmax, T, tsv_src, term_src, tabs);
+            }
+            std::lock_guard<std::mutex> g(msg_mu);
             ms_up += ms;
-            if (status != PDN_OK) { g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status); break; }
-            // this rank's contiguous slice of the TSV sources and of the terminal sources (everything if unsharded)
-            const int W_ = c->shard_world, r_ = c->shard_rank;
-            std::vector<int> tsv_src, term_src;
-            for (int k = (int)((int64_t)r_ * T.ntsv / W_); k < (int)((int64_t)(r_ + 1) * T.ntsv / W_); ++k) tsv_src.push_back(k);
-            for (int k = (int)((int64_t)r_ * T.nterm / W_); k < (int)((int64_t)(r_ + 1) * T.nterm / W_); ++k) term_src.push_back(T.ntsv + k);
-            status = reduce_tier(c, L, H, W, Bmax, T, tsv_src, term_src, tabs);
-            if (status != PDN_OK) g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status);
+            if (st != PDN_OK && first_msg.empty()) {
+                const std::string detail = g_last_error;
+                first_msg = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(st) + (detail.empty() ? "" : " (" + detail + ")");
+            }
+            return st;
+        };
+        // Small meshes (configs[0..1]: 32^2, 128^2) are bound by the serial latency of many tiny launches, not by the
+        // device: their tiers -- independent 2D problems -- are solved concurrently, one host thread
+        // and one stream per tier (up to four), each with its own hierarchy and workspace.  Large meshes fill the
+        // device with one tier and keep the single-stream path (and one shared spectral table).
+        const int n_workers = (n <= 256 && d >= 2) ? std::min(d, 4) : 1;
+        c->stats.n_levels = 1;
+        for (int cur = n; cur > COARSEST_MAX; cur = (cur + 1) / 2) c->stats.n_levels++;
+        if (n_workers == 1) {
+            SpectralTables tabs;
+            Hierarchy H;
+            H.allocate(n);
+            DevBuf stage;  // staging for host-resident planes
+            if (o.flags & PDN_TIERS_ON_HOST) stage.alloc((size_t)2 * n * n * sizeof(double));
+            const int Bmax = pick_batch(H, qmax, o);
+            Work W;
+            if (H.nlev > 1) W.allocate(H, Bmax, qmax);
+            for (int t = 0; t < d && status == PDN_OK; ++t) status = run_tier(t, L, H, W, Bmax, stage, tabs, ev[1], ev[2]);
+        } else {
+            cudaEvent_t ev_start;
+            CK(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
+            CK(cudaEventRecord(ev_start, L.s));
+            std::vector<int> wst(n_workers, PDN_OK);
+            std::vector<cudaEvent_t> ev_done(n_workers, nullptr);
+            std::vector<std::thread> th;
+            for (int w = 0; w < n_workers; ++w)
+                th.emplace_back([&, w] {
+                    cudaStream_t ws = nullptr;
+                    cudaEvent_t e0 = nullptr, e1 = nullptr;
+                    try {
+                        CK(cudaSetDevice(c->device));
+                        CK(cudaStreamCreateWithFlags(&ws, cudaStreamNonBlocking));
+                        CK(cudaStreamWaitEvent(ws, ev_start, 0));
+                        CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+                        CK(cudaEventCreateWithFlags(&ev_done[w], cudaEventDisableTiming));
+                        Launcher TL{c, ws};
+                        SpectralTables tabs;
+                        Hierarchy H;
+                        H.allocate(n);
+                        DevBuf stage;
+                        if (o.flags & PDN_TIERS_ON_HOST) stage.alloc((size_t)2 * n * n * sizeof(double));
+                        int qw = 1;
+                        for (int t = w; t < d; t += n_workers) qw = std::max(qw, c->tiers[t].q);
+                        const int Bmax = pick_batch(H, qw, o);
+                        Work W;
+                        if (H.nlev > 1) W.allocate(H, Bmax, qw);
+                        for (int t = w; t < d && wst[w] == PDN_OK; t += n_workers) wst[w] = run_tier(t, TL, H, W, Bmax, stage, tabs, e0, e1);
+                        CK(cudaStreamSynchronize(ws));  // the worker's buffers are released when it returns
+                        CK(cudaEventRecord(ev_done[w], ws));
+                    } catch (const CudaFail& f) {
+                        wst[w] = f.e == cudaErrorMemoryAllocation ? PDN_E_NOMEM : PDN_E_CUDA;
+                        cudaGetLastError();
+                        std::lock_guard<std::mutex> g(msg_mu);
+                        if (first_msg.empty()) first_msg = std::string(f.what) + ": " + cudaGetErrorString(f.e);
+                    } catch (const StatusFail& f) {
+                        wst[w] = f.status;
+                        std::lock_guard<std::mutex> g(msg_mu);
+                        if (first_msg.empty()) first_msg = f.msg;
+                    } catch (const std::bad_alloc&) {
+                        wst[w] = PDN_E_NOMEM;
+                        std::lock_guard<std::mutex> g(msg_mu);
+                        if (first_msg.empty()) first_msg = "host allocation failed";
+                    }
+                    if (e0) cudaEventDestroy(e0);
+                    if (e1) cudaEventDestroy(e1);
+                    if (ws) cudaStreamDestroy(ws);
+                });
+            for (auto& t_ : th) t_.join();
+            for (int w = 0; w < n_workers; ++w) {
+                if (ev_done[w]) { cudaStreamWaitEvent(L.s, ev_done[w], 0); cudaEventDestroy(ev_done[w]); }
+                if (wst[w] != PDN_OK && status == PDN_OK) status = wst[w];
+            }
+            cudaEventDestroy(ev_start);
         }
+        if (status != PDN_OK) g_last_error = first_msg;
         CK(cudaEventRecord(ev[2], L.s));
         // ---- S2 + S3 (a sharded context stays open until its rows are complete: pdn_finish)
         if (status == PDN_OK && !c->open) {
