@@ -828,6 +828,30 @@ def test_binding_refuses_buffers_the_library_would_misread():
     pdn.close()
 
 
+def test_more_than_65535_terminals():
+    """m + n_loads > 65535: the kernels that used to put that dimension in gridDim.y (limit 65535) now walk it; a
+    sample of the 1.04e9 pairs through the pair list against the oracle, and the terminal diagonals from 66 000
+    bump / load solves on a 256^2 mesh (which start from the closed-form guess)."""
+    from oracle.reff_oracle import Oracle
+    from paper_2607_05818_b200 import Pdn
+    torch = torch_cuda()
+    m, nl = 40000, 26000
+    net = P.make_random(97, d=2, n=256, p=8, m=m, nl=nl)
+    assert m + nl > 65535 and len({tuple(b) for b in net.bumps.tolist()}) == m
+    pdn = Pdn.from_network(net, device="cuda:0")
+    rng = np.random.default_rng(3)
+    bi = np.concatenate([[0, m - 1], rng.integers(0, m, 22)]).astype(np.int32)
+    li = np.concatenate([[nl - 1, 0], rng.integers(0, nl, 22)]).astype(np.int32)
+    out = torch.empty(bi.size, dtype=torch.float64, device="cuda:0")
+    pdn.reff(out, torch.from_numpy(bi).cuda(), torch.from_numpy(li).cuda())
+    st = pdn.stats()
+    pdn.close()
+    o = Oracle(net)
+    want = np.array([o.reff(int(b), int(l)) for b, l in zip(bi, li)])
+    check(out.cpu().numpy(), want)
+    assert st["n_guess_tiers"] == 2
+
+
 def test_permuting_the_bump_and_load_lists_permutes_the_output():
     """S4 pin: R depends on the pair, not on where it sits in the create-time lists."""
     net = P.make_random(11, d=3, n=40, p=7, m=6, nl=9, drop=0.02)
