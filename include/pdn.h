@@ -147,7 +147,7 @@ typedef struct {
     double class_bytes[8];       /* algorithmic bytes moved per kernel class                      */
     int64_t class_launches[8];   /* launches per kernel class                                     */
     int32_t n_guess_tiers;       /* tier reductions whose port solves started from the closed-form guess */
-    int32_t reserved_;
+    int32_t n_guess_rejected;    /* right-hand sides of those whose guess did not help and that started from x0 = 0 */
 } pdn_stats;
 
 /* S0-S3.  tiers: HOST array of n_tiers descriptors (all tiers must have the same n).  tsvs, bumps,

@@ -51,7 +51,7 @@ class PdnStats(C.Structure):
                 ("ms_dense", C.c_double), ("ms_total", C.c_double), ("stencil_bytes", C.c_double),
                 ("ms_update_stencil", C.c_double), ("ms_update_dense", C.c_double), ("update_solves", C.c_int64),
                 ("class_ms", C.c_double * 8), ("class_bytes", C.c_double * 8),
-                ("class_launches", C.c_int64 * 8), ("n_guess_tiers", C.c_int32), ("reserved_", C.c_int32)]
+                ("class_launches", C.c_int64 * 8), ("n_guess_tiers", C.c_int32), ("n_guess_rejected", C.c_int32)]
 
 
 EXPORTS = ("pdn_create", "pdn_reff", "pdn_reff_host", "pdn_destroy", "pdn_strerror", "pdn_last_error",

@@ -461,7 +461,14 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     else
         L.run(KC_SMALL, 0, [&] { k_finish_tsv<<<dim3(cdiv(ngather, 128), B), 128, 0, L.s>>>(W.xport.as<double>(), W.s.xmean, ngather, src, T.ZT.as<double>(), B); });
     CK(cudaMemcpyAsync(W.h_relres, W.s.relres, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, L.s));
+    std::vector<int> h_keep;
+    if (guess) {
+        h_keep.resize(B);
+        CK(cudaMemcpyAsync(h_keep.data(), W.g_keep, (size_t)B * sizeof(int), cudaMemcpyDeviceToHost, L.s));
+    }
     CK(cudaStreamSynchronize(L.s));
+    int rejected = 0;
+    for (int v : h_keep) rejected += v == 0;
     double worst = 0.0;
     bool nonfinite = false;  // a NaN / Inf residual froze its right-hand side (k_scal_check): that is a failure, not convergence
     for (int b = 0; b < B; ++b) {
@@ -478,6 +485,7 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
         c->stats.pcg_iters_max = std::max(c->stats.pcg_iters_max, it);
         c->stats.pcg_iters_sum += it;
         c->stats.rhs_iterations += active_sum;
+        c->stats.n_guess_rejected += rejected;
     }
     if (c->debug)
         fprintf(stderr, "[pdn] batch src0=%d B=%d %s: %d iterations, rhs-iterations %ld (of %ld without skipping), worst relres %.2e\n", src0, B,

@@ -828,6 +828,29 @@ def test_binding_refuses_buffers_the_library_would_misread():
     pdn.close()
 
 
+def test_initial_guess_is_rejected_where_it_does_not_help():
+    """The closed-form guess comes from the tier's MEAN mesh.  A tier made of two halves whose conductances differ
+    2.5-fold has a coefficient of variation of 0.43 -- the guess is tried -- but near most sources the mean mesh is off
+    by a factor of 1.4-1.75, so the guess does not halve the residual there: those right-hand sides must fall back to
+    x0 = 0 on the device (k_guess_check) and every result must still match the oracle; with the guess switched off the
+    result is the same to solver tolerance."""
+    from oracle.reff_oracle import Oracle
+    from paper_2607_05818_b200 import PDN_NO_INITIAL_GUESS
+    n = 200
+    net = P.make_random(55, d=2, n=n, p=80, m=40, nl=40, r_lo=0.9, r_hi=1.1)   # >= n/2 right-hand sides per tier: a table is built
+    for t in range(2):
+        net.gx[t][:, : n // 2] *= 2.5
+        net.gy[t][:, : n // 2] *= 2.5
+    got, st = gpu_all_pairs(net)
+    assert st["n_guess_tiers"] == 2 and 0 < st["n_guess_rejected"]
+    check(got, Oracle(net).reff_all())
+    ref, st0 = gpu_all_pairs(net, flags=PDN_NO_INITIAL_GUESS)
+    assert st0["n_guess_tiers"] == 0 and st0["n_guess_rejected"] == 0
+    assert np.allclose(got, ref, rtol=1e-7, atol=0)
+    print(f"guess rejected for {st['n_guess_rejected']} of {2 * (80 + 40)} right-hand sides; "
+          f"rhs-iterations {st['rhs_iterations']} (x0 = 0 everywhere: {st0['rhs_iterations']})")
+
+
 def test_more_than_65535_terminals():
     """m + n_loads > 65535: the kernels that used to put that dimension in gridDim.y (limit 65535) now walk it; a
     sample of the 1.04e9 pairs through the pair list against the oracle, and the terminal diagonals from 66 000
