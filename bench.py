@@ -406,7 +406,7 @@ def run_cuda(a):
         out_n = torch.empty(k * k, dtype=torch.float64, device=dev)
         pdn = Pdn(net.n, gx_d, gy_d, *args[1], flags=base_flags, rtol=a.rtol, nu=a.nu, rhs_batch=a.rhs_batch)
         tn, tm = [], []
-        stride = max(1, net.n // 32)
+        stride = a.map_stride if a.map_stride > 0 else max(1, net.n // 32)
         for rep in range(a.warmup + a.steps):
             torch.cuda.synchronize()
             t0 = time.perf_counter()
@@ -463,6 +463,8 @@ def main():
                     help="also time the NEXT-3 leg: context with PDN_TERMINAL_PAIRS, load-load R_eff, Eq. (4) voltages")
     ap.add_argument("--nodes", type=int, default=0, metavar="K",
                     help="also time pdn_reff_nodes on K random probes over all tiers and an R_eff map of the bottom tier (NEXT-3)")
+    ap.add_argument("--map-stride", type=int, default=0, metavar="S",
+                    help="with --nodes: stride of the R_eff map of the bottom tier (default n/32; 1 = every node: pdn_reff_from)")
     ap.add_argument("--nodes-check", type=int, default=0, metavar="J", help="with --nodes: check J of the pairs against the oracle")
     ap.add_argument("--shard", action="store_true",
                     help="N > 1: ONE network, its port solves sharded over the ranks (NEXT-4, strong scaling) instead "

@@ -213,6 +213,16 @@ typedef struct pdn_node {
 } pdn_node;
 int pdn_reff_nodes(pdn_ctx *ctx, int32_t n_nodes, const pdn_node *nodes, double *out);
 
+/* One source against many nodes -- the R_eff map of Fig. 6(d).  src: HOST, one node; nodes: HOST
+ * array of n_nodes probes on any tiers (duplicates and the source itself allowed); out: DEVICE fp64, n_nodes values,
+ * out[a] = R_eff(src, nodes[a]) in the whole 3D network.  Same algebra as pdn_reff_nodes, but only one row and the
+ * diagonal of its matrix are formed: on every tier that holds probes the TSV-port solves are repeated with the probes
+ * in the gather list (by reciprocity they deliver Z_t[TSV port, probe]), every probe costs one DIAGONAL solve (loose
+ * tolerance, second-order accurate like the bump / load solves of pdn_create), and the kept factor of C is applied
+ * once to all n_nodes + 1 columns.  Memory is O((P + q_t) n_nodes) instead of pdn_reff_nodes' O(n_nodes^2), so a map
+ * over every node of a tier is possible (it costs about one diagonal solve per node).  The context is not changed. */
+int pdn_reff_from(pdn_ctx *ctx, const pdn_node *src, int32_t n_nodes, const pdn_node *nodes, double *out);
+
 /* NEXT-4: one network sharded over several GPUs, one process per GPU.  The port solves of
  * a tier are independent, so with opts->shard_world = W > 1 pdn_create (same arguments on every
  * rank) imports all tiers but solves only slice opts->shard_rank of each tier's TSV sources and of its bump / load

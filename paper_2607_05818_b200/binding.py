@@ -57,7 +57,7 @@ class PdnStats(C.Structure):
 EXPORTS = ("pdn_create", "pdn_reff", "pdn_reff_host", "pdn_destroy", "pdn_strerror", "pdn_last_error",
            "pdn_get_stats", "pdn_port_count", "pdn_get_port_matrix", "pdn_release_cache", "pdn_update_tsvs",
            "pdn_reff_same_side", "pdn_load_voltages", "pdn_reff_nodes", "pdn_shard_slice", "pdn_shard_buffers",
-           "pdn_finish", "pdn_set_solver_opts")
+           "pdn_finish", "pdn_set_solver_opts", "pdn_reff_from")
 
 _lib = None
 
@@ -94,6 +94,8 @@ def load_library() -> C.CDLL:
     lib.pdn_load_voltages.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_double, C.c_void_p]
     lib.pdn_reff_nodes.restype = C.c_int
     lib.pdn_reff_nodes.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+    lib.pdn_reff_from.restype = C.c_int
+    lib.pdn_reff_from.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
     lib.pdn_shard_slice.restype = C.c_int
     lib.pdn_shard_slice.argtypes = [C.c_void_p, C.c_int32, C.c_int32] + [C.POINTER(C.c_int32)] * 4
     lib.pdn_shard_buffers.restype = C.c_int
@@ -320,19 +322,28 @@ class Pdn:
             raise PdnError(st, "pdn_reff_nodes")
         return out
 
+    def reff_from(self, src, nodes, out):
+        """pdn_reff_from: `src` = (tier, y, x); `nodes` an (k, 3) integer array of (tier, y, x) probes on the host; `out`
+        a torch CUDA tensor of k doubles that receives R_eff(src, node) for every probe."""
+        sr = np.ascontiguousarray(np.asarray(src, dtype=np.int32).reshape(1, 3))
+        nd = np.ascontiguousarray(np.asarray(nodes, dtype=np.int32).reshape(-1, 3))
+        k = int(nd.shape[0])
+        st = self._lib.pdn_reff_from(self._h, sr.ctypes.data, k, nd.ctypes.data, _ptr(out, "f8", "out", k))
+        if st != PDN_OK:
+            raise PdnError(st, "pdn_reff_from")
+        return out
+
     def reff_map(self, src, tier: int, stride: int = 1):
         """R_eff map (Fig. 6(d) of the paper): effective resistance from the node `src` = (tier, y, x)
         to every `stride`-th node (rows and columns 0, stride, 2*stride, ...) of tier `tier`, as a 2-D numpy array.
-        One pdn_reff_nodes call with the source and the grid nodes as probes; only marshalling and slicing here."""
+        One pdn_reff_from call with the grid nodes as probes; only marshalling and reshaping here."""
         import torch
         ys = np.arange(0, self.n, stride, dtype=np.int32)
         yy, xx = np.meshgrid(ys, ys, indexing="ij")
-        nodes = np.vstack([np.asarray(src, dtype=np.int32).reshape(1, 3),
-                           np.stack([np.full(yy.size, tier, dtype=np.int32), yy.ravel(), xx.ravel()], axis=1)])
-        k = nodes.shape[0]
-        out = torch.empty(k * k, dtype=torch.float64, device=self._device)
-        self.reff_nodes(nodes, out)
-        return out[1:k].cpu().numpy().reshape(ys.size, ys.size)
+        nodes = np.stack([np.full(yy.size, tier, dtype=np.int32), yy.ravel(), xx.ravel()], axis=1)
+        out = torch.empty(nodes.shape[0], dtype=torch.float64, device=self._device)
+        self.reff_from(src, nodes, out)
+        return out.cpu().numpy().reshape(ys.size, ys.size)
 
     # ---- NEXT-4: one network sharded over several GPUs (argument marshalling + the exchange plumbing only)
     def shard_pieces(self, rank: int):

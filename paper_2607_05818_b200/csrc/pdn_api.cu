@@ -128,7 +128,8 @@ struct SpectralTables {
 // S1 of one tier whose hierarchy H has just been built: fills rows `tsv_src` of ZT (each against all ports of
 // the tier) and, if `terminals`, zdiag.  Meshes with n <= 4 and uniform tiers (Eq. 3) are reduced whole.
 int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPorts& T, const std::vector<int>& tsv_src,
-                const std::vector<int>& term, SpectralTables& tabs) {  // term: port indices (>= ntsv) of the terminal sources to solve
+                const std::vector<int>& term, SpectralTables& tabs,  // term: port indices (>= ntsv) of the terminal sources to solve
+                bool diag_only_terms = false) {                      // ... for their diagonal only, whatever PDN_TERMINAL_PAIRS says
     T.whole = false;
     const pdn_opts& o = c->opts;
     const int n = c->n;
@@ -212,7 +213,7 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
         status = solve_batch(c, L, H, W, T, ch, tsv_src.data() + s0, (int)std::min<size_t>(Bmax, tsv_src.size() - s0), false, o.rtol, o.max_iter, guess);
     if (!term.empty()) {
         // with the terminal rows kept they are ordinary rows of ZT: full tolerance, gathered at every port
-        const bool rows = c->terminal_pairs;
+        const bool rows = c->terminal_pairs && !diag_only_terms;
         for (size_t s0 = 0; s0 < term.size() && status == PDN_OK; s0 += Bmax)
             status = solve_batch(c, L, H, W, T, ch, term.data() + s0, (int)std::min<size_t>(Bmax, term.size() - s0), !rows,
                                  rows ? o.rtol : rtol_term, o.max_iter, guess);
@@ -852,6 +853,118 @@ int pdn_reff_nodes(pdn_ctx* ctx, int32_t n_nodes, const pdn_node* nodes, double*
             }
             gemm(L, np, np, dm1, -1.0, Cs.as<double>(), 1, np, mu.as<double>(), np, 1, 1.0, M.as<double>(), np);
             L.run(KC_PAIR, (double)np * np * 8.0, [&] { k_probe_pairs<<<dim3(cdiv(np, 128), grid_rows(np)), 128, 0, L.s>>>(np, M.as<double>(), out); });
+        }
+        CK(cudaStreamSynchronize(L.s));
+        L.resolve();
+    } catch (const CudaFail& f) {
+        g_last_error = std::string(f.what) + ": " + cudaGetErrorString(f.e);
+        cudaGetLastError();
+        status = f.e == cudaErrorMemoryAllocation ? PDN_E_NOMEM : PDN_E_CUDA;
+    } catch (const StatusFail& f) {
+        g_last_error = f.msg;
+        status = f.status;
+    } catch (const std::bad_alloc&) {
+        g_last_error = "host allocation failed";
+        status = PDN_E_NOMEM;
+    }
+    const int64_t launches = c->stats.kernel_launches, stencil_launches = c->stats.stencil_launches;
+    c->stats = stats0;
+    c->stats.kernel_launches = launches;
+    c->stats.stencil_launches = stencil_launches;
+    return status;
+}
+
+// NEXT-3: one source against many nodes (port.cuh: k_from_scatter has the algebra).
+int pdn_reff_from(pdn_ctx* ctx, const pdn_node* src_node, int32_t n_nodes, const pdn_node* nodes, double* out) {
+    if (!ctx || !src_node || !nodes || !out || n_nodes < 1) return fail_arg("null context / source / node list / output or empty list");
+    PDN_CHECK_DEVICE(ctx);
+    if (ctx->open) return fail_arg("sharded context is still open: exchange the rows and call pdn_finish first");
+    if (ctx->d < 2) return fail_arg("pdn_reff_from needs at least 2 tiers (on one tier list the nodes as bumps and loads)");
+    pdn_ctx* c = ctx;
+    const int d = c->d, n = c->n, dm1 = d - 1, np = n_nodes + 1;
+    std::vector<pdn_node> pr(np);
+    pr[0] = *src_node;
+    for (int a = 1; a < np; ++a) pr[a] = nodes[a - 1];
+    for (int a = 0; a < np; ++a) {
+        if (pr[a].tier < 0 || pr[a].tier >= d) return fail_arg("probe tier out of range");
+        if (pr[a].y < 0 || pr[a].y >= n || pr[a].x < 0 || pr[a].x >= n) return fail_arg("probe site out of range");
+    }
+    int status = PDN_OK;
+    const pdn_stats stats0 = c->stats;  // the solve statistics describe pdn_create / pdn_update_tsvs only
+    try {
+        Launcher L{c, c->stream};
+        std::vector<DevBuf> F(dm1), X(dm1);
+        DevBuf Zd, Zs, qd, qs, G, Cs, mu, d_tier;
+        for (int i = 0; i < dm1; ++i) {
+            F[i].alloc((size_t)c->p[i] * np * sizeof(double));
+            X[i].alloc((size_t)c->p[i] * np * sizeof(double));
+            CK(cudaMemsetAsync(F[i].p, 0, (size_t)c->p[i] * np * sizeof(double), L.s));
+        }
+        Zd.alloc((size_t)np * sizeof(double)); Zs.alloc((size_t)np * sizeof(double));
+        qd.alloc((size_t)np * sizeof(double)); qs.alloc((size_t)np * sizeof(double));
+        for (DevBuf* b : {&Zd, &Zs, &qd, &qs}) CK(cudaMemsetAsync(b->p, 0, (size_t)np * sizeof(double), L.s));
+        std::vector<int> h_tier(np);
+        for (int a = 0; a < np; ++a) h_tier[a] = pr[a].tier;
+        d_tier.alloc((size_t)np * sizeof(int));
+        CK(cudaMemcpyAsync(d_tier.p, h_tier.data(), (size_t)np * sizeof(int), cudaMemcpyHostToDevice, L.s));
+        // ---- per tier with probes: TSV-port solves gathered at the probes (+ the source's own row), one diagonal solve per probe
+        SpectralTables tabs;
+        Hierarchy H;
+        bool h_ready = false;
+        for (int t = 0; t < d && status == PDN_OK; ++t) {
+            std::vector<int> probe;  // columns of the np-wide arrays; the source first if it sits on this tier
+            for (int a = 0; a < np; ++a) if (pr[a].tier == t) probe.push_back(a);
+            if (probe.empty()) continue;
+            const TierPorts& T = c->tiers[t];
+            const bool has_src = pr[0].tier == t;
+            const int k = (int)probe.size(), nrow = T.ntsv + (has_src ? 1 : 0), kterm = k - (has_src ? 1 : 0);
+            TierPorts Tp;
+            Tp.node.assign(T.node.begin(), T.node.begin() + T.ntsv);
+            for (int a : probe) Tp.node.push_back(pr[a].y * pitch_of(n) + pr[a].x);
+            Tp.ntsv = nrow; Tp.nterm = kterm; Tp.q = T.ntsv + k; Tp.nrows = nrow;
+            Tp.d_node.alloc((size_t)Tp.q * sizeof(int));
+            CK(cudaMemcpyAsync(Tp.d_node.p, Tp.node.data(), (size_t)Tp.q * sizeof(int), cudaMemcpyHostToDevice, L.s));
+            Tp.ZT.alloc((size_t)std::max(nrow, 1) * Tp.q * sizeof(double));
+            Tp.zdiag.alloc((size_t)std::max(kterm, 1) * sizeof(double));
+            if (!h_ready) { H.allocate(n); h_ready = true; }
+            status = H.build(L, T.gx0.as<double>(), T.gy0.as<double>(), false, true);
+            if (status != PDN_OK) break;
+            const int Bmax = pick_batch(H, Tp.q, c->opts);
+            Work W;
+            if (H.nlev > 1) W.allocate(H, Bmax, Tp.q);
+            std::vector<int> rows(nrow), term(kterm);
+            for (int j = 0; j < nrow; ++j) rows[j] = j;
+            for (int j = 0; j < kterm; ++j) term[j] = nrow + j;
+            status = reduce_tier(c, L, H, W, Bmax, Tp, rows, term, tabs, true);
+            if (status != PDN_OK) { g_last_error = std::string("tier ") + std::to_string(t) + ": " + pdn_strerror(status); break; }
+            std::vector<int> col(k);
+            for (int j = 0; j < k; ++j) col[j] = T.ntsv + j;
+            DevBuf d_probe, d_col;
+            d_probe.alloc((size_t)k * sizeof(int)); d_col.alloc((size_t)k * sizeof(int));
+            CK(cudaMemcpyAsync(d_probe.p, probe.data(), (size_t)k * sizeof(int), cudaMemcpyHostToDevice, L.s));
+            CK(cudaMemcpyAsync(d_col.p, col.data(), (size_t)k * sizeof(int), cudaMemcpyHostToDevice, L.s));
+            const int plo = t > 0 ? c->p[t - 1] : 0;
+            double* Fup = t < dm1 ? F[t].as<double>() : nullptr;
+            double* Flo = t > 0 ? F[t - 1].as<double>() : nullptr;
+            L.run(KC_DENSE, 0, [&] { k_from_scatter<<<dim3(cdiv((size_t)T.ntsv + 1, 128), grid_rows(k)), 128, 0, L.s>>>(k, T.ntsv, nrow, plo, np, has_src ? T.ntsv : -1, d_col.as<int>(), d_probe.as<int>(), Tp.ZT.as<double>(), Tp.q, Tp.zdiag.as<double>(), Fup, Flo, Zd.as<double>(), Zs.as<double>()); });
+            CK(cudaStreamSynchronize(L.s));  // the host vectors and the tier's buffers are released here
+        }
+        if (status == PDN_OK) {
+            // ---- X = currents of C^-1 [F; Cs] for all np columns; then one row and the diagonal of M
+            for (int i = 0; i < dm1; ++i) CK(cudaMemcpyAsync(X[i].p, F[i].p, (size_t)c->p[i] * np * sizeof(double), cudaMemcpyDeviceToDevice, L.s));
+            block_substitute(c, L, X, np);
+            G.alloc((size_t)dm1 * np * sizeof(double));
+            Cs.alloc((size_t)dm1 * np * sizeof(double));
+            mu.alloc((size_t)dm1 * np * sizeof(double));
+            for (int i = 0; i < dm1; ++i)
+                L.run(KC_DENSE, 0, [&] { k_colsum<<<cdiv(np, 128), 128, 0, L.s>>>(c->p[i], np, X[i].as<double>(), G.as<double>() + (size_t)i * np); });
+            L.run(KC_DENSE, 0, [&] { k_probe_multipliers<<<cdiv(np, 128), 128, 0, L.s>>>(dm1, np, G.as<double>(), c->Sinv.as<double>(), d_tier.as<int>(), Cs.as<double>(), mu.as<double>()); });
+            for (int i = 0; i < dm1; ++i) {
+                const int pi = c->p[i];
+                gemm(L, pi, np, dm1, -1.0, c->KB[i].as<double>(), dm1, 1, mu.as<double>(), np, 1, 1.0, X[i].as<double>(), np);
+                L.run(KC_DENSE, 0, [&] { k_from_dots<<<cdiv(np, 128), 128, 0, L.s>>>(pi, np, F[i].as<double>(), X[i].as<double>(), qd.as<double>(), qs.as<double>()); });
+            }
+            L.run(KC_PAIR, (double)np * 8.0, [&] { k_from_finish<<<cdiv(np, 128), 128, 0, L.s>>>(dm1, np, Cs.as<double>(), mu.as<double>(), Zd.as<double>(), Zs.as<double>(), qd.as<double>(), qs.as<double>(), out); });
         }
         CK(cudaStreamSynchronize(L.s));
         L.resolve();

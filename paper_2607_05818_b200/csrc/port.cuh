@@ -272,6 +272,61 @@ __global__ void k_probe_pairs(int np, const double* __restrict__ M, double* __re
         R[(int64_t)a * np + b] = a == b ? 0.0 : (M[(int64_t)a * np + a] + M[(int64_t)b * np + b]) - (M[(int64_t)a * np + b] + M[(int64_t)b * np + a]);
 }
 
+// One source against many probes (pdn_reff_from): only the row M[s][.] and the diagonal of M are needed, so the
+// probe columns of Z_t at the TSV ports come from the TSV-SOURCE solves gathered at the probes (reciprocity,
+// Z_t[tsv, a] = x_tsv[a]) and every probe costs only a diagonal (second-order, loosely converged) solve.
+//   Zp: rows = the tier's TSV ports [+ the source if it sits on this tier] (nrow of them), columns = [those rows'
+//   ports] ++ [the other probes] (q = nrow + k); zd[j] = Z_t[a_j, a_j] of the other probes; col[j] = column of probe j
+//   in Zp, probe[j] = its column in the np-wide arrays; src_row = row of the source in Zp or -1.
+__global__ void k_from_scatter(int nprobe, int ntsv, int nrow, int plo, int np, int src_row, const int* __restrict__ col,
+                               const int* __restrict__ probe, const double* __restrict__ Zp, int64_t q,
+                               const double* __restrict__ zd, double* __restrict__ Fup, double* __restrict__ Flo,
+                               double* __restrict__ Zd, double* __restrict__ Zs) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    for (int j = blockIdx.y; j < nprobe; j += gridDim.y) {
+        const int c = col[j], a = probe[j];
+        if (r < ntsv) {
+            const double v = Zp[(int64_t)r * q + c];
+            if (r < plo) { if (Flo) Flo[(int64_t)r * np + a] = -v; }
+            else if (Fup) Fup[(int64_t)(r - plo) * np + a] = v;
+        } else if (r == ntsv) {
+            Zd[a] = c < nrow ? Zp[(int64_t)c * q + c] : zd[c - nrow];
+            Zs[a] = src_row >= 0 ? Zp[(int64_t)src_row * q + c] : 0.0;
+        }
+    }
+}
+
+// qd[a] += sum_r F[r][a] X[r][a],  qs[a] += sum_r F[r][0] X[r][a]   (one interface block; column 0 is the source)
+__global__ void k_from_dots(int p, int np, const double* __restrict__ F, const double* __restrict__ X,
+                            double* __restrict__ qd, double* __restrict__ qs) {
+    const int a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= np) return;
+    double d = 0.0, s = 0.0;
+    for (int r = 0; r < p; ++r) {
+        const double x = X[(int64_t)r * np + a];
+        d = fma(F[(int64_t)r * np + a], x, d);
+        s = fma(F[(int64_t)r * np], x, s);
+    }
+    qd[a] += d;
+    qs[a] += s;
+}
+
+// R(s, a) = M_ss + M_aa - 2 M_sa,  M_ab = Zloc_ab - (F_a . X_b + Cs_a . mu_b);  out[a - 1] for the probes a >= 1
+__global__ void k_from_finish(int dm1, int np, const double* __restrict__ Cs, const double* __restrict__ mu,
+                              const double* __restrict__ Zd, const double* __restrict__ Zs, const double* __restrict__ qd,
+                              const double* __restrict__ qs, double* __restrict__ out) {
+    const int a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a < 1 || a >= np) return;
+    double cd = 0.0, cs = 0.0, c0 = 0.0;
+    for (int i = 0; i < dm1; ++i) {
+        cd = fma(Cs[(int64_t)i * np + a], mu[(int64_t)i * np + a], cd);
+        cs = fma(Cs[(int64_t)i * np], mu[(int64_t)i * np + a], cs);
+        c0 = fma(Cs[(int64_t)i * np], mu[(int64_t)i * np], c0);
+    }
+    const double mss = Zd[0] - (qd[0] + c0), maa = Zd[a] - (qd[a] + cd), msa = Zs[a] - (qs[a] + cs);
+    out[a - 1] = (mss + maa) - 2.0 * msa;
+}
+
 // Eq. (4): with bump b at v_bump and load k drawing I[k],
 //   v[j] = v_bump - 1/2 sum_k I[k] ( R_b[j] + R_b[k] - R_LL[j][k] )       one warp per load j
 __global__ void k_load_voltages(int n, const double* __restrict__ Rb, const double* __restrict__ RLL,

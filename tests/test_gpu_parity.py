@@ -371,6 +371,16 @@ def test_arbitrary_tier_endpoints_against_the_oracle(seed, d, n, p, kw):
         full = torch.empty(net.m * net.nl, dtype=torch.float64, device="cuda:0")
         pdn.reff(full)
         assert abs(got[k - 3, k - 2] / full.cpu().numpy().reshape(net.m, net.nl)[0, 2] - 1.0) <= 1e-8
+        # pdn_reff_from: one source against all the others (one row of the same matrix, by diagonal solves +
+        # reciprocity), for a source on the top tier, on a middle / bottom tier and on a TSV site
+        for s_ in (0, 3, 9):
+            row = torch.empty(k, dtype=torch.float64, device="cuda:0")
+            pdn.reff_from(nodes[s_], nodes, row)
+            r_ = row.cpu().numpy()
+            nzr = want[s_] > 0
+            relr = np.abs(r_[nzr] - want[s_][nzr]) / want[s_][nzr]
+            assert relr.max() <= MAX_REL and relr.mean() <= MEAN_REL, (s_, relr.max(), relr.mean())
+            assert np.abs(r_[~nzr]).max() <= 1e-8 * want.max()
 
     check(Oracle(net))
     if n > 4:
@@ -667,6 +677,13 @@ def test_randomised_stacks_through_every_entry_point(block, rtol):
         gid = nodes[:, 0].astype(np.int64) * n * n + nodes[:, 1] * n + nodes[:, 2]
         want = np.array([[o.reff_nodes(int(a), int(b)) for b in gid] for a in gid])
         assert rel_err(rn.cpu().numpy().reshape(k, k), want) <= 1e-8, what
+        row = torch.empty(k, dtype=torch.float64, device="cuda:0")     # pdn_reff_from: the first probe against all of them
+        pdn.reff_from(nodes[0], nodes, row)
+        if rtol is None:
+            assert rel_err(row.cpu().numpy(), want[0]) <= 1e-8, what
+        else:   # the probes' diagonals come from loosely converged (second-order) solves whatever rtol is
+            nz0 = want[0] > 0
+            assert np.abs(row.cpu().numpy()[nz0] / want[0][nz0] - 1.0).max(initial=0.0) <= 1e-7, what
         if n * n > p + 1:
             new = [x for x in P._distinct_sites(np.random.default_rng(seed + 5), n, min(n * n, p + 3)).tolist()
                    if x not in net.tsv_site[0].tolist()][:1]
