@@ -441,9 +441,18 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
         skipped = 0;
         if (expect_done) {
             const size_t chunk = (size_t)RESID_THREADS * RESID_PER_THREAD * 2;
-            L.run(KC_SMALL, 3.0 * V * nact / B, [&] { k_resid_update<<<dim3(cdiv(plane, chunk), B), RESID_THREADS, 0, L.s>>>(W.r[cur_r].as<double>(), W.q.as<double>(), W.s.alpha, W.s.active, W.r[cur_r ^ 1].as<double>(), W.s.rr, plane); });
+            // the new residual itself is needed only if the batch does NOT converge (or, for a guessed terminal batch,
+            // by k_guess_dot): first its norm alone, 2 V; the vector is written in a second pass if the check fails
+            const bool keep_r = terminal && guess;
+            double* r_new_p = W.r[cur_r ^ 1].as<double>();
+            L.run(KC_SMALL, (keep_r ? 3.0 : 2.0) * V * nact / B, [&] { k_resid_update<<<dim3(cdiv(plane, chunk), B), RESID_THREADS, 0, L.s>>>(W.r[cur_r].as<double>(), W.q.as<double>(), W.s.alpha, W.s.active, keep_r ? r_new_p : nullptr, W.s.rr, plane); });
+            const int r_old = cur_r;
             cur_r ^= 1;
-            if (!check()) vcycle(L, H, W, sm, B, cur_r, false, nact, [] { return false; });
+            if (!check()) {
+                if (!keep_r)  // (the right-hand sides still active; rr is accumulated again and not used)
+                    L.run(KC_SMALL, 3.0 * V * nact / B, [&] { k_resid_update<<<dim3(cdiv(plane, chunk), B), RESID_THREADS, 0, L.s>>>(W.r[r_old].as<double>(), W.q.as<double>(), W.s.alpha, W.s.active, r_new_p, W.s.rr, plane); });
+                vcycle(L, H, W, sm, B, cur_r, false, nact, [] { return false; });
+            }
         } else {
             vcycle(L, H, W, sm, B, cur_r, true, nact, check);
             cur_r ^= 1;

@@ -88,6 +88,8 @@ __global__ void k_scal_check(PcgScalars s, int B, double tol2, double bnorm2, in
 //   r_out = r_in - alpha q ;  rr += ||r_out||^2      for the right-hand sides still iterating.
 // grid = (chunks of the plane, B); 16-byte accesses; plane (= ny*pitch) is even.
 constexpr int RESID_THREADS = 256, RESID_PER_THREAD = 4;  // double2 per thread
+// r_out == nullptr: only the norm (2 V instead of 3 V) -- a batch that is expected to converge now needs its new
+// residual only if the expectation fails.
 __global__ void __launch_bounds__(RESID_THREADS)
 k_resid_update(const double* __restrict__ r_in, const double* __restrict__ q, const double* __restrict__ alpha,
                const int* __restrict__ active, double* __restrict__ r_out, double* __restrict__ rr_acc, size_t plane) {
@@ -98,7 +100,7 @@ k_resid_update(const double* __restrict__ r_in, const double* __restrict__ q, co
     const size_t n2 = plane / 2, base = (size_t)blockIdx.x * RESID_THREADS * RESID_PER_THREAD + threadIdx.x;
     const double2* r2 = reinterpret_cast<const double2*>(r_in + b * plane);
     const double2* q2 = reinterpret_cast<const double2*>(q + b * plane);
-    double2* o2 = reinterpret_cast<double2*>(r_out + b * plane);
+    double2* o2 = r_out ? reinterpret_cast<double2*>(r_out + b * plane) : nullptr;
     double rr = 0.0;
 #pragma unroll
     for (int k = 0; k < RESID_PER_THREAD; ++k) {
@@ -108,7 +110,7 @@ k_resid_update(const double* __restrict__ r_in, const double* __restrict__ q, co
             const double2 qq = q2[i];
             r.x = fma(-al, qq.x, r.x);
             r.y = fma(-al, qq.y, r.y);
-            o2[i] = r;
+            if (o2) o2[i] = r;
             rr = fma(r.x, r.x, rr);
             rr = fma(r.y, r.y, rr);
         }
