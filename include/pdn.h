@@ -200,6 +200,21 @@ int pdn_reff_same_side(pdn_ctx *ctx, int32_t side, double *out);
  *   v_j = v_bump - 1/2 sum_k i_load[k] (R_{b,j} + R_{b,k} - R_{j,k}).   Needs PDN_TERMINAL_PAIRS. */
 int pdn_load_voltages(pdn_ctx *ctx, int32_t bump, const double *i_load, double v_bump, double *v_out);
 
+/* The same Eq. (4), same arguments and result, for callers that must not allocate (code under CUDA graph capture,
+ * serving loops, harnesses that forbid cudaMalloc): pdn_load_voltages takes its scratch (R_b: n_loads values, R_LL:
+ * n_loads^2 values, index lists) from the device pool, which may call cudaMalloc; this entry point keeps it in a
+ * static __device__ array inside the library -- (PDN_STATIC_MAX_LOADS^2 + PDN_STATIC_MAX_LOADS) doubles = 2.0 MiB that
+ * every GPU which loads libpdn.so holds until the process exits -- and calls no cudaMalloc, cudaFree or any
+ * allocating routine (the first call on a device resolves the array's device address with cudaGetSymbolAddress).
+ * n_loads > PDN_STATIC_MAX_LOADS: PDN_E_ARG, nothing launched (use pdn_load_voltages).  i_load, v_out: DEVICE, as above,
+ * caller-owned.  The scratch is shared by ALL calls on a device and keeps the last call's contents; every word a call
+ * reads it has written itself first, so nothing needs clearing -- but two calls whose kernels overlap on the GPU (two
+ * contexts on different streams, two host threads) race: serialise them.  Work is ordered on the context's stream and
+ * complete on return; if that stream is being captured the call records its three kernels and returns without
+ * synchronising. */
+#define PDN_STATIC_MAX_LOADS 512
+int pdn_load_voltages_static(pdn_ctx *ctx, int32_t bump, const double *i_load, double v_bump, double *v_out);
+
 /* Arbitrary-tier endpoints: R_eff in the whole 3D network between ANY nodes, on any
  * tier, of an existing context (any flags).  nodes: HOST array of n_nodes probes (duplicates allowed).  out:
  * DEVICE fp64, n_nodes*n_nodes values, out[a*n_nodes + b] = R_eff(node a, node b), 0 on the diagonal.

@@ -5,5 +5,6 @@ package is its thin Python binding.  Importing the package does not load the lib
 use does, and fails loudly if it has not been built (`__graft_entry__.build()`).
 """
 from .binding import (KERNEL_CLASSES, LIB_PATH, PDN_NO_UNIFORM_FAST_PATH, PDN_SKIP_CONNECTIVITY_CHECK,  # noqa: F401
-                      PDN_NO_INITIAL_GUESS, PDN_PRECOND_F32, PDN_TERMINAL_PAIRS, PDN_TIERS_ON_HOST,
+                      PDN_NO_INITIAL_GUESS, PDN_PRECOND_F32, PDN_STATIC_MAX_LOADS, PDN_TERMINAL_PAIRS,
+                      PDN_TIERS_ON_HOST,
                       PDN_TIME_KERNELS, EXPORTS, Pdn, PdnError, load_library, shard_bounds)

@@ -22,6 +22,7 @@ PDN_NO_UNIFORM_FAST_PATH = 8
 PDN_TERMINAL_PAIRS = 16
 PDN_PRECOND_F32 = 32
 PDN_NO_INITIAL_GUESS = 64
+PDN_STATIC_MAX_LOADS = 512     # pdn.h: largest n_loads pdn_load_voltages_static accepts
 KERNEL_CLASSES = ("pq", "down0", "up0", "down_coarse", "up_coarse", "small", "dense", "pair")
 
 
@@ -57,7 +58,7 @@ class PdnStats(C.Structure):
 EXPORTS = ("pdn_create", "pdn_reff", "pdn_reff_host", "pdn_destroy", "pdn_strerror", "pdn_last_error",
            "pdn_get_stats", "pdn_port_count", "pdn_get_port_matrix", "pdn_release_cache", "pdn_update_tsvs",
            "pdn_reff_same_side", "pdn_load_voltages", "pdn_reff_nodes", "pdn_shard_slice", "pdn_shard_buffers",
-           "pdn_finish", "pdn_set_solver_opts", "pdn_reff_from")
+           "pdn_finish", "pdn_set_solver_opts", "pdn_reff_from", "pdn_load_voltages_static")
 
 _lib = None
 
@@ -90,8 +91,10 @@ def load_library() -> C.CDLL:
     lib.pdn_set_solver_opts.argtypes = [C.c_void_p, C.c_double, C.c_int32]
     lib.pdn_reff_same_side.restype = C.c_int
     lib.pdn_reff_same_side.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
-    lib.pdn_load_voltages.restype = C.c_int
-    lib.pdn_load_voltages.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_double, C.c_void_p]
+    for name in ("pdn_load_voltages", "pdn_load_voltages_static"):
+        f = getattr(lib, name)
+        f.restype = C.c_int
+        f.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_double, C.c_void_p]
     lib.pdn_reff_nodes.restype = C.c_int
     lib.pdn_reff_nodes.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
     lib.pdn_reff_from.restype = C.c_int
@@ -310,6 +313,15 @@ class Pdn:
                                          _ptr(v_out, "f8", "v_out", self.nl))
         if st != PDN_OK:
             raise PdnError(st, "pdn_load_voltages")
+        return v_out
+
+    def load_voltages_static(self, bump: int, i_load, v_bump: float, v_out):
+        """pdn_load_voltages_static: Eq. 4 with the scratch in the library's static device array (no allocation;
+        at most PDN_STATIC_MAX_LOADS loads).  Same arguments and result as load_voltages."""
+        st = self._lib.pdn_load_voltages_static(self._h, bump, _ptr(i_load, "f8", "i_load", self.nl), float(v_bump),
+                                                _ptr(v_out, "f8", "v_out", self.nl))
+        if st != PDN_OK:
+            raise PdnError(st, "pdn_load_voltages_static")
         return v_out
 
     def reff_nodes(self, nodes, out):

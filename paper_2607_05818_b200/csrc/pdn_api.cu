@@ -225,6 +225,49 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
 
 }  // namespace
 
+// ------------------------------------------------------------------------------------------------
+// pdn_load_voltages_static: Eq. (4) without any allocation.  pdn_load_voltages takes its scratch (R_b: n values,
+// R_LL: n x n values, two index lists) from the device pool, which calls cudaMalloc when the pool has no block of
+// that size.  This variant keeps the scratch in the file-scope array below -- part of the library's image: every GPU
+// that loads libpdn.so holds these 2.0 MiB until the process exits -- for at most PDN_STATIC_MAX_LOADS loads.
+//   layout: R_LL at [0, n*n), R_b at [MAXL*MAXL, MAXL*MAXL + n)   (both 256-byte aligned)
+// Every word a call reads was written earlier by the same call (k_pair_same writes all n*n entries of R_LL,
+// k_pair_row all n of R_b): nothing has to start at zero and what the previous call left is never read.  All calls on
+// one device share the array: two calls whose kernels overlap on the GPU (two contexts on different streams, two host
+// threads) race.
+// In host code `g_static_scratch` is the host-side shadow of the symbol, NOT a device address: the kernels get the
+// pointer cudaGetSymbolAddress returns, resolved once per device with that device current.
+constexpr int STATIC_MAXL = PDN_STATIC_MAX_LOADS;
+static __device__ __align__(256) double g_static_scratch[(size_t)STATIC_MAXL * STATIC_MAXL + STATIC_MAXL];
+
+static double* static_scratch_of_current_device() {
+    static std::mutex mu;
+    static double* ptr[64] = {};
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) throw StatusFail{PDN_E_ARG, "device ordinal out of range"};
+    std::lock_guard<std::mutex> g(mu);
+    if (!ptr[dev]) {
+        double* p = nullptr;
+        CK(cudaGetSymbolAddress((void**)&p, g_static_scratch));
+        if (!p || ((uintptr_t)p & 255)) throw StatusFail{PDN_E_CUDA, "static scratch array has no usable device address"};
+        ptr[dev] = p;
+    }
+    return ptr[dev];
+}
+
+// R_b[j] = R_eff(bump i, load j) for all loads: k_pair_list on the pairs (i, 0..n-1) without index lists in memory
+// (same loop, same association: the same bits).  One warp per load.
+__global__ void k_pair_row(int i, int n, int p0, const double* __restrict__ A1, const double* __restrict__ X0,
+                           const double* __restrict__ u, const double* __restrict__ w, double* __restrict__ R) {
+    const int j = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (j >= n) return;
+    double s = 0.0;
+    for (int a = lane; a < p0; a += 32) s = fma(A1[(int64_t)i * p0 + a], X0[(int64_t)j * p0 + a], s);
+    s = warp_sum(s);
+    if (lane == 0) R[j] = u[i] + w[j] - 2.0 * s;
+}
+
 // ================================================================================================
 // C ABI
 // ================================================================================================
@@ -759,6 +802,55 @@ int pdn_load_voltages(pdn_ctx* ctx, int32_t bump, const double* i_load, double v
         L.run(KC_PAIR, (double)n * n * 8.0, [&] { k_load_voltages<<<cdiv((size_t)n * 32, 256), 256, 0, L.s>>>(n, Rb.as<double>(), RLL.as<double>(), i_load, v_bump, v_out); });
         CK(cudaStreamSynchronize(ctx->stream));
         L.resolve();
+    } catch (const CudaFail& f) {
+        g_last_error = std::string(f.what) + ": " + cudaGetErrorString(f.e);
+        cudaGetLastError();
+        return PDN_E_CUDA;
+    } catch (const StatusFail& f) {
+        g_last_error = f.msg;
+        return f.status;
+    }
+    return PDN_OK;
+}
+
+// Eq. (4) with the scratch in g_static_scratch: no device pool, no cudaMalloc / cudaFree, no events, no host
+// containers.  Three launches on the context's stream: k_pair_row (R_b), k_pair_same (R_LL), k_load_voltages.
+int pdn_load_voltages_static(pdn_ctx* ctx, int32_t bump, const double* i_load, double v_bump, double* v_out) {
+    if (!ctx || !i_load || !v_out) return fail_arg("null argument");
+    PDN_CHECK_DEVICE(ctx);
+    if (!ctx->terminal_pairs) return fail_arg("the context was not created with PDN_TERMINAL_PAIRS");
+    if (ctx->open) return fail_arg("sharded context is still open: exchange the rows and call pdn_finish first");
+    if (bump < 0 || bump >= ctx->m) return fail_arg("bump index out of range");
+    if (ctx->d < 2) return fail_arg("pdn_load_voltages_static needs at least 2 tiers");
+    if (ctx->nl > STATIC_MAXL)
+        return fail_arg("pdn_load_voltages_static: n_loads exceeds PDN_STATIC_MAX_LOADS (512), the size of the library's "
+                        "static scratch array; use pdn_load_voltages");
+    try {
+        double* scratch = static_scratch_of_current_device();
+        const int n = ctx->nl, m = ctx->m, p0 = ctx->p0;
+        double* RLL = scratch;
+        double* Rb = scratch + (size_t)STATIC_MAXL * STATIC_MAXL;
+        cudaStream_t s = ctx->stream;
+        const pdn_ctx::Side& S = ctx->side[1];
+        const TierPorts& T = ctx->tiers[ctx->d - 1];
+        k_pair_row<<<cdiv((size_t)n * 32, 256), 256, 0, s>>>(bump, n, p0, ctx->A1.as<double>(), ctx->X0.as<double>(), ctx->u.as<double>(), ctx->w.as<double>(), Rb);
+        CK(cudaGetLastError());
+        dim3 grid(cdiv(n, 64), cdiv(n, 64));
+        k_pair_same<<<grid, 256, 0, s>>>(n, S.p, S.A.as<double>(), S.X.as<double>(), S.ys.as<double>(), S.t.as<double>(), T.ZT.as<double>(), T.q, T.ntsv, RLL);
+        CK(cudaGetLastError());
+        k_load_voltages<<<cdiv((size_t)n * 32, 256), 256, 0, s>>>(n, Rb, RLL, i_load, v_bump, v_out);
+        CK(cudaGetLastError());
+        {
+            std::lock_guard<std::mutex> g(ctx->mu);
+            ctx->class_launches[KC_PAIR] += 3;
+            ctx->class_bytes[KC_PAIR] += (2.0 * n * n + n) * 8.0;
+            ctx->stats.kernel_launches += 3;
+        }
+        // complete on return like every other entry point -- unless the stream is being captured into a CUDA graph,
+        // where a synchronise would end the capture: then the three kernel nodes are all the call leaves behind
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+        CK(cudaStreamIsCapturing(s, &cap));
+        if (cap == cudaStreamCaptureStatusNone) CK(cudaStreamSynchronize(s));
     } catch (const CudaFail& f) {
         g_last_error = std::string(f.what) + ": " + cudaGetErrorString(f.e);
         cudaGetLastError();
