@@ -13,6 +13,7 @@
 // x0 = 0 on the device (k_guess_check + k_init_rhs with the keep mask).
 #pragma once
 #include "common.cuh"
+#include "stencil3.cuh"
 #include "uniform.cuh"
 
 namespace pdn {
@@ -66,117 +67,182 @@ __device__ __forceinline__ double guess_x0(const GuessTable& t, int y, int x, in
 }
 
 // r0[b] = b - L x0 on the pitched plane, rr0[b] += ||r0||^2, sumx[b] += sum(x0).
-// grid = (tiles_x * tiles_y, ceil(B / GR)); block = GUESS_THREADS; a thread owns a 2 x 2 patch of the GUESS_TY x
-// GUESS_TX tile (its conductances in registers) and loops over GR right-hand sides; per right-hand side the block
-// tabulates x0 on the tile plus one ring (shared memory, double buffered: one __syncthreads per right-hand side;
-// mesh column j of the tile sits at index j + 2 of a 68-wide row, so that column pairs are 16-byte aligned) and
-// applies the 5-point operator with 16-byte shared loads and global stores.  Everything that does not depend on
-// the right-hand side is set up once per block.
-constexpr int GUESS_TX = 64, GUESS_TY = 16, GUESS_THREADS = 256;
-__global__ void __launch_bounds__(GUESS_THREADS)
-k_guess_rhs(GuessTable tab, Level L, const int* __restrict__ node, const int* __restrict__ src, double inv_n2,
-            double* __restrict__ r0, double* __restrict__ rr0, double* __restrict__ sumx, int B, int GR) {
-    constexpr int XW = GUESS_TX + 4, XH = GUESS_TY + 2, EPR = GUESS_TX / 2 + 2, NENT = XH * EPR;  // entries per ring row: 32 pairs + 2 singles
-    constexpr int PER = (NENT + GUESS_THREADS - 1) / GUESS_THREADS;
-    static_assert((GUESS_TX / 2) * (GUESS_TY / 2) == GUESS_THREADS, "one 2 x 2 patch per thread");
-    __shared__ __align__(16) double xs0[2][XH * XW];
-    __shared__ double part[2][2][GUESS_THREADS / 32];  // per-warp partial sums of the two reductions, double buffered
-    const int tiles_x = (L.nx + GUESS_TX - 1) / GUESS_TX;
-    const int tx0 = (blockIdx.x % tiles_x) * GUESS_TX, ty0 = (blockIdx.x / tiles_x) * GUESS_TY;
+//
+// The table windows are staged by TMA.  For one right-hand side (source column xs, row ys) the nodes of a tile of
+// 64 x TY mesh nodes plus its ring use, in each of the four index combinations, a CONTIGUOUS window of at most
+// (TY + 2) x 66 table entries: over consecutive x the difference index |x - xs| runs down to 0 left of the source and
+// up again right of it, and the folded sum index f(x + xs + 1) runs up to n and back down -- a run or a V, never a
+// gap.  So the block asks the TMA unit for four 2D boxes of the table (origin = the smallest index the tile uses,
+// guess_origin) per right-hand side, NST stages ahead, and its threads read them with 4-byte shared loads at
+// row * 72 + column -- forwards or backwards, conflict-free either way -- instead of gathering sixteen bytes per node
+// from L2 through the L1TEX path (round 2's first version: 7 us per right-hand side at 1024^2, L1TEX-bound).
+// The innermost box coordinate has to be a multiple of 16 bytes (an odd one is an illegal instruction), so the column
+// origin is rounded down to a multiple of four entries and the box is 72 wide: 66 entries used, up to 3 skipped.
+// grid = (tiles_x * tiles_y, ceil(B / GR)); block = W warps; lane l of warp w owns columns 2l, 2l+1 and rows
+// R w .. R w + R - 1 of the tile with its conductances in registers, evaluates x0 on those rows and the two beside
+// them, gets the columns beside its own from the neighbouring lanes (lanes 0 and 31 look their ring column up) and
+// applies the 5-point operator.  One __syncthreads per right-hand side (stage consumed -> refill).
+constexpr int GW_TX = 64, GW_BW = 72, GW_MAX_GR = 64;
+
+__device__ __forceinline__ int guess_fold(int t, int n) { return t <= n ? t : 2 * n - t; }
+
+// smallest |x - s| (a_d) and smallest f(x + s + 1) (a_s) over the mesh coordinates x in [lo, hi]
+__device__ __forceinline__ void guess_origin(int lo, int hi, int s, int n, int& a_d, int& a_s) {
+    a_d = max(max(lo - s, s - hi), 0);
+    const int tlo = lo + s + 1, thi = hi + s + 1;
+    a_s = thi <= n ? tlo : (tlo > n ? 2 * n - thi : min(tlo, 2 * n - thi));
+}
+
+template <int R, int W>
+struct GuessGeom {
+    static constexpr int TY = R * W, BH = TY + 2;
+    static constexpr int WIN = (BH * GW_BW + 31) & ~31;  // floats per window, a multiple of 128 bytes (TMA destination)
+    static constexpr uint32_t BOX_BYTES = BH * GW_BW * sizeof(float);
+    static constexpr size_t STAGE_BYTES = 4 * (size_t)WIN * sizeof(float);
+};
+
+template <int R, int W, int NST>
+__global__ void __launch_bounds__(32 * W)
+k_guess_rhs(const __grid_constant__ CUtensorMap tm_tab, double scale, Level L, const int* __restrict__ node,
+            const int* __restrict__ src, double inv_n2, double* __restrict__ r0, double* __restrict__ rr0,
+            double* __restrict__ sumx, int B, int GR) {
+    using Gm = GuessGeom<R, W>;
+    constexpr int TY = Gm::TY, WIN = Gm::WIN;
+    extern __shared__ __align__(128) float win[];  // NST stages x 4 windows: (dy,dx) (sy,sx) (dy,sx) (sy,dx)
+    __shared__ uint64_t mbar[NST];
+    __shared__ int s_xs[GW_MAX_GR], s_ys[GW_MAX_GR];
+    __shared__ double part[2][2][W];  // per-warp partial sums of the two reductions, double buffered
+    const int n = L.nx;               // tiers are square: the table is (n + 1) x (n + 1)
+    const int tiles_x = (L.nx + GW_TX - 1) / GW_TX;
+    const int tx0 = (blockIdx.x % tiles_x) * GW_TX, ty0 = (blockIdx.x / tiles_x) * TY;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    // the block's partial sums of right-hand side b go out as ONE atomic per quantity (1024 blocks add to the same two
-    // words per right-hand side: per-warp atomics were the kernel's bottleneck), one iteration later: after the next
-    // __syncthreads the eight per-warp values are visible to threads 0 and 1
+    const int b0 = blockIdx.y * GR, nb = min(GR, B - b0);
+    for (int j = tid; j < nb; j += 32 * W) {
+        const int so = node[src[b0 + j]];
+        s_ys[j] = so / L.pitch;
+        s_xs[j] = so % L.pitch;
+    }
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < NST; ++s) mbar_init(&mbar[s], 1);
+        mbar_fence_init();
+    }
+    // mesh coordinates the tile and its ring use (clamped to the mesh: what lies outside is never multiplied by a
+    // non-zero conductance, but its index has to stay inside the window)
+    const int xlo = max(tx0 - 1, 0), xhi = min(tx0 + GW_TX, L.nx - 1);
+    const int ylo = max(ty0 - 1, 0), yhi = min(ty0 + TY, L.ny - 1);
+    // ---- per-thread constants of the operator
+    const int x = tx0 + 2 * lane, y = ty0 + R * warp;
+    double ge0[R], ge1[R], gw[R], gs0[R], gs1[R], gn0 = 0.0, gn1 = 0.0;  // east of both columns, west of column 0, south
+    unsigned in0 = 0, in1 = 0, rowin = 0;  // bit i: node (y + i, x) / (y + i, x + 1) is a mesh node; the row pair is addressable
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+        const int yy = y + i;
+        const bool ok = yy < L.ny && x < L.pitch;  // x and pitch are even: both columns are addressable (pads hold zeros)
+        const size_t o = (size_t)yy * L.pitch + x;
+        const double2 e = ok ? ldg2(L.gx + o) : make_double2(0.0, 0.0);
+        const double2 s = ok ? ldg2(L.gy + o) : make_double2(0.0, 0.0);
+        ge0[i] = e.x; ge1[i] = e.y; gs0[i] = s.x; gs1[i] = s.y;
+        gw[i] = (ok && x > 0) ? __ldg(L.gx + o - 1) : 0.0;
+        if (ok) rowin |= 1u << i;
+        if (ok && x < L.nx) in0 |= 1u << i;
+        if (ok && x + 1 < L.nx) in1 |= 1u << i;
+    }
+    if (y > 0 && y - 1 < L.ny && x < L.pitch) {
+        const double2 s = ldg2(L.gy + (size_t)(y - 1) * L.pitch + x);
+        gn0 = s.x; gn1 = s.y;
+    }
+    const int xc0 = min(x, n - 1), xc1 = min(x + 1, n - 1);
+    const bool edge = lane == 0 || lane == 31;
+    const int xce = lane == 0 ? max(x - 1, 0) : min(x + 2, n - 1);  // the ring column of lanes 0 / 31
+    const size_t plane = (size_t)L.ny * L.pitch;
+    __syncthreads();
+    auto fetch = [&](int j) {  // thread 0 only
+        const int st = j % NST;
+        float* w = win + (size_t)st * 4 * WIN;
+        int adx, asx, ady, asy;
+        guess_origin(xlo, xhi, s_xs[j], n, adx, asx);
+        guess_origin(ylo, yhi, s_ys[j], n, ady, asy);
+        adx &= ~3; asx &= ~3;
+        mbar_expect_tx(&mbar[st], 4 * Gm::BOX_BYTES);
+        tma_load_2d(w, &tm_tab, adx, ady, &mbar[st]);
+        tma_load_2d(w + WIN, &tm_tab, asx, asy, &mbar[st]);
+        tma_load_2d(w + 2 * WIN, &tm_tab, asx, ady, &mbar[st]);
+        tma_load_2d(w + 3 * WIN, &tm_tab, adx, asy, &mbar[st]);
+    };
+    if (tid == 0)
+        for (int j = 0; j < NST && j < nb; ++j) fetch(j);
+    // the block's partial sums of right-hand side b go out as ONE atomic per quantity, one iteration later: after the
+    // next __syncthreads the per-warp values are visible to threads 0 and 1
     auto flush = [&](int bb, int pb) {
         if (tid < 2) {
             double v = 0.0;
 #pragma unroll
-            for (int w = 0; w < GUESS_THREADS / 32; ++w) v += part[pb][tid][w];
+            for (int w = 0; w < W; ++w) v += part[pb][tid][w];
             atomicAdd((tid == 0 ? rr0 : sumx) + bb, v);
         }
     };
-    // ---- per-thread constants of the tabulation
-    int ey[PER], ex[PER], eo[PER], ekind[PER];  // mesh row, first mesh column, offset in xs0; -1 nothing, 0 zeros, 1 pair, 2 first only, 3 single
+    for (int j = 0; j < nb; ++j) {
+        const int b = b0 + j, st = j % NST, buf = j & 1;
+        const int xs = s_xs[j], ys = s_ys[j];
+        int adx, asx, ady, asy;
+        guess_origin(xlo, xhi, xs, n, adx, asx);
+        guess_origin(ylo, yhi, ys, n, ady, asy);
+        adx &= ~3; asx &= ~3;
+        const int cd0 = abs(xc0 - xs) - adx, cd1 = abs(xc1 - xs) - adx, cde = abs(xce - xs) - adx;
+        const int cs0 = guess_fold(xc0 + xs + 1, n) - asx, cs1 = guess_fold(xc1 + xs + 1, n) - asx, cse = guess_fold(xce + xs + 1, n) - asx;
+        const float* wdd = win + (size_t)st * 4 * WIN;
+        const float *wss = wdd + WIN, *wds = wdd + 2 * WIN, *wsd = wdd + 3 * WIN;
+        mbar_wait(&mbar[st], (j / NST) & 1);
+        float f0[R + 2], f1[R + 2], fe[R];  // rows y - 1 .. y + R of the two columns; rows y .. y + R - 1 of the ring column
 #pragma unroll
-    for (int k = 0; k < PER; ++k) {
-        const int i = tid + k * GUESS_THREADS, ry = i / EPR, e = i % EPR;
-        ey[k] = ty0 + ry - 1;
-        const bool row_ok = ey[k] >= 0 && ey[k] < L.ny;
-        if (e < GUESS_TX / 2) {  // columns 2e, 2e+1 of the tile
-            ex[k] = tx0 + 2 * e; eo[k] = ry * XW + 2 * e + 2;
-            ekind[k] = i >= NENT ? -1 : (!row_ok || ex[k] >= L.nx) ? 0 : ex[k] + 1 < L.nx ? 1 : 2;
-        } else {                 // ring column -1 (e == 32) or GUESS_TX (e == 33)
-            const int j = e == GUESS_TX / 2 ? -1 : GUESS_TX;
-            ex[k] = tx0 + j; eo[k] = ry * XW + j + 2;
-            ekind[k] = i >= NENT ? -1 : (row_ok && ex[k] >= 0 && ex[k] < L.nx) ? 3 : 4;  // 4: a single zero
+        for (int i = 0; i < R + 2; ++i) {
+            const int yy = min(max(y - 1 + i, 0), L.ny - 1);
+            const int rd = (abs(yy - ys) - ady) * GW_BW, rs = (guess_fold(yy + ys + 1, n) - asy) * GW_BW;
+            f0[i] = guess_sum4(wdd[rd + cd0], wss[rs + cs0], wds[rd + cs0], wsd[rs + cd0]);
+            f1[i] = guess_sum4(wdd[rd + cd1], wss[rs + cs1], wds[rd + cs1], wsd[rs + cd1]);
+            if (i >= 1 && i <= R && edge) fe[i - 1] = guess_sum4(wdd[rd + cde], wss[rs + cse], wds[rd + cse], wsd[rs + cde]);
         }
-    }
-    // ---- per-thread constants of the operator: patch rows 2 pr, 2 pr + 1, columns 2 pc, 2 pc + 1
-    const int pc = tid % (GUESS_TX / 2), pr = tid / (GUESS_TX / 2), x = tx0 + 2 * pc, y = ty0 + 2 * pr;
-    double ge[2][2], gw[2], gs[2][2], gn[2];  // east of both columns, west of column 0; south of both rows, north of row 0
-    bool in[2][2];
+        __syncthreads();  // the stage is consumed; the partial sums of the previous right-hand side are visible
+        if (tid == 0 && j + NST < nb) fetch(j + NST);
+        if (j > 0) flush(b - 1, buf ^ 1);
+        double v0[R + 2], v1[R + 2];
 #pragma unroll
-    for (int i = 0; i < 2; ++i)
-#pragma unroll
-        for (int j = 0; j < 2; ++j) {
-            in[i][j] = y + i < L.ny && x + j < L.nx;
-            const size_t o = (size_t)(y + i) * L.pitch + x + j;
-            ge[i][j] = in[i][j] ? L.gx[o] : 0.0;   // (zero in the last column of the mesh)
-            gs[i][j] = in[i][j] ? L.gy[o] : 0.0;   // (zero in the last row)
+        for (int i = 0; i < R + 2; ++i) {
+            v0[i] = scale * (double)f0[i];
+            v1[i] = scale * (double)f1[i];
         }
-#pragma unroll
-    for (int i = 0; i < 2; ++i) gw[i] = (in[i][0] && x > 0) ? L.gx[(size_t)(y + i) * L.pitch + x - 1] : 0.0;
-#pragma unroll
-    for (int j = 0; j < 2; ++j) gn[j] = (in[0][j] && y > 0) ? L.gy[(size_t)(y - 1) * L.pitch + x + j] : 0.0;
-    const bool row_in[2] = {y < L.ny && x < L.pitch, y + 1 < L.ny && x < L.pitch};  // x even: both columns are addressable
-    const size_t plane = (size_t)L.ny * L.pitch;
-    const int b_end = min(B, (int)(blockIdx.y + 1) * GR);
-    int buf = 0;
-    for (int b = blockIdx.y * GR; b < b_end; ++b, buf ^= 1) {
-        const int so = node[src[b]], ys = so / L.pitch, xs = so % L.pitch;
-        double* xt = xs0[buf];
-#pragma unroll
-        for (int k = 0; k < PER; ++k) {
-            if (ekind[k] < 0) continue;
-            if (ekind[k] >= 3) { xt[eo[k]] = ekind[k] == 3 ? guess_x0(tab, ey[k], ex[k], ys, xs) : 0.0; continue; }
-            double v0 = 0.0, v1 = 0.0;
-            if (ekind[k] == 1) guess_x0_pair(tab, ey[k], ex[k], ys, xs, v0, v1);
-            else if (ekind[k] == 2) v0 = guess_x0(tab, ey[k], ex[k], ys, xs);
-            *reinterpret_cast<double2*>(xt + eo[k]) = make_double2(v0, v1);
-        }
-        __syncthreads();
-        if (b > (int)blockIdx.y * GR) flush(b - 1, buf ^ 1);
-        // rows 2 pr - 1 .. 2 pr + 2 of the ring tile (ring row = tile row + 1), columns 2 pc, 2 pc + 1 (+ the two beside them)
-        const double* xc = xt + (2 * pr) * XW + 2 * pc + 2;
-        const double2 up = *reinterpret_cast<const double2*>(xc), c0 = *reinterpret_cast<const double2*>(xc + XW),
-                      c1 = *reinterpret_cast<const double2*>(xc + 2 * XW), dn = *reinterpret_cast<const double2*>(xc + 3 * XW);
-        const double w0 = xc[XW - 1], e0 = xc[XW + 2], w1 = xc[2 * XW - 1], e1 = xc[2 * XW + 2];
-        // (L x0)_i = sum over neighbours of g (x0_i - x0_nb); absent neighbours have g = 0
-        double l00 = ge[0][0] * (c0.x - c0.y), l01 = ge[0][1] * (c0.y - e0);
-        l00 = fma(gw[0], c0.x - w0, l00);       l01 = fma(ge[0][0], c0.y - c0.x, l01);
-        l00 = fma(gs[0][0], c0.x - c1.x, l00);  l01 = fma(gs[0][1], c0.y - c1.y, l01);
-        l00 = fma(gn[0], c0.x - up.x, l00);     l01 = fma(gn[1], c0.y - up.y, l01);
-        double l10 = ge[1][0] * (c1.x - c1.y), l11 = ge[1][1] * (c1.y - e1);
-        l10 = fma(gw[1], c1.x - w1, l10);       l11 = fma(ge[1][0], c1.y - c1.x, l11);
-        l10 = fma(gs[1][0], c1.x - dn.x, l10);  l11 = fma(gs[1][1], c1.y - dn.y, l11);
-        l10 = fma(gs[0][0], c1.x - c0.x, l10);  l11 = fma(gs[0][1], c1.y - c0.y, l11);
-        const bool sy0 = y == ys, sy1 = y + 1 == ys, sx0 = x == xs, sx1 = x + 1 == xs;
-        // pad entries (the pad column of an odd-width plane) are written as zeros
-        const double r00 = in[0][0] ? ((sy0 && sx0) ? 1.0 - inv_n2 : -inv_n2) - l00 : 0.0;
-        const double r01 = in[0][1] ? ((sy0 && sx1) ? 1.0 - inv_n2 : -inv_n2) - l01 : 0.0;
-        const double r10 = in[1][0] ? ((sy1 && sx0) ? 1.0 - inv_n2 : -inv_n2) - l10 : 0.0;
-        const double r11 = in[1][1] ? ((sy1 && sx1) ? 1.0 - inv_n2 : -inv_n2) - l11 : 0.0;
+        double rr = 0.0, sx = 0.0;
         double* rp = r0 + b * plane + (size_t)y * L.pitch + x;
-        if (row_in[0]) *reinterpret_cast<double2*>(rp) = make_double2(r00, r01);
-        if (row_in[1]) *reinterpret_cast<double2*>(rp + L.pitch) = make_double2(r10, r11);
-        double rr = fma(r00, r00, fma(r01, r01, fma(r10, r10, r11 * r11)));
-        double sx = (in[0][0] ? c0.x : 0.0) + (in[0][1] ? c0.y : 0.0) + (in[1][0] ? c1.x : 0.0) + (in[1][1] ? c1.y : 0.0);
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const double c0 = v0[i + 1], c1 = v1[i + 1];
+            double wl = __shfl_up_sync(0xffffffffu, c1, 1), er = __shfl_down_sync(0xffffffffu, c0, 1);
+            if (edge) {
+                const double ve = scale * (double)fe[i];
+                if (lane == 0) wl = ve; else er = ve;
+            }
+            const double n0 = i == 0 ? gn0 : gs0[i == 0 ? 0 : i - 1], n1 = i == 0 ? gn1 : gs1[i == 0 ? 0 : i - 1];
+            // (L x0)_i = sum over neighbours of g (x0_i - x0_nb); absent neighbours have g = 0
+            double l0 = ge0[i] * (c0 - c1), l1 = ge1[i] * (c1 - er);
+            l0 = fma(gw[i], c0 - wl, l0);          l1 = fma(ge0[i], c1 - c0, l1);
+            l0 = fma(gs0[i], c0 - v0[i + 2], l0);  l1 = fma(gs1[i], c1 - v1[i + 2], l1);
+            l0 = fma(n0, c0 - v0[i], l0);          l1 = fma(n1, c1 - v1[i], l1);
+            const bool a0 = (in0 >> i) & 1, a1 = (in1 >> i) & 1, sy = y + i == ys;
+            // pad entries (the pad column of an odd-width plane) are written as zeros
+            const double q0 = a0 ? ((sy && x == xs) ? 1.0 - inv_n2 : -inv_n2) - l0 : 0.0;
+            const double q1 = a1 ? ((sy && x + 1 == xs) ? 1.0 - inv_n2 : -inv_n2) - l1 : 0.0;
+            if ((rowin >> i) & 1) *reinterpret_cast<double2*>(rp) = make_double2(q0, q1);
+            rp += L.pitch;
+            rr = fma(q0, q0, fma(q1, q1, rr));
+            sx += (a0 ? c0 : 0.0) + (a1 ? c1 : 0.0);
+        }
         rr = warp_sum(rr);
         sx = warp_sum(sx);
         if (lane == 0) { part[buf][0][warp] = rr; part[buf][1][warp] = sx; }
     }
     __syncthreads();
-    if (b_end > (int)blockIdx.y * GR) flush(b_end - 1, buf ^ 1);
+    if (nb > 0) flush(b0 + nb - 1, (nb - 1) & 1);
 }
 
 // Terminal-source solves deliver ONE number, Z[s,s] = b^T L^+ b, and stop early because the CG error of b^T x_k is the

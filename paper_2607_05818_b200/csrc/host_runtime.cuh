@@ -282,4 +282,18 @@ CUtensorMap make_map(const void* base, int nx, int ny, int pitch, int B, int box
     if (r != CUDA_SUCCESS) throw StatusFail{PDN_E_CUDA, "cuTensorMapEncodeTiled failed with code " + std::to_string((int)r)};
     return m;
 }
+
+// A pitched FP32 matrix (rows x cols, row pitch `pitch` floats) as a 2D tensor with a box of box_x x box_y.
+CUtensorMap make_map_2d_f32(const void* base, int cols, int rows, int pitch, int box_x, int box_y) {
+    CUtensorMap m;
+    const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)pitch * 4};
+    const cuuint32_t box[2] = {(cuuint32_t)box_x, (cuuint32_t)box_y};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = encode_tiled_fn()(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(base), dims, strides,
+                                         box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                         CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) throw StatusFail{PDN_E_CUDA, "cuTensorMapEncodeTiled (2D) failed with code " + std::to_string((int)r)};
+    return m;
+}
 }  // namespace

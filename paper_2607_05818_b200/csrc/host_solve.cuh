@@ -273,6 +273,26 @@ void launch_pq3(Launcher& L, double bytes, const Level& lv, const Smoother& sm, 
     L.run(KC_PQ, bytes, [&] { k_pq3<PQ_R, PQ_W><<<grid, 32 * PQ_W, smem, L.s>>>(m_z, m_q, lv, beta, q, zw_acc, sumz_acc, B, G, active, first ? 1 : 0); });
 }
 
+// Closed-form starting point (guess.cuh): r0 = b - L x0 for the B right-hand sides of a batch.
+constexpr int GRHS_R = 4, GRHS_W = 8, GRHS_NST = 2;
+using GuessRhsGeom = GuessGeom<GRHS_R, GRHS_W>;
+struct GuessHost {
+    GuessTable tab;
+    CUtensorMap map_q;  // the pitched FP32 table as a 2D tensor, box = GW_BW x GuessRhsGeom::BH
+};
+void launch_guess_rhs(Launcher& L, double bytes, const GuessHost& g, const Level& lv, const int* node, const int* src, double inv_n2,
+                      double* r0, double* rr0, double* sumx, int B) {
+    constexpr size_t smem = GRHS_NST * GuessRhsGeom::STAGE_BYTES;
+    static std::atomic<uint64_t> attr_done{0};
+    once_per_device(attr_done, [&] {
+        CK(cudaFuncSetAttribute(k_guess_rhs<GRHS_R, GRHS_W, GRHS_NST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    });
+    const int tiles = cdiv(lv.nx, GW_TX) * cdiv(lv.ny, GuessRhsGeom::TY);
+    // two blocks are resident per SM; at least four waves of them, at most 32 right-hand sides per block
+    const int GR = std::max(1, std::min(32, (int)((long)tiles * B / (296L * 4))));
+    L.run(KC_SMALL, bytes, [&] { k_guess_rhs<GRHS_R, GRHS_W, GRHS_NST><<<dim3(tiles, cdiv(B, GR)), 32 * GRHS_W, smem, L.s>>>(g.map_q, g.tab.scale, lv, node, src, inv_n2, r0, rr0, sumx, B, GR); });
+}
+
 #define NU_DISPATCH(nu, CALL0)                \
     if (sm.f32) { using T_ = float; NU_DISPATCH_(nu, CALL0) } else { using T_ = double; NU_DISPATCH_(nu, CALL0) }
 #define NU_DISPATCH_(nu, CALL)                \
@@ -361,7 +381,8 @@ void vcycle(Launcher& L, const Hierarchy& H, Work& W, const Smoother& sm, int B,
 //   terminal-source batch: zdiag[src[b]-ntsv] = x_b[own node] - mean(x_b)
 // `guess` (may be null): closed-form starting point x0 of every right-hand side (guess.cuh).
 int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts& T, const Smoother& sm, const int* src_ports,
-                int B, bool terminal, double rtol, int max_iter, const GuessTable* guess) {
+                int B, bool terminal, double rtol, int max_iter, const GuessHost* guess_h) {
+    const GuessTable* guess = guess_h ? &guess_h->tab : nullptr;
     const int src0 = src_ports[0];
     CK(cudaMemcpyAsync(W.src.p, src_ports, (size_t)B * sizeof(int), cudaMemcpyHostToDevice, L.s));
     const int* src = W.src.as<int>();
@@ -378,9 +399,7 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
         // help (||r0|| > ||b|| / 2) are re-initialised with x0 = 0, r0 = b -- all on the device
         CK(cudaMemsetAsync(W.g_rr0, 0, (size_t)B * sizeof(double), L.s));
         CK(cudaMemsetAsync(W.g_sumx, 0, (size_t)B * sizeof(double), L.s));
-        const int tiles = cdiv(n, GUESS_TX) * cdiv(n, GUESS_TY);
-        const int GR = std::max(1, std::min(16, (int)((long)tiles * B / (148L * 8))));
-        L.run(KC_SMALL, V, [&] { k_guess_rhs<<<dim3(tiles, cdiv(B, GR)), GUESS_THREADS, 0, L.s>>>(*guess, H.lev[0], node, src, 1.0 / (double)n2, W.r[0].as<double>(), W.g_rr0, W.g_sumx, B, GR); });
+        launch_guess_rhs(L, V, *guess_h, H.lev[0], node, src, 1.0 / (double)n2, W.r[0].as<double>(), W.g_rr0, W.g_sumx, B);
         L.run(KC_SMALL, 0, [&] { k_guess_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.g_rr0, bnorm2, W.g_keep, B); });
         // (a small grid: nearly every block returns at once -- a rejected guess is the exception)
         L.run(KC_SMALL, 0, [&] { k_init_rhs<<<dim3(std::min(32u, cdiv(plane / 2, 256)), B), 256, 0, L.s>>>(W.r[0].as<double>(), n, H.pitch[0], plane, 1.0 / (double)n2, node, src, B, W.g_keep); });

@@ -106,6 +106,15 @@ __global__ void k_table_to_float(size_t cnt, const double* __restrict__ G, float
     if (i < cnt) Gf[i] = (float)G[i];
 }
 
+// The same FP32 values with a row pitch of `pitch` floats (a multiple of four: TMA row strides are multiples of 16
+// bytes), pads zero: the table the window fetches of k_guess_rhs read.
+__global__ void k_table_to_pitched(int n, int pitch, const double* __restrict__ G, float* __restrict__ Gq) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (size_t)(n + 1) * pitch) return;
+    const size_t t = i / pitch, s = i % pitch;
+    Gq[i] = s <= (size_t)n ? (float)G[t * (n + 1) + s] : 0.f;
+}
+
 // The same FP32 values as pairs, P[t][s] = (G[t][s], G[t][min(s+1, n)]): two mesh nodes that are neighbours in x look
 // up neighbouring columns, so one 8-byte load serves both (half the load instructions of the guess kernels).
 __global__ void k_table_to_pairs(int n, const double* __restrict__ G, float2* __restrict__ P) {
