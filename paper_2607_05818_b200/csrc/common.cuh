@@ -54,6 +54,7 @@ struct PcgScalars {
     double* psum;    // sum(p) of the current direction, by recurrence: sum(z) + beta sum(p_old)
     double* alpha;
     double* beta;
+    double* arho;    // sum_j alpha_j rho_j = ||x_k - x_0||_L^2 (Hestenes-Stiefel): the energy a terminal solve has gained
     double* xmean;   // mean of the (implicit) solution x = sum_k alpha_k p_k
     double* relres;  // ||r|| / ||b|| at the last check
     int* active;     // 1 while the right-hand side has not converged

@@ -8,7 +8,7 @@
 // i.e. about one PCG iteration ahead, and the gathered port values are x0[port] + the PCG correction.  The guess
 // only moves the starting point: the operator, the stopping test (||r|| <= rtol ||b||) and therefore the accuracy
 // of the result are those of the plain solve, whatever the quality (or the FP32 storage) of the table -- provided
-// the SAME x0 enters r0 and the gathered result, which is why both kernels below evaluate it through guess_x0().
+// the SAME x0 enters r0 and the gathered result: k_guess_rhs sums the same four FP32 values in the order of guess_x0().
 // A right-hand side whose guess does not help (||r0|| > ||b|| / 2: a tier far from its mean mesh) falls back to
 // x0 = 0 on the device (k_guess_check + k_init_rhs with the keep mask).
 #pragma once
@@ -20,7 +20,6 @@ namespace pdn {
 
 struct GuessTable {
     const float* G;   // table of (rho, 1), (n+1) x (n+1)
-    const float2* P;  // the same values as pairs (G[t][s], G[t][s+1])
     double scale;     // 1 / mean g_y
     int n;
 };
@@ -32,31 +31,6 @@ __device__ __forceinline__ float guess_sum4(float dd, float ss, float ds, float 
     return __fmul_rn(0.25f, __fadd_rn(__fadd_rn(dd, ss), __fadd_rn(ds, sd)));
 }
 
-// columns a, b = a +- 1 of table row t with one 8-byte load
-__device__ __forceinline__ void guess_pair(const GuessTable& t, int row, int a, int b, float& va, float& vb) {
-    const float2 v = __ldg(t.P + (size_t)row * (t.n + 1) + min(a, b));
-    va = a < b ? v.x : v.y;
-    vb = a < b ? v.y : v.x;
-}
-
-// x0 at the two nodes (y, x) and (y, x + 1): bit-identical to guess_x0 of each (same values, same association)
-__device__ __forceinline__ void guess_x0_pair(const GuessTable& t, int y, int x, int ys, int xs, double& v0, double& v1) {
-    const int n = t.n, dy = abs(y - ys);
-    int sy = y + ys + 1;
-    sy = sy <= n ? sy : 2 * n - sy;
-    const int dxa = abs(x - xs), dxb = abs(x + 1 - xs);
-    int sxa = x + xs + 1, sxb = x + xs + 2;
-    sxa = sxa <= n ? sxa : 2 * n - sxa;
-    sxb = sxb <= n ? sxb : 2 * n - sxb;
-    float ddA, ddB, dsA, dsB, sdA, sdB, ssA, ssB;  // G[dy][dx], G[dy][sx], G[sy][dx], G[sy][sx] at nodes A, B
-    guess_pair(t, dy, dxa, dxb, ddA, ddB);
-    guess_pair(t, dy, sxa, sxb, dsA, dsB);
-    guess_pair(t, sy, dxa, dxb, sdA, sdB);
-    guess_pair(t, sy, sxa, sxb, ssA, ssB);
-    v0 = t.scale * (double)guess_sum4(ddA, ssA, dsA, sdA);
-    v1 = t.scale * (double)guess_sum4(ddB, ssB, dsB, sdB);
-}
-
 __device__ __forceinline__ double guess_x0(const GuessTable& t, int y, int x, int ys, int xs) {
     const int n = t.n, dx = abs(x - xs), dy = abs(y - ys);
     int sx = x + xs + 1, sy = y + ys + 1;
@@ -66,7 +40,7 @@ __device__ __forceinline__ double guess_x0(const GuessTable& t, int y, int x, in
     return t.scale * (double)guess_sum4(__ldg(t.G + dy * ld + dx), __ldg(t.G + sy * ld + sx), __ldg(t.G + dy * ld + sx), __ldg(t.G + sy * ld + dx));
 }
 
-// r0[b] = b - L x0 on the pitched plane, rr0[b] += ||r0||^2, sumx[b] += sum(x0).
+// r0[b] = b - L x0 on the pitched plane, rr0[b] += ||r0||^2, sumx[b] += sum(x0), xr0[b] += x0 . r0.
 //
 // The table windows are staged by TMA.  For one right-hand side (source column xs, row ys) the nodes of a tile of
 // 64 x TY mesh nodes plus its ring use, in each of the four index combinations, a CONTIGUOUS window of at most
@@ -105,13 +79,13 @@ template <int R, int W, int NST>
 __global__ void __launch_bounds__(32 * W)
 k_guess_rhs(const __grid_constant__ CUtensorMap tm_tab, double scale, Level L, const int* __restrict__ node,
             const int* __restrict__ src, double inv_n2, double* __restrict__ r0, double* __restrict__ rr0,
-            double* __restrict__ sumx, int B, int GR) {
+            double* __restrict__ sumx, double* __restrict__ xr0, int B, int GR) {
     using Gm = GuessGeom<R, W>;
     constexpr int TY = Gm::TY, WIN = Gm::WIN;
     extern __shared__ __align__(128) float win[];  // NST stages x 4 windows: (dy,dx) (sy,sx) (dy,sx) (sy,dx)
     __shared__ uint64_t mbar[NST];
     __shared__ int s_xs[GW_MAX_GR], s_ys[GW_MAX_GR];
-    __shared__ double part[2][2][W];  // per-warp partial sums of the two reductions, double buffered
+    __shared__ double part[2][3][W];  // per-warp partial sums of the three reductions, double buffered
     const int n = L.nx;               // tiers are square: the table is (n + 1) x (n + 1)
     const int tiles_x = (L.nx + GW_TX - 1) / GW_TX;
     const int tx0 = (blockIdx.x % tiles_x) * GW_TX, ty0 = (blockIdx.x / tiles_x) * TY;
@@ -173,13 +147,13 @@ k_guess_rhs(const __grid_constant__ CUtensorMap tm_tab, double scale, Level L, c
     if (tid == 0)
         for (int j = 0; j < NST && j < nb; ++j) fetch(j);
     // the block's partial sums of right-hand side b go out as ONE atomic per quantity, one iteration later: after the
-    // next __syncthreads the per-warp values are visible to threads 0 and 1
+    // next __syncthreads the per-warp values are visible to threads 0 .. 2
     auto flush = [&](int bb, int pb) {
-        if (tid < 2) {
+        if (tid < 3) {
             double v = 0.0;
 #pragma unroll
             for (int w = 0; w < W; ++w) v += part[pb][tid][w];
-            atomicAdd((tid == 0 ? rr0 : sumx) + bb, v);
+            atomicAdd((tid == 0 ? rr0 : tid == 1 ? sumx : xr0) + bb, v);
         }
     };
     for (int j = 0; j < nb; ++j) {
@@ -212,7 +186,7 @@ k_guess_rhs(const __grid_constant__ CUtensorMap tm_tab, double scale, Level L, c
             v0[i] = scale * (double)f0[i];
             v1[i] = scale * (double)f1[i];
         }
-        double rr = 0.0, sx = 0.0;
+        double rr = 0.0, sx = 0.0, xr = 0.0;
         double* rp = r0 + b * plane + (size_t)y * L.pitch + x;
 #pragma unroll
         for (int i = 0; i < R; ++i) {
@@ -235,11 +209,13 @@ k_guess_rhs(const __grid_constant__ CUtensorMap tm_tab, double scale, Level L, c
             if ((rowin >> i) & 1) *reinterpret_cast<double2*>(rp) = make_double2(q0, q1);
             rp += L.pitch;
             rr = fma(q0, q0, fma(q1, q1, rr));
+            xr = fma(c0, q0, fma(c1, q1, xr));  // (q = 0 outside the mesh)
             sx += (a0 ? c0 : 0.0) + (a1 ? c1 : 0.0);
         }
         rr = warp_sum(rr);
         sx = warp_sum(sx);
-        if (lane == 0) { part[buf][0][warp] = rr; part[buf][1][warp] = sx; }
+        xr = warp_sum(xr);
+        if (lane == 0) { part[buf][0][warp] = rr; part[buf][1][warp] = sx; part[buf][2][warp] = xr; }
     }
     __syncthreads();
     if (nb > 0) flush(b0 + nb - 1, (nb - 1) & 1);
@@ -247,38 +223,27 @@ k_guess_rhs(const __grid_constant__ CUtensorMap tm_tab, double scale, Level L, c
 
 // Terminal-source solves deliver ONE number, Z[s,s] = b^T L^+ b, and stop early because the CG error of b^T x_k is the
 // SQUARE of the energy-norm error -- but only when x_0 = 0: from a guess, b^T (x - x_k) = e_k^T L x_0 + e_k^T L e_k is
-// first order again.  The energy form of the same number, 2 b^T x_k - x_k^T L x_k = b^T x_k + x_k^T r_k, is second
-// order from any starting point, and CG makes x_k - x_0 orthogonal to r_k, so the correction is the single dot
-//     dot[b] = x_0^T r_k      (x_0 re-evaluated from the table; r_k = the right-hand side's last residual),
-// added to x_k[s] - mean(x_k) by k_finish_term.  r_k lives in the ping-pong buffer that was current when the
-// right-hand side converged (rbuf_of[b], recorded by k_scal_check).  grid = (tiles, B), 64 x 64 nodes per block.
-constexpr int GDOT_T = 64;
-__global__ void __launch_bounds__(256)
-k_guess_dot(GuessTable tab, int ny, int nx, int pitch, size_t plane, const int* __restrict__ node, const int* __restrict__ src,
-            const int* __restrict__ keep, const double* __restrict__ ra, const double* __restrict__ rb,
-            const int* __restrict__ rbuf_of, double* __restrict__ dot) {
-    const int b = blockIdx.y;
-    if (!keep[b]) return;
-    const int tiles_x = (nx + GDOT_T - 1) / GDOT_T;
-    const int tx0 = (blockIdx.x % tiles_x) * GDOT_T, ty0 = (blockIdx.x / tiles_x) * GDOT_T;
-    const double* r = (rbuf_of[b] ? rb : ra) + b * plane;
-    const int so = node[src[b]], ys = so / pitch, xs = so % pitch;
-    double s = 0.0;
-    for (int i = threadIdx.x; i < GDOT_T * (GDOT_T / 2); i += 256) {  // two neighbouring columns per step
-        const int y = ty0 + i / (GDOT_T / 2), x = tx0 + 2 * (i % (GDOT_T / 2));
-        if (y >= ny || x >= nx) continue;
-        if (x + 1 < nx) {
-            double v0, v1;
-            guess_x0_pair(tab, y, x, ys, xs, v0, v1);
-            const double2 rv = *reinterpret_cast<const double2*>(r + (size_t)y * pitch + x);  // x and pitch are even
-            s = fma(v0, rv.x, s);
-            s = fma(v1, rv.y, s);
-        } else {
-            s = fma(guess_x0(tab, y, x, ys, xs), r[(size_t)y * pitch + x], s);
-        }
+// first order again.  The energy form of the same number, E(x_k) = 2 b^T x_k - x_k^T L x_k, is second order from any
+// starting point, and CG climbs it by exactly alpha_j rho_j per iteration (Hestenes & Stiefel: ||x - x_j||_L^2 -
+// ||x - x_{j+1}||_L^2 = alpha_j rho_j, rho_j = r_j . z_j), so
+//     Z[s,s] ~ E(x_k) = E(x_0) + sum_{j<k} alpha_j rho_j,    E(x_0) = b^T x_0 + x_0^T r_0,
+// with b^T x_0 = x_0[s] - mean(x_0): the dot x_0 . r_0 is reduced by k_guess_rhs while both are in registers, the sum by
+// k_scal_alpha -- no pass over a vector.  (The round's first version evaluated x_0 . r_k from the last residual: one
+// more table evaluation and one more vector read per terminal right-hand side, 3 us each at 1024^2, and the
+// expected-last probe had to write r_k for it.)  A right-hand side whose guess was rejected started from x_0 = 0:
+// b^T x_k is second order there.
+__global__ void k_finish_term_guess(GuessTable tab, int pitch, const int* __restrict__ node, const int* __restrict__ src,
+                                    const int* __restrict__ keep, const double* __restrict__ sumx, const double* __restrict__ xr0,
+                                    const double* __restrict__ arho, double inv_n2, const double* __restrict__ xown,
+                                    const double* __restrict__ xmean, int ntsv, double* __restrict__ zdiag, int B) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    double z = xown[b] - xmean[b];
+    if (keep[b]) {
+        const int so = node[src[b]], ys = so / pitch, xs = so % pitch;
+        z = (guess_x0(tab, ys, xs, ys, xs) - sumx[b] * inv_n2) + xr0[b] + arho[b];
     }
-    s = warp_sum(s);
-    if ((threadIdx.x & 31) == 0) atomicAdd(dot + b, s);
+    zdiag[src[b] - ntsv] = z;
 }
 
 // keep[b] = 1 if the guess of right-hand side b is used (it at least halves the residual), else 0

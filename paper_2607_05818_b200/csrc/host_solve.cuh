@@ -149,8 +149,8 @@ struct Work {
     CUtensorMap m_rl[MAX_LEVELS], m_ya[MAX_LEVELS], m_ec[MAX_LEVELS];  // m_ec[l]: zb[l] as the coarse box of level l-1
     DevBuf scal, xport, xown, pport, iact, src;  // pport: the search direction at the gathered nodes (+ B own nodes);
                                                  // src: port index each right-hand side of the batch is the source of
-    double *g_rr0 = nullptr, *g_sumx = nullptr, *g_dot = nullptr;  // initial guess (guess.cuh): ||r0||^2, sum(x0), x0.r_k per right-hand side
-    int *g_keep = nullptr, *g_rbuf = nullptr;     // ... whether the guess is used; buffer of the last residual
+    double *g_rr0 = nullptr, *g_sumx = nullptr, *g_xr0 = nullptr;  // initial guess (guess.cuh): ||r0||^2, sum(x0), x0.r0 per right-hand side
+    int* g_keep = nullptr;                        // ... whether the guess is used
     PcgScalars s{};
     int* h_nact = nullptr;                           // pinned (a block of g_pinned, owned while the workspace lives)
     double* h_relres = nullptr;                      // pinned, Bmax
@@ -180,17 +180,16 @@ struct Work {
             m_rl[l] = fine(rl[l], l); m_ya[l] = fine(ya[l], l);
             m_ec[l] = make_map(zb[l].p, H.nx[l], H.ny[l], H.pitch[l], B, T3_ECW, T3_EH / 2);
         }
-        scal.alloc((size_t)14 * B * sizeof(double));
+        scal.alloc((size_t)15 * B * sizeof(double));
         double* sp = scal.as<double>();
         s.rho = sp; s.rz = sp + B; s.pq = sp + 2 * B; s.rr = sp + 3 * B; s.sump = sp + 4 * B;
         s.alpha = sp + 5 * B; s.beta = sp + 6 * B; s.xmean = sp + 7 * B; s.relres = sp + 8 * B;
-        g_rr0 = sp + 9 * B; g_sumx = sp + 10 * B; g_dot = sp + 11 * B;
-        s.pap = sp + 12 * B; s.psum = sp + 13 * B;
-        iact.alloc((size_t)(3 * B + 1) * sizeof(int));
+        g_rr0 = sp + 9 * B; g_sumx = sp + 10 * B; g_xr0 = sp + 11 * B;
+        s.pap = sp + 12 * B; s.psum = sp + 13 * B; s.arho = sp + 14 * B;
+        iact.alloc((size_t)(2 * B + 1) * sizeof(int));
         s.active = iact.as<int>();
         s.n_active = iact.as<int>() + B;
         g_keep = iact.as<int>() + B + 1;
-        g_rbuf = iact.as<int>() + 2 * B + 1;
         xport.alloc((size_t)B * std::max(qmax, 1) * sizeof(double));
         xown.alloc((size_t)B * sizeof(double));
         pport.alloc((size_t)B * (std::max(qmax, 1) + 1) * sizeof(double));
@@ -281,7 +280,7 @@ struct GuessHost {
     CUtensorMap map_q;  // the pitched FP32 table as a 2D tensor, box = GW_BW x GuessRhsGeom::BH
 };
 void launch_guess_rhs(Launcher& L, double bytes, const GuessHost& g, const Level& lv, const int* node, const int* src, double inv_n2,
-                      double* r0, double* rr0, double* sumx, int B) {
+                      double* r0, double* rr0, double* sumx, double* xr0, int B) {
     constexpr size_t smem = GRHS_NST * GuessRhsGeom::STAGE_BYTES;
     static std::atomic<uint64_t> attr_done{0};
     once_per_device(attr_done, [&] {
@@ -290,7 +289,7 @@ void launch_guess_rhs(Launcher& L, double bytes, const GuessHost& g, const Level
     const int tiles = cdiv(lv.nx, GW_TX) * cdiv(lv.ny, GuessRhsGeom::TY);
     // two blocks are resident per SM; at least four waves of them, at most 32 right-hand sides per block
     const int GR = std::max(1, std::min(32, (int)((long)tiles * B / (296L * 4))));
-    L.run(KC_SMALL, bytes, [&] { k_guess_rhs<GRHS_R, GRHS_W, GRHS_NST><<<dim3(tiles, cdiv(B, GR)), 32 * GRHS_W, smem, L.s>>>(g.map_q, g.tab.scale, lv, node, src, inv_n2, r0, rr0, sumx, B, GR); });
+    L.run(KC_SMALL, bytes, [&] { k_guess_rhs<GRHS_R, GRHS_W, GRHS_NST><<<dim3(tiles, cdiv(B, GR)), 32 * GRHS_W, smem, L.s>>>(g.map_q, g.tab.scale, lv, node, src, inv_n2, r0, rr0, sumx, xr0, B, GR); });
 }
 
 #define NU_DISPATCH(nu, CALL0)                \
@@ -397,9 +396,8 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     if (guess) {
         // x0 = column `src` of the mean mesh's closed-form pseudo-inverse, r0 = b - L x0; right-hand sides it does not
         // help (||r0|| > ||b|| / 2) are re-initialised with x0 = 0, r0 = b -- all on the device
-        CK(cudaMemsetAsync(W.g_rr0, 0, (size_t)B * sizeof(double), L.s));
-        CK(cudaMemsetAsync(W.g_sumx, 0, (size_t)B * sizeof(double), L.s));
-        launch_guess_rhs(L, V, *guess_h, H.lev[0], node, src, 1.0 / (double)n2, W.r[0].as<double>(), W.g_rr0, W.g_sumx, B);
+        CK(cudaMemsetAsync(W.g_rr0, 0, (size_t)3 * W.Bmax * sizeof(double), L.s));  // g_rr0, g_sumx, g_xr0: adjacent arrays of Bmax (not B) values
+        launch_guess_rhs(L, V, *guess_h, H.lev[0], node, src, 1.0 / (double)n2, W.r[0].as<double>(), W.g_rr0, W.g_sumx, W.g_xr0, B);
         L.run(KC_SMALL, 0, [&] { k_guess_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.g_rr0, bnorm2, W.g_keep, B); });
         // (a small grid: nearly every block returns at once -- a rejected guess is the exception)
         L.run(KC_SMALL, 0, [&] { k_init_rhs<<<dim3(std::min(32u, cdiv(plane / 2, 256)), B), 256, 0, L.s>>>(W.r[0].as<double>(), n, H.pitch[0], plane, 1.0 / (double)n2, node, src, B, W.g_keep); });
@@ -422,9 +420,8 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
         L.run(KC_SMALL, 0, [&] { k_xport<<<dim3(cdiv(std::max(ngather, 1), 128), B), 128, 0, L.s>>>(W.z.as<double>(), plane, W.s.alpha, W.s.beta, node, ngather, src, W.pport.as<double>(), W.pport.as<double>() + (size_t)B * std::max(ngather, 1), W.xport.as<double>(), W.xown.as<double>(), B, it == 0 ? 1 : 0); });
         ++it;
         bool done = false;
-        int r_new = cur_r ^ 1;  // the buffer this iteration's residual update writes
         auto check = [&] {
-            L.run(KC_SMALL, 0, [&] { k_scal_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, rtol * rtol, bnorm2, r_new, W.g_rbuf); });
+            L.run(KC_SMALL, 0, [&] { k_scal_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, rtol * rtol, bnorm2); });
             CK(cudaMemcpyAsync(W.h_nact, W.s.n_active, sizeof(int), cudaMemcpyDeviceToHost, L.s));
             CK(cudaMemcpyAsync(W.h_relres, W.s.relres, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, L.s));
             CK(cudaStreamSynchronize(L.s));
@@ -448,7 +445,7 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
         if (cheap && it >= 2 && it < max_iter && predicted > 30.0 * rtol && skipped < 2) {  // at most two in a row
             ++skipped;
             vcycle(L, H, W, sm, B, cur_r, true, nact, [&] {
-                L.run(KC_SMALL, 0, [&] { k_scal_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, rtol * rtol, bnorm2, r_new, W.g_rbuf); });
+                L.run(KC_SMALL, 0, [&] { k_scal_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, rtol * rtol, bnorm2); });
                 return false;
             });
             cur_r ^= 1;
@@ -460,16 +457,13 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
         skipped = 0;
         if (expect_done) {
             const size_t chunk = (size_t)RESID_THREADS * RESID_PER_THREAD * 2;
-            // the new residual itself is needed only if the batch does NOT converge (or, for a guessed terminal batch,
-            // by k_guess_dot): first its norm alone, 2 V; the vector is written in a second pass if the check fails
-            const bool keep_r = terminal && guess;
-            double* r_new_p = W.r[cur_r ^ 1].as<double>();
-            L.run(KC_SMALL, (keep_r ? 3.0 : 2.0) * V * nact / B, [&] { k_resid_update<<<dim3(cdiv(plane, chunk), B), RESID_THREADS, 0, L.s>>>(W.r[cur_r].as<double>(), W.q.as<double>(), W.s.alpha, W.s.active, keep_r ? r_new_p : nullptr, W.s.rr, plane); });
+            // the new residual itself is needed only if the batch does NOT converge: first its norm alone, 2 V; the
+            // vector is written in a second pass if the check fails
+            L.run(KC_SMALL, 2.0 * V * nact / B, [&] { k_resid_update<<<dim3(cdiv(plane, chunk), B), RESID_THREADS, 0, L.s>>>(W.r[cur_r].as<double>(), W.q.as<double>(), W.s.alpha, W.s.active, nullptr, W.s.rr, plane); });
             const int r_old = cur_r;
             cur_r ^= 1;
-            if (!check()) {
-                if (!keep_r)  // (the right-hand sides still active; rr is accumulated again and not used)
-                    L.run(KC_SMALL, 3.0 * V * nact / B, [&] { k_resid_update<<<dim3(cdiv(plane, chunk), B), RESID_THREADS, 0, L.s>>>(W.r[r_old].as<double>(), W.q.as<double>(), W.s.alpha, W.s.active, r_new_p, W.s.rr, plane); });
+            if (!check()) {  // (the right-hand sides still active; rr is accumulated again and not used)
+                L.run(KC_SMALL, 3.0 * V * nact / B, [&] { k_resid_update<<<dim3(cdiv(plane, chunk), B), RESID_THREADS, 0, L.s>>>(W.r[r_old].as<double>(), W.q.as<double>(), W.s.alpha, W.s.active, W.r[cur_r].as<double>(), W.s.rr, plane); });
                 vcycle(L, H, W, sm, B, cur_r, false, nact, [] { return false; });
             }
         } else {
@@ -480,12 +474,10 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
         if (it >= max_iter) { status = PDN_E_NOCONV; break; }
     }
     // results + statistics
-    if (terminal && guess) {  // second-order form of the diagonal from a non-zero starting point: + x0 . r_k (guess.cuh)
-        CK(cudaMemsetAsync(W.g_dot, 0, (size_t)B * sizeof(double), L.s));
-        L.run(KC_SMALL, V, [&] { k_guess_dot<<<dim3(cdiv(n, GDOT_T) * cdiv(n, GDOT_T), B), 256, 0, L.s>>>(*guess, n, n, H.pitch[0], plane, node, src, W.g_keep, W.r[0].as<double>(), W.r[1].as<double>(), W.g_rbuf, W.g_dot); });
-    }
-    if (terminal)
-        L.run(KC_SMALL, 0, [&] { k_finish_term<<<cdiv(B, 128), 128, 0, L.s>>>(W.xown.as<double>(), W.s.xmean, src, T.ntsv, T.zdiag.as<double>(), B, guess ? W.g_dot : nullptr); });
+    if (terminal && guess)  // the diagonal in its energy form, second order from the guess: b.x0 + x0.r0 + sum alpha rho (guess.cuh)
+        L.run(KC_SMALL, 0, [&] { k_finish_term_guess<<<cdiv(B, 128), 128, 0, L.s>>>(*guess, H.pitch[0], node, src, W.g_keep, W.g_sumx, W.g_xr0, W.s.arho, 1.0 / (double)n2, W.xown.as<double>(), W.s.xmean, T.ntsv, T.zdiag.as<double>(), B); });
+    else if (terminal)
+        L.run(KC_SMALL, 0, [&] { k_finish_term<<<cdiv(B, 128), 128, 0, L.s>>>(W.xown.as<double>(), W.s.xmean, src, T.ntsv, T.zdiag.as<double>(), B); });
     else
         L.run(KC_SMALL, 0, [&] { k_finish_tsv<<<dim3(cdiv(ngather, 128), B), 128, 0, L.s>>>(W.xport.as<double>(), W.s.xmean, ngather, src, T.ZT.as<double>(), B); });
     CK(cudaMemcpyAsync(W.h_relres, W.s.relres, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, L.s));

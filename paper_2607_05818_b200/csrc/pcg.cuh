@@ -33,7 +33,7 @@ __global__ void k_pcg_init(PcgScalars s, int B) {
     if (b == 0) *s.n_active = B;
     if (b >= B) return;
     s.rho[b] = 1.0; s.rz[b] = 0.0; s.pq[b] = 0.0; s.rr[b] = 0.0; s.sump[b] = 0.0; s.pap[b] = 0.0; s.psum[b] = 0.0;
-    s.alpha[b] = 0.0; s.beta[b] = 0.0; s.xmean[b] = 0.0; s.relres[b] = 1.0; s.active[b] = 1;
+    s.alpha[b] = 0.0; s.beta[b] = 0.0; s.xmean[b] = 0.0; s.arho[b] = 0.0; s.relres[b] = 1.0; s.active[b] = 1;
 }
 
 // After the V-cycle: beta = rz / rho_old (0 on the first iteration or when frozen); rho = rz.
@@ -64,20 +64,18 @@ __global__ void k_scal_alpha(PcgScalars s, int B, double inv_n2) {
     s.psum[b] = psum;
     const double a = pap > 0.0 ? s.rho[b] / pap : 0.0;
     s.alpha[b] = a;
+    s.arho[b] = fma(a, s.rho[b], s.arho[b]);
     s.xmean[b] = fma(a * inv_n2, psum, s.xmean[b]);
     s.rr[b] = 0.0;
 }
 
 // After r -= alpha q: convergence test  ||r||^2 <= tol2 * ||b||^2  (||b||^2 = 1 - 1/n2).
-// rbuf_of[b] (optional) records which of the two residual buffers holds the last residual of a right-hand side
-// (`rbuf` = the buffer this iteration wrote; a frozen right-hand side is never written again).
-__global__ void k_scal_check(PcgScalars s, int B, double tol2, double bnorm2, int rbuf = 0, int* __restrict__ rbuf_of = nullptr) {
+__global__ void k_scal_check(PcgScalars s, int B, double tol2, double bnorm2) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= B) return;
     if (s.active[b]) {
         const double rr = s.rr[b];
         s.relres[b] = sqrt(rr / bnorm2);
-        if (rbuf_of) rbuf_of[b] = rbuf;
         if (!(rr > tol2 * bnorm2)) s.active[b] = 0;  // also freezes on NaN (reported by the host: PDN_E_NUMERIC)
         else atomicAdd(s.n_active, 1);
     }
@@ -87,7 +85,7 @@ __global__ void k_scal_check(PcgScalars s, int B, double tol2, double bnorm2, in
 // in this iteration, so that the smoothing of a cycle nobody needs is not run:
 //   r_out = r_in - alpha q ;  rr += ||r_out||^2      for the right-hand sides still iterating.
 // grid = (chunks of the plane, B); 16-byte accesses; plane (= ny*pitch) is even.
-constexpr int RESID_THREADS = 256, RESID_PER_THREAD = 4;  // double2 per thread
+constexpr int RESID_THREADS = 256, RESID_PER_THREAD = 8;  // double2 per thread and vector: all loads are issued before the first use
 // r_out == nullptr: only the norm (2 V instead of 3 V) -- a batch that is expected to converge now needs its new
 // residual only if the expectation fails.
 __global__ void __launch_bounds__(RESID_THREADS)
@@ -101,19 +99,24 @@ k_resid_update(const double* __restrict__ r_in, const double* __restrict__ q, co
     const double2* r2 = reinterpret_cast<const double2*>(r_in + b * plane);
     const double2* q2 = reinterpret_cast<const double2*>(q + b * plane);
     double2* o2 = r_out ? reinterpret_cast<double2*>(r_out + b * plane) : nullptr;
+    double2 rv[RESID_PER_THREAD], qv[RESID_PER_THREAD];
+#pragma unroll
+    for (int k = 0; k < RESID_PER_THREAD; ++k) {
+        const size_t i = base + (size_t)k * RESID_THREADS;
+        const bool ok = i < n2;
+        rv[k] = ok ? __ldcs(r2 + i) : make_double2(0.0, 0.0);  // (streaming: neither vector is read again soon)
+        qv[k] = ok ? __ldcs(q2 + i) : make_double2(0.0, 0.0);
+    }
     double rr = 0.0;
 #pragma unroll
     for (int k = 0; k < RESID_PER_THREAD; ++k) {
         const size_t i = base + (size_t)k * RESID_THREADS;
-        if (i < n2) {
-            double2 r = r2[i];
-            const double2 qq = q2[i];
-            r.x = fma(-al, qq.x, r.x);
-            r.y = fma(-al, qq.y, r.y);
-            if (o2) o2[i] = r;
-            rr = fma(r.x, r.x, rr);
-            rr = fma(r.y, r.y, rr);
-        }
+        double2 r = rv[k];
+        r.x = fma(-al, qv[k].x, r.x);
+        r.y = fma(-al, qv[k].y, r.y);
+        if (o2 && i < n2) o2[i] = r;
+        rr = fma(r.x, r.x, rr);
+        rr = fma(r.y, r.y, rr);
     }
     rr = block_sum(rr, red);
     if (threadIdx.x == 0) atomicAdd(rr_acc + b, rr);
@@ -155,12 +158,10 @@ __global__ void k_finish_tsv(const double* __restrict__ xport, const double* __r
     if (k < ngather) ZT[(size_t)src[b] * ngather + k] = xport[(size_t)b * ngather + k] - xmean[b];
 }
 
-// (+ extra[b], the second-order correction of a solve that started from a guess: guess.cuh)
 __global__ void k_finish_term(const double* __restrict__ xown, const double* __restrict__ xmean,
-                              const int* __restrict__ src, int ntsv, double* __restrict__ zdiag, int B,
-                              const double* __restrict__ extra = nullptr) {
+                              const int* __restrict__ src, int ntsv, double* __restrict__ zdiag, int B) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b < B) zdiag[src[b] - ntsv] = (xown[b] - xmean[b]) + (extra ? extra[b] : 0.0);
+    if (b < B) zdiag[src[b] - ntsv] = xown[b] - xmean[b];
 }
 
 // TSV re-planning (pdn_update_tsvs): copy the kept entries of a tier's port matrix into its new layout.

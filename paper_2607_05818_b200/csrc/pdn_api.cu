@@ -90,7 +90,7 @@ int pick_batch(const Hierarchy& H, int want, const pdn_opts& o) {
 // differ by a scale factor share a table (a uniform stack builds one table, not one per tier; the initial guess of
 // BASELINE's workloads builds one per call).
 struct SpectralTables {
-    struct Entry { int n; double rho; DevBuf G, Gf, Gp, Gq; CUtensorMap map_q; };  // Gq: FP32, pitched, behind map_q
+    struct Entry { int n; double rho; DevBuf G, Gf, Gq; CUtensorMap map_q; };  // Gq: FP32, pitched, behind map_q
     std::vector<Entry> list;
     Entry* find(int n, double rho, double rel_tol) {
         for (Entry& e : list)
@@ -119,11 +119,9 @@ struct SpectralTables {
         if (e.Gf.p) return;
         const size_t cnt = ((size_t)e.n + 1) * (e.n + 1);
         e.Gf.alloc(cnt * sizeof(float));
-        e.Gp.alloc(cnt * sizeof(float2));
         const int pq = (e.n + 1 + 3) & ~3;
         e.Gq.alloc((size_t)(e.n + 1) * pq * sizeof(float));
         L.run(KC_SMALL, 0, [&] { k_table_to_float<<<cdiv(cnt, 256), 256, 0, L.s>>>(cnt, e.G.as<double>(), e.Gf.as<float>()); });
-        L.run(KC_SMALL, 0, [&] { k_table_to_pairs<<<cdiv(cnt, 256), 256, 0, L.s>>>(e.n, e.G.as<double>(), e.Gp.as<float2>()); });
         L.run(KC_SMALL, 0, [&] { k_table_to_pitched<<<cdiv((size_t)(e.n + 1) * pq, 256), 256, 0, L.s>>>(e.n, pq, e.G.as<double>(), e.Gq.as<float>()); });
         e.map_q = make_map_2d_f32(e.Gq.p, e.n + 1, e.n + 1, pq, GW_BW, GuessRhsGeom::BH);
     }
@@ -185,7 +183,7 @@ int reduce_tier(pdn_ctx* c, Launcher& L, Hierarchy& H, Work& W, int Bmax, TierPo
         if (!e && (long)(tsv_src.size() + term.size()) >= n / 2) e = &tabs.build(L, n, rho, true);
         if (e) {
             tabs.float_copy(L, *e);
-            gtab = GuessHost{GuessTable{e->Gf.as<float>(), e->Gp.as<float2>(), 1.0 / H.mean_gy, n}, e->map_q};
+            gtab = GuessHost{GuessTable{e->Gf.as<float>(), 1.0 / H.mean_gy, n}, e->map_q};
             guess = &gtab;
             { std::lock_guard<std::mutex> g(c->mu); c->stats.n_guess_tiers++; }
         }

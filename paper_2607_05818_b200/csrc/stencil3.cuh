@@ -284,6 +284,7 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
     const unsigned interior = interior_mask<R, H, Gm::IW, Gm::IH>(L, lane, warp, gx, gy0);
     const size_t plane = (size_t)L.ny * L.pitch, cplane = (size_t)cny * cpitch;
     const size_t goff = (size_t)gy0 * L.pitch + gx;
+    const ptrdiff_t coff = (ptrdiff_t)(gy0 >> 1) * cpitch + (gx >> 1);  // coarse node of the patch's first 2x2 aggregate (gy0, gx even)
     __shared__ ActiveList al;
     active_list_build(al, active, blockIdx.z * G, min(G, B - (int)blockIdx.z * G), FUSED ? alpha : nullptr);
     if (threadIdx.x == 0) {
@@ -309,6 +310,7 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
         const double alj = FUSED ? al.s[j] : 0.0;
         T y0r[R], y1r[R], rh0[R], rh1[R];
         double rr = 0.0;
+        double* rp = FUSED ? r_out + b * plane + goff : nullptr;
 #pragma unroll
         for (int i = 0; i < R; ++i) {
             double2 r = ld2(rbuf + st * Gm::TILE + slot0 + i * T3_EW);
@@ -316,11 +318,12 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
                 const double2 q = ld2(qbuf + st * Gm::TILE + slot0 + i * T3_EW);
                 r.x = fma(-alj, q.x, r.x);
                 r.y = fma(-alj, q.y, r.y);
-                const bool in = (interior >> i) & 1;
-                if (in) st2(r_out + b * plane + goff + (size_t)i * L.pitch, r);
-                const double mx = in ? r.x : 0.0, my = in ? r.y : 0.0;
-                rr = fma(mx, mx, rr);
-                rr = fma(my, my, rr);
+                if ((interior >> i) & 1) {
+                    st2(rp, r);
+                    rr = fma(r.x, r.x, rr);
+                    rr = fma(r.y, r.y, rr);
+                }
+                rp += L.pitch;
             }
             const float2 s2 = sc_slot[i * 32];
             rh0[i] = (T)s2.x * (T)r.x;
@@ -352,6 +355,7 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
         });
         if (NU == 1 && threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
         // residual of the unscaled system at the patch nodes, summed over 2x2 aggregates
+        double* rcp = rc + b * cplane + coff;
 #pragma unroll
         for (int i = 0; i < R; i += 2) {
             const float2 sa = sc_slot[SD_OFF + i * 32], sb = sc_slot[SD_OFF + (i + 1) * 32];
@@ -359,8 +363,8 @@ k_down3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtens
             v = fma((T)sa.y, t1[i] - y1r[i], v);
             v = fma((T)sb.x, t0[i + 1] - y0r[i + 1], v);
             v = fma((T)sb.y, t1[i + 1] - y1r[i + 1], v);
-            if ((interior >> i) & 1)  // rows i and i+1 are interior together (H, R, y0 even)
-                rc[b * cplane + (size_t)((gy0 + i) >> 1) * cpitch + (gx >> 1)] = (double)v;
+            if ((interior >> i) & 1) *rcp = (double)v;  // rows i and i+1 are interior together (H, R, y0 even)
+            rcp += cpitch;
         }
     }
 }
@@ -447,16 +451,18 @@ k_up3(const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensor
             if (k == 0 && threadIdx.x == 0 && j + 2 < nb) fetch(j + 2);
         }
         double rz = 0.0;
+        double* zp = z_out + b * plane + goff;  // (one pointer stepped by the pitch: the per-row form recomputed the 64-bit offset)
 #pragma unroll
         for (int i = 0; i < R; ++i) {
-            const bool in = (interior >> i) & 1;
-            const float2 s2 = sc_slot[i * 32];
-            if (in) st2(z_out + b * plane + goff + (size_t)i * L.pitch,
-                        make_double2((double)((T)s2.x * y0r[i]), (double)((T)s2.y * y1r[i])));
-            if (DOT) {  // r.z = r.(s y) = (s r).y = r^.y
-                rz = fma(in ? (double)rh0[i] : 0.0, (double)y0r[i], rz);
-                rz = fma(in ? (double)rh1[i] : 0.0, (double)y1r[i], rz);
+            if ((interior >> i) & 1) {
+                const float2 s2 = sc_slot[i * 32];
+                st2(zp, make_double2((double)((T)s2.x * y0r[i]), (double)((T)s2.y * y1r[i])));
+                if (DOT) {  // r.z = r.(s y) = (s r).y = r^.y
+                    rz = fma((double)rh0[i], (double)y0r[i], rz);
+                    rz = fma((double)rh1[i], (double)y1r[i], rz);
+                }
             }
+            zp += L.pitch;
         }
         rz_pend = rz;
         b_pend = b;

@@ -115,13 +115,4 @@ __global__ void k_table_to_pitched(int n, int pitch, const double* __restrict__ 
     Gq[i] = s <= (size_t)n ? (float)G[t * (n + 1) + s] : 0.f;
 }
 
-// The same FP32 values as pairs, P[t][s] = (G[t][s], G[t][min(s+1, n)]): two mesh nodes that are neighbours in x look
-// up neighbouring columns, so one 8-byte load serves both (half the load instructions of the guess kernels).
-__global__ void k_table_to_pairs(int n, const double* __restrict__ G, float2* __restrict__ P) {
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x, ld = (size_t)n + 1;
-    if (i >= ld * ld) return;
-    const size_t s = i % ld;
-    P[i] = make_float2((float)G[i], (float)G[s < (size_t)n ? i + 1 : i]);
-}
-
 }  // namespace pdn
