@@ -54,6 +54,9 @@ struct PcgScalars {
     double* psum;    // sum(p) of the current direction, by recurrence: sum(z) + beta sum(p_old)
     double* alpha;
     double* beta;
+    double* qq;      // accumulator: ||q||^2 of this iteration (k_pq3_last only)
+    double* rq;      // accumulator: r.q of this iteration (k_pq3_last only)
+    double* rrk;     // ||r_k||^2 as of the last convergence check
     double* arho;    // sum_j alpha_j rho_j = ||x_k - x_0||_L^2 (Hestenes-Stiefel): the energy a terminal solve has gained
     double* xmean;   // mean of the (implicit) solution x = sum_k alpha_k p_k
     double* relres;  // ||r|| / ||b|| at the last check

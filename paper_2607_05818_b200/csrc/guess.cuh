@@ -246,10 +246,14 @@ __global__ void k_finish_term_guess(GuessTable tab, int pitch, const int* __rest
     zdiag[src[b] - ntsv] = z;
 }
 
-// keep[b] = 1 if the guess of right-hand side b is used (it at least halves the residual), else 0
-__global__ void k_guess_check(const double* __restrict__ rr0, double bnorm2, int* __restrict__ keep, int B) {
+// keep[b] = 1 if the guess of right-hand side b is used (it at least halves the residual), else 0;
+// rrk[b] = ||r0||^2 of the starting point the right-hand side ends up with
+__global__ void k_guess_check(const double* __restrict__ rr0, double bnorm2, int* __restrict__ keep, double* __restrict__ rrk, int B) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b < B) keep[b] = rr0[b] <= 0.25 * bnorm2 ? 1 : 0;
+    if (b >= B) return;
+    const bool use = rr0[b] <= 0.25 * bnorm2;
+    keep[b] = use ? 1 : 0;
+    rrk[b] = use ? rr0[b] : bnorm2;
 }
 
 // Starting values of the accumulators the PCG loop adds to: the gathered port values

@@ -146,6 +146,7 @@ struct Work {
     DevBuf r[2], y0, z, q;                                 // level 0 (r is a ping-pong pair: halos are read across blocks)
     DevBuf rl[MAX_LEVELS], ya[MAX_LEVELS], zb[MAX_LEVELS];  // levels >= 1: residual, scaled iterate, correction
     CUtensorMap m_r[2], m_y0, m_z, m_q;
+    CUtensorMap m_ri[2], m_qi;  // r and q as interior-only boxes (k_pq3_last)
     CUtensorMap m_rl[MAX_LEVELS], m_ya[MAX_LEVELS], m_ec[MAX_LEVELS];  // m_ec[l]: zb[l] as the coarse box of level l-1
     DevBuf scal, xport, xown, pport, iact, src;  // pport: the search direction at the gathered nodes (+ B own nodes);
                                                  // src: port index each right-hand side of the batch is the source of
@@ -174,18 +175,22 @@ struct Work {
         auto fine = [&](const DevBuf& d, int l) { return make_map(d.p, H.nx[l], H.ny[l], H.pitch[l], B, T3_EW, T3_EH); };
         for (int i = 0; i < 2; ++i) m_r[i] = fine(r[i], 0);
         m_y0 = fine(y0, 0); m_z = fine(z, 0); m_q = fine(q, 0);
+        auto inner = [&](const DevBuf& d) { return make_map(d.p, H.nx[0], H.ny[0], H.pitch[0], B, T3_EW - 4, T3_EH - 4); };
+        for (int i = 0; i < 2; ++i) m_ri[i] = inner(r[i]);
+        m_qi = inner(q);
         for (int l = 1; l < H.nlev; ++l) {
             const size_t vl = (size_t)B * H.plane(l) * sizeof(double);
             rl[l].alloc(vl); ya[l].alloc(vl); zb[l].alloc(vl);
             m_rl[l] = fine(rl[l], l); m_ya[l] = fine(ya[l], l);
             m_ec[l] = make_map(zb[l].p, H.nx[l], H.ny[l], H.pitch[l], B, T3_ECW, T3_EH / 2);
         }
-        scal.alloc((size_t)15 * B * sizeof(double));
+        scal.alloc((size_t)18 * B * sizeof(double));
         double* sp = scal.as<double>();
         s.rho = sp; s.rz = sp + B; s.pq = sp + 2 * B; s.rr = sp + 3 * B; s.sump = sp + 4 * B;
         s.alpha = sp + 5 * B; s.beta = sp + 6 * B; s.xmean = sp + 7 * B; s.relres = sp + 8 * B;
         g_rr0 = sp + 9 * B; g_sumx = sp + 10 * B; g_xr0 = sp + 11 * B;
         s.pap = sp + 12 * B; s.psum = sp + 13 * B; s.arho = sp + 14 * B;
+        s.qq = sp + 15 * B; s.rq = sp + 16 * B; s.rrk = sp + 17 * B;
         iact.alloc((size_t)(2 * B + 1) * sizeof(int));
         s.active = iact.as<int>();
         s.n_active = iact.as<int>() + B;
@@ -292,6 +297,19 @@ void launch_guess_rhs(Launcher& L, double bytes, const GuessHost& g, const Level
     L.run(KC_SMALL, bytes, [&] { k_guess_rhs<GRHS_R, GRHS_W, GRHS_NST><<<dim3(tiles, cdiv(B, GR)), 32 * GRHS_W, smem, L.s>>>(g.map_q, g.tab.scale, lv, node, src, inv_n2, r0, rr0, sumx, xr0, B, GR); });
 }
 
+void launch_pq3_last(Launcher& L, double bytes, const Level& lv, const Smoother& sm, int B, const CUtensorMap& m_z,
+                     const CUtensorMap& m_qi, const CUtensorMap& m_ri, const PcgScalars& s, bool first) {
+    constexpr int H = 2, IW = T3_EW - 2 * H, IH = T3_EH - 2 * H;
+    const int tx = cdiv(lv.nx, IW), ty = cdiv(lv.ny, IH), G = rhs_per_block(tx * ty, B, sm.G, T3_MAX_G_PQ);
+    dim3 grid(tx, ty, cdiv(B, G));
+    constexpr size_t smem = 2 * T3_TILE_BYTES + 4 * (size_t)IW * IH * sizeof(double) + sizeof(Exch<PQ_W>);  // 2 z stages + 2 x (q_old, r)
+    static std::atomic<uint64_t> attr_done{0};
+    once_per_device(attr_done, [&] {
+        CK(cudaFuncSetAttribute(k_pq3_last<PQ_R, PQ_W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    });
+    L.run(KC_PQ, bytes, [&] { k_pq3_last<PQ_R, PQ_W><<<grid, 32 * PQ_W, smem, L.s>>>(m_z, m_qi, m_ri, lv, s.beta, s.pq, s.sump, s.qq, s.rq, B, G, s.active, first ? 1 : 0); });
+}
+
 #define NU_DISPATCH(nu, CALL0)                \
     if (sm.f32) { using T_ = float; NU_DISPATCH_(nu, CALL0) } else { using T_ = double; NU_DISPATCH_(nu, CALL0) }
 #define NU_DISPATCH_(nu, CALL)                \
@@ -392,13 +410,13 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     const int ngather = terminal ? 0 : T.q;
     int cur_r = 0;
     const double bnorm2 = 1.0 - 1.0 / (double)n2;
-    L.run(KC_SMALL, 0, [&] { k_pcg_init<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B); });
+    L.run(KC_SMALL, 0, [&] { k_pcg_init<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, bnorm2); });
     if (guess) {
         // x0 = column `src` of the mean mesh's closed-form pseudo-inverse, r0 = b - L x0; right-hand sides it does not
         // help (||r0|| > ||b|| / 2) are re-initialised with x0 = 0, r0 = b -- all on the device
         CK(cudaMemsetAsync(W.g_rr0, 0, (size_t)3 * W.Bmax * sizeof(double), L.s));  // g_rr0, g_sumx, g_xr0: adjacent arrays of Bmax (not B) values
         launch_guess_rhs(L, V, *guess_h, H.lev[0], node, src, 1.0 / (double)n2, W.r[0].as<double>(), W.g_rr0, W.g_sumx, W.g_xr0, B);
-        L.run(KC_SMALL, 0, [&] { k_guess_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.g_rr0, bnorm2, W.g_keep, B); });
+        L.run(KC_SMALL, 0, [&] { k_guess_check<<<cdiv(B, 128), 128, 0, L.s>>>(W.g_rr0, bnorm2, W.g_keep, W.s.rrk, B); });
         // (a small grid: nearly every block returns at once -- a rejected guess is the exception)
         L.run(KC_SMALL, 0, [&] { k_init_rhs<<<dim3(std::min(32u, cdiv(plane / 2, 256)), B), 256, 0, L.s>>>(W.r[0].as<double>(), n, H.pitch[0], plane, 1.0 / (double)n2, node, src, B, W.g_keep); });
         L.run(KC_SMALL, 0, [&] { k_guess_ports<<<dim3(cdiv(std::max(ngather, 1), 128), B), 128, 0, L.s>>>(*guess, H.pitch[0], node, ngather, src, W.g_keep, W.g_sumx, 1.0 / (double)n2, W.xport.as<double>(), W.xown.as<double>(), W.s.xmean, B); });
@@ -414,8 +432,15 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
     double rel_prev = 1.0, rel_cur = 1.0;  // max relative residual over the batch after the last two iterations
     int skipped = 0;                       // consecutive iterations whose outcome the host did not read
     while (true) {
+        // CG residuals contract roughly geometrically.  If the next one is expected below the tolerance, this iteration
+        // is run in its terminal form: k_pq3_last reads z, q_old and r, writes nothing and leaves the sums from which
+        // k_scal_estimate gets the new residual norm (3 V instead of the 5 V of k_pq3 + a pass over r and q, and no
+        // V-cycle); only if that expectation was wrong are q and the new residual formed after all.
+        const double predicted = rel_prev > 0.0 ? rel_cur * (rel_cur / rel_prev) : 1.0;
+        const bool expect_done = predicted <= rtol;
         L.run(KC_SMALL, 0, [&] { k_scal_beta<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, it == 0); });
-        launch_pq3(L, (it == 0 ? 2.0 : 3.0) * V * nact / B, H.lev[0], sm, B, W.m_z, W.m_q, W.s.beta, W.q.as<double>(), W.s.pq, W.s.sump, W.s.active, it == 0);
+        if (expect_done) launch_pq3_last(L, (it == 0 ? 2.0 : 3.0) * V * nact / B, H.lev[0], sm, B, W.m_z, W.m_qi, W.m_ri[cur_r], W.s, it == 0);
+        else launch_pq3(L, (it == 0 ? 2.0 : 3.0) * V * nact / B, H.lev[0], sm, B, W.m_z, W.m_q, W.s.beta, W.q.as<double>(), W.s.pq, W.s.sump, W.s.active, it == 0);
         L.run(KC_SMALL, 0, [&] { k_scal_alpha<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B, 1.0 / (double)n2); });
         L.run(KC_SMALL, 0, [&] { k_xport<<<dim3(cdiv(std::max(ngather, 1), 128), B), 128, 0, L.s>>>(W.z.as<double>(), plane, W.s.alpha, W.s.beta, node, ngather, src, W.pport.as<double>(), W.pport.as<double>() + (size_t)B * std::max(ngather, 1), W.xport.as<double>(), W.xown.as<double>(), B, it == 0 ? 1 : 0); });
         ++it;
@@ -431,16 +456,13 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
             rel_prev = rel_cur;
             rel_cur = 0.0;
             for (int b = 0; b < B; ++b) rel_cur = std::max(rel_cur, W.h_relres[b]);  // (a NaN is caught after the loop)
-            if (c->debug) fprintf(stderr, "[pdn]   it %d: max relres %.3e, active %d\n", it, rel_cur, nact);
+            if (c->debug) fprintf(stderr, "[pdn]   it %d: max relres %.3e, active %d%s\n", it, rel_cur, nact, expect_done ? " (terminal form)" : "");
             return done || it >= max_iter;
         };
-        // CG residuals contract roughly geometrically: if the next one is expected below the tolerance, update the
-        // residual alone first (3 V of traffic) and run the V-cycle only if that expectation was wrong
-        const double predicted = rel_prev > 0.0 ? rel_cur * (rel_cur / rel_prev) : 1.0;
-        const bool expect_done = predicted <= rtol;
-        // ... and if it is expected far above it while an iteration is short (small meshes / batches), the host
-        // does not wait for the outcome at all: the device still freezes what converged (k_scal_check), the
-        // next iteration is enqueued behind it, and the prediction is carried forward.  Iteration 1 is always read.
+        // If the next residual is expected far above the tolerance while an iteration is short (small meshes /
+        // batches), the host does not wait for the outcome at all: the device still freezes what converged
+        // (k_scal_check), the next iteration is enqueued behind it, and the prediction is carried forward.
+        // Iteration 1 is always read.
         const bool cheap = 13.3 * V < 2.0e9;  // under ~0.5 ms of HBM traffic
         if (cheap && it >= 2 && it < max_iter && predicted > 30.0 * rtol && skipped < 2) {  // at most two in a row
             ++skipped;
@@ -456,14 +478,14 @@ int solve_batch(pdn_ctx* c, Launcher& L, const Hierarchy& H, Work& W, TierPorts&
         }
         skipped = 0;
         if (expect_done) {
-            const size_t chunk = (size_t)RESID_THREADS * RESID_PER_THREAD * 2;
-            // the new residual itself is needed only if the batch does NOT converge: first its norm alone, 2 V; the
-            // vector is written in a second pass if the check fails
-            L.run(KC_SMALL, 2.0 * V * nact / B, [&] { k_resid_update<<<dim3(cdiv(plane, chunk), B), RESID_THREADS, 0, L.s>>>(W.r[cur_r].as<double>(), W.q.as<double>(), W.s.alpha, W.s.active, nullptr, W.s.rr, plane); });
-            const int r_old = cur_r;
-            cur_r ^= 1;
-            if (!check()) {  // (the right-hand sides still active; rr is accumulated again and not used)
-                L.run(KC_SMALL, 3.0 * V * nact / B, [&] { k_resid_update<<<dim3(cdiv(plane, chunk), B), RESID_THREADS, 0, L.s>>>(W.r[r_old].as<double>(), W.q.as<double>(), W.s.alpha, W.s.active, W.r[cur_r].as<double>(), W.s.rr, plane); });
+            L.run(KC_SMALL, 0, [&] { k_scal_estimate<<<cdiv(B, 128), 128, 0, L.s>>>(W.s, B); });
+            if (!check()) {
+                // not converged after all: q = L z + beta q_old and r - alpha q as vectors, for the right-hand sides still
+                // active (the sums k_pq3 and k_resid_update add once more are reset before anything reads them)
+                const size_t chunk = (size_t)RESID_THREADS * RESID_PER_THREAD * 2;
+                launch_pq3(L, (it == 1 ? 2.0 : 3.0) * V * nact / B, H.lev[0], sm, B, W.m_z, W.m_q, W.s.beta, W.q.as<double>(), W.s.pq, W.s.sump, W.s.active, it == 1);
+                L.run(KC_SMALL, 3.0 * V * nact / B, [&] { k_resid_update<<<dim3(cdiv(plane, chunk), B), RESID_THREADS, 0, L.s>>>(W.r[cur_r].as<double>(), W.q.as<double>(), W.s.alpha, W.s.active, W.r[cur_r ^ 1].as<double>(), W.s.rr, plane); });
+                cur_r ^= 1;
                 vcycle(L, H, W, sm, B, cur_r, false, nact, [] { return false; });
             }
         } else {

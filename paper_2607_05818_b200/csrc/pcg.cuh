@@ -28,12 +28,12 @@ __global__ void k_init_rhs(double* __restrict__ r, int nx, int pitch, size_t pla
     }
 }
 
-__global__ void k_pcg_init(PcgScalars s, int B) {
+__global__ void k_pcg_init(PcgScalars s, int B, double bnorm2) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b == 0) *s.n_active = B;
     if (b >= B) return;
     s.rho[b] = 1.0; s.rz[b] = 0.0; s.pq[b] = 0.0; s.rr[b] = 0.0; s.sump[b] = 0.0; s.pap[b] = 0.0; s.psum[b] = 0.0;
-    s.alpha[b] = 0.0; s.beta[b] = 0.0; s.xmean[b] = 0.0; s.arho[b] = 0.0; s.relres[b] = 1.0; s.active[b] = 1;
+    s.alpha[b] = 0.0; s.beta[b] = 0.0; s.xmean[b] = 0.0; s.arho[b] = 0.0; s.qq[b] = 0.0; s.rq[b] = 0.0; s.rrk[b] = bnorm2; s.relres[b] = 1.0; s.active[b] = 1;
 }
 
 // After the V-cycle: beta = rz / rho_old (0 on the first iteration or when frozen); rho = rz.
@@ -46,6 +46,8 @@ __global__ void k_scal_beta(PcgScalars s, int B, int first) {
     s.rz[b] = 0.0;
     s.pq[b] = 0.0;
     s.sump[b] = 0.0;
+    s.qq[b] = 0.0;
+    s.rq[b] = 0.0;
 }
 
 // After w = L z, q = w + beta q_old (k_pq3).  The direction p = z + beta p_old is implicit:
@@ -69,12 +71,28 @@ __global__ void k_scal_alpha(PcgScalars s, int B, double inv_n2) {
     s.rr[b] = 0.0;
 }
 
+// After k_pq3_last and k_scal_alpha, in place of a pass over r and q:
+//   ||r - alpha q||^2 = ||r||^2 - 2 alpha r.q + alpha^2 ||q||^2
+// from the sums k_pq3_last left and ||r||^2 of the last check.  The three terms cancel down to the new norm, so the
+// rounding error of the sum is bounded by ~1e-13 of their magnitudes (FP64 sums over <= 1e8 nodes); an estimate below
+// 100 times that bound is not trusted and the right-hand side is reported as it was (not converged: the host then
+// forms the residual itself).
+__global__ void k_scal_estimate(PcgScalars s, int B) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B || !s.active[b]) return;
+    const double a = s.alpha[b], r0 = s.rrk[b], t1 = 2.0 * a * s.rq[b], t2 = a * a * s.qq[b];
+    const double est = (r0 - t1) + t2;
+    const double noise = 1e-13 * (r0 + fabs(t1) + t2);
+    s.rr[b] = (est > 100.0 * noise) ? est : r0;
+}
+
 // After r -= alpha q: convergence test  ||r||^2 <= tol2 * ||b||^2  (||b||^2 = 1 - 1/n2).
 __global__ void k_scal_check(PcgScalars s, int B, double tol2, double bnorm2) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= B) return;
     if (s.active[b]) {
         const double rr = s.rr[b];
+        s.rrk[b] = rr;
         s.relres[b] = sqrt(rr / bnorm2);
         if (!(rr > tol2 * bnorm2)) s.active[b] = 0;  // also freezes on NaN (reported by the host: PDN_E_NUMERIC)
         else atomicAdd(s.n_active, 1);

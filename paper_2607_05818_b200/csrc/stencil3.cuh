@@ -599,4 +599,132 @@ k_pq3(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensor
     if (b_pend >= 0) flush();
 }
 
+// ---------------------------------------------------------------------------------------------
+// The operator apply of an iteration that is EXPECTED TO BE THE LAST of its batch (the host predicts the next residual
+// from the contraction so far).  Such an iteration needs neither q nor the new residual as vectors -- only
+//   alpha = rho / p.Lp  (for the update of x at the port nodes)   and   ||r - alpha q||^2  (to confirm convergence),
+// and the second is a quadratic in alpha whose coefficients do not depend on it:
+//   ||r - alpha q||^2 = ||r||^2 - 2 alpha r.q + alpha^2 ||q||^2,    q = L z + beta q_old.
+// So this variant reads z, q_old and r (3 V), forms q in registers and reduces z.Lz, sum(z), ||q||^2 and r.q; nothing is
+// written.  k_pq3 + the norm probe moved 5 V for the same outcome.  k_scal_estimate turns the sums into ||r_new||^2
+// (with a bound on the cancellation error: an estimate it cannot vouch for counts as "not converged"); if the batch
+// has not converged after all, the host runs the ordinary k_pq3 and the residual update and carries on.
+// q_old and r are needed at the block's interior nodes only: they come as 60 x 68 boxes (their own tensor maps), two
+// stages each, refilled one iteration after their use (they are consumed at the end of an iteration).
+template <int R, int W>
+__global__ void __launch_bounds__(32 * W, 1)
+k_pq3_last(const __grid_constant__ CUtensorMap tm_z, const __grid_constant__ CUtensorMap tm_qi,
+           const __grid_constant__ CUtensorMap tm_ri, Level L, const double* __restrict__ beta,
+           double* __restrict__ zw_acc, double* __restrict__ sumz_acc, double* __restrict__ qq_acc,
+           double* __restrict__ rq_acc, int B, int G, const int* __restrict__ active, int first) {
+    constexpr int H = 2;
+    using Gm = Geom<R, W, H>;
+    constexpr int ITILE = Gm::IW * Gm::IH;
+    constexpr uint32_t ITILE_BYTES = ITILE * sizeof(double);
+    static_assert(ITILE_BYTES % 128 == 0, "TMA destinations are 128-byte aligned");
+    extern __shared__ __align__(128) double smem_dyn[];
+    double* zbuf = smem_dyn;              // 2 stages, tile + halo
+    double* qbuf = zbuf + 2 * Gm::TILE;   // 2 stages, interior only
+    double* rbuf = qbuf + 2 * ITILE;      // 2 stages, interior only
+    Exch<W>& x = *reinterpret_cast<Exch<W>*>(rbuf + 2 * ITILE);
+    __shared__ uint64_t mbar[3];  // two z stages + the row-exchange barrier
+    __shared__ uint64_t mbi[2];   // the (q_old, r) stages
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int x0 = blockIdx.x * Gm::IW - H, y0 = blockIdx.y * Gm::IH - H;
+    const int gx = x0 + 2 * lane, gy0 = y0 + R * warp;
+    const int slot0 = (R * warp) * T3_EW + 2 * lane;
+    const int islot0 = (R * warp - H) * Gm::IW + 2 * lane - H;  // the same node in an interior-only tile
+    Patch<R> c;
+    patch_init<R, double>(c, L.gx, L.gy, nullptr, L, gx, gy0, nullptr, 0);
+    const double zero[R] = {};
+    double d0[R], d1[R];  // diagonal = sum of the incident conductances
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+        const double n0 = i == 0 ? c.hN0 : c.hS0[i == 0 ? 0 : i - 1], n1 = i == 0 ? c.hN1 : c.hS1[i == 0 ? 0 : i - 1];
+        d0[i] = (c.hE0[i] + c.hW0[i]) + (c.hS0[i] + n0);
+        d1[i] = (c.hE1[i] + c.hE0[i]) + (c.hS1[i] + n1);
+    }
+    exch_clear<R, W, double>(x);
+    const unsigned interior = interior_mask<R, H, Gm::IW, Gm::IH>(L, lane, warp, gx, gy0);
+    __shared__ ActiveList al;
+    active_list_build(al, active, blockIdx.z * G, min(G, B - (int)blockIdx.z * G), beta);
+    if (threadIdx.x == 0) {
+        mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); mbar_init(&mbar[2], 32 * W);
+        mbar_init(&mbi[0], 1); mbar_init(&mbi[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    const int nb = al.n;
+    auto fetch_z = [&](int j) {  // thread 0 only
+        const int st = j & 1;
+        mbar_expect_tx(&mbar[st], Gm::TILE_BYTES);
+        tma_load_3d(zbuf + st * Gm::TILE, &tm_z, x0, y0, al.b[j], &mbar[st]);
+    };
+    auto fetch_i = [&](int j) {  // thread 0 only
+        const int st = j & 1;
+        mbar_expect_tx(&mbi[st], (first ? 1 : 2) * ITILE_BYTES);
+        tma_load_3d(rbuf + st * ITILE, &tm_ri, x0 + H, y0 + H, al.b[j], &mbi[st]);
+        if (!first) tma_load_3d(qbuf + st * ITILE, &tm_qi, x0 + H, y0 + H, al.b[j], &mbi[st]);
+    };
+    if (threadIdx.x == 0 && nb > 0) {  // nb == 0: every right-hand side of the group has converged
+        fetch_z(0); fetch_i(0);
+        if (nb > 1) { fetch_z(1); fetch_i(1); }
+    }
+    Xchg<W> xc{&x, &mbar[2], 0, 0u, warp, lane};
+    double pend[4] = {0.0, 0.0, 0.0, 0.0};  // partials of the previous right-hand side, reduced one iteration later
+    int b_pend = -1;
+    auto flush = [&] {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) pend[k] = warp_sum(pend[k]);
+        if (lane == 0) {
+            atomicAdd(zw_acc + b_pend, pend[0]);
+            atomicAdd(sumz_acc + b_pend, pend[1]);
+            atomicAdd(qq_acc + b_pend, pend[2]);
+            atomicAdd(rq_acc + b_pend, pend[3]);
+        }
+    };
+    for (int j = 0; j < nb; ++j) {
+        const int b = al.b[j], st = j & 1;
+        mbar_wait(&mbar[st], (j >> 1) & 1);
+        const double bt = al.s[j];
+        double z0[R], z1[R], sumz = 0.0, zw = 0.0, qq = 0.0, rq = 0.0;
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const double2 zz = ld2(zbuf + st * Gm::TILE + slot0 + i * T3_EW);
+            sumz += ((interior >> i) & 1) ? zz.x + zz.y : 0.0;
+            z0[i] = zz.x;
+            z1[i] = zz.y;
+        }
+        if (b_pend >= 0) flush();
+        double t0[R], t1[R];
+        apply_step<R, W, double>(xc, c, z0, z1, zero, zero, t0, t1);
+        // past this exchange every thread has read its z tile of this iteration and its (q_old, r) tiles of the previous one
+        if (threadIdx.x == 0) {
+            if (j + 2 < nb) fetch_z(j + 2);
+            if (j >= 1 && j + 1 < nb) fetch_i(j + 1);  // stage (j+1) & 1 = (j-1) & 1
+        }
+        mbar_wait(&mbi[st], (j >> 1) & 1);
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            if ((interior >> i) & 1) {
+                const double w0 = fma(d0[i], z0[i], -t0[i]), w1 = fma(d1[i], z1[i], -t1[i]);
+                const double2 rr = ld2(rbuf + st * ITILE + islot0 + i * Gm::IW);
+                double q0 = w0, q1 = w1;
+                if (!first) {
+                    const double2 qo = ld2(qbuf + st * ITILE + islot0 + i * Gm::IW);
+                    q0 = fma(bt, qo.x, w0);
+                    q1 = fma(bt, qo.y, w1);
+                }
+                zw = fma(z0[i], w0, zw); zw = fma(z1[i], w1, zw);
+                qq = fma(q0, q0, qq);    qq = fma(q1, q1, qq);
+                rq = fma(rr.x, q0, rq);  rq = fma(rr.y, q1, rq);
+            }
+        }
+        pend[0] = zw; pend[1] = sumz; pend[2] = qq; pend[3] = rq;
+        b_pend = b;
+    }
+    if (b_pend >= 0) flush();
+}
+
 }  // namespace pdn
