@@ -48,8 +48,10 @@ __device__ __forceinline__ double guess_x0(const GuessTable& t, int y, int x, in
 // up again right of it, and the folded sum index f(x + xs + 1) runs up to n and back down -- a run or a V, never a
 // gap.  So the block asks the TMA unit for four 2D boxes of the table (origin = the smallest index the tile uses,
 // guess_origin) per right-hand side, NST stages ahead, and its threads read them with 4-byte shared loads at
-// row * 72 + column -- forwards or backwards, conflict-free either way -- instead of gathering sixteen bytes per node
-// from L2 through the L1TEX path (round 2's first version: 7 us per right-hand side at 1024^2, L1TEX-bound).
+// row * 72 + column -- forwards or backwards; a lane's two columns make the warp's addresses 8 bytes apart, a two-way
+// bank conflict at worst -- instead of gathering sixteen bytes per node from L2 through the L1TEX path (round 2's
+// first version: 7 us per right-hand side at 1024^2, L1TEX-bound; this one 4.1 us, bound by instruction issue and
+// latency at 16 warps per SM: ablating the TMA fetches or the stores changes nothing).
 // The innermost box coordinate has to be a multiple of 16 bytes (an odd one is an illegal instruction), so the column
 // origin is rounded down to a multiple of four entries and the box is 72 wide: 66 entries used, up to 3 skipped.
 // grid = (tiles_x * tiles_y, ceil(B / GR)); block = W warps; lane l of warp w owns columns 2l, 2l+1 and rows
